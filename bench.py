@@ -1,0 +1,361 @@
+#!/usr/bin/env python
+"""bench.py — MLUPS / roofline fraction / WCTpDT of the ISLBM hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload NAME]
+
+One bench "step" is one pass of the whole hot path over one batch: LBM_PER_STEP
+time steps (collide + stream/interpolate + walls)
+followed by one Nusselt/Reynolds reduction (row a6).  `value` is whole-job MLUPS
+(Eq. 38) with the state resident in HBM; `e2e` is the same metric
+with the pre-collision state uploaded from pinned host memory inside the timed
+region.  N > 1 runs N independent cavities (one per rank, no data-path
+collective): weak scaling.  Rank 0 prints ONE JSON line.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+LBM_PER_STEP = 20                       # LBM time steps per bench step
+DEFAULT_WORKLOAD = "c5_256cu"           # 256^3 D3Q19+D3Q7 fp64, 3.5 GB per buffer >> L2: the HBM-bound config
+BYTES_PER_UPDATE = {(2, 0): 224, (2, 1): 112, (3, 0): 416, (3, 1): 208}   # 2*Q*sizeof
+METRIC = "MLUPS"
+
+
+def read_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            return float(json.load(fh)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
+
+
+def read_traffic(workload, kernel):
+    """dram bytes per launch from the committed ncu capture, if one exists for this kernel."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            return json.load(fh).get(f"{workload}:{kernel}")
+    return None
+
+
+class ClockSampler:
+    FIELDS = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+              "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={index}", f"--query-gpu={self.FIELDS}", "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            pass
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+            out, _ = self.proc.communicate()
+        sm, mx, reasons = [], [], set()
+        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
+        for line in out.splitlines():
+            parts = [p.strip() for p in line.split(",")]
+            if len(parts) < 6:
+                continue
+            try:
+                sm.append(float(parts[0]))
+                mx.append(float(parts[1]))
+            except ValueError:
+                continue
+            for nm, val in zip(names, parts[2:6]):
+                if val.lower().startswith("active"):
+                    reasons.add(nm)
+        sm.sort()
+        return {"sm_mhz": sm[len(sm) // 2] if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def dist_setup(n_gpus):
+    """torch.distributed over NCCL when launched by torchrun; returns (rank, world, local_rank)."""
+    import torch
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world == 1:
+        return 0, 1, 0
+    import torch.distributed as dist
+    rank, local = int(os.environ["RANK"]), int(os.environ.get("LOCAL_RANK", "0"))
+    torch.cuda.set_device(local)
+    dist.init_process_group(backend="nccl", device_id=torch.device("cuda", local))
+    return rank, world, local
+
+
+def dist_max_sum(t_local, units_local, device):
+    """max over ranks of the timed duration, sum over ranks of the processed units."""
+    import torch
+    import torch.distributed as dist
+    if not (dist.is_available() and dist.is_initialized()):
+        return t_local, units_local
+    tt = torch.tensor([t_local], dtype=torch.float64, device=device)
+    uu = torch.tensor([units_local], dtype=torch.float64, device=device)
+    dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+    dist.all_reduce(uu, op=dist.ReduceOp.SUM)
+    return tt.item(), uu.item()
+
+
+def barrier():
+    import torch.distributed as dist
+    if dist.is_available() and dist.is_initialized():
+        dist.barrier()
+
+
+def oracle_threads():
+    return max(1, len(os.sched_getaffinity(0)))
+
+
+def oracle_sample(w, cores, target_seconds=2.0):
+    """A bounded sample of workload w for the CPU oracle: the same mesh in x and y and the
+    first nz_s z-planes (a wall-adjacent slab), sized for ~target_seconds per oracle step."""
+    import numpy as np
+    n = len(w.coords[0])
+    per_core_mlups = 1.0 if w.dim == 3 else 1.3         # measured on this container (single thread)
+    budget = int(cores * per_core_mlups * 1e6 * target_seconds)
+    if w.dim == 2 or n ** 3 <= budget:
+        return [np.array(c) for c in w.coords], "full mesh"
+    nz_s = max(8, min(n, budget // (n * n)))
+    coords = [np.array(w.coords[0]), np.array(w.coords[1]), np.array(w.coords[2][:nz_s])]
+    return coords, f"x,y full ({n}x{n}), first {nz_s} z-planes of the same mesh"
+
+
+def time_oracle(w, steps, warmup, cores):
+    from oracle.oracle import Oracle
+    coords, what = oracle_sample(w, cores)
+    orc = Oracle(coords, w.delta, w.Ra, w.Pr, w.Ma, threads=cores)
+    orc.init(w.seed, w.noise_amp)
+    nodes = 1
+    for c in coords:
+        nodes *= len(c)
+    for _ in range(warmup):
+        orc.step(1)
+    t0 = time.perf_counter()
+    for _ in range(steps):
+        orc.step(1)
+    dt = time.perf_counter() - t0
+    orc.close()
+    return nodes * steps / dt / 1e6, dt / steps, what, nodes
+
+
+def run_reference(args):
+    """--impl reference: the oracle, as it stands, on the host cores (rank 0 only)."""
+    if int(os.environ.get("RANK", "0")) != 0:
+        return
+    from paper_2509_01099_b200 import inputs
+    w = inputs.workload(args.workload)
+    cores = oracle_threads()
+    mlups, sec_per_step, what, nodes = time_oracle(w, args.steps, args.warmup, cores)
+    line = {
+        "impl": "reference", "metric": METRIC, "value": mlups, "unit": "MLUPS", "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": sec_per_step * 1e3, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": args.workload, "nodes": w.nodes, "lattice": "D2Q9+D2Q5" if w.dim == 2 else "D3Q19+D3Q7",
+                   "step": "one oracle time step on the sample"},
+        "cpu_baseline": {"value": mlups, "unit": "MLUPS", "cores": cores, "kind": "oracle", "sample": f"{what}; {nodes} nodes per step"},
+        "e2e": {"value": mlups, "unit": "MLUPS", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }
+    print(json.dumps(line), flush=True)
+
+
+def time_device(sim, nodes, steps, warmup, lbm_per_step, flush=None):
+    """K bench steps on the device; returns (seconds total, seconds inside islbm_step, launches, last Nu)."""
+    import torch
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * steps + 2)]
+    for _ in range(warmup):
+        sim.step(lbm_per_step)
+        nu = sim.nusselt()
+    torch.cuda.synchronize()
+    barrier()
+    l0 = sim.launch_count
+    ev[0].record()
+    for k in range(steps):
+        ev[1 + 2 * k].record()
+        sim.step(lbm_per_step)
+        ev[2 + 2 * k].record()
+        nu = sim.nusselt()
+    ev[-1].record()
+    torch.cuda.synchronize()
+    barrier()
+    total = ev[0].elapsed_time(ev[-1]) * 1e-3
+    in_step = sum(ev[1 + 2 * k].elapsed_time(ev[2 + 2 * k]) for k in range(steps)) * 1e-3
+    return total, in_step, sim.launch_count - l0, nu
+
+
+def time_e2e(sim, orc_state_host, steps, lbm_per_step):
+    """End to end through the C-ABI with HOST buffers: every step uploads the pre-collision state from
+    pinned host memory (islbm_set_populations), advances, and reads the diagnostics back."""
+    import torch
+    f_h, g_h = orc_state_host
+    f_d = torch.empty_like(f_h, device="cuda")
+    g_d = torch.empty_like(g_h, device="cuda")
+    h2d = f_h.numel() * 8 + g_h.numel() * 8
+    for _ in range(1):
+        f_d.copy_(f_h, non_blocking=True)
+        g_d.copy_(g_h, non_blocking=True)
+        sim.set_populations(f_d, g_d)
+        sim.step(lbm_per_step)
+        sim.nusselt()
+    torch.cuda.synchronize()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        f_d.copy_(f_h, non_blocking=True)
+        g_d.copy_(g_h, non_blocking=True)
+        sim.set_populations(f_d, g_d)
+        sim.step(lbm_per_step)
+        nu = sim.nusselt()          # 5 doubles device -> host, synchronises
+    e1.record()
+    torch.cuda.synchronize()
+    barrier()
+    return e0.elapsed_time(e1) * 1e-3, h2d, 40, nu
+
+
+def measure_workload(islbm, inputs, name, precision, steps, warmup, lbm_per_step, kernel=0):
+    w = inputs.workload(name)
+    sim = islbm.Islbm(w.coords, w.delta, w.Ra, w.Pr, w.Ma, precision=precision)
+    if kernel:
+        sim.set_kernel(kernel)
+    sim.init(w.seed, w.noise_amp)
+    total, in_step, launches, nu = time_device(sim, w.nodes, steps, warmup, lbm_per_step)
+    p = sim.params()
+    t_lbm = in_step / (steps * lbm_per_step)
+    out = {
+        "mlups": w.nodes * steps * lbm_per_step / total / 1e6,
+        "mlups_step_kernel_only": w.nodes / t_lbm / 1e6,
+        "us_per_lbm_step": t_lbm * 1e6,
+        "wctpdt_s": (total / (steps * lbm_per_step)) * p["H_lu"] / p["U"],
+        "kernel": sim.kernel_name, "launches": launches, "Nu_hot": nu["Nu_hot"], "Re": nu["Re"],
+        "total_s": total, "in_step_s": in_step, "H_lu": p["H_lu"],
+    }
+    return sim, w, out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default=DEFAULT_WORKLOAD)
+    ap.add_argument("--precision", default="f64", choices=["f64", "f32"])
+    ap.add_argument("--lbm-per-step", type=int, default=LBM_PER_STEP)
+    ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 generic, 2 tiled")
+    ap.add_argument("--no-extras", action="store_true", help="skip the secondary workloads, e2e and CPU baseline")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    from paper_2509_01099_b200 import inputs, islbm     # raises if libislbm.so is missing: no fallback
+
+    rank, world, local = dist_setup(args.gpus)
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    prec = 0 if args.precision == "f64" else 1
+    sampler = ClockSampler(local) if rank == 0 else None
+    sim, w, r = measure_workload(islbm, inputs, args.workload, prec, args.steps, args.warmup, args.lbm_per_step, args.kernel)
+    clocks = sampler.stop() if sampler else None
+    units = float(w.nodes) * args.steps * args.lbm_per_step
+    t_max, units_sum = dist_max_sum(r["total_s"], units, dev)
+    value = units_sum / t_max / 1e6
+
+    peak, peak_src = read_peaks()
+    bpu = BYTES_PER_UPDATE[(w.dim, prec)]
+    t_launch = r["in_step_s"] / (args.steps * args.lbm_per_step)
+    achieved = bpu * w.nodes / t_launch / 1e9
+    roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                "traffic": read_traffic(args.workload, r["kernel"]), "kernel": r["kernel"],
+                "algorithmic_bytes_per_launch": bpu * w.nodes, "bytes_per_update": bpu,
+                "avg_launch_us": t_launch * 1e6, "peak_source": peak_src}
+
+    e2e = None
+    cpu = None
+    extras = {}
+    if not args.no_extras:
+        # e2e: pre-collision state from pinned host memory, uploaded every step
+        f, g = sim.get_populations()
+        f_h = torch.empty(f.shape, dtype=torch.float64, pin_memory=True)
+        g_h = torch.empty(g.shape, dtype=torch.float64, pin_memory=True)
+        f_h.copy_(f)
+        g_h.copy_(g)
+        del f, g
+        n_e2e = min(args.steps, 3)
+        t_e2e, h2d, d2h, _ = time_e2e(sim, (f_h, g_h), n_e2e, args.lbm_per_step)
+        t_e2e_max, u_e2e = dist_max_sum(t_e2e, float(w.nodes) * n_e2e * args.lbm_per_step, dev)
+        e2e = {"value": u_e2e / t_e2e_max / 1e6, "unit": "MLUPS", "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+               "steps": n_e2e, "what": "H2D of f_t,g_t from pinned host memory + islbm_set_populations + "
+                                       f"islbm_step({args.lbm_per_step}) + islbm_nusselt (D2H)"}
+        del f_h, g_h
+    sim.close()
+    del sim
+    torch.cuda.empty_cache()
+
+    if not args.no_extras and rank == 0 and world == 1:
+        for nm, pr in (("c5_256cu_uniform", 0), ("c5_256cu", 1), ("c3_1024sq", 0), ("c3_1024sq_uniform", 0), ("c3_1024sq", 1),
+                       ("c2_512sq", 0), ("c4_128cu", 0)):
+            if nm == args.workload and pr == prec:
+                continue
+            try:
+                lps = args.lbm_per_step if "256" in nm or "128" in nm else 200
+                s2, w2, r2 = measure_workload(islbm, inputs, nm, pr, max(3, args.steps // 2), 3, lps, args.kernel)
+                b2 = BYTES_PER_UPDATE[(w2.dim, pr)]
+                extras[nm + ("_f32" if pr else "")] = {
+                    "mlups": r2["mlups"], "roofline_frac": b2 * w2.nodes / (r2["us_per_lbm_step"] * 1e-6) / 1e9 / peak,
+                    "us_per_lbm_step": r2["us_per_lbm_step"], "wctpdt_s": r2["wctpdt_s"], "kernel": r2["kernel"],
+                    "state_bytes_per_buffer": (w2.nodes * b2) // 2}
+                s2.close()
+                del s2
+                torch.cuda.empty_cache()
+            except Exception as exc:   # a secondary workload must not take the headline down
+                extras[nm + ("_f32" if pr else "")] = {"error": str(exc)[:200]}
+        cores = oracle_threads()
+        mlups_cpu, _, what, nodes_s = time_oracle(w, 3, 1, cores)
+        cpu = {"value": mlups_cpu, "unit": "MLUPS", "cores": cores, "kind": "oracle",
+               "sample": f"{what}; {nodes_s} nodes x 3 steps after 1 warm-up"}
+
+    if rank == 0:
+        line = {
+            "metric": METRIC, "value": value, "unit": "MLUPS", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": t_max / args.steps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64" if prec == 0 else "f64 arithmetic, f32 storage", "data": "synthetic",
+            "config": {"workload": args.workload, "nodes_per_gpu": w.nodes, "lattice": "D2Q9+D2Q5" if w.dim == 2 else "D3Q19+D3Q7",
+                       "mesh": f"{w.mesh} stretch {w.stretch}", "Ra": w.Ra, "Pr": w.Pr, "U_lu": 0.1,
+                       "step": f"{args.lbm_per_step} LBM time steps + 1 Nu/Re reduction",
+                       "l2": f"state {w.nodes * bpu // 2} B per buffer, two buffers, vs 126 MB L2: inputs larger than L2"
+                             if w.nodes * bpu > 3e8 else "state fits in L2: fraction is not an HBM fraction",
+                       "parallelism": f"{world} independent cavities (replicas, no data-path collective)"},
+            "wctpdt_s": r["wctpdt_s"], "Nu_hot": r["Nu_hot"], "Re": r["Re"],
+            "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": r["launches"], "clocks": clocks,
+            "also": extras,
+        }
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

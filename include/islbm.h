@@ -1,0 +1,164 @@
+/*
+ * islbm.h — C-ABI boundary of the B200-native ISLBM hot path.
+ *
+ * The library implements ONE thing: the per-timestep double-distribution
+ * update of the interpolation-supplemented lattice Boltzmann method for the
+ * side-heated cavity of arXiv 2509.01099 ("PAPER.md" below is
+ * /root/reference/PAPER.md), on a tensor-product non-uniform mesh:
+ *
+ *   collision of the flow (D2Q9 / D3Q19, MRT + Guo forcing, Eq. 9-13, 17) and
+ *   temperature (D2Q5 / D3Q7, MRT, Eq. 14-16, 19) populations with the
+ *   Boussinesq force, virtual streaming by one lattice
+ *   displacement (Eq. 18, 20), separable quadratic interpolation back onto the
+ *   mesh nodes, half-way bounce-back / anti-bounce-back
+ *   walls (Eq. 21-23), and the Nusselt / Reynolds reductions (Eq. 27-34, 40-42).
+ *
+ * Every step of that path runs in CUDA kernels compiled for sm_100a.  There is
+ * no CPU fallback: a call that needs the device and finds none returns
+ * ISLBM_ERR_CUDA.
+ *
+ * Conventions
+ *   - plain C types only; pointers are marked HOST or DEVICE below.
+ *   - every function returns 0 (ISLBM_OK) or a negative ISLBM_ERR_* code and
+ *     never aborts or throws; islbm_last_error() returns a thread-local,
+ *     human-readable message for the last failing call on this thread.
+ *   - population arrays: [q][z][y][x], x fastest, fp64, dense (no padding);
+ *     field arrays: [z][y][x], fp64.  nz = 1 in 2-D.
+ *   - direction ordering (reading A5; the paper prints only the
+ *     moment ordering of Eq. 10/11/15/16):
+ *       D2Q9 : 0 (0,0) 1 (1,0) 2 (0,1) 3 (-1,0) 4 (0,-1) 5 (1,1) 6 (-1,1)
+ *              7 (-1,-1) 8 (1,-1);                     D2Q5 = first five.
+ *       D3Q19: 0 rest; 1..6 (+x)(-x)(+y)(-y)(+z)(-z);
+ *              7..10 (1,1,0)(-1,1,0)(1,-1,0)(-1,-1,0);
+ *              11..14 (1,0,1)(-1,0,1)(1,0,-1)(-1,0,-1);
+ *              15..18 (0,1,1)(0,-1,1)(0,1,-1)(0,-1,-1);  D3Q7 = first seven.
+ *   - the problem is fixed (BASELINE.json configs): x-lo
+ *     wall isothermal T = +0.5, x-hi wall isothermal T = -0.5, all other walls
+ *     adiabatic, all walls no-slip, T0 = 0, buoyancy along +y.
+ *   - all device work is enqueued on the CUDA stream given to islbm_create and
+ *     is asynchronous unless stated otherwise.
+ */
+#ifndef ISLBM_H
+#define ISLBM_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct islbm islbm_t; /* opaque; owned by the library */
+
+typedef struct {
+  int dim;            /* 2 or 3 */
+  int n[3];           /* FLUID nodes per axis (n[2] = 1 in 2-D); every node is updated */
+  const double *x[3]; /* HOST; strictly increasing node coordinates per axis;
+                         borrowed for the call and copied; x[2] ignored in 2-D */
+  double delta;       /* lattice unit in mesh units (1 l.u. = minimal
+                         spacing); the walls sit at x[a][0] - delta/2 and
+                         x[a][n-1] + delta/2 (half-way schemes) */
+} islbm_mesh;
+
+enum { ISLBM_D2Q9_D2Q5 = 0, ISLBM_D3Q19_D3Q7 = 1 };
+enum { ISLBM_F64 = 0, ISLBM_F32_STORAGE = 1 };
+
+enum {
+  ISLBM_OK = 0,
+  ISLBM_ERR_ARG = -1,       /* NULL pointer, bad dim / lattice / precision combination, n < 3 */
+  ISLBM_ERR_MESH = -2,      /* non-monotone coordinates or a spacing < delta (the departure
+                               point must stay inside the adjacent cell) */
+  ISLBM_ERR_PARAM = -3,     /* Ra, Pr, Ma <= 0; tau_f <= 1/2; a_T outside (-4,1) / (-6,1) */
+  ISLBM_ERR_WORKSPACE = -4, /* workspace NULL, misaligned (256 B) or too small */
+  ISLBM_ERR_CUDA = -5,      /* a CUDA runtime call failed (message has the CUDA error) */
+  ISLBM_ERR_STATE = -6,     /* call not valid in the current state (e.g. step before init) */
+  ISLBM_ERR_NONFINITE = -7  /* islbm_nusselt found a non-finite result */
+};
+
+/* Parameters derived by islbm_create (Table 1). */
+typedef struct {
+  double U;        /* free-fall velocity in lattice units = Ma * c_s              */
+  double H_lu;     /* characteristic length in lattice units = L_eff,y / delta    */
+  double nu;       /* U * H_lu * sqrt(Pr/Ra)                                      */
+  double alpha;    /* nu / Pr                                                     */
+  double gbeta;    /* U^2 / H_lu  (Delta_T = 1)                                   */
+  double tau_f;    /* 3 nu + 1/2                                                  */
+  double a_T;      /* 20 sqrt3 alpha - 4  (2-D),  42 sqrt3 alpha - 6  (3-D)       */
+  double omega_bc; /* (4 + a_T)/10 (2-D), (6 + a_T)/21 (3-D)                      */
+  double dt_star;  /* free-fall time advanced by one step = U / H_lu              */
+  double L_eff[3]; /* x[n-1] - x[0] + delta per axis (1 for the unused axis)      */
+} islbm_params;
+
+/* Bytes of DEVICE workspace islbm_create needs for this mesh / lattice /
+ * precision (two ping-pong population buffers + interpolation tables +
+ * reduction scratch).  Pure host arithmetic. */
+int islbm_workspace_bytes(const islbm_mesh *mesh, int lattice, int precision,
+                          size_t *bytes);
+
+/* Create a solver.  mesh: HOST.  Ma = U / c_s (BASELINE.json's U = 0.1 l.u. is
+ * Ma = 0.1*sqrt(3); the paper's runs use Ma = 0.1).
+ * dev_workspace: DEVICE, 256-byte aligned, >= islbm_workspace_bytes; owned by
+ * the caller and kept alive until islbm_destroy.  cuda_stream: a cudaStream_t
+ * (NULL = the legacy default stream).  Uploads the tables; state is undefined
+ * until islbm_init or islbm_set_populations. */
+int islbm_create(islbm_t **out, const islbm_mesh *mesh, int lattice, double Ra,
+                 double Pr, double Ma, int precision, void *dev_workspace,
+                 size_t bytes, void *cuda_stream);
+
+void islbm_destroy(islbm_t *h);
+
+/* Derived parameters (HOST out). */
+int islbm_get_params(const islbm_t *h, islbm_params *out);
+
+/* Rest state: rho = 1, u = 0, T = noise_amp * (2 r_k - 1) with r_k in [0,1) the
+ * top 53 bits of the (k+1)-th SplitMix64 output for `seed`, k the linear node
+ * index (reading A15); populations are the equilibria of that state. */
+int islbm_init(islbm_t *h, unsigned long long seed, double noise_amp);
+
+/* Load / read the PRE-collision populations f_t, g_t (the paper's state
+ * variable).  f: DEVICE [qf][z][y][x], g: DEVICE [qg][z][y][x],
+ * fp64, dense.  Internally the library keeps post-collision populations
+ * (DESIGN.md "state convention"); set collides once, get re-runs the streaming
+ * half of the last step on the previous buffer. */
+int islbm_set_populations(islbm_t *h, const double *f, const double *g);
+int islbm_get_populations(islbm_t *h, double *f, double *g);
+
+/* Advance n time steps: n x (collide, stream + interpolate + walls). */
+int islbm_step(islbm_t *h, int n);
+
+/* Macroscopic fields of the current state: rho = sum f,
+ * u = (sum e f + F/2)/rho, T = sum g.  DEVICE outputs [z][y][x]; any of them
+ * may be NULL (w is ignored in 2-D). */
+int islbm_fields(islbm_t *h, double *rho, double *u, double *v, double *w,
+                 double *T);
+
+/* HOST out[5]: Nu_hot (Eq. 32/41), Nu_cold (Eq. 41), <Re> (Eq. 34/42),
+ * <u*^2>_V, <Nu> (Eq. 31/40); wall derivative per Eq. 28, averages per Eq. 29
+ * normalised by the effective lengths.  Synchronises the stream.
+ * Returns ISLBM_ERR_NONFINITE (out still written) if any entry is not finite. */
+int islbm_nusselt(islbm_t *h, double out[5]);
+
+/* Steady-state residuals of Eq. 30 between the current fields and the fields
+ * saved by the previous call (first call saves and returns 1, 1):
+ * HOST out[2] = { sum|u - u_prev|_2 / sum|u_prev|_2, sum|T - T_prev| / sum|T_prev| }.
+ * Needs the optional snapshot area (requested with islbm_workspace_bytes'
+ * default sizing).  Synchronises the stream. */
+int islbm_steady_residual(islbm_t *h, double out[2]);
+
+/* Test / study hooks (not part of the four-call contract). */
+int islbm_set_buoyancy_scale(islbm_t *h, double s); /* multiplies g*beta; 0 for pin P5 */
+/* 0 = auto (fastest kernel for this mesh), 1 = generic global-memory kernel,
+ * 2 = shared-memory tiled kernel, 3 = uniform-mesh pure-shift kernel (only
+ * valid when every spacing equals delta). */
+int islbm_set_kernel(islbm_t *h, int which);
+/* Number of kernels launched by this handle since creation. */
+long long islbm_launch_count(const islbm_t *h);
+/* Name of the step kernel variant that islbm_step currently dispatches to. */
+const char *islbm_kernel_name(const islbm_t *h);
+
+const char *islbm_last_error(void);
+const char *islbm_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* ISLBM_H */

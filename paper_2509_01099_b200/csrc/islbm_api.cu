@@ -1,0 +1,509 @@
+// islbm_api.cu — C-ABI of the ISLBM hot path (include/islbm.h): host-side
+// setup (parameter map, interpolation tables, workspace carving) and kernel
+// dispatch.  No torch types, no CPU fallback.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include <vector>
+
+#include "../../include/islbm.h"
+#include "islbm_kernels.cuh"
+#include "islbm_reduce.cuh"
+#include "islbm_tiled.cuh"
+
+using namespace islbmk;
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const std::string &msg) {
+  g_err = msg;
+  return code;
+}
+
+#define CUDA_TRY(expr)                                                                 \
+  do {                                                                                 \
+    cudaError_t e_ = (expr);                                                           \
+    if (e_ != cudaSuccess)                                                             \
+      return fail(ISLBM_ERR_CUDA, std::string(#expr) + ": " + cudaGetErrorString(e_)); \
+  } while (0)
+
+constexpr size_t kAlign = 256;
+size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
+
+constexpr int kMaxRedBlocks = 148 * 8;
+
+struct Carve {
+  size_t buf[2], wtab, avgw, partial, red_out, snap, total;
+};
+
+Carve carve(long long nn, int q, size_t st_bytes, int npad) {
+  Carve c{};
+  size_t off = 0;
+  for (int i = 0; i < 2; ++i) {
+    c.buf[i] = off;
+    off = align_up(off + (size_t)q * (size_t)nn * st_bytes);
+  }
+  c.wtab = off;    off = align_up(off + sizeof(double) * 18 * (size_t)npad);
+  c.avgw = off;    off = align_up(off + sizeof(double) * 3 * (size_t)npad);
+  c.partial = off; off = align_up(off + sizeof(double) * kRedSlots * kMaxRedBlocks);
+  c.red_out = off; off = align_up(off + sizeof(double) * 8);
+  c.snap = off;    off = align_up(off + sizeof(double) * 4 * (size_t)nn);
+  c.total = off;
+  return c;
+}
+
+int check_mesh_args(const islbm_mesh *mesh, int lattice, int precision) {
+  if (!mesh) return fail(ISLBM_ERR_ARG, "mesh is NULL");
+  if (mesh->dim != 2 && mesh->dim != 3) return fail(ISLBM_ERR_ARG, "dim must be 2 or 3");
+  if ((mesh->dim == 2) != (lattice == ISLBM_D2Q9_D2Q5) || (mesh->dim == 3) != (lattice == ISLBM_D3Q19_D3Q7))
+    return fail(ISLBM_ERR_ARG, "lattice does not match dim (2-D: D2Q9+D2Q5, 3-D: D3Q19+D3Q7)");
+  if (precision != ISLBM_F64 && precision != ISLBM_F32_STORAGE) return fail(ISLBM_ERR_ARG, "unknown precision");
+  for (int a = 0; a < mesh->dim; ++a)
+    if (mesh->n[a] < 3) return fail(ISLBM_ERR_ARG, "need at least 3 nodes per axis");
+  return ISLBM_OK;
+}
+
+int npad_of(const islbm_mesh *mesh) {
+  int mx = 0;
+  for (int a = 0; a < mesh->dim; ++a) mx = mesh->n[a] > mx ? mesh->n[a] : mx;
+  return (mx + 31) / 32 * 32;
+}
+
+}  // namespace
+
+struct islbm {
+  int dim, precision;
+  int n[3];
+  long long nn;
+  int q, qf, qg;
+  size_t st_bytes;
+  double Ra, Pr, Ma, delta;
+  islbm_params prm;
+  double buoy;
+  DevMesh dm;
+  NodeParams np;
+  DiagParams dp;
+  bool uniform;            // every spacing == delta (pure-shift kernel valid)
+  char *ws;
+  Carve cv;
+  cudaStream_t stream;
+  int cur;                 // buf[cur] holds S_t (post-collision)
+  bool has_state;
+  bool other_is_pre;       // buf[1-cur] holds f_t itself (right after init / set)
+  bool snap_valid;
+  int kernel_choice;       // 0 auto, 1 generic, 2 tiled, 3 uniform shift
+  long long launches;
+  TiledPlan tiled;
+};
+
+extern "C" const char *islbm_last_error(void) { return g_err.c_str(); }
+extern "C" const char *islbm_version(void) { return "islbm-b200 0.1 (sm_100a)"; }
+
+extern "C" int islbm_workspace_bytes(const islbm_mesh *mesh, int lattice, int precision, size_t *bytes) {
+  if (!bytes) return fail(ISLBM_ERR_ARG, "bytes is NULL");
+  int rc = check_mesh_args(mesh, lattice, precision);
+  if (rc) return rc;
+  long long nn = 1;
+  for (int a = 0; a < mesh->dim; ++a) nn *= mesh->n[a];
+  const int q = mesh->dim == 2 ? 14 : 26;
+  *bytes = carve(nn, q, precision == ISLBM_F64 ? 8 : 4, npad_of(mesh)).total;
+  return ISLBM_OK;
+}
+
+// Parameter map: PAPER.md:53-72 (free-fall scaling), :248 (Ma = u_f/c_s, c_s = 1/sqrt 3), Table 1
+// (:206-212, characteristic length = effective height / minimal resolution), :124 (a_T), :177 (omega).
+static int derive_params(islbm *h, const islbm_mesh *mesh) {
+  islbm_params &p = h->prm;
+  for (int a = 0; a < 3; ++a)
+    p.L_eff[a] = a < h->dim ? mesh->x[a][h->n[a] - 1] - mesh->x[a][0] + h->delta : 1.0;
+  p.U = h->Ma / std::sqrt(3.0);
+  p.H_lu = p.L_eff[1] / h->delta;
+  p.nu = p.U * p.H_lu * std::sqrt(h->Pr / h->Ra);
+  p.alpha = p.nu / h->Pr;
+  p.gbeta = p.U * p.U / p.H_lu;
+  p.tau_f = 3.0 * p.nu + 0.5;
+  p.a_T = h->dim == 2 ? 20.0 * std::sqrt(3.0) * p.alpha - 4.0 : 42.0 * std::sqrt(3.0) * p.alpha - 6.0;
+  p.omega_bc = h->dim == 2 ? (4.0 + p.a_T) / 10.0 : (6.0 + p.a_T) / 21.0;
+  p.dt_star = p.U / p.H_lu;
+  if (!(p.tau_f > 0.5) || !std::isfinite(p.tau_f)) return fail(ISLBM_ERR_PARAM, "tau_f <= 1/2");
+  const double lo = h->dim == 2 ? -4.0 : -6.0;
+  if (!(p.a_T > lo && p.a_T < 1.0)) {
+    char b[160];
+    snprintf(b, sizeof b, "a_T = %.6g outside (%g, 1): temperature equilibrium weights would be negative", p.a_T, lo);
+    return fail(ISLBM_ERR_PARAM, b);
+  }
+  return ISLBM_OK;
+}
+
+static void set_node_params(islbm *h) {
+  const double tau = h->prm.tau_f;
+  NodeParams &np = h->np;
+  np.gbeta = h->prm.gbeta * h->buoy;
+  np.s_nu = 1.0 / tau;                                   // DESIGN.md A7
+  np.s_q = 8.0 * (2.0 * tau - 1.0) / (8.0 * tau - 1.0);
+  np.hs_nu = 1.0 - 0.5 * np.s_nu;
+  np.hs_q = 1.0 - 0.5 * np.s_q;
+  np.q_k = 3.0 - std::sqrt(3.0);
+  np.q_e = 4.0 * std::sqrt(3.0) - 6.0;
+  np.a_T = h->prm.a_T;
+}
+
+// 3-point Lagrange weights of the departure point x_j - c*delta on the
+// destination-centred stencil (A2, A3).  Offsets are
+// taken relative to x_j so that an exact unit spacing gives exactly (1,0,0)/(0,0,1).
+static void build_tables(const islbm *h, const islbm_mesh *mesh, int npad, std::vector<double> &wtab,
+                         std::vector<double> &avgw) {
+  wtab.assign((size_t)18 * npad, 0.0);
+  avgw.assign((size_t)3 * npad, 1.0);
+  for (int a = 0; a < h->dim; ++a) {
+    const int n = h->n[a];
+    const double *x = mesh->x[a];
+    for (int s = 0; s < 2; ++s) {
+      const double xi = s == 0 ? h->delta : -h->delta;   // c = -1 -> +delta ; c = +1 -> -delta
+      for (int j = 0; j < n; ++j) {
+        int b = j - 1 < 0 ? 0 : j - 1;
+        if (b > n - 3) b = n - 3;
+        const double d0 = x[b] - x[j], d1 = x[b + 1] - x[j], d2 = x[b + 2] - x[j];
+        double *w = &wtab[(size_t)((a * 2 + s) * 3) * npad + j];
+        w[0] = ((xi - d1) * (xi - d2)) / ((d0 - d1) * (d0 - d2));
+        w[(size_t)npad] = ((xi - d0) * (xi - d2)) / ((d1 - d0) * (d1 - d2));
+        w[(size_t)2 * npad] = ((xi - d0) * (xi - d1)) / ((d2 - d0) * (d2 - d1));
+      }
+    }
+    for (int j = 0; j < n; ++j) {   // Eq. 29 with ghost points one lattice unit outside (A14)
+      const double xm = j == 0 ? x[0] - h->delta : x[j - 1];
+      const double xp = j == n - 1 ? x[n - 1] + h->delta : x[j + 1];
+      avgw[(size_t)a * npad + j] = 0.5 * (xp - xm);
+    }
+  }
+}
+
+extern "C" int islbm_create(islbm_t **out, const islbm_mesh *mesh, int lattice, double Ra, double Pr, double Ma,
+                            int precision, void *dev_workspace, size_t bytes, void *cuda_stream) {
+  if (!out) return fail(ISLBM_ERR_ARG, "out is NULL");
+  *out = nullptr;
+  int rc = check_mesh_args(mesh, lattice, precision);
+  if (rc) return rc;
+  if (!(Ra > 0.0) || !(Pr > 0.0) || !(Ma > 0.0) || !std::isfinite(Ra + Pr + Ma))
+    return fail(ISLBM_ERR_PARAM, "Ra, Pr, Ma must be positive and finite");
+  if (!(mesh->delta > 0.0)) return fail(ISLBM_ERR_MESH, "delta must be positive");
+  bool uniform = true;
+  for (int a = 0; a < mesh->dim; ++a) {
+    if (!mesh->x[a]) return fail(ISLBM_ERR_ARG, "coordinate array is NULL");
+    for (int j = 1; j < mesh->n[a]; ++j) {
+      const double d = mesh->x[a][j] - mesh->x[a][j - 1];
+      if (!(d > 0.0)) return fail(ISLBM_ERR_MESH, "coordinates must be strictly increasing");
+      if (!(d >= mesh->delta * (1.0 - 1e-12)))
+        return fail(ISLBM_ERR_MESH, "a mesh spacing is smaller than delta: the departure point would leave the adjacent cell");
+      if (d != mesh->delta) uniform = false;
+    }
+  }
+  islbm *h = new islbm();
+  h->dim = mesh->dim;
+  h->precision = precision;
+  h->nn = 1;
+  for (int a = 0; a < 3; ++a) {
+    h->n[a] = a < mesh->dim ? mesh->n[a] : 1;
+    h->nn *= h->n[a];
+  }
+  h->qf = h->dim == 2 ? 9 : 19;
+  h->qg = h->dim == 2 ? 5 : 7;
+  h->q = h->qf + h->qg;
+  h->st_bytes = precision == ISLBM_F64 ? 8 : 4;
+  h->Ra = Ra; h->Pr = Pr; h->Ma = Ma; h->delta = mesh->delta;
+  h->buoy = 1.0;
+  h->uniform = uniform;
+  rc = derive_params(h, mesh);
+  if (rc) { delete h; return rc; }
+  set_node_params(h);
+  const int npad = npad_of(mesh);
+  h->cv = carve(h->nn, h->q, h->st_bytes, npad);
+  if (!dev_workspace) { delete h; return fail(ISLBM_ERR_WORKSPACE, "workspace is NULL"); }
+  if ((uintptr_t)dev_workspace % kAlign) { delete h; return fail(ISLBM_ERR_WORKSPACE, "workspace must be 256-byte aligned"); }
+  if (bytes < h->cv.total) {
+    char b[128];
+    snprintf(b, sizeof b, "workspace too small: %zu < %zu bytes", bytes, h->cv.total);
+    delete h;
+    return fail(ISLBM_ERR_WORKSPACE, b);
+  }
+  h->ws = (char *)dev_workspace;
+  h->stream = (cudaStream_t)cuda_stream;
+  std::vector<double> wtab, avgw;
+  build_tables(h, mesh, npad, wtab, avgw);
+  cudaError_t e = cudaMemcpy(h->ws + h->cv.wtab, wtab.data(), wtab.size() * sizeof(double), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess)
+    e = cudaMemcpy(h->ws + h->cv.avgw, avgw.data(), avgw.size() * sizeof(double), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) {
+    delete h;
+    return fail(ISLBM_ERR_CUDA, std::string("table upload: ") + cudaGetErrorString(e));
+  }
+  DevMesh &dm = h->dm;
+  dm.nx = h->n[0]; dm.ny = h->n[1]; dm.nz = h->n[2];
+  dm.npad = npad;
+  dm.nn = h->nn;
+  dm.wtab = (const double *)(h->ws + h->cv.wtab);
+  dm.avgw = (const double *)(h->ws + h->cv.avgw);
+  dm.omega_bc = h->prm.omega_bc;
+  dm.T_hot = 0.5;      // PAPER.md:237, 430; BASELINE.json configs (A11)
+  dm.T_cold = -0.5;
+  h->dp.q_lo = (mesh->x[0][1] - mesh->x[0][0]) / mesh->delta;
+  h->dp.q_hi = (mesh->x[0][h->n[0] - 1] - mesh->x[0][h->n[0] - 2]) / mesh->delta;
+  h->dp.T0 = 0.0;
+  h->cur = 0;
+  h->has_state = false;
+  h->other_is_pre = false;
+  h->snap_valid = false;
+  h->kernel_choice = 0;
+  h->launches = 0;
+  rc = tiled_plan_create(h->tiled, h->dim, h->n, h->precision, h->ws + h->cv.buf[0], h->ws + h->cv.buf[1], g_err);
+  if (rc) { delete h; return rc; }
+  *out = h;
+  return ISLBM_OK;
+}
+
+extern "C" void islbm_destroy(islbm_t *h) { delete h; }
+
+extern "C" int islbm_get_params(const islbm_t *h, islbm_params *out) {
+  if (!h || !out) return fail(ISLBM_ERR_ARG, "NULL argument");
+  *out = h->prm;
+  return ISLBM_OK;
+}
+
+extern "C" int islbm_set_buoyancy_scale(islbm_t *h, double s) {
+  if (!h) return fail(ISLBM_ERR_ARG, "NULL handle");
+  if (h->has_state && s != h->buoy)
+    return fail(ISLBM_ERR_STATE, "set the buoyancy scale before islbm_init / islbm_set_populations "
+                                 "(the stored post-collision state already contains the force)");
+  h->buoy = s;
+  set_node_params(h);
+  return ISLBM_OK;
+}
+
+extern "C" long long islbm_launch_count(const islbm_t *h) { return h ? h->launches : 0; }
+
+// ---------------------------------------------------------------------------
+// dispatch helpers
+// ---------------------------------------------------------------------------
+#define DISPATCH(h, CALL)                                                     \
+  do {                                                                        \
+    if ((h)->dim == 2) {                                                      \
+      if ((h)->precision == ISLBM_F64) { CALL(2, double); } else { CALL(2, float); } \
+    } else {                                                                  \
+      if ((h)->precision == ISLBM_F64) { CALL(3, double); } else { CALL(3, float); } \
+    }                                                                         \
+  } while (0)
+
+static inline unsigned cdiv(long long a, long long b) { return (unsigned)((a + b - 1) / b); }
+
+static void generic_geometry(const islbm *h, dim3 &grid, dim3 &block) {
+  block = h->dim == 2 ? dim3(64, 4, 1) : dim3(32, 4, 2);
+  grid = dim3(cdiv(h->n[0], block.x), cdiv(h->n[1], block.y), cdiv(h->n[2], block.z));
+}
+
+template <int DIM, typename ST>
+static void launch_load(islbm *h, const double *f, const double *g, bool generate, unsigned long long seed, double amp) {
+  ST *pre = (ST *)(h->ws + h->cv.buf[1 - h->cur]);
+  ST *post = (ST *)(h->ws + h->cv.buf[h->cur]);
+  const unsigned blocks = cdiv(h->nn, 256);
+  if (generate)
+    k_load_state<DIM, ST, true><<<blocks, 256, 0, h->stream>>>(h->dm, h->np, nullptr, nullptr, seed, amp, pre, post);
+  else
+    k_load_state<DIM, ST, false><<<blocks, 256, 0, h->stream>>>(h->dm, h->np, f, g, 0ull, 0.0, pre, post);
+  h->launches++;
+}
+
+static int load_state(islbm *h, const double *f, const double *g, bool generate, unsigned long long seed, double amp) {
+#define CALL(D, T) launch_load<D, T>(h, f, g, generate, seed, amp)
+  DISPATCH(h, CALL);
+#undef CALL
+  CUDA_TRY(cudaPeekAtLastError());
+  h->has_state = true;
+  h->other_is_pre = true;
+  h->snap_valid = false;
+  return ISLBM_OK;
+}
+
+extern "C" int islbm_init(islbm_t *h, unsigned long long seed, double noise_amp) {
+  if (!h) return fail(ISLBM_ERR_ARG, "NULL handle");
+  return load_state(h, nullptr, nullptr, true, seed, noise_amp);
+}
+
+extern "C" int islbm_set_populations(islbm_t *h, const double *f, const double *g) {
+  if (!h || !f || !g) return fail(ISLBM_ERR_ARG, "NULL argument");
+  return load_state(h, f, g, false, 0ull, 0.0);
+}
+
+template <int DIM, typename ST>
+static void launch_generic_step(islbm *h, bool collide, double *fout, double *gout) {
+  dim3 grid, block;
+  generic_geometry(h, grid, block);
+  if (collide) {
+    const ST *src = (const ST *)(h->ws + h->cv.buf[h->cur]);
+    ST *dst = (ST *)(h->ws + h->cv.buf[1 - h->cur]);
+    k_step_generic<DIM, ST, true><<<grid, block, 0, h->stream>>>(h->dm, h->np, src, dst, nullptr, nullptr);
+  } else {
+    const ST *src = (const ST *)(h->ws + h->cv.buf[1 - h->cur]);
+    k_step_generic<DIM, ST, false><<<grid, block, 0, h->stream>>>(h->dm, h->np, src, nullptr, fout, gout);
+  }
+  h->launches++;
+}
+
+static int effective_kernel(const islbm *h) {
+  if (h->kernel_choice != 0) return h->kernel_choice;
+  return h->tiled.available ? 2 : 1;
+}
+
+extern "C" const char *islbm_kernel_name(const islbm_t *h) {
+  if (!h) return "";
+  switch (effective_kernel(h)) {
+    case 2: return h->tiled.name;
+    case 3: return "uniform_shift";
+    default: return "generic_global";
+  }
+}
+
+extern "C" int islbm_set_kernel(islbm_t *h, int which) {
+  if (!h) return fail(ISLBM_ERR_ARG, "NULL handle");
+  if (which < 0 || which > 3) return fail(ISLBM_ERR_ARG, "kernel selector must be 0..3");
+  if (which == 2 && !h->tiled.available) return fail(ISLBM_ERR_ARG, "tiled kernel not available for this mesh");
+  if (which == 3) return fail(ISLBM_ERR_ARG, "uniform-shift kernel not built yet");
+  h->kernel_choice = which;
+  return ISLBM_OK;
+}
+
+extern "C" int islbm_step(islbm_t *h, int n) {
+  if (!h) return fail(ISLBM_ERR_ARG, "NULL handle");
+  if (n < 0) return fail(ISLBM_ERR_ARG, "n < 0");
+  if (!h->has_state) return fail(ISLBM_ERR_STATE, "islbm_step before islbm_init / islbm_set_populations");
+  const int which = effective_kernel(h);
+  for (int s = 0; s < n; ++s) {
+    if (which == 2) {
+      int rc = tiled_step(h->tiled, h->dm, h->np, h->cur, h->stream, g_err);
+      if (rc) return rc;
+      h->launches += h->tiled.launches_per_step;
+    } else {
+#define CALL(D, T) launch_generic_step<D, T>(h, true, nullptr, nullptr)
+      DISPATCH(h, CALL);
+#undef CALL
+    }
+    h->cur ^= 1;
+    h->other_is_pre = false;
+  }
+  CUDA_TRY(cudaPeekAtLastError());
+  return ISLBM_OK;
+}
+
+template <int DIM, typename ST>
+static void launch_export(islbm *h, double *f, double *g) {
+  const ST *buf = (const ST *)(h->ws + h->cv.buf[1 - h->cur]);
+  k_export<DIM, ST><<<cdiv(h->nn, 256), 256, 0, h->stream>>>(h->dm, buf, f, g);
+  h->launches++;
+}
+
+extern "C" int islbm_get_populations(islbm_t *h, double *f, double *g) {
+  if (!h || !f || !g) return fail(ISLBM_ERR_ARG, "NULL argument");
+  if (!h->has_state) return fail(ISLBM_ERR_STATE, "no state");
+  if (h->other_is_pre) {
+#define CALL(D, T) launch_export<D, T>(h, f, g)
+    DISPATCH(h, CALL);
+#undef CALL
+  } else {
+    // f_t = stream/interpolate/walls(S_{t-1}); the previous ping-pong buffer is intact
+#define CALL(D, T) launch_generic_step<D, T>(h, false, f, g)
+    DISPATCH(h, CALL);
+#undef CALL
+  }
+  CUDA_TRY(cudaPeekAtLastError());
+  return ISLBM_OK;
+}
+
+template <int DIM, typename ST>
+static void launch_fields(islbm *h, double *rho, double *u, double *v, double *w, double *T) {
+  const ST *S = (const ST *)(h->ws + h->cv.buf[h->cur]);
+  k_fields<DIM, ST><<<cdiv(h->nn, 256), 256, 0, h->stream>>>(h->dm, h->np, S, rho, u, v, w, T);
+  h->launches++;
+}
+
+extern "C" int islbm_fields(islbm_t *h, double *rho, double *u, double *v, double *w, double *T) {
+  if (!h) return fail(ISLBM_ERR_ARG, "NULL handle");
+  if (!h->has_state) return fail(ISLBM_ERR_STATE, "no state");
+#define CALL(D, T_) launch_fields<D, T_>(h, rho, u, v, w, T)
+  DISPATCH(h, CALL);
+#undef CALL
+  CUDA_TRY(cudaPeekAtLastError());
+  return ISLBM_OK;
+}
+
+static int red_blocks(const islbm *h) {
+  long long b = (h->nn + kRedThreads - 1) / kRedThreads;
+  return (int)(b < kMaxRedBlocks ? b : kMaxRedBlocks);
+}
+
+template <int DIM, typename ST>
+static void launch_nusselt(islbm *h, int nb) {
+  const ST *S = (const ST *)(h->ws + h->cv.buf[h->cur]);
+  double *partial = (double *)(h->ws + h->cv.partial);
+  k_nusselt_partial<DIM, ST><<<nb, kRedThreads, 0, h->stream>>>(h->dm, h->np, h->dp, S, partial);
+  k_reduce_final<<<1, kRedThreads, 0, h->stream>>>(partial, nb, (double *)(h->ws + h->cv.red_out));
+  h->launches += 2;
+}
+
+extern "C" int islbm_nusselt(islbm_t *h, double out[5]) {
+  if (!h || !out) return fail(ISLBM_ERR_ARG, "NULL argument");
+  if (!h->has_state) return fail(ISLBM_ERR_STATE, "no state");
+  const int nb = red_blocks(h);
+#define CALL(D, T) launch_nusselt<D, T>(h, nb)
+  DISPATCH(h, CALL);
+#undef CALL
+  CUDA_TRY(cudaPeekAtLastError());
+  double s[kRedSlots];
+  CUDA_TRY(cudaMemcpyAsync(s, h->ws + h->cv.red_out, sizeof s, cudaMemcpyDeviceToHost, h->stream));
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  const islbm_params &p = h->prm;
+  const double area = p.L_eff[1] * (h->dim == 3 ? p.L_eff[2] : 1.0);
+  const double vol = area * p.L_eff[0];
+  out[0] = -p.H_lu * s[0] / area;
+  out[1] = -p.H_lu * s[1] / area;
+  out[2] = std::sqrt(h->Ra / h->Pr) * (s[2] / vol) / p.U;
+  out[3] = (s[3] / vol) / (p.U * p.U);
+  out[4] = std::sqrt(h->Ra * h->Pr) * (s[4] / vol) / p.U + 1.0;
+  for (int i = 0; i < 5; ++i)
+    if (!std::isfinite(out[i])) return fail(ISLBM_ERR_NONFINITE, "non-finite diagnostic: the run has diverged");
+  return ISLBM_OK;
+}
+
+template <int DIM, typename ST>
+static void launch_residual(islbm *h, int nb) {
+  const ST *S = (const ST *)(h->ws + h->cv.buf[h->cur]);
+  double *partial = (double *)(h->ws + h->cv.partial);
+  k_residual_partial<DIM, ST><<<nb, kRedThreads, 0, h->stream>>>(h->dm, h->np, S, (double *)(h->ws + h->cv.snap), partial);
+  k_reduce_final<<<1, kRedThreads, 0, h->stream>>>(partial, nb, (double *)(h->ws + h->cv.red_out));
+  h->launches += 2;
+}
+
+extern "C" int islbm_steady_residual(islbm_t *h, double out[2]) {
+  if (!h || !out) return fail(ISLBM_ERR_ARG, "NULL argument");
+  if (!h->has_state) return fail(ISLBM_ERR_STATE, "no state");
+  if (!h->snap_valid) CUDA_TRY(cudaMemsetAsync(h->ws + h->cv.snap, 0, sizeof(double) * 4 * (size_t)h->nn, h->stream));
+  const int nb = red_blocks(h);
+#define CALL(D, T) launch_residual<D, T>(h, nb)
+  DISPATCH(h, CALL);
+#undef CALL
+  CUDA_TRY(cudaPeekAtLastError());
+  double s[kRedSlots];
+  CUDA_TRY(cudaMemcpyAsync(s, h->ws + h->cv.red_out, sizeof s, cudaMemcpyDeviceToHost, h->stream));
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  if (!h->snap_valid) {
+    out[0] = out[1] = 1.0;
+    h->snap_valid = true;
+  } else {
+    out[0] = s[1] > 0.0 ? s[0] / s[1] : (s[0] > 0.0 ? 1.0 : 0.0);
+    out[1] = s[3] > 0.0 ? s[2] / s[3] : (s[2] > 0.0 ? 1.0 : 0.0);
+  }
+  return ISLBM_OK;
+}

@@ -1,0 +1,282 @@
+// islbm_kernels.cuh — device-side data model and the generic (global-memory)
+// kernels of the ISLBM step.
+//
+// State convention: HBM holds POST-collision populations S_t =
+// collide(f_t).  One step is  f_{t+1} = stream/interpolate/walls(S_t)  followed,
+// in the same kernel, by  S_{t+1} = collide(f_{t+1}),  so each node collides
+// once per step and every population is read once and written once
+// (PAPER.md:150-154 gives the collide -> stream order this is equivalent to).
+//
+// Layout: structure-of-arrays planes [q][z][y][x], flow planes first, then the
+// temperature planes; storage type ST is double, or float holding the
+// deviation f_q - w_q (ISLBM_F32_STORAGE).
+#pragma once
+
+#include <cstdint>
+#include <utility>
+
+#include "islbm_lattice.cuh"
+
+namespace islbmk {
+
+constexpr int kMaxQ = 26;
+
+struct DevMesh {
+  int nx, ny, nz;
+  int npad;              // pitch of the per-axis tables
+  long long nn;          // nx*ny*nz
+  // interpolation weights, [axis 3][sign 2 (0: c=-1, 1: c=+1)][k 3][npad]; the
+  // stencil of node j is {b, b+1, b+2}, b = clamp(j-1, 0, n-3) (A2)
+  const double *wtab;
+  const double *avgw;    // Eq. 29 weights, [axis 3][npad]
+  double omega_bc;       // Eq. 22 weight
+  double T_hot, T_cold;  // x-lo / x-hi wall temperatures
+};
+
+__device__ __forceinline__ const double *wrow(const DevMesh &m, int axis, int sign, int k) {
+  return m.wtab + ((axis * 2 + sign) * 3 + k) * (long long)m.npad;
+}
+
+// storage <-> fp64 value of flow population q (deviation storage for float)
+template <typename ST, int DIM> struct Store;
+template <int DIM> struct Store<double, DIM> {
+  static __device__ __forceinline__ double bias(int) { return 0.0; }
+};
+template <int DIM> struct Store<float, DIM> {
+  static __device__ __forceinline__ double bias(int q) { return wflow<DIM>(q); }
+};
+
+template <typename ST>
+__device__ __forceinline__ double ldv(const ST *p) { return (double)__ldg(p); }
+
+// SplitMix64 by counter (A15): the (k+1)-th output for `seed`.
+__device__ __forceinline__ unsigned long long splitmix64_at(unsigned long long seed, unsigned long long k) {
+  unsigned long long z = seed + (k + 1ull) * 0x9E3779B97F4A7C15ull;
+  z = (z ^ (z >> 30)) * 0xBF58476D1CE4E5B9ull;
+  z = (z ^ (z >> 27)) * 0x94D049BB133111EBull;
+  return z ^ (z >> 31);
+}
+
+// ---------------------------------------------------------------------------
+// per-thread stencil context of the generic kernel
+// ---------------------------------------------------------------------------
+template <int DIM>
+struct NodeCtx {
+  int i[3];        // node index
+  int b[3];        // stencil base per axis
+  bool lo[3], hi[3];
+  double w[3][2][3];
+  long long c;     // linear node index
+};
+
+template <int DIM>
+__device__ __forceinline__ void make_ctx(const DevMesh &m, int ix, int iy, int iz, NodeCtx<DIM> &cx) {
+  const int n[3] = {m.nx, m.ny, m.nz};
+  cx.i[0] = ix; cx.i[1] = iy; cx.i[2] = iz;
+  cx.c = ((long long)iz * m.ny + iy) * m.nx + ix;
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    if (a < DIM) {
+      cx.lo[a] = cx.i[a] == 0;
+      cx.hi[a] = cx.i[a] == n[a] - 1;
+      cx.b[a] = min(max(cx.i[a] - 1, 0), n[a] - 3);
+#pragma unroll
+      for (int s = 0; s < 2; ++s)
+#pragma unroll
+        for (int k = 0; k < 3; ++k) cx.w[a][s][k] = __ldg(wrow(m, a, s, k) + cx.i[a]);
+    } else {
+      cx.lo[a] = cx.hi[a] = false;
+      cx.b[a] = 0;
+    }
+  }
+}
+
+// Does the departure point of velocity (EX,EY,EZ) lie beyond a wall? (A4)
+template <int DIM, int EX, int EY, int EZ>
+__device__ __forceinline__ bool crosses(const NodeCtx<DIM> &cx) {
+  bool r = false;
+  if (EX == 1) r |= cx.lo[0];
+  if (EX == -1) r |= cx.hi[0];
+  if (EY == 1) r |= cx.lo[1];
+  if (EY == -1) r |= cx.hi[1];
+  if (DIM == 3 && EZ == 1) r |= cx.lo[2];
+  if (DIM == 3 && EZ == -1) r |= cx.hi[2];
+  return r;
+}
+
+// Separable 3-point Lagrange interpolation of one plane at the departure point
+// x - e*delta; x first, then y, then z.
+template <int DIM, int EX, int EY, int EZ, typename ST>
+__device__ __forceinline__ double interp_plane(const DevMesh &m, const ST *__restrict__ plane,
+                                               const NodeCtx<DIM> &cx) {
+  constexpr int CX = EX != 0 ? 3 : 1, CY = EY != 0 ? 3 : 1, CZ = (DIM == 3 && EZ != 0) ? 3 : 1;
+  constexpr int SX = EX > 0 ? 1 : 0, SY = EY > 0 ? 1 : 0, SZ = EZ > 0 ? 1 : 0;
+  const int x0 = EX != 0 ? cx.b[0] : cx.i[0];
+  const int y0 = EY != 0 ? cx.b[1] : cx.i[1];
+  const int z0 = (DIM == 3 && EZ != 0) ? cx.b[2] : cx.i[2];
+  double accz = 0.0;
+#pragma unroll
+  for (int kz = 0; kz < CZ; ++kz) {
+    double accy = 0.0;
+#pragma unroll
+    for (int ky = 0; ky < CY; ++ky) {
+      const ST *row = plane + ((long long)(z0 + kz) * m.ny + (y0 + ky)) * m.nx + x0;
+      double accx;
+      if (CX == 3) {
+        accx = cx.w[0][SX][0] * ldv(row);
+        accx = fma(cx.w[0][SX][1], ldv(row + 1), accx);
+        accx = fma(cx.w[0][SX][2], ldv(row + 2), accx);
+      } else {
+        accx = ldv(row);
+      }
+      accy = CY == 3 ? (ky == 0 ? cx.w[1][SY][0] * accx : fma(cx.w[1][SY][ky], accx, accy)) : accx;
+    }
+    accz = CZ == 3 ? (kz == 0 ? cx.w[2][SZ][0] * accy : fma(cx.w[2][SZ][kz], accy, accz)) : accy;
+  }
+  return accz;
+}
+
+// New value of flow population Q at the node: interpolation, or half-way
+// bounce-back f_Q(x,t+1) = f+_opp(Q)(x,t) (Eq. 21).
+template <int DIM, int Q, typename ST>
+__device__ __forceinline__ double pull_f(const DevMesh &m, const ST *__restrict__ src, const NodeCtx<DIM> &cx) {
+  constexpr int EX = evel<DIM>(Q, 0), EY = evel<DIM>(Q, 1), EZ = evel<DIM>(Q, 2);
+  if (crosses<DIM, EX, EY, EZ>(cx)) return ldv(src + (long long)opposite<DIM>(Q) * m.nn + cx.c);
+  return interp_plane<DIM, EX, EY, EZ>(m, src + (long long)Q * m.nn, cx);
+}
+
+// Temperature population Q: interpolation; anti-bounce-back on the isothermal
+// x-walls (Eq. 22); bounce-back on the adiabatic walls (Eq. 23).
+template <int DIM, int Q, typename ST>
+__device__ __forceinline__ double pull_g(const DevMesh &m, const ST *__restrict__ srcg, const NodeCtx<DIM> &cx) {
+  constexpr int EX = evel<DIM>(Q, 0), EY = evel<DIM>(Q, 1), EZ = evel<DIM>(Q, 2);
+  if (crosses<DIM, EX, EY, EZ>(cx)) {
+    const double gb = ldv(srcg + (long long)opposite<DIM>(Q) * m.nn + cx.c);
+    if (EX != 0) return -gb + m.omega_bc * (cx.lo[0] ? m.T_hot : m.T_cold);
+    return gb;
+  }
+  return interp_plane<DIM, EX, EY, EZ>(m, srcg + (long long)Q * m.nn, cx);
+}
+
+template <int DIM, typename ST, int... Qs>
+__device__ __forceinline__ void pull_all_f(const DevMesh &m, const ST *src, const NodeCtx<DIM> &cx,
+                                           double *f, std::integer_sequence<int, Qs...>) {
+  ((f[Qs] = pull_f<DIM, Qs>(m, src, cx)), ...);
+}
+template <int DIM, typename ST, int... Qs>
+__device__ __forceinline__ void pull_all_g(const DevMesh &m, const ST *srcg, const NodeCtx<DIM> &cx,
+                                           double *g, std::integer_sequence<int, Qs...>) {
+  ((g[Qs] = pull_g<DIM, Qs>(m, srcg, cx)), ...);
+}
+
+// ---------------------------------------------------------------------------
+// generic step: one thread per node, neighbours read from global memory
+// through L1/L2.  COLLIDE = false writes the pre-collision f_{t+1}, g_{t+1} as
+// fp64 to fout/gout (islbm_get_populations).
+// ---------------------------------------------------------------------------
+template <int DIM, typename ST, bool COLLIDE>
+__global__ void __launch_bounds__(256)
+k_step_generic(DevMesh m, NodeParams np, const ST *__restrict__ src, ST *__restrict__ dst,
+               double *__restrict__ fout, double *__restrict__ gout) {
+  constexpr int QF = Lat<DIM>::QF, QG = Lat<DIM>::QG;
+  const int ix = blockIdx.x * blockDim.x + threadIdx.x;
+  const int iy = blockIdx.y * blockDim.y + threadIdx.y;
+  const int iz = blockIdx.z * blockDim.z + threadIdx.z;
+  if (ix >= m.nx || iy >= m.ny || iz >= m.nz) return;
+  NodeCtx<DIM> cx;
+  make_ctx<DIM>(m, ix, iy, iz, cx);
+  double f[QF], g[QG];
+  pull_all_f<DIM>(m, src, cx, f, std::make_integer_sequence<int, QF>{});
+  pull_all_g<DIM>(m, src + (long long)QF * m.nn, cx, g, std::make_integer_sequence<int, QG>{});
+#pragma unroll
+  for (int q = 0; q < QF; ++q) f[q] += Store<ST, DIM>::bias(q);
+  if (COLLIDE) {
+    collide_node(f, g, np);
+#pragma unroll
+    for (int q = 0; q < QF; ++q) dst[(long long)q * m.nn + cx.c] = (ST)(f[q] - Store<ST, DIM>::bias(q));
+#pragma unroll
+    for (int q = 0; q < QG; ++q) dst[(long long)(QF + q) * m.nn + cx.c] = (ST)g[q];
+  } else {
+#pragma unroll
+    for (int q = 0; q < QF; ++q) fout[(long long)q * m.nn + cx.c] = f[q];
+#pragma unroll
+    for (int q = 0; q < QG; ++q) gout[(long long)q * m.nn + cx.c] = g[q];
+  }
+}
+
+// ---------------------------------------------------------------------------
+// state load / init / export
+// ---------------------------------------------------------------------------
+
+// pre-collision f,g (fp64, user arrays, or generated) -> `pre` buffer (storage
+// form, kept for islbm_get_populations) and collided -> `post` buffer.
+template <int DIM, typename ST, bool GENERATE>
+__global__ void __launch_bounds__(256)
+k_load_state(DevMesh m, NodeParams np, const double *__restrict__ fin, const double *__restrict__ gin,
+             unsigned long long seed, double amp, ST *__restrict__ pre, ST *__restrict__ post) {
+  constexpr int QF = Lat<DIM>::QF, QG = Lat<DIM>::QG;
+  const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= m.nn) return;
+  double f[QF], g[QG];
+  if (GENERATE) {
+    const unsigned long long z = splitmix64_at(seed, (unsigned long long)c);
+    const double r = (double)(z >> 11) * (1.0 / 9007199254740992.0);
+    rest_equilibrium<QF, QG>(f, g, amp * (2.0 * r - 1.0), np.a_T);
+  } else {
+#pragma unroll
+    for (int q = 0; q < QF; ++q) f[q] = fin[(long long)q * m.nn + c];
+#pragma unroll
+    for (int q = 0; q < QG; ++q) g[q] = gin[(long long)q * m.nn + c];
+  }
+#pragma unroll
+  for (int q = 0; q < QF; ++q) pre[(long long)q * m.nn + c] = (ST)(f[q] - Store<ST, DIM>::bias(q));
+#pragma unroll
+  for (int q = 0; q < QG; ++q) pre[(long long)(QF + q) * m.nn + c] = (ST)g[q];
+  collide_node(f, g, np);
+#pragma unroll
+  for (int q = 0; q < QF; ++q) post[(long long)q * m.nn + c] = (ST)(f[q] - Store<ST, DIM>::bias(q));
+#pragma unroll
+  for (int q = 0; q < QG; ++q) post[(long long)(QF + q) * m.nn + c] = (ST)g[q];
+}
+
+// storage-form buffer -> fp64 user arrays
+template <int DIM, typename ST>
+__global__ void __launch_bounds__(256)
+k_export(DevMesh m, const ST *__restrict__ buf, double *__restrict__ fout, double *__restrict__ gout) {
+  constexpr int QF = Lat<DIM>::QF, QG = Lat<DIM>::QG;
+  const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= m.nn) return;
+#pragma unroll
+  for (int q = 0; q < QF; ++q) fout[(long long)q * m.nn + c] = (double)buf[(long long)q * m.nn + c] + Store<ST, DIM>::bias(q);
+#pragma unroll
+  for (int q = 0; q < QG; ++q) gout[(long long)q * m.nn + c] = (double)buf[(long long)(QF + q) * m.nn + c];
+}
+
+template <int DIM, typename ST>
+__device__ __forceinline__ void load_post_node(const DevMesh &m, const ST *__restrict__ S, long long c,
+                                               double (&f)[Lat<DIM>::QF], double (&g)[Lat<DIM>::QG]) {
+  constexpr int QF = Lat<DIM>::QF, QG = Lat<DIM>::QG;
+#pragma unroll
+  for (int q = 0; q < QF; ++q) f[q] = ldv(S + (long long)q * m.nn + c) + Store<ST, DIM>::bias(q);
+#pragma unroll
+  for (int q = 0; q < QG; ++q) g[q] = ldv(S + (long long)(QF + q) * m.nn + c);
+}
+
+// macroscopic fields from the post-collision state
+template <int DIM, typename ST>
+__global__ void __launch_bounds__(256)
+k_fields(DevMesh m, NodeParams np, const ST *__restrict__ S, double *rho, double *u, double *v, double *w, double *T) {
+  const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (c >= m.nn) return;
+  double f[Lat<DIM>::QF], g[Lat<DIM>::QG];
+  load_post_node<DIM>(m, S, c, f, g);
+  double r, uu, vv, ww, tt;
+  fields_from_post(f, g, np, r, uu, vv, ww, tt);
+  if (rho) rho[c] = r;
+  if (u) u[c] = uu;
+  if (v) v[c] = vv;
+  if (w && DIM == 3) w[c] = ww;
+  if (T) T[c] = tt;
+}
+
+}  // namespace islbmk

@@ -1,0 +1,293 @@
+// islbm_lattice.cuh — node-local arithmetic of the ISLBM step for sm_100a.
+//
+// Hand-factored MRT collisions (no dense M / M^-1 products): the moments of
+// Eq. 10/11 and Eq. 15/16 are formed from symmetric /
+// antisymmetric partial sums of the populations, relaxed per Eq. 17 / Eq. 19
+// with the Guo forcing moments of Eq. 12/13 (PAPER.md:100-
+// 104; last entry of Eq. 12 read as u*Fy + v*Fx, A8), and mapped back
+// with M^-1 = M^T diag(1/|row|^2) (rows are mutually orthogonal).  The body
+// force is F = rho*g*beta*(T - T0)*y^ with T0 = 0, so Fx = Fz = 0
+// is folded in.  Relaxation rates: DESIGN.md A7.
+//
+// Direction ordering: include/islbm.h.  Everything here is fp64.
+#pragma once
+
+#ifndef ISLBM_HD
+#ifdef __CUDACC__
+#define ISLBM_HD __host__ __device__ __forceinline__
+#else
+#define ISLBM_HD inline
+#endif
+#endif
+
+namespace islbmk {
+
+struct NodeParams {
+  double gbeta;   // g*beta in lattice units, times the buoyancy test scale
+  double s_nu;    // 1/tau_f         (e, eps, stress moments)
+  double s_q;     // 8(2tau-1)/(8tau-1)  (heat-flux-like and third-order moments)
+  double hs_nu;   // 1 - s_nu/2
+  double hs_q;    // 1 - s_q/2
+  double q_k;     // 3 - sqrt(3)     (temperature flux moments)
+  double q_e;     // 4 sqrt(3) - 6   (remaining temperature moments)
+  double a_T;     // Eq. 15/16
+};
+
+template <int DIM> struct Lat;
+template <> struct Lat<2> { static constexpr int QF = 9, QG = 5; };
+template <> struct Lat<3> { static constexpr int QF = 19, QG = 7; };
+
+// velocity component a of flow direction q (temperature directions are the first QG)
+template <int DIM>
+ISLBM_HD constexpr int evel(int q, int a) {
+  if (DIM == 2) {
+    constexpr int t[9][3] = {{0, 0, 0}, {1, 0, 0}, {0, 1, 0}, {-1, 0, 0}, {0, -1, 0},
+                             {1, 1, 0}, {-1, 1, 0}, {-1, -1, 0}, {1, -1, 0}};
+    return t[q][a];
+  } else {
+    constexpr int t[19][3] = {{0, 0, 0},
+                              {1, 0, 0}, {-1, 0, 0}, {0, 1, 0}, {0, -1, 0}, {0, 0, 1}, {0, 0, -1},
+                              {1, 1, 0}, {-1, 1, 0}, {1, -1, 0}, {-1, -1, 0},
+                              {1, 0, 1}, {-1, 0, 1}, {1, 0, -1}, {-1, 0, -1},
+                              {0, 1, 1}, {0, -1, 1}, {0, 1, -1}, {0, -1, -1}};
+    return t[q][a];
+  }
+}
+
+template <int DIM>
+ISLBM_HD constexpr int opposite(int q) {
+  if (DIM == 2) {
+    constexpr int t[9] = {0, 3, 4, 1, 2, 7, 8, 5, 6};
+    return t[q];
+  } else {
+    constexpr int t[19] = {0, 2, 1, 4, 3, 6, 5, 10, 9, 8, 7, 14, 13, 12, 11, 18, 17, 16, 15};
+    return t[q];
+  }
+}
+
+// lattice weights of the rest equilibrium (rho = 1, u = 0): M^-1 m_eq
+template <int DIM>
+ISLBM_HD constexpr double wflow(int q) {
+  if (DIM == 2) return q == 0 ? 4.0 / 9.0 : (q < 5 ? 1.0 / 9.0 : 1.0 / 36.0);
+  return q == 0 ? 1.0 / 3.0 : (q < 7 ? 1.0 / 18.0 : 1.0 / 36.0);
+}
+
+// ---------------------------------------------------------------------------
+// D2Q9 + D2Q5
+// ---------------------------------------------------------------------------
+ISLBM_HD void collide_node(double (&f)[9], double (&g)[5], const NodeParams &p) {
+  const double T = g[0] + g[1] + g[2] + g[3] + g[4];
+  const double sa = (f[1] + f[3]) + (f[2] + f[4]);   // axis shell
+  const double sd = (f[5] + f[7]) + (f[6] + f[8]);   // diagonal shell
+  const double rho = f[0] + sa + sd;
+  const double Fy = rho * p.gbeta * T;
+  const double ax = f[1] - f[3], ay = f[2] - f[4];
+  const double dx = (f[5] - f[7]) + (f[8] - f[6]);    // sum cx over diagonals
+  const double dy = (f[5] - f[7]) + (f[6] - f[8]);    // sum cy over diagonals
+  const double jx = ax + dx, jy = ay + dy;
+  const double inv = 1.0 / rho;
+  const double u = jx * inv, v = (jy + 0.5 * Fy) * inv;
+  const double u2 = u * u + v * v;
+  // moments (Eq. 10 order): e, eps, qx, qy, pxx, pxy
+  const double me = -4.0 * f[0] - sa + 2.0 * sd;
+  const double meps = 4.0 * f[0] - 2.0 * sa + sd;
+  const double mqx = -2.0 * ax + dx;
+  const double mqy = -2.0 * ay + dy;
+  const double mpxx = (f[1] + f[3]) - (f[2] + f[4]);
+  const double mpxy = (f[5] + f[7]) - (f[6] + f[8]);
+  const double vF = v * Fy;
+  // Delta m_k / |row_k|^2
+  const double de = (-p.s_nu * (me - rho * (-2.0 + 3.0 * u2)) + p.hs_nu * (6.0 * vF)) * (1.0 / 36.0);
+  const double deps = (-p.s_nu * (meps - rho * (1.0 - 3.0 * u2)) - p.hs_nu * (6.0 * vF)) * (1.0 / 36.0);
+  const double djy = Fy * (1.0 / 6.0);
+  const double dqx = (-p.s_q * (mqx + rho * u)) * (1.0 / 12.0);
+  const double dqy = (-p.s_q * (mqy + rho * v) - p.hs_q * Fy) * (1.0 / 12.0);
+  const double dpxx = (-p.s_nu * (mpxx - rho * (u * u - v * v)) - p.hs_nu * (2.0 * vF)) * 0.25;
+  const double dpxy = (-p.s_nu * (mpxy - rho * (u * v)) + p.hs_nu * (u * Fy)) * 0.25;
+  // temperature moments (Eq. 15 order)
+  const double n1 = g[1] - g[3], n2 = g[2] - g[4];
+  const double gs = (g[1] + g[3]) + (g[2] + g[4]);
+  const double n3 = -4.0 * g[0] + gs;
+  const double n4 = (g[1] + g[3]) - (g[2] + g[4]);
+  const double e1 = (-p.q_k * (n1 - u * T)) * 0.5;
+  const double e2 = (-p.q_k * (n2 - v * T)) * 0.5;
+  const double e3 = (-p.q_e * (n3 - p.a_T * T)) * (1.0 / 20.0);
+  const double e4 = (-p.q_e * n4) * 0.25;
+  // f+ = f + M^T d
+  const double ca = -de - 2.0 * deps;          // common part, axis shell
+  const double cd = 2.0 * de + deps;           // common part, diagonal shell
+  const double tx = -2.0 * dqx, ty = djy - 2.0 * dqy;
+  const double sx = dqx, sy = djy + dqy;
+  f[0] += -4.0 * de + 4.0 * deps;
+  f[1] += ca + tx + dpxx;
+  f[2] += ca + ty - dpxx;
+  f[3] += ca - tx + dpxx;
+  f[4] += ca - ty - dpxx;
+  f[5] += cd + sx + sy + dpxy;
+  f[6] += cd - sx + sy - dpxy;
+  f[7] += cd - sx - sy + dpxy;
+  f[8] += cd + sx - sy - dpxy;
+  g[0] += -4.0 * e3;
+  g[1] += e1 + e3 + e4;
+  g[2] += e2 + e3 - e4;
+  g[3] += -e1 + e3 + e4;
+  g[4] += -e2 + e3 - e4;
+}
+
+// macroscopic fields from POST-collision populations: rho and T are collision
+// invariants and sum e f+ = sum e f + F, so u = (j+ - F/2)/rho.
+ISLBM_HD void fields_from_post(const double (&f)[9], const double (&g)[5], const NodeParams &p,
+                               double &rho, double &u, double &v, double &w, double &T) {
+  T = g[0] + g[1] + g[2] + g[3] + g[4];
+  rho = f[0] + ((f[1] + f[3]) + (f[2] + f[4])) + ((f[5] + f[7]) + (f[6] + f[8]));
+  const double Fy = rho * p.gbeta * T;
+  const double jx = (f[1] - f[3]) + ((f[5] - f[7]) + (f[8] - f[6]));
+  const double jy = (f[2] - f[4]) + ((f[5] - f[7]) + (f[6] - f[8]));
+  u = jx / rho;
+  v = (jy - 0.5 * Fy) / rho;
+  w = 0.0;
+}
+
+// ---------------------------------------------------------------------------
+// D3Q19 + D3Q7
+// ---------------------------------------------------------------------------
+ISLBM_HD void collide_node(double (&f)[19], double (&g)[7], const NodeParams &p) {
+  const double T = g[0] + ((g[1] + g[2]) + (g[3] + g[4]) + (g[5] + g[6]));
+  // pair sums / differences
+  const double px = f[1] + f[2], py = f[3] + f[4], pz = f[5] + f[6];
+  const double ax = f[1] - f[2], ay = f[3] - f[4], az = f[5] - f[6];
+  // xy diagonals 7(+,+) 8(-,+) 9(+,-) 10(-,-)
+  const double xy_s = (f[7] + f[10]) + (f[8] + f[9]);
+  const double xy_x = (f[7] - f[10]) + (f[9] - f[8]);    // sum cx
+  const double xy_y = (f[7] - f[10]) + (f[8] - f[9]);    // sum cy
+  const double xy_p = (f[7] + f[10]) - (f[8] + f[9]);    // sum cx*cy
+  // xz diagonals 11(+,+) 12(-,+) 13(+,-) 14(-,-)   (signs: x, z)
+  const double xz_s = (f[11] + f[14]) + (f[12] + f[13]);
+  const double xz_x = (f[11] - f[14]) + (f[13] - f[12]);
+  const double xz_z = (f[11] - f[14]) + (f[12] - f[13]);
+  const double xz_p = (f[11] + f[14]) - (f[12] + f[13]);
+  // yz diagonals 15(+,+) 16(-,+) 17(+,-) 18(-,-)   (signs: y, z)
+  const double yz_s = (f[15] + f[18]) + (f[16] + f[17]);
+  const double yz_y = (f[15] - f[18]) + (f[17] - f[16]);
+  const double yz_z = (f[15] - f[18]) + (f[16] - f[17]);
+  const double yz_p = (f[15] + f[18]) - (f[16] + f[17]);
+
+  const double sa = px + py + pz;
+  const double sd = xy_s + xz_s + yz_s;
+  const double rho = f[0] + sa + sd;
+  const double Fy = rho * p.gbeta * T;
+  const double dxs = xy_x + xz_x, dys = xy_y + yz_y, dzs = xz_z + yz_z;
+  const double jx = ax + dxs, jy = ay + dys, jz = az + dzs;
+  const double inv = 1.0 / rho;
+  const double u = jx * inv, v = (jy + 0.5 * Fy) * inv, w = jz * inv;
+  const double u2 = u * u + v * v + w * w;
+  // moments in the order of Eq. 11
+  const double me = -30.0 * f[0] - 11.0 * sa + 8.0 * sd;
+  const double meps = 12.0 * f[0] - 4.0 * sa + sd;
+  const double mqx = -4.0 * ax + dxs, mqy = -4.0 * ay + dys, mqz = -4.0 * az + dzs;
+  const double a3 = 2.0 * px - py - pz;                 // axis part of 3pxx
+  const double d3 = xy_s + xz_s - 2.0 * yz_s;           // diagonal part of 3pxx
+  const double m3pxx = a3 + d3;
+  const double m3pixx = -2.0 * a3 + d3;
+  const double aw = py - pz, dw = xy_s - xz_s;
+  const double mpww = aw + dw;
+  const double mpiww = -2.0 * aw + dw;
+  const double mmx = xy_x - xz_x, mmy = yz_y - xy_y, mmz = xz_z - yz_z;
+  const double vF = v * Fy;
+  const double q3 = 2.0 * u * u - v * v - w * w, qw = v * v - w * w;
+  // Delta m_k / |row_k|^2
+  const double de = (-p.s_nu * (me - rho * (-11.0 + 19.0 * u2)) + p.hs_nu * (38.0 * vF)) * (1.0 / 2394.0);
+  const double deps = (-p.s_nu * (meps - rho * (3.0 - 5.5 * u2)) - p.hs_nu * (11.0 * vF)) * (1.0 / 252.0);
+  const double djy = Fy * 0.1;
+  const double dqx = (-p.s_q * (mqx + (2.0 / 3.0) * rho * u)) * (1.0 / 40.0);
+  const double dqy = (-p.s_q * (mqy + (2.0 / 3.0) * rho * v) - p.hs_q * ((2.0 / 3.0) * Fy)) * (1.0 / 40.0);
+  const double dqz = (-p.s_q * (mqz + (2.0 / 3.0) * rho * w)) * (1.0 / 40.0);
+  const double d3pxx = (-p.s_nu * (m3pxx - rho * q3) - p.hs_nu * (2.0 * vF)) * (1.0 / 36.0);
+  const double d3pixx = (-p.s_nu * (m3pixx + 0.5 * rho * q3) + p.hs_nu * vF) * (1.0 / 72.0);
+  const double dpww = (-p.s_nu * (mpww - rho * qw) + p.hs_nu * (2.0 * vF)) * (1.0 / 12.0);
+  const double dpiww = (-p.s_nu * (mpiww + 0.5 * rho * qw) - p.hs_nu * vF) * (1.0 / 24.0);
+  const double dpxy = (-p.s_nu * (xy_p - rho * (u * v)) + p.hs_nu * (u * Fy)) * 0.25;
+  const double dpyz = (-p.s_nu * (yz_p - rho * (v * w)) + p.hs_nu * (w * Fy)) * 0.25;
+  const double dpxz = (-p.s_nu * (xz_p - rho * (u * w))) * 0.25;
+  const double dmx = (-p.s_q * mmx) * 0.125, dmy = (-p.s_q * mmy) * 0.125, dmz = (-p.s_q * mmz) * 0.125;
+  // temperature moments (Eq. 16 order)
+  const double gx = g[1] + g[2], gy = g[3] + g[4], gz = g[5] + g[6];
+  const double e1 = (-p.q_k * ((g[1] - g[2]) - u * T)) * 0.5;
+  const double e2 = (-p.q_k * ((g[3] - g[4]) - v * T)) * 0.5;
+  const double e3 = (-p.q_k * ((g[5] - g[6]) - w * T)) * 0.5;
+  const double e4 = (-p.q_e * ((-6.0 * g[0] + (gx + gy + gz)) - p.a_T * T)) * (1.0 / 42.0);
+  const double e5 = (-p.q_e * (2.0 * gx - gy - gz)) * (1.0 / 12.0);
+  const double e6 = (-p.q_e * (gy - gz)) * 0.25;
+  // f+ = f + M^T d
+  const double ca = -11.0 * de - 4.0 * deps;
+  const double cd = 8.0 * de + deps;
+  const double tx = -4.0 * dqx, ty = djy - 4.0 * dqy, tz = -4.0 * dqz;
+  const double sx = dqx, sy = djy + dqy, sz = dqz;
+  const double nax = 2.0 * d3pxx - 4.0 * d3pixx;                         // axis x normal-stress part
+  const double nay = -d3pxx + 2.0 * d3pixx + dpww - 2.0 * dpiww;         // axis y
+  const double naz = -d3pxx + 2.0 * d3pixx - dpww + 2.0 * dpiww;         // axis z
+  const double nxy = d3pxx + d3pixx + dpww + dpiww;                      // xy diagonals
+  const double nxz = d3pxx + d3pixx - dpww - dpiww;                      // xz diagonals
+  const double nyz = -2.0 * (d3pxx + d3pixx);                            // yz diagonals
+  f[0] += -30.0 * de + 12.0 * deps;
+  f[1] += ca + tx + nax;
+  f[2] += ca - tx + nax;
+  f[3] += ca + ty + nay;
+  f[4] += ca - ty + nay;
+  f[5] += ca + tz + naz;
+  f[6] += ca - tz + naz;
+  // xy: + sx*cx + sy*cy + cx*cy*dpxy + cx*dmx - cy*dmy
+  f[7] += cd + nxy + (sx + dmx) + (sy - dmy) + dpxy;
+  f[8] += cd + nxy - (sx + dmx) + (sy - dmy) - dpxy;
+  f[9] += cd + nxy + (sx + dmx) - (sy - dmy) - dpxy;
+  f[10] += cd + nxy - (sx + dmx) - (sy - dmy) + dpxy;
+  // xz: + sx*cx + sz*cz + cx*cz*dpxz - cx*dmx + cz*dmz
+  f[11] += cd + nxz + (sx - dmx) + (sz + dmz) + dpxz;
+  f[12] += cd + nxz - (sx - dmx) + (sz + dmz) - dpxz;
+  f[13] += cd + nxz + (sx - dmx) - (sz + dmz) - dpxz;
+  f[14] += cd + nxz - (sx - dmx) - (sz + dmz) + dpxz;
+  // yz: + sy*cy + sz*cz + cy*cz*dpyz + cy*dmy - cz*dmz
+  f[15] += cd + nyz + (sy + dmy) + (sz - dmz) + dpyz;
+  f[16] += cd + nyz - (sy + dmy) + (sz - dmz) - dpyz;
+  f[17] += cd + nyz + (sy + dmy) - (sz - dmz) - dpyz;
+  f[18] += cd + nyz - (sy + dmy) - (sz - dmz) + dpyz;
+  g[0] += -6.0 * e4;
+  g[1] += e1 + e4 + 2.0 * e5;
+  g[2] += -e1 + e4 + 2.0 * e5;
+  g[3] += e2 + e4 - e5 + e6;
+  g[4] += -e2 + e4 - e5 + e6;
+  g[5] += e3 + e4 - e5 - e6;
+  g[6] += -e3 + e4 - e5 - e6;
+}
+
+ISLBM_HD void fields_from_post(const double (&f)[19], const double (&g)[7], const NodeParams &p,
+                               double &rho, double &u, double &v, double &w, double &T) {
+  T = g[0] + ((g[1] + g[2]) + (g[3] + g[4]) + (g[5] + g[6]));
+  const double sa = (f[1] + f[2]) + (f[3] + f[4]) + (f[5] + f[6]);
+  const double sd = ((f[7] + f[10]) + (f[8] + f[9])) + ((f[11] + f[14]) + (f[12] + f[13])) +
+                    ((f[15] + f[18]) + (f[16] + f[17]));
+  rho = f[0] + sa + sd;
+  const double Fy = rho * p.gbeta * T;
+  const double jx = (f[1] - f[2]) + ((f[7] - f[10]) + (f[9] - f[8])) + ((f[11] - f[14]) + (f[13] - f[12]));
+  const double jy = (f[3] - f[4]) + ((f[7] - f[10]) + (f[8] - f[9])) + ((f[15] - f[18]) + (f[17] - f[16]));
+  const double jz = (f[5] - f[6]) + ((f[11] - f[14]) + (f[12] - f[13])) + ((f[15] - f[18]) + (f[16] - f[17]));
+  u = jx / rho;
+  v = (jy - 0.5 * Fy) / rho;
+  w = jz / rho;
+}
+
+// pre-collision macroscopic fields (used by init checks / diagnostics on f_t)
+template <int QF, int QG>
+ISLBM_HD void rest_equilibrium(double (&f)[QF], double (&g)[QG], double T, double a_T) {
+  constexpr int DIM = QF == 9 ? 2 : 3;
+#pragma unroll
+  for (int q = 0; q < QF; ++q) f[q] = wflow<DIM>(q);
+  // N^-1 n_eq(T, u = 0): rest weight (1 - a_T)/5 | (1 - a_T)/7, moving weight (4 + a_T)/20 | (6 + a_T)/42
+  const double wm = DIM == 2 ? (4.0 + a_T) * (1.0 / 20.0) : (6.0 + a_T) * (1.0 / 42.0);
+  const double w0 = DIM == 2 ? (1.0 - a_T) * 0.2 : (1.0 - a_T) * (1.0 / 7.0);
+  g[0] = w0 * T;
+#pragma unroll
+  for (int q = 1; q < QG; ++q) g[q] = wm * T;
+}
+
+}  // namespace islbmk

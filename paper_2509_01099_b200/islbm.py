@@ -1,0 +1,194 @@
+"""Thin Python binding of the C-ABI in include/islbm.h (argument marshalling only).
+
+PyTorch supplies device memory and the CUDA stream; every step of the path runs
+in the kernels of libislbm.so.  There is no fallback: if the library has not been
+built, importing this module raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libislbm.so")
+
+D2Q9_D2Q5, D3Q19_D3Q7 = 0, 1
+F64, F32_STORAGE = 0, 1
+KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED, KERNEL_UNIFORM_SHIFT = 0, 1, 2, 3
+
+EXPORTS = (
+    "islbm_workspace_bytes", "islbm_create", "islbm_destroy", "islbm_get_params", "islbm_init",
+    "islbm_set_populations", "islbm_get_populations", "islbm_step", "islbm_fields", "islbm_nusselt",
+    "islbm_steady_residual", "islbm_set_buoyancy_scale", "islbm_set_kernel", "islbm_launch_count",
+    "islbm_kernel_name", "islbm_last_error", "islbm_version",
+)
+
+
+class _Mesh(C.Structure):
+    _fields_ = [("dim", C.c_int), ("n", C.c_int * 3), ("x", C.POINTER(C.c_double) * 3), ("delta", C.c_double)]
+
+
+class _Params(C.Structure):
+    _fields_ = [(k, C.c_double) for k in ("U", "H_lu", "nu", "alpha", "gbeta", "tau_f", "a_T", "omega_bc", "dt_star")] + [
+        ("L_eff", C.c_double * 3)]
+
+
+class IslbmError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"islbm error {code}: {msg}")
+        self.code = code
+
+
+def _load():
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: run `python -c 'import __graft_entry__ as g; g.build()'` "
+                          "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    vp, dp = C.c_void_p, C.POINTER(C.c_double)
+    lib.islbm_workspace_bytes.argtypes = [C.POINTER(_Mesh), C.c_int, C.c_int, C.POINTER(C.c_size_t)]
+    lib.islbm_create.argtypes = [C.POINTER(vp), C.POINTER(_Mesh), C.c_int, C.c_double, C.c_double, C.c_double,
+                                 C.c_int, vp, C.c_size_t, vp]
+    lib.islbm_destroy.argtypes = [vp]
+    lib.islbm_destroy.restype = None
+    lib.islbm_get_params.argtypes = [vp, C.POINTER(_Params)]
+    lib.islbm_init.argtypes = [vp, C.c_ulonglong, C.c_double]
+    lib.islbm_set_populations.argtypes = [vp, vp, vp]
+    lib.islbm_get_populations.argtypes = [vp, vp, vp]
+    lib.islbm_step.argtypes = [vp, C.c_int]
+    lib.islbm_fields.argtypes = [vp, vp, vp, vp, vp, vp]
+    lib.islbm_nusselt.argtypes = [vp, dp]
+    lib.islbm_steady_residual.argtypes = [vp, dp]
+    lib.islbm_set_buoyancy_scale.argtypes = [vp, C.c_double]
+    lib.islbm_set_kernel.argtypes = [vp, C.c_int]
+    lib.islbm_launch_count.argtypes = [vp]
+    lib.islbm_launch_count.restype = C.c_longlong
+    lib.islbm_kernel_name.argtypes = [vp]
+    lib.islbm_kernel_name.restype = C.c_char_p
+    lib.islbm_last_error.restype = C.c_char_p
+    lib.islbm_version.restype = C.c_char_p
+    return lib
+
+
+lib = _load()
+
+
+def _check(rc):
+    if rc != 0:
+        raise IslbmError(rc, lib.islbm_last_error().decode())
+
+
+def _mesh_struct(coords, delta):
+    dim = len(coords)
+    arrs = [np.ascontiguousarray(c, dtype=np.float64) for c in coords]
+    m = _Mesh()
+    m.dim = dim
+    for a in range(3):
+        m.n[a] = len(arrs[a]) if a < dim else 1
+        m.x[a] = arrs[a].ctypes.data_as(C.POINTER(C.c_double)) if a < dim else None
+    m.delta = float(delta)
+    return m, arrs   # keep arrs alive while m is used
+
+
+def workspace_bytes(coords, delta, precision=F64):
+    m, _keep = _mesh_struct(coords, delta)
+    out = C.c_size_t(0)
+    _check(lib.islbm_workspace_bytes(C.byref(m), D2Q9_D2Q5 if m.dim == 2 else D3Q19_D3Q7, precision, C.byref(out)))
+    return out.value
+
+
+def _dev_ptr(t, n_expected=None):
+    if t is None:
+        return None
+    assert t.is_cuda and t.dtype == torch.float64 and t.is_contiguous()
+    if n_expected is not None:
+        assert t.numel() == n_expected, (t.shape, n_expected)
+    return C.c_void_p(t.data_ptr())
+
+
+class Islbm:
+    """islbm_create / islbm_step / islbm_fields / islbm_nusselt on one CUDA device."""
+
+    def __init__(self, coords, delta, Ra, Pr, Ma, precision=F64, device="cuda", stream=None):
+        self.dim = len(coords)
+        self.precision = precision
+        self.device = torch.device(device)
+        m, keep = _mesh_struct(coords, delta)
+        self.n = tuple(m.n)
+        self.shape = (self.n[2], self.n[1], self.n[0])
+        self.nodes = self.n[0] * self.n[1] * self.n[2]
+        self.qf, self.qg = (9, 5) if self.dim == 2 else (19, 7)
+        lattice = D2Q9_D2Q5 if self.dim == 2 else D3Q19_D3Q7
+        nbytes = C.c_size_t(0)
+        _check(lib.islbm_workspace_bytes(C.byref(m), lattice, precision, C.byref(nbytes)))
+        self.workspace = torch.empty(nbytes.value, dtype=torch.uint8, device=self.device)   # owned here
+        self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
+        self.h = C.c_void_p()
+        _check(lib.islbm_create(C.byref(self.h), C.byref(m), lattice, float(Ra), float(Pr), float(Ma), precision,
+                                C.c_void_p(self.workspace.data_ptr()), nbytes.value, C.c_void_p(self.stream.cuda_stream)))
+        del keep
+
+    def close(self):
+        if getattr(self, "h", None):
+            lib.islbm_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def params(self):
+        p = _Params()
+        _check(lib.islbm_get_params(self.h, C.byref(p)))
+        d = {k: getattr(p, k) for k, _ in _Params._fields_ if k != "L_eff"}
+        d.update(L_eff_x=p.L_eff[0], L_eff_y=p.L_eff[1], L_eff_z=p.L_eff[2])
+        return d
+
+    def set_buoyancy_scale(self, s):
+        _check(lib.islbm_set_buoyancy_scale(self.h, float(s)))
+
+    def set_kernel(self, which):
+        _check(lib.islbm_set_kernel(self.h, int(which)))
+
+    @property
+    def kernel_name(self):
+        return lib.islbm_kernel_name(self.h).decode()
+
+    @property
+    def launch_count(self):
+        return int(lib.islbm_launch_count(self.h))
+
+    def init(self, seed=0, noise_amp=1e-3):
+        _check(lib.islbm_init(self.h, int(seed), float(noise_amp)))
+
+    def set_populations(self, f, g):
+        _check(lib.islbm_set_populations(self.h, _dev_ptr(f, self.qf * self.nodes), _dev_ptr(g, self.qg * self.nodes)))
+
+    def get_populations(self):
+        f = torch.empty((self.qf,) + self.shape, dtype=torch.float64, device=self.device)
+        g = torch.empty((self.qg,) + self.shape, dtype=torch.float64, device=self.device)
+        _check(lib.islbm_get_populations(self.h, _dev_ptr(f), _dev_ptr(g)))
+        return f, g
+
+    def step(self, n=1):
+        _check(lib.islbm_step(self.h, int(n)))
+
+    def fields(self, names=("rho", "u", "v", "w", "T")):
+        out = {k: torch.empty(self.shape, dtype=torch.float64, device=self.device)
+               for k in names if not (k == "w" and self.dim == 2)}
+        _check(lib.islbm_fields(self.h, *[_dev_ptr(out.get(k)) for k in ("rho", "u", "v", "w", "T")]))
+        return out
+
+    def nusselt(self):
+        out = (C.c_double * 5)()
+        _check(lib.islbm_nusselt(self.h, out))
+        return dict(zip(("Nu_hot", "Nu_cold", "Re", "u2", "Nu_vol"), list(out)))
+
+    def steady_residual(self):
+        out = (C.c_double * 2)()
+        _check(lib.islbm_steady_residual(self.h, out))
+        return out[0], out[1]

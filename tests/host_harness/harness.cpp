@@ -1,0 +1,52 @@
+// Test-only host build of the node-local device functions (csrc/islbm_lattice.cuh)
+// so that the hand-factored collisions can be compared with the oracle on a box
+// without a GPU.  Not linked into the product library.
+#include "../../paper_2509_01099_b200/csrc/islbm_lattice.cuh"
+
+extern "C" void harness_collide(int dim, double *f, double *g, const double *prm) {
+  islbmk::NodeParams p;
+  p.gbeta = prm[0]; p.s_nu = prm[1]; p.s_q = prm[2];
+  p.hs_nu = 1.0 - 0.5 * p.s_nu; p.hs_q = 1.0 - 0.5 * p.s_q;
+  p.q_k = prm[3]; p.q_e = prm[4]; p.a_T = prm[5];
+  if (dim == 2) {
+    double ff[9], gg[5];
+    for (int i = 0; i < 9; ++i) ff[i] = f[i];
+    for (int i = 0; i < 5; ++i) gg[i] = g[i];
+    islbmk::collide_node(ff, gg, p);
+    for (int i = 0; i < 9; ++i) f[i] = ff[i];
+    for (int i = 0; i < 5; ++i) g[i] = gg[i];
+  } else {
+    double ff[19], gg[7];
+    for (int i = 0; i < 19; ++i) ff[i] = f[i];
+    for (int i = 0; i < 7; ++i) gg[i] = g[i];
+    islbmk::collide_node(ff, gg, p);
+    for (int i = 0; i < 19; ++i) f[i] = ff[i];
+    for (int i = 0; i < 7; ++i) g[i] = gg[i];
+  }
+}
+
+// out: rho,u,v,w,T from post-collision populations
+extern "C" void harness_fields_post(int dim, const double *f, const double *g, const double *prm, double *out) {
+  islbmk::NodeParams p{};
+  p.gbeta = prm[0];
+  if (dim == 2) {
+    double ff[9], gg[5];
+    for (int i = 0; i < 9; ++i) ff[i] = f[i];
+    for (int i = 0; i < 5; ++i) gg[i] = g[i];
+    islbmk::fields_from_post(ff, gg, p, out[0], out[1], out[2], out[3], out[4]);
+  } else {
+    double ff[19], gg[7];
+    for (int i = 0; i < 19; ++i) ff[i] = f[i];
+    for (int i = 0; i < 7; ++i) gg[i] = g[i];
+    islbmk::fields_from_post(ff, gg, p, out[0], out[1], out[2], out[3], out[4]);
+  }
+}
+
+extern "C" void harness_tables(int dim, int *e, int *opp, double *w) {
+  int qf = dim == 2 ? 9 : 19;
+  for (int q = 0; q < qf; ++q) {
+    for (int a = 0; a < 3; ++a) e[3 * q + a] = dim == 2 ? islbmk::evel<2>(q, a) : islbmk::evel<3>(q, a);
+    opp[q] = dim == 2 ? islbmk::opposite<2>(q) : islbmk::opposite<3>(q);
+    w[q] = dim == 2 ? islbmk::wflow<2>(q) : islbmk::wflow<3>(q);
+  }
+}

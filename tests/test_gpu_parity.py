@@ -1,0 +1,314 @@
+"""Parity of the CUDA path (through the C-ABI binding) with the CPU oracle.
+
+Tolerances (BASELINE.json north_star): fp64 populations after 1 step: max abs
+difference per population plane / max abs oracle value of that plane <= 1e-12;
+u, v, w (normalised by max |u|) and T (normalised by Delta_T = 1) after 1000
+steps <= 1e-9; fp32-storage path: u and T after 1000 steps <= 1e-5.
+"""
+import math
+import os
+import zlib
+
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from oracle.oracle import Oracle  # noqa: E402
+from paper_2509_01099_b200 import inputs  # noqa: E402
+
+NTHREADS = max(1, min(32, len(os.sched_getaffinity(0))))
+SQ3 = math.sqrt(3.0)
+
+
+@pytest.fixture(scope="module")
+def islbm():
+    import __graft_entry__ as graft
+    graft.build()
+    from paper_2509_01099_b200 import islbm as mod
+    assert torch.cuda.is_available()
+    return mod
+
+
+def pair(islbm, coords, delta, Ra, Pr=0.71, Ma=0.1 * SQ3, precision=0, kernel=0, threads=NTHREADS):
+    sim = islbm.Islbm(coords, delta, Ra, Pr, Ma, precision=precision)
+    if kernel:
+        sim.set_kernel(kernel)
+    orc = Oracle(coords, delta, Ra, Pr, Ma, threads=threads)
+    return sim, orc
+
+
+def plane_err(a, b):
+    """max over planes of max|a-b| / max|b| (reading A17)."""
+    a = a.reshape(a.shape[0], -1)
+    b = b.reshape(b.shape[0], -1)
+    return float((np.abs(a - b).max(1) / np.abs(b).max(1)).max())
+
+
+def ragged_coords(dim, ns, stretches):
+    out = []
+    for n, s in zip(ns[:dim], stretches[:dim]):
+        out.append(inputs.tanh_mesh(n, s)[0])
+    delta = min(float(np.diff(c).min()) for c in out)
+    return out, delta
+
+
+def kernels_for(islbm, sim):
+    ks = [islbm.KERNEL_GENERIC]
+    try:
+        sim.set_kernel(islbm.KERNEL_TILED)
+        ks.append(islbm.KERNEL_TILED)
+    except islbm.IslbmError:
+        pass
+    sim.set_kernel(islbm.KERNEL_AUTO)
+    return ks
+
+
+# ---------------------------------------------------------------------------
+# one step from a far-from-equilibrium random state: every population
+# ---------------------------------------------------------------------------
+CASES_1STEP = [
+    ("2d_64sq_c1", 2, (64, 64, 1), (1.2, 1.2, 0)),
+    ("2d_ragged_70x45", 2, (70, 45, 1), (1.6, 1.1, 0)),
+    ("2d_ragged_131x67", 2, (131, 67, 1), (1.3, 1.9, 0)),
+    ("2d_min_3x3", 2, (3, 3, 1), (0.5, 0.5, 0)),
+    ("2d_thin_3x40", 2, (3, 40, 1), (0.5, 1.5, 0)),
+    ("3d_ragged_37x21x19", 3, (37, 21, 19), (1.5, 1.2, 1.7)),
+    ("3d_ragged_66x10x35", 3, (66, 10, 35), (1.1, 1.4, 1.3)),
+    ("3d_min_3x3x3", 3, (3, 3, 3), (0.5, 0.5, 0.5)),
+    ("3d_thin_5x3x33", 3, (5, 3, 33), (0.7, 0.5, 1.5)),
+]
+
+
+@pytest.mark.parametrize("name,dim,ns,st", CASES_1STEP, ids=[c[0] for c in CASES_1STEP])
+def test_one_step_all_populations(islbm, name, dim, ns, st):
+    coords, delta = ragged_coords(dim, ns, st)
+    sim, orc = pair(islbm, coords, delta, Ra=2e4)
+    f0, g0 = inputs.random_state(orc.shape, orc.qf, orc.qg, seed=zlib.crc32(name.encode()) % 1000, amp=0.05)
+    orc.set_populations(f0, g0)
+    orc.step(1)
+    fo, go = orc.get_populations()
+    for k in kernels_for(islbm, sim):
+        sim.set_kernel(k)
+        sim.set_populations(torch.from_numpy(f0).cuda(), torch.from_numpy(g0).cuda())
+        f_back, g_back = sim.get_populations()            # before any step: the input itself
+        assert np.array_equal(f_back.cpu().numpy(), f0) and np.array_equal(g_back.cpu().numpy(), g0)
+        sim.step(1)
+        f1, g1 = sim.get_populations()
+        ef, eg = plane_err(f1.cpu().numpy(), fo), plane_err(g1.cpu().numpy(), go)
+        assert ef <= 1e-12 and eg <= 1e-12, (name, sim.kernel_name, ef, eg)
+    # second and third step (ping-pong both ways)
+    sim.step(2)
+    orc.step(2)
+    f3, g3 = sim.get_populations()
+    fo, go = orc.get_populations()
+    assert plane_err(f3.cpu().numpy(), fo) <= 3e-12 and plane_err(g3.cpu().numpy(), go) <= 3e-12
+
+
+def test_uniform_mesh_one_step(islbm):
+    for dim, n in ((2, 32), (3, 16)):
+        w = inputs.custom_workload("u", dim, n, mesh="uniform", Ra=1e4)
+        sim, orc = pair(islbm, w.coords, w.delta, w.Ra)
+        f0, g0 = inputs.random_state(orc.shape, orc.qf, orc.qg, seed=dim, amp=0.05)
+        orc.set_populations(f0, g0)
+        orc.step(1)
+        fo, go = orc.get_populations()
+        for k in kernels_for(islbm, sim):
+            sim.set_kernel(k)
+            sim.set_populations(torch.from_numpy(f0).cuda(), torch.from_numpy(g0).cuda())
+            sim.step(1)
+            f1, g1 = sim.get_populations()
+            assert plane_err(f1.cpu().numpy(), fo) <= 1e-12 and plane_err(g1.cpu().numpy(), go) <= 1e-12
+        # mass is conserved to round-off on the uniform mesh (pin P4 on the GPU path)
+        sim.step(200)
+        rho = sim.fields(("rho",))["rho"]
+        assert abs(rho.sum().item() - f0.sum()) / f0.sum() < 1e-13
+
+
+# ---------------------------------------------------------------------------
+# BASELINE.json config 1: 1000 steps, populations and fields
+# ---------------------------------------------------------------------------
+def field_err(sim, orc):
+    fs, fo = sim.fields(), orc.fields()
+    umax = max(np.abs(fo[k]).max() for k in ("u", "v", "w"))
+    out = {k: float(np.abs(fs[k].cpu().numpy() - fo[k]).max() / umax) for k in fs if k in ("u", "v", "w")}
+    out["T"] = float(np.abs(fs["T"].cpu().numpy() - fo["T"]).max())      # Delta_T = 1
+    out["rho"] = float(np.abs(fs["rho"].cpu().numpy() - fo["rho"]).max())
+    return out
+
+
+def test_config1_init_and_1000_steps(islbm):
+    w = inputs.workload("c1_64sq")
+    sim, orc = pair(islbm, w.coords, w.delta, w.Ra, w.Pr, w.Ma)
+    ps, po = sim.params(), orc.params()
+    for k in po:
+        assert ps[k] == pytest.approx(po[k], rel=1e-14), k
+    sim.init(w.seed, w.noise_amp)
+    orc.init(w.seed, w.noise_amp)
+    f, g = sim.get_populations()
+    fo, go = orc.get_populations()
+    assert np.abs(f.cpu().numpy() - fo).max() < 1e-16 and np.abs(g.cpu().numpy() - go).max() < 1e-18
+    sim.step(1)
+    orc.step(1)
+    f, g = sim.get_populations()
+    fo, go = orc.get_populations()
+    assert plane_err(f.cpu().numpy(), fo) <= 1e-12 and plane_err(g.cpu().numpy(), go) <= 1e-12
+    sim.step(999)
+    orc.step(999)
+    err = field_err(sim, orc)
+    assert max(err.values()) <= 1e-9, err
+    f, g = sim.get_populations()
+    fo, go = orc.get_populations()
+    assert plane_err(f.cpu().numpy(), fo) <= 1e-9 and plane_err(g.cpu().numpy(), go) <= 1e-9
+    ns, no = sim.nusselt(), orc.nusselt()
+    for k in no:
+        assert ns[k] == pytest.approx(no[k], rel=1e-9, abs=1e-12), k
+
+
+def test_config1_fp32_storage_1000_steps(islbm):
+    w = inputs.workload("c1_64sq")
+    sim, orc = pair(islbm, w.coords, w.delta, w.Ra, w.Pr, w.Ma, precision=1)
+    sim.init(w.seed, w.noise_amp)
+    orc.init(w.seed, w.noise_amp)
+    sim.step(1000)
+    orc.step(1000)
+    err = field_err(sim, orc)
+    assert err["u"] <= 1e-5 and err["v"] <= 1e-5 and err["T"] <= 1e-5, err
+
+
+def test_3d_small_200_steps_fields_and_nusselt(islbm):
+    w = inputs.custom_workload("c4_small", 3, 32, stretch=1.5, Ra=1e5)
+    sim, orc = pair(islbm, w.coords, w.delta, w.Ra, w.Pr, w.Ma)
+    sim.init(0, 1e-3)
+    orc.init(0, 1e-3)
+    sim.step(200)
+    orc.step(200)
+    err = field_err(sim, orc)
+    assert max(err.values()) <= 1e-9, err
+    ns, no = sim.nusselt(), orc.nusselt()
+    for k in no:
+        assert ns[k] == pytest.approx(no[k], rel=1e-9, abs=1e-12), k
+    # fp32 storage, 3-D
+    sim32 = islbm.Islbm(w.coords, w.delta, w.Ra, w.Pr, w.Ma, precision=1)
+    sim32.init(0, 1e-3)
+    sim32.step(200)
+    e32 = field_err(sim32, orc)
+    assert e32["u"] <= 1e-5 and e32["v"] <= 1e-5 and e32["w"] <= 1e-5 and e32["T"] <= 1e-5, e32
+
+
+# ---------------------------------------------------------------------------
+# BASELINE.json configs 2-5 at full size, in the launch configuration bench.py times
+# ---------------------------------------------------------------------------
+@pytest.mark.parametrize("name,steps", [("c2_512sq", 20), ("c3_1024sq", 5), ("c4_128cu", 3),
+                                        ("c2_512sq_uniform", 5)])
+def test_full_size_configs_few_steps(islbm, name, steps):
+    w = inputs.workload(name)
+    sim, orc = pair(islbm, w.coords, w.delta, w.Ra, w.Pr, w.Ma)
+    sim.init(w.seed, w.noise_amp)
+    orc.init(w.seed, w.noise_amp)
+    sim.step(1)
+    orc.step(1)
+    f, g = sim.get_populations()
+    fo, go = orc.get_populations()
+    assert plane_err(f.cpu().numpy(), fo) <= 1e-12 and plane_err(g.cpu().numpy(), go) <= 1e-12
+    del f, g
+    sim.step(steps - 1)
+    orc.step(steps - 1)
+    err = field_err(sim, orc)
+    assert max(err.values()) <= 1e-10, err
+    ns, no = sim.nusselt(), orc.nusselt()
+    assert ns["Nu_hot"] == pytest.approx(no["Nu_hot"], rel=1e-10)
+
+
+def test_config5_256cu_sampled_nodes(islbm):
+    """256^3: the oracle computes sampled nodes one by one (oracle_step_node) from the
+    seeded initial state; walls, edges, corners and tile seams are all in the sample."""
+    w = inputs.workload("c5_256cu")
+    sim = islbm.Islbm(w.coords, w.delta, w.Ra, w.Pr, w.Ma)
+    orc = Oracle(w.coords, w.delta, w.Ra, w.Pr, w.Ma)
+    sim.init(w.seed, w.noise_amp)
+    orc.init(w.seed, w.noise_amp)
+    sim.step(1)
+    f, g = sim.get_populations()
+    n = 256
+    special = [0, 1, 2, 7, 8, 15, 16, 31, 32, 33, 63, 64, 127, 128, 191, 192, 253, 254, 255]
+    rng = np.random.default_rng(5)
+    pts = [(a, b, c) for a in (0, 1, 128, 254, 255) for b in (0, 31, 32, 255) for c in (0, 8, 255)]
+    pts += [tuple(rng.choice(special, 3)) for _ in range(300)]
+    pts += [tuple(rng.integers(0, n, 3)) for _ in range(700)]
+    idx = torch.tensor(pts, device="cuda")
+    fs = f[:, idx[:, 2], idx[:, 1], idx[:, 0]].cpu().numpy()
+    gs = g[:, idx[:, 2], idx[:, 1], idx[:, 0]].cpu().numpy()
+    fo = np.empty_like(fs)
+    go = np.empty_like(gs)
+    for k, (ix, iy, iz) in enumerate(pts):
+        fo[:, k], go[:, k] = orc.step_node(int(ix), int(iy), int(iz))
+    assert plane_err(fs, fo) <= 1e-12 and plane_err(gs, go) <= 1e-12
+    # properties that hold at any size: rho ~ 1, T within the noise amplitude, everything finite
+    fl = sim.fields(("rho", "T"))
+    assert torch.isfinite(fl["rho"]).all() and (fl["rho"] - 1).abs().max().item() < 1e-6
+    assert fl["T"].abs().max().item() < 0.2     # one anti-bounce-back kick of omega*T_w at the x-walls
+
+
+# ---------------------------------------------------------------------------
+# method-level properties on the GPU path
+# ---------------------------------------------------------------------------
+def test_conduction_fixed_point_on_gpu(islbm):
+    """Pin P5 on the CUDA path: buoyancy off, linear-T state, stretched mesh."""
+    w = inputs.custom_workload("p5", 2, 48, stretch=1.6, Ra=1e5)
+    sim, orc = pair(islbm, w.coords, w.delta, w.Ra)
+    sim.set_buoyancy_scale(0.0)
+    p = orc.params()
+    qk = 3.0 - SQ3
+    x = w.coords[0]
+    G = -1.0 / p["H_lu"]
+    T = 0.5 + G * (x - (x[0] - w.delta / 2)) / w.delta
+    wr = np.full(5, p["omega_bc"] / 2)
+    wr[0] = 1 - wr[1:].sum()
+    ex = np.array([0, 1, 0, -1, 0])
+    f0 = np.empty((9,) + orc.shape)
+    f0[:] = np.array([4 / 9] + [1 / 9] * 4 + [1 / 36] * 4)[:, None, None, None]
+    g0 = np.empty((5,) + orc.shape)
+    for i in range(5):
+        g0[i] = (wr[i] * T - wr[i] / qk * ex[i] * G)[None, None, :]
+    sim.set_populations(torch.from_numpy(f0).cuda(), torch.from_numpy(g0).cuda())
+    sim.step(1000)
+    f1, g1 = sim.get_populations()
+    assert np.abs(f1.cpu().numpy() - f0).max() < 1e-13 and np.abs(g1.cpu().numpy() - g0).max() < 1e-13
+    nu = sim.nusselt()
+    assert nu["Nu_hot"] == pytest.approx(1.0, abs=1e-10) and nu["Nu_cold"] == pytest.approx(1.0, abs=1e-10)
+
+
+def test_state_errors_and_launch_accounting(islbm):
+    w = inputs.custom_workload("s", 2, 16)
+    sim = islbm.Islbm(w.coords, w.delta, w.Ra, w.Pr, w.Ma)
+    with pytest.raises(islbm.IslbmError) as e:
+        sim.step(1)
+    assert e.value.code == -6
+    sim.init(0, 1e-3)
+    n0 = sim.launch_count
+    sim.step(10)
+    assert sim.launch_count - n0 >= 10
+    with pytest.raises(islbm.IslbmError):
+        sim.set_buoyancy_scale(0.5)
+    r0 = sim.steady_residual()
+    sim.step(10)
+    r1 = sim.steady_residual()
+    assert r0 == (1.0, 1.0) and 0 < r1[1] < 10 and r1[0] >= 0
+
+
+def test_steady_residual_matches_definition(islbm):
+    """Eq. 30 on the device vs the same sums formed from islbm_fields outputs."""
+    w = inputs.custom_workload("r", 2, 40, stretch=1.4, Ra=1e5)
+    sim = islbm.Islbm(w.coords, w.delta, w.Ra, w.Pr, w.Ma)
+    sim.init(0, 1e-3)
+    sim.step(300)
+    a = sim.fields()
+    sim.steady_residual()
+    sim.step(50)
+    b = sim.fields()
+    ru, rT = sim.steady_residual()
+    du = torch.sqrt((b["u"] - a["u"]) ** 2 + (b["v"] - a["v"]) ** 2).sum() / torch.sqrt(a["u"] ** 2 + a["v"] ** 2).sum()
+    dT = (b["T"] - a["T"]).abs().sum() / a["T"].abs().sum()
+    assert ru == pytest.approx(du.item(), rel=1e-10) and rT == pytest.approx(dT.item(), rel=1e-10)
