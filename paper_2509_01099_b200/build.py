@@ -10,7 +10,7 @@ LIB = os.path.join(HERE, "libislbm.so")
 SOURCES = ["islbm_api.cu"]
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-    "--compiler-options", "-fPIC", "-shared", "-lcuda",
+    "--compiler-options", "-fPIC", "-shared",
 ]
 
 

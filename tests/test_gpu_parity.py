@@ -76,6 +76,10 @@ CASES_1STEP = [
     ("2d_thin_3x40", 2, (3, 40, 1), (0.5, 1.5, 0)),
     ("3d_ragged_37x21x19", 3, (37, 21, 19), (1.5, 1.2, 1.7)),
     ("3d_ragged_66x10x35", 3, (66, 10, 35), (1.1, 1.4, 1.3)),
+    ("3d_tiled_64x24x40", 3, (64, 24, 40), (1.3, 1.2, 1.5)),
+    ("3d_tiled_34x18x7", 3, (34, 18, 7), (1.2, 1.1, 0.9)),
+    ("3d_tiled_96x50x33", 3, (96, 50, 33), (1.6, 1.4, 1.2)),
+    ("3d_tiled_4x4x3", 3, (4, 4, 3), (0.5, 0.5, 0.5)),
     ("3d_min_3x3x3", 3, (3, 3, 3), (0.5, 0.5, 0.5)),
     ("3d_thin_5x3x33", 3, (5, 3, 33), (0.7, 0.5, 1.5)),
 ]
