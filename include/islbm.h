@@ -147,9 +147,17 @@ int islbm_steady_residual(islbm_t *h, double out[2]);
 /* Test / study hooks (not part of the four-call contract). */
 int islbm_set_buoyancy_scale(islbm_t *h, double s); /* multiplies g*beta; 0 for pin P5 */
 /* 0 = auto (fastest kernel for this mesh), 1 = generic global-memory kernel,
- * 2 = shared-memory tiled kernel, 3 = uniform-mesh pure-shift kernel (only
- * valid when every spacing equals delta). */
+ * 2 = TMA-staged shared-memory kernel (y-marching in 2-D, z-marching in 3-D),
+ * 3 = uniform-mesh pure-shift kernel (only valid when every spacing equals
+ * delta bit-exactly; Eq. 17-20 on the uniform mesh of Eq. 24-25). */
 int islbm_set_kernel(islbm_t *h, int which);
+/* Run-time knobs of the TMA-staged kernels.  key: "chunk" (marching
+ * chunk length, 0 = automatic), "l2promo" (tensor-map L2 promotion 0 none, 1 64 B,
+ * 2 128 B, 3 256 B), "load_policy" / "store_policy" (L2 eviction policy 0 normal,
+ * 1 evict_first, 2 evict_last), "tx2d" (2-D strip width 0 auto, 128, 224),
+ * "serpentine" (2-D: reverse the CTA order on odd steps).  Results do not depend on
+ * any of them.  Unknown key or negative value: ISLBM_ERR_ARG. */
+int islbm_set_tuning(islbm_t *h, const char *key, int value);
 /* Number of kernels launched by this handle since creation. */
 long long islbm_launch_count(const islbm_t *h);
 /* Name of the step kernel variant that islbm_step currently dispatches to. */

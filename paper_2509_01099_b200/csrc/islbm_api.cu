@@ -12,7 +12,9 @@
 #include "../../include/islbm.h"
 #include "islbm_kernels.cuh"
 #include "islbm_reduce.cuh"
-#include "islbm_tiled.cuh"
+#include "islbm_tiled2.cuh"
+#include "islbm_tiled3.cuh"
+#include "islbm_uniform.cuh"
 
 using namespace islbmk;
 
@@ -98,8 +100,24 @@ struct islbm {
   bool snap_valid;
   int kernel_choice;       // 0 auto, 1 generic, 2 tiled, 3 uniform shift
   long long launches;
-  TiledPlan tiled;
+  Tuning tune;
+  Plan2 plan2;
+  Plan3 plan3;
+  bool tiled_ok() const { return dim == 2 ? plan2.available : plan3.available; }
+  const char *tiled_why_not() const { return dim == 2 ? plan2.why_not : plan3.why_not; }
 };
+
+// (re)build the TMA plan of the tiled kernel for the current tuning
+static void make_tiled_plan(islbm *h) {
+  void *b0 = h->ws + h->cv.buf[0], *b1 = h->ws + h->cv.buf[1];
+  if (h->dim == 2) {
+    if (h->precision == ISLBM_F64) plan2_create<double>(h->plan2, h->n, b0, b1, h->tune);
+    else plan2_create<float>(h->plan2, h->n, b0, b1, h->tune);
+  } else {
+    if (h->precision == ISLBM_F64) plan3_create<double>(h->plan3, h->n, b0, b1, h->tune);
+    else plan3_create<float>(h->plan3, h->n, b0, b1, h->tune);
+  }
+}
 
 extern "C" const char *islbm_last_error(void) { return g_err.c_str(); }
 extern "C" const char *islbm_version(void) { return "islbm-b200 0.1 (sm_100a)"; }
@@ -260,8 +278,7 @@ extern "C" int islbm_create(islbm_t **out, const islbm_mesh *mesh, int lattice, 
   h->snap_valid = false;
   h->kernel_choice = 0;
   h->launches = 0;
-  rc = tiled_plan_create(h->tiled, h->dim, h->n, h->precision, h->ws + h->cv.buf[0], h->ws + h->cv.buf[1], g_err);
-  if (rc) { delete h; return rc; }
+  make_tiled_plan(h);
   *out = h;
   return ISLBM_OK;
 }
@@ -353,15 +370,25 @@ static void launch_generic_step(islbm *h, bool collide, double *fout, double *go
   h->launches++;
 }
 
+template <int DIM, typename ST>
+static void launch_shift_step(islbm *h) {
+  dim3 grid, block;
+  generic_geometry(h, grid, block);
+  const ST *src = (const ST *)(h->ws + h->cv.buf[h->cur]);
+  ST *dst = (ST *)(h->ws + h->cv.buf[1 - h->cur]);
+  k_step_shift<DIM, ST><<<grid, block, 0, h->stream>>>(h->dm, h->np, src, dst);
+  h->launches++;
+}
+
 static int effective_kernel(const islbm *h) {
   if (h->kernel_choice != 0) return h->kernel_choice;
-  return h->tiled.available ? 2 : 1;
+  return h->tiled_ok() ? 2 : 1;
 }
 
 extern "C" const char *islbm_kernel_name(const islbm_t *h) {
   if (!h) return "";
   switch (effective_kernel(h)) {
-    case 2: return h->tiled.name;
+    case 2: return h->dim == 2 ? (h->plan2.tx == 224 ? "tiled_ymarch_tma_tx224" : "tiled_ymarch_tma_tx128") : "tiled_zmarch_tma";
     case 3: return "uniform_shift";
     default: return "generic_global";
   }
@@ -370,9 +397,25 @@ extern "C" const char *islbm_kernel_name(const islbm_t *h) {
 extern "C" int islbm_set_kernel(islbm_t *h, int which) {
   if (!h) return fail(ISLBM_ERR_ARG, "NULL handle");
   if (which < 0 || which > 3) return fail(ISLBM_ERR_ARG, "kernel selector must be 0..3");
-  if (which == 2 && !h->tiled.available) return fail(ISLBM_ERR_ARG, "tiled kernel not available for this mesh");
-  if (which == 3) return fail(ISLBM_ERR_ARG, "uniform-shift kernel not built yet");
+  if (which == 2 && !h->tiled_ok()) return fail(ISLBM_ERR_ARG, std::string("tiled kernel not available: ") + h->tiled_why_not());
+  if (which == 3 && !h->uniform) return fail(ISLBM_ERR_ARG, "uniform-shift kernel needs every spacing to equal delta");
   h->kernel_choice = which;
+  return ISLBM_OK;
+}
+
+extern "C" int islbm_set_tuning(islbm_t *h, const char *key, int value) {
+  if (!h || !key) return fail(ISLBM_ERR_ARG, "NULL argument");
+  const std::string k(key);
+  Tuning &t = h->tune;
+  if (k == "chunk") t.chunk = value;
+  else if (k == "l2promo") t.l2promo = value;
+  else if (k == "load_policy") t.load_policy = value;
+  else if (k == "store_policy") t.store_policy = value;
+  else if (k == "tx2d") { if (value != 0 && value != 128 && value != 224) return fail(ISLBM_ERR_ARG, "tx2d must be 0, 128 or 224"); t.tx2d = value; }
+  else if (k == "serpentine") t.serpentine = value;
+  else return fail(ISLBM_ERR_ARG, "unknown tuning key: " + k);
+  if (value < 0) return fail(ISLBM_ERR_ARG, "tuning values are non-negative");
+  make_tiled_plan(h);
   return ISLBM_OK;
 }
 
@@ -383,9 +426,20 @@ extern "C" int islbm_step(islbm_t *h, int n) {
   const int which = effective_kernel(h);
   for (int s = 0; s < n; ++s) {
     if (which == 2) {
-      int rc = tiled_step(h->tiled, h->dm, h->np, h->cur, h->stream, g_err);
-      if (rc) return rc;
-      h->launches += h->tiled.launches_per_step;
+      void *bufs[2] = {h->ws + h->cv.buf[0], h->ws + h->cv.buf[1]};
+      cudaError_t e;
+      if (h->dim == 2)
+        e = h->precision == ISLBM_F64 ? launch2<double>(h->plan2, h->n, h->dm, h->np, h->cur, bufs, h->tune, h->stream)
+                                      : launch2<float>(h->plan2, h->n, h->dm, h->np, h->cur, bufs, h->tune, h->stream);
+      else
+        e = h->precision == ISLBM_F64 ? launch3<double>(h->plan3, h->n, h->dm, h->np, h->cur, bufs, h->tune, h->stream)
+                                      : launch3<float>(h->plan3, h->n, h->dm, h->np, h->cur, bufs, h->tune, h->stream);
+      if (e != cudaSuccess) return fail(ISLBM_ERR_CUDA, std::string("tiled step launch: ") + cudaGetErrorString(e));
+      h->launches++;
+    } else if (which == 3) {
+#define CALL(D, T) launch_shift_step<D, T>(h)
+      DISPATCH(h, CALL);
+#undef CALL
     } else {
 #define CALL(D, T) launch_generic_step<D, T>(h, true, nullptr, nullptr)
       DISPATCH(h, CALL);

@@ -1,0 +1,294 @@
+// islbm_tiled2.cuh — fused, TMA-staged ISLBM step for D2Q9 + D2Q5 on sm_100a.
+//
+// "y-marching" design, the 2-D counterpart of islbm_tiled3.cuh:
+//   * a CTA owns a strip of TX nodes in x (one thread per x) and marches
+//     through a chunk of rows;
+//   * one elected thread streams, per row, one TMA box per population plane
+//     (cp.async.bulk.tensor.2d over the view (x, q*ny + y)) into a ring of
+//     shared-memory stages guarded by full/empty mbarriers; planes with e_x != 0
+//     (f1 f3 g1 g3 f5..f8) carry a 16-byte x-halo on each side, the others
+//     (f0 g0 f2 f4 g2 g4) none;
+//   * consumers interpolate along x from shared memory; the y-direction of the
+//     separable interpolation is a 3-row combination kept
+//     in REGISTERS for the 8 populations with e_y != 0, so every post-collision
+//     value is staged once and there is no y-halo at all;
+//   * the node collides once and stores its 14 values with coalesced stores.
+// Summation order is the oracle's: x, then y.
+#pragma once
+
+#include "islbm_tiled3.cuh"
+
+namespace islbmk {
+
+template <typename ST, int TX_, int STAGES_>
+struct Tile2 {
+  static constexpr int TX = TX_, STAGES = STAGES_;
+  static constexpr int XH = 16 / (int)sizeof(ST);
+  static constexpr int HX = TX + 2 * XH;
+  static constexpr int N_X = 8, N_C = 6;
+  static constexpr int B_X = HX * (int)sizeof(ST), B_C = TX * (int)sizeof(ST);
+  static constexpr int S_X = pad128(B_X), S_C = pad128(B_C);
+  static constexpr int OFF_X = 0, OFF_C = N_X * S_X;
+  static constexpr int STAGE_BYTES = OFF_C + N_C * S_C;
+  static constexpr int WARPS = TX / 32;
+  static constexpr uint32_t Y_BYTES = 4u * B_X + 2u * B_C;   // planes of the emitted row
+  static constexpr uint32_t M_BYTES = 4u * B_X + 4u * B_C;   // planes of the y-stencil row
+  static constexpr size_t SMEM_BYTES = (size_t)STAGES * STAGE_BYTES + 2 * STAGES * 8 + 128;
+};
+
+struct Maps2 {
+  CUtensorMap x, c;
+};
+
+// stage s < 2 : the first two rows of the y-stencil of the chunk's first row;
+// stage s >= 2: the planes of emitted row y = y0+s-2, plus the new y-stencil row if the stencil base moves.
+template <typename T>
+__device__ __forceinline__ void issue_stage2(int s, int y0, int ny, int x0, unsigned char *stage0, uint64_t *full,
+                                             uint64_t *empty, const Maps2 &mp, uint64_t pol) {
+  const int st = s % T::STAGES;
+  const uint32_t ph = (uint32_t)(s / T::STAGES) & 1u;
+  if (s >= T::STAGES) mbar_wait(&empty[st], ph ^ 1u);
+  int mrow = -1, yrow = -1;
+  if (s < 2) {
+    mrow = sbase(y0, ny) + s;
+  } else {
+    yrow = y0 + (s - 2);
+    if (s == 2 || sbase(yrow, ny) != sbase(yrow - 1, ny)) mrow = sbase(yrow, ny) + 2;
+  }
+  mbar_expect_tx(&full[st], (mrow >= 0 ? T::M_BYTES : 0u) + (yrow >= 0 ? T::Y_BYTES : 0u));
+  unsigned char *sb = stage0 + (size_t)st * T::STAGE_BYTES;
+  uint64_t *bar = &full[st];
+  const int xh = x0 - T::XH;
+  if (yrow >= 0) {
+    tma_load_2d(sb + T::OFF_X + 0 * T::S_X, &mp.x, bar, xh, 1 * ny + yrow, pol);         // f1
+    tma_load_2d(sb + T::OFF_X + 1 * T::S_X, &mp.x, bar, xh, 3 * ny + yrow, pol);         // f3
+    tma_load_2d(sb + T::OFF_X + 2 * T::S_X, &mp.x, bar, xh, (9 + 1) * ny + yrow, pol);   // g1
+    tma_load_2d(sb + T::OFF_X + 3 * T::S_X, &mp.x, bar, xh, (9 + 3) * ny + yrow, pol);   // g3
+    tma_load_2d(sb + T::OFF_C + 0 * T::S_C, &mp.c, bar, x0, 0 * ny + yrow, pol);         // f0
+    tma_load_2d(sb + T::OFF_C + 1 * T::S_C, &mp.c, bar, x0, 9 * ny + yrow, pol);         // g0
+  }
+  if (mrow >= 0) {
+#pragma unroll
+    for (int k = 0; k < 4; ++k)
+      tma_load_2d(sb + T::OFF_X + (4 + k) * T::S_X, &mp.x, bar, xh, (5 + k) * ny + mrow, pol);   // f5..f8
+    tma_load_2d(sb + T::OFF_C + 2 * T::S_C, &mp.c, bar, x0, 2 * ny + mrow, pol);         // f2
+    tma_load_2d(sb + T::OFF_C + 3 * T::S_C, &mp.c, bar, x0, 4 * ny + mrow, pol);         // f4
+    tma_load_2d(sb + T::OFF_C + 4 * T::S_C, &mp.c, bar, x0, (9 + 2) * ny + mrow, pol);   // g2
+    tma_load_2d(sb + T::OFF_C + 5 * T::S_C, &mp.c, bar, x0, (9 + 4) * ny + mrow, pol);   // g4
+  }
+}
+
+template <typename ST, int TX, int STAGES, int MINB>
+__global__ void __launch_bounds__(TX, MINB)
+k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const ST *__restrict__ src, ST *__restrict__ dst,
+              int ychunk, int load_policy, int store_policy, int reverse) {
+  using T = Tile2<ST, TX, STAGES>;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  unsigned char *stage0 = smem_raw;
+  uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + (size_t)T::STAGES * T::STAGE_BYTES);
+  uint64_t *empty = full + T::STAGES;
+
+  const int bx = reverse ? gridDim.x - 1 - blockIdx.x : blockIdx.x;
+  const int by = reverse ? gridDim.y - 1 - blockIdx.y : blockIdx.y;
+  const int x0 = bx * T::TX;
+  const int y0 = by * ychunk, y1 = min(y0 + ychunk, m.ny);
+  const int nstage = 2 + (y1 - y0);
+
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < T::STAGES; ++s) {
+      mbar_init(&full[s], 1);
+      mbar_init(&empty[s], T::WARPS);
+    }
+    fence_barrier_init();
+  }
+  __syncthreads();
+
+  const uint64_t lpol = make_policy(load_policy);
+  const uint64_t spol = make_policy(store_policy);
+  if (threadIdx.x == 0) {
+    tma_prefetch_desc(&mp.x);
+    tma_prefetch_desc(&mp.c);
+    for (int s = 0; s < T::STAGES - 1 && s < nstage; ++s) issue_stage2<T>(s, y0, m.ny, x0, stage0, full, empty, mp, lpol);
+  }
+
+  const int tx = threadIdx.x;
+  const int x = x0 + tx;
+  const bool valid = x < m.nx;
+  WallFlags wf;
+  wf.lo[0] = valid && x == 0;
+  wf.hi[0] = valid && x == m.nx - 1;
+  wf.lo[2] = wf.hi[2] = false;
+  const bool wall_x = wf.lo[0] | wf.hi[0];
+  const int sx = wf.lo[0] ? 1 : (wf.hi[0] ? -1 : 0);
+  const int o_x = tx + T::XH - 1 + sx;
+  double wx[2][3];
+#pragma unroll
+  for (int s = 0; s < 2; ++s)
+#pragma unroll
+    for (int k = 0; k < 3; ++k) wx[s][k] = valid ? __ldg(wrow(m, 0, s, k) + x) : 0.0;
+
+  // x-interpolated values of the three y-stencil rows for the 8 populations with e_y != 0:
+  //   index: 0 f2, 1 f4, 2 g2, 3 g4, 4 f5, 5 f6, 6 f7, 7 f8
+  double A[8], B[8], C[8];
+#pragma unroll
+  for (int i = 0; i < 8; ++i) A[i] = B[i] = C[i] = 0.0;
+
+#pragma unroll 1
+  for (int s = 0; s < nstage; ++s) {
+    const int st = s % T::STAGES;
+    const uint32_t ph = (uint32_t)(s / T::STAGES) & 1u;
+    const int y = y0 + (s - 2);
+    const bool has_emit = s >= 2;
+    const bool has_mov = s <= 2 || sbase(y, m.ny) != sbase(y - 1, m.ny);
+    const unsigned char *sb = stage0 + (size_t)st * T::STAGE_BYTES;
+    auto PX = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_X + k * T::S_X); };
+    auto PC = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_C + k * T::S_C); };
+    if (threadIdx.x == 0 && s + T::STAGES - 1 < nstage)
+      issue_stage2<T>(s + T::STAGES - 1, y0, m.ny, x0, stage0, full, empty, mp, lpol);
+    __syncwarp();
+    mbar_wait(&full[st], ph);
+
+    if (has_mov) {
+#pragma unroll
+      for (int i = 0; i < 8; ++i) { A[i] = B[i]; B[i] = C[i]; }
+      C[0] = (double)PC(2)[tx];                      // f2
+      C[1] = (double)PC(3)[tx];                      // f4
+      C[2] = (double)PC(4)[tx];                      // g2
+      C[3] = (double)PC(5)[tx];                      // g4
+      C[4] = tap3(PX(4) + o_x, 1, wx[1]);            // f5 ( 1, 1)
+      C[5] = tap3(PX(5) + o_x, 1, wx[0]);            // f6 (-1, 1)
+      C[6] = tap3(PX(6) + o_x, 1, wx[0]);            // f7 (-1,-1)
+      C[7] = tap3(PX(7) + o_x, 1, wx[1]);            // f8 ( 1,-1)
+    }
+
+    if (has_emit) {
+      double wy[2][3];
+#pragma unroll
+      for (int sg = 0; sg < 2; ++sg)
+#pragma unroll
+        for (int k = 0; k < 3; ++k) wy[sg][k] = __ldg(wrow(m, 1, sg, k) + y);
+      double f[9], g[5];
+      f[0] = (double)PC(0)[tx];
+      g[0] = (double)PC(1)[tx];
+      f[1] = tap3(PX(0) + o_x, 1, wx[1]);
+      f[3] = tap3(PX(1) + o_x, 1, wx[0]);
+      g[1] = tap3(PX(2) + o_x, 1, wx[1]);
+      g[3] = tap3(PX(3) + o_x, 1, wx[0]);
+      __syncwarp();
+      if ((threadIdx.x & 31) == 0) mbar_arrive(&empty[st]);
+      f[2] = comb3(wy[1], A[0], B[0], C[0]);
+      f[4] = comb3(wy[0], A[1], B[1], C[1]);
+      g[2] = comb3(wy[1], A[2], B[2], C[2]);
+      g[4] = comb3(wy[0], A[3], B[3], C[3]);
+      f[5] = comb3(wy[1], A[4], B[4], C[4]);
+      f[6] = comb3(wy[1], A[5], B[5], C[5]);
+      f[7] = comb3(wy[0], A[6], B[6], C[6]);
+      f[8] = comb3(wy[0], A[7], B[7], C[7]);
+      const long long c = (long long)y * m.nx + x;
+      wf.lo[1] = y == 0;
+      wf.hi[1] = y == m.ny - 1;
+      if (valid && (wall_x | wf.lo[1] | wf.hi[1])) {
+        bb_fix_all_f<2>(f, wf, src, m.nn, c, std::make_integer_sequence<int, 8>{});
+        bb_fix_all_g<2>(g, wf, src + 9 * m.nn, m.nn, c, m, std::make_integer_sequence<int, 4>{});
+      }
+#pragma unroll
+      for (int q = 0; q < 9; ++q) f[q] += Store<ST, 2>::bias(q);
+      collide_node(f, g, np);
+      if (valid) {
+#pragma unroll
+        for (int q = 0; q < 9; ++q) st_hint(dst + (long long)q * m.nn + c, (ST)(f[q] - Store<ST, 2>::bias(q)), spol);
+#pragma unroll
+        for (int q = 0; q < 5; ++q) st_hint(dst + (long long)(9 + q) * m.nn + c, (ST)g[q], spol);
+      }
+    } else {
+      __syncwarp();
+      if ((threadIdx.x & 31) == 0) mbar_arrive(&empty[st]);
+    }
+  }
+}
+
+// ------------------------------ host side ---------------------------------
+struct Plan2 {
+  bool available = false;
+  Maps2 maps[2];
+  int tx = 128;
+  int ychunk = 32;
+  char why_not[96] = "";
+};
+
+// the two instantiated strip widths: (TX, STAGES, min CTAs/SM)
+template <typename ST> struct Cfg2a { using T = Tile2<ST, 128, 4>; static constexpr int MINB = 3; };
+template <typename ST> struct Cfg2b { using T = Tile2<ST, 224, 3>; static constexpr int MINB = 2; };
+
+template <typename ST, typename CFG>
+inline bool plan2_setup(Plan2 &p, const int *n, void *buf0, void *buf1, const Tuning &tn) {
+  using T = typename CFG::T;
+  auto kern = k_step_ymarch<ST, T::TX, T::STAGES, CFG::MINB>;
+  void *bufs[2] = {buf0, buf1};
+  for (int i = 0; i < 2; ++i)
+    if (!make_map(&p.maps[i].x, bufs[i], 2, (int)sizeof(ST), n[0], 1, 14LL * n[1], T::HX, 1, tn.l2promo) ||
+        !make_map(&p.maps[i].c, bufs[i], 2, (int)sizeof(ST), n[0], 1, 14LL * n[1], T::TX, 1, tn.l2promo))
+      return false;
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM_BYTES) != cudaSuccess) {
+    cudaGetLastError();
+    return false;
+  }
+  int occ = 1, dev = 0, sms = 148;
+  cudaGetDevice(&dev);
+  cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, T::TX, T::SMEM_BYTES) != cudaSuccess || occ < 1) {
+    cudaGetLastError();
+    occ = 1;
+  }
+  // one full wave of resident CTAs, chunks of at least 8 rows to amortise the 2-row prologue
+  const int strips = (n[0] + T::TX - 1) / T::TX;
+  int chunk;
+  if (tn.chunk > 0) {
+    chunk = tn.chunk;
+  } else {
+    int nchunks = (sms * occ) / strips;
+    if (nchunks < 1) nchunks = 1;
+    chunk = (n[1] + nchunks - 1) / nchunks;
+    if (chunk < 8) chunk = 8;
+  }
+  p.ychunk = chunk < n[1] ? chunk : n[1];
+  p.tx = T::TX;
+  return true;
+}
+
+template <typename ST>
+inline bool plan2_create(Plan2 &p, const int *n, void *buf0, void *buf1, const Tuning &tn) {
+  p.available = false;
+  auto no = [&](const char *why) { snprintf(p.why_not, sizeof p.why_not, "%s", why); return false; };
+  if (n[0] < 3 || n[1] < 3) return no("tiled kernel: n >= 3");
+  if (n[0] % (16 / (int)sizeof(ST))) return no("tiled kernel: TMA needs a 16-byte row pitch");
+  int dev = 0, cc_major = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return no("no device");
+  cudaDeviceGetAttribute(&cc_major, cudaDevAttrComputeCapabilityMajor, dev);
+  if (cc_major < 10) return no("tiled kernel: needs sm_100");
+  const int tx = tn.tx2d ? tn.tx2d : 128;   // a TMA box is at most 256 elements wide: TX + 2*XH <= 256
+  const bool ok = tx == 224 ? plan2_setup<ST, Cfg2b<ST>>(p, n, buf0, buf1, tn) : plan2_setup<ST, Cfg2a<ST>>(p, n, buf0, buf1, tn);
+  if (!ok) return no("tiled kernel: tensor map / attribute setup failed");
+  p.available = true;
+  return true;
+}
+
+template <typename ST, typename CFG>
+inline void launch2_cfg(const Plan2 &p, const int *n, const DevMesh &m, const NodeParams &np, int cur, void *const *buf,
+                        const Tuning &tn, cudaStream_t stream) {
+  using T = typename CFG::T;
+  dim3 grid((n[0] + T::TX - 1) / T::TX, (n[1] + p.ychunk - 1) / p.ychunk, 1);
+  k_step_ymarch<ST, T::TX, T::STAGES, CFG::MINB><<<grid, T::TX, T::SMEM_BYTES, stream>>>(
+      p.maps[cur], m, np, (const ST *)buf[cur], (ST *)buf[1 - cur], p.ychunk, tn.load_policy, tn.store_policy,
+      tn.serpentine ? cur : 0);
+}
+
+template <typename ST>
+inline cudaError_t launch2(const Plan2 &p, const int *n, const DevMesh &m, const NodeParams &np, int cur, void *const *buf,
+                           const Tuning &tn, cudaStream_t stream) {
+  if (p.tx == 224) launch2_cfg<ST, Cfg2b<ST>>(p, n, m, np, cur, buf, tn, stream);
+  else launch2_cfg<ST, Cfg2a<ST>>(p, n, m, np, cur, buf, tn, stream);
+  return cudaPeekAtLastError();
+}
+
+}  // namespace islbmk

@@ -22,7 +22,7 @@ KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED, KERNEL_UNIFORM_SHIFT = 0, 1, 2, 3
 EXPORTS = (
     "islbm_workspace_bytes", "islbm_create", "islbm_destroy", "islbm_get_params", "islbm_init",
     "islbm_set_populations", "islbm_get_populations", "islbm_step", "islbm_fields", "islbm_nusselt",
-    "islbm_steady_residual", "islbm_set_buoyancy_scale", "islbm_set_kernel", "islbm_launch_count",
+    "islbm_steady_residual", "islbm_set_buoyancy_scale", "islbm_set_kernel", "islbm_set_tuning", "islbm_launch_count",
     "islbm_kernel_name", "islbm_last_error", "islbm_version",
 )
 
@@ -63,6 +63,7 @@ def _load():
     lib.islbm_steady_residual.argtypes = [vp, dp]
     lib.islbm_set_buoyancy_scale.argtypes = [vp, C.c_double]
     lib.islbm_set_kernel.argtypes = [vp, C.c_int]
+    lib.islbm_set_tuning.argtypes = [vp, C.c_char_p, C.c_int]
     lib.islbm_launch_count.argtypes = [vp]
     lib.islbm_launch_count.restype = C.c_longlong
     lib.islbm_kernel_name.argtypes = [vp]
@@ -153,6 +154,10 @@ class Islbm:
 
     def set_kernel(self, which):
         _check(lib.islbm_set_kernel(self.h, int(which)))
+
+    def set_tuning(self, **kv):
+        for k, v in kv.items():
+            _check(lib.islbm_set_tuning(self.h, k.encode(), int(v)))
 
     @property
     def kernel_name(self):

@@ -55,14 +55,35 @@ def ragged_coords(dim, ns, stretches):
 
 
 def kernels_for(islbm, sim):
-    ks = [islbm.KERNEL_GENERIC]
+    """(kernel, tuning) variants valid for this mesh: the generic kernel, the TMA-staged kernel in the
+    launch configurations bench.py can select (strip width, chunk length incl. ragged chunks, L2 policies,
+    serpentine order), and the pure-shift kernel on uniform meshes."""
+    ks = [(islbm.KERNEL_GENERIC, {})]
     try:
         sim.set_kernel(islbm.KERNEL_TILED)
-        ks.append(islbm.KERNEL_TILED)
+        ks.append((islbm.KERNEL_TILED, {}))
+        ks.append((islbm.KERNEL_TILED, dict(chunk=5, load_policy=1, store_policy=2, l2promo=2)))
+        if sim.dim == 2:
+            ks.append((islbm.KERNEL_TILED, dict(tx2d=128, chunk=7, serpentine=1)))
+            ks.append((islbm.KERNEL_TILED, dict(tx2d=224, chunk=3)))
+            ks.append((islbm.KERNEL_TILED, dict(tx2d=224, chunk=0, serpentine=1, load_policy=1)))
+    except islbm.IslbmError:
+        pass
+    try:
+        sim.set_kernel(islbm.KERNEL_UNIFORM_SHIFT)
+        ks.append((islbm.KERNEL_UNIFORM_SHIFT, {}))
     except islbm.IslbmError:
         pass
     sim.set_kernel(islbm.KERNEL_AUTO)
     return ks
+
+
+DEFAULT_TUNING = dict(chunk=0, l2promo=3, load_policy=0, store_policy=0, tx2d=0, serpentine=0)
+
+
+def select(sim, k, tune):
+    sim.set_tuning(**{**DEFAULT_TUNING, **tune})
+    sim.set_kernel(k)
 
 
 # ---------------------------------------------------------------------------
@@ -72,6 +93,11 @@ CASES_1STEP = [
     ("2d_64sq_c1", 2, (64, 64, 1), (1.2, 1.2, 0)),
     ("2d_ragged_70x45", 2, (70, 45, 1), (1.6, 1.1, 0)),
     ("2d_ragged_131x67", 2, (131, 67, 1), (1.3, 1.9, 0)),
+    ("2d_strips_300x40", 2, (300, 40, 1), (1.5, 1.3, 0)),
+    ("2d_strips_516x37", 2, (516, 37, 1), (1.8, 1.2, 0)),
+    ("2d_strips_258x9", 2, (258, 9, 1), (1.4, 0.8, 0)),
+    ("2d_strips_130x3", 2, (130, 3, 1), (1.4, 0.5, 0)),
+    ("2d_tiled_4x4", 2, (4, 4, 1), (0.5, 0.5, 0)),
     ("2d_min_3x3", 2, (3, 3, 1), (0.5, 0.5, 0)),
     ("2d_thin_3x40", 2, (3, 40, 1), (0.5, 1.5, 0)),
     ("3d_ragged_37x21x19", 3, (37, 21, 19), (1.5, 1.2, 1.7)),
@@ -95,21 +121,47 @@ def test_one_step_all_populations(islbm, name, dim, ns, st):
     orc.set_populations(f0, g0)
     orc.step(1)
     fo, go = orc.get_populations()
-    for k in kernels_for(islbm, sim):
-        sim.set_kernel(k)
+    orc.step(2)
+    fo3, go3 = orc.get_populations()
+    for k, tune in kernels_for(islbm, sim):
+        select(sim, k, tune)
         sim.set_populations(torch.from_numpy(f0).cuda(), torch.from_numpy(g0).cuda())
         f_back, g_back = sim.get_populations()            # before any step: the input itself
         assert np.array_equal(f_back.cpu().numpy(), f0) and np.array_equal(g_back.cpu().numpy(), g0)
         sim.step(1)
         f1, g1 = sim.get_populations()
         ef, eg = plane_err(f1.cpu().numpy(), fo), plane_err(g1.cpu().numpy(), go)
-        assert ef <= 1e-12 and eg <= 1e-12, (name, sim.kernel_name, ef, eg)
-    # second and third step (ping-pong both ways)
-    sim.step(2)
-    orc.step(2)
-    f3, g3 = sim.get_populations()
+        assert ef <= 1e-12 and eg <= 1e-12, (name, sim.kernel_name, tune, ef, eg)
+        # second and third step (ping-pong both ways)
+        sim.step(2)
+        f3, g3 = sim.get_populations()
+        ef, eg = plane_err(f3.cpu().numpy(), fo3), plane_err(g3.cpu().numpy(), go3)
+        assert ef <= 3e-12 and eg <= 3e-12, (name, sim.kernel_name, tune, ef, eg)
+
+
+@pytest.mark.parametrize("dim,ns,st", [(2, (132, 45, 1), (1.5, 1.2, 0)), (2, (520, 21, 1), (1.7, 1.1, 0)),
+                                       (3, (36, 18, 9), (1.3, 1.2, 1.1)), (3, (68, 27, 20), (1.5, 1.1, 1.4))])
+def test_fp32_storage_every_kernel_three_steps(islbm, dim, ns, st):
+    """fp32 storage of f_q - w_q and g_q, fp64 arithmetic: every kernel variant against the fp64 oracle.
+    Tolerance: 3 steps x one fp32 rounding (2^-24 relative to |f_q - w_q| <= 0.4) per stored value, amplified
+    by the 9-point interpolation weights (|w| sums <= ~2): 2e-6 of the plane maximum."""
+    coords, delta = ragged_coords(dim, ns, st)
+    H_lu = (coords[1][-1] - coords[1][0] + delta) / delta
+    Ra = 0.71 * (0.1 * H_lu / 0.03) ** 2
+    sim, orc = pair(islbm, coords, delta, Ra=Ra, precision=1)
+    f0, g0 = inputs.random_state(orc.shape, orc.qf, orc.qg, seed=11 + dim, amp=0.05)
+    orc.set_populations(f0, g0)
+    orc.step(3)
     fo, go = orc.get_populations()
-    assert plane_err(f3.cpu().numpy(), fo) <= 3e-12 and plane_err(g3.cpu().numpy(), go) <= 3e-12
+    variants = kernels_for(islbm, sim)
+    assert any(k == islbm.KERNEL_TILED for k, _ in variants)
+    for k, tune in variants:
+        select(sim, k, tune)
+        sim.set_populations(torch.from_numpy(f0).cuda(), torch.from_numpy(g0).cuda())
+        sim.step(3)
+        f3, g3 = sim.get_populations()
+        ef, eg = plane_err(f3.cpu().numpy(), fo), plane_err(g3.cpu().numpy(), go)
+        assert ef <= 2e-6 and eg <= 2e-6, (sim.kernel_name, tune, ef, eg)
 
 
 def test_uniform_mesh_one_step(islbm):
@@ -120,12 +172,14 @@ def test_uniform_mesh_one_step(islbm):
         orc.set_populations(f0, g0)
         orc.step(1)
         fo, go = orc.get_populations()
-        for k in kernels_for(islbm, sim):
-            sim.set_kernel(k)
+        variants = kernels_for(islbm, sim)
+        assert (islbm.KERNEL_UNIFORM_SHIFT, {}) in variants
+        for k, tune in variants:
+            select(sim, k, tune)
             sim.set_populations(torch.from_numpy(f0).cuda(), torch.from_numpy(g0).cuda())
             sim.step(1)
             f1, g1 = sim.get_populations()
-            assert plane_err(f1.cpu().numpy(), fo) <= 1e-12 and plane_err(g1.cpu().numpy(), go) <= 1e-12
+            assert plane_err(f1.cpu().numpy(), fo) <= 1e-12 and plane_err(g1.cpu().numpy(), go) <= 1e-12, (dim, k, tune)
         # mass is conserved to round-off on the uniform mesh (pin P4 on the GPU path)
         sim.step(200)
         rho = sim.fields(("rho",))["rho"]
