@@ -13,7 +13,10 @@
 //     in REGISTERS for the 8 populations with e_y != 0, so every post-collision
 //     value is staged once and there is no y-halo at all;
 //   * the node collides once and stores its 14 values with coalesced stores.
-// Summation order is the oracle's: x, then y.
+// DIR = +1 marches a chunk upwards, DIR = -1 downwards ("serpentine" tuning: odd
+// steps march downwards, so a step starts on the rows the previous step wrote
+// last, which are the ones most likely still in L2; the 2-D states are of the
+// order of the 126 MB L2).  Summation order is the oracle's either way: x, then y.
 #pragma once
 
 #include "islbm_tiled3.cuh"
@@ -33,27 +36,30 @@ struct Tile2 {
   static constexpr int WARPS = TX / 32;
   static constexpr uint32_t Y_BYTES = 4u * B_X + 2u * B_C;   // planes of the emitted row
   static constexpr uint32_t M_BYTES = 4u * B_X + 4u * B_C;   // planes of the y-stencil row
-  static constexpr size_t SMEM_BYTES = (size_t)STAGES * STAGE_BYTES + 2 * STAGES * 8 + 128;
+  static constexpr int BAR_OFF = STAGES * STAGE_BYTES;
+  static constexpr int W_OFF = BAR_OFF + 64;                 // y-weights of the chunk [sign][k][kMaxChunk]
+  static constexpr size_t SMEM_BYTES = (size_t)W_OFF + 6 * kMaxChunk * 8 + 128;
 };
 
 struct Maps2 {
   CUtensorMap x, c;
 };
 
-// stage s < 2 : the first two rows of the y-stencil of the chunk's first row;
-// stage s >= 2: the planes of emitted row y = y0+s-2, plus the new y-stencil row if the stencil base moves.
-template <typename T>
-__device__ __forceinline__ void issue_stage2(int s, int y0, int ny, int x0, unsigned char *stage0, uint64_t *full,
+// yf = first emitted row of the chunk (its lowest row for DIR = +1, its highest for DIR = -1).
+// stage s < 2 : the first two rows (in marching order) of the y-stencil of row yf;
+// stage s >= 2: the planes of emitted row y = yf + DIR*(s-2), plus the next y-stencil row if the stencil base moves.
+template <typename T, int DIR>
+__device__ __forceinline__ void issue_stage2(int s, int yf, int ny, int x0, unsigned char *stage0, uint64_t *full,
                                              uint64_t *empty, const Maps2 &mp, uint64_t pol) {
   const int st = s % T::STAGES;
   const uint32_t ph = (uint32_t)(s / T::STAGES) & 1u;
   if (s >= T::STAGES) mbar_wait(&empty[st], ph ^ 1u);
   int mrow = -1, yrow = -1;
   if (s < 2) {
-    mrow = sbase(y0, ny) + s;
+    mrow = DIR > 0 ? sbase(yf, ny) + s : sbase(yf, ny) + 2 - s;
   } else {
-    yrow = y0 + (s - 2);
-    if (s == 2 || sbase(yrow, ny) != sbase(yrow - 1, ny)) mrow = sbase(yrow, ny) + 2;
+    yrow = yf + DIR * (s - 2);
+    if (s == 2 || sbase(yrow, ny) != sbase(yrow - DIR, ny)) mrow = DIR > 0 ? sbase(yrow, ny) + 2 : sbase(yrow, ny);
   }
   mbar_expect_tx(&full[st], (mrow >= 0 ? T::M_BYTES : 0u) + (yrow >= 0 ? T::Y_BYTES : 0u));
   unsigned char *sb = stage0 + (size_t)st * T::STAGE_BYTES;
@@ -78,21 +84,25 @@ __device__ __forceinline__ void issue_stage2(int s, int y0, int ny, int x0, unsi
   }
 }
 
-template <typename ST, int TX, int STAGES, int MINB>
+template <typename ST, int TX, int STAGES, int MINB, int DIR>
 __global__ void __launch_bounds__(TX, MINB)
 k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const ST *__restrict__ src, ST *__restrict__ dst,
-              int ychunk, int load_policy, int store_policy, int reverse) {
+              int ychunk, int load_policy, int store_policy) {
   using T = Tile2<ST, TX, STAGES>;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   unsigned char *stage0 = smem_raw;
-  uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + (size_t)T::STAGES * T::STAGE_BYTES);
+  uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + T::BAR_OFF);
   uint64_t *empty = full + T::STAGES;
+  double *wys = reinterpret_cast<double *>(smem_raw + T::W_OFF);
 
-  const int bx = reverse ? gridDim.x - 1 - blockIdx.x : blockIdx.x;
-  const int by = reverse ? gridDim.y - 1 - blockIdx.y : blockIdx.y;
-  const int x0 = bx * T::TX;
-  const int y0 = by * ychunk, y1 = min(y0 + ychunk, m.ny);
+  const int x0 = blockIdx.x * T::TX;
+  const int y0 = blockIdx.y * ychunk, y1 = min(y0 + ychunk, m.ny);
+  const int yf = DIR > 0 ? y0 : y1 - 1;
   const int nstage = 2 + (y1 - y0);
+  for (int i = threadIdx.x; i < 6 * (y1 - y0); i += T::TX) {
+    const int sk = i / (y1 - y0), yi = i - sk * (y1 - y0);
+    wys[sk * kMaxChunk + yi] = __ldg(wrow(m, 1, sk / 3, sk % 3) + y0 + yi);
+  }
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < T::STAGES; ++s) {
@@ -108,7 +118,7 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
   if (threadIdx.x == 0) {
     tma_prefetch_desc(&mp.x);
     tma_prefetch_desc(&mp.c);
-    for (int s = 0; s < T::STAGES - 1 && s < nstage; ++s) issue_stage2<T>(s, y0, m.ny, x0, stage0, full, empty, mp, lpol);
+    for (int s = 0; s < T::STAGES - 1 && s < nstage; ++s) issue_stage2<T, DIR>(s, yf, m.ny, x0, stage0, full, empty, mp, lpol);
   }
 
   const int tx = threadIdx.x;
@@ -127,8 +137,8 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
 #pragma unroll
     for (int k = 0; k < 3; ++k) wx[s][k] = valid ? __ldg(wrow(m, 0, s, k) + x) : 0.0;
 
-  // x-interpolated values of the three y-stencil rows for the 8 populations with e_y != 0:
-  //   index: 0 f2, 1 f4, 2 g2, 3 g4, 4 f5, 5 f6, 6 f7, 7 f8
+  // x-interpolated values of the three y-stencil rows (A oldest, C newest in marching order) for the 8
+  // populations with e_y != 0:   index: 0 f2, 1 f4, 2 g2, 3 g4, 4 f5, 5 f6, 6 f7, 7 f8
   double A[8], B[8], C[8];
 #pragma unroll
   for (int i = 0; i < 8; ++i) A[i] = B[i] = C[i] = 0.0;
@@ -137,14 +147,14 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
   for (int s = 0; s < nstage; ++s) {
     const int st = s % T::STAGES;
     const uint32_t ph = (uint32_t)(s / T::STAGES) & 1u;
-    const int y = y0 + (s - 2);
+    const int y = yf + DIR * (s - 2);
     const bool has_emit = s >= 2;
-    const bool has_mov = s <= 2 || sbase(y, m.ny) != sbase(y - 1, m.ny);
+    const bool has_mov = s <= 2 || sbase(y, m.ny) != sbase(y - DIR, m.ny);
     const unsigned char *sb = stage0 + (size_t)st * T::STAGE_BYTES;
     auto PX = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_X + k * T::S_X); };
     auto PC = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_C + k * T::S_C); };
     if (threadIdx.x == 0 && s + T::STAGES - 1 < nstage)
-      issue_stage2<T>(s + T::STAGES - 1, y0, m.ny, x0, stage0, full, empty, mp, lpol);
+      issue_stage2<T, DIR>(s + T::STAGES - 1, yf, m.ny, x0, stage0, full, empty, mp, lpol);
     __syncwarp();
     mbar_wait(&full[st], ph);
 
@@ -166,7 +176,7 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
 #pragma unroll
       for (int sg = 0; sg < 2; ++sg)
 #pragma unroll
-        for (int k = 0; k < 3; ++k) wy[sg][k] = __ldg(wrow(m, 1, sg, k) + y);
+        for (int k = 0; k < 3; ++k) wy[sg][k] = wys[(sg * 3 + k) * kMaxChunk + (y - y0)];
       double f[9], g[5];
       f[0] = (double)PC(0)[tx];
       g[0] = (double)PC(1)[tx];
@@ -176,14 +186,16 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
       g[3] = tap3(PX(3) + o_x, 1, wx[0]);
       __syncwarp();
       if ((threadIdx.x & 31) == 0) mbar_arrive(&empty[st]);
-      f[2] = comb3(wy[1], A[0], B[0], C[0]);
-      f[4] = comb3(wy[0], A[1], B[1], C[1]);
-      g[2] = comb3(wy[1], A[2], B[2], C[2]);
-      g[4] = comb3(wy[0], A[3], B[3], C[3]);
-      f[5] = comb3(wy[1], A[4], B[4], C[4]);
-      f[6] = comb3(wy[1], A[5], B[5], C[5]);
-      f[7] = comb3(wy[0], A[6], B[6], C[6]);
-      f[8] = comb3(wy[0], A[7], B[7], C[7]);
+      // stencil rows in ascending-y order are (A,B,C) when marching up and (C,B,A) when marching down
+      auto ycomb = [&](const double (&w)[3], int i) { return DIR > 0 ? comb3(w, A[i], B[i], C[i]) : comb3(w, C[i], B[i], A[i]); };
+      f[2] = ycomb(wy[1], 0);
+      f[4] = ycomb(wy[0], 1);
+      g[2] = ycomb(wy[1], 2);
+      g[4] = ycomb(wy[0], 3);
+      f[5] = ycomb(wy[1], 4);
+      f[6] = ycomb(wy[1], 5);
+      f[7] = ycomb(wy[0], 6);
+      f[8] = ycomb(wy[0], 7);
       const long long c = (long long)y * m.nx + x;
       wf.lo[1] = y == 0;
       wf.hi[1] = y == m.ny - 1;
@@ -217,19 +229,21 @@ struct Plan2 {
 };
 
 // the two instantiated strip widths: (TX, STAGES, min CTAs/SM)
-template <typename ST> struct Cfg2a { using T = Tile2<ST, 128, 4>; static constexpr int MINB = 3; };
+template <typename ST> struct Cfg2a { using T = Tile2<ST, 128, 3>; static constexpr int MINB = 4; };
 template <typename ST> struct Cfg2b { using T = Tile2<ST, 224, 3>; static constexpr int MINB = 2; };
 
 template <typename ST, typename CFG>
 inline bool plan2_setup(Plan2 &p, const int *n, void *buf0, void *buf1, const Tuning &tn) {
   using T = typename CFG::T;
-  auto kern = k_step_ymarch<ST, T::TX, T::STAGES, CFG::MINB>;
+  auto kern = k_step_ymarch<ST, T::TX, T::STAGES, CFG::MINB, 1>;
+  auto kern_dn = k_step_ymarch<ST, T::TX, T::STAGES, CFG::MINB, -1>;
   void *bufs[2] = {buf0, buf1};
   for (int i = 0; i < 2; ++i)
     if (!make_map(&p.maps[i].x, bufs[i], 2, (int)sizeof(ST), n[0], 1, 14LL * n[1], T::HX, 1, tn.l2promo) ||
         !make_map(&p.maps[i].c, bufs[i], 2, (int)sizeof(ST), n[0], 1, 14LL * n[1], T::TX, 1, tn.l2promo))
       return false;
-  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM_BYTES) != cudaSuccess) {
+  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM_BYTES) != cudaSuccess ||
+      cudaFuncSetAttribute(kern_dn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM_BYTES) != cudaSuccess) {
     cudaGetLastError();
     return false;
   }
@@ -251,6 +265,7 @@ inline bool plan2_setup(Plan2 &p, const int *n, void *buf0, void *buf1, const Tu
     chunk = (n[1] + nchunks - 1) / nchunks;
     if (chunk < 8) chunk = 8;
   }
+  if (chunk > kMaxChunk) chunk = kMaxChunk;
   p.ychunk = chunk < n[1] ? chunk : n[1];
   p.tx = T::TX;
   return true;
@@ -278,9 +293,12 @@ inline void launch2_cfg(const Plan2 &p, const int *n, const DevMesh &m, const No
                         const Tuning &tn, cudaStream_t stream) {
   using T = typename CFG::T;
   dim3 grid((n[0] + T::TX - 1) / T::TX, (n[1] + p.ychunk - 1) / p.ychunk, 1);
-  k_step_ymarch<ST, T::TX, T::STAGES, CFG::MINB><<<grid, T::TX, T::SMEM_BYTES, stream>>>(
-      p.maps[cur], m, np, (const ST *)buf[cur], (ST *)buf[1 - cur], p.ychunk, tn.load_policy, tn.store_policy,
-      tn.serpentine ? cur : 0);
+  if (tn.serpentine && cur)
+    k_step_ymarch<ST, T::TX, T::STAGES, CFG::MINB, -1><<<grid, T::TX, T::SMEM_BYTES, stream>>>(
+        p.maps[cur], m, np, (const ST *)buf[cur], (ST *)buf[1 - cur], p.ychunk, tn.load_policy, tn.store_policy);
+  else
+    k_step_ymarch<ST, T::TX, T::STAGES, CFG::MINB, 1><<<grid, T::TX, T::SMEM_BYTES, stream>>>(
+        p.maps[cur], m, np, (const ST *)buf[cur], (ST *)buf[1 - cur], p.ychunk, tn.load_policy, tn.store_policy);
 }
 
 template <typename ST>

@@ -32,9 +32,11 @@
 
 namespace islbmk {
 
-template <typename ST>
+constexpr int kMaxChunk = 64;   // longest marching chunk (its weights are staged in shared memory)
+
+template <typename ST, int TX_ = 32, int TY_ = 8>
 struct Tile3 {
-  static constexpr int TX = 32, TY = 8;
+  static constexpr int TX = TX_, TY = TY_;
   // TMA needs a 16-byte aligned box origin (measured: a misaligned origin raises an illegal-instruction
   // fault), so the x-halo is 16 bytes wide on each side: 2 nodes in fp64, 4 in fp32 storage
   static constexpr int XH = 16 / (int)sizeof(ST);
@@ -50,7 +52,9 @@ struct Tile3 {
   static constexpr int THREADS = TX * TY;                // thread 0 doubles as the TMA producer
   static constexpr uint32_t Z_BYTES = 4u * B_XY + 4u * B_X + 4u * B_Y + 2u * B_C;   // planes of the emitted slice
   static constexpr uint32_t M_BYTES = 4u * B_X + 4u * B_Y + 4u * B_C;              // planes of the z-stencil slice
-  static constexpr size_t SMEM_BYTES = (size_t)STAGES * STAGE_BYTES + 2 * STAGES * 8 + 128;
+  static constexpr int BAR_OFF = STAGES * STAGE_BYTES;             // full[STAGES], empty[STAGES]
+  static constexpr int W_OFF = BAR_OFF + 64;                        // marching-axis weights [sign][k][kMaxChunk]
+  static constexpr size_t SMEM_BYTES = (size_t)W_OFF + 6 * kMaxChunk * 8 + 128;
 };
 
 struct Maps3 {
@@ -123,10 +127,9 @@ __device__ __forceinline__ int sbase(int j, int n) { return min(max(j - 1, 0), n
 // One pipeline stage = the TMA boxes one z-iteration needs.  Issued by one thread.
 //   stage s < 2 : the first two slices of the z-stencil of the chunk's first slice;
 //   stage s >= 2: the planes of emitted slice z = z0+s-2, plus the new z-stencil slice if the stencil base moves.
-template <typename ST>
+template <typename T>
 __device__ __forceinline__ void issue_stage3(int s, int z0, int nz, int x0, int y0, unsigned char *stage0, uint64_t *full,
                                              uint64_t *empty, const Maps3 &mp, uint64_t pol) {
-  using T = Tile3<ST>;
   const int st = s % T::STAGES;
   const uint32_t ph = (uint32_t)(s / T::STAGES) & 1u;
   if (s >= T::STAGES) mbar_wait(&empty[st], ph ^ 1u);   // every consumer warp has released the slot
@@ -170,19 +173,24 @@ __device__ __forceinline__ void issue_stage3(int s, int z0, int nz, int x0, int 
 }
 
 // ------------------------------ the kernel --------------------------------
-template <typename ST>
-__global__ void __launch_bounds__(Tile3<ST>::THREADS, 1)
+template <typename ST, int TX, int TY>
+__global__ void __launch_bounds__(TX * TY, 1)
 k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const ST *__restrict__ src,
               ST *__restrict__ dst, int zchunk, int load_policy, int store_policy) {
-  using T = Tile3<ST>;
+  using T = Tile3<ST, TX, TY>;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   unsigned char *stage0 = smem_raw;
-  uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + (size_t)T::STAGES * T::STAGE_BYTES);
+  uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + T::BAR_OFF);
   uint64_t *empty = full + T::STAGES;
+  double *wzs = reinterpret_cast<double *>(smem_raw + T::W_OFF);
 
   const int x0 = blockIdx.x * T::TX, y0 = blockIdx.y * T::TY;
   const int z0 = blockIdx.z * zchunk, z1 = min(z0 + zchunk, m.nz);
   const int nstage = 2 + (z1 - z0);
+  for (int i = threadIdx.x; i < 6 * (z1 - z0); i += T::THREADS) {
+    const int sk = i / (z1 - z0), zi = i - sk * (z1 - z0);
+    wzs[sk * kMaxChunk + zi] = __ldg(wrow(m, 2, sk / 3, sk % 3) + z0 + zi);
+  }
 
   if (threadIdx.x == 0) {
     for (int s = 0; s < T::STAGES; ++s) {
@@ -202,10 +210,10 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
     tma_prefetch_desc(&mp.y);
     tma_prefetch_desc(&mp.c);
     for (int s = 0; s < T::STAGES - 1 && s < nstage; ++s)
-      issue_stage3<ST>(s, z0, m.nz, x0, y0, stage0, full, empty, mp, lpol);
+      issue_stage3<T>(s, z0, m.nz, x0, y0, stage0, full, empty, mp, lpol);
   }
 
-  const int tx = threadIdx.x & 31, ty = threadIdx.x >> 5;
+  const int tx = threadIdx.x % T::TX, ty = threadIdx.x / T::TX;
   const int x = x0 + tx, y = y0 + ty;
   const bool valid = x < m.nx && y < m.ny;
   WallFlags wf;
@@ -249,7 +257,7 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
     auto PY = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_Y + k * T::S_Y); };
     auto PC = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_C + k * T::S_C); };
     if (threadIdx.x == 0 && s + T::STAGES - 1 < nstage)
-      issue_stage3<ST>(s + T::STAGES - 1, z0, m.nz, x0, y0, stage0, full, empty, mp, lpol);
+      issue_stage3<T>(s + T::STAGES - 1, z0, m.nz, x0, y0, stage0, full, empty, mp, lpol);
     __syncwarp();
     mbar_wait(&full[st], ph);
 
@@ -275,7 +283,7 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
 #pragma unroll
       for (int sg = 0; sg < 2; ++sg)
 #pragma unroll
-        for (int k = 0; k < 3; ++k) wz[sg][k] = __ldg(wrow(m, 2, sg, k) + z);
+        for (int k = 0; k < 3; ++k) wz[sg][k] = wzs[(sg * 3 + k) * kMaxChunk + (s - 2)];
       double f[19], g[7];
       f[0] = (double)PC(0)[o_c];
       g[0] = (double)PC(1)[o_c];
@@ -334,12 +342,13 @@ struct Plan3 {
   bool available = false;
   Maps3 maps[2];            // per ping-pong buffer
   int zchunk = 32;
+  int shape = 0;            // tile shape index: 0 32x8, 1 64x4, 2 128x2
   char why_not[96] = "";
 };
 
-template <typename ST>
-inline bool plan3_create(Plan3 &p, const int *n, void *buf0, void *buf1, const Tuning &tn) {
-  using T = Tile3<ST>;
+template <typename ST, int TX, int TY>
+inline bool plan3_setup(Plan3 &p, const int *n, void *buf0, void *buf1, const Tuning &tn) {
+  using T = Tile3<ST, TX, TY>;
   p.available = false;
   auto no = [&](const char *why) { snprintf(p.why_not, sizeof p.why_not, "%s", why); return false; };
   if (n[0] < 3 || n[1] < 3 || n[2] < 3) return no("tiled kernel: n >= 3");
@@ -360,30 +369,52 @@ inline bool plan3_create(Plan3 &p, const int *n, void *buf0, void *buf1, const T
         !make_map(&p.maps[i].c, bufs[i], 3, eb, n[0], n[1], ns, T::TX, T::TY, tn.l2promo))
       return no("cuTensorMapEncodeTiled failed");
   }
-  if (cudaFuncSetAttribute(k_step_zmarch<ST>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM_BYTES) != cudaSuccess) {
+  if (cudaFuncSetAttribute(k_step_zmarch<ST, TX, TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM_BYTES) != cudaSuccess) {
     cudaGetLastError();
     return no("cudaFuncSetAttribute failed");
   }
-  // z-chunks: enough CTAs for >= ~6 waves of 148 SMs, chunk >= 16 slices to amortise the 2-slice prologue
+  // z-chunks: enough CTAs for >= ~12 waves of 148 SMs (measured: shorter chunks win up to there), chunk >= 16
+  // slices to amortise the 2-slice prologue
   const int tiles = ((n[0] + T::TX - 1) / T::TX) * ((n[1] + T::TY - 1) / T::TY);
   int chunk = n[2];
   if (tn.chunk > 0) {
     chunk = tn.chunk < n[2] ? tn.chunk : n[2];
   } else {
-    while (chunk > 16 && (long long)tiles * ((n[2] + chunk - 1) / chunk) < 148 * 6) chunk = (chunk + 1) / 2;
+    if (chunk > kMaxChunk) chunk = kMaxChunk;
+    while (chunk > 16 && (long long)tiles * ((n[2] + chunk - 1) / chunk) < 148 * 12) chunk = (chunk + 1) / 2;
   }
-  p.zchunk = chunk;
+  p.zchunk = chunk < kMaxChunk ? chunk : kMaxChunk;
   p.available = true;
   return true;
 }
 
 template <typename ST>
+inline bool plan3_create(Plan3 &p, const int *n, void *buf0, void *buf1, const Tuning &tn) {
+  p.shape = tn.shape3d;
+  switch (tn.shape3d) {
+    case 1: return plan3_setup<ST, 64, 4>(p, n, buf0, buf1, tn);
+    case 2: return plan3_setup<ST, 128, 2>(p, n, buf0, buf1, tn);
+    default: p.shape = 0; return plan3_setup<ST, 32, 8>(p, n, buf0, buf1, tn);
+  }
+}
+
+template <typename ST, int TX, int TY>
+inline void launch3_shape(const Plan3 &p, const int *n, const DevMesh &m, const NodeParams &np, int cur, void *const *buf,
+                          const Tuning &tn, cudaStream_t stream) {
+  using T = Tile3<ST, TX, TY>;
+  dim3 grid((n[0] + T::TX - 1) / T::TX, (n[1] + T::TY - 1) / T::TY, (n[2] + p.zchunk - 1) / p.zchunk);
+  k_step_zmarch<ST, TX, TY><<<grid, T::THREADS, T::SMEM_BYTES, stream>>>(
+      p.maps[cur], m, np, (const ST *)buf[cur], (ST *)buf[1 - cur], p.zchunk, tn.load_policy, tn.store_policy);
+}
+
+template <typename ST>
 inline cudaError_t launch3(const Plan3 &p, const int *n, const DevMesh &m, const NodeParams &np, int cur, void *const *buf,
                            const Tuning &tn, cudaStream_t stream) {
-  using T = Tile3<ST>;
-  dim3 grid((n[0] + T::TX - 1) / T::TX, (n[1] + T::TY - 1) / T::TY, (n[2] + p.zchunk - 1) / p.zchunk);
-  k_step_zmarch<ST><<<grid, T::THREADS, T::SMEM_BYTES, stream>>>(p.maps[cur], m, np, (const ST *)buf[cur], (ST *)buf[1 - cur],
-                                                                 p.zchunk, tn.load_policy, tn.store_policy);
+  switch (p.shape) {
+    case 1: launch3_shape<ST, 64, 4>(p, n, m, np, cur, buf, tn, stream); break;
+    case 2: launch3_shape<ST, 128, 2>(p, n, m, np, cur, buf, tn, stream); break;
+    default: launch3_shape<ST, 32, 8>(p, n, m, np, cur, buf, tn, stream);
+  }
   return cudaPeekAtLastError();
 }
 

@@ -132,10 +132,11 @@ constexpr int pad128(int bytes) { return (bytes + 127) / 128 * 128; }
 // run-time knobs of the tiled kernels (islbm_set_tuning); defaults chosen from measurements (profiles/)
 struct Tuning {
   int chunk = 0;        // marching-chunk length (slices / rows); 0 = automatic
-  int l2promo = 3;      // tensor-map L2 promotion: 0 none, 1 64 B, 2 128 B, 3 256 B
+  int l2promo = 0;      // tensor-map L2 promotion: 0 none, 1 64 B, 2 128 B, 3 256 B (none measured fastest)
   int load_policy = 0;  // L2 eviction policy of the TMA loads: 0 normal, 1 evict_first, 2 evict_last
   int store_policy = 0; // ... of the population stores
   int tx2d = 0;         // 2-D strip width: 128 or 224; 0 = automatic
+  int shape3d = 0;      // 3-D tile shape: 0 32x8, 1 64x4, 2 128x2 (x by y nodes per CTA)
   int serpentine = 0;   // 2-D: reverse the CTA -> chunk map on odd steps (L2 reuse of the freshly written rows)
 };
 
