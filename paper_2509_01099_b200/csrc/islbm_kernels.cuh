@@ -7,9 +7,10 @@
 // once per step and every population is read once and written once
 // (PAPER.md:150-154 gives the collide -> stream order this is equivalent to).
 //
-// Layout: structure-of-arrays planes [q][z][y][x], flow planes first, then the
-// temperature planes; storage type ST is double, or float holding the
-// deviation f_q - w_q (ISLBM_F32_STORAGE).
+// Layout: structure-of-arrays planes [plane][z][y][x]; the plane of each
+// population is plane_f / plane_g (islbm_lattice.cuh: ordered by TMA halo
+// group); storage type ST is double, or float holding the deviation f_q - w_q
+// (ISLBM_F32_STORAGE).
 #pragma once
 
 #include <cstdint>
@@ -141,21 +142,21 @@ __device__ __forceinline__ double interp_plane(const DevMesh &m, const ST *__res
 template <int DIM, int Q, typename ST>
 __device__ __forceinline__ double pull_f(const DevMesh &m, const ST *__restrict__ src, const NodeCtx<DIM> &cx) {
   constexpr int EX = evel<DIM>(Q, 0), EY = evel<DIM>(Q, 1), EZ = evel<DIM>(Q, 2);
-  if (crosses<DIM, EX, EY, EZ>(cx)) return ldv(src + (long long)opposite<DIM>(Q) * m.nn + cx.c);
-  return interp_plane<DIM, EX, EY, EZ>(m, src + (long long)Q * m.nn, cx);
+  if (crosses<DIM, EX, EY, EZ>(cx)) return ldv(src + (long long)plane_f<DIM>(opposite<DIM>(Q)) * m.nn + cx.c);
+  return interp_plane<DIM, EX, EY, EZ>(m, src + (long long)plane_f<DIM>(Q) * m.nn, cx);
 }
 
 // Temperature population Q: interpolation; anti-bounce-back on the isothermal
 // x-walls (Eq. 22); bounce-back on the adiabatic walls (Eq. 23).
 template <int DIM, int Q, typename ST>
-__device__ __forceinline__ double pull_g(const DevMesh &m, const ST *__restrict__ srcg, const NodeCtx<DIM> &cx) {
+__device__ __forceinline__ double pull_g(const DevMesh &m, const ST *__restrict__ src, const NodeCtx<DIM> &cx) {
   constexpr int EX = evel<DIM>(Q, 0), EY = evel<DIM>(Q, 1), EZ = evel<DIM>(Q, 2);
   if (crosses<DIM, EX, EY, EZ>(cx)) {
-    const double gb = ldv(srcg + (long long)opposite<DIM>(Q) * m.nn + cx.c);
+    const double gb = ldv(src + (long long)plane_g<DIM>(opposite<DIM>(Q)) * m.nn + cx.c);
     if (EX != 0) return -gb + m.omega_bc * (cx.lo[0] ? m.T_hot : m.T_cold);
     return gb;
   }
-  return interp_plane<DIM, EX, EY, EZ>(m, srcg + (long long)Q * m.nn, cx);
+  return interp_plane<DIM, EX, EY, EZ>(m, src + (long long)plane_g<DIM>(Q) * m.nn, cx);
 }
 
 template <int DIM, typename ST, int... Qs>
@@ -164,9 +165,9 @@ __device__ __forceinline__ void pull_all_f(const DevMesh &m, const ST *src, cons
   ((f[Qs] = pull_f<DIM, Qs>(m, src, cx)), ...);
 }
 template <int DIM, typename ST, int... Qs>
-__device__ __forceinline__ void pull_all_g(const DevMesh &m, const ST *srcg, const NodeCtx<DIM> &cx,
+__device__ __forceinline__ void pull_all_g(const DevMesh &m, const ST *src, const NodeCtx<DIM> &cx,
                                            double *g, std::integer_sequence<int, Qs...>) {
-  ((g[Qs] = pull_g<DIM, Qs>(m, srcg, cx)), ...);
+  ((g[Qs] = pull_g<DIM, Qs>(m, src, cx)), ...);
 }
 
 // ---------------------------------------------------------------------------
@@ -187,15 +188,15 @@ k_step_generic(DevMesh m, NodeParams np, const ST *__restrict__ src, ST *__restr
   make_ctx<DIM>(m, ix, iy, iz, cx);
   double f[QF], g[QG];
   pull_all_f<DIM>(m, src, cx, f, std::make_integer_sequence<int, QF>{});
-  pull_all_g<DIM>(m, src + (long long)QF * m.nn, cx, g, std::make_integer_sequence<int, QG>{});
+  pull_all_g<DIM>(m, src, cx, g, std::make_integer_sequence<int, QG>{});
 #pragma unroll
   for (int q = 0; q < QF; ++q) f[q] += Store<ST, DIM>::bias(q);
   if (COLLIDE) {
     collide_node(f, g, np);
 #pragma unroll
-    for (int q = 0; q < QF; ++q) dst[(long long)q * m.nn + cx.c] = (ST)(f[q] - Store<ST, DIM>::bias(q));
+    for (int q = 0; q < QF; ++q) dst[(long long)plane_f<DIM>(q) * m.nn + cx.c] = (ST)(f[q] - Store<ST, DIM>::bias(q));
 #pragma unroll
-    for (int q = 0; q < QG; ++q) dst[(long long)(QF + q) * m.nn + cx.c] = (ST)g[q];
+    for (int q = 0; q < QG; ++q) dst[(long long)plane_g<DIM>(q) * m.nn + cx.c] = (ST)g[q];
   } else {
 #pragma unroll
     for (int q = 0; q < QF; ++q) fout[(long long)q * m.nn + cx.c] = f[q];
@@ -229,14 +230,14 @@ k_load_state(DevMesh m, NodeParams np, const double *__restrict__ fin, const dou
     for (int q = 0; q < QG; ++q) g[q] = gin[(long long)q * m.nn + c];
   }
 #pragma unroll
-  for (int q = 0; q < QF; ++q) pre[(long long)q * m.nn + c] = (ST)(f[q] - Store<ST, DIM>::bias(q));
+  for (int q = 0; q < QF; ++q) pre[(long long)plane_f<DIM>(q) * m.nn + c] = (ST)(f[q] - Store<ST, DIM>::bias(q));
 #pragma unroll
-  for (int q = 0; q < QG; ++q) pre[(long long)(QF + q) * m.nn + c] = (ST)g[q];
+  for (int q = 0; q < QG; ++q) pre[(long long)plane_g<DIM>(q) * m.nn + c] = (ST)g[q];
   collide_node(f, g, np);
 #pragma unroll
-  for (int q = 0; q < QF; ++q) post[(long long)q * m.nn + c] = (ST)(f[q] - Store<ST, DIM>::bias(q));
+  for (int q = 0; q < QF; ++q) post[(long long)plane_f<DIM>(q) * m.nn + c] = (ST)(f[q] - Store<ST, DIM>::bias(q));
 #pragma unroll
-  for (int q = 0; q < QG; ++q) post[(long long)(QF + q) * m.nn + c] = (ST)g[q];
+  for (int q = 0; q < QG; ++q) post[(long long)plane_g<DIM>(q) * m.nn + c] = (ST)g[q];
 }
 
 // storage-form buffer -> fp64 user arrays
@@ -247,9 +248,9 @@ k_export(DevMesh m, const ST *__restrict__ buf, double *__restrict__ fout, doubl
   const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= m.nn) return;
 #pragma unroll
-  for (int q = 0; q < QF; ++q) fout[(long long)q * m.nn + c] = (double)buf[(long long)q * m.nn + c] + Store<ST, DIM>::bias(q);
+  for (int q = 0; q < QF; ++q) fout[(long long)q * m.nn + c] = (double)buf[(long long)plane_f<DIM>(q) * m.nn + c] + Store<ST, DIM>::bias(q);
 #pragma unroll
-  for (int q = 0; q < QG; ++q) gout[(long long)q * m.nn + c] = (double)buf[(long long)(QF + q) * m.nn + c];
+  for (int q = 0; q < QG; ++q) gout[(long long)q * m.nn + c] = (double)buf[(long long)plane_g<DIM>(q) * m.nn + c];
 }
 
 template <int DIM, typename ST>
@@ -257,9 +258,9 @@ __device__ __forceinline__ void load_post_node(const DevMesh &m, const ST *__res
                                                double (&f)[Lat<DIM>::QF], double (&g)[Lat<DIM>::QG]) {
   constexpr int QF = Lat<DIM>::QF, QG = Lat<DIM>::QG;
 #pragma unroll
-  for (int q = 0; q < QF; ++q) f[q] = ldv(S + (long long)q * m.nn + c) + Store<ST, DIM>::bias(q);
+  for (int q = 0; q < QF; ++q) f[q] = ldv(S + (long long)plane_f<DIM>(q) * m.nn + c) + Store<ST, DIM>::bias(q);
 #pragma unroll
-  for (int q = 0; q < QG; ++q) g[q] = ldv(S + (long long)(QF + q) * m.nn + c);
+  for (int q = 0; q < QG; ++q) g[q] = ldv(S + (long long)plane_g<DIM>(q) * m.nn + c);
 }
 
 // macroscopic fields from the post-collision state

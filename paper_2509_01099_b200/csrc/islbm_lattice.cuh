@@ -65,6 +65,43 @@ ISLBM_HD constexpr int opposite(int q) {
   }
 }
 
+// Storage plane of flow population q / temperature population q inside a population buffer.  The public
+// arrays of include/islbm.h are [q][z][y][x] in direction order; INSIDE the workspace the planes are ordered
+// by the halo group the TMA-staged kernels load with one box:
+//   2-D: f0 g0 | f1 f3 g1 g3 | f2 f4 g2 g4 | f5 f6 f7 f8
+//   3-D: f0 g0 | f1 f2 g1 g2 | f3 f4 g3 g4 | f7..f10 | f5 f6 g5 g6 | f11..f14 | f15..f18
+template <int DIM>
+ISLBM_HD constexpr int plane_f(int q) {
+  if (DIM == 2) {
+    constexpr int t[9] = {0, 2, 6, 3, 7, 10, 11, 12, 13};
+    return t[q];
+  } else {
+    constexpr int t[19] = {0, 2, 3, 6, 7, 14, 15, 10, 11, 12, 13, 18, 19, 20, 21, 22, 23, 24, 25};
+    return t[q];
+  }
+}
+template <int DIM>
+ISLBM_HD constexpr int plane_g(int q) {
+  if (DIM == 2) {
+    constexpr int t[5] = {1, 4, 8, 5, 9};
+    return t[q];
+  } else {
+    constexpr int t[7] = {1, 4, 5, 8, 9, 16, 17};
+    return t[q];
+  }
+}
+
+// inverse of plane_f / plane_g: the population stored in plane p (flow q as q, temperature q as QF + q)
+template <int DIM>
+ISLBM_HD constexpr int pop_of_plane(int p) {
+  constexpr int QF = DIM == 2 ? 9 : 19, QG = DIM == 2 ? 5 : 7;
+  for (int q = 0; q < QF; ++q)
+    if (plane_f<DIM>(q) == p) return q;
+  for (int q = 0; q < QG; ++q)
+    if (plane_g<DIM>(q) == p) return QF + q;
+  return -1;
+}
+
 // lattice weights of the rest equilibrium (rho = 1, u = 0): M^-1 m_eq
 template <int DIM>
 ISLBM_HD constexpr double wflow(int q) {

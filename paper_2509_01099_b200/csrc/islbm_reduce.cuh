@@ -51,7 +51,7 @@ __device__ __forceinline__ double node_temperature(const DevMesh &m, const ST *_
   constexpr int QF = Lat<DIM>::QF, QG = Lat<DIM>::QG;
   double g[QG];
 #pragma unroll
-  for (int q = 0; q < QG; ++q) g[q] = ldv(S + (long long)(QF + q) * m.nn + c);
+  for (int q = 0; q < QG; ++q) g[q] = ldv(S + (long long)plane_g<DIM>(q) * m.nn + c);
   if constexpr (DIM == 2) return g[0] + g[1] + g[2] + g[3] + g[4];
   else return g[0] + ((g[1] + g[2]) + (g[3] + g[4]) + (g[5] + g[6]));
 }

@@ -3,15 +3,17 @@
 // "y-marching" design, the 2-D counterpart of islbm_tiled3.cuh:
 //   * a CTA owns a strip of TX nodes in x (one thread per x) and marches
 //     through a chunk of rows;
-//   * one elected thread streams, per row, one TMA box per population plane
-//     (cp.async.bulk.tensor.2d over the view (x, q*ny + y)) into a ring of
-//     shared-memory stages guarded by full/empty mbarriers; planes with e_x != 0
-//     (f1 f3 g1 g3 f5..f8) carry a 16-byte x-halo on each side, the others
-//     (f0 g0 f2 f4 g2 g4) none;
+//   * one elected thread streams, per row, FOUR TMA boxes
+//     (cp.async.bulk.tensor.3d over the view (x, y, plane); the storage planes
+//     are ordered so that a box covers consecutive planes, plane_f / plane_g)
+//     into a ring of shared-memory stages guarded by full/empty mbarriers;
+//     planes with e_x != 0 (f1 f3 g1 g3 | f5..f8) carry a 16-byte x-halo on each
+//     side, the others (f0 g0 | f2 f4 g2 g4) none;
 //   * consumers interpolate along x from shared memory; the y-direction of the
 //     separable interpolation is a 3-row combination kept
-//     in REGISTERS for the 8 populations with e_y != 0, so every post-collision
-//     value is staged once and there is no y-halo at all;
+//     in REGISTERS (three rotating register sets) for the 8 populations with
+//     e_y != 0, so every post-collision value is staged once and there is no
+//     y-halo at all;
 //   * the node collides once and stores its 14 values with coalesced stores.
 // DIR = +1 marches a chunk upwards, DIR = -1 downwards ("serpentine" tuning: odd
 // steps march downwards, so a step starts on the rows the previous step wrote
@@ -28,21 +30,25 @@ struct Tile2 {
   static constexpr int TX = TX_, STAGES = STAGES_;
   static constexpr int XH = 16 / (int)sizeof(ST);
   static constexpr int HX = TX + 2 * XH;
-  static constexpr int N_X = 8, N_C = 6;
-  static constexpr int B_X = HX * (int)sizeof(ST), B_C = TX * (int)sizeof(ST);
-  static constexpr int S_X = pad128(B_X), S_C = pad128(B_C);
-  static constexpr int OFF_X = 0, OFF_C = N_X * S_X;
-  static constexpr int STAGE_BYTES = OFF_C + N_C * S_C;
+  static constexpr int P_X = HX * (int)sizeof(ST), P_C = TX * (int)sizeof(ST);   // bytes of one plane row in a box
+  // groups of a stage, in storage-plane order (each starts 128-byte aligned):
+  //   emitted row y:      C2 = f0 g0, XR = f1 f3 g1 g3        y-stencil row (m):  C4 = f2 f4 g2 g4, XM = f5..f8
+  static constexpr int OFF_C2 = 0;
+  static constexpr int OFF_XR = pad128(OFF_C2 + 2 * P_C);
+  static constexpr int OFF_C4 = pad128(OFF_XR + 4 * P_X);
+  static constexpr int OFF_XM = pad128(OFF_C4 + 4 * P_C);
+  static constexpr int STAGE_BYTES = pad128(OFF_XM + 4 * P_X);
   static constexpr int WARPS = TX / 32;
-  static constexpr uint32_t Y_BYTES = 4u * B_X + 2u * B_C;   // planes of the emitted row
-  static constexpr uint32_t M_BYTES = 4u * B_X + 4u * B_C;   // planes of the y-stencil row
+  static constexpr uint32_t Y_BYTES = 2u * P_C + 4u * P_X;   // planes of the emitted row
+  static constexpr uint32_t M_BYTES = 4u * P_C + 4u * P_X;   // planes of the y-stencil row
   static constexpr int BAR_OFF = STAGES * STAGE_BYTES;
   static constexpr int W_OFF = BAR_OFF + 64;                 // y-weights of the chunk [sign][k][kMaxChunk]
   static constexpr size_t SMEM_BYTES = (size_t)W_OFF + 6 * kMaxChunk * 8 + 128;
 };
 
+// tensor maps over (x, y, plane): one per box shape
 struct Maps2 {
-  CUtensorMap x, c;
+  CUtensorMap c2, c4, x;
 };
 
 // yf = first emitted row of the chunk (its lowest row for DIR = +1, its highest for DIR = -1).
@@ -66,23 +72,40 @@ __device__ __forceinline__ void issue_stage2(int s, int yf, int ny, int x0, unsi
   uint64_t *bar = &full[st];
   const int xh = x0 - T::XH;
   if (yrow >= 0) {
-    tma_load_2d(sb + T::OFF_X + 0 * T::S_X, &mp.x, bar, xh, 1 * ny + yrow, pol);         // f1
-    tma_load_2d(sb + T::OFF_X + 1 * T::S_X, &mp.x, bar, xh, 3 * ny + yrow, pol);         // f3
-    tma_load_2d(sb + T::OFF_X + 2 * T::S_X, &mp.x, bar, xh, (9 + 1) * ny + yrow, pol);   // g1
-    tma_load_2d(sb + T::OFF_X + 3 * T::S_X, &mp.x, bar, xh, (9 + 3) * ny + yrow, pol);   // g3
-    tma_load_2d(sb + T::OFF_C + 0 * T::S_C, &mp.c, bar, x0, 0 * ny + yrow, pol);         // f0
-    tma_load_2d(sb + T::OFF_C + 1 * T::S_C, &mp.c, bar, x0, 9 * ny + yrow, pol);         // g0
+    tma_load_3d(sb + T::OFF_C2, &mp.c2, bar, x0, yrow, 0, pol);    // f0 g0
+    tma_load_3d(sb + T::OFF_XR, &mp.x, bar, xh, yrow, 2, pol);     // f1 f3 g1 g3
   }
   if (mrow >= 0) {
-#pragma unroll
-    for (int k = 0; k < 4; ++k)
-      tma_load_2d(sb + T::OFF_X + (4 + k) * T::S_X, &mp.x, bar, xh, (5 + k) * ny + mrow, pol);   // f5..f8
-    tma_load_2d(sb + T::OFF_C + 2 * T::S_C, &mp.c, bar, x0, 2 * ny + mrow, pol);         // f2
-    tma_load_2d(sb + T::OFF_C + 3 * T::S_C, &mp.c, bar, x0, 4 * ny + mrow, pol);         // f4
-    tma_load_2d(sb + T::OFF_C + 4 * T::S_C, &mp.c, bar, x0, (9 + 2) * ny + mrow, pol);   // g2
-    tma_load_2d(sb + T::OFF_C + 5 * T::S_C, &mp.c, bar, x0, (9 + 4) * ny + mrow, pol);   // g4
+    tma_load_3d(sb + T::OFF_C4, &mp.c4, bar, x0, mrow, 6, pol);    // f2 f4 g2 g4
+    tma_load_3d(sb + T::OFF_XM, &mp.x, bar, xh, mrow, 10, pol);    // f5..f8
   }
 }
+
+// x-interpolated values of one y-stencil row for the 8 populations with e_y != 0:
+//   index: 0 f2, 1 f4, 2 g2, 3 g4, 4 f5, 5 f6, 6 f7, 7 f8
+#define ISLBM_LOAD_M2(S)                                     \
+  do {                                                       \
+    S[0] = (double)PC4(0)[tx];               /* f2 */        \
+    S[1] = (double)PC4(1)[tx];               /* f4 */        \
+    S[2] = (double)PC4(2)[tx];               /* g2 */        \
+    S[3] = (double)PC4(3)[tx];               /* g4 */        \
+    S[4] = tap3(PXM(0) + o_x, 1, wx[1]);     /* f5 ( 1, 1) */ \
+    S[5] = tap3(PXM(1) + o_x, 1, wx[0]);     /* f6 (-1, 1) */ \
+    S[6] = tap3(PXM(2) + o_x, 1, wx[0]);     /* f7 (-1,-1) */ \
+    S[7] = tap3(PXM(3) + o_x, 1, wx[1]);     /* f8 ( 1,-1) */ \
+  } while (0)
+// y-direction of the separable interpolation; (P0,P1,P2) = stencil rows in ascending y
+#define ISLBM_YCOMB2(P0, P1, P2)                 \
+  do {                                           \
+    f[2] = comb3(wy[1], P0[0], P1[0], P2[0]);    \
+    f[4] = comb3(wy[0], P0[1], P1[1], P2[1]);    \
+    g[2] = comb3(wy[1], P0[2], P1[2], P2[2]);    \
+    g[4] = comb3(wy[0], P0[3], P1[3], P2[3]);    \
+    f[5] = comb3(wy[1], P0[4], P1[4], P2[4]);    \
+    f[6] = comb3(wy[1], P0[5], P1[5], P2[5]);    \
+    f[7] = comb3(wy[0], P0[6], P1[6], P2[6]);    \
+    f[8] = comb3(wy[0], P0[7], P1[7], P2[7]);    \
+  } while (0)
 
 template <typename ST, int TX, int STAGES, int MINB, int DIR>
 __global__ void __launch_bounds__(TX, MINB)
@@ -116,8 +139,9 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
   const uint64_t lpol = make_policy(load_policy);
   const uint64_t spol = make_policy(store_policy);
   if (threadIdx.x == 0) {
+    tma_prefetch_desc(&mp.c2);
+    tma_prefetch_desc(&mp.c4);
     tma_prefetch_desc(&mp.x);
-    tma_prefetch_desc(&mp.c);
     for (int s = 0; s < T::STAGES - 1 && s < nstage; ++s) issue_stage2<T, DIR>(s, yf, m.ny, x0, stage0, full, empty, mp, lpol);
   }
 
@@ -137,11 +161,10 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
 #pragma unroll
     for (int k = 0; k < 3; ++k) wx[s][k] = valid ? __ldg(wrow(m, 0, s, k) + x) : 0.0;
 
-  // x-interpolated values of the three y-stencil rows (A oldest, C newest in marching order) for the 8
-  // populations with e_y != 0:   index: 0 f2, 1 f4, 2 g2, 3 g4, 4 f5, 5 f6, 6 f7, 7 f8
-  double A[8], B[8], C[8];
-#pragma unroll
-  for (int i = 0; i < 8; ++i) A[i] = B[i] = C[i] = 0.0;
+  // three register sets hold the y-stencil rows; `newest` names the one written last, so the marching order
+  // (oldest first) is (newest+1, newest+2, newest) mod 3 and nothing is ever copied between sets
+  double S0[8], S1[8], S2[8];
+  int newest = 2;
 
 #pragma unroll 1
   for (int s = 0; s < nstage; ++s) {
@@ -151,24 +174,20 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
     const bool has_emit = s >= 2;
     const bool has_mov = s <= 2 || sbase(y, m.ny) != sbase(y - DIR, m.ny);
     const unsigned char *sb = stage0 + (size_t)st * T::STAGE_BYTES;
-    auto PX = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_X + k * T::S_X); };
-    auto PC = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_C + k * T::S_C); };
+    auto PC2 = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_C2 + k * T::P_C); };
+    auto PXR = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_XR + k * T::P_X); };
+    auto PC4 = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_C4 + k * T::P_C); };
+    auto PXM = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_XM + k * T::P_X); };
     if (threadIdx.x == 0 && s + T::STAGES - 1 < nstage)
       issue_stage2<T, DIR>(s + T::STAGES - 1, yf, m.ny, x0, stage0, full, empty, mp, lpol);
     __syncwarp();
     mbar_wait(&full[st], ph);
 
     if (has_mov) {
-#pragma unroll
-      for (int i = 0; i < 8; ++i) { A[i] = B[i]; B[i] = C[i]; }
-      C[0] = (double)PC(2)[tx];                      // f2
-      C[1] = (double)PC(3)[tx];                      // f4
-      C[2] = (double)PC(4)[tx];                      // g2
-      C[3] = (double)PC(5)[tx];                      // g4
-      C[4] = tap3(PX(4) + o_x, 1, wx[1]);            // f5 ( 1, 1)
-      C[5] = tap3(PX(5) + o_x, 1, wx[0]);            // f6 (-1, 1)
-      C[6] = tap3(PX(6) + o_x, 1, wx[0]);            // f7 (-1,-1)
-      C[7] = tap3(PX(7) + o_x, 1, wx[1]);            // f8 ( 1,-1)
+      newest = newest == 2 ? 0 : newest + 1;
+      if (newest == 0) ISLBM_LOAD_M2(S0);
+      else if (newest == 1) ISLBM_LOAD_M2(S1);
+      else ISLBM_LOAD_M2(S2);
     }
 
     if (has_emit) {
@@ -178,40 +197,35 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
 #pragma unroll
         for (int k = 0; k < 3; ++k) wy[sg][k] = wys[(sg * 3 + k) * kMaxChunk + (y - y0)];
       double f[9], g[5];
-      f[0] = (double)PC(0)[tx];
-      g[0] = (double)PC(1)[tx];
-      f[1] = tap3(PX(0) + o_x, 1, wx[1]);
-      f[3] = tap3(PX(1) + o_x, 1, wx[0]);
-      g[1] = tap3(PX(2) + o_x, 1, wx[1]);
-      g[3] = tap3(PX(3) + o_x, 1, wx[0]);
+      f[0] = (double)PC2(0)[tx];
+      g[0] = (double)PC2(1)[tx];
+      f[1] = tap3(PXR(0) + o_x, 1, wx[1]);
+      f[3] = tap3(PXR(1) + o_x, 1, wx[0]);
+      g[1] = tap3(PXR(2) + o_x, 1, wx[1]);
+      g[3] = tap3(PXR(3) + o_x, 1, wx[0]);
       __syncwarp();
       if ((threadIdx.x & 31) == 0) mbar_arrive(&empty[st]);
-      // stencil rows in ascending-y order are (A,B,C) when marching up and (C,B,A) when marching down
-      auto ycomb = [&](const double (&w)[3], int i) { return DIR > 0 ? comb3(w, A[i], B[i], C[i]) : comb3(w, C[i], B[i], A[i]); };
-      f[2] = ycomb(wy[1], 0);
-      f[4] = ycomb(wy[0], 1);
-      g[2] = ycomb(wy[1], 2);
-      g[4] = ycomb(wy[0], 3);
-      f[5] = ycomb(wy[1], 4);
-      f[6] = ycomb(wy[1], 5);
-      f[7] = ycomb(wy[0], 6);
-      f[8] = ycomb(wy[0], 7);
+      // ascending-y order of the stencil rows: the marching order when DIR = +1, its reverse when DIR = -1
+      if (DIR > 0) {
+        if (newest == 0) ISLBM_YCOMB2(S1, S2, S0);
+        else if (newest == 1) ISLBM_YCOMB2(S2, S0, S1);
+        else ISLBM_YCOMB2(S0, S1, S2);
+      } else {
+        if (newest == 0) ISLBM_YCOMB2(S0, S2, S1);
+        else if (newest == 1) ISLBM_YCOMB2(S1, S0, S2);
+        else ISLBM_YCOMB2(S2, S1, S0);
+      }
       const long long c = (long long)y * m.nx + x;
       wf.lo[1] = y == 0;
       wf.hi[1] = y == m.ny - 1;
       if (valid && (wall_x | wf.lo[1] | wf.hi[1])) {
         bb_fix_all_f<2>(f, wf, src, m.nn, c, std::make_integer_sequence<int, 8>{});
-        bb_fix_all_g<2>(g, wf, src + 9 * m.nn, m.nn, c, m, std::make_integer_sequence<int, 4>{});
+        bb_fix_all_g<2>(g, wf, src, m.nn, c, m, std::make_integer_sequence<int, 4>{});
       }
 #pragma unroll
       for (int q = 0; q < 9; ++q) f[q] += Store<ST, 2>::bias(q);
       collide_node(f, g, np);
-      if (valid) {
-#pragma unroll
-        for (int q = 0; q < 9; ++q) st_hint(dst + (long long)q * m.nn + c, (ST)(f[q] - Store<ST, 2>::bias(q)), spol);
-#pragma unroll
-        for (int q = 0; q < 5; ++q) st_hint(dst + (long long)(9 + q) * m.nn + c, (ST)g[q], spol);
-      }
+      if (valid) store_node<2>(dst + c, m.nn, f, g, spol, std::make_integer_sequence<int, 14>{});
     } else {
       __syncwarp();
       if ((threadIdx.x & 31) == 0) mbar_arrive(&empty[st]);
@@ -238,9 +252,12 @@ inline bool plan2_setup(Plan2 &p, const int *n, void *buf0, void *buf1, const Tu
   auto kern = k_step_ymarch<ST, T::TX, T::STAGES, CFG::MINB, 1>;
   auto kern_dn = k_step_ymarch<ST, T::TX, T::STAGES, CFG::MINB, -1>;
   void *bufs[2] = {buf0, buf1};
+  const long long dims[3] = {n[0], n[1], 14};
+  const int b_c2[3] = {T::TX, 1, 2}, b_c4[3] = {T::TX, 1, 4}, b_x[3] = {T::HX, 1, 4};
   for (int i = 0; i < 2; ++i)
-    if (!make_map(&p.maps[i].x, bufs[i], 2, (int)sizeof(ST), n[0], 1, 14LL * n[1], T::HX, 1, tn.l2promo) ||
-        !make_map(&p.maps[i].c, bufs[i], 2, (int)sizeof(ST), n[0], 1, 14LL * n[1], T::TX, 1, tn.l2promo))
+    if (!make_map(&p.maps[i].c2, bufs[i], (int)sizeof(ST), 3, dims, b_c2, tn.l2promo) ||
+        !make_map(&p.maps[i].c4, bufs[i], (int)sizeof(ST), 3, dims, b_c4, tn.l2promo) ||
+        !make_map(&p.maps[i].x, bufs[i], (int)sizeof(ST), 3, dims, b_x, tn.l2promo))
       return false;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM_BYTES) != cudaSuccess ||
       cudaFuncSetAttribute(kern_dn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM_BYTES) != cudaSuccess) {

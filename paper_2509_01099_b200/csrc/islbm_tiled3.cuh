@@ -3,17 +3,20 @@
 // "z-marching" design:
 //   * a CTA owns a TX x TY column of nodes (one thread per (x,y)) and marches
 //     through a chunk of z-slices;
-//   * one elected thread streams, per z-slice, one TMA box per population plane
-//     (cp.async.bulk.tensor.3d) into a ring of shared-memory stages guarded by
-//     full/empty mbarriers.  The box of a plane carries a halo only along the
-//     axes its velocity has a component on:
-//        XY (TX+2XH)x(TY+2): f7..f10          X (TX+2XH)xTY: f1 f2 g1 g2 f11..f14
-//        Y  TX x(TY+2): f3 f4 g3 g4 f15..f18   C  TX x TY: f0 g0 f5 f6 g5 g6
+//   * one elected thread streams, per z-slice, SEVEN TMA boxes
+//     (cp.async.bulk.tensor.4d over the view (x, y, z, plane)) into a ring of
+//     shared-memory stages guarded by full/empty mbarriers.  The storage planes
+//     are ordered so that each box covers the 2 or 4 consecutive planes that
+//     share a halo shape (plane_f / plane_g in islbm_lattice.cuh), and a plane
+//     carries a halo only along the axes its velocity has a component on:
+//        C  TX x TY: f0 g0 | f5 f6 g5 g6          X (TX+2XH)xTY: f1 f2 g1 g2 | f11..f14
+//        Y  TX x(TY+2): f3 f4 g3 g4 | f15..f18     XY (TX+2XH)x(TY+2): f7..f10
 //   * consumer threads interpolate in-plane (x, then y) from shared memory;
 //     the z-direction of the separable interpolation is a
 //     3-slice combination kept in REGISTERS: for the 12 populations with
-//     e_z != 0 each thread carries the in-plane-interpolated values of the two
-//     previous slices, so every post-collision value is staged once;
+//     e_z != 0 each thread carries the in-plane-interpolated values of three
+//     slices in three register sets whose roles rotate (no register shifting),
+//     so every post-collision value is staged once;
 //   * the node then collides once (islbm_lattice.cuh) and stores its 26
 //     post-collision values with coalesced stores.
 // Bounce-back / anti-bounce-back values (Eq. 21-23) are the node's own
@@ -41,24 +44,33 @@ struct Tile3 {
   // fault), so the x-halo is 16 bytes wide on each side: 2 nodes in fp64, 4 in fp32 storage
   static constexpr int XH = 16 / (int)sizeof(ST);
   static constexpr int HX = TX + 2 * XH, HY = TY + 2;
-  static constexpr int N_XY = 4, N_X = 8, N_Y = 8, N_C = 6;
-  static constexpr int B_XY = HX * HY * (int)sizeof(ST), B_X = HX * TY * (int)sizeof(ST);
-  static constexpr int B_Y = TX * HY * (int)sizeof(ST), B_C = TX * TY * (int)sizeof(ST);
-  static constexpr int S_XY = pad128(B_XY), S_X = pad128(B_X), S_Y = pad128(B_Y), S_C = pad128(B_C);
-  static constexpr int OFF_XY = 0, OFF_X = OFF_XY + N_XY * S_XY, OFF_Y = OFF_X + N_X * S_X, OFF_C = OFF_Y + N_Y * S_Y;
-  static constexpr int STAGE_BYTES = OFF_C + N_C * S_C;
+  // bytes of one plane inside a box of each shape
+  static constexpr int P_XY = HX * HY * (int)sizeof(ST), P_X = HX * TY * (int)sizeof(ST);
+  static constexpr int P_Y = TX * HY * (int)sizeof(ST), P_C = TX * TY * (int)sizeof(ST);
+  // groups of a stage, in storage-plane order (each starts 128-byte aligned):
+  //   emitted slice z:      C2 = f0 g0, XZ = f1 f2 g1 g2, YZ = f3 f4 g3 g4, XY = f7..f10
+  //   z-stencil slice (m):  C4 = f5 f6 g5 g6, XM = f11..f14, YM = f15..f18
+  static constexpr int OFF_C2 = 0;
+  static constexpr int OFF_XZ = pad128(OFF_C2 + 2 * P_C);
+  static constexpr int OFF_YZ = pad128(OFF_XZ + 4 * P_X);
+  static constexpr int OFF_XY = pad128(OFF_YZ + 4 * P_Y);
+  static constexpr int OFF_C4 = pad128(OFF_XY + 4 * P_XY);
+  static constexpr int OFF_XM = pad128(OFF_C4 + 4 * P_C);
+  static constexpr int OFF_YM = pad128(OFF_XM + 4 * P_X);
+  static constexpr int STAGE_BYTES = pad128(OFF_YM + 4 * P_Y);
   static constexpr int STAGES = 3;
   static constexpr int CONSUMER_WARPS = TX * TY / 32;
   static constexpr int THREADS = TX * TY;                // thread 0 doubles as the TMA producer
-  static constexpr uint32_t Z_BYTES = 4u * B_XY + 4u * B_X + 4u * B_Y + 2u * B_C;   // planes of the emitted slice
-  static constexpr uint32_t M_BYTES = 4u * B_X + 4u * B_Y + 4u * B_C;              // planes of the z-stencil slice
+  static constexpr uint32_t Z_BYTES = 2u * P_C + 4u * P_X + 4u * P_Y + 4u * P_XY;   // planes of the emitted slice
+  static constexpr uint32_t M_BYTES = 4u * P_C + 4u * P_X + 4u * P_Y;               // planes of the z-stencil slice
   static constexpr int BAR_OFF = STAGES * STAGE_BYTES;             // full[STAGES], empty[STAGES]
   static constexpr int W_OFF = BAR_OFF + 64;                        // marching-axis weights [sign][k][kMaxChunk]
   static constexpr size_t SMEM_BYTES = (size_t)W_OFF + 6 * kMaxChunk * 8 + 128;
 };
 
+// tensor maps over (x, y, z, plane): one per box shape
 struct Maps3 {
-  CUtensorMap xy, x, y, c;
+  CUtensorMap c2, c4, x, y, xy;
 };
 
 // ------------------------------ device helpers -----------------------------
@@ -96,18 +108,18 @@ __device__ __forceinline__ void bb_fix_f(double &v, const WallFlags &wf, const S
   if (EY == -1) cross |= wf.hi[1];
   if (DIM == 3 && EZ == 1) cross |= wf.lo[2];
   if (DIM == 3 && EZ == -1) cross |= wf.hi[2];
-  if (cross) v = ldv(src + (long long)opposite<DIM>(Q) * nn + c);
+  if (cross) v = ldv(src + (long long)plane_f<DIM>(opposite<DIM>(Q)) * nn + c);
 }
 // Eq. 22 (isothermal x-walls) and Eq. 23 (adiabatic walls)
 template <int DIM, int Q, typename ST>
-__device__ __forceinline__ void bb_fix_g(double &v, const WallFlags &wf, const ST *__restrict__ srcg, long long nn,
+__device__ __forceinline__ void bb_fix_g(double &v, const WallFlags &wf, const ST *__restrict__ src, long long nn,
                                          long long c, const DevMesh &m) {
   constexpr int EX = evel<DIM>(Q, 0), EY = evel<DIM>(Q, 1), EZ = evel<DIM>(Q, 2);
   constexpr int A = EX != 0 ? 0 : (EY != 0 ? 1 : 2);
   constexpr int S = EX + EY + EZ;
   const bool cross = S == 1 ? wf.lo[A] : wf.hi[A];
   if (cross) {
-    const double gb = ldv(srcg + (long long)opposite<DIM>(Q) * nn + c);
+    const double gb = ldv(src + (long long)plane_g<DIM>(opposite<DIM>(Q)) * nn + c);
     v = A == 0 ? -gb + m.omega_bc * (wf.lo[0] ? m.T_hot : m.T_cold) : gb;
   }
 }
@@ -117,9 +129,23 @@ __device__ __forceinline__ void bb_fix_all_f(double *f, const WallFlags &wf, con
   (bb_fix_f<DIM, Qs + 1>(f[Qs + 1], wf, src, nn, c), ...);
 }
 template <int DIM, typename ST, int... Qs>
-__device__ __forceinline__ void bb_fix_all_g(double *g, const WallFlags &wf, const ST *srcg, long long nn, long long c,
+__device__ __forceinline__ void bb_fix_all_g(double *g, const WallFlags &wf, const ST *src, long long nn, long long c,
                                              const DevMesh &m, std::integer_sequence<int, Qs...>) {
-  (bb_fix_g<DIM, Qs + 1>(g[Qs + 1], wf, srcg, nn, c, m), ...);
+  (bb_fix_g<DIM, Qs + 1>(g[Qs + 1], wf, src, nn, c, m), ...);
+}
+
+// store the node's populations plane by plane in storage order (one pointer walked by the plane pitch)
+template <int DIM, int P, typename ST>
+__device__ __forceinline__ void store_plane(ST *p, const double *f, const double *g, uint64_t spol) {
+  constexpr int QF = Lat<DIM>::QF;
+  constexpr int code = pop_of_plane<DIM>(P);
+  if constexpr (code < QF) st_hint(p, (ST)(f[code] - Store<ST, DIM>::bias(code)), spol);
+  else st_hint(p, (ST)g[code - QF], spol);
+}
+template <int DIM, typename ST, int... Ps>
+__device__ __forceinline__ void store_node(ST *p, long long nn, const double *f, const double *g, uint64_t spol,
+                                           std::integer_sequence<int, Ps...>) {
+  (store_plane<DIM, Ps>(p + (long long)Ps * nn, f, g, spol), ...);
 }
 
 __device__ __forceinline__ int sbase(int j, int n) { return min(max(j - 1, 0), n - 3); }
@@ -145,34 +171,53 @@ __device__ __forceinline__ void issue_stage3(int s, int z0, int nz, int x0, int 
   uint64_t *bar = &full[st];
   const int xh = x0 - T::XH, yh = y0 - 1;
   if (zslice >= 0) {
-#pragma unroll
-    for (int k = 0; k < 4; ++k)   // f7..f10
-      tma_load_3d(sb + T::OFF_XY + k * T::S_XY, &mp.xy, bar, xh, yh, (7 + k) * nz + zslice, pol);
-    tma_load_3d(sb + T::OFF_X + 0 * T::S_X, &mp.x, bar, xh, y0, 1 * nz + zslice, pol);          // f1
-    tma_load_3d(sb + T::OFF_X + 1 * T::S_X, &mp.x, bar, xh, y0, 2 * nz + zslice, pol);          // f2
-    tma_load_3d(sb + T::OFF_X + 2 * T::S_X, &mp.x, bar, xh, y0, (19 + 1) * nz + zslice, pol);   // g1
-    tma_load_3d(sb + T::OFF_X + 3 * T::S_X, &mp.x, bar, xh, y0, (19 + 2) * nz + zslice, pol);   // g2
-    tma_load_3d(sb + T::OFF_Y + 0 * T::S_Y, &mp.y, bar, x0, yh, 3 * nz + zslice, pol);          // f3
-    tma_load_3d(sb + T::OFF_Y + 1 * T::S_Y, &mp.y, bar, x0, yh, 4 * nz + zslice, pol);          // f4
-    tma_load_3d(sb + T::OFF_Y + 2 * T::S_Y, &mp.y, bar, x0, yh, (19 + 3) * nz + zslice, pol);   // g3
-    tma_load_3d(sb + T::OFF_Y + 3 * T::S_Y, &mp.y, bar, x0, yh, (19 + 4) * nz + zslice, pol);   // g4
-    tma_load_3d(sb + T::OFF_C + 0 * T::S_C, &mp.c, bar, x0, y0, 0 * nz + zslice, pol);          // f0
-    tma_load_3d(sb + T::OFF_C + 1 * T::S_C, &mp.c, bar, x0, y0, 19 * nz + zslice, pol);         // g0
+    tma_load_4d(sb + T::OFF_C2, &mp.c2, bar, x0, y0, zslice, 0, pol);     // f0 g0
+    tma_load_4d(sb + T::OFF_XZ, &mp.x, bar, xh, y0, zslice, 2, pol);      // f1 f2 g1 g2
+    tma_load_4d(sb + T::OFF_YZ, &mp.y, bar, x0, yh, zslice, 6, pol);      // f3 f4 g3 g4
+    tma_load_4d(sb + T::OFF_XY, &mp.xy, bar, xh, yh, zslice, 10, pol);    // f7..f10
   }
   if (mslice >= 0) {
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-      tma_load_3d(sb + T::OFF_X + (4 + k) * T::S_X, &mp.x, bar, xh, y0, (11 + k) * nz + mslice, pol);   // f11..f14
-      tma_load_3d(sb + T::OFF_Y + (4 + k) * T::S_Y, &mp.y, bar, x0, yh, (15 + k) * nz + mslice, pol);   // f15..f18
-    }
-    tma_load_3d(sb + T::OFF_C + 2 * T::S_C, &mp.c, bar, x0, y0, 5 * nz + mslice, pol);          // f5
-    tma_load_3d(sb + T::OFF_C + 3 * T::S_C, &mp.c, bar, x0, y0, 6 * nz + mslice, pol);          // f6
-    tma_load_3d(sb + T::OFF_C + 4 * T::S_C, &mp.c, bar, x0, y0, (19 + 5) * nz + mslice, pol);   // g5
-    tma_load_3d(sb + T::OFF_C + 5 * T::S_C, &mp.c, bar, x0, y0, (19 + 6) * nz + mslice, pol);   // g6
+    tma_load_4d(sb + T::OFF_C4, &mp.c4, bar, x0, y0, mslice, 14, pol);    // f5 f6 g5 g6
+    tma_load_4d(sb + T::OFF_XM, &mp.x, bar, xh, y0, mslice, 18, pol);     // f11..f14
+    tma_load_4d(sb + T::OFF_YM, &mp.y, bar, x0, yh, mslice, 22, pol);     // f15..f18
   }
 }
 
 // ------------------------------ the kernel --------------------------------
+// in-plane-interpolated values of one z-stencil slice for the 12 populations with e_z != 0:
+//   index: 0 f5, 1 f6, 2..5 f11..f14, 6..9 f15..f18, 10 g5, 11 g6
+#define ISLBM_LOAD_M3(S)                                        \
+  do {                                                          \
+    S[0] = (double)PC4(0)[o_c];                 /* f5 */        \
+    S[1] = (double)PC4(1)[o_c];                 /* f6 */        \
+    S[2] = tap3(PXM(0) + o_x, 1, wx[1]);        /* f11 ( 1,0, 1) */ \
+    S[3] = tap3(PXM(1) + o_x, 1, wx[0]);        /* f12 (-1,0, 1) */ \
+    S[4] = tap3(PXM(2) + o_x, 1, wx[1]);        /* f13 ( 1,0,-1) */ \
+    S[5] = tap3(PXM(3) + o_x, 1, wx[0]);        /* f14 (-1,0,-1) */ \
+    S[6] = tap3(PYM(0) + o_y, T::TX, wy[1]);    /* f15 (0, 1, 1) */ \
+    S[7] = tap3(PYM(1) + o_y, T::TX, wy[0]);    /* f16 (0,-1, 1) */ \
+    S[8] = tap3(PYM(2) + o_y, T::TX, wy[1]);    /* f17 (0, 1,-1) */ \
+    S[9] = tap3(PYM(3) + o_y, T::TX, wy[0]);    /* f18 (0,-1,-1) */ \
+    S[10] = (double)PC4(2)[o_c];                /* g5 */        \
+    S[11] = (double)PC4(3)[o_c];                /* g6 */        \
+  } while (0)
+// z-direction of the separable interpolation; (P0,P1,P2) = stencil slices in ascending z
+#define ISLBM_ZCOMB3(P0, P1, P2)                  \
+  do {                                            \
+    f[5] = comb3(wz[1], P0[0], P1[0], P2[0]);     \
+    f[6] = comb3(wz[0], P0[1], P1[1], P2[1]);     \
+    f[11] = comb3(wz[1], P0[2], P1[2], P2[2]);    \
+    f[12] = comb3(wz[1], P0[3], P1[3], P2[3]);    \
+    f[13] = comb3(wz[0], P0[4], P1[4], P2[4]);    \
+    f[14] = comb3(wz[0], P0[5], P1[5], P2[5]);    \
+    f[15] = comb3(wz[1], P0[6], P1[6], P2[6]);    \
+    f[16] = comb3(wz[1], P0[7], P1[7], P2[7]);    \
+    f[17] = comb3(wz[0], P0[8], P1[8], P2[8]);    \
+    f[18] = comb3(wz[0], P0[9], P1[9], P2[9]);    \
+    g[5] = comb3(wz[1], P0[10], P1[10], P2[10]);  \
+    g[6] = comb3(wz[0], P0[11], P1[11], P2[11]);  \
+  } while (0)
+
 template <typename ST, int TX, int TY>
 __global__ void __launch_bounds__(TX * TY, 1)
 k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const ST *__restrict__ src,
@@ -205,10 +250,11 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
   const uint64_t lpol = make_policy(load_policy);
   const uint64_t spol = make_policy(store_policy);
   if (threadIdx.x == 0) {
-    tma_prefetch_desc(&mp.xy);
+    tma_prefetch_desc(&mp.c2);
+    tma_prefetch_desc(&mp.c4);
     tma_prefetch_desc(&mp.x);
     tma_prefetch_desc(&mp.y);
-    tma_prefetch_desc(&mp.c);
+    tma_prefetch_desc(&mp.xy);
     for (int s = 0; s < T::STAGES - 1 && s < nstage; ++s)
       issue_stage3<T>(s, z0, m.nz, x0, y0, stage0, full, empty, mp, lpol);
   }
@@ -238,11 +284,10 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
   const long long plane = (long long)m.nx * m.ny;
   const long long cxy = (long long)y * m.nx + x;
 
-  // in-plane-interpolated values of the three z-stencil slices for the 12 populations with e_z != 0:
-  //   index: 0 f5, 1 f6, 2..5 f11..f14, 6..9 f15..f18, 10 g5, 11 g6
-  double A[12], B[12], C[12];
-#pragma unroll
-  for (int i = 0; i < 12; ++i) A[i] = B[i] = C[i] = 0.0;
+  // three register sets hold the z-stencil slices; `newest` names the one written last, so the ascending-z
+  // order is (newest+1, newest+2, newest) mod 3 and nothing is ever copied between sets
+  double S0[12], S1[12], S2[12];
+  int newest = 2;
 
 #pragma unroll 1
   for (int s = 0; s < nstage; ++s) {
@@ -252,30 +297,23 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
     const bool has_emit = s >= 2;
     const bool has_mov = s <= 2 || sbase(z, m.nz) != sbase(z - 1, m.nz);
     const unsigned char *sb = stage0 + (size_t)st * T::STAGE_BYTES;
-    auto XY = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_XY + k * T::S_XY); };
-    auto PX = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_X + k * T::S_X); };
-    auto PY = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_Y + k * T::S_Y); };
-    auto PC = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_C + k * T::S_C); };
+    auto PC2 = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_C2 + k * T::P_C); };
+    auto PXZ = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_XZ + k * T::P_X); };
+    auto PYZ = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_YZ + k * T::P_Y); };
+    auto PXY = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_XY + k * T::P_XY); };
+    auto PC4 = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_C4 + k * T::P_C); };
+    auto PXM = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_XM + k * T::P_X); };
+    auto PYM = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_YM + k * T::P_Y); };
     if (threadIdx.x == 0 && s + T::STAGES - 1 < nstage)
       issue_stage3<T>(s + T::STAGES - 1, z0, m.nz, x0, y0, stage0, full, empty, mp, lpol);
     __syncwarp();
     mbar_wait(&full[st], ph);
 
     if (has_mov) {
-#pragma unroll
-      for (int i = 0; i < 12; ++i) { A[i] = B[i]; B[i] = C[i]; }
-      C[0] = (double)PC(2)[o_c];                          // f5
-      C[1] = (double)PC(3)[o_c];                          // f6
-      C[2] = tap3(PX(4) + o_x, 1, wx[1]);                 // f11 ( 1,0, 1)
-      C[3] = tap3(PX(5) + o_x, 1, wx[0]);                 // f12 (-1,0, 1)
-      C[4] = tap3(PX(6) + o_x, 1, wx[1]);                 // f13 ( 1,0,-1)
-      C[5] = tap3(PX(7) + o_x, 1, wx[0]);                 // f14 (-1,0,-1)
-      C[6] = tap3(PY(4) + o_y, T::TX, wy[1]);             // f15 (0, 1, 1)
-      C[7] = tap3(PY(5) + o_y, T::TX, wy[0]);             // f16 (0,-1, 1)
-      C[8] = tap3(PY(6) + o_y, T::TX, wy[1]);             // f17 (0, 1,-1)
-      C[9] = tap3(PY(7) + o_y, T::TX, wy[0]);             // f18 (0,-1,-1)
-      C[10] = (double)PC(4)[o_c];                         // g5
-      C[11] = (double)PC(5)[o_c];                         // g6
+      newest = newest == 2 ? 0 : newest + 1;
+      if (newest == 0) ISLBM_LOAD_M3(S0);
+      else if (newest == 1) ISLBM_LOAD_M3(S1);
+      else ISLBM_LOAD_M3(S2);
     }
 
     if (has_emit) {
@@ -285,51 +323,37 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
 #pragma unroll
         for (int k = 0; k < 3; ++k) wz[sg][k] = wzs[(sg * 3 + k) * kMaxChunk + (s - 2)];
       double f[19], g[7];
-      f[0] = (double)PC(0)[o_c];
-      g[0] = (double)PC(1)[o_c];
-      f[1] = tap3(PX(0) + o_x, 1, wx[1]);
-      f[2] = tap3(PX(1) + o_x, 1, wx[0]);
-      g[1] = tap3(PX(2) + o_x, 1, wx[1]);
-      g[2] = tap3(PX(3) + o_x, 1, wx[0]);
-      f[3] = tap3(PY(0) + o_y, T::TX, wy[1]);
-      f[4] = tap3(PY(1) + o_y, T::TX, wy[0]);
-      g[3] = tap3(PY(2) + o_y, T::TX, wy[1]);
-      g[4] = tap3(PY(3) + o_y, T::TX, wy[0]);
-      f[7] = tap9(XY(0) + o_xy, T::HX, wx[1], wy[1]);
-      f[8] = tap9(XY(1) + o_xy, T::HX, wx[0], wy[1]);
-      f[9] = tap9(XY(2) + o_xy, T::HX, wx[1], wy[0]);
-      f[10] = tap9(XY(3) + o_xy, T::HX, wx[0], wy[0]);
+      f[0] = (double)PC2(0)[o_c];
+      g[0] = (double)PC2(1)[o_c];
+      f[1] = tap3(PXZ(0) + o_x, 1, wx[1]);
+      f[2] = tap3(PXZ(1) + o_x, 1, wx[0]);
+      g[1] = tap3(PXZ(2) + o_x, 1, wx[1]);
+      g[2] = tap3(PXZ(3) + o_x, 1, wx[0]);
+      f[3] = tap3(PYZ(0) + o_y, T::TX, wy[1]);
+      f[4] = tap3(PYZ(1) + o_y, T::TX, wy[0]);
+      g[3] = tap3(PYZ(2) + o_y, T::TX, wy[1]);
+      g[4] = tap3(PYZ(3) + o_y, T::TX, wy[0]);
+      f[7] = tap9(PXY(0) + o_xy, T::HX, wx[1], wy[1]);
+      f[8] = tap9(PXY(1) + o_xy, T::HX, wx[0], wy[1]);
+      f[9] = tap9(PXY(2) + o_xy, T::HX, wx[1], wy[0]);
+      f[10] = tap9(PXY(3) + o_xy, T::HX, wx[0], wy[0]);
       // all shared-memory reads of this stage are done: hand the slot back to the producer
       __syncwarp();
       if ((threadIdx.x & 31) == 0) mbar_arrive(&empty[st]);
-      f[5] = comb3(wz[1], A[0], B[0], C[0]);
-      f[6] = comb3(wz[0], A[1], B[1], C[1]);
-      f[11] = comb3(wz[1], A[2], B[2], C[2]);
-      f[12] = comb3(wz[1], A[3], B[3], C[3]);
-      f[13] = comb3(wz[0], A[4], B[4], C[4]);
-      f[14] = comb3(wz[0], A[5], B[5], C[5]);
-      f[15] = comb3(wz[1], A[6], B[6], C[6]);
-      f[16] = comb3(wz[1], A[7], B[7], C[7]);
-      f[17] = comb3(wz[0], A[8], B[8], C[8]);
-      f[18] = comb3(wz[0], A[9], B[9], C[9]);
-      g[5] = comb3(wz[1], A[10], B[10], C[10]);
-      g[6] = comb3(wz[0], A[11], B[11], C[11]);
+      if (newest == 0) ISLBM_ZCOMB3(S1, S2, S0);
+      else if (newest == 1) ISLBM_ZCOMB3(S2, S0, S1);
+      else ISLBM_ZCOMB3(S0, S1, S2);
       const long long c = (long long)z * plane + cxy;
       wf.lo[2] = z == 0;
       wf.hi[2] = z == m.nz - 1;
       if (valid && (wall_xy | wf.lo[2] | wf.hi[2])) {
         bb_fix_all_f<3>(f, wf, src, m.nn, c, std::make_integer_sequence<int, 18>{});
-        bb_fix_all_g<3>(g, wf, src + 19 * m.nn, m.nn, c, m, std::make_integer_sequence<int, 6>{});
+        bb_fix_all_g<3>(g, wf, src, m.nn, c, m, std::make_integer_sequence<int, 6>{});
       }
 #pragma unroll
       for (int q = 0; q < 19; ++q) f[q] += Store<ST, 3>::bias(q);
       collide_node(f, g, np);
-      if (valid) {
-#pragma unroll
-        for (int q = 0; q < 19; ++q) st_hint(dst + (long long)q * m.nn + c, (ST)(f[q] - Store<ST, 3>::bias(q)), spol);
-#pragma unroll
-        for (int q = 0; q < 7; ++q) st_hint(dst + (long long)(19 + q) * m.nn + c, (ST)g[q], spol);
-      }
+      if (valid) store_node<3>(dst + c, m.nn, f, g, spol, std::make_integer_sequence<int, 26>{});
     } else {
       __syncwarp();
       if ((threadIdx.x & 31) == 0) mbar_arrive(&empty[st]);
@@ -361,12 +385,15 @@ inline bool plan3_setup(Plan3 &p, const int *n, void *buf0, void *buf1, const Tu
   if (cc_major < 10 || (size_t)smem_optin < T::SMEM_BYTES) return no("tiled kernel: needs sm_100 and its shared memory");
   void *bufs[2] = {buf0, buf1};
   const int eb = (int)sizeof(ST);
-  const long long ns = 26LL * n[2];
+  const long long dims[4] = {n[0], n[1], n[2], 26};
+  const int b_c2[4] = {T::TX, T::TY, 1, 2}, b_c4[4] = {T::TX, T::TY, 1, 4}, b_x[4] = {T::HX, T::TY, 1, 4};
+  const int b_y[4] = {T::TX, T::HY, 1, 4}, b_xy[4] = {T::HX, T::HY, 1, 4};
   for (int i = 0; i < 2; ++i) {
-    if (!make_map(&p.maps[i].xy, bufs[i], 3, eb, n[0], n[1], ns, T::HX, T::HY, tn.l2promo) ||
-        !make_map(&p.maps[i].x, bufs[i], 3, eb, n[0], n[1], ns, T::HX, T::TY, tn.l2promo) ||
-        !make_map(&p.maps[i].y, bufs[i], 3, eb, n[0], n[1], ns, T::TX, T::HY, tn.l2promo) ||
-        !make_map(&p.maps[i].c, bufs[i], 3, eb, n[0], n[1], ns, T::TX, T::TY, tn.l2promo))
+    if (!make_map(&p.maps[i].c2, bufs[i], eb, 4, dims, b_c2, tn.l2promo) ||
+        !make_map(&p.maps[i].c4, bufs[i], eb, 4, dims, b_c4, tn.l2promo) ||
+        !make_map(&p.maps[i].x, bufs[i], eb, 4, dims, b_x, tn.l2promo) ||
+        !make_map(&p.maps[i].y, bufs[i], eb, 4, dims, b_y, tn.l2promo) ||
+        !make_map(&p.maps[i].xy, bufs[i], eb, 4, dims, b_xy, tn.l2promo))
       return no("cuTensorMapEncodeTiled failed");
   }
   if (cudaFuncSetAttribute(k_step_zmarch<ST, TX, TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM_BYTES) != cudaSuccess) {

@@ -59,6 +59,14 @@ __device__ __forceinline__ void tma_load_3d(void *dst, const CUtensorMap *map, u
       "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "l"(policy)
       : "memory");
 }
+__device__ __forceinline__ void tma_load_4d(void *dst, const CUtensorMap *map, uint64_t *bar, int c0, int c1, int c2, int c3,
+                                            uint64_t policy) {
+  asm volatile(
+      "cp.async.bulk.tensor.4d.shared::cluster.global.mbarrier::complete_tx::bytes.L2::cache_hint"
+      " [%0], [%1, {%3, %4, %5, %6}], [%2], %7;" ::"r"(smem_u32(dst)),
+      "l"(map), "r"(smem_u32(bar)), "r"(c0), "r"(c1), "r"(c2), "r"(c3), "l"(policy)
+      : "memory");
+}
 __device__ __forceinline__ void tma_load_2d(void *dst, const CUtensorMap *map, uint64_t *bar, int c0, int c1,
                                             uint64_t policy) {
   asm volatile(
@@ -104,26 +112,23 @@ inline CUtensorMapL2promotion promo_of(int k) {
   }
 }
 
-// Tensor view of one population buffer, zero fill outside the mesh in x and y:
-//   rank 3: (x, y, q*nz + z)  box (bx, by, 1);   rank 2: (x, q*ny + y)  box (bx, 1).
-// elem_bytes 8 (fp64) or 4 (fp32 storage).
-inline bool make_map(CUtensorMap *m, void *base, int rank, int elem_bytes, int nx, int ny, long long nslices, int bx, int by,
-                     int promo) {
+// Dense tensor view of one population buffer for TMA: dims[0] is x (fastest); the last dimension is the
+// storage plane; zero fill outside.  elem_bytes 8 (fp64) or 4 (fp32 storage).
+inline bool make_map(CUtensorMap *m, void *base, int elem_bytes, int rank, const long long *dims, const int *box, int promo) {
   EncodeTiledFn enc = get_encode_fn();
-  if (!enc) return false;
+  if (!enc || rank < 2 || rank > 5) return false;
   const CUtensorMapDataType dt = elem_bytes == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
-  cuuint32_t es[3] = {1, 1, 1};
-  if (rank == 3) {
-    cuuint64_t dims[3] = {(cuuint64_t)nx, (cuuint64_t)ny, (cuuint64_t)nslices};
-    cuuint64_t strides[2] = {(cuuint64_t)nx * elem_bytes, (cuuint64_t)nx * ny * elem_bytes};
-    cuuint32_t box[3] = {(cuuint32_t)bx, (cuuint32_t)by, 1};
-    return enc(m, dt, 3, base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
-               promo_of(promo), CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+  cuuint64_t gd[5], gs[4];
+  cuuint32_t bx[5], es[5];
+  unsigned long long pitch = (unsigned long long)elem_bytes;
+  for (int i = 0; i < rank; ++i) {
+    gd[i] = (cuuint64_t)dims[i];
+    bx[i] = (cuuint32_t)box[i];
+    es[i] = 1;
+    pitch *= (unsigned long long)dims[i];
+    if (i < rank - 1) gs[i] = (cuuint64_t)pitch;
   }
-  cuuint64_t dims[2] = {(cuuint64_t)nx, (cuuint64_t)nslices};
-  cuuint64_t strides[1] = {(cuuint64_t)nx * elem_bytes};
-  cuuint32_t box[2] = {(cuuint32_t)bx, (cuuint32_t)by};
-  return enc(m, dt, 2, base, dims, strides, box, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
+  return enc(m, dt, (cuuint32_t)rank, base, gd, gs, bx, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,
              promo_of(promo), CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 

@@ -15,21 +15,21 @@ namespace islbmk {
 template <int DIM, int Q, typename ST>
 __device__ __forceinline__ double shift_f(const DevMesh &m, const ST *__restrict__ src, const NodeCtx<DIM> &cx) {
   constexpr int EX = evel<DIM>(Q, 0), EY = evel<DIM>(Q, 1), EZ = evel<DIM>(Q, 2);
-  if (crosses<DIM, EX, EY, EZ>(cx)) return ldv(src + (long long)opposite<DIM>(Q) * m.nn + cx.c);
+  if (crosses<DIM, EX, EY, EZ>(cx)) return ldv(src + (long long)plane_f<DIM>(opposite<DIM>(Q)) * m.nn + cx.c);
   const long long off = (long long)EX + (long long)EY * m.nx + (long long)EZ * m.nx * m.ny;
-  return ldv(src + (long long)Q * m.nn + cx.c - off);
+  return ldv(src + (long long)plane_f<DIM>(Q) * m.nn + cx.c - off);
 }
 
 template <int DIM, int Q, typename ST>
-__device__ __forceinline__ double shift_g(const DevMesh &m, const ST *__restrict__ srcg, const NodeCtx<DIM> &cx) {
+__device__ __forceinline__ double shift_g(const DevMesh &m, const ST *__restrict__ src, const NodeCtx<DIM> &cx) {
   constexpr int EX = evel<DIM>(Q, 0), EY = evel<DIM>(Q, 1), EZ = evel<DIM>(Q, 2);
   if (crosses<DIM, EX, EY, EZ>(cx)) {
-    const double gb = ldv(srcg + (long long)opposite<DIM>(Q) * m.nn + cx.c);
+    const double gb = ldv(src + (long long)plane_g<DIM>(opposite<DIM>(Q)) * m.nn + cx.c);
     if (EX != 0) return -gb + m.omega_bc * (cx.lo[0] ? m.T_hot : m.T_cold);   // Eq. 22
     return gb;                                                                // Eq. 23
   }
   const long long off = (long long)EX + (long long)EY * m.nx + (long long)EZ * m.nx * m.ny;
-  return ldv(srcg + (long long)Q * m.nn + cx.c - off);
+  return ldv(src + (long long)plane_g<DIM>(Q) * m.nn + cx.c - off);
 }
 
 template <int DIM, typename ST, int... Qs>
@@ -38,9 +38,9 @@ __device__ __forceinline__ void shift_all_f(const DevMesh &m, const ST *src, con
   ((f[Qs] = shift_f<DIM, Qs>(m, src, cx)), ...);
 }
 template <int DIM, typename ST, int... Qs>
-__device__ __forceinline__ void shift_all_g(const DevMesh &m, const ST *srcg, const NodeCtx<DIM> &cx, double *g,
+__device__ __forceinline__ void shift_all_g(const DevMesh &m, const ST *src, const NodeCtx<DIM> &cx, double *g,
                                             std::integer_sequence<int, Qs...>) {
-  ((g[Qs] = shift_g<DIM, Qs>(m, srcg, cx)), ...);
+  ((g[Qs] = shift_g<DIM, Qs>(m, src, cx)), ...);
 }
 
 template <int DIM, typename ST>
@@ -59,14 +59,14 @@ k_step_shift(DevMesh m, NodeParams np, const ST *__restrict__ src, ST *__restric
   cx.lo[2] = DIM == 3 && iz == 0; cx.hi[2] = DIM == 3 && iz == m.nz - 1;
   double f[QF], g[QG];
   shift_all_f<DIM>(m, src, cx, f, std::make_integer_sequence<int, QF>{});
-  shift_all_g<DIM>(m, src + (long long)QF * m.nn, cx, g, std::make_integer_sequence<int, QG>{});
+  shift_all_g<DIM>(m, src, cx, g, std::make_integer_sequence<int, QG>{});
 #pragma unroll
   for (int q = 0; q < QF; ++q) f[q] += Store<ST, DIM>::bias(q);
   collide_node(f, g, np);
 #pragma unroll
-  for (int q = 0; q < QF; ++q) dst[(long long)q * m.nn + cx.c] = (ST)(f[q] - Store<ST, DIM>::bias(q));
+  for (int q = 0; q < QF; ++q) dst[(long long)plane_f<DIM>(q) * m.nn + cx.c] = (ST)(f[q] - Store<ST, DIM>::bias(q));
 #pragma unroll
-  for (int q = 0; q < QG; ++q) dst[(long long)(QF + q) * m.nn + cx.c] = (ST)g[q];
+  for (int q = 0; q < QG; ++q) dst[(long long)plane_g<DIM>(q) * m.nn + cx.c] = (ST)g[q];
 }
 
 }  // namespace islbmk

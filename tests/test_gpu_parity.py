@@ -78,7 +78,7 @@ def kernels_for(islbm, sim):
     return ks
 
 
-DEFAULT_TUNING = dict(chunk=0, l2promo=0, load_policy=0, store_policy=0, tx2d=0, serpentine=0)
+DEFAULT_TUNING = dict(chunk=0, l2promo=0, load_policy=0, store_policy=0, tx2d=0, serpentine=0, shape3d=0)
 
 
 def select(sim, k, tune):
