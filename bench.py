@@ -261,7 +261,7 @@ def main():
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD)
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"])
     ap.add_argument("--lbm-per-step", type=int, default=LBM_PER_STEP)
-    ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 generic, 2 tiled")
+    ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 generic, 2 TMA-staged, 3 uniform pure shift")
     ap.add_argument("--no-extras", action="store_true", help="skip the secondary workloads, e2e and CPU baseline")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
@@ -314,15 +314,19 @@ def main():
     torch.cuda.empty_cache()
 
     if not args.no_extras and rank == 0 and world == 1:
-        for nm, pr in (("c5_256cu_uniform", 0), ("c5_256cu", 1), ("c3_1024sq", 0), ("c3_1024sq_uniform", 0), ("c3_1024sq", 1),
-                       ("c2_512sq", 0), ("c4_128cu", 0)):
-            if nm == args.workload and pr == prec:
+        # secondary workloads: (name, precision, kernel); kernel 0 = the library's default for that mesh,
+        # 3 = the pure-shift kernel (the paper's "uniform" runs)
+        for nm, pr, kn in (("c5_256cu_uniform", 0, 0), ("c5_256cu_uniform", 0, 3), ("c5_256cu", 1, 0), ("c5_256cu_uniform", 1, 3),
+                           ("c3_1024sq", 0, 0), ("c3_1024sq_uniform", 0, 0), ("c3_1024sq_uniform", 0, 3), ("c3_1024sq", 1, 0),
+                           ("c2_512sq", 0, 0), ("c2_512sq_uniform", 0, 3), ("c4_128cu", 0, 0), ("c1_64sq", 0, 0)):
+            if nm == args.workload and pr == prec and kn == args.kernel:
                 continue
+            key = nm + ("_f32" if pr else "") + ("_shift" if kn == 3 else "")
             try:
                 lps = args.lbm_per_step if "256" in nm or "128" in nm else 200
-                s2, w2, r2 = measure_workload(islbm, inputs, nm, pr, max(3, args.steps // 2), 3, lps, args.kernel)
+                s2, w2, r2 = measure_workload(islbm, inputs, nm, pr, max(3, args.steps // 2), 3, lps, kn)
                 b2 = BYTES_PER_UPDATE[(w2.dim, pr)]
-                extras[nm + ("_f32" if pr else "")] = {
+                extras[key] = {
                     "mlups": r2["mlups"], "roofline_frac": b2 * w2.nodes / (r2["us_per_lbm_step"] * 1e-6) / 1e9 / peak,
                     "us_per_lbm_step": r2["us_per_lbm_step"], "wctpdt_s": r2["wctpdt_s"], "kernel": r2["kernel"],
                     "state_bytes_per_buffer": (w2.nodes * b2) // 2}
@@ -330,7 +334,18 @@ def main():
                 del s2
                 torch.cuda.empty_cache()
             except Exception as exc:   # a secondary workload must not take the headline down
-                extras[nm + ("_f32" if pr else "")] = {"error": str(exc)[:200]}
+                extras[key] = {"error": str(exc)[:200]}
+        # non-uniform / uniform ratios the paper reports: MLUPS ratio and WCTpDT ratio
+        ratios = {}
+        head = {"mlups": r["mlups"], "wctpdt_s": r["wctpdt_s"]}
+        for nu, un in ((args.workload if prec == 0 else None, "c5_256cu_uniform_shift"), ("c3_1024sq", "c3_1024sq_uniform_shift"),
+                       ("c2_512sq", "c2_512sq_uniform_shift")):
+            a = head if nu == args.workload else extras.get(nu)
+            b = extras.get(un)
+            if a and b and "mlups" in a and "mlups" in b:
+                ratios[nu] = {"mlups_nonuniform_over_uniform": a["mlups"] / b["mlups"],
+                              "wctpdt_nonuniform_over_uniform": a["wctpdt_s"] / b["wctpdt_s"]}
+        extras["ratios"] = ratios
         cores = oracle_threads()
         mlups_cpu, _, what, nodes_s = time_oracle(w, 3, 1, cores)
         cpu = {"value": mlups_cpu, "unit": "MLUPS", "cores": cores, "kind": "oracle",

@@ -48,7 +48,7 @@ __device__ __forceinline__ void block_reduce_store(double (&acc)[kRedSlots], dou
 
 template <int DIM, typename ST>
 __device__ __forceinline__ double node_temperature(const DevMesh &m, const ST *__restrict__ S, long long c) {
-  constexpr int QF = Lat<DIM>::QF, QG = Lat<DIM>::QG;
+  constexpr int QG = Lat<DIM>::QG;
   double g[QG];
 #pragma unroll
   for (int q = 0; q < QG; ++q) g[q] = ldv(S + (long long)plane_g<DIM>(q) * m.nn + c);

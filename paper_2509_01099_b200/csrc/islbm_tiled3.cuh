@@ -134,18 +134,21 @@ __device__ __forceinline__ void bb_fix_all_g(double *g, const WallFlags &wf, con
   (bb_fix_g<DIM, Qs + 1>(g[Qs + 1], wf, src, nn, c, m), ...);
 }
 
-// store the node's populations plane by plane in storage order (one pointer walked by the plane pitch)
+// store the node's populations plane by plane in storage order.  The pointer is walked by the plane pitch and made
+// opaque after each step, so that ptxas keeps two integer adds per plane instead of a 64-bit multiply-add
 template <int DIM, int P, typename ST>
-__device__ __forceinline__ void store_plane(ST *p, const double *f, const double *g, uint64_t spol) {
+__device__ __forceinline__ void store_plane(ST *&p, long long nn, const double *f, const double *g, uint64_t spol) {
   constexpr int QF = Lat<DIM>::QF;
   constexpr int code = pop_of_plane<DIM>(P);
   if constexpr (code < QF) st_hint(p, (ST)(f[code] - Store<ST, DIM>::bias(code)), spol);
   else st_hint(p, (ST)g[code - QF], spol);
+  p += nn;
+  asm volatile("" : "+l"(p));
 }
 template <int DIM, typename ST, int... Ps>
 __device__ __forceinline__ void store_node(ST *p, long long nn, const double *f, const double *g, uint64_t spol,
                                            std::integer_sequence<int, Ps...>) {
-  (store_plane<DIM, Ps>(p + (long long)Ps * nn, f, g, spol), ...);
+  (store_plane<DIM, Ps>(p, nn, f, g, spol), ...);
 }
 
 __device__ __forceinline__ int sbase(int j, int n) { return min(max(j - 1, 0), n - 3); }
