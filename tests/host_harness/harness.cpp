@@ -50,3 +50,11 @@ extern "C" void harness_tables(int dim, int *e, int *opp, double *w) {
     w[q] = dim == 2 ? islbmk::wflow<2>(q) : islbmk::wflow<3>(q);
   }
 }
+
+// storage-plane permutation of the workspace (plane_f / plane_g) and its inverse
+extern "C" void harness_planes(int dim, int *pf, int *pg, int *inv) {
+  const int qf = dim == 2 ? 9 : 19, qg = dim == 2 ? 5 : 7;
+  for (int q = 0; q < qf; ++q) pf[q] = dim == 2 ? islbmk::plane_f<2>(q) : islbmk::plane_f<3>(q);
+  for (int q = 0; q < qg; ++q) pg[q] = dim == 2 ? islbmk::plane_g<2>(q) : islbmk::plane_g<3>(q);
+  for (int p = 0; p < qf + qg; ++p) inv[p] = dim == 2 ? islbmk::pop_of_plane<2>(p) : islbmk::pop_of_plane<3>(p);
+}

@@ -42,6 +42,15 @@ def test_version_and_cubin_arch(binding):
     assert "sm_100a" in out
 
 
+def test_library_holds_tma_and_mbarrier_instructions(binding):
+    """The step kernels are TMA-staged: the sm_100a SASS must contain bulk-tensor loads and mbarrier waits."""
+    import subprocess
+    sass = subprocess.run(["cuobjdump", "-sass", binding.LIB_PATH], capture_output=True, text=True).stdout
+    assert "UTMALDG" in sass and "SYNCS" in sass
+    for kern in ("k_step_zmarch", "k_step_ymarch", "k_step_shift", "k_step_generic", "k_nusselt_partial"):
+        assert kern in sass, kern
+
+
 def test_workspace_bytes_scales_with_mesh(binding):
     w = inputs.workload("c1_64sq")
     b64 = binding.workspace_bytes(w.coords, w.delta, binding.F64)

@@ -78,3 +78,35 @@ def test_direction_tables_match_oracle(harness, dim):
     o.init(0, 0.0)
     f, _ = o.get_populations()
     assert np.allclose(wt, f[:, 0, 0, 0], atol=1e-16)
+
+
+@pytest.mark.parametrize("dim", [2, 3])
+def test_storage_planes_are_a_permutation_grouped_by_halo_shape(harness, dim):
+    """plane_f / plane_g (csrc/islbm_lattice.cuh) must be a bijection onto 0..Q-1 whose consecutive runs are
+    the groups one TMA box loads: same halo shape (which of e_x, e_y is non-zero) and same marching role
+    (e_march == 0: read at the emitted slice; != 0: read at the stencil slices)."""
+    w = inputs.custom_workload("t", dim, 4)
+    o = Oracle(w.coords, w.delta, w.Ra, w.Pr, w.Ma)
+    ef, eg = o.velocities()
+    qf, qg = o.qf, o.qg
+    ip = C.POINTER(C.c_int)
+    pf, pg, inv = np.empty(qf, np.int32), np.empty(qg, np.int32), np.empty(qf + qg, np.int32)
+    harness.harness_planes(dim, pf.ctypes.data_as(ip), pg.ctypes.data_as(ip), inv.ctypes.data_as(ip))
+    assert sorted(list(pf) + list(pg)) == list(range(qf + qg))
+    for q in range(qf):
+        assert inv[pf[q]] == q
+    for q in range(qg):
+        assert inv[pg[q]] == qf + q
+    march = dim - 1                      # y in 2-D, z in 3-D
+    inplane = [a for a in range(dim) if a != march]
+    vel = {int(pf[q]): ef[q] for q in range(qf)}
+    vel.update({int(pg[q]): eg[q] for q in range(qg)})
+    key = lambda p: (bool(vel[p][march] != 0), tuple(bool(vel[p][a] != 0) for a in inplane))
+    runs = []
+    for p in range(qf + qg):
+        if not runs or key(runs[-1][0]) != key(p):
+            runs.append([p])
+        else:
+            runs[-1].append(p)
+    assert [len(r) for r in runs] == ([2, 4, 4, 4] if dim == 2 else [2, 4, 4, 4, 4, 4, 4])
+    assert len({key(r[0]) for r in runs}) == len(runs)
