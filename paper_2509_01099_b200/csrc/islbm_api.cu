@@ -43,12 +43,15 @@ struct Carve {
   size_t buf[2], wtab, avgw, partial, red_out, snap, total;
 };
 
-Carve carve(long long nn, int q, size_t st_bytes, int npad) {
+// row pitch of the workspace planes: nx rounded up to 16 elements (see DevMesh::nxp)
+int row_pitch(int nx) { return (nx + 15) / 16 * 16; }
+
+Carve carve(long long nn, long long nnp, int q, size_t st_bytes, int npad) {
   Carve c{};
   size_t off = 0;
   for (int i = 0; i < 2; ++i) {
     c.buf[i] = off;
-    off = align_up(off + (size_t)q * (size_t)nn * st_bytes);
+    off = align_up(off + (size_t)q * (size_t)nnp * st_bytes);
   }
   c.wtab = off;    off = align_up(off + sizeof(double) * 18 * (size_t)npad);
   c.avgw = off;    off = align_up(off + sizeof(double) * 3 * (size_t)npad);
@@ -111,11 +114,11 @@ struct islbm {
 static void make_tiled_plan(islbm *h) {
   void *b0 = h->ws + h->cv.buf[0], *b1 = h->ws + h->cv.buf[1];
   if (h->dim == 2) {
-    if (h->precision == ISLBM_F64) plan2_create<double>(h->plan2, h->n, b0, b1, h->tune);
-    else plan2_create<float>(h->plan2, h->n, b0, b1, h->tune);
+    if (h->precision == ISLBM_F64) plan2_create<double>(h->plan2, h->n, h->dm.nxp, b0, b1, h->tune);
+    else plan2_create<float>(h->plan2, h->n, h->dm.nxp, b0, b1, h->tune);
   } else {
-    if (h->precision == ISLBM_F64) plan3_create<double>(h->plan3, h->n, b0, b1, h->tune);
-    else plan3_create<float>(h->plan3, h->n, b0, b1, h->tune);
+    if (h->precision == ISLBM_F64) plan3_create<double>(h->plan3, h->n, h->dm.nxp, b0, b1, h->tune);
+    else plan3_create<float>(h->plan3, h->n, h->dm.nxp, b0, b1, h->tune);
   }
 }
 
@@ -129,7 +132,8 @@ extern "C" int islbm_workspace_bytes(const islbm_mesh *mesh, int lattice, int pr
   long long nn = 1;
   for (int a = 0; a < mesh->dim; ++a) nn *= mesh->n[a];
   const int q = mesh->dim == 2 ? 14 : 26;
-  *bytes = carve(nn, q, precision == ISLBM_F64 ? 8 : 4, npad_of(mesh)).total;
+  const long long nnp = nn / mesh->n[0] * row_pitch(mesh->n[0]);
+  *bytes = carve(nn, nnp, q, precision == ISLBM_F64 ? 8 : 4, npad_of(mesh)).total;
   return ISLBM_OK;
 }
 
@@ -240,7 +244,9 @@ extern "C" int islbm_create(islbm_t **out, const islbm_mesh *mesh, int lattice, 
   if (rc) { delete h; return rc; }
   set_node_params(h);
   const int npad = npad_of(mesh);
-  h->cv = carve(h->nn, h->q, h->st_bytes, npad);
+  const int nxp = row_pitch(h->n[0]);
+  const long long nnp = h->nn / h->n[0] * nxp;
+  h->cv = carve(h->nn, nnp, h->q, h->st_bytes, npad);
   if (!dev_workspace) { delete h; return fail(ISLBM_ERR_WORKSPACE, "workspace is NULL"); }
   if ((uintptr_t)dev_workspace % kAlign) { delete h; return fail(ISLBM_ERR_WORKSPACE, "workspace must be 256-byte aligned"); }
   if (bytes < h->cv.total) {
@@ -264,6 +270,8 @@ extern "C" int islbm_create(islbm_t **out, const islbm_mesh *mesh, int lattice, 
   dm.nx = h->n[0]; dm.ny = h->n[1]; dm.nz = h->n[2];
   dm.npad = npad;
   dm.nn = h->nn;
+  dm.nxp = nxp;
+  dm.nnp = nnp;
   dm.wtab = (const double *)(h->ws + h->cv.wtab);
   dm.avgw = (const double *)(h->ws + h->cv.avgw);
   dm.omega_bc = h->prm.omega_bc;

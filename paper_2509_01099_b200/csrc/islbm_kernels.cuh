@@ -25,7 +25,10 @@ constexpr int kMaxQ = 26;
 struct DevMesh {
   int nx, ny, nz;
   int npad;              // pitch of the per-axis tables
-  long long nn;          // nx*ny*nz
+  long long nn;          // nx*ny*nz: nodes (and the pitch of the PUBLIC dense arrays)
+  int nxp;               // row pitch of the workspace planes in elements (nx rounded up to 16: TMA needs a
+                         // 16-byte pitch, and 128-byte row starts keep the stores coalesced); columns >= nx are padding
+  long long nnp;         // plane pitch of the workspace = nxp*ny*nz
   // interpolation weights, [axis 3][sign 2 (0: c=-1, 1: c=+1)][k 3][npad]; the
   // stencil of node j is {b, b+1, b+2}, b = clamp(j-1, 0, n-3) (A2)
   const double *wtab;
@@ -33,6 +36,13 @@ struct DevMesh {
   double omega_bc;       // Eq. 22 weight
   double T_hot, T_cold;  // x-lo / x-hi wall temperatures
 };
+
+// workspace (padded-row) index of dense node index c
+__device__ __forceinline__ long long sidx(const DevMesh &m, long long c) {
+  if (m.nxp == m.nx) return c;
+  const long long r = c / m.nx;
+  return r * m.nxp + (c - r * m.nx);
+}
 
 __device__ __forceinline__ const double *wrow(const DevMesh &m, int axis, int sign, int k) {
   return m.wtab + ((axis * 2 + sign) * 3 + k) * (long long)m.npad;
@@ -67,14 +77,16 @@ struct NodeCtx {
   int b[3];        // stencil base per axis
   bool lo[3], hi[3];
   double w[3][2][3];
-  long long c;     // linear node index
+  long long c;     // workspace index (padded rows)
+  long long cd;    // dense node index (public arrays)
 };
 
 template <int DIM>
 __device__ __forceinline__ void make_ctx(const DevMesh &m, int ix, int iy, int iz, NodeCtx<DIM> &cx) {
   const int n[3] = {m.nx, m.ny, m.nz};
   cx.i[0] = ix; cx.i[1] = iy; cx.i[2] = iz;
-  cx.c = ((long long)iz * m.ny + iy) * m.nx + ix;
+  cx.c = ((long long)iz * m.ny + iy) * m.nxp + ix;
+  cx.cd = ((long long)iz * m.ny + iy) * m.nx + ix;
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
     if (a < DIM) {
@@ -121,7 +133,7 @@ __device__ __forceinline__ double interp_plane(const DevMesh &m, const ST *__res
     double accy = 0.0;
 #pragma unroll
     for (int ky = 0; ky < CY; ++ky) {
-      const ST *row = plane + ((long long)(z0 + kz) * m.ny + (y0 + ky)) * m.nx + x0;
+      const ST *row = plane + ((long long)(z0 + kz) * m.ny + (y0 + ky)) * m.nxp + x0;
       double accx;
       if (CX == 3) {
         accx = cx.w[0][SX][0] * ldv(row);
@@ -142,8 +154,8 @@ __device__ __forceinline__ double interp_plane(const DevMesh &m, const ST *__res
 template <int DIM, int Q, typename ST>
 __device__ __forceinline__ double pull_f(const DevMesh &m, const ST *__restrict__ src, const NodeCtx<DIM> &cx) {
   constexpr int EX = evel<DIM>(Q, 0), EY = evel<DIM>(Q, 1), EZ = evel<DIM>(Q, 2);
-  if (crosses<DIM, EX, EY, EZ>(cx)) return ldv(src + (long long)plane_f<DIM>(opposite<DIM>(Q)) * m.nn + cx.c);
-  return interp_plane<DIM, EX, EY, EZ>(m, src + (long long)plane_f<DIM>(Q) * m.nn, cx);
+  if (crosses<DIM, EX, EY, EZ>(cx)) return ldv(src + (long long)plane_f<DIM>(opposite<DIM>(Q)) * m.nnp + cx.c);
+  return interp_plane<DIM, EX, EY, EZ>(m, src + (long long)plane_f<DIM>(Q) * m.nnp, cx);
 }
 
 // Temperature population Q: interpolation; anti-bounce-back on the isothermal
@@ -152,11 +164,11 @@ template <int DIM, int Q, typename ST>
 __device__ __forceinline__ double pull_g(const DevMesh &m, const ST *__restrict__ src, const NodeCtx<DIM> &cx) {
   constexpr int EX = evel<DIM>(Q, 0), EY = evel<DIM>(Q, 1), EZ = evel<DIM>(Q, 2);
   if (crosses<DIM, EX, EY, EZ>(cx)) {
-    const double gb = ldv(src + (long long)plane_g<DIM>(opposite<DIM>(Q)) * m.nn + cx.c);
+    const double gb = ldv(src + (long long)plane_g<DIM>(opposite<DIM>(Q)) * m.nnp + cx.c);
     if (EX != 0) return -gb + m.omega_bc * (cx.lo[0] ? m.T_hot : m.T_cold);
     return gb;
   }
-  return interp_plane<DIM, EX, EY, EZ>(m, src + (long long)plane_g<DIM>(Q) * m.nn, cx);
+  return interp_plane<DIM, EX, EY, EZ>(m, src + (long long)plane_g<DIM>(Q) * m.nnp, cx);
 }
 
 template <int DIM, typename ST, int... Qs>
@@ -194,14 +206,14 @@ k_step_generic(DevMesh m, NodeParams np, const ST *__restrict__ src, ST *__restr
   if (COLLIDE) {
     collide_node(f, g, np);
 #pragma unroll
-    for (int q = 0; q < QF; ++q) dst[(long long)plane_f<DIM>(q) * m.nn + cx.c] = (ST)(f[q] - Store<ST, DIM>::bias(q));
+    for (int q = 0; q < QF; ++q) dst[(long long)plane_f<DIM>(q) * m.nnp + cx.c] = (ST)(f[q] - Store<ST, DIM>::bias(q));
 #pragma unroll
-    for (int q = 0; q < QG; ++q) dst[(long long)plane_g<DIM>(q) * m.nn + cx.c] = (ST)g[q];
+    for (int q = 0; q < QG; ++q) dst[(long long)plane_g<DIM>(q) * m.nnp + cx.c] = (ST)g[q];
   } else {
 #pragma unroll
-    for (int q = 0; q < QF; ++q) fout[(long long)q * m.nn + cx.c] = f[q];
+    for (int q = 0; q < QF; ++q) fout[(long long)q * m.nn + cx.cd] = f[q];
 #pragma unroll
-    for (int q = 0; q < QG; ++q) gout[(long long)q * m.nn + cx.c] = g[q];
+    for (int q = 0; q < QG; ++q) gout[(long long)q * m.nn + cx.cd] = g[q];
   }
 }
 
@@ -229,15 +241,16 @@ k_load_state(DevMesh m, NodeParams np, const double *__restrict__ fin, const dou
 #pragma unroll
     for (int q = 0; q < QG; ++q) g[q] = gin[(long long)q * m.nn + c];
   }
+  const long long cs = sidx(m, c);
 #pragma unroll
-  for (int q = 0; q < QF; ++q) pre[(long long)plane_f<DIM>(q) * m.nn + c] = (ST)(f[q] - Store<ST, DIM>::bias(q));
+  for (int q = 0; q < QF; ++q) pre[(long long)plane_f<DIM>(q) * m.nnp + cs] = (ST)(f[q] - Store<ST, DIM>::bias(q));
 #pragma unroll
-  for (int q = 0; q < QG; ++q) pre[(long long)plane_g<DIM>(q) * m.nn + c] = (ST)g[q];
+  for (int q = 0; q < QG; ++q) pre[(long long)plane_g<DIM>(q) * m.nnp + cs] = (ST)g[q];
   collide_node(f, g, np);
 #pragma unroll
-  for (int q = 0; q < QF; ++q) post[(long long)plane_f<DIM>(q) * m.nn + c] = (ST)(f[q] - Store<ST, DIM>::bias(q));
+  for (int q = 0; q < QF; ++q) post[(long long)plane_f<DIM>(q) * m.nnp + cs] = (ST)(f[q] - Store<ST, DIM>::bias(q));
 #pragma unroll
-  for (int q = 0; q < QG; ++q) post[(long long)plane_g<DIM>(q) * m.nn + c] = (ST)g[q];
+  for (int q = 0; q < QG; ++q) post[(long long)plane_g<DIM>(q) * m.nnp + cs] = (ST)g[q];
 }
 
 // storage-form buffer -> fp64 user arrays
@@ -247,20 +260,21 @@ k_export(DevMesh m, const ST *__restrict__ buf, double *__restrict__ fout, doubl
   constexpr int QF = Lat<DIM>::QF, QG = Lat<DIM>::QG;
   const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= m.nn) return;
+  const long long cs = sidx(m, c);
 #pragma unroll
-  for (int q = 0; q < QF; ++q) fout[(long long)q * m.nn + c] = (double)buf[(long long)plane_f<DIM>(q) * m.nn + c] + Store<ST, DIM>::bias(q);
+  for (int q = 0; q < QF; ++q) fout[(long long)q * m.nn + c] = (double)buf[(long long)plane_f<DIM>(q) * m.nnp + cs] + Store<ST, DIM>::bias(q);
 #pragma unroll
-  for (int q = 0; q < QG; ++q) gout[(long long)q * m.nn + c] = (double)buf[(long long)plane_g<DIM>(q) * m.nn + c];
+  for (int q = 0; q < QG; ++q) gout[(long long)q * m.nn + c] = (double)buf[(long long)plane_g<DIM>(q) * m.nnp + cs];
 }
 
 template <int DIM, typename ST>
-__device__ __forceinline__ void load_post_node(const DevMesh &m, const ST *__restrict__ S, long long c,
+__device__ __forceinline__ void load_post_node(const DevMesh &m, const ST *__restrict__ S, long long c /* workspace index */,
                                                double (&f)[Lat<DIM>::QF], double (&g)[Lat<DIM>::QG]) {
   constexpr int QF = Lat<DIM>::QF, QG = Lat<DIM>::QG;
 #pragma unroll
-  for (int q = 0; q < QF; ++q) f[q] = ldv(S + (long long)plane_f<DIM>(q) * m.nn + c) + Store<ST, DIM>::bias(q);
+  for (int q = 0; q < QF; ++q) f[q] = ldv(S + (long long)plane_f<DIM>(q) * m.nnp + c) + Store<ST, DIM>::bias(q);
 #pragma unroll
-  for (int q = 0; q < QG; ++q) g[q] = ldv(S + (long long)plane_g<DIM>(q) * m.nn + c);
+  for (int q = 0; q < QG; ++q) g[q] = ldv(S + (long long)plane_g<DIM>(q) * m.nnp + c);
 }
 
 // macroscopic fields from the post-collision state
@@ -270,7 +284,7 @@ k_fields(DevMesh m, NodeParams np, const ST *__restrict__ S, double *rho, double
   const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
   if (c >= m.nn) return;
   double f[Lat<DIM>::QF], g[Lat<DIM>::QG];
-  load_post_node<DIM>(m, S, c, f, g);
+  load_post_node<DIM>(m, S, sidx(m, c), f, g);
   double r, uu, vv, ww, tt;
   fields_from_post(f, g, np, r, uu, vv, ww, tt);
   if (rho) rho[c] = r;

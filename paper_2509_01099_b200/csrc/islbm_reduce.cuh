@@ -51,7 +51,7 @@ __device__ __forceinline__ double node_temperature(const DevMesh &m, const ST *_
   constexpr int QG = Lat<DIM>::QG;
   double g[QG];
 #pragma unroll
-  for (int q = 0; q < QG; ++q) g[q] = ldv(S + (long long)plane_g<DIM>(q) * m.nn + c);
+  for (int q = 0; q < QG; ++q) g[q] = ldv(S + (long long)plane_g<DIM>(q) * m.nnp + c);
   if constexpr (DIM == 2) return g[0] + g[1] + g[2] + g[3] + g[4];
   else return g[0] + ((g[1] + g[2]) + (g[3] + g[4]) + (g[5] + g[6]));
 }
@@ -68,7 +68,8 @@ k_nusselt_partial(DevMesh m, NodeParams np, DiagParams dp, const ST *__restrict_
     const long long r = c / m.nx;
     const int iy = (int)(r % m.ny), iz = (int)(r / m.ny);
     double f[Lat<DIM>::QF], g[Lat<DIM>::QG];
-    load_post_node<DIM>(m, S, c, f, g);
+    const long long cs = (long long)r * m.nxp + ix;
+    load_post_node<DIM>(m, S, cs, f, g);
     double rho, u, v, w, T;
     fields_from_post(f, g, np, rho, u, v, w, T);
     const double wa = __ldg(m.avgw + m.npad + iy) * (DIM == 3 ? __ldg(m.avgw + 2 * m.npad + iz) : 1.0);
@@ -78,11 +79,11 @@ k_nusselt_partial(DevMesh m, NodeParams np, DiagParams dp, const ST *__restrict_
     acc[3] += wv * sp2;
     acc[4] += wv * u * (T - dp.T0);
     if (ix == 0) {
-      const double T1 = node_temperature<DIM>(m, S, c + 1);
+      const double T1 = node_temperature<DIM>(m, S, cs + 1);
       acc[0] += wa * wall_derivative(dp.q_lo, m.T_hot, T, T1);
     }
     if (ix == m.nx - 1) {
-      const double T1 = node_temperature<DIM>(m, S, c - 1);
+      const double T1 = node_temperature<DIM>(m, S, cs - 1);
       acc[1] += wa * (-wall_derivative(dp.q_hi, m.T_cold, T, T1));
     }
   }
@@ -109,7 +110,7 @@ k_residual_partial(DevMesh m, NodeParams np, const ST *__restrict__ S, double *_
   const long long stride = (long long)gridDim.x * kRedThreads;
   for (long long c = (long long)blockIdx.x * kRedThreads + threadIdx.x; c < m.nn; c += stride) {
     double f[Lat<DIM>::QF], g[Lat<DIM>::QG];
-    load_post_node<DIM>(m, S, c, f, g);
+    load_post_node<DIM>(m, S, sidx(m, c), f, g);
     double rho, u, v, w, T;
     fields_from_post(f, g, np, rho, u, v, w, T);
     const double pu = snap[c], pv = snap[m.nn + c], pw = snap[2 * m.nn + c], pT = snap[3 * m.nn + c];

@@ -215,17 +215,17 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
         else if (newest == 1) ISLBM_YCOMB2(S1, S0, S2);
         else ISLBM_YCOMB2(S2, S1, S0);
       }
-      const long long c = (long long)y * m.nx + x;
+      const long long c = (long long)y * m.nxp + x;
       wf.lo[1] = y == 0;
       wf.hi[1] = y == m.ny - 1;
       if (valid && (wall_x | wf.lo[1] | wf.hi[1])) {
-        bb_fix_all_f<2>(f, wf, src, m.nn, c, std::make_integer_sequence<int, 8>{});
-        bb_fix_all_g<2>(g, wf, src, m.nn, c, m, std::make_integer_sequence<int, 4>{});
+        bb_fix_all_f<2>(f, wf, src, m.nnp, c, std::make_integer_sequence<int, 8>{});
+        bb_fix_all_g<2>(g, wf, src, m.nnp, c, m, std::make_integer_sequence<int, 4>{});
       }
 #pragma unroll
       for (int q = 0; q < 9; ++q) f[q] += Store<ST, 2>::bias(q);
       collide_node(f, g, np);
-      if (valid) store_node<2>(dst + c, m.nn, f, g, spol, std::make_integer_sequence<int, 14>{});
+      if (valid) store_node<2>(dst + c, m.nnp, f, g, spol, std::make_integer_sequence<int, 14>{});
     } else {
       __syncwarp();
       if ((threadIdx.x & 31) == 0) mbar_arrive(&empty[st]);
@@ -247,7 +247,7 @@ template <typename ST> struct Cfg2a { using T = Tile2<ST, 128, 3>; static conste
 template <typename ST> struct Cfg2b { using T = Tile2<ST, 224, 3>; static constexpr int MINB = 2; };
 
 template <typename ST, typename CFG>
-inline bool plan2_setup(Plan2 &p, const int *n, void *buf0, void *buf1, const Tuning &tn) {
+inline bool plan2_setup(Plan2 &p, const int *n, int nxp, void *buf0, void *buf1, const Tuning &tn) {
   using T = typename CFG::T;
   auto kern = k_step_ymarch<ST, T::TX, T::STAGES, CFG::MINB, 1>;
   auto kern_dn = k_step_ymarch<ST, T::TX, T::STAGES, CFG::MINB, -1>;
@@ -255,9 +255,9 @@ inline bool plan2_setup(Plan2 &p, const int *n, void *buf0, void *buf1, const Tu
   const long long dims[3] = {n[0], n[1], 14};
   const int b_c2[3] = {T::TX, 1, 2}, b_c4[3] = {T::TX, 1, 4}, b_x[3] = {T::HX, 1, 4};
   for (int i = 0; i < 2; ++i)
-    if (!make_map(&p.maps[i].c2, bufs[i], (int)sizeof(ST), 3, dims, b_c2, tn.l2promo) ||
-        !make_map(&p.maps[i].c4, bufs[i], (int)sizeof(ST), 3, dims, b_c4, tn.l2promo) ||
-        !make_map(&p.maps[i].x, bufs[i], (int)sizeof(ST), 3, dims, b_x, tn.l2promo))
+    if (!make_map(&p.maps[i].c2, bufs[i], (int)sizeof(ST), 3, dims, b_c2, tn.l2promo, nxp) ||
+        !make_map(&p.maps[i].c4, bufs[i], (int)sizeof(ST), 3, dims, b_c4, tn.l2promo, nxp) ||
+        !make_map(&p.maps[i].x, bufs[i], (int)sizeof(ST), 3, dims, b_x, tn.l2promo, nxp))
       return false;
   if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM_BYTES) != cudaSuccess ||
       cudaFuncSetAttribute(kern_dn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM_BYTES) != cudaSuccess) {
@@ -289,17 +289,17 @@ inline bool plan2_setup(Plan2 &p, const int *n, void *buf0, void *buf1, const Tu
 }
 
 template <typename ST>
-inline bool plan2_create(Plan2 &p, const int *n, void *buf0, void *buf1, const Tuning &tn) {
+inline bool plan2_create(Plan2 &p, const int *n, int nxp, void *buf0, void *buf1, const Tuning &tn) {
   p.available = false;
   auto no = [&](const char *why) { snprintf(p.why_not, sizeof p.why_not, "%s", why); return false; };
   if (n[0] < 3 || n[1] < 3) return no("tiled kernel: n >= 3");
-  if (n[0] % (16 / (int)sizeof(ST))) return no("tiled kernel: TMA needs a 16-byte row pitch");
+  if ((nxp * (int)sizeof(ST)) % 16) return no("tiled kernel: TMA needs a 16-byte row pitch");
   int dev = 0, cc_major = 0;
   if (cudaGetDevice(&dev) != cudaSuccess) return no("no device");
   cudaDeviceGetAttribute(&cc_major, cudaDevAttrComputeCapabilityMajor, dev);
   if (cc_major < 10) return no("tiled kernel: needs sm_100");
   const int tx = tn.tx2d ? tn.tx2d : 128;   // a TMA box is at most 256 elements wide: TX + 2*XH <= 256
-  const bool ok = tx == 224 ? plan2_setup<ST, Cfg2b<ST>>(p, n, buf0, buf1, tn) : plan2_setup<ST, Cfg2a<ST>>(p, n, buf0, buf1, tn);
+  const bool ok = tx == 224 ? plan2_setup<ST, Cfg2b<ST>>(p, n, nxp, buf0, buf1, tn) : plan2_setup<ST, Cfg2a<ST>>(p, n, nxp, buf0, buf1, tn);
   if (!ok) return no("tiled kernel: tensor map / attribute setup failed");
   p.available = true;
   return true;

@@ -232,7 +232,9 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
   uint64_t *empty = full + T::STAGES;
   double *wzs = reinterpret_cast<double *>(smem_raw + T::W_OFF);
 
-  const int x0 = blockIdx.x * T::TX, y0 = blockIdx.y * T::TY;
+  // the last y-tile is pulled back inside the mesh (it recomputes a few rows of its neighbour, bit-identically),
+  // so that the shifted wall stencil of row ny-1 never leaves the box
+  const int x0 = blockIdx.x * T::TX, y0 = min((int)blockIdx.y * T::TY, max(m.ny - T::TY, 0));
   const int z0 = blockIdx.z * zchunk, z1 = min(z0 + zchunk, m.nz);
   const int nstage = 2 + (z1 - z0);
   for (int i = threadIdx.x; i < 6 * (z1 - z0); i += T::THREADS) {
@@ -284,8 +286,8 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
       wx[s][k] = valid ? __ldg(wrow(m, 0, s, k) + x) : 0.0;
       wy[s][k] = valid ? __ldg(wrow(m, 1, s, k) + y) : 0.0;
     }
-  const long long plane = (long long)m.nx * m.ny;
-  const long long cxy = (long long)y * m.nx + x;
+  const long long plane = (long long)m.nxp * m.ny;
+  const long long cxy = (long long)y * m.nxp + x;
 
   // three register sets hold the z-stencil slices; `newest` names the one written last, so the ascending-z
   // order is (newest+1, newest+2, newest) mod 3 and nothing is ever copied between sets
@@ -350,13 +352,13 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
       wf.lo[2] = z == 0;
       wf.hi[2] = z == m.nz - 1;
       if (valid && (wall_xy | wf.lo[2] | wf.hi[2])) {
-        bb_fix_all_f<3>(f, wf, src, m.nn, c, std::make_integer_sequence<int, 18>{});
-        bb_fix_all_g<3>(g, wf, src, m.nn, c, m, std::make_integer_sequence<int, 6>{});
+        bb_fix_all_f<3>(f, wf, src, m.nnp, c, std::make_integer_sequence<int, 18>{});
+        bb_fix_all_g<3>(g, wf, src, m.nnp, c, m, std::make_integer_sequence<int, 6>{});
       }
 #pragma unroll
       for (int q = 0; q < 19; ++q) f[q] += Store<ST, 3>::bias(q);
       collide_node(f, g, np);
-      if (valid) store_node<3>(dst + c, m.nn, f, g, spol, std::make_integer_sequence<int, 26>{});
+      if (valid) store_node<3>(dst + c, m.nnp, f, g, spol, std::make_integer_sequence<int, 26>{});
     } else {
       __syncwarp();
       if ((threadIdx.x & 31) == 0) mbar_arrive(&empty[st]);
@@ -374,13 +376,12 @@ struct Plan3 {
 };
 
 template <typename ST, int TX, int TY>
-inline bool plan3_setup(Plan3 &p, const int *n, void *buf0, void *buf1, const Tuning &tn) {
+inline bool plan3_setup(Plan3 &p, const int *n, int nxp, void *buf0, void *buf1, const Tuning &tn) {
   using T = Tile3<ST, TX, TY>;
   p.available = false;
   auto no = [&](const char *why) { snprintf(p.why_not, sizeof p.why_not, "%s", why); return false; };
   if (n[0] < 3 || n[1] < 3 || n[2] < 3) return no("tiled kernel: n >= 3");
-  if (n[0] % T::XH) return no("tiled kernel: TMA needs a 16-byte row pitch");
-  if (n[1] % T::TY == 1) return no("tiled kernel: last tile would hold a single row");
+  if ((nxp * (int)sizeof(ST)) % 16) return no("tiled kernel: TMA needs a 16-byte row pitch");
   int dev = 0, cc_major = 0, smem_optin = 0;
   if (cudaGetDevice(&dev) != cudaSuccess) return no("no device");
   cudaDeviceGetAttribute(&cc_major, cudaDevAttrComputeCapabilityMajor, dev);
@@ -392,11 +393,11 @@ inline bool plan3_setup(Plan3 &p, const int *n, void *buf0, void *buf1, const Tu
   const int b_c2[4] = {T::TX, T::TY, 1, 2}, b_c4[4] = {T::TX, T::TY, 1, 4}, b_x[4] = {T::HX, T::TY, 1, 4};
   const int b_y[4] = {T::TX, T::HY, 1, 4}, b_xy[4] = {T::HX, T::HY, 1, 4};
   for (int i = 0; i < 2; ++i) {
-    if (!make_map(&p.maps[i].c2, bufs[i], eb, 4, dims, b_c2, tn.l2promo) ||
-        !make_map(&p.maps[i].c4, bufs[i], eb, 4, dims, b_c4, tn.l2promo) ||
-        !make_map(&p.maps[i].x, bufs[i], eb, 4, dims, b_x, tn.l2promo) ||
-        !make_map(&p.maps[i].y, bufs[i], eb, 4, dims, b_y, tn.l2promo) ||
-        !make_map(&p.maps[i].xy, bufs[i], eb, 4, dims, b_xy, tn.l2promo))
+    if (!make_map(&p.maps[i].c2, bufs[i], eb, 4, dims, b_c2, tn.l2promo, nxp) ||
+        !make_map(&p.maps[i].c4, bufs[i], eb, 4, dims, b_c4, tn.l2promo, nxp) ||
+        !make_map(&p.maps[i].x, bufs[i], eb, 4, dims, b_x, tn.l2promo, nxp) ||
+        !make_map(&p.maps[i].y, bufs[i], eb, 4, dims, b_y, tn.l2promo, nxp) ||
+        !make_map(&p.maps[i].xy, bufs[i], eb, 4, dims, b_xy, tn.l2promo, nxp))
       return no("cuTensorMapEncodeTiled failed");
   }
   if (cudaFuncSetAttribute(k_step_zmarch<ST, TX, TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM_BYTES) != cudaSuccess) {
@@ -419,12 +420,12 @@ inline bool plan3_setup(Plan3 &p, const int *n, void *buf0, void *buf1, const Tu
 }
 
 template <typename ST>
-inline bool plan3_create(Plan3 &p, const int *n, void *buf0, void *buf1, const Tuning &tn) {
+inline bool plan3_create(Plan3 &p, const int *n, int nxp, void *buf0, void *buf1, const Tuning &tn) {
   p.shape = tn.shape3d;
   switch (tn.shape3d) {
-    case 1: return plan3_setup<ST, 64, 4>(p, n, buf0, buf1, tn);
-    case 2: return plan3_setup<ST, 128, 2>(p, n, buf0, buf1, tn);
-    default: p.shape = 0; return plan3_setup<ST, 32, 8>(p, n, buf0, buf1, tn);
+    case 1: return plan3_setup<ST, 64, 4>(p, n, nxp, buf0, buf1, tn);
+    case 2: return plan3_setup<ST, 128, 2>(p, n, nxp, buf0, buf1, tn);
+    default: p.shape = 0; return plan3_setup<ST, 32, 8>(p, n, nxp, buf0, buf1, tn);
   }
 }
 

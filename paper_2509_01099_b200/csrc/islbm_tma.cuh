@@ -112,9 +112,11 @@ inline CUtensorMapL2promotion promo_of(int k) {
   }
 }
 
-// Dense tensor view of one population buffer for TMA: dims[0] is x (fastest); the last dimension is the
-// storage plane; zero fill outside.  elem_bytes 8 (fp64) or 4 (fp32 storage).
-inline bool make_map(CUtensorMap *m, void *base, int elem_bytes, int rank, const long long *dims, const int *box, int promo) {
+// Tensor view of one population buffer for TMA: dims[0] = nx is x (fastest) with a row pitch of row_pitch >= nx
+// elements (the padding columns lie outside the tensor, so they read as zero like every out-of-mesh element);
+// the other dimensions are dense; the last one is the storage plane.  elem_bytes 8 (fp64) or 4 (fp32 storage).
+inline bool make_map(CUtensorMap *m, void *base, int elem_bytes, int rank, const long long *dims, const int *box, int promo,
+                     long long row_pitch) {
   EncodeTiledFn enc = get_encode_fn();
   if (!enc || rank < 2 || rank > 5) return false;
   const CUtensorMapDataType dt = elem_bytes == 8 ? CU_TENSOR_MAP_DATA_TYPE_FLOAT64 : CU_TENSOR_MAP_DATA_TYPE_FLOAT32;
@@ -125,7 +127,7 @@ inline bool make_map(CUtensorMap *m, void *base, int elem_bytes, int rank, const
     gd[i] = (cuuint64_t)dims[i];
     bx[i] = (cuuint32_t)box[i];
     es[i] = 1;
-    pitch *= (unsigned long long)dims[i];
+    pitch *= (unsigned long long)(i == 0 ? row_pitch : dims[i]);
     if (i < rank - 1) gs[i] = (cuuint64_t)pitch;
   }
   return enc(m, dt, (cuuint32_t)rank, base, gd, gs, bx, es, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_NONE,

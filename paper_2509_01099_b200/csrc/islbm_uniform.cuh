@@ -15,21 +15,21 @@ namespace islbmk {
 template <int DIM, int Q, typename ST>
 __device__ __forceinline__ double shift_f(const DevMesh &m, const ST *__restrict__ src, const NodeCtx<DIM> &cx) {
   constexpr int EX = evel<DIM>(Q, 0), EY = evel<DIM>(Q, 1), EZ = evel<DIM>(Q, 2);
-  if (crosses<DIM, EX, EY, EZ>(cx)) return ldv(src + (long long)plane_f<DIM>(opposite<DIM>(Q)) * m.nn + cx.c);
-  const long long off = (long long)EX + (long long)EY * m.nx + (long long)EZ * m.nx * m.ny;
-  return ldv(src + (long long)plane_f<DIM>(Q) * m.nn + cx.c - off);
+  if (crosses<DIM, EX, EY, EZ>(cx)) return ldv(src + (long long)plane_f<DIM>(opposite<DIM>(Q)) * m.nnp + cx.c);
+  const long long off = (long long)EX + (long long)EY * m.nxp + (long long)EZ * m.nxp * m.ny;
+  return ldv(src + (long long)plane_f<DIM>(Q) * m.nnp + cx.c - off);
 }
 
 template <int DIM, int Q, typename ST>
 __device__ __forceinline__ double shift_g(const DevMesh &m, const ST *__restrict__ src, const NodeCtx<DIM> &cx) {
   constexpr int EX = evel<DIM>(Q, 0), EY = evel<DIM>(Q, 1), EZ = evel<DIM>(Q, 2);
   if (crosses<DIM, EX, EY, EZ>(cx)) {
-    const double gb = ldv(src + (long long)plane_g<DIM>(opposite<DIM>(Q)) * m.nn + cx.c);
+    const double gb = ldv(src + (long long)plane_g<DIM>(opposite<DIM>(Q)) * m.nnp + cx.c);
     if (EX != 0) return -gb + m.omega_bc * (cx.lo[0] ? m.T_hot : m.T_cold);   // Eq. 22
     return gb;                                                                // Eq. 23
   }
-  const long long off = (long long)EX + (long long)EY * m.nx + (long long)EZ * m.nx * m.ny;
-  return ldv(src + (long long)plane_g<DIM>(Q) * m.nn + cx.c - off);
+  const long long off = (long long)EX + (long long)EY * m.nxp + (long long)EZ * m.nxp * m.ny;
+  return ldv(src + (long long)plane_g<DIM>(Q) * m.nnp + cx.c - off);
 }
 
 template <int DIM, typename ST, int... Qs>
@@ -53,7 +53,7 @@ k_step_shift(DevMesh m, NodeParams np, const ST *__restrict__ src, ST *__restric
   if (ix >= m.nx || iy >= m.ny || iz >= m.nz) return;
   NodeCtx<DIM> cx;
   cx.i[0] = ix; cx.i[1] = iy; cx.i[2] = iz;
-  cx.c = ((long long)iz * m.ny + iy) * m.nx + ix;
+  cx.c = ((long long)iz * m.ny + iy) * m.nxp + ix;
   cx.lo[0] = ix == 0; cx.hi[0] = ix == m.nx - 1;
   cx.lo[1] = iy == 0; cx.hi[1] = iy == m.ny - 1;
   cx.lo[2] = DIM == 3 && iz == 0; cx.hi[2] = DIM == 3 && iz == m.nz - 1;
@@ -64,9 +64,9 @@ k_step_shift(DevMesh m, NodeParams np, const ST *__restrict__ src, ST *__restric
   for (int q = 0; q < QF; ++q) f[q] += Store<ST, DIM>::bias(q);
   collide_node(f, g, np);
 #pragma unroll
-  for (int q = 0; q < QF; ++q) dst[(long long)plane_f<DIM>(q) * m.nn + cx.c] = (ST)(f[q] - Store<ST, DIM>::bias(q));
+  for (int q = 0; q < QF; ++q) dst[(long long)plane_f<DIM>(q) * m.nnp + cx.c] = (ST)(f[q] - Store<ST, DIM>::bias(q));
 #pragma unroll
-  for (int q = 0; q < QG; ++q) dst[(long long)plane_g<DIM>(q) * m.nn + cx.c] = (ST)g[q];
+  for (int q = 0; q < QG; ++q) dst[(long long)plane_g<DIM>(q) * m.nnp + cx.c] = (ST)g[q];
 }
 
 }  // namespace islbmk

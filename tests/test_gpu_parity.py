@@ -106,6 +106,8 @@ CASES_1STEP = [
     ("3d_tiled_34x18x7", 3, (34, 18, 7), (1.2, 1.1, 0.9)),
     ("3d_tiled_96x50x33", 3, (96, 50, 33), (1.6, 1.4, 1.2)),
     ("3d_tiled_4x4x3", 3, (4, 4, 3), (0.5, 0.5, 0.5)),
+    ("3d_clamp_33x17x9", 3, (33, 17, 9), (1.2, 1.3, 1.1)),
+    ("3d_clamp_65x9x5", 3, (65, 9, 5), (1.4, 0.9, 0.7)),
     ("3d_min_3x3x3", 3, (3, 3, 3), (0.5, 0.5, 0.5)),
     ("3d_thin_5x3x33", 3, (5, 3, 33), (0.7, 0.5, 1.5)),
 ]
@@ -123,7 +125,9 @@ def test_one_step_all_populations(islbm, name, dim, ns, st):
     fo, go = orc.get_populations()
     orc.step(2)
     fo3, go3 = orc.get_populations()
-    for k, tune in kernels_for(islbm, sim):
+    variants = kernels_for(islbm, sim)
+    assert any(k == islbm.KERNEL_TILED for k, _ in variants), "the TMA kernel must take every mesh with n >= 3"
+    for k, tune in variants:
         select(sim, k, tune)
         sim.set_populations(torch.from_numpy(f0).cuda(), torch.from_numpy(g0).cuda())
         f_back, g_back = sim.get_populations()            # before any step: the input itself
@@ -140,7 +144,9 @@ def test_one_step_all_populations(islbm, name, dim, ns, st):
 
 
 @pytest.mark.parametrize("dim,ns,st", [(2, (132, 45, 1), (1.5, 1.2, 0)), (2, (520, 21, 1), (1.7, 1.1, 0)),
-                                       (3, (36, 18, 9), (1.3, 1.2, 1.1)), (3, (68, 27, 20), (1.5, 1.1, 1.4))])
+                                       (2, (131, 67, 1), (1.3, 1.9, 0)), (3, (36, 18, 9), (1.3, 1.2, 1.1)),
+                                       (3, (68, 27, 20), (1.5, 1.1, 1.4)), (3, (37, 21, 19), (1.5, 1.2, 1.7)),
+                                       (3, (33, 17, 9), (1.2, 1.3, 1.1))])
 def test_fp32_storage_every_kernel_three_steps(islbm, dim, ns, st):
     """fp32 storage of f_q - w_q and g_q, fp64 arithmetic: every kernel variant against the fp64 oracle.
     Tolerance: 3 steps x one fp32 rounding (2^-24 relative to |f_q - w_q| <= 0.4) per stored value, amplified
