@@ -271,7 +271,8 @@ inline bool plan2_setup(Plan2 &p, const int *n, int nxp, void *buf0, void *buf1,
     cudaGetLastError();
     occ = 1;
   }
-  // one full wave of resident CTAs, chunks of at least 8 rows to amortise the 2-row prologue
+  // one full wave of resident CTAs; small meshes get chunks down to 2 rows (measured: a 2-D CTA needs ~1.5 us per
+  // row whatever the mesh, so latency, not the doubled prologue traffic, decides there)
   const int strips = (n[0] + T::TX - 1) / T::TX;
   int chunk;
   if (tn.chunk > 0) {
@@ -280,7 +281,7 @@ inline bool plan2_setup(Plan2 &p, const int *n, int nxp, void *buf0, void *buf1,
     int nchunks = (sms * occ) / strips;
     if (nchunks < 1) nchunks = 1;
     chunk = (n[1] + nchunks - 1) / nchunks;
-    if (chunk < 8) chunk = 8;
+    if (chunk < 2) chunk = 2;
   }
   if (chunk > kMaxChunk) chunk = kMaxChunk;
   p.ychunk = chunk < n[1] ? chunk : n[1];

@@ -404,15 +404,16 @@ inline bool plan3_setup(Plan3 &p, const int *n, int nxp, void *buf0, void *buf1,
     cudaGetLastError();
     return no("cudaFuncSetAttribute failed");
   }
-  // z-chunks: enough CTAs for >= ~12 waves of 148 SMs (measured: shorter chunks win up to there), chunk >= 16
-  // slices to amortise the 2-slice prologue
+  // z-chunks (measured, profiles/): a CTA needs ~2 us per slice whatever the mesh, so small meshes want one
+  // full wave of short chunks; large meshes want >= ~12 waves of CTAs and chunks >= 8 to amortise the prologue
   const int tiles = ((n[0] + T::TX - 1) / T::TX) * ((n[1] + T::TY - 1) / T::TY);
-  int chunk = n[2];
+  auto ctas = [&](int c) { return (long long)tiles * ((n[2] + c - 1) / c); };
+  int chunk = n[2] < kMaxChunk ? n[2] : kMaxChunk;
   if (tn.chunk > 0) {
     chunk = tn.chunk < n[2] ? tn.chunk : n[2];
   } else {
-    if (chunk > kMaxChunk) chunk = kMaxChunk;
-    while (chunk > 16 && (long long)tiles * ((n[2] + chunk - 1) / chunk) < 148 * 12) chunk = (chunk + 1) / 2;
+    while (chunk > 4 && ctas((chunk + 1) / 2) <= 148 + 16) chunk = (chunk + 1) / 2;
+    while (chunk > 8 && ctas(chunk) < 148 * 12) chunk = (chunk + 1) / 2;
   }
   p.zchunk = chunk < kMaxChunk ? chunk : kMaxChunk;
   p.available = true;
