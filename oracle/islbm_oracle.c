@@ -800,6 +800,47 @@ void oracle_nusselt(const oracle_t *h, double out[5]) {
   free(w);
 }
 
+/* Nu_middle, Eq. 33: line (area) average over the vertical centre plane x* = 0.5 of
+ * sqrt(Ra Pr) u* T* - dT* / dx*.  The paper does not say how the derivative is taken or what happens when
+ * no node column sits at x* = 0.5 (reading A23): dT/dx at a node column is the derivative of the
+ * parabola through the column and its two neighbours (second order on the stretched mesh), and the flux is
+ * interpolated linearly between the two columns that bracket the midpoint of the two x-walls.  Averaging
+ * weights and normalisation as for Nu_hot (Eq. 29). */
+double oracle_nusselt_middle(const oracle_t *h) {
+  const long nn = (long)h->nn;
+  const int nx = h->n[0], ny = h->n[1], nz = h->n[2];
+  double *T = (double *)malloc(sizeof(double) * (size_t)nn);
+  double *u = (double *)malloc(sizeof(double) * (size_t)nn);
+  oracle_fields(h, NULL, u, NULL, NULL, T);
+  const double *x = h->x[0];
+  double xmid = 0.5 * ((x[0] - 0.5 * h->delta) + (x[nx - 1] + 0.5 * h->delta));
+  int i0 = 1;
+  while (i0 < nx - 3 && x[i0 + 1] <= xmid) ++i0;          /* x[i0] <= xmid < x[i0+1], 1 <= i0 <= nx-3 */
+  double a1 = (xmid - x[i0]) / (x[i0 + 1] - x[i0]);
+  if (a1 < 0.0 || nx < 4) a1 = 0.0;                        /* nx = 3: the only interior column */
+  if (a1 > 1.0) a1 = 1.0;
+  double a[2] = {1.0 - a1, a1};
+  double area = h->L_eff[1] * (h->dim == 3 ? h->L_eff[2] : 1.0);
+  double s = 0.0;
+  for (int iz = 0; iz < nz; ++iz)
+    for (int iy = 0; iy < ny; ++iy) {
+      double wa = h->avgw[1][iy] * h->avgw[2][iz];
+      long r = ((long)iz * ny + iy) * nx;
+      for (int k = 0; k < 2; ++k) {
+        int i = i0 + k;
+        if (a[k] == 0.0) continue;
+        double hm = (x[i] - x[i - 1]) / h->delta, hp = (x[i + 1] - x[i]) / h->delta;   /* lattice units */
+        double dTdx = -hp / (hm * (hm + hp)) * T[r + i - 1] + (hp - hm) / (hm * hp) * T[r + i] +
+                      hm / (hp * (hm + hp)) * T[r + i + 1];
+        double flux = sqrt(h->Ra * h->Pr) * (u[r + i] / h->U) * (T[r + i] - h->T0) - h->H_lu * dTdx;
+        s += wa * a[k] * flux;
+      }
+    }
+  free(T);
+  free(u);
+  return s / area;
+}
+
 void oracle_mass(const oracle_t *h, double out[2]) {
   const long nn = (long)h->nn;
   const int nx = h->n[0], ny = h->n[1], nz = h->n[2];

@@ -84,6 +84,9 @@ void oracle_fields(const oracle_t *h, double *rho, double *u, double *v,
  * out[3]=<u*^2>_V, out[4]=<Nu> (Eq. 31/40). */
 void oracle_nusselt(const oracle_t *h, double out[5]);
 
+/* Nu_middle, Eq. 33: average over the vertical centre plane of sqrt(RaPr) u.T - dT/dx in free-fall units (reading A23). */
+double oracle_nusselt_middle(const oracle_t *h);
+
 /* Eq. 29-weighted total mass  sum rho * wx*wy(*wz)  and plain sum rho. */
 void oracle_mass(const oracle_t *h, double out[2]);
 

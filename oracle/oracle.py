@@ -72,6 +72,7 @@ def load():
         "oracle_step_node": (None, [vp, C.c_int, C.c_int, C.c_int, _dp, _dp]),
         "oracle_fields": (None, [vp, _dp, _dp, _dp, _dp, _dp]),
         "oracle_nusselt": (None, [vp, _dp]),
+        "oracle_nusselt_middle": (C.c_double, [vp]),
         "oracle_mass": (None, [vp, _dp]),
         "oracle_qf": (C.c_int, [vp]),
         "oracle_qg": (C.c_int, [vp]),
@@ -198,6 +199,9 @@ class Oracle:
         out = np.empty(5)
         self.lib.oracle_nusselt(self.h, _ptr(out))
         return dict(zip(NUSSELT_NAMES, out.tolist()))
+
+    def nusselt_middle(self):
+        return float(self.lib.oracle_nusselt_middle(self.h))
 
     def mass(self):
         out = np.empty(2)

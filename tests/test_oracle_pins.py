@@ -680,3 +680,63 @@ def test_create_rejects_bad_input():
         Oracle([x, x], 2 * d, 1e5, 0.71, 0.1)                     # spacing < delta
     with pytest.raises(ValueError):
         Oracle([x[:2], x], d, 1e5, 0.71, 0.1)                     # n < 3
+
+
+# ---------------------------------------------------------------------------
+# Nu_middle, Eq. 33 (reading A23)
+# ---------------------------------------------------------------------------
+def _state_with(o, T_of_x, u0=0.0):
+    """rest-weight flow populations carrying a uniform x-velocity u0, temperature populations w_i * T(x)."""
+    ef, _ = o.velocities()
+    o.init(0, 0.0)
+    f0, _ = o.get_populations()
+    w = f0[:, 0, 0, 0].copy()
+    f = np.empty((o.qf,) + o.shape)
+    for i in range(o.qf):
+        f[i] = w[i] * (1.0 + 3.0 * ef[i][0] * u0)
+    T = T_of_x(np.asarray(o.coords[0]))
+    g = np.empty((o.qg,) + o.shape)
+    wg = np.full(o.qg, o.params()["omega_bc"] / 2)
+    wg[0] = 1 - wg[1:].sum()
+    for i in range(o.qg):
+        g[i] = (wg[i] * T)[None, None, :]
+    return f, g
+
+
+@pytest.mark.parametrize("dim,n", [(2, 21), (2, 20), (3, 9), (3, 8), (2, 3)])
+def test_nu_middle_is_exact_on_quadratic_temperature_and_uniform_advection(dim, n):
+    """Eq. 33 on states whose centre-plane flux has a closed form: T quadratic in x (the 3-point derivative and the
+    linear interpolation between the bracketing columns are then exact, odd and even n), plus a uniform u0."""
+    w = inputs.custom_workload("m", dim, n, stretch=1.3, Ra=2e4)
+    o = Oracle(w.coords, w.delta, w.Ra, w.Pr, w.Ma)
+    p = o.params()
+    x = np.asarray(w.coords[0])
+    xw = x[0] - w.delta / 2
+    L = (x[-1] - x[0] + w.delta)
+    xm = xw + L / 2
+    a, b, c = 0.3, -0.8, (0.0 if n == 3 else 0.45)
+    s = lambda xx: (xx - xw) / w.delta                       # lattice units from the hot wall
+    Tq = lambda xx: a + b * s(xx) / p["H_lu"] + c * (s(xx) / p["H_lu"]) ** 2
+    u0 = 0.01 * p["U"]
+    f, g = _state_with(o, Tq, u0)
+    o.set_populations(f, g)
+    dTdxstar = b + 2 * c * s(xm) / p["H_lu"]                 # d T / d x*  with x* = x_lu / H_lu
+    if n % 2 == 1:
+        T_mid = Tq(xm)
+    else:                                                    # linear interpolation of u*T between two columns
+        i0 = n // 2 - 1
+        a1 = (xm - x[i0]) / (x[i0 + 1] - x[i0])
+        T_mid = (1 - a1) * Tq(x[i0]) + a1 * Tq(x[i0 + 1])
+    expect = math.sqrt(w.Ra * w.Pr) * 0.01 * T_mid - dTdxstar
+    assert o.nusselt_middle() == pytest.approx(expect, rel=1e-11, abs=1e-12)
+
+
+def test_nu_middle_of_the_conduction_state_is_one():
+    w = inputs.custom_workload("m", 2, 24, stretch=1.5, Ra=1e5)
+    o = Oracle(w.coords, w.delta, w.Ra, w.Pr, w.Ma)
+    p = o.params()
+    x = np.asarray(w.coords[0])
+    lin = lambda xx: 0.5 - ((xx - (x[0] - w.delta / 2)) / w.delta) / p["H_lu"]
+    f, g = _state_with(o, lin)
+    o.set_populations(f, g)
+    assert o.nusselt_middle() == pytest.approx(1.0, abs=1e-12)
