@@ -137,6 +137,12 @@ int islbm_fields(islbm_t *h, double *rho, double *u, double *v, double *w,
  * Returns ISLBM_ERR_NONFINITE (out still written) if any entry is not finite. */
 int islbm_nusselt(islbm_t *h, double out[5]);
 
+/* HOST *out = Nu_middle (Eq. 33): average over the vertical centre plane x* = 0.5 of
+ * sqrt(Ra Pr) u* T* - dT* / dx*; the derivative at a node column is that of the parabola through the column and
+ * its two neighbours, and the flux is interpolated linearly between the two columns bracketing the midpoint of
+ * the x-walls (reading A23).  Synchronises the stream.  ISLBM_ERR_NONFINITE as for islbm_nusselt. */
+int islbm_nusselt_middle(islbm_t *h, double *out);
+
 /* Steady-state residuals of Eq. 30 between the current fields and the fields
  * saved by the previous call (first call saves and returns 1, 1):
  * HOST out[2] = { sum|u - u_prev|_2 / sum|u_prev|_2, sum|T - T_prev| / sum|T_prev| }.
@@ -146,6 +152,12 @@ int islbm_steady_residual(islbm_t *h, double out[2]);
 
 /* Test / study hooks (not part of the four-call contract). */
 int islbm_set_buoyancy_scale(islbm_t *h, double s); /* multiplies g*beta; 0 for pin P5 */
+/* Reference temperature T0 of the buoyancy force F = rho g beta (T - T0) y^ and of T* in
+ * Eq. 31/33.  Default 0 = the mean of the wall temperatures (BASELINE.json configs).  The paper's own runs have
+ * T* = (T - T0)/Delta_T in [0,1], i.e. T0 = the cold-wall temperature = -0.5 here (reading A9): in the
+ * weakly compressible model that breaks the centro-symmetry of the solution, which is what Table 3 prints.
+ * Must be called before islbm_init / islbm_set_populations. */
+int islbm_set_reference_temperature(islbm_t *h, double T0);
 /* 0 = auto (fastest kernel for this mesh), 1 = generic global-memory kernel,
  * 2 = TMA-staged shared-memory kernel (y-marching in 2-D, z-marching in 3-D),
  * 3 = uniform-mesh pure-shift kernel (only valid when every spacing equals

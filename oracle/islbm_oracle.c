@@ -344,6 +344,10 @@ void oracle_set_threads(oracle_t *h, int nthreads) {
 #endif
 }
 int oracle_get_threads(const oracle_t *h) { return h->nthreads; }
+/* reference temperature T0 of F = rho g beta (T - T0) y^ and of T* = (T - T0)/Delta_T.
+ * Default 0 (mean of the walls, BASELINE.json); the paper's T* in [0,1] corresponds to T0 = T_cold (reading A9). */
+void oracle_set_reference_temperature(oracle_t *h, double T0) { h->T0 = T0; }
+
 void oracle_set_buoyancy_scale(oracle_t *h, double s) { h->buoy = s; }
 
 /* ------------------------------------------------------------------------ */

@@ -52,6 +52,9 @@ void oracle_destroy(oracle_t *h);
 void oracle_set_threads(oracle_t *h, int nthreads);
 int  oracle_get_threads(const oracle_t *h);
 
+/* reference temperature T0 of the buoyancy force and of T* (default 0; the paper's runs: T_cold, reading A9). */
+void oracle_set_reference_temperature(oracle_t *h, double T0);
+
 /* test hook: scale on the buoyancy force (1 = paper; 0 = pin P5). */
 void oracle_set_buoyancy_scale(oracle_t *h, double s);
 

@@ -90,6 +90,7 @@ struct islbm {
   double Ra, Pr, Ma, delta;
   islbm_params prm;
   double buoy;
+  double T0;               // reference temperature of the buoyancy force
   DevMesh dm;
   NodeParams np;
   DiagParams dp;
@@ -173,6 +174,8 @@ static void set_node_params(islbm *h) {
   np.q_k = 3.0 - std::sqrt(3.0);
   np.q_e = 4.0 * std::sqrt(3.0) - 6.0;
   np.a_T = h->prm.a_T;
+  np.T0 = h->T0;
+  h->dp.T0 = h->T0;
 }
 
 // 3-point Lagrange weights of the departure point x_j - c*delta on the
@@ -239,6 +242,7 @@ extern "C" int islbm_create(islbm_t **out, const islbm_mesh *mesh, int lattice, 
   h->st_bytes = precision == ISLBM_F64 ? 8 : 4;
   h->Ra = Ra; h->Pr = Pr; h->Ma = Ma; h->delta = mesh->delta;
   h->buoy = 1.0;
+  h->T0 = 0.0;             // BASELINE.json configs: walls at +-0.5, reference = their mean (A9)
   h->uniform = uniform;
   rc = derive_params(h, mesh);
   if (rc) { delete h; return rc; }
@@ -279,7 +283,28 @@ extern "C" int islbm_create(islbm_t **out, const islbm_mesh *mesh, int lattice, 
   dm.T_cold = -0.5;
   h->dp.q_lo = (mesh->x[0][1] - mesh->x[0][0]) / mesh->delta;
   h->dp.q_hi = (mesh->x[0][h->n[0] - 1] - mesh->x[0][h->n[0] - 2]) / mesh->delta;
-  h->dp.T0 = 0.0;
+  h->dp.T0 = h->T0;
+  {   // Eq. 33 tables (A23)
+    const double *x = mesh->x[0];
+    const int nx = h->n[0];
+    const double xmid = 0.5 * ((x[0] - 0.5 * mesh->delta) + (x[nx - 1] + 0.5 * mesh->delta));
+    int i0 = 1;
+    while (i0 < nx - 3 && x[i0 + 1] <= xmid) ++i0;
+    double a1 = (xmid - x[i0]) / (x[i0 + 1] - x[i0]);
+    if (a1 < 0.0 || nx < 4) a1 = 0.0;
+    if (a1 > 1.0) a1 = 1.0;
+    h->dp.mid_i = i0;
+    h->dp.mid_a[0] = 1.0 - a1;
+    h->dp.mid_a[1] = a1;
+    for (int k = 0; k < 2; ++k) {
+      const int i = i0 + k;
+      if (i + 1 > nx - 1) { h->dp.mid_c[k][0] = h->dp.mid_c[k][1] = h->dp.mid_c[k][2] = 0.0; continue; }
+      const double hm = (x[i] - x[i - 1]) / mesh->delta, hp = (x[i + 1] - x[i]) / mesh->delta;
+      h->dp.mid_c[k][0] = -hp / (hm * (hm + hp));
+      h->dp.mid_c[k][1] = (hp - hm) / (hm * hp);
+      h->dp.mid_c[k][2] = hm / (hp * (hm + hp));
+    }
+  }
   h->cur = 0;
   h->has_state = false;
   h->other_is_pre = false;
@@ -309,6 +334,17 @@ extern "C" int islbm_set_buoyancy_scale(islbm_t *h, double s) {
     return fail(ISLBM_ERR_STATE, "set the buoyancy scale before islbm_init / islbm_set_populations "
                                  "(the stored post-collision state already contains the force)");
   h->buoy = s;
+  set_node_params(h);
+  return ISLBM_OK;
+}
+
+extern "C" int islbm_set_reference_temperature(islbm_t *h, double T0) {
+  if (!h) return fail(ISLBM_ERR_ARG, "NULL handle");
+  if (!std::isfinite(T0)) return fail(ISLBM_ERR_ARG, "T0 must be finite");
+  if (h->has_state && T0 != h->T0)
+    return fail(ISLBM_ERR_STATE, "set the reference temperature before islbm_init / islbm_set_populations "
+                                 "(the stored post-collision state already contains the force)");
+  h->T0 = T0;
   set_node_params(h);
   return ISLBM_OK;
 }
@@ -520,17 +556,37 @@ static void launch_nusselt(islbm *h, int nb) {
   h->launches += 2;
 }
 
-extern "C" int islbm_nusselt(islbm_t *h, double out[5]) {
-  if (!h || !out) return fail(ISLBM_ERR_ARG, "NULL argument");
-  if (!h->has_state) return fail(ISLBM_ERR_STATE, "no state");
+// one pass of the Nu / Re reduction; s[kRedSlots] on the host, stream synchronised
+static int run_diag_reduction(islbm *h, double *s) {
   const int nb = red_blocks(h);
 #define CALL(D, T) launch_nusselt<D, T>(h, nb)
   DISPATCH(h, CALL);
 #undef CALL
   CUDA_TRY(cudaPeekAtLastError());
-  double s[kRedSlots];
-  CUDA_TRY(cudaMemcpyAsync(s, h->ws + h->cv.red_out, sizeof s, cudaMemcpyDeviceToHost, h->stream));
+  CUDA_TRY(cudaMemcpyAsync(s, h->ws + h->cv.red_out, sizeof(double) * kRedSlots, cudaMemcpyDeviceToHost, h->stream));
   CUDA_TRY(cudaStreamSynchronize(h->stream));
+  return ISLBM_OK;
+}
+
+extern "C" int islbm_nusselt_middle(islbm_t *h, double *out) {
+  if (!h || !out) return fail(ISLBM_ERR_ARG, "NULL argument");
+  if (!h->has_state) return fail(ISLBM_ERR_STATE, "no state");
+  double s[kRedSlots];
+  int rc = run_diag_reduction(h, s);
+  if (rc) return rc;
+  const islbm_params &p = h->prm;
+  const double area = p.L_eff[1] * (h->dim == 3 ? p.L_eff[2] : 1.0);
+  *out = std::sqrt(h->Ra * h->Pr) * (s[5] / area) / p.U - p.H_lu * (s[6] / area);
+  if (!std::isfinite(*out)) return fail(ISLBM_ERR_NONFINITE, "non-finite diagnostic: the run has diverged");
+  return ISLBM_OK;
+}
+
+extern "C" int islbm_nusselt(islbm_t *h, double out[5]) {
+  if (!h || !out) return fail(ISLBM_ERR_ARG, "NULL argument");
+  if (!h->has_state) return fail(ISLBM_ERR_STATE, "no state");
+  double s[kRedSlots];
+  int rc = run_diag_reduction(h, s);
+  if (rc) return rc;
   const islbm_params &p = h->prm;
   const double area = p.L_eff[1] * (h->dim == 3 ? p.L_eff[2] : 1.0);
   const double vol = area * p.L_eff[0];

@@ -6,7 +6,7 @@
 // with the Guo forcing moments of Eq. 12/13 (PAPER.md:100-
 // 104; last entry of Eq. 12 read as u*Fy + v*Fx, A8), and mapped back
 // with M^-1 = M^T diag(1/|row|^2) (rows are mutually orthogonal).  The body
-// force is F = rho*g*beta*(T - T0)*y^ with T0 = 0, so Fx = Fz = 0
+// force is F = rho*g*beta*(T - T0)*y^ (T0: DESIGN.md A9), so Fx = Fz = 0
 // is folded in.  Relaxation rates: DESIGN.md A7.
 //
 // Direction ordering: include/islbm.h.  Everything here is fp64.
@@ -31,6 +31,7 @@ struct NodeParams {
   double q_k;     // 3 - sqrt(3)     (temperature flux moments)
   double q_e;     // 4 sqrt(3) - 6   (remaining temperature moments)
   double a_T;     // Eq. 15/16
+  double T0;      // reference temperature of the buoyancy force
 };
 
 template <int DIM> struct Lat;
@@ -117,7 +118,7 @@ ISLBM_HD void collide_node(double (&f)[9], double (&g)[5], const NodeParams &p) 
   const double sa = (f[1] + f[3]) + (f[2] + f[4]);   // axis shell
   const double sd = (f[5] + f[7]) + (f[6] + f[8]);   // diagonal shell
   const double rho = f[0] + sa + sd;
-  const double Fy = rho * p.gbeta * T;
+  const double Fy = rho * p.gbeta * (T - p.T0);
   const double ax = f[1] - f[3], ay = f[2] - f[4];
   const double dx = (f[5] - f[7]) + (f[8] - f[6]);    // sum cx over diagonals
   const double dy = (f[5] - f[7]) + (f[6] - f[8]);    // sum cy over diagonals
@@ -177,7 +178,7 @@ ISLBM_HD void fields_from_post(const double (&f)[9], const double (&g)[5], const
                                double &rho, double &u, double &v, double &w, double &T) {
   T = g[0] + g[1] + g[2] + g[3] + g[4];
   rho = f[0] + ((f[1] + f[3]) + (f[2] + f[4])) + ((f[5] + f[7]) + (f[6] + f[8]));
-  const double Fy = rho * p.gbeta * T;
+  const double Fy = rho * p.gbeta * (T - p.T0);
   const double jx = (f[1] - f[3]) + ((f[5] - f[7]) + (f[8] - f[6]));
   const double jy = (f[2] - f[4]) + ((f[5] - f[7]) + (f[6] - f[8]));
   u = jx / rho;
@@ -212,7 +213,7 @@ ISLBM_HD void collide_node(double (&f)[19], double (&g)[7], const NodeParams &p)
   const double sa = px + py + pz;
   const double sd = xy_s + xz_s + yz_s;
   const double rho = f[0] + sa + sd;
-  const double Fy = rho * p.gbeta * T;
+  const double Fy = rho * p.gbeta * (T - p.T0);
   const double dxs = xy_x + xz_x, dys = xy_y + yz_y, dzs = xz_z + yz_z;
   const double jx = ax + dxs, jy = ay + dys, jz = az + dzs;
   const double inv = 1.0 / rho;
@@ -304,7 +305,7 @@ ISLBM_HD void fields_from_post(const double (&f)[19], const double (&g)[7], cons
   const double sd = ((f[7] + f[10]) + (f[8] + f[9])) + ((f[11] + f[14]) + (f[12] + f[13])) +
                     ((f[15] + f[18]) + (f[16] + f[17]));
   rho = f[0] + sa + sd;
-  const double Fy = rho * p.gbeta * T;
+  const double Fy = rho * p.gbeta * (T - p.T0);
   const double jx = (f[1] - f[2]) + ((f[7] - f[10]) + (f[9] - f[8])) + ((f[11] - f[14]) + (f[13] - f[12]));
   const double jy = (f[3] - f[4]) + ((f[7] - f[10]) + (f[8] - f[9])) + ((f[15] - f[18]) + (f[17] - f[16]));
   const double jz = (f[5] - f[6]) + ((f[11] - f[14]) + (f[12] - f[13])) + ((f[15] - f[18]) + (f[16] - f[17]));

@@ -13,12 +13,17 @@
 
 namespace islbmk {
 
-constexpr int kRedSlots = 5;
+constexpr int kRedSlots = 7;
 constexpr int kRedThreads = 256;
 
 struct DiagParams {
   double q_lo, q_hi;   // (x1-x0)/delta, (x_{n-1}-x_{n-2})/delta for Eq. 28
   double T0;
+  // Eq. 33 (A23): the two node columns mid_i, mid_i+1 that bracket x* = 0.5, their linear-interpolation
+  // weights, and the 3-point derivative coefficients (lattice units) at each of them
+  int mid_i;
+  double mid_a[2];
+  double mid_c[2][3];
 };
 
 // Eq. 28, bottom-wall form with Delta = 1 l.u.
@@ -58,10 +63,11 @@ __device__ __forceinline__ double node_temperature(const DevMesh &m, const ST *_
 
 // pass 1: per-block partial sums of
 //   [0] wa*dT/dx|hot  [1] wa*dT/dx|cold  [2] wv*|u|  [3] wv*|u|^2  [4] wv*u*(T-T0)
+//   [5] wa*a_k*u*(T-T0) and [6] wa*a_k*dT/dx on the two columns bracketing the centre plane (Eq. 33)
 template <int DIM, typename ST>
 __global__ void __launch_bounds__(kRedThreads)
 k_nusselt_partial(DevMesh m, NodeParams np, DiagParams dp, const ST *__restrict__ S, double *__restrict__ partial) {
-  double acc[kRedSlots] = {0.0, 0.0, 0.0, 0.0, 0.0};
+  double acc[kRedSlots] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
   const long long stride = (long long)gridDim.x * kRedThreads;
   for (long long c = (long long)blockIdx.x * kRedThreads + threadIdx.x; c < m.nn; c += stride) {
     const int ix = (int)(c % m.nx);
@@ -86,6 +92,13 @@ k_nusselt_partial(DevMesh m, NodeParams np, DiagParams dp, const ST *__restrict_
       const double T1 = node_temperature<DIM>(m, S, cs - 1);
       acc[1] += wa * (-wall_derivative(dp.q_hi, m.T_cold, T, T1));
     }
+    const int km = ix - dp.mid_i;
+    if ((km == 0 || km == 1) && dp.mid_a[km] != 0.0) {
+      const double Tm = node_temperature<DIM>(m, S, cs - 1), Tp = node_temperature<DIM>(m, S, cs + 1);
+      const double dTdx = dp.mid_c[km][0] * Tm + dp.mid_c[km][1] * T + dp.mid_c[km][2] * Tp;
+      acc[5] += wa * dp.mid_a[km] * (u * (T - dp.T0));
+      acc[6] += wa * dp.mid_a[km] * dTdx;
+    }
   }
   block_reduce_store(acc, partial);
 }
@@ -93,7 +106,7 @@ k_nusselt_partial(DevMesh m, NodeParams np, DiagParams dp, const ST *__restrict_
 // pass 2: one block, fixed order
 __global__ void __launch_bounds__(kRedThreads)
 k_reduce_final(const double *__restrict__ partial, int nblocks, double *__restrict__ out) {
-  double acc[kRedSlots] = {0.0, 0.0, 0.0, 0.0, 0.0};
+  double acc[kRedSlots] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
   for (int b = threadIdx.x; b < nblocks; b += kRedThreads)
 #pragma unroll
     for (int s = 0; s < kRedSlots; ++s) acc[s] += partial[(long long)b * kRedSlots + s];
@@ -106,7 +119,7 @@ template <int DIM, typename ST>
 __global__ void __launch_bounds__(kRedThreads)
 k_residual_partial(DevMesh m, NodeParams np, const ST *__restrict__ S, double *__restrict__ snap,
                    double *__restrict__ partial) {
-  double acc[kRedSlots] = {0.0, 0.0, 0.0, 0.0, 0.0};
+  double acc[kRedSlots] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
   const long long stride = (long long)gridDim.x * kRedThreads;
   for (long long c = (long long)blockIdx.x * kRedThreads + threadIdx.x; c < m.nn; c += stride) {
     double f[Lat<DIM>::QF], g[Lat<DIM>::QG];

@@ -21,8 +21,8 @@ KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED, KERNEL_UNIFORM_SHIFT = 0, 1, 2, 3
 
 EXPORTS = (
     "islbm_workspace_bytes", "islbm_create", "islbm_destroy", "islbm_get_params", "islbm_init",
-    "islbm_set_populations", "islbm_get_populations", "islbm_step", "islbm_fields", "islbm_nusselt",
-    "islbm_steady_residual", "islbm_set_buoyancy_scale", "islbm_set_kernel", "islbm_set_tuning", "islbm_launch_count",
+    "islbm_set_populations", "islbm_get_populations", "islbm_step", "islbm_fields", "islbm_nusselt", "islbm_nusselt_middle",
+    "islbm_steady_residual", "islbm_set_buoyancy_scale", "islbm_set_reference_temperature", "islbm_set_kernel", "islbm_set_tuning", "islbm_launch_count",
     "islbm_kernel_name", "islbm_last_error", "islbm_version",
 )
 
@@ -60,8 +60,10 @@ def _load():
     lib.islbm_step.argtypes = [vp, C.c_int]
     lib.islbm_fields.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.islbm_nusselt.argtypes = [vp, dp]
+    lib.islbm_nusselt_middle.argtypes = [vp, dp]
     lib.islbm_steady_residual.argtypes = [vp, dp]
     lib.islbm_set_buoyancy_scale.argtypes = [vp, C.c_double]
+    lib.islbm_set_reference_temperature.argtypes = [vp, C.c_double]
     lib.islbm_set_kernel.argtypes = [vp, C.c_int]
     lib.islbm_set_tuning.argtypes = [vp, C.c_char_p, C.c_int]
     lib.islbm_launch_count.argtypes = [vp]
@@ -152,6 +154,9 @@ class Islbm:
     def set_buoyancy_scale(self, s):
         _check(lib.islbm_set_buoyancy_scale(self.h, float(s)))
 
+    def set_reference_temperature(self, T0):
+        _check(lib.islbm_set_reference_temperature(self.h, float(T0)))
+
     def set_kernel(self, which):
         _check(lib.islbm_set_kernel(self.h, int(which)))
 
@@ -192,6 +197,11 @@ class Islbm:
         out = (C.c_double * 5)()
         _check(lib.islbm_nusselt(self.h, out))
         return dict(zip(("Nu_hot", "Nu_cold", "Re", "u2", "Nu_vol"), list(out)))
+
+    def nusselt_middle(self):
+        out = C.c_double(0.0)
+        _check(lib.islbm_nusselt_middle(self.h, C.byref(out)))
+        return out.value
 
     def steady_residual(self):
         out = (C.c_double * 2)()

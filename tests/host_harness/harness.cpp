@@ -7,7 +7,7 @@ extern "C" void harness_collide(int dim, double *f, double *g, const double *prm
   islbmk::NodeParams p;
   p.gbeta = prm[0]; p.s_nu = prm[1]; p.s_q = prm[2];
   p.hs_nu = 1.0 - 0.5 * p.s_nu; p.hs_q = 1.0 - 0.5 * p.s_q;
-  p.q_k = prm[3]; p.q_e = prm[4]; p.a_T = prm[5];
+  p.q_k = prm[3]; p.q_e = prm[4]; p.a_T = prm[5]; p.T0 = 0.0;
   if (dim == 2) {
     double ff[9], gg[5];
     for (int i = 0; i < 9; ++i) ff[i] = f[i];

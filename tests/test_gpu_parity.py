@@ -232,6 +232,7 @@ def test_config1_init_and_1000_steps(islbm):
     ns, no = sim.nusselt(), orc.nusselt()
     for k in no:
         assert ns[k] == pytest.approx(no[k], rel=1e-9, abs=1e-12), k
+    assert sim.nusselt_middle() == pytest.approx(orc.nusselt_middle(), rel=1e-9, abs=1e-12)   # Eq. 33, even n
 
 
 def test_config1_fp32_storage_1000_steps(islbm):
@@ -257,6 +258,7 @@ def test_3d_small_200_steps_fields_and_nusselt(islbm):
     ns, no = sim.nusselt(), orc.nusselt()
     for k in no:
         assert ns[k] == pytest.approx(no[k], rel=1e-9, abs=1e-12), k
+    assert sim.nusselt_middle() == pytest.approx(orc.nusselt_middle(), rel=1e-9, abs=1e-12)
     # fp32 storage, 3-D
     sim32 = islbm.Islbm(w.coords, w.delta, w.Ra, w.Pr, w.Ma, precision=1)
     sim32.init(0, 1e-3)
@@ -387,13 +389,15 @@ def test_steady_residual_matches_definition(islbm):
 # ---------------------------------------------------------------------------
 def test_paper_mode_table2_ra1e6_257(islbm, golden):
     """Paper mode: erf mesh Eq. 26 with a = 1.5 (257 points, fluid nodes 1..255, delta = y_1), Ma = 0.1, Ra = 1e6,
-    run on the CUDA path to the steady-state criterion of Eq. 30, against Table 2
-    (PAPER.md:295).  <Nu> and Nu_hot within 0.3 % (the paper's own 257^2 -> infinity spread is 0.1-0.35 %); the
-    printed <Re> matches sqrt(Ra/Pr) * sqrt(<u*^2>_V) (reading A22), not the mean speed of Eq. 34 as printed."""
+    reference temperature T0 = T_cold (the paper's T* in [0,1], reading A9), run on the CUDA path to the steady-state
+    criterion of Eq. 30, against Table 2 and Table 3.
+    <Nu>, Nu_hot, Nu_middle within 0.3 % (the paper's own 257^2 -> infinity spread is 0.1-0.35 %); the printed <Re>
+    matches sqrt(Ra/Pr) * sqrt(<u*^2>_V) (reading A22), not the mean speed of Eq. 34 as printed."""
     ref = golden["table2"]["Ra1e6"]["257"]
     w = inputs.custom_workload("paper", 2, 257, mesh="erf", stretch=1.5, Ra=1e6, Ma=0.1)
     assert len(w.coords[0]) == 255
     sim = islbm.Islbm(w.coords, w.delta, w.Ra, w.Pr, w.Ma)
+    sim.set_reference_temperature(-0.5)
     sim.init(0, 0.0)
     sim.steady_residual()
     for _ in range(1500):                       # at most 3e6 steps; converges after ~1.45e6
@@ -403,13 +407,53 @@ def test_paper_mode_table2_ra1e6_257(islbm, golden):
             break
     assert ru < 1e-9 and rT < 1e-9
     nu = sim.nusselt()
+    nm = sim.nusselt_middle()
     assert nu["Nu_vol"] == pytest.approx(ref[0], rel=3e-3)
     assert nu["Nu_hot"] == pytest.approx(ref[1], rel=3e-3)
-    assert nu["Nu_cold"] == pytest.approx(nu["Nu_hot"], rel=1e-6)          # steady state: what enters leaves
-    assert nu["Nu_vol"] == pytest.approx(nu["Nu_hot"], rel=1e-3)
+    assert nm == pytest.approx(ref[2], rel=3e-3)
+    assert nu["Nu_cold"] == pytest.approx(nu["Nu_hot"], rel=2e-6)          # steady state: what enters leaves
+    assert nm == pytest.approx(nu["Nu_vol"], rel=5e-4)                     # every vertical plane carries the same flux
+    # with T0 = T_cold the weakly compressible model gives <Nu> below Nu_hot, as Table 2 prints (8.8282 vs 8.8509)
+    assert 0.5 * (ref[1] - ref[0]) < nu["Nu_hot"] - nu["Nu_vol"] < 1.5 * (ref[1] - ref[0])
     re_rms = math.sqrt(1e6 / 0.71 * nu["u2"])
     assert re_rms == pytest.approx(ref[3], rel=3e-3)
     assert nu["Re"] < 0.8 * ref[3]                                        # Eq. 34 as printed is a different number
+    # cell-centre values, Table 3: T_c on the paper's [0,1] scale = ours + 0.5, u_c in free-fall units;
+    # node 127 of the 255 fluid nodes sits at x* = y* = 0.5 exactly.  With T0 = mean the solution is centro-symmetric
+    # (T_c = 0.5, u_c = 0 to round-off); the paper's non-zero values are the signature of T0 = T_cold.  The paper's
+    # own u_c moves by 9 % from 257^2 to infinity (-1.2163e-4 -> -1.3320e-4): 15 % tolerance; v_c (1e-5) is not asserted.
+    c3 = golden["table3"]["Ra1e6"]["257"]
+    fl = sim.fields(("u", "v", "T"))
+    U = sim.params()["U"]
+    T_c = fl["T"][0, 127, 127].item() + 0.5
+    assert T_c < 0.4999 and T_c == pytest.approx(c3["T_c"], abs=3e-4)
+    assert fl["u"][0, 127, 127].item() / U == pytest.approx(c3["u_c"], rel=0.15)
+    assert fl["v"][0, 127, 127].item() > 0.0
+
+
+def test_reference_temperature_parity_and_symmetry(islbm):
+    """T0 = T_cold (paper) against the oracle; T0 = mean keeps the centro-symmetry T(1-x,1-y) = -T(x,y)."""
+    w = inputs.custom_workload("t0", 2, 41, stretch=1.4, Ra=1e5)
+    sim, orc = pair(islbm, w.coords, w.delta, w.Ra, w.Pr, w.Ma)
+    sim.set_reference_temperature(-0.5)
+    orc.set_reference_temperature(-0.5)
+    sim.init(0, 1e-3)
+    orc.init(0, 1e-3)
+    sim.step(300)
+    orc.step(300)
+    err = field_err(sim, orc)
+    assert max(err.values()) <= 1e-9, err
+    ns, no = sim.nusselt(), orc.nusselt()
+    for k in no:
+        assert ns[k] == pytest.approx(no[k], rel=1e-9, abs=1e-12), k
+    assert sim.nusselt_middle() == pytest.approx(orc.nusselt_middle(), rel=1e-9, abs=1e-12)
+    with pytest.raises(islbm.IslbmError):
+        sim.set_reference_temperature(0.25)         # state already holds the force
+    sym = islbm.Islbm(w.coords, w.delta, w.Ra, w.Pr, w.Ma)
+    sym.init(0, 0.0)
+    sym.step(2000)
+    T = sym.fields(("T",))["T"][0]
+    assert (T + torch.flip(T, (0, 1))).abs().max().item() < 1e-12 and T.abs().max().item() > 0.3
 
 
 def test_paper_mode_table4_ra1e5_129(islbm, golden):
@@ -420,6 +464,7 @@ def test_paper_mode_table4_ra1e5_129(islbm, golden):
     w = inputs.custom_workload("paper3", 3, 129, mesh="erf", stretch=1.5, Ra=1e5, Ma=0.1)
     sim = islbm.Islbm(w.coords, w.delta, w.Ra, w.Pr, w.Ma)
     assert sim.kernel_name == "tiled_zmarch_tma"
+    sim.set_reference_temperature(-0.5)         # the paper's T* in [0,1] (reading A9)
     sim.init(0, 0.0)
     sim.steady_residual()
     for _ in range(400):
