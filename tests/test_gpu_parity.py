@@ -321,6 +321,29 @@ def test_config5_256cu_sampled_nodes(islbm):
     assert fl["T"].abs().max().item() < 0.2     # one anti-bounce-back kick of omega*T_w at the x-walls
 
 
+def test_config5_256cu_full_mesh_20_steps(islbm):
+    """256^3 full size, launch configuration of bench.py: all fields after 20 steps against the OpenMP oracle
+    (bit-identical to its single-thread mode, test_threads_are_bit_identical), fp64 and fp32 storage."""
+    w = inputs.workload("c5_256cu")
+    sim, orc = pair(islbm, w.coords, w.delta, w.Ra, w.Pr, w.Ma, threads=len(os.sched_getaffinity(0)))
+    assert sim.kernel_name == "tiled_zmarch_tma"
+    sim.init(w.seed, w.noise_amp)
+    orc.init(w.seed, w.noise_amp)
+    sim.step(20)
+    orc.step(20)
+    err = field_err(sim, orc)
+    assert max(err.values()) <= 1e-10, err
+    ns, no = sim.nusselt(), orc.nusselt()
+    for k in no:
+        assert ns[k] == pytest.approx(no[k], rel=1e-9, abs=1e-12), k
+    sim.close()
+    sim32 = islbm.Islbm(w.coords, w.delta, w.Ra, w.Pr, w.Ma, precision=1)
+    sim32.init(w.seed, w.noise_amp)
+    sim32.step(20)
+    e32 = field_err(sim32, orc)
+    assert e32["u"] <= 1e-5 and e32["v"] <= 1e-5 and e32["w"] <= 1e-5 and e32["T"] <= 1e-5, e32
+
+
 # ---------------------------------------------------------------------------
 # method-level properties on the GPU path
 # ---------------------------------------------------------------------------
