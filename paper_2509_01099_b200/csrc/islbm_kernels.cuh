@@ -51,11 +51,26 @@ __device__ __forceinline__ const double *wrow(const DevMesh &m, int axis, int si
 // storage <-> fp64 value of flow population q (deviation storage for float)
 template <typename ST, int DIM> struct Store;
 template <int DIM> struct Store<double, DIM> {
+  static constexpr bool kBiased = false;
   static __device__ __forceinline__ double bias(int) { return 0.0; }
 };
 template <int DIM> struct Store<float, DIM> {
+  static constexpr bool kBiased = true;
   static __device__ __forceinline__ double bias(int q) { return wflow<DIM>(q); }
 };
+// storage form -> value and back (no arithmetic at all for fp64 storage: x + 0.0 is not a no-op for the compiler)
+template <typename ST, int DIM, int QF>
+__device__ __forceinline__ void add_bias(double (&f)[QF]) {
+  if constexpr (Store<ST, DIM>::kBiased) {
+#pragma unroll
+    for (int q = 0; q < QF; ++q) f[q] += Store<ST, DIM>::bias(q);
+  }
+}
+template <typename ST, int DIM>
+__device__ __forceinline__ ST to_storage(double v, int q) {
+  if constexpr (Store<ST, DIM>::kBiased) return (ST)(v - Store<ST, DIM>::bias(q));
+  else return (ST)v;
+}
 
 template <typename ST>
 __device__ __forceinline__ double ldv(const ST *p) { return (double)__ldg(p); }
@@ -201,12 +216,11 @@ k_step_generic(DevMesh m, NodeParams np, const ST *__restrict__ src, ST *__restr
   double f[QF], g[QG];
   pull_all_f<DIM>(m, src, cx, f, std::make_integer_sequence<int, QF>{});
   pull_all_g<DIM>(m, src, cx, g, std::make_integer_sequence<int, QG>{});
-#pragma unroll
-  for (int q = 0; q < QF; ++q) f[q] += Store<ST, DIM>::bias(q);
+  add_bias<ST, DIM>(f);
   if (COLLIDE) {
     collide_node(f, g, np);
 #pragma unroll
-    for (int q = 0; q < QF; ++q) dst[(long long)plane_f<DIM>(q) * m.nnp + cx.c] = (ST)(f[q] - Store<ST, DIM>::bias(q));
+    for (int q = 0; q < QF; ++q) dst[(long long)plane_f<DIM>(q) * m.nnp + cx.c] = to_storage<ST, DIM>(f[q], q);
 #pragma unroll
     for (int q = 0; q < QG; ++q) dst[(long long)plane_g<DIM>(q) * m.nnp + cx.c] = (ST)g[q];
   } else {
@@ -243,12 +257,12 @@ k_load_state(DevMesh m, NodeParams np, const double *__restrict__ fin, const dou
   }
   const long long cs = sidx(m, c);
 #pragma unroll
-  for (int q = 0; q < QF; ++q) pre[(long long)plane_f<DIM>(q) * m.nnp + cs] = (ST)(f[q] - Store<ST, DIM>::bias(q));
+  for (int q = 0; q < QF; ++q) pre[(long long)plane_f<DIM>(q) * m.nnp + cs] = to_storage<ST, DIM>(f[q], q);
 #pragma unroll
   for (int q = 0; q < QG; ++q) pre[(long long)plane_g<DIM>(q) * m.nnp + cs] = (ST)g[q];
   collide_node(f, g, np);
 #pragma unroll
-  for (int q = 0; q < QF; ++q) post[(long long)plane_f<DIM>(q) * m.nnp + cs] = (ST)(f[q] - Store<ST, DIM>::bias(q));
+  for (int q = 0; q < QF; ++q) post[(long long)plane_f<DIM>(q) * m.nnp + cs] = to_storage<ST, DIM>(f[q], q);
 #pragma unroll
   for (int q = 0; q < QG; ++q) post[(long long)plane_g<DIM>(q) * m.nnp + cs] = (ST)g[q];
 }

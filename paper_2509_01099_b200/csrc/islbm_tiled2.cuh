@@ -222,8 +222,7 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
         bb_fix_all_f<2>(f, wf, src, m.nnp, c, std::make_integer_sequence<int, 8>{});
         bb_fix_all_g<2>(g, wf, src, m.nnp, c, m, std::make_integer_sequence<int, 4>{});
       }
-#pragma unroll
-      for (int q = 0; q < 9; ++q) f[q] += Store<ST, 2>::bias(q);
+      add_bias<ST, 2>(f);
       collide_node(f, g, np);
       if (valid) store_node<2>(dst + c, m.nnp, f, g, spol, std::make_integer_sequence<int, 14>{});
     } else {

@@ -140,7 +140,7 @@ template <int DIM, int P, typename ST>
 __device__ __forceinline__ void store_plane(ST *&p, long long nn, const double *f, const double *g, uint64_t spol) {
   constexpr int QF = Lat<DIM>::QF;
   constexpr int code = pop_of_plane<DIM>(P);
-  if constexpr (code < QF) st_hint(p, (ST)(f[code] - Store<ST, DIM>::bias(code)), spol);
+  if constexpr (code < QF) st_hint(p, to_storage<ST, DIM>(f[code], code), spol);
   else st_hint(p, (ST)g[code - QF], spol);
   p += nn;
   asm volatile("" : "+l"(p));
@@ -355,8 +355,7 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
         bb_fix_all_f<3>(f, wf, src, m.nnp, c, std::make_integer_sequence<int, 18>{});
         bb_fix_all_g<3>(g, wf, src, m.nnp, c, m, std::make_integer_sequence<int, 6>{});
       }
-#pragma unroll
-      for (int q = 0; q < 19; ++q) f[q] += Store<ST, 3>::bias(q);
+      add_bias<ST, 3>(f);
       collide_node(f, g, np);
       if (valid) store_node<3>(dst + c, m.nnp, f, g, spol, std::make_integer_sequence<int, 26>{});
     } else {

@@ -60,11 +60,10 @@ k_step_shift(DevMesh m, NodeParams np, const ST *__restrict__ src, ST *__restric
   double f[QF], g[QG];
   shift_all_f<DIM>(m, src, cx, f, std::make_integer_sequence<int, QF>{});
   shift_all_g<DIM>(m, src, cx, g, std::make_integer_sequence<int, QG>{});
-#pragma unroll
-  for (int q = 0; q < QF; ++q) f[q] += Store<ST, DIM>::bias(q);
+  add_bias<ST, DIM>(f);
   collide_node(f, g, np);
 #pragma unroll
-  for (int q = 0; q < QF; ++q) dst[(long long)plane_f<DIM>(q) * m.nnp + cx.c] = (ST)(f[q] - Store<ST, DIM>::bias(q));
+  for (int q = 0; q < QF; ++q) dst[(long long)plane_f<DIM>(q) * m.nnp + cx.c] = to_storage<ST, DIM>(f[q], q);
 #pragma unroll
   for (int q = 0; q < QG; ++q) dst[(long long)plane_g<DIM>(q) * m.nnp + cx.c] = (ST)g[q];
 }
