@@ -114,7 +114,7 @@ def _dev_ptr(t, n_expected=None):
 class Islbm:
     """islbm_create / islbm_step / islbm_fields / islbm_nusselt on one CUDA device."""
 
-    def __init__(self, coords, delta, Ra, Pr, Ma, precision=F64, device="cuda", stream=None):
+    def __init__(self, coords, delta, Ra, Pr, Ma, precision=F64, device="cuda", stream=None, guard_bytes=0):
         self.dim = len(coords)
         self.precision = precision
         self.device = torch.device(device)
@@ -126,12 +126,22 @@ class Islbm:
         lattice = D2Q9_D2Q5 if self.dim == 2 else D3Q19_D3Q7
         nbytes = C.c_size_t(0)
         _check(lib.islbm_workspace_bytes(C.byref(m), lattice, precision, C.byref(nbytes)))
-        self.workspace = torch.empty(nbytes.value, dtype=torch.uint8, device=self.device)   # owned here
+        # owned here; guard_bytes (a multiple of 256) adds canary bands around the workspace for the out-of-bounds test
+        assert guard_bytes % 256 == 0
+        self.guard_bytes = guard_bytes
+        self._alloc = torch.full((nbytes.value + 2 * guard_bytes,), 0xA5, dtype=torch.uint8, device=self.device) \
+            if guard_bytes else torch.empty(nbytes.value, dtype=torch.uint8, device=self.device)
+        self.workspace = self._alloc[guard_bytes:guard_bytes + nbytes.value]
         self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         self.h = C.c_void_p()
         _check(lib.islbm_create(C.byref(self.h), C.byref(m), lattice, float(Ra), float(Pr), float(Ma), precision,
                                 C.c_void_p(self.workspace.data_ptr()), nbytes.value, C.c_void_p(self.stream.cuda_stream)))
         del keep
+
+    def guards_intact(self):
+        """True if no kernel wrote into the canary bands around the workspace."""
+        g = self.guard_bytes
+        return bool((self._alloc[:g] == 0xA5).all().item() and (self._alloc[self._alloc.numel() - g:] == 0xA5).all().item())
 
     def close(self):
         if getattr(self, "h", None):

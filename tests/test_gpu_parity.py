@@ -373,6 +373,56 @@ def test_conduction_fixed_point_on_gpu(islbm):
     assert nu["Nu_hot"] == pytest.approx(1.0, abs=1e-10) and nu["Nu_cold"] == pytest.approx(1.0, abs=1e-10)
 
 
+def test_more_than_2_pow_31_elements_per_buffer(islbm):
+    """Maximum sizes: 640 x 640 x 224 nodes = 2.39e9 stored values per buffer (> 2^31, 19 GB), so every index must be
+    64-bit.  The oracle would need 76 GB of host memory at this size; the check is the TMA kernel (tensor-map
+    coordinates) against the generic kernel (explicit 64-bit indices), which share no indexing code and are each
+    checked against the oracle at small sizes, plus size-independent properties of the state."""
+    free, _ = torch.cuda.mem_get_info()
+    if free < 110e9:
+        pytest.skip("needs 110 GB of free device memory")
+    ns = (640, 640, 224)
+    coords = [inputs.tanh_mesh(n, 1.6)[0] for n in ns]
+    delta = min(float(np.diff(c).min()) for c in coords)
+    H_lu = (coords[1][-1] - coords[1][0] + delta) / delta
+    sim = islbm.Islbm(coords, delta, 0.71 * (0.1 * H_lu / 0.03) ** 2, 0.71, 0.1 * SQ3)
+    assert sim.nodes * 26 > 2 ** 31 and sim.kernel_name == "tiled_zmarch_tma"
+    sim.init(7, 1e-3)
+    sim.step(2)
+    f_t, g_t = sim.get_populations()
+    sim.init(7, 1e-3)
+    sim.set_kernel(islbm.KERNEL_GENERIC)
+    sim.step(2)
+    f_g, g_g = sim.get_populations()
+    for a, b in ((f_t, f_g), (g_t, g_g)):
+        for q in range(a.shape[0]):
+            assert (a[q] - b[q]).abs().max().item() <= 1e-13 * max(b[q].abs().max().item(), 1e-30), q
+    del f_g, g_g
+    assert torch.isfinite(f_t).all() and torch.isfinite(g_t).all()
+    assert abs(f_t.sum(0).mean().item() - 1.0) < 1e-9                     # rho ~ 1 everywhere
+    assert (f_t[:, -1, -1, -1] > 0).all() and g_t[:, -1, -1, -1].abs().max().item() < 1.0   # the very last node was written
+
+
+@pytest.mark.parametrize("dim,ns,prec", [(2, (70, 45), 0), (2, (131, 67), 1), (2, (3, 3), 0), (3, (37, 21, 19), 0),
+                                         (3, (33, 17, 9), 1), (3, (64, 24, 40), 0), (3, (3, 3, 3), 1)])
+def test_no_kernel_writes_outside_the_workspace(islbm, dim, ns, prec):
+    """Canary bands of 1 MiB on both sides of the workspace stay intact through every kernel variant, the
+    reductions, the residual and get/set (compute-sanitizer is not available on the GPU pool)."""
+    coords, delta = ragged_coords(dim, ns + (1,), (1.3, 1.2, 1.1))
+    H_lu = (coords[1][-1] - coords[1][0] + delta) / delta
+    sim = islbm.Islbm(coords, delta, 0.71 * (0.1 * H_lu / 0.03) ** 2, 0.71, 0.1 * SQ3, precision=prec, guard_bytes=1 << 20)
+    sim.init(0, 1e-3)
+    for k, tune in kernels_for(islbm, sim):
+        select(sim, k, tune)
+        sim.step(3)
+        f, g = sim.get_populations()
+        sim.set_populations(f, g)
+        sim.step(2)
+    sim.nusselt(), sim.nusselt_middle(), sim.steady_residual(), sim.steady_residual(), sim.fields()
+    torch.cuda.synchronize()
+    assert sim.guards_intact()
+
+
 def test_state_errors_and_launch_accounting(islbm):
     w = inputs.custom_workload("s", 2, 16)
     sim = islbm.Islbm(w.coords, w.delta, w.Ra, w.Pr, w.Ma)
