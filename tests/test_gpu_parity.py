@@ -486,8 +486,9 @@ def test_paper_mode_table2_ra1e6_257(islbm, golden):
     assert nm == pytest.approx(ref[2], rel=3e-3)
     assert nu["Nu_cold"] == pytest.approx(nu["Nu_hot"], rel=2e-6)          # steady state: what enters leaves
     assert nm == pytest.approx(nu["Nu_vol"], rel=5e-4)                     # every vertical plane carries the same flux
-    # with T0 = T_cold the weakly compressible model gives <Nu> below Nu_hot, as Table 2 prints (8.8282 vs 8.8509)
-    assert 0.5 * (ref[1] - ref[0]) < nu["Nu_hot"] - nu["Nu_vol"] < 1.5 * (ref[1] - ref[0])
+    # with T0 = T_cold the estimator <Nu> = sqrt(RaPr)<u*T*> + 1 sits a resolution-independent 0.025 below the wall
+    # value (weak compressibility: <u*>_V != 0 multiplies the 0.5 offset of T*); Nu_hot itself does not depend on T0
+    assert 0.015 < nu["Nu_hot"] - nu["Nu_vol"] < 0.035
     re_rms = math.sqrt(1e6 / 0.71 * nu["u2"])
     assert re_rms == pytest.approx(ref[3], rel=3e-3)
     assert nu["Re"] < 0.8 * ref[3]                                        # Eq. 34 as printed is a different number
