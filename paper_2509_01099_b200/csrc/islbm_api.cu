@@ -462,6 +462,7 @@ extern "C" int islbm_set_tuning(islbm_t *h, const char *key, int value) {
   else if (k == "tx2d") { if (value != 0 && value != 128 && value != 224) return fail(ISLBM_ERR_ARG, "tx2d must be 0, 128 or 224"); t.tx2d = value; }
   else if (k == "serpentine") t.serpentine = value;
   else if (k == "shape3d") t.shape3d = value;
+  else if (k == "pdl") t.pdl = value;
   else return fail(ISLBM_ERR_ARG, "unknown tuning key: " + k);
   if (value < 0) return fail(ISLBM_ERR_ARG, "tuning values are non-negative");
   make_tiled_plan(h);

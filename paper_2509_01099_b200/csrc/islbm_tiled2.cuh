@@ -117,6 +117,7 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
   uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + T::BAR_OFF);
   uint64_t *empty = full + T::STAGES;
   double *wys = reinterpret_cast<double *>(smem_raw + T::W_OFF);
+  pdl_launch_dependents();
 
   const int x0 = blockIdx.x * T::TX;
   const int y0 = blockIdx.y * ychunk, y1 = min(y0 + ychunk, m.ny);
@@ -138,6 +139,7 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
 
   const uint64_t lpol = make_policy(load_policy);
   const uint64_t spol = make_policy(store_policy);
+  pdl_wait();   // everything above read only the weight tables; the population buffers are touched from here on
   if (threadIdx.x == 0) {
     tma_prefetch_desc(&mp.c2);
     tma_prefetch_desc(&mp.c4);
@@ -311,11 +313,11 @@ inline void launch2_cfg(const Plan2 &p, const int *n, const DevMesh &m, const No
   using T = typename CFG::T;
   dim3 grid((n[0] + T::TX - 1) / T::TX, (n[1] + p.ychunk - 1) / p.ychunk, 1);
   if (tn.serpentine && cur)
-    k_step_ymarch<ST, T::TX, T::STAGES, CFG::MINB, -1><<<grid, T::TX, T::SMEM_BYTES, stream>>>(
-        p.maps[cur], m, np, (const ST *)buf[cur], (ST *)buf[1 - cur], p.ychunk, tn.load_policy, tn.store_policy);
+    launch_step(k_step_ymarch<ST, T::TX, T::STAGES, CFG::MINB, -1>, grid, dim3(T::TX), T::SMEM_BYTES, stream, tn.pdl != 0,
+                p.maps[cur], m, np, (const ST *)buf[cur], (ST *)buf[1 - cur], p.ychunk, tn.load_policy, tn.store_policy);
   else
-    k_step_ymarch<ST, T::TX, T::STAGES, CFG::MINB, 1><<<grid, T::TX, T::SMEM_BYTES, stream>>>(
-        p.maps[cur], m, np, (const ST *)buf[cur], (ST *)buf[1 - cur], p.ychunk, tn.load_policy, tn.store_policy);
+    launch_step(k_step_ymarch<ST, T::TX, T::STAGES, CFG::MINB, 1>, grid, dim3(T::TX), T::SMEM_BYTES, stream, tn.pdl != 0,
+                p.maps[cur], m, np, (const ST *)buf[cur], (ST *)buf[1 - cur], p.ychunk, tn.load_policy, tn.store_policy);
 }
 
 template <typename ST>

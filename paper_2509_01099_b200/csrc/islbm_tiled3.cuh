@@ -231,6 +231,7 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
   uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + T::BAR_OFF);
   uint64_t *empty = full + T::STAGES;
   double *wzs = reinterpret_cast<double *>(smem_raw + T::W_OFF);
+  pdl_launch_dependents();
 
   // the last y-tile is pulled back inside the mesh (it recomputes a few rows of its neighbour, bit-identically),
   // so that the shifted wall stencil of row ny-1 never leaves the box
@@ -251,6 +252,7 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
   }
   __syncthreads();
 
+  pdl_wait();   // everything above read only the weight tables; the population buffers are touched from here on
   // thread 0 is also the TMA producer: it runs STAGES-1 stages ahead of the consumers
   const uint64_t lpol = make_policy(load_policy);
   const uint64_t spol = make_policy(store_policy);
@@ -434,8 +436,8 @@ inline void launch3_shape(const Plan3 &p, const int *n, const DevMesh &m, const 
                           const Tuning &tn, cudaStream_t stream) {
   using T = Tile3<ST, TX, TY>;
   dim3 grid((n[0] + T::TX - 1) / T::TX, (n[1] + T::TY - 1) / T::TY, (n[2] + p.zchunk - 1) / p.zchunk);
-  k_step_zmarch<ST, TX, TY><<<grid, T::THREADS, T::SMEM_BYTES, stream>>>(
-      p.maps[cur], m, np, (const ST *)buf[cur], (ST *)buf[1 - cur], p.zchunk, tn.load_policy, tn.store_policy);
+  launch_step(k_step_zmarch<ST, TX, TY>, grid, dim3(T::THREADS), T::SMEM_BYTES, stream, tn.pdl != 0, p.maps[cur], m, np,
+              (const ST *)buf[cur], (ST *)buf[1 - cur], p.zchunk, tn.load_policy, tn.store_policy);
 }
 
 template <typename ST>

@@ -7,6 +7,7 @@
 #include <cuda_runtime.h>
 
 #include <cstdint>
+#include <utility>
 
 namespace islbmk {
 
@@ -38,6 +39,13 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
       "r"(parity)
       : "memory");
 }
+
+// Programmatic dependent launch (PDL): a step kernel lets the next step's CTAs become resident as soon as its own
+// have all started, so their prologue (barrier init, weight staging, descriptor prefetch) and this grid's tail
+// overlap; the dependent touches the population buffers only after pdl_wait(), which returns when the
+// preceding grid has completed and its stores are visible.
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
 // L2 eviction policy: 0 normal, 1 evict_first, 2 evict_last
 __device__ __forceinline__ uint64_t make_policy(int kind) {
@@ -134,6 +142,23 @@ inline bool make_map(CUtensorMap *m, void *base, int elem_bytes, int rank, const
              promo_of(promo), CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
+// launch with or without the programmatic-stream-serialization attribute
+template <typename... KArgs, typename... Args>
+inline cudaError_t launch_step(void (*kern)(KArgs...), dim3 grid, dim3 block, size_t smem, cudaStream_t stream, bool pdl,
+                               Args &&...args) {
+  cudaLaunchConfig_t cfg{};
+  cfg.gridDim = grid;
+  cfg.blockDim = block;
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = pdl ? 1 : 0;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  return cudaLaunchKernelEx(&cfg, kern, KArgs(std::forward<Args>(args))...);
+}
+
 constexpr int pad128(int bytes) { return (bytes + 127) / 128 * 128; }
 
 // run-time knobs of the tiled kernels (islbm_set_tuning); defaults chosen from measurements (profiles/)
@@ -144,6 +169,7 @@ struct Tuning {
   int store_policy = 0; // ... of the population stores
   int tx2d = 0;         // 2-D strip width: 128 or 224; 0 = automatic
   int shape3d = 0;      // 3-D tile shape: 0 32x8, 1 64x4, 2 128x2 (x by y nodes per CTA)
+  int pdl = 1;          // programmatic dependent launch of consecutive step kernels
   int serpentine = 0;   // 2-D: reverse the CTA -> chunk map on odd steps (L2 reuse of the freshly written rows)
 };
 

@@ -62,7 +62,7 @@ def kernels_for(islbm, sim):
     try:
         sim.set_kernel(islbm.KERNEL_TILED)
         ks.append((islbm.KERNEL_TILED, {}))
-        ks.append((islbm.KERNEL_TILED, dict(chunk=5, load_policy=1, store_policy=2, l2promo=3)))
+        ks.append((islbm.KERNEL_TILED, dict(chunk=5, load_policy=1, store_policy=2, l2promo=3, pdl=0)))
         if sim.dim == 2:
             ks.append((islbm.KERNEL_TILED, dict(tx2d=128, chunk=7, serpentine=1)))
             ks.append((islbm.KERNEL_TILED, dict(tx2d=224, chunk=3)))
@@ -78,7 +78,7 @@ def kernels_for(islbm, sim):
     return ks
 
 
-DEFAULT_TUNING = dict(chunk=0, l2promo=0, load_policy=0, store_policy=0, tx2d=0, serpentine=0, shape3d=0)
+DEFAULT_TUNING = dict(chunk=0, l2promo=0, load_policy=0, store_policy=0, tx2d=0, serpentine=0, shape3d=0, pdl=1)
 
 
 def select(sim, k, tune):
