@@ -121,6 +121,10 @@ int islbm_init(islbm_t *h, unsigned long long seed, double noise_amp);
  * half of the last step on the previous buffer. */
 int islbm_set_populations(islbm_t *h, const double *f, const double *g);
 int islbm_get_populations(islbm_t *h, double *f, double *g);
+/* As islbm_set_populations with HOST arrays (pinned memory makes the copies asynchronous): the library stages them
+ * slab by slab through the Eq. 30 snapshot area of the workspace (which it invalidates) with cudaMemcpyAsync on
+ * the handle's stream.  The arrays must stay valid until the stream has passed the call. */
+int islbm_set_populations_host(islbm_t *h, const double *f, const double *g);
 
 /* Advance n time steps: n x (collide, stream + interpolate + walls). */
 int islbm_step(islbm_t *h, int n);

@@ -376,9 +376,20 @@ static void launch_load(islbm *h, const double *f, const double *g, bool generat
   ST *post = (ST *)(h->ws + h->cv.buf[h->cur]);
   const unsigned blocks = cdiv(h->nn, 256);
   if (generate)
-    k_load_state<DIM, ST, true><<<blocks, 256, 0, h->stream>>>(h->dm, h->np, nullptr, nullptr, seed, amp, pre, post);
+    k_load_state<DIM, ST, true><<<blocks, 256, 0, h->stream>>>(h->dm, h->np, nullptr, nullptr, seed, amp, pre, post, h->nn, 0, h->nn);
   else
-    k_load_state<DIM, ST, false><<<blocks, 256, 0, h->stream>>>(h->dm, h->np, f, g, 0ull, 0.0, pre, post);
+    k_load_state<DIM, ST, false><<<blocks, 256, 0, h->stream>>>(h->dm, h->np, f, g, 0ull, 0.0, pre, post, h->nn, 0, h->nn);
+  h->launches++;
+}
+
+// one staged slab of islbm_set_populations_host: nodes [c0, c0 + count), staging planes at pitch `pitch`
+template <int DIM, typename ST>
+static void launch_load_slab(islbm *h, const double *stage_f, const double *stage_g, long long pitch, long long c0,
+                             long long count) {
+  ST *pre = (ST *)(h->ws + h->cv.buf[1 - h->cur]);
+  ST *post = (ST *)(h->ws + h->cv.buf[h->cur]);
+  k_load_state<DIM, ST, false><<<cdiv(count, 256), 256, 0, h->stream>>>(h->dm, h->np, stage_f, stage_g, 0ull, 0.0, pre, post,
+                                                                      pitch, c0, count);
   h->launches++;
 }
 
@@ -401,6 +412,33 @@ extern "C" int islbm_init(islbm_t *h, unsigned long long seed, double noise_amp)
 extern "C" int islbm_set_populations(islbm_t *h, const double *f, const double *g) {
   if (!h || !f || !g) return fail(ISLBM_ERR_ARG, "NULL argument");
   return load_state(h, f, g, false, 0ull, 0.0);
+}
+
+// HOST arrays: staged through the snapshot area of the workspace (4*nn doubles) in slabs of nodes; per slab one
+// H2D copy per plane and one conversion + collision kernel, all on the handle's stream.
+extern "C" int islbm_set_populations_host(islbm_t *h, const double *f, const double *g) {
+  if (!h || !f || !g) return fail(ISLBM_ERR_ARG, "NULL argument");
+  double *stage = (double *)(h->ws + h->cv.snap);
+  long long slab = (4 * h->nn) / h->q;              // nodes per slab: q planes of `slab` doubles fit the staging area
+  if (slab < 1) return fail(ISLBM_ERR_WORKSPACE, "staging area too small");
+  if (slab > h->nn) slab = h->nn;
+  for (long long c0 = 0; c0 < h->nn; c0 += slab) {
+    const long long count = c0 + slab <= h->nn ? slab : h->nn - c0;
+    for (int q = 0; q < h->qf; ++q)
+      CUDA_TRY(cudaMemcpyAsync(stage + (long long)q * slab, f + (long long)q * h->nn + c0, sizeof(double) * count,
+                               cudaMemcpyHostToDevice, h->stream));
+    for (int q = 0; q < h->qg; ++q)
+      CUDA_TRY(cudaMemcpyAsync(stage + (long long)(h->qf + q) * slab, g + (long long)q * h->nn + c0, sizeof(double) * count,
+                               cudaMemcpyHostToDevice, h->stream));
+#define CALL(D, T) launch_load_slab<D, T>(h, stage, stage + (long long)h->qf * slab, slab, c0, count)
+    DISPATCH(h, CALL);
+#undef CALL
+  }
+  CUDA_TRY(cudaPeekAtLastError());
+  h->has_state = true;
+  h->other_is_pre = true;
+  h->snap_valid = false;
+  return ISLBM_OK;
 }
 
 template <int DIM, typename ST>

@@ -236,14 +236,19 @@ k_step_generic(DevMesh m, NodeParams np, const ST *__restrict__ src, ST *__restr
 // ---------------------------------------------------------------------------
 
 // pre-collision f,g (fp64, user arrays, or generated) -> `pre` buffer (storage
-// form, kept for islbm_get_populations) and collided -> `post` buffer.
+// form, kept for islbm_get_populations) and collided -> `post` buffer.  The
+// kernel handles the node range [c0, c0 + count); fin/gin hold that range with
+// a plane pitch of `pitch` elements (pitch = nn, c0 = 0 for whole dense arrays;
+// a staged slab for islbm_set_populations_host).
 template <int DIM, typename ST, bool GENERATE>
 __global__ void __launch_bounds__(256)
 k_load_state(DevMesh m, NodeParams np, const double *__restrict__ fin, const double *__restrict__ gin,
-             unsigned long long seed, double amp, ST *__restrict__ pre, ST *__restrict__ post) {
+             unsigned long long seed, double amp, ST *__restrict__ pre, ST *__restrict__ post, long long pitch,
+             long long c0, long long count) {
   constexpr int QF = Lat<DIM>::QF, QG = Lat<DIM>::QG;
-  const long long c = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (c >= m.nn) return;
+  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= count) return;
+  const long long c = c0 + i;
   double f[QF], g[QG];
   if (GENERATE) {
     const unsigned long long z = splitmix64_at(seed, (unsigned long long)c);
@@ -251,9 +256,9 @@ k_load_state(DevMesh m, NodeParams np, const double *__restrict__ fin, const dou
     rest_equilibrium<QF, QG>(f, g, amp * (2.0 * r - 1.0), np.a_T);
   } else {
 #pragma unroll
-    for (int q = 0; q < QF; ++q) f[q] = fin[(long long)q * m.nn + c];
+    for (int q = 0; q < QF; ++q) f[q] = fin[(long long)q * pitch + i];
 #pragma unroll
-    for (int q = 0; q < QG; ++q) g[q] = gin[(long long)q * m.nn + c];
+    for (int q = 0; q < QG; ++q) g[q] = gin[(long long)q * pitch + i];
   }
   const long long cs = sidx(m, c);
 #pragma unroll

@@ -21,7 +21,7 @@ KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED, KERNEL_UNIFORM_SHIFT = 0, 1, 2, 3
 
 EXPORTS = (
     "islbm_workspace_bytes", "islbm_create", "islbm_destroy", "islbm_get_params", "islbm_init",
-    "islbm_set_populations", "islbm_get_populations", "islbm_step", "islbm_fields", "islbm_nusselt", "islbm_nusselt_middle",
+    "islbm_set_populations", "islbm_set_populations_host", "islbm_get_populations", "islbm_step", "islbm_fields", "islbm_nusselt", "islbm_nusselt_middle",
     "islbm_steady_residual", "islbm_set_buoyancy_scale", "islbm_set_reference_temperature", "islbm_set_kernel", "islbm_set_tuning", "islbm_launch_count",
     "islbm_kernel_name", "islbm_last_error", "islbm_version",
 )
@@ -56,6 +56,7 @@ def _load():
     lib.islbm_get_params.argtypes = [vp, C.POINTER(_Params)]
     lib.islbm_init.argtypes = [vp, C.c_ulonglong, C.c_double]
     lib.islbm_set_populations.argtypes = [vp, vp, vp]
+    lib.islbm_set_populations_host.argtypes = [vp, vp, vp]
     lib.islbm_get_populations.argtypes = [vp, vp, vp]
     lib.islbm_step.argtypes = [vp, C.c_int]
     lib.islbm_fields.argtypes = [vp, vp, vp, vp, vp, vp]
@@ -187,6 +188,16 @@ class Islbm:
 
     def set_populations(self, f, g):
         _check(lib.islbm_set_populations(self.h, _dev_ptr(f, self.qf * self.nodes), _dev_ptr(g, self.qg * self.nodes)))
+
+    def set_populations_host(self, f, g):
+        """f, g: HOST torch tensors (pinned for asynchronous copies) or numpy arrays, fp64, dense [q][z][y][x]."""
+        def hp(a, n):
+            if isinstance(a, np.ndarray):
+                assert a.dtype == np.float64 and a.flags.c_contiguous and a.size == n
+                return C.c_void_p(a.ctypes.data)
+            assert (not a.is_cuda) and a.dtype == torch.float64 and a.is_contiguous() and a.numel() == n
+            return C.c_void_p(a.data_ptr())
+        _check(lib.islbm_set_populations_host(self.h, hp(f, self.qf * self.nodes), hp(g, self.qg * self.nodes)))
 
     def get_populations(self):
         f = torch.empty((self.qf,) + self.shape, dtype=torch.float64, device=self.device)
