@@ -182,6 +182,7 @@ def time_device(sim, nodes, steps, warmup, lbm_per_step, flush=None):
     """K bench steps on the device; returns (seconds total, seconds inside islbm_step, launches, last Nu)."""
     import torch
     ev = [torch.cuda.Event(enable_timing=True) for _ in range(2 * steps + 2)]
+    nus = []
     for _ in range(warmup):
         sim.step(lbm_per_step)
         nu = sim.nusselt()
@@ -194,11 +195,15 @@ def time_device(sim, nodes, steps, warmup, lbm_per_step, flush=None):
         sim.step(lbm_per_step)
         ev[2 + 2 * k].record()
         nu = sim.nusselt()
+        nus.append(nu)
     ev[-1].record()
     torch.cuda.synchronize()
     barrier()
     total = ev[0].elapsed_time(ev[-1]) * 1e-3
     in_step = sum(ev[1 + 2 * k].elapsed_time(ev[2 + 2 * k]) for k in range(steps)) * 1e-3
+    # time averages over the timed window (BASELINE.json config 3; A20: plain mean of the samples)
+    nu = dict(nu, Nu_hot_mean=sum(n["Nu_hot"] for n in nus) / len(nus), Re_mean=sum(n["Re"] for n in nus) / len(nus),
+              samples=len(nus))
     return total, in_step, sim.launch_count - l0, nu
 
 
@@ -241,6 +246,7 @@ def measure_workload(islbm, inputs, name, precision, steps, warmup, lbm_per_step
         "us_per_lbm_step": t_lbm * 1e6,
         "wctpdt_s": (total / (steps * lbm_per_step)) * p["H_lu"] / p["U"],
         "kernel": sim.kernel_name, "launches": launches, "Nu_hot": nu["Nu_hot"], "Re": nu["Re"],
+        "Nu_hot_mean": nu["Nu_hot_mean"], "Re_mean": nu["Re_mean"], "nu_samples": nu["samples"],
         "total_s": total, "in_step_s": in_step, "H_lu": p["H_lu"],
     }
     return sim, w, out
@@ -323,6 +329,7 @@ def main():
                 extras[key] = {
                     "mlups": r2["mlups"], "roofline_frac": b2 * w2.nodes / (r2["us_per_lbm_step"] * 1e-6) / 1e9 / peak,
                     "us_per_lbm_step": r2["us_per_lbm_step"], "wctpdt_s": r2["wctpdt_s"], "kernel": r2["kernel"],
+                    "Nu_hot_time_mean": r2["Nu_hot_mean"], "Re_time_mean": r2["Re_mean"], "nu_samples": r2["nu_samples"],
                     "state_bytes_per_buffer": (w2.nodes * b2) // 2}
                 s2.close()
                 del s2
@@ -357,6 +364,7 @@ def main():
                              if w.nodes * bpu > 3e8 else "state fits in L2: fraction is not an HBM fraction",
                        "parallelism": f"{world} independent cavities (replicas, no data-path collective)"},
             "wctpdt_s": r["wctpdt_s"], "Nu_hot": r["Nu_hot"], "Re": r["Re"],
+            "Nu_hot_time_mean": r["Nu_hot_mean"], "Re_time_mean": r["Re_mean"], "nu_samples": r["nu_samples"],
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": r["launches"], "clocks": clocks,
             "also": extras,
         }

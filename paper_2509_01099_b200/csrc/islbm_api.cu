@@ -492,6 +492,7 @@ extern "C" int islbm_set_kernel(islbm_t *h, int which) {
 extern "C" int islbm_set_tuning(islbm_t *h, const char *key, int value) {
   if (!h || !key) return fail(ISLBM_ERR_ARG, "NULL argument");
   const std::string k(key);
+  if (value < 0) return fail(ISLBM_ERR_ARG, "tuning values are non-negative");
   Tuning &t = h->tune;
   if (k == "chunk") t.chunk = value;
   else if (k == "l2promo") t.l2promo = value;
@@ -502,7 +503,6 @@ extern "C" int islbm_set_tuning(islbm_t *h, const char *key, int value) {
   else if (k == "shape3d") t.shape3d = value;
   else if (k == "pdl") t.pdl = value;
   else return fail(ISLBM_ERR_ARG, "unknown tuning key: " + k);
-  if (value < 0) return fail(ISLBM_ERR_ARG, "tuning values are non-negative");
   make_tiled_plan(h);
   return ISLBM_OK;
 }

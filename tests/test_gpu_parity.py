@@ -466,6 +466,26 @@ def test_state_errors_and_launch_accounting(islbm):
     assert r0 == (1.0, 1.0) and 0 < r1[1] < 10 and r1[0] >= 0
 
 
+def test_tuning_and_kernel_selection_errors(islbm):
+    w = inputs.custom_workload("e", 2, 24, stretch=1.4, Ra=1e5)
+    sim = islbm.Islbm(w.coords, w.delta, w.Ra, w.Pr, w.Ma)
+    for bad in (dict(nonsense=1), dict(tx2d=100), dict(chunk=-1)):
+        with pytest.raises(islbm.IslbmError) as e:
+            sim.set_tuning(**bad)
+        assert e.value.code == -1
+    with pytest.raises(islbm.IslbmError):
+        sim.set_kernel(7)
+    with pytest.raises(islbm.IslbmError) as e:
+        sim.set_kernel(islbm.KERNEL_UNIFORM_SHIFT)           # stretched mesh: the pure shift is not valid
+    assert "delta" in str(e.value)
+    with pytest.raises(islbm.IslbmError):
+        sim.nusselt_middle()                                  # no state yet
+    sim.init(0, 1e-3)
+    sim.set_tuning(chunk=1000)                                # clamped to the longest supported chunk
+    sim.step(3)
+    assert np.isfinite(sim.nusselt_middle())
+
+
 def test_steady_residual_matches_definition(islbm):
     """Eq. 30 on the device vs the same sums formed from islbm_fields outputs."""
     w = inputs.custom_workload("r", 2, 40, stretch=1.4, Ra=1e5)
