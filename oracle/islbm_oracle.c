@@ -46,6 +46,7 @@ struct oracle {
   double U, H_lu, nu, alpha, gbeta, tau_f, a_T, omega_bc;
   double L_eff[3];
   double T_hot, T_cold, T0, buoy;
+  int stencil; /* 0: destination-centred {j-1,j,j+1} (reading A2); 1: upwind {j-2,j-1,j} / {j,j+1,j+2} (A2 alternative) */
   /* interpolation tables: axis a, sign index s (0: c=-1, 1: c=+1) */
   int *base[3][2];
   double *wgt[3][2];
@@ -242,7 +243,10 @@ static void build_weights(oracle_t *h) {
       h->base[a][s] = (int *)malloc(sizeof(int) * (size_t)n);
       h->wgt[a][s] = (double *)malloc(sizeof(double) * 3 * (size_t)n);
       for (int j = 0; j < n; ++j) {
-        int b = j - 1;
+        /* central: {j-1,j,j+1}.  upwind (A2 alternative): the triple that ends at j on the side the population
+         * comes from, {j-2,j-1,j} for c = +1 and {j,j+1,j+2} for c = -1.  Either way the departure point lies in
+         * [x_{j-1}, x_j] (c = +1) or [x_j, x_{j+1}] (c = -1), inside the triple after clamping to the mesh. */
+        int b = h->stencil == 0 ? j - 1 : (s == 1 ? j - 2 : j);
         if (b < 0) b = 0;
         if (b > n - 3) b = n - 3;
         h->base[a][s][j] = b;
@@ -347,6 +351,19 @@ int oracle_get_threads(const oracle_t *h) { return h->nthreads; }
 /* reference temperature T0 of F = rho g beta (T - T0) y^ and of T* = (T - T0)/Delta_T.
  * Default 0 (mean of the walls, BASELINE.json); the paper's T* in [0,1] corresponds to T0 = T_cold (reading A9). */
 void oracle_set_reference_temperature(oracle_t *h, double T0) { h->T0 = T0; }
+
+/* A2 alternative stencil: rebuilds the interpolation tables.  kind 0 central (default), 1 upwind. */
+void oracle_set_stencil(oracle_t *h, int kind) {
+  for (int a = 0; a < 3; ++a) {
+    for (int s = 0; s < 2; ++s) {
+      free(h->base[a][s]);
+      free(h->wgt[a][s]);
+    }
+    free(h->avgw[a]);
+  }
+  h->stencil = kind ? 1 : 0;
+  build_weights(h);
+}
 
 void oracle_set_buoyancy_scale(oracle_t *h, double s) { h->buoy = s; }
 

@@ -55,6 +55,10 @@ int  oracle_get_threads(const oracle_t *h);
 /* reference temperature T0 of the buoyancy force and of T* (default 0; the paper's runs: T_cold, reading A9). */
 void oracle_set_reference_temperature(oracle_t *h, double T0);
 
+/* interpolation stencil: 0 destination-centred {j-1,j,j+1} (reading A2, default), 1 upwind {j-2,j-1,j} for
+ * c = +1 and {j,j+1,j+2} for c = -1 (the A2 alternative of SURVEY.md 8(f)-3).  Rebuilds the tables. */
+void oracle_set_stencil(oracle_t *h, int kind);
+
 /* test hook: scale on the buoyancy force (1 = paper; 0 = pin P5). */
 void oracle_set_buoyancy_scale(oracle_t *h, double s);
 

@@ -62,6 +62,7 @@ def load():
         "oracle_get_threads": (C.c_int, [vp]),
         "oracle_set_buoyancy_scale": (None, [vp, C.c_double]),
         "oracle_set_reference_temperature": (None, [vp, C.c_double]),
+        "oracle_set_stencil": (None, [vp, C.c_int]),
         "oracle_init": (None, [vp, C.c_ulonglong, C.c_double]),
         "oracle_set_populations": (None, [vp, _dp, _dp]),
         "oracle_get_populations": (None, [vp, _dp, _dp]),
@@ -139,6 +140,9 @@ class Oracle:
 
     def set_buoyancy_scale(self, s):
         self.lib.oracle_set_buoyancy_scale(self.h, float(s))
+
+    def set_stencil(self, kind):
+        self.lib.oracle_set_stencil(self.h, int(kind))
 
     def set_reference_temperature(self, T0):
         self.lib.oracle_set_reference_temperature(self.h, float(T0))

@@ -740,3 +740,56 @@ def test_nu_middle_of_the_conduction_state_is_one():
     f, g = _state_with(o, lin)
     o.set_populations(f, g)
     assert o.nusselt_middle() == pytest.approx(1.0, abs=1e-12)
+
+
+# ---------------------------------------------------------------------------
+# A2 alternative: upwind stencil {j-2,j-1,j} / {j,j+1,j+2}
+# ---------------------------------------------------------------------------
+@pytest.mark.parametrize("dim", [2, 3])
+def test_upwind_stencil_weights_bracket_the_departure_point_and_reproduce_quadratics(dim):
+    o, w = make(dim, 17, stretch=1.8)
+    o.set_stencil(1)
+    for axis in range(dim):
+        x = w.coords[axis]
+        n = len(x)
+        for c in (-1, 1):
+            base, wt = o.weights(axis, c)
+            for j in range(n):
+                if (j == 0 and c == 1) or (j == n - 1 and c == -1):
+                    continue
+                want = min(max(j - 2 if c == 1 else j, 0), n - 3)
+                assert base[j] == want
+                xd = x[j] - c * w.delta
+                xs = x[base[j]: base[j] + 3]
+                assert xs[0] - 1e-15 <= xd <= xs[2] + 1e-15
+                assert wt[j].sum() == pytest.approx(1.0, abs=1e-13)
+                for poly in (lambda t: 1 + 0 * t, lambda t: t, lambda t: 3 * t * t - t + 0.5):
+                    assert wt[j] @ poly(xs) == pytest.approx(float(poly(xd)), abs=1e-13)
+    o.set_stencil(0)                                           # and back: the central tables are restored
+    base, _ = o.weights(0, 1)
+    assert list(base[:4]) == [0, 0, 1, 2]
+
+
+@pytest.mark.parametrize("dim,n", [(2, 16), (3, 8)])
+def test_upwind_stencil_on_uniform_mesh_is_textbook_streaming_bitwise(dim, n):
+    o, w = make(dim, n, mesh="uniform")
+    o.set_stencil(1)
+    ef, eg = o.velocities()
+    opp_f = [int(np.where((ef == -ef[i]).all(1))[0][0]) for i in range(o.qf)]
+    fp, gp = inputs.random_state(o.shape, o.qf, o.qg, seed=6)
+    o.set_post_collision(fp, gp)
+    o.stream()
+    f, _ = o.get_populations()
+    assert np.array_equal(f, textbook_stream(fp, ef, opp_f, lambda i, a, idx, v: v))
+
+
+def test_upwind_and_central_stencils_differ_on_a_stretched_mesh_but_share_the_conduction_fixed_point():
+    w = inputs.custom_workload("s", 2, 24, stretch=1.5, Ra=1e5)
+    res = []
+    for kind in (0, 1):
+        o = Oracle(w.coords, w.delta, w.Ra, w.Pr, w.Ma)
+        o.set_stencil(kind)
+        o.init(0, 1e-3)
+        o.step(50)
+        res.append(o.fields()["T"].copy())
+    assert 1e-9 < np.abs(res[0] - res[1]).max() < 1e-2
