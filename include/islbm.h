@@ -162,6 +162,10 @@ int islbm_set_buoyancy_scale(islbm_t *h, double s); /* multiplies g*beta; 0 for 
  * weakly compressible model that breaks the centro-symmetry of the solution, which is what Table 3 prints.
  * Must be called before islbm_init / islbm_set_populations. */
 int islbm_set_reference_temperature(islbm_t *h, double T0);
+/* Interpolation stencil: 0 = destination-centred {j-1,j,j+1} (default, reading A2), 1 = upwind
+ * {j-2,j-1,j} for c = +1 and {j,j+1,j+2} for c = -1 (the A2 alternative; study mode, generic kernel only).
+ * Before islbm_init / islbm_set_populations. */
+int islbm_set_stencil(islbm_t *h, int kind);
 /* 0 = auto (fastest kernel for this mesh), 1 = generic global-memory kernel,
  * 2 = TMA-staged shared-memory kernel (y-marching in 2-D, z-marching in 3-D),
  * 3 = uniform-mesh pure-shift kernel (only valid when every spacing equals

@@ -88,6 +88,9 @@ struct islbm {
   int q, qf, qg;
   size_t st_bytes;
   double Ra, Pr, Ma, delta;
+  std::vector<double> xs[3];   // node coordinates (kept for islbm_set_stencil)
+  int stencil;                 // 0 central, 1 upwind
+  int npad;
   islbm_params prm;
   double buoy;
   double T0;               // reference temperature of the buoyancy force
@@ -181,17 +184,18 @@ static void set_node_params(islbm *h) {
 // 3-point Lagrange weights of the departure point x_j - c*delta on the
 // destination-centred stencil (A2, A3).  Offsets are
 // taken relative to x_j so that an exact unit spacing gives exactly (1,0,0)/(0,0,1).
-static void build_tables(const islbm *h, const islbm_mesh *mesh, int npad, std::vector<double> &wtab,
+static void build_tables(const islbm *h, const double *const *xs, int stencil, int npad, std::vector<double> &wtab,
                          std::vector<double> &avgw) {
   wtab.assign((size_t)18 * npad, 0.0);
   avgw.assign((size_t)3 * npad, 1.0);
   for (int a = 0; a < h->dim; ++a) {
     const int n = h->n[a];
-    const double *x = mesh->x[a];
+    const double *x = xs[a];
     for (int s = 0; s < 2; ++s) {
       const double xi = s == 0 ? h->delta : -h->delta;   // c = -1 -> +delta ; c = +1 -> -delta
       for (int j = 0; j < n; ++j) {
-        int b = j - 1 < 0 ? 0 : j - 1;
+        int b = stencil == 0 ? j - 1 : (s == 1 ? j - 2 : j);   // s = 1 is c = +1 (A2 and its alternative)
+        if (b < 0) b = 0;
         if (b > n - 3) b = n - 3;
         const double d0 = x[b] - x[j], d1 = x[b + 1] - x[j], d2 = x[b + 2] - x[j];
         double *w = &wtab[(size_t)((a * 2 + s) * 3) * npad + j];
@@ -206,6 +210,15 @@ static void build_tables(const islbm *h, const islbm_mesh *mesh, int npad, std::
       avgw[(size_t)a * npad + j] = 0.5 * (xp - xm);
     }
   }
+}
+
+static int upload_tables(islbm *h) {
+  std::vector<double> wtab, avgw;
+  const double *xs[3] = {h->xs[0].data(), h->xs[1].data(), h->xs[2].data()};
+  build_tables(h, xs, h->stencil, h->npad, wtab, avgw);
+  CUDA_TRY(cudaMemcpy(h->ws + h->cv.wtab, wtab.data(), wtab.size() * sizeof(double), cudaMemcpyHostToDevice));
+  CUDA_TRY(cudaMemcpy(h->ws + h->cv.avgw, avgw.data(), avgw.size() * sizeof(double), cudaMemcpyHostToDevice));
+  return ISLBM_OK;
 }
 
 extern "C" int islbm_create(islbm_t **out, const islbm_mesh *mesh, int lattice, double Ra, double Pr, double Ma,
@@ -261,15 +274,11 @@ extern "C" int islbm_create(islbm_t **out, const islbm_mesh *mesh, int lattice, 
   }
   h->ws = (char *)dev_workspace;
   h->stream = (cudaStream_t)cuda_stream;
-  std::vector<double> wtab, avgw;
-  build_tables(h, mesh, npad, wtab, avgw);
-  cudaError_t e = cudaMemcpy(h->ws + h->cv.wtab, wtab.data(), wtab.size() * sizeof(double), cudaMemcpyHostToDevice);
-  if (e == cudaSuccess)
-    e = cudaMemcpy(h->ws + h->cv.avgw, avgw.data(), avgw.size() * sizeof(double), cudaMemcpyHostToDevice);
-  if (e != cudaSuccess) {
-    delete h;
-    return fail(ISLBM_ERR_CUDA, std::string("table upload: ") + cudaGetErrorString(e));
-  }
+  for (int a = 0; a < h->dim; ++a) h->xs[a].assign(mesh->x[a], mesh->x[a] + h->n[a]);
+  h->stencil = 0;
+  h->npad = npad;
+  rc = upload_tables(h);
+  if (rc) { delete h; return rc; }
   DevMesh &dm = h->dm;
   dm.nx = h->n[0]; dm.ny = h->n[1]; dm.nz = h->n[2];
   dm.npad = npad;
@@ -281,6 +290,7 @@ extern "C" int islbm_create(islbm_t **out, const islbm_mesh *mesh, int lattice, 
   dm.omega_bc = h->prm.omega_bc;
   dm.T_hot = 0.5;      // PAPER.md:237, 430; BASELINE.json configs (A11)
   dm.T_cold = -0.5;
+  dm.stencil = 0;
   h->dp.q_lo = (mesh->x[0][1] - mesh->x[0][0]) / mesh->delta;
   h->dp.q_hi = (mesh->x[0][h->n[0] - 1] - mesh->x[0][h->n[0] - 2]) / mesh->delta;
   h->dp.T0 = h->T0;
@@ -347,6 +357,18 @@ extern "C" int islbm_set_reference_temperature(islbm_t *h, double T0) {
   h->T0 = T0;
   set_node_params(h);
   return ISLBM_OK;
+}
+
+extern "C" int islbm_set_stencil(islbm_t *h, int kind) {
+  if (!h) return fail(ISLBM_ERR_ARG, "NULL handle");
+  if (kind != 0 && kind != 1) return fail(ISLBM_ERR_ARG, "stencil must be 0 (central) or 1 (upwind)");
+  if (h->has_state && kind != h->stencil)
+    return fail(ISLBM_ERR_STATE, "set the stencil before islbm_init / islbm_set_populations");
+  if (kind == 1 && h->kernel_choice == 2) return fail(ISLBM_ERR_ARG, "the TMA kernels take the central stencil only");
+  h->stencil = kind;
+  h->dm.stencil = kind;
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  return upload_tables(h);
 }
 
 extern "C" long long islbm_launch_count(const islbm_t *h) { return h ? h->launches : 0; }
@@ -467,6 +489,7 @@ static void launch_shift_step(islbm *h) {
 }
 
 static int effective_kernel(const islbm *h) {
+  if (h->stencil != 0 && h->kernel_choice != 3) return 1;   // only the generic kernel reads a 2-node upwind stencil
   if (h->kernel_choice != 0) return h->kernel_choice;
   return h->tiled_ok() ? 2 : 1;
 }
@@ -483,6 +506,7 @@ extern "C" const char *islbm_kernel_name(const islbm_t *h) {
 extern "C" int islbm_set_kernel(islbm_t *h, int which) {
   if (!h) return fail(ISLBM_ERR_ARG, "NULL handle");
   if (which < 0 || which > 3) return fail(ISLBM_ERR_ARG, "kernel selector must be 0..3");
+  if (which == 2 && h->stencil != 0) return fail(ISLBM_ERR_ARG, "the TMA kernels take the central stencil only");
   if (which == 2 && !h->tiled_ok()) return fail(ISLBM_ERR_ARG, std::string("tiled kernel not available: ") + h->tiled_why_not());
   if (which == 3 && !h->uniform) return fail(ISLBM_ERR_ARG, "uniform-shift kernel needs every spacing to equal delta");
   h->kernel_choice = which;

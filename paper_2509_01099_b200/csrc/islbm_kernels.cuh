@@ -35,6 +35,8 @@ struct DevMesh {
   const double *avgw;    // Eq. 29 weights, [axis 3][npad]
   double omega_bc;       // Eq. 22 weight
   double T_hot, T_cold;  // x-lo / x-hi wall temperatures
+  int stencil;           // 0: {j-1,j,j+1} (A2); 1: upwind {j-2,j-1,j} for c=+1, {j,j+1,j+2} for c=-1
+                         // (generic kernel only; the TMA kernels stage a 1-node halo and take stencil 0)
 };
 
 // workspace (padded-row) index of dense node index c
@@ -89,7 +91,7 @@ __device__ __forceinline__ unsigned long long splitmix64_at(unsigned long long s
 template <int DIM>
 struct NodeCtx {
   int i[3];        // node index
-  int b[3];        // stencil base per axis
+  int b[3][2];     // stencil base per axis and sign (0: c=-1, 1: c=+1)
   bool lo[3], hi[3];
   double w[3][2][3];
   long long c;     // workspace index (padded rows)
@@ -107,14 +109,15 @@ __device__ __forceinline__ void make_ctx(const DevMesh &m, int ix, int iy, int i
     if (a < DIM) {
       cx.lo[a] = cx.i[a] == 0;
       cx.hi[a] = cx.i[a] == n[a] - 1;
-      cx.b[a] = min(max(cx.i[a] - 1, 0), n[a] - 3);
+      cx.b[a][0] = min(max(m.stencil ? cx.i[a] : cx.i[a] - 1, 0), n[a] - 3);
+      cx.b[a][1] = min(max(m.stencil ? cx.i[a] - 2 : cx.i[a] - 1, 0), n[a] - 3);
 #pragma unroll
       for (int s = 0; s < 2; ++s)
 #pragma unroll
         for (int k = 0; k < 3; ++k) cx.w[a][s][k] = __ldg(wrow(m, a, s, k) + cx.i[a]);
     } else {
       cx.lo[a] = cx.hi[a] = false;
-      cx.b[a] = 0;
+      cx.b[a][0] = cx.b[a][1] = 0;
     }
   }
 }
@@ -139,9 +142,9 @@ __device__ __forceinline__ double interp_plane(const DevMesh &m, const ST *__res
                                                const NodeCtx<DIM> &cx) {
   constexpr int CX = EX != 0 ? 3 : 1, CY = EY != 0 ? 3 : 1, CZ = (DIM == 3 && EZ != 0) ? 3 : 1;
   constexpr int SX = EX > 0 ? 1 : 0, SY = EY > 0 ? 1 : 0, SZ = EZ > 0 ? 1 : 0;
-  const int x0 = EX != 0 ? cx.b[0] : cx.i[0];
-  const int y0 = EY != 0 ? cx.b[1] : cx.i[1];
-  const int z0 = (DIM == 3 && EZ != 0) ? cx.b[2] : cx.i[2];
+  const int x0 = EX != 0 ? cx.b[0][SX] : cx.i[0];
+  const int y0 = EY != 0 ? cx.b[1][SY] : cx.i[1];
+  const int z0 = (DIM == 3 && EZ != 0) ? cx.b[2][SZ] : cx.i[2];
   double accz = 0.0;
 #pragma unroll
   for (int kz = 0; kz < CZ; ++kz) {

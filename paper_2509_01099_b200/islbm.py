@@ -22,7 +22,7 @@ KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED, KERNEL_UNIFORM_SHIFT = 0, 1, 2, 3
 EXPORTS = (
     "islbm_workspace_bytes", "islbm_create", "islbm_destroy", "islbm_get_params", "islbm_init",
     "islbm_set_populations", "islbm_set_populations_host", "islbm_get_populations", "islbm_step", "islbm_fields", "islbm_nusselt", "islbm_nusselt_middle",
-    "islbm_steady_residual", "islbm_set_buoyancy_scale", "islbm_set_reference_temperature", "islbm_set_kernel", "islbm_set_tuning", "islbm_launch_count",
+    "islbm_steady_residual", "islbm_set_buoyancy_scale", "islbm_set_reference_temperature", "islbm_set_stencil", "islbm_set_kernel", "islbm_set_tuning", "islbm_launch_count",
     "islbm_kernel_name", "islbm_last_error", "islbm_version",
 )
 
@@ -65,6 +65,7 @@ def _load():
     lib.islbm_steady_residual.argtypes = [vp, dp]
     lib.islbm_set_buoyancy_scale.argtypes = [vp, C.c_double]
     lib.islbm_set_reference_temperature.argtypes = [vp, C.c_double]
+    lib.islbm_set_stencil.argtypes = [vp, C.c_int]
     lib.islbm_set_kernel.argtypes = [vp, C.c_int]
     lib.islbm_set_tuning.argtypes = [vp, C.c_char_p, C.c_int]
     lib.islbm_launch_count.argtypes = [vp]
@@ -167,6 +168,9 @@ class Islbm:
 
     def set_reference_temperature(self, T0):
         _check(lib.islbm_set_reference_temperature(self.h, float(T0)))
+
+    def set_stencil(self, kind):
+        _check(lib.islbm_set_stencil(self.h, int(kind)))
 
     def set_kernel(self, which):
         _check(lib.islbm_set_kernel(self.h, int(which)))

@@ -195,6 +195,30 @@ def test_set_populations_host_equals_device_path(islbm, dim, ns, prec):
     assert b.steady_residual() == (1.0, 1.0)                 # the upload invalidated the Eq. 30 snapshot
 
 
+@pytest.mark.parametrize("dim,ns", [(2, (70, 45, 1)), (2, (3, 5, 1)), (3, (37, 21, 19)), (3, (4, 3, 6))])
+def test_upwind_stencil_parity(islbm, dim, ns):
+    """A2 alternative ({j-2,j-1,j} / {j,j+1,j+2}): generic kernel against the oracle's table-driven stream."""
+    coords, delta = ragged_coords(dim, ns, (1.4, 1.2, 1.3))
+    H_lu = (coords[1][-1] - coords[1][0] + delta) / delta
+    sim, orc = pair(islbm, coords, delta, Ra=0.71 * (0.1 * H_lu / 0.03) ** 2)
+    sim.set_stencil(1)
+    orc.set_stencil(1)
+    assert sim.kernel_name == "generic_global"
+    with pytest.raises(islbm.IslbmError):
+        sim.set_kernel(islbm.KERNEL_TILED)
+    f0, g0 = inputs.random_state(orc.shape, orc.qf, orc.qg, seed=3, amp=0.05)
+    orc.set_populations(f0, g0)
+    sim.set_populations(torch.from_numpy(f0).cuda(), torch.from_numpy(g0).cuda())
+    for n, tol in ((1, 1e-12), (2, 3e-12)):
+        sim.step(n)
+        orc.step(n)
+        f1, g1 = sim.get_populations()
+        fo, go = orc.get_populations()
+        assert plane_err(f1.cpu().numpy(), fo) <= tol and plane_err(g1.cpu().numpy(), go) <= tol
+    with pytest.raises(islbm.IslbmError):
+        sim.set_stencil(0)                      # the state exists: too late
+
+
 def test_uniform_mesh_one_step(islbm):
     for dim, n in ((2, 32), (3, 16)):
         w = inputs.custom_workload("u", dim, n, mesh="uniform", Ra=1e4)
