@@ -356,7 +356,7 @@ def main():
         line = {
             "metric": METRIC, "value": value, "unit": "MLUPS", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": t_max / args.steps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64" if prec == 0 else "f64 arithmetic, f32 storage", "data": "synthetic",
+            "dtype": "f64" if prec == 0 else "f64 collision, f32 storage and stencil interpolation", "data": "synthetic",
             "config": {"workload": args.workload, "nodes_per_gpu": w.nodes, "lattice": "D2Q9+D2Q5" if w.dim == 2 else "D3Q19+D3Q7",
                        "mesh": f"{w.mesh} stretch {w.stretch}", "Ra": w.Ra, "Pr": w.Pr, "U_lu": 0.1,
                        "step": f"{args.lbm_per_step} LBM time steps + 1 Nu/Re reduction",

@@ -60,6 +60,10 @@ typedef struct {
 } islbm_mesh;
 
 enum { ISLBM_D2Q9_D2Q5 = 0, ISLBM_D3Q19_D3Q7 = 1 };
+/* ISLBM_F32_STORAGE: the workspace holds f_q - w_q and g_q as fp32; the TMA kernels interpolate those stored
+ * deviations in fp32 (one or two more fp32 roundings of the deviation per step, the size of the storage rounding
+ * itself) and collide in fp64; everything else (API arrays, diagnostics, weights) is fp64.  Tolerance against the
+ * fp64 oracle: 1e-5 on u and T after 1000 steps (BASELINE.json). */
 enum { ISLBM_F64 = 0, ISLBM_F32_STORAGE = 1 };
 
 enum {

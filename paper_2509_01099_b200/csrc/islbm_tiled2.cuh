@@ -85,10 +85,10 @@ __device__ __forceinline__ void issue_stage2(int s, int yf, int ny, int x0, unsi
 //   index: 0 f2, 1 f4, 2 g2, 3 g4, 4 f5, 5 f6, 6 f7, 7 f8
 #define ISLBM_LOAD_M2(S)                                     \
   do {                                                       \
-    S[0] = (double)PC4(0)[tx];               /* f2 */        \
-    S[1] = (double)PC4(1)[tx];               /* f4 */        \
-    S[2] = (double)PC4(2)[tx];               /* g2 */        \
-    S[3] = (double)PC4(3)[tx];               /* g4 */        \
+    S[0] = (AT)PC4(0)[tx];                   /* f2 */        \
+    S[1] = (AT)PC4(1)[tx];                   /* f4 */        \
+    S[2] = (AT)PC4(2)[tx];                   /* g2 */        \
+    S[3] = (AT)PC4(3)[tx];                   /* g4 */        \
     S[4] = tap3(PXM(0) + o_x, 1, wx[1]);     /* f5 ( 1, 1) */ \
     S[5] = tap3(PXM(1) + o_x, 1, wx[0]);     /* f6 (-1, 1) */ \
     S[6] = tap3(PXM(2) + o_x, 1, wx[0]);     /* f7 (-1,-1) */ \
@@ -97,14 +97,14 @@ __device__ __forceinline__ void issue_stage2(int s, int yf, int ny, int x0, unsi
 // y-direction of the separable interpolation; (P0,P1,P2) = stencil rows in ascending y
 #define ISLBM_YCOMB2(P0, P1, P2)                 \
   do {                                           \
-    f[2] = comb3(wy[1], P0[0], P1[0], P2[0]);    \
-    f[4] = comb3(wy[0], P0[1], P1[1], P2[1]);    \
-    g[2] = comb3(wy[1], P0[2], P1[2], P2[2]);    \
-    g[4] = comb3(wy[0], P0[3], P1[3], P2[3]);    \
-    f[5] = comb3(wy[1], P0[4], P1[4], P2[4]);    \
-    f[6] = comb3(wy[1], P0[5], P1[5], P2[5]);    \
-    f[7] = comb3(wy[0], P0[6], P1[6], P2[6]);    \
-    f[8] = comb3(wy[0], P0[7], P1[7], P2[7]);    \
+    f[2] = (double)comb3(wy[1], P0[0], P1[0], P2[0]);    \
+    f[4] = (double)comb3(wy[0], P0[1], P1[1], P2[1]);    \
+    g[2] = (double)comb3(wy[1], P0[2], P1[2], P2[2]);    \
+    g[4] = (double)comb3(wy[0], P0[3], P1[3], P2[3]);    \
+    f[5] = (double)comb3(wy[1], P0[4], P1[4], P2[4]);    \
+    f[6] = (double)comb3(wy[1], P0[5], P1[5], P2[5]);    \
+    f[7] = (double)comb3(wy[0], P0[6], P1[6], P2[6]);    \
+    f[8] = (double)comb3(wy[0], P0[7], P1[7], P2[7]);    \
   } while (0)
 
 template <typename ST, int TX, int STAGES, int MINB, int DIR>
@@ -112,11 +112,12 @@ __global__ void __launch_bounds__(TX, MINB)
 k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const ST *__restrict__ src, ST *__restrict__ dst,
               int ychunk, int load_policy, int store_policy) {
   using T = Tile2<ST, TX, STAGES>;
+  using AT = typename Acc<ST>::type;   // fp32 storage interpolates the stored deviations in fp32 (islbm_tiled3.cuh)
   extern __shared__ __align__(128) unsigned char smem_raw[];
   unsigned char *stage0 = smem_raw;
   uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + T::BAR_OFF);
   uint64_t *empty = full + T::STAGES;
-  double *wys = reinterpret_cast<double *>(smem_raw + T::W_OFF);
+  AT *wys = reinterpret_cast<AT *>(smem_raw + T::W_OFF);
   pdl_launch_dependents();
 
   const int x0 = blockIdx.x * T::TX;
@@ -125,7 +126,7 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
   const int nstage = 2 + (y1 - y0);
   for (int i = threadIdx.x; i < 6 * (y1 - y0); i += T::TX) {
     const int sk = i / (y1 - y0), yi = i - sk * (y1 - y0);
-    wys[sk * kMaxChunk + yi] = __ldg(wrow(m, 1, sk / 3, sk % 3) + y0 + yi);
+    wys[sk * kMaxChunk + yi] = (AT)__ldg(wrow(m, 1, sk / 3, sk % 3) + y0 + yi);
   }
 
   if (threadIdx.x == 0) {
@@ -157,15 +158,15 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
   const bool wall_x = wf.lo[0] | wf.hi[0];
   const int sx = wf.lo[0] ? 1 : (wf.hi[0] ? -1 : 0);
   const int o_x = tx + T::XH - 1 + sx;
-  double wx[2][3];
+  AT wx[2][3];
 #pragma unroll
   for (int s = 0; s < 2; ++s)
 #pragma unroll
-    for (int k = 0; k < 3; ++k) wx[s][k] = valid ? __ldg(wrow(m, 0, s, k) + x) : 0.0;
+    for (int k = 0; k < 3; ++k) wx[s][k] = valid ? (AT)__ldg(wrow(m, 0, s, k) + x) : (AT)0;
 
   // three register sets hold the y-stencil rows; `newest` names the one written last, so the marching order
   // (oldest first) is (newest+1, newest+2, newest) mod 3 and nothing is ever copied between sets
-  double S0[8], S1[8], S2[8];
+  AT S0[8], S1[8], S2[8];
   int newest = 2;
 
 #pragma unroll 1
@@ -193,7 +194,7 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
     }
 
     if (has_emit) {
-      double wy[2][3];
+      AT wy[2][3];
 #pragma unroll
       for (int sg = 0; sg < 2; ++sg)
 #pragma unroll
@@ -201,10 +202,10 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
       double f[9], g[5];
       f[0] = (double)PC2(0)[tx];
       g[0] = (double)PC2(1)[tx];
-      f[1] = tap3(PXR(0) + o_x, 1, wx[1]);
-      f[3] = tap3(PXR(1) + o_x, 1, wx[0]);
-      g[1] = tap3(PXR(2) + o_x, 1, wx[1]);
-      g[3] = tap3(PXR(3) + o_x, 1, wx[0]);
+      f[1] = (double)tap3(PXR(0) + o_x, 1, wx[1]);
+      f[3] = (double)tap3(PXR(1) + o_x, 1, wx[0]);
+      g[1] = (double)tap3(PXR(2) + o_x, 1, wx[1]);
+      g[3] = (double)tap3(PXR(3) + o_x, 1, wx[0]);
       __syncwarp();
       if ((threadIdx.x & 31) == 0) mbar_arrive(&empty[st]);
       // ascending-y order of the stencil rows: the marching order when DIR = +1, its reverse when DIR = -1

@@ -74,20 +74,29 @@ struct Maps3 {
 };
 
 // ------------------------------ device helpers -----------------------------
+// Arithmetic type of the stencil interpolation: fp64 for fp64 storage (bit-compatible with the oracle's order of
+// operations).  For fp32 storage the stored deviations f_q - w_q are interpolated in fp32 and converted once per
+// population: the result then carries one or two more fp32 roundings of the deviation, the same size as the storage
+// rounding itself, and the node needs 52 instead of 116 conversions between 32- and 64-bit floats, which issue at a
+// quarter of the fp64 rate and were the bottleneck of the fp32-storage path (profiles/).  Collision: always fp64.
+template <typename ST> struct Acc { using type = double; };
+template <> struct Acc<float> { using type = float; };
+
 // 3-point sums in the oracle's order: ((w0*v0) + w1*v1) + w2*v2
-template <typename ST>
-__device__ __forceinline__ double tap3(const ST *__restrict__ s, int stride, const double (&w)[3]) {
-  double a = w[0] * (double)s[0];
-  a = fma(w[1], (double)s[stride], a);
-  return fma(w[2], (double)s[2 * stride], a);
+template <typename ST, typename AT>
+__device__ __forceinline__ AT tap3(const ST *__restrict__ s, int stride, const AT (&w)[3]) {
+  AT a = w[0] * (AT)s[0];
+  a = fma(w[1], (AT)s[stride], a);
+  return fma(w[2], (AT)s[2 * stride], a);
 }
-template <typename ST>
-__device__ __forceinline__ double tap9(const ST *__restrict__ s, int pitch, const double (&wx)[3], const double (&wy)[3]) {
-  double a = wy[0] * tap3(s, 1, wx);
+template <typename ST, typename AT>
+__device__ __forceinline__ AT tap9(const ST *__restrict__ s, int pitch, const AT (&wx)[3], const AT (&wy)[3]) {
+  AT a = wy[0] * tap3(s, 1, wx);
   a = fma(wy[1], tap3(s + pitch, 1, wx), a);
   return fma(wy[2], tap3(s + 2 * pitch, 1, wx), a);
 }
-__device__ __forceinline__ double comb3(const double (&w)[3], double a, double b, double c) {
+template <typename AT>
+__device__ __forceinline__ AT comb3(const AT (&w)[3], AT a, AT b, AT c) {
   return fma(w[2], c, fma(w[1], b, w[0] * a));
 }
 
@@ -191,8 +200,8 @@ __device__ __forceinline__ void issue_stage3(int s, int z0, int nz, int x0, int 
 //   index: 0 f5, 1 f6, 2..5 f11..f14, 6..9 f15..f18, 10 g5, 11 g6
 #define ISLBM_LOAD_M3(S)                                        \
   do {                                                          \
-    S[0] = (double)PC4(0)[o_c];                 /* f5 */        \
-    S[1] = (double)PC4(1)[o_c];                 /* f6 */        \
+    S[0] = (AT)PC4(0)[o_c];                     /* f5 */        \
+    S[1] = (AT)PC4(1)[o_c];                     /* f6 */        \
     S[2] = tap3(PXM(0) + o_x, 1, wx[1]);        /* f11 ( 1,0, 1) */ \
     S[3] = tap3(PXM(1) + o_x, 1, wx[0]);        /* f12 (-1,0, 1) */ \
     S[4] = tap3(PXM(2) + o_x, 1, wx[1]);        /* f13 ( 1,0,-1) */ \
@@ -201,24 +210,24 @@ __device__ __forceinline__ void issue_stage3(int s, int z0, int nz, int x0, int 
     S[7] = tap3(PYM(1) + o_y, T::TX, wy[0]);    /* f16 (0,-1, 1) */ \
     S[8] = tap3(PYM(2) + o_y, T::TX, wy[1]);    /* f17 (0, 1,-1) */ \
     S[9] = tap3(PYM(3) + o_y, T::TX, wy[0]);    /* f18 (0,-1,-1) */ \
-    S[10] = (double)PC4(2)[o_c];                /* g5 */        \
-    S[11] = (double)PC4(3)[o_c];                /* g6 */        \
+    S[10] = (AT)PC4(2)[o_c];                    /* g5 */        \
+    S[11] = (AT)PC4(3)[o_c];                    /* g6 */        \
   } while (0)
 // z-direction of the separable interpolation; (P0,P1,P2) = stencil slices in ascending z
 #define ISLBM_ZCOMB3(P0, P1, P2)                  \
   do {                                            \
-    f[5] = comb3(wz[1], P0[0], P1[0], P2[0]);     \
-    f[6] = comb3(wz[0], P0[1], P1[1], P2[1]);     \
-    f[11] = comb3(wz[1], P0[2], P1[2], P2[2]);    \
-    f[12] = comb3(wz[1], P0[3], P1[3], P2[3]);    \
-    f[13] = comb3(wz[0], P0[4], P1[4], P2[4]);    \
-    f[14] = comb3(wz[0], P0[5], P1[5], P2[5]);    \
-    f[15] = comb3(wz[1], P0[6], P1[6], P2[6]);    \
-    f[16] = comb3(wz[1], P0[7], P1[7], P2[7]);    \
-    f[17] = comb3(wz[0], P0[8], P1[8], P2[8]);    \
-    f[18] = comb3(wz[0], P0[9], P1[9], P2[9]);    \
-    g[5] = comb3(wz[1], P0[10], P1[10], P2[10]);  \
-    g[6] = comb3(wz[0], P0[11], P1[11], P2[11]);  \
+    f[5] = (double)comb3(wz[1], P0[0], P1[0], P2[0]);     \
+    f[6] = (double)comb3(wz[0], P0[1], P1[1], P2[1]);     \
+    f[11] = (double)comb3(wz[1], P0[2], P1[2], P2[2]);    \
+    f[12] = (double)comb3(wz[1], P0[3], P1[3], P2[3]);    \
+    f[13] = (double)comb3(wz[0], P0[4], P1[4], P2[4]);    \
+    f[14] = (double)comb3(wz[0], P0[5], P1[5], P2[5]);    \
+    f[15] = (double)comb3(wz[1], P0[6], P1[6], P2[6]);    \
+    f[16] = (double)comb3(wz[1], P0[7], P1[7], P2[7]);    \
+    f[17] = (double)comb3(wz[0], P0[8], P1[8], P2[8]);    \
+    f[18] = (double)comb3(wz[0], P0[9], P1[9], P2[9]);    \
+    g[5] = (double)comb3(wz[1], P0[10], P1[10], P2[10]);  \
+    g[6] = (double)comb3(wz[0], P0[11], P1[11], P2[11]);  \
   } while (0)
 
 template <typename ST, int TX, int TY>
@@ -226,11 +235,12 @@ __global__ void __launch_bounds__(TX * TY, 1)
 k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const ST *__restrict__ src,
               ST *__restrict__ dst, int zchunk, int load_policy, int store_policy) {
   using T = Tile3<ST, TX, TY>;
+  using AT = typename Acc<ST>::type;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   unsigned char *stage0 = smem_raw;
   uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + T::BAR_OFF);
   uint64_t *empty = full + T::STAGES;
-  double *wzs = reinterpret_cast<double *>(smem_raw + T::W_OFF);
+  AT *wzs = reinterpret_cast<AT *>(smem_raw + T::W_OFF);
   pdl_launch_dependents();
 
   // the last y-tile is pulled back inside the mesh (it recomputes a few rows of its neighbour, bit-identically),
@@ -240,7 +250,7 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
   const int nstage = 2 + (z1 - z0);
   for (int i = threadIdx.x; i < 6 * (z1 - z0); i += T::THREADS) {
     const int sk = i / (z1 - z0), zi = i - sk * (z1 - z0);
-    wzs[sk * kMaxChunk + zi] = __ldg(wrow(m, 2, sk / 3, sk % 3) + z0 + zi);
+    wzs[sk * kMaxChunk + zi] = (AT)__ldg(wrow(m, 2, sk / 3, sk % 3) + z0 + zi);
   }
 
   if (threadIdx.x == 0) {
@@ -280,20 +290,20 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
   const int o_x = ty * T::HX + (tx + T::XH - 1 + sx);            // x-stencil, taps +0,+1,+2
   const int o_y = (ty + sy) * T::TX + tx;                        // y-stencil, taps +0,+TX,+2TX
   const int o_c = ty * T::TX + tx;
-  double wx[2][3], wy[2][3];
+  AT wx[2][3], wy[2][3];
 #pragma unroll
   for (int s = 0; s < 2; ++s)
 #pragma unroll
     for (int k = 0; k < 3; ++k) {
-      wx[s][k] = valid ? __ldg(wrow(m, 0, s, k) + x) : 0.0;
-      wy[s][k] = valid ? __ldg(wrow(m, 1, s, k) + y) : 0.0;
+      wx[s][k] = valid ? (AT)__ldg(wrow(m, 0, s, k) + x) : (AT)0;
+      wy[s][k] = valid ? (AT)__ldg(wrow(m, 1, s, k) + y) : (AT)0;
     }
   const long long plane = (long long)m.nxp * m.ny;
   const long long cxy = (long long)y * m.nxp + x;
 
   // three register sets hold the z-stencil slices; `newest` names the one written last, so the ascending-z
   // order is (newest+1, newest+2, newest) mod 3 and nothing is ever copied between sets
-  double S0[12], S1[12], S2[12];
+  AT S0[12], S1[12], S2[12];
   int newest = 2;
 
 #pragma unroll 1
@@ -324,7 +334,7 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
     }
 
     if (has_emit) {
-      double wz[2][3];
+      AT wz[2][3];
 #pragma unroll
       for (int sg = 0; sg < 2; ++sg)
 #pragma unroll
@@ -332,18 +342,18 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
       double f[19], g[7];
       f[0] = (double)PC2(0)[o_c];
       g[0] = (double)PC2(1)[o_c];
-      f[1] = tap3(PXZ(0) + o_x, 1, wx[1]);
-      f[2] = tap3(PXZ(1) + o_x, 1, wx[0]);
-      g[1] = tap3(PXZ(2) + o_x, 1, wx[1]);
-      g[2] = tap3(PXZ(3) + o_x, 1, wx[0]);
-      f[3] = tap3(PYZ(0) + o_y, T::TX, wy[1]);
-      f[4] = tap3(PYZ(1) + o_y, T::TX, wy[0]);
-      g[3] = tap3(PYZ(2) + o_y, T::TX, wy[1]);
-      g[4] = tap3(PYZ(3) + o_y, T::TX, wy[0]);
-      f[7] = tap9(PXY(0) + o_xy, T::HX, wx[1], wy[1]);
-      f[8] = tap9(PXY(1) + o_xy, T::HX, wx[0], wy[1]);
-      f[9] = tap9(PXY(2) + o_xy, T::HX, wx[1], wy[0]);
-      f[10] = tap9(PXY(3) + o_xy, T::HX, wx[0], wy[0]);
+      f[1] = (double)tap3(PXZ(0) + o_x, 1, wx[1]);
+      f[2] = (double)tap3(PXZ(1) + o_x, 1, wx[0]);
+      g[1] = (double)tap3(PXZ(2) + o_x, 1, wx[1]);
+      g[2] = (double)tap3(PXZ(3) + o_x, 1, wx[0]);
+      f[3] = (double)tap3(PYZ(0) + o_y, T::TX, wy[1]);
+      f[4] = (double)tap3(PYZ(1) + o_y, T::TX, wy[0]);
+      g[3] = (double)tap3(PYZ(2) + o_y, T::TX, wy[1]);
+      g[4] = (double)tap3(PYZ(3) + o_y, T::TX, wy[0]);
+      f[7] = (double)tap9(PXY(0) + o_xy, T::HX, wx[1], wy[1]);
+      f[8] = (double)tap9(PXY(1) + o_xy, T::HX, wx[0], wy[1]);
+      f[9] = (double)tap9(PXY(2) + o_xy, T::HX, wx[1], wy[0]);
+      f[10] = (double)tap9(PXY(3) + o_xy, T::HX, wx[0], wy[0]);
       // all shared-memory reads of this stage are done: hand the slot back to the producer
       __syncwarp();
       if ((threadIdx.x & 31) == 0) mbar_arrive(&empty[st]);
