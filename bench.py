@@ -252,6 +252,67 @@ def measure_workload(islbm, inputs, name, precision, steps, warmup, lbm_per_step
     return sim, w, out
 
 
+def run_slab(args):
+    """--decomp slab: ONE cavity decomposed into z-slabs (y-slabs in 2-D), one rank per GPU, a halo exchange of one
+    layer of the planes with a velocity component along the slab axis after every time step (torch.distributed
+    point-to-point over NCCL) and an all-reduce of 8 doubles per Nu/Re reduction: strong scaling.  The default
+    multi-GPU mode stays `replicas` (BASELINE.json: everything runs on one GPU)."""
+    import torch
+    from paper_2509_01099_b200 import inputs, slab
+
+    rank, world, local = dist_setup(args.gpus)
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    prec = 0 if args.precision == "f64" else 1
+    w = inputs.workload(args.workload)
+    cav = slab.SlabCavity(w.coords, w.delta, w.Ra, w.Pr, w.Ma, rank, world, precision=prec, device=dev)
+    cav.init(w.seed, w.noise_amp)
+    sampler = ClockSampler(local) if rank == 0 else None
+    for _ in range(args.warmup):
+        cav.step(args.lbm_per_step)
+        nu = cav.diagnostics()
+    torch.cuda.synchronize()
+    barrier()
+    l0 = cav.sim.launch_count
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(args.steps):
+        cav.step(args.lbm_per_step)
+        nu = cav.diagnostics()
+    e1.record()
+    torch.cuda.synchronize()
+    barrier()
+    t_local = e0.elapsed_time(e1) * 1e-3
+    clocks = sampler.stop() if sampler else None
+    t_max, _ = dist_max_sum(t_local, 0.0, dev)
+    units = float(w.nodes) * args.steps * args.lbm_per_step          # the whole cavity, processed once
+    if rank == 0:
+        peak, peak_src = read_peaks()
+        bpu = BYTES_PER_UPDATE[(w.dim, prec)]
+        p = cav.sim.params()
+        line = {
+            "metric": METRIC, "value": units / t_max / 1e6, "unit": "MLUPS", "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": t_max / args.steps * 1e3, "higher_is_better": True, "scaling": "strong",
+            "vs_baseline": None, "dtype": "f64" if prec == 0 else "f64 collision, f32 storage and stencil interpolation",
+            "data": "synthetic",
+            "config": {"workload": args.workload, "nodes_total": w.nodes, "lattice": "D2Q9+D2Q5" if w.dim == 2 else "D3Q19+D3Q7",
+                       "mesh": f"{w.mesh} stretch {w.stretch}", "Ra": w.Ra, "Pr": w.Pr, "U_lu": 0.1,
+                       "step": f"{args.lbm_per_step} LBM time steps (each followed by a halo exchange) + 1 Nu/Re reduction",
+                       "parallelism": f"slab decomposition over {world} rank(s) along the slowest axis, 1-layer halo, "
+                                      f"{'12 of 26' if w.dim == 3 else '8 of 14'} planes per face per step"},
+            "wctpdt_s": (t_max / (args.steps * args.lbm_per_step)) * p["H_lu"] / p["U"], "Nu_hot": nu["Nu_hot"], "Re": nu["Re"],
+            "roofline": {"bound": "hbm", "achieved": bpu * w.nodes / world / (t_max / (args.steps * args.lbm_per_step)) / 1e9,
+                         "peak": peak, "unit": "GB/s", "frac": bpu * w.nodes / world / (t_max / (args.steps * args.lbm_per_step)) / 1e9 / peak,
+                         "traffic": None, "kernel": cav.sim.kernel_name, "peak_source": peak_src,
+                         "note": "per rank, whole step including the halo exchange and the reduction"},
+            "cpu_baseline": None, "e2e": None, "gpu_launches": cav.sim.launch_count - l0, "clocks": clocks,
+        }
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        import torch.distributed as dist
+        dist.destroy_process_group()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -262,11 +323,15 @@ def main():
     ap.add_argument("--precision", default="f64", choices=["f64", "f32"])
     ap.add_argument("--lbm-per-step", type=int, default=LBM_PER_STEP)
     ap.add_argument("--kernel", type=int, default=0, help="0 auto, 1 generic, 2 TMA-staged, 3 uniform pure shift")
+    ap.add_argument("--decomp", default="replicas", choices=["replicas", "slab"],
+                    help="N > 1: independent cavities (weak scaling, default) or one cavity in slabs (strong scaling)")
     ap.add_argument("--no-extras", action="store_true", help="skip the secondary workloads, e2e and CPU baseline")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         return run_reference(args)
+    if args.decomp == "slab":
+        return run_slab(args)
 
     import torch
     from paper_2509_01099_b200 import inputs, islbm     # raises if libislbm.so is missing: no fallback

@@ -92,6 +92,25 @@ typedef struct {
   double L_eff[3]; /* x[n-1] - x[0] + delta per axis (1 for the unused axis)      */
 } islbm_params;
 
+/* A slab of a larger cavity along its slowest axis (y in 2-D, z in 3-D), for a one-rank-per-GPU decomposition
+ * (DESIGN.md 8).  The mesh given to islbm_create_slab holds the slab's owned layers plus ONE ghost layer at each
+ * end that is not a wall; the other axes are complete. */
+typedef struct {
+  int lo_is_wall, hi_is_wall; /* is the first / last layer of this mesh a cavity wall (no ghost layer there)? */
+  double L_eff_global;        /* effective length of the slab axis of the WHOLE cavity (x[n-1] - x[0] + delta) */
+  long long node_offset;      /* global linear index of this mesh's node 0 (islbm_init draws noise by global index) */
+} islbm_slab;
+
+/* Where the halo of one side lives in the workspace, for the CURRENT state (call again after islbm_step). */
+typedef struct {
+  int is_wall;                /* 1: this side is a wall, nothing to exchange */
+  int first_plane, n_planes;  /* the storage planes whose velocity has a component along the slab axis */
+  size_t plane_pitch_bytes;   /* distance between consecutive planes */
+  size_t layer_bytes;         /* contiguous bytes of one layer of one plane */
+  size_t send_offset;         /* workspace byte offset of the first/last OWNED layer of plane first_plane */
+  size_t recv_offset;         /* ... of the ghost layer on this side */
+} islbm_halo_info;
+
 /* Bytes of DEVICE workspace islbm_create needs for this mesh / lattice /
  * precision (two ping-pong population buffers + interpolation tables +
  * reduction scratch).  Pure host arithmetic. */
@@ -107,6 +126,24 @@ int islbm_workspace_bytes(const islbm_mesh *mesh, int lattice, int precision,
 int islbm_create(islbm_t **out, const islbm_mesh *mesh, int lattice, double Ra,
                  double Pr, double Ma, int precision, void *dev_workspace,
                  size_t bytes, void *cuda_stream);
+
+/* As islbm_create for a slab (see islbm_slab).  After every islbm_step(h, 1) the caller copies, for each plane
+ * first_plane .. first_plane + n_planes - 1, the neighbour's send layer into this handle's recv layer (NCCL
+ * send/recv or a peer copy on the handle's stream; islbm_halo gives the offsets).  islbm_nusselt,
+ * islbm_nusselt_middle and islbm_steady_residual refuse slab handles: use islbm_diag_sums on every rank, add the
+ * arrays, and islbm_diag_from_sums.  islbm_get_populations / islbm_fields return the local mesh; their ghost
+ * layers are undefined. */
+int islbm_create_slab(islbm_t **out, const islbm_mesh *mesh, int lattice, double Ra, double Pr, double Ma,
+                      int precision, void *dev_workspace, size_t bytes, void *cuda_stream, const islbm_slab *slab);
+int islbm_halo(islbm_t *h, int side /* 0 low, 1 high */, islbm_halo_info *out);
+/* HOST s[8]: this handle's Eq. 29-weighted partial sums (ghost layers weigh 0); synchronises the stream. */
+int islbm_diag_sums(islbm_t *h, double s[8]);
+/* HOST out[6] = Nu_hot, Nu_cold, <Re>, <u*^2>_V, <Nu>, Nu_middle from sums added over all slabs (pure host). */
+int islbm_diag_from_sums(const islbm_t *h, const double s[8], double out[6]);
+/* HOST s[4]: the four sums of Eq. 30 over this handle's owned nodes against the snapshot of the previous call
+ * (then overwritten); *first = 1 if there was no snapshot (sums meaningless).  Residuals of the whole cavity:
+ * (sum of s[0]) / (sum of s[1]) and (sum of s[2]) / (sum of s[3]) over the ranks.  Synchronises the stream. */
+int islbm_residual_sums(islbm_t *h, double s[4], int *first);
 
 void islbm_destroy(islbm_t *h);
 

@@ -91,6 +91,8 @@ struct islbm {
   std::vector<double> xs[3];   // node coordinates (kept for islbm_set_stencil)
   int stencil;                 // 0 central, 1 upwind
   int npad;
+  bool is_slab;                // slab of a larger cavity along the slowest axis (islbm_create_slab)
+  islbm_slab slab;
   islbm_params prm;
   double buoy;
   double T0;               // reference temperature of the buoyancy force
@@ -147,6 +149,7 @@ static int derive_params(islbm *h, const islbm_mesh *mesh) {
   islbm_params &p = h->prm;
   for (int a = 0; a < 3; ++a)
     p.L_eff[a] = a < h->dim ? mesh->x[a][h->n[a] - 1] - mesh->x[a][0] + h->delta : 1.0;
+  if (h->is_slab) p.L_eff[h->dim - 1] = h->slab.L_eff_global;   // the whole cavity's extent, not this slab's
   p.U = h->Ma / std::sqrt(3.0);
   p.H_lu = p.L_eff[1] / h->delta;
   p.nu = p.U * p.H_lu * std::sqrt(h->Pr / h->Ra);
@@ -204,10 +207,14 @@ static void build_tables(const islbm *h, const double *const *xs, int stencil, i
         w[(size_t)2 * npad] = ((xi - d0) * (xi - d1)) / ((d2 - d0) * (d2 - d1));
       }
     }
+    const bool slab_axis = h->is_slab && a == h->dim - 1;
     for (int j = 0; j < n; ++j) {   // Eq. 29 with ghost points one lattice unit outside (A14)
       const double xm = j == 0 ? x[0] - h->delta : x[j - 1];
       const double xp = j == n - 1 ? x[n - 1] + h->delta : x[j + 1];
       avgw[(size_t)a * npad + j] = 0.5 * (xp - xm);
+      // a slab's ghost layers belong to the neighbouring rank: weight 0, so every weighted sum is this rank's share
+      if (slab_axis && ((j == 0 && !h->slab.lo_is_wall) || (j == n - 1 && !h->slab.hi_is_wall)))
+        avgw[(size_t)a * npad + j] = 0.0;
     }
   }
 }
@@ -221,8 +228,27 @@ static int upload_tables(islbm *h) {
   return ISLBM_OK;
 }
 
+static int create_impl(islbm_t **out, const islbm_mesh *mesh, int lattice, double Ra, double Pr, double Ma, int precision,
+                       void *dev_workspace, size_t bytes, void *cuda_stream, const islbm_slab *slab);
+
 extern "C" int islbm_create(islbm_t **out, const islbm_mesh *mesh, int lattice, double Ra, double Pr, double Ma,
                             int precision, void *dev_workspace, size_t bytes, void *cuda_stream) {
+  return create_impl(out, mesh, lattice, Ra, Pr, Ma, precision, dev_workspace, bytes, cuda_stream, nullptr);
+}
+
+extern "C" int islbm_create_slab(islbm_t **out, const islbm_mesh *mesh, int lattice, double Ra, double Pr, double Ma,
+                                 int precision, void *dev_workspace, size_t bytes, void *cuda_stream,
+                                 const islbm_slab *slab) {
+  if (!slab) return fail(ISLBM_ERR_ARG, "slab is NULL");
+  if (!(slab->L_eff_global > 0.0) || slab->node_offset < 0) return fail(ISLBM_ERR_ARG, "bad slab description");
+  if (mesh && mesh->dim >= 2 && mesh->dim <= 3 &&
+      mesh->n[mesh->dim - 1] - (slab->lo_is_wall ? 0 : 1) - (slab->hi_is_wall ? 0 : 1) < 1)
+    return fail(ISLBM_ERR_ARG, "a slab needs at least one owned layer besides its ghost layers");
+  return create_impl(out, mesh, lattice, Ra, Pr, Ma, precision, dev_workspace, bytes, cuda_stream, slab);
+}
+
+static int create_impl(islbm_t **out, const islbm_mesh *mesh, int lattice, double Ra, double Pr, double Ma, int precision,
+                       void *dev_workspace, size_t bytes, void *cuda_stream, const islbm_slab *slab) {
   if (!out) return fail(ISLBM_ERR_ARG, "out is NULL");
   *out = nullptr;
   int rc = check_mesh_args(mesh, lattice, precision);
@@ -254,6 +280,8 @@ extern "C" int islbm_create(islbm_t **out, const islbm_mesh *mesh, int lattice, 
   h->q = h->qf + h->qg;
   h->st_bytes = precision == ISLBM_F64 ? 8 : 4;
   h->Ra = Ra; h->Pr = Pr; h->Ma = Ma; h->delta = mesh->delta;
+  h->is_slab = slab != nullptr;
+  if (slab) h->slab = *slab;
   h->buoy = 1.0;
   h->T0 = 0.0;             // BASELINE.json configs: walls at +-0.5, reference = their mean (A9)
   h->uniform = uniform;
@@ -291,6 +319,14 @@ extern "C" int islbm_create(islbm_t **out, const islbm_mesh *mesh, int lattice, 
   dm.T_hot = 0.5;      // PAPER.md:237, 430; BASELINE.json configs (A11)
   dm.T_cold = -0.5;
   dm.stencil = 0;
+  {
+    const int nm = h->n[h->dim - 1];
+    dm.wall_mlo = !slab || slab->lo_is_wall;
+    dm.wall_mhi = !slab || slab->hi_is_wall;
+    dm.em_lo = dm.wall_mlo ? 0 : 1;
+    dm.em_hi = dm.wall_mhi ? nm : nm - 1;
+    dm.node_offset = slab ? slab->node_offset : 0;
+  }
   h->dp.q_lo = (mesh->x[0][1] - mesh->x[0][0]) / mesh->delta;
   h->dp.q_hi = (mesh->x[0][h->n[0] - 1] - mesh->x[0][h->n[0] - 2]) / mesh->delta;
   h->dp.T0 = h->T0;
@@ -631,8 +667,54 @@ static int run_diag_reduction(islbm *h, double *s) {
   return ISLBM_OK;
 }
 
+// ---- slab decomposition: halo layout, partial sums -----------------------------------------------------------
+extern "C" int islbm_halo(islbm_t *h, int side, islbm_halo_info *out) {
+  if (!h || !out) return fail(ISLBM_ERR_ARG, "NULL argument");
+  if (side != 0 && side != 1) return fail(ISLBM_ERR_ARG, "side must be 0 (low) or 1 (high)");
+  const int nm = h->n[h->dim - 1];
+  const size_t layer = (size_t)h->dm.nxp * (h->dim == 3 ? h->n[1] : 1) * h->st_bytes;
+  out->first_plane = h->dim == 2 ? 6 : 14;     // the planes with a velocity component along the slab axis
+  out->n_planes = h->dim == 2 ? 8 : 12;
+  out->plane_pitch_bytes = (size_t)h->dm.nnp * h->st_bytes;
+  out->layer_bytes = layer;
+  out->is_wall = side == 0 ? h->dm.wall_mlo : h->dm.wall_mhi;
+  const size_t base = h->cv.buf[h->cur] + (size_t)out->first_plane * out->plane_pitch_bytes;
+  const int send_layer = side == 0 ? h->dm.em_lo : h->dm.em_hi - 1;
+  const int recv_layer = side == 0 ? 0 : nm - 1;
+  out->send_offset = base + (size_t)send_layer * layer;
+  out->recv_offset = base + (size_t)recv_layer * layer;
+  return ISLBM_OK;
+}
+
+extern "C" int islbm_diag_sums(islbm_t *h, double s[8]) {
+  if (!h || !s) return fail(ISLBM_ERR_ARG, "NULL argument");
+  if (!h->has_state) return fail(ISLBM_ERR_STATE, "no state");
+  double t[kRedSlots];
+  int rc = run_diag_reduction(h, t);
+  if (rc) return rc;
+  for (int i = 0; i < 8; ++i) s[i] = i < kRedSlots ? t[i] : 0.0;
+  return ISLBM_OK;
+}
+
+extern "C" int islbm_diag_from_sums(const islbm_t *h, const double s[8], double out[6]) {
+  if (!h || !s || !out) return fail(ISLBM_ERR_ARG, "NULL argument");
+  const islbm_params &p = h->prm;
+  const double area = p.L_eff[1] * (h->dim == 3 ? p.L_eff[2] : 1.0);
+  const double vol = area * p.L_eff[0];
+  out[0] = -p.H_lu * s[0] / area;
+  out[1] = -p.H_lu * s[1] / area;
+  out[2] = std::sqrt(h->Ra / h->Pr) * (s[2] / vol) / p.U;
+  out[3] = (s[3] / vol) / (p.U * p.U);
+  out[4] = std::sqrt(h->Ra * h->Pr) * (s[4] / vol) / p.U + 1.0;
+  out[5] = std::sqrt(h->Ra * h->Pr) * (s[5] / area) / p.U - p.H_lu * (s[6] / area);
+  for (int i = 0; i < 6; ++i)
+    if (!std::isfinite(out[i])) return fail(ISLBM_ERR_NONFINITE, "non-finite diagnostic: the run has diverged");
+  return ISLBM_OK;
+}
+
 extern "C" int islbm_nusselt_middle(islbm_t *h, double *out) {
   if (!h || !out) return fail(ISLBM_ERR_ARG, "NULL argument");
+  if (h->is_slab) return fail(ISLBM_ERR_STATE, "slab handle: use islbm_diag_sums, sum over ranks, islbm_diag_from_sums");
   if (!h->has_state) return fail(ISLBM_ERR_STATE, "no state");
   double s[kRedSlots];
   int rc = run_diag_reduction(h, s);
@@ -646,6 +728,7 @@ extern "C" int islbm_nusselt_middle(islbm_t *h, double *out) {
 
 extern "C" int islbm_nusselt(islbm_t *h, double out[5]) {
   if (!h || !out) return fail(ISLBM_ERR_ARG, "NULL argument");
+  if (h->is_slab) return fail(ISLBM_ERR_STATE, "slab handle: use islbm_diag_sums, sum over ranks, islbm_diag_from_sums");
   if (!h->has_state) return fail(ISLBM_ERR_STATE, "no state");
   double s[kRedSlots];
   int rc = run_diag_reduction(h, s);
@@ -672,21 +755,43 @@ static void launch_residual(islbm *h, int nb) {
   h->launches += 2;
 }
 
-extern "C" int islbm_steady_residual(islbm_t *h, double out[2]) {
-  if (!h || !out) return fail(ISLBM_ERR_ARG, "NULL argument");
-  if (!h->has_state) return fail(ISLBM_ERR_STATE, "no state");
+// Eq. 30 sums between the current fields and the snapshot (which the kernel then overwrites): s[0..3] =
+// sum|u-u_prev|_2, sum|u_prev|_2, sum|T-T_prev|, sum|T_prev| over the owned nodes; *first = no snapshot existed.
+static int run_residual(islbm *h, double s[4], bool *first) {
   if (!h->snap_valid) CUDA_TRY(cudaMemsetAsync(h->ws + h->cv.snap, 0, sizeof(double) * 4 * (size_t)h->nn, h->stream));
   const int nb = red_blocks(h);
 #define CALL(D, T) launch_residual<D, T>(h, nb)
   DISPATCH(h, CALL);
 #undef CALL
   CUDA_TRY(cudaPeekAtLastError());
-  double s[kRedSlots];
-  CUDA_TRY(cudaMemcpyAsync(s, h->ws + h->cv.red_out, sizeof s, cudaMemcpyDeviceToHost, h->stream));
+  double t[kRedSlots];
+  CUDA_TRY(cudaMemcpyAsync(t, h->ws + h->cv.red_out, sizeof t, cudaMemcpyDeviceToHost, h->stream));
   CUDA_TRY(cudaStreamSynchronize(h->stream));
-  if (!h->snap_valid) {
+  for (int i = 0; i < 4; ++i) s[i] = t[i];
+  *first = !h->snap_valid;
+  h->snap_valid = true;
+  return ISLBM_OK;
+}
+
+extern "C" int islbm_residual_sums(islbm_t *h, double s[4], int *first) {
+  if (!h || !s || !first) return fail(ISLBM_ERR_ARG, "NULL argument");
+  if (!h->has_state) return fail(ISLBM_ERR_STATE, "no state");
+  bool f = false;
+  int rc = run_residual(h, s, &f);
+  *first = f ? 1 : 0;
+  return rc;
+}
+
+extern "C" int islbm_steady_residual(islbm_t *h, double out[2]) {
+  if (!h || !out) return fail(ISLBM_ERR_ARG, "NULL argument");
+  if (h->is_slab) return fail(ISLBM_ERR_STATE, "slab handle: use islbm_residual_sums and add the sums over ranks");
+  if (!h->has_state) return fail(ISLBM_ERR_STATE, "no state");
+  double s[4];
+  bool first = false;
+  int rc = run_residual(h, s, &first);
+  if (rc) return rc;
+  if (first) {
     out[0] = out[1] = 1.0;
-    h->snap_valid = true;
   } else {
     out[0] = s[1] > 0.0 ? s[0] / s[1] : (s[0] > 0.0 ? 1.0 : 0.0);
     out[1] = s[3] > 0.0 ? s[2] / s[3] : (s[2] > 0.0 ? 1.0 : 0.0);

@@ -35,6 +35,12 @@ struct DevMesh {
   const double *avgw;    // Eq. 29 weights, [axis 3][npad]
   double omega_bc;       // Eq. 22 weight
   double T_hot, T_cold;  // x-lo / x-hi wall temperatures
+  // slab decomposition along the slowest axis (y in 2-D, z in 3-D): the local mesh may carry one
+  // ghost layer at either end, which is read but not updated; the layers [em_lo, em_hi) are the owned ones, and an
+  // end is a wall only if its flag says so.  Whole cavity: em_lo = 0, em_hi = n, both walls.
+  int em_lo, em_hi;
+  int wall_mlo, wall_mhi;
+  long long node_offset; // global linear index of local node 0 (islbm_init draws the noise by global index)
   int stencil;           // 0: {j-1,j,j+1} (A2); 1: upwind {j-2,j-1,j} for c=+1, {j,j+1,j+2} for c=-1
                          // (generic kernel only; the TMA kernels stage a 1-node halo and take stencil 0)
 };
@@ -107,8 +113,8 @@ __device__ __forceinline__ void make_ctx(const DevMesh &m, int ix, int iy, int i
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
     if (a < DIM) {
-      cx.lo[a] = cx.i[a] == 0;
-      cx.hi[a] = cx.i[a] == n[a] - 1;
+      cx.lo[a] = cx.i[a] == 0 && (a != DIM - 1 || m.wall_mlo);
+      cx.hi[a] = cx.i[a] == n[a] - 1 && (a != DIM - 1 || m.wall_mhi);
       cx.b[a][0] = min(max(m.stencil ? cx.i[a] : cx.i[a] - 1, 0), n[a] - 3);
       cx.b[a][1] = min(max(m.stencil ? cx.i[a] - 2 : cx.i[a] - 1, 0), n[a] - 3);
 #pragma unroll
@@ -214,6 +220,7 @@ k_step_generic(DevMesh m, NodeParams np, const ST *__restrict__ src, ST *__restr
   const int iy = blockIdx.y * blockDim.y + threadIdx.y;
   const int iz = blockIdx.z * blockDim.z + threadIdx.z;
   if (ix >= m.nx || iy >= m.ny || iz >= m.nz) return;
+  if (COLLIDE && ((DIM == 3 ? iz : iy) < m.em_lo || (DIM == 3 ? iz : iy) >= m.em_hi)) return;   // ghost layer
   NodeCtx<DIM> cx;
   make_ctx<DIM>(m, ix, iy, iz, cx);
   double f[QF], g[QG];
@@ -254,7 +261,7 @@ k_load_state(DevMesh m, NodeParams np, const double *__restrict__ fin, const dou
   const long long c = c0 + i;
   double f[QF], g[QG];
   if (GENERATE) {
-    const unsigned long long z = splitmix64_at(seed, (unsigned long long)c);
+    const unsigned long long z = splitmix64_at(seed, (unsigned long long)(c + m.node_offset));
     const double r = (double)(z >> 11) * (1.0 / 9007199254740992.0);
     rest_equilibrium<QF, QG>(f, g, amp * (2.0 * r - 1.0), np.a_T);
   } else {

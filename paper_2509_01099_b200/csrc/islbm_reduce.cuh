@@ -122,6 +122,10 @@ k_residual_partial(DevMesh m, NodeParams np, const ST *__restrict__ S, double *_
   double acc[kRedSlots] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
   const long long stride = (long long)gridDim.x * kRedThreads;
   for (long long c = (long long)blockIdx.x * kRedThreads + threadIdx.x; c < m.nn; c += stride) {
+    {   // ghost layers of a slab are not part of this rank's sums (their snapshot entries stay zero)
+      const long long layer = c / ((long long)m.nx * (DIM == 3 ? m.ny : 1));
+      if (layer < m.em_lo || layer >= m.em_hi) continue;
+    }
     double f[Lat<DIM>::QF], g[Lat<DIM>::QG];
     load_post_node<DIM>(m, S, sidx(m, c), f, g);
     double rho, u, v, w, T;

@@ -121,7 +121,7 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
   pdl_launch_dependents();
 
   const int x0 = blockIdx.x * T::TX;
-  const int y0 = blockIdx.y * ychunk, y1 = min(y0 + ychunk, m.ny);
+  const int y0 = m.em_lo + blockIdx.y * ychunk, y1 = min(y0 + ychunk, m.em_hi);
   const int yf = DIR > 0 ? y0 : y1 - 1;
   const int nstage = 2 + (y1 - y0);
   for (int i = threadIdx.x; i < 6 * (y1 - y0); i += T::TX) {
@@ -219,8 +219,8 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
         else ISLBM_YCOMB2(S2, S1, S0);
       }
       const long long c = (long long)y * m.nxp + x;
-      wf.lo[1] = y == 0;
-      wf.hi[1] = y == m.ny - 1;
+      wf.lo[1] = y == 0 && m.wall_mlo;
+      wf.hi[1] = y == m.ny - 1 && m.wall_mhi;
       if (valid && (wall_x | wf.lo[1] | wf.hi[1])) {
         bb_fix_all_f<2>(f, wf, src, m.nnp, c, std::make_integer_sequence<int, 8>{});
         bb_fix_all_g<2>(g, wf, src, m.nnp, c, m, std::make_integer_sequence<int, 4>{});
@@ -312,7 +312,7 @@ template <typename ST, typename CFG>
 inline void launch2_cfg(const Plan2 &p, const int *n, const DevMesh &m, const NodeParams &np, int cur, void *const *buf,
                         const Tuning &tn, cudaStream_t stream) {
   using T = typename CFG::T;
-  dim3 grid((n[0] + T::TX - 1) / T::TX, (n[1] + p.ychunk - 1) / p.ychunk, 1);
+  dim3 grid((n[0] + T::TX - 1) / T::TX, (m.em_hi - m.em_lo + p.ychunk - 1) / p.ychunk, 1);
   if (tn.serpentine && cur)
     launch_step(k_step_ymarch<ST, T::TX, T::STAGES, CFG::MINB, -1>, grid, dim3(T::TX), T::SMEM_BYTES, stream, tn.pdl != 0,
                 p.maps[cur], m, np, (const ST *)buf[cur], (ST *)buf[1 - cur], p.ychunk, tn.load_policy, tn.store_policy);

@@ -246,7 +246,7 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
   // the last y-tile is pulled back inside the mesh (it recomputes a few rows of its neighbour, bit-identically),
   // so that the shifted wall stencil of row ny-1 never leaves the box
   const int x0 = blockIdx.x * T::TX, y0 = min((int)blockIdx.y * T::TY, max(m.ny - T::TY, 0));
-  const int z0 = blockIdx.z * zchunk, z1 = min(z0 + zchunk, m.nz);
+  const int z0 = m.em_lo + blockIdx.z * zchunk, z1 = min(z0 + zchunk, m.em_hi);
   const int nstage = 2 + (z1 - z0);
   for (int i = threadIdx.x; i < 6 * (z1 - z0); i += T::THREADS) {
     const int sk = i / (z1 - z0), zi = i - sk * (z1 - z0);
@@ -361,8 +361,8 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
       else if (newest == 1) ISLBM_ZCOMB3(S2, S0, S1);
       else ISLBM_ZCOMB3(S0, S1, S2);
       const long long c = (long long)z * plane + cxy;
-      wf.lo[2] = z == 0;
-      wf.hi[2] = z == m.nz - 1;
+      wf.lo[2] = z == 0 && m.wall_mlo;
+      wf.hi[2] = z == m.nz - 1 && m.wall_mhi;
       if (valid && (wall_xy | wf.lo[2] | wf.hi[2])) {
         bb_fix_all_f<3>(f, wf, src, m.nnp, c, std::make_integer_sequence<int, 18>{});
         bb_fix_all_g<3>(g, wf, src, m.nnp, c, m, std::make_integer_sequence<int, 6>{});
@@ -445,7 +445,7 @@ template <typename ST, int TX, int TY>
 inline void launch3_shape(const Plan3 &p, const int *n, const DevMesh &m, const NodeParams &np, int cur, void *const *buf,
                           const Tuning &tn, cudaStream_t stream) {
   using T = Tile3<ST, TX, TY>;
-  dim3 grid((n[0] + T::TX - 1) / T::TX, (n[1] + T::TY - 1) / T::TY, (n[2] + p.zchunk - 1) / p.zchunk);
+  dim3 grid((n[0] + T::TX - 1) / T::TX, (n[1] + T::TY - 1) / T::TY, (m.em_hi - m.em_lo + p.zchunk - 1) / p.zchunk);
   launch_step(k_step_zmarch<ST, TX, TY>, grid, dim3(T::THREADS), T::SMEM_BYTES, stream, tn.pdl != 0, p.maps[cur], m, np,
               (const ST *)buf[cur], (ST *)buf[1 - cur], p.zchunk, tn.load_policy, tn.store_policy);
 }

@@ -55,8 +55,9 @@ k_step_shift(DevMesh m, NodeParams np, const ST *__restrict__ src, ST *__restric
   cx.i[0] = ix; cx.i[1] = iy; cx.i[2] = iz;
   cx.c = ((long long)iz * m.ny + iy) * m.nxp + ix;
   cx.lo[0] = ix == 0; cx.hi[0] = ix == m.nx - 1;
-  cx.lo[1] = iy == 0; cx.hi[1] = iy == m.ny - 1;
-  cx.lo[2] = DIM == 3 && iz == 0; cx.hi[2] = DIM == 3 && iz == m.nz - 1;
+  cx.lo[1] = iy == 0 && (DIM == 3 || m.wall_mlo); cx.hi[1] = iy == m.ny - 1 && (DIM == 3 || m.wall_mhi);
+  cx.lo[2] = DIM == 3 && iz == 0 && m.wall_mlo; cx.hi[2] = DIM == 3 && iz == m.nz - 1 && m.wall_mhi;
+  if ((DIM == 3 ? iz : iy) < m.em_lo || (DIM == 3 ? iz : iy) >= m.em_hi) return;   // ghost layer: read, not updated
   double f[QF], g[QG];
   shift_all_f<DIM>(m, src, cx, f, std::make_integer_sequence<int, QF>{});
   shift_all_g<DIM>(m, src, cx, g, std::make_integer_sequence<int, QG>{});

@@ -20,7 +20,8 @@ F64, F32_STORAGE = 0, 1
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED, KERNEL_UNIFORM_SHIFT = 0, 1, 2, 3
 
 EXPORTS = (
-    "islbm_workspace_bytes", "islbm_create", "islbm_destroy", "islbm_get_params", "islbm_init",
+    "islbm_workspace_bytes", "islbm_create", "islbm_create_slab", "islbm_halo", "islbm_diag_sums", "islbm_diag_from_sums",
+    "islbm_residual_sums", "islbm_destroy", "islbm_get_params", "islbm_init",
     "islbm_set_populations", "islbm_set_populations_host", "islbm_get_populations", "islbm_step", "islbm_fields", "islbm_nusselt", "islbm_nusselt_middle",
     "islbm_steady_residual", "islbm_set_buoyancy_scale", "islbm_set_reference_temperature", "islbm_set_stencil", "islbm_set_kernel", "islbm_set_tuning", "islbm_launch_count",
     "islbm_kernel_name", "islbm_last_error", "islbm_version",
@@ -29,6 +30,15 @@ EXPORTS = (
 
 class _Mesh(C.Structure):
     _fields_ = [("dim", C.c_int), ("n", C.c_int * 3), ("x", C.POINTER(C.c_double) * 3), ("delta", C.c_double)]
+
+
+class _Slab(C.Structure):
+    _fields_ = [("lo_is_wall", C.c_int), ("hi_is_wall", C.c_int), ("L_eff_global", C.c_double), ("node_offset", C.c_longlong)]
+
+
+class _Halo(C.Structure):
+    _fields_ = [("is_wall", C.c_int), ("first_plane", C.c_int), ("n_planes", C.c_int), ("plane_pitch_bytes", C.c_size_t),
+                ("layer_bytes", C.c_size_t), ("send_offset", C.c_size_t), ("recv_offset", C.c_size_t)]
 
 
 class _Params(C.Structure):
@@ -51,6 +61,12 @@ def _load():
     lib.islbm_workspace_bytes.argtypes = [C.POINTER(_Mesh), C.c_int, C.c_int, C.POINTER(C.c_size_t)]
     lib.islbm_create.argtypes = [C.POINTER(vp), C.POINTER(_Mesh), C.c_int, C.c_double, C.c_double, C.c_double,
                                  C.c_int, vp, C.c_size_t, vp]
+    lib.islbm_create_slab.argtypes = [C.POINTER(vp), C.POINTER(_Mesh), C.c_int, C.c_double, C.c_double, C.c_double,
+                                      C.c_int, vp, C.c_size_t, vp, C.POINTER(_Slab)]
+    lib.islbm_halo.argtypes = [vp, C.c_int, C.POINTER(_Halo)]
+    lib.islbm_diag_sums.argtypes = [vp, dp]
+    lib.islbm_diag_from_sums.argtypes = [vp, dp, dp]
+    lib.islbm_residual_sums.argtypes = [vp, dp, C.POINTER(C.c_int)]
     lib.islbm_destroy.argtypes = [vp]
     lib.islbm_destroy.restype = None
     lib.islbm_get_params.argtypes = [vp, C.POINTER(_Params)]
@@ -116,7 +132,9 @@ def _dev_ptr(t, n_expected=None):
 class Islbm:
     """islbm_create / islbm_step / islbm_fields / islbm_nusselt on one CUDA device."""
 
-    def __init__(self, coords, delta, Ra, Pr, Ma, precision=F64, device="cuda", stream=None, guard_bytes=0):
+    def __init__(self, coords, delta, Ra, Pr, Ma, precision=F64, device="cuda", stream=None, guard_bytes=0, slab=None):
+        """slab = None, or dict(lo_is_wall, hi_is_wall, L_eff_global, node_offset): a slab of a larger cavity whose
+        slowest-axis coordinates include one ghost layer at each non-wall end (islbm_create_slab)."""
         self.dim = len(coords)
         self.precision = precision
         self.device = torch.device(device)
@@ -136,8 +154,14 @@ class Islbm:
         self.workspace = self._alloc[guard_bytes:guard_bytes + nbytes.value]
         self.stream = stream if stream is not None else torch.cuda.current_stream(self.device)
         self.h = C.c_void_p()
-        _check(lib.islbm_create(C.byref(self.h), C.byref(m), lattice, float(Ra), float(Pr), float(Ma), precision,
-                                C.c_void_p(self.workspace.data_ptr()), nbytes.value, C.c_void_p(self.stream.cuda_stream)))
+        if slab is None:
+            _check(lib.islbm_create(C.byref(self.h), C.byref(m), lattice, float(Ra), float(Pr), float(Ma), precision,
+                                    C.c_void_p(self.workspace.data_ptr()), nbytes.value, C.c_void_p(self.stream.cuda_stream)))
+        else:
+            sl = _Slab(int(slab["lo_is_wall"]), int(slab["hi_is_wall"]), float(slab["L_eff_global"]), int(slab["node_offset"]))
+            _check(lib.islbm_create_slab(C.byref(self.h), C.byref(m), lattice, float(Ra), float(Pr), float(Ma), precision,
+                                         C.c_void_p(self.workspace.data_ptr()), nbytes.value,
+                                         C.c_void_p(self.stream.cuda_stream), C.byref(sl)))
         del keep
 
     def guards_intact(self):
@@ -222,6 +246,33 @@ class Islbm:
         out = (C.c_double * 5)()
         _check(lib.islbm_nusselt(self.h, out))
         return dict(zip(("Nu_hot", "Nu_cold", "Re", "u2", "Nu_vol"), list(out)))
+
+    def halo(self, side):
+        """(is_wall, [send views], [recv views]) of the current state: uint8 views of the workspace, one per plane."""
+        hi = _Halo()
+        _check(lib.islbm_halo(self.h, int(side), C.byref(hi)))
+        send = [self.workspace[hi.send_offset + p * hi.plane_pitch_bytes: hi.send_offset + p * hi.plane_pitch_bytes + hi.layer_bytes]
+                for p in range(hi.n_planes)]
+        recv = [self.workspace[hi.recv_offset + p * hi.plane_pitch_bytes: hi.recv_offset + p * hi.plane_pitch_bytes + hi.layer_bytes]
+                for p in range(hi.n_planes)]
+        return bool(hi.is_wall), send, recv
+
+    def diag_sums(self):
+        s = (C.c_double * 8)()
+        _check(lib.islbm_diag_sums(self.h, s))
+        return list(s)
+
+    def diag_from_sums(self, sums):
+        s = (C.c_double * 8)(*[float(v) for v in sums])
+        out = (C.c_double * 6)()
+        _check(lib.islbm_diag_from_sums(self.h, s, out))
+        return dict(zip(("Nu_hot", "Nu_cold", "Re", "u2", "Nu_vol", "Nu_middle"), list(out)))
+
+    def residual_sums(self):
+        s = (C.c_double * 4)()
+        first = C.c_int(0)
+        _check(lib.islbm_residual_sums(self.h, s, C.byref(first)))
+        return list(s), bool(first.value)
 
     def nusselt_middle(self):
         out = C.c_double(0.0)

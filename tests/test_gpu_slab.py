@@ -1,0 +1,107 @@
+"""Slab decomposition on ONE GPU: K slab handles in one process, halo exchanged by direct copies, against the
+single-domain handle (bit for bit on the owned layers) and against the oracle.  No rank waits on another: the
+slabs are stepped one after the other on the same stream."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+torch = pytest.importorskip("torch")
+pytestmark = pytest.mark.gpu
+
+from oracle.oracle import Oracle  # noqa: E402
+from paper_2509_01099_b200 import inputs, slab  # noqa: E402
+
+SQ3 = math.sqrt(3.0)
+
+
+@pytest.fixture(scope="module")
+def islbm():
+    import __graft_entry__ as graft
+    graft.build()
+    from paper_2509_01099_b200 import islbm as mod
+    return mod
+
+
+def mesh(dim, ns, st):
+    coords = [inputs.tanh_mesh(n, s)[0] for n, s in zip(ns[:dim], st[:dim])]
+    delta = min(float(np.diff(c).min()) for c in coords)
+    H_lu = (coords[1][-1] - coords[1][0] + delta) / delta
+    return coords, delta, 0.71 * (0.1 * H_lu / 0.03) ** 2
+
+
+@pytest.mark.parametrize("dim,ns,world,prec,kernel", [
+    (2, (70, 45), 2, 0, 0), (2, (70, 45), 4, 0, 0), (2, (131, 20), 5, 1, 0), (2, (40, 33), 3, 0, 1),
+    (3, (40, 24, 37), 3, 0, 0), (3, (33, 17, 9), 2, 1, 0), (3, (36, 18, 16), 8, 0, 0), (3, (20, 12, 11), 2, 0, 1)])
+def test_slabs_equal_the_single_domain_bitwise(islbm, dim, ns, world, prec, kernel):
+    coords, delta, Ra = mesh(dim, ns, (1.4, 1.2, 1.3))
+    Ma = 0.1 * SQ3
+    whole = islbm.Islbm(coords, delta, Ra, 0.71, Ma, precision=prec)
+    slabs = [slab.SlabCavity(coords, delta, Ra, 0.71, Ma, r, world, precision=prec, exchange=lambda: None) for r in range(world)]
+    if kernel:
+        whole.set_kernel(kernel)
+        for s in slabs:
+            s.sim.set_kernel(kernel)
+    whole.init(3, 1e-3)
+    for s in slabs:
+        s.init(3, 1e-3)
+        assert whole.params()["H_lu"] == s.sim.params()["H_lu"]
+    for _ in range(7):
+        whole.step(1)
+        for s in slabs:
+            s.sim.step(1)
+        slab.exchange_local(slabs)
+    fw = whole.fields()
+    fw_pop, gw_pop = whole.get_populations()
+    for s in slabs:
+        lo, hi = s.own
+        fl = s.sim.fields()
+        for k in fl:
+            ref = fw[k][..., lo:hi, :] if dim == 2 else fw[k][lo:hi]
+            assert torch.equal(s.owned(fl[k]), ref), (k, s.rank)
+        fp, gp = s.sim.get_populations()
+        reff = fw_pop[..., lo:hi, :] if dim == 2 else fw_pop[:, lo:hi]
+        assert torch.equal(s.owned(fp), reff)
+    # diagnostics: partial sums added over the slabs == the single-domain reduction (different summation order)
+    total = np.sum([s.sim.diag_sums() for s in slabs], axis=0)
+    d = slabs[0].sim.diag_from_sums(total)
+    nu = whole.nusselt()
+    for k in nu:
+        assert d[k] == pytest.approx(nu[k], rel=1e-11, abs=1e-13), k
+    assert d["Nu_middle"] == pytest.approx(whole.nusselt_middle(), rel=1e-11, abs=1e-13)
+    # Eq. 30 residual from sums
+    r0 = [s.sim.residual_sums() for s in slabs]
+    whole.steady_residual()
+    assert all(first for _, first in r0)
+    whole.step(1)
+    for s in slabs:
+        s.sim.step(1)
+    slab.exchange_local(slabs)
+    sums = np.sum([s.sim.residual_sums()[0] for s in slabs], axis=0)
+    ru, rT = whole.steady_residual()
+    assert sums[0] / sums[1] == pytest.approx(ru, rel=1e-10) and sums[2] / sums[3] == pytest.approx(rT, rel=1e-10)
+    with pytest.raises(islbm.IslbmError):
+        slabs[0].sim.nusselt()
+
+
+def test_slabs_against_the_oracle(islbm):
+    coords, delta, Ra = mesh(3, (24, 16, 21), (1.3, 1.2, 1.4))
+    orc = Oracle(coords, delta, Ra, 0.71, 0.1 * SQ3, threads=max(1, min(16, len(os.sched_getaffinity(0)))))
+    slabs = [slab.SlabCavity(coords, delta, Ra, 0.71, 0.1 * SQ3, r, 3, exchange=lambda: None) for r in range(3)]
+    orc.init(0, 1e-3)
+    for s in slabs:
+        s.init(0, 1e-3)
+    orc.step(20)
+    for _ in range(20):
+        for s in slabs:
+            s.sim.step(1)
+        slab.exchange_local(slabs)
+    fo = orc.fields()
+    umax = max(np.abs(fo[k]).max() for k in ("u", "v", "w"))
+    for s in slabs:
+        lo, hi = s.own
+        fl = s.sim.fields()
+        for k in ("u", "v", "w"):
+            assert np.abs(s.owned(fl[k]).cpu().numpy() - fo[k][lo:hi]).max() <= 1e-10 * max(umax, 1e-4)
+        assert np.abs(s.owned(fl["T"]).cpu().numpy() - fo["T"][lo:hi]).max() <= 1e-12
