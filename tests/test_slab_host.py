@@ -23,7 +23,7 @@ def test_split_covers_every_layer_once():
         slab.split(3, 4)
 
 
-@pytest.mark.parametrize("dim,n,world", [(2, 45, 2), (3, 19, 3), (3, 8, 8)])
+@pytest.mark.parametrize("dim,n,world", [(2, 45, 2), (3, 19, 3), (3, 16, 8)])
 def test_slab_inputs_ghosts_offsets_and_extent(dim, n, world):
     x, delta = inputs.tanh_mesh(n, 1.4)
     coords = [inputs.tanh_mesh(12, 1.2)[0] for _ in range(dim - 1)] + [x]
@@ -40,6 +40,12 @@ def test_slab_inputs_ghosts_offsets_and_extent(dim, n, world):
         assert sl["node_offset"] == (lo - glo) * 12 ** (dim - 1)
         covered += list(range(lo, hi))
     assert covered == list(range(n))
+
+
+def test_slab_inputs_refuse_slabs_thinner_than_the_stencil():
+    x, delta = inputs.tanh_mesh(8, 1.2)
+    with pytest.raises(ValueError):
+        slab.slab_inputs([x, x, x], delta, 0, 8)      # 1 owned + 1 ghost layer < 3
 
 
 _WORKER = r"""
