@@ -57,9 +57,7 @@ struct Maps2 {
 template <typename T, int DIR>
 __device__ __forceinline__ void issue_stage2(int s, int yf, int ny, int x0, unsigned char *stage0, uint64_t *full,
                                              uint64_t *empty, const Maps2 &mp, uint64_t pol) {
-  const int st = s % T::STAGES;
-  const uint32_t ph = (uint32_t)(s / T::STAGES) & 1u;
-  if (s >= T::STAGES) mbar_wait(&empty[st], ph ^ 1u);
+  const int st = s % T::STAGES;   // the caller knows the slot is free (initial fill, or it saw the last release)
   int mrow = -1, yrow = -1;
   if (s < 2) {
     mrow = DIR > 0 ? sbase(yf, ny) + s : sbase(yf, ny) + 2 - s;
@@ -118,6 +116,7 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
   uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + T::BAR_OFF);
   uint64_t *empty = full + T::STAGES;
   AT *wys = reinterpret_cast<AT *>(smem_raw + T::W_OFF);
+  int *claim = reinterpret_cast<int *>(smem_raw + T::BAR_OFF + 2 * T::STAGES * 8);   // refill generation per slot
   pdl_launch_dependents();
 
   const int x0 = blockIdx.x * T::TX;
@@ -133,6 +132,7 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
     for (int s = 0; s < T::STAGES; ++s) {
       mbar_init(&full[s], 1);
       mbar_init(&empty[s], T::WARPS);
+      claim[s] = 0;
     }
     fence_barrier_init();
   }
@@ -145,7 +145,7 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
     tma_prefetch_desc(&mp.c2);
     tma_prefetch_desc(&mp.c4);
     tma_prefetch_desc(&mp.x);
-    for (int s = 0; s < T::STAGES - 1 && s < nstage; ++s) issue_stage2<T, DIR>(s, yf, m.ny, x0, stage0, full, empty, mp, lpol);
+    for (int s = 0; s < T::STAGES && s < nstage; ++s) issue_stage2<T, DIR>(s, yf, m.ny, x0, stage0, full, empty, mp, lpol);
   }
 
   const int tx = threadIdx.x;
@@ -181,9 +181,6 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
     auto PXR = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_XR + k * T::P_X); };
     auto PC4 = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_C4 + k * T::P_C); };
     auto PXM = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_XM + k * T::P_X); };
-    if (threadIdx.x == 0 && s + T::STAGES - 1 < nstage)
-      issue_stage2<T, DIR>(s + T::STAGES - 1, yf, m.ny, x0, stage0, full, empty, mp, lpol);
-    __syncwarp();
     mbar_wait(&full[st], ph);
 
     if (has_mov) {
@@ -206,8 +203,12 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
       f[3] = (double)tap3(PXR(1) + o_x, 1, wx[0]);
       g[1] = (double)tap3(PXR(2) + o_x, 1, wx[1]);
       g[3] = (double)tap3(PXR(3) + o_x, 1, wx[0]);
+      // hand the slot back; the warp whose release is the last one refills it at once with stage s + STAGES, so
+      // STAGES - 1 stages are in flight whenever one is being consumed
       __syncwarp();
-      if ((threadIdx.x & 31) == 0) mbar_arrive(&empty[st]);
+      if ((threadIdx.x & 31) == 0 && mbar_arrive_is_last(&empty[st]) && s + T::STAGES < nstage &&
+          atomicCAS(&claim[st], s / T::STAGES, s / T::STAGES + 1) == s / T::STAGES)
+        issue_stage2<T, DIR>(s + T::STAGES, yf, m.ny, x0, stage0, full, empty, mp, lpol);
       // ascending-y order of the stencil rows: the marching order when DIR = +1, its reverse when DIR = -1
       if (DIR > 0) {
         if (newest == 0) ISLBM_YCOMB2(S1, S2, S0);
@@ -229,8 +230,12 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
       collide_node(f, g, np);
       if (valid) store_node<2>(dst + c, m.nnp, f, g, spol, std::make_integer_sequence<int, 14>{});
     } else {
+      // hand the slot back; the warp whose release is the last one refills it at once with stage s + STAGES, so
+      // STAGES - 1 stages are in flight whenever one is being consumed
       __syncwarp();
-      if ((threadIdx.x & 31) == 0) mbar_arrive(&empty[st]);
+      if ((threadIdx.x & 31) == 0 && mbar_arrive_is_last(&empty[st]) && s + T::STAGES < nstage &&
+          atomicCAS(&claim[st], s / T::STAGES, s / T::STAGES + 1) == s / T::STAGES)
+        issue_stage2<T, DIR>(s + T::STAGES, yf, m.ny, x0, stage0, full, empty, mp, lpol);
     }
   }
 }

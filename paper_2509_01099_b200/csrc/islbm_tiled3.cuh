@@ -168,9 +168,7 @@ __device__ __forceinline__ int sbase(int j, int n) { return min(max(j - 1, 0), n
 template <typename T>
 __device__ __forceinline__ void issue_stage3(int s, int z0, int nz, int x0, int y0, unsigned char *stage0, uint64_t *full,
                                              uint64_t *empty, const Maps3 &mp, uint64_t pol) {
-  const int st = s % T::STAGES;
-  const uint32_t ph = (uint32_t)(s / T::STAGES) & 1u;
-  if (s >= T::STAGES) mbar_wait(&empty[st], ph ^ 1u);   // every consumer warp has released the slot
+  const int st = s % T::STAGES;   // the caller knows the slot is free (initial fill, or it saw the last release)
   int mslice = -1, zslice = -1;
   if (s < 2) {
     mslice = sbase(z0, nz) + s;
@@ -236,11 +234,17 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
               ST *__restrict__ dst, int zchunk, int load_policy, int store_policy) {
   using T = Tile3<ST, TX, TY>;
   using AT = typename Acc<ST>::type;
+  // Ring refill policy (measured, profiles/): with fp64 storage the launch is DRAM-bound and thread 0 refilling the
+  // slot released in the previous iteration (STAGES - 2 .. STAGES - 1 stages in flight) is 1.7 % faster; with fp32
+  // storage the stages are half as large and the SM side dominates, and refilling each slot the moment its last
+  // reader releases it (always STAGES - 1 stages in flight) is 6 % faster.
+  constexpr bool EARLY = sizeof(ST) == 4;
   extern __shared__ __align__(128) unsigned char smem_raw[];
   unsigned char *stage0 = smem_raw;
   uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + T::BAR_OFF);
   uint64_t *empty = full + T::STAGES;
   AT *wzs = reinterpret_cast<AT *>(smem_raw + T::W_OFF);
+  int *claim = reinterpret_cast<int *>(smem_raw + T::BAR_OFF + 2 * T::STAGES * 8);   // refill generation per slot
   pdl_launch_dependents();
 
   // the last y-tile is pulled back inside the mesh (it recomputes a few rows of its neighbour, bit-identically),
@@ -257,13 +261,14 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
     for (int s = 0; s < T::STAGES; ++s) {
       mbar_init(&full[s], 1);
       mbar_init(&empty[s], T::CONSUMER_WARPS);
+      claim[s] = 0;
     }
     fence_barrier_init();
   }
   __syncthreads();
 
   pdl_wait();   // everything above read only the weight tables; the population buffers are touched from here on
-  // thread 0 is also the TMA producer: it runs STAGES-1 stages ahead of the consumers
+  // thread 0 fills the ring; afterwards thread 0 (fp64 storage) or the last releasing warp (fp32) refills the slots
   const uint64_t lpol = make_policy(load_policy);
   const uint64_t spol = make_policy(store_policy);
   if (threadIdx.x == 0) {
@@ -272,7 +277,7 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
     tma_prefetch_desc(&mp.x);
     tma_prefetch_desc(&mp.y);
     tma_prefetch_desc(&mp.xy);
-    for (int s = 0; s < T::STAGES - 1 && s < nstage; ++s)
+    for (int s = 0; s < T::STAGES - (EARLY ? 0 : 1) && s < nstage; ++s)
       issue_stage3<T>(s, z0, m.nz, x0, y0, stage0, full, empty, mp, lpol);
   }
 
@@ -321,8 +326,11 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
     auto PC4 = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_C4 + k * T::P_C); };
     auto PXM = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_XM + k * T::P_X); };
     auto PYM = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_YM + k * T::P_Y); };
-    if (threadIdx.x == 0 && s + T::STAGES - 1 < nstage)
-      issue_stage3<T>(s + T::STAGES - 1, z0, m.nz, x0, y0, stage0, full, empty, mp, lpol);
+    if (!EARLY && threadIdx.x == 0 && s + T::STAGES - 1 < nstage) {
+      const int sn = s + T::STAGES - 1;
+      if (sn >= T::STAGES) mbar_wait(&empty[sn % T::STAGES], ((uint32_t)(sn / T::STAGES) & 1u) ^ 1u);
+      issue_stage3<T>(sn, z0, m.nz, x0, y0, stage0, full, empty, mp, lpol);
+    }
     __syncwarp();
     mbar_wait(&full[st], ph);
 
@@ -355,8 +363,14 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
       f[9] = (double)tap9(PXY(2) + o_xy, T::HX, wx[1], wy[0]);
       f[10] = (double)tap9(PXY(3) + o_xy, T::HX, wx[0], wy[0]);
       // all shared-memory reads of this stage are done: hand the slot back to the producer
+      // hand the slot back (EARLY: the warp whose release is the last one refills it at once with stage s + STAGES)
       __syncwarp();
-      if ((threadIdx.x & 31) == 0) mbar_arrive(&empty[st]);
+      if ((threadIdx.x & 31) == 0) {
+        if (!EARLY) mbar_arrive(&empty[st]);
+        else if (mbar_arrive_is_last(&empty[st]) && s + T::STAGES < nstage &&
+                 atomicCAS(&claim[st], s / T::STAGES, s / T::STAGES + 1) == s / T::STAGES)
+          issue_stage3<T>(s + T::STAGES, z0, m.nz, x0, y0, stage0, full, empty, mp, lpol);
+      }
       if (newest == 0) ISLBM_ZCOMB3(S1, S2, S0);
       else if (newest == 1) ISLBM_ZCOMB3(S2, S0, S1);
       else ISLBM_ZCOMB3(S0, S1, S2);
@@ -371,8 +385,14 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
       collide_node(f, g, np);
       if (valid) store_node<3>(dst + c, m.nnp, f, g, spol, std::make_integer_sequence<int, 26>{});
     } else {
+      // hand the slot back (EARLY: the warp whose release is the last one refills it at once with stage s + STAGES)
       __syncwarp();
-      if ((threadIdx.x & 31) == 0) mbar_arrive(&empty[st]);
+      if ((threadIdx.x & 31) == 0) {
+        if (!EARLY) mbar_arrive(&empty[st]);
+        else if (mbar_arrive_is_last(&empty[st]) && s + T::STAGES < nstage &&
+                 atomicCAS(&claim[st], s / T::STAGES, s / T::STAGES + 1) == s / T::STAGES)
+          issue_stage3<T>(s + T::STAGES, z0, m.nz, x0, y0, stage0, full, empty, mp, lpol);
+      }
     }
   }
 }

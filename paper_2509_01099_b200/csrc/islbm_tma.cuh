@@ -26,6 +26,22 @@ __device__ __forceinline__ void mbar_expect_tx(uint64_t *bar, uint32_t bytes) {
 __device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
   asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
+// arrive and learn whether this arrival completed the barrier's phase (i.e. every consumer warp has released the slot)
+__device__ __forceinline__ bool mbar_arrive_is_last(uint64_t *bar) {
+  uint32_t done;
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      ".reg .b64 t;\n"
+      "mbarrier.arrive.shared::cta.b64 t, [%1];\n"
+      "mbarrier.test_wait.shared::cta.b64 p, [%1], t;\n"
+      "selp.u32 %0, 1, 0, p;\n"
+      "}\n"
+      : "=r"(done)
+      : "r"(smem_u32(bar))
+      : "memory");
+  return done != 0;
+}
 __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
   asm volatile(
       "{\n"
