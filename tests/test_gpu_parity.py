@@ -340,6 +340,28 @@ def test_full_size_configs_few_steps(islbm, name, steps):
     assert ns["Nu_hot"] == pytest.approx(no["Nu_hot"], rel=1e-10)
 
 
+@pytest.mark.parametrize("name,steps", [("c2_512sq", 1000), ("c4_128cu", 100)])
+def test_full_size_configs_long_runs(islbm, name, steps):
+    """north_star: 1e-9 on u, v, w and T after 1000 steps, at BASELINE.json's full size with the OpenMP oracle
+    (512^2: 1000 steps; 128^3: 100 steps to keep the oracle within ~20 s)."""
+    w = inputs.workload(name)
+    sim, orc = pair(islbm, w.coords, w.delta, w.Ra, w.Pr, w.Ma, threads=len(os.sched_getaffinity(0)))
+    sim.init(w.seed, w.noise_amp)
+    orc.init(w.seed, w.noise_amp)
+    sim.step(steps)
+    orc.step(steps)
+    err = field_err(sim, orc)
+    assert max(err.values()) <= 1e-9, err
+    ns, no = sim.nusselt(), orc.nusselt()
+    for k in no:
+        assert ns[k] == pytest.approx(no[k], rel=1e-9, abs=1e-12), k
+    # islbm_step(0) is a no-op
+    f0, g0 = sim.get_populations()
+    sim.step(0)
+    f1, g1 = sim.get_populations()
+    assert torch.equal(f0, f1) and torch.equal(g0, g1)
+
+
 def test_config5_256cu_sampled_nodes(islbm):
     """256^3: the oracle computes sampled nodes one by one (oracle_step_node) from the
     seeded initial state; walls, edges, corners and tile seams are all in the sample."""
