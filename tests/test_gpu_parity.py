@@ -362,6 +362,21 @@ def test_full_size_configs_long_runs(islbm, name, steps):
     assert torch.equal(f0, f1) and torch.equal(g0, g1)
 
 
+def test_config3_1024sq_1000_steps_fp64_and_fp32(islbm):
+    """BASELINE.json config 3 at full size, 1000 steps: fp64 within 1e-9 and fp32 storage within 1e-5 on u, v, T."""
+    w = inputs.workload("c3_1024sq")
+    sim, orc = pair(islbm, w.coords, w.delta, w.Ra, w.Pr, w.Ma, threads=len(os.sched_getaffinity(0)))
+    sim32 = islbm.Islbm(w.coords, w.delta, w.Ra, w.Pr, w.Ma, precision=1)
+    assert sim.kernel_name.startswith("tiled_ymarch_tma") and sim32.kernel_name.startswith("tiled_ymarch_tma")
+    for s_ in (sim, sim32, orc):
+        s_.init(w.seed, w.noise_amp)
+        s_.step(1000)
+    err = field_err(sim, orc)
+    assert max(err.values()) <= 1e-9, err
+    e32 = field_err(sim32, orc)
+    assert e32["u"] <= 1e-5 and e32["v"] <= 1e-5 and e32["T"] <= 1e-5, e32
+
+
 def test_config5_256cu_sampled_nodes(islbm):
     """256^3: the oracle computes sampled nodes one by one (oracle_step_node) from the
     seeded initial state; walls, edges, corners and tile seams are all in the sample."""
