@@ -136,6 +136,25 @@ int islbm_create(islbm_t **out, const islbm_mesh *mesh, int lattice, double Ra,
 int islbm_create_slab(islbm_t **out, const islbm_mesh *mesh, int lattice, double Ra, double Pr, double Ma,
                       int precision, void *dev_workspace, size_t bytes, void *cuda_stream, const islbm_slab *slab);
 int islbm_halo(islbm_t *h, int side /* 0 low, 1 high */, islbm_halo_info *out);
+/* Fused halo exchange over peer memory.  islbm_halo_layout describes where this handle's ghost layer of `side`
+ * lives in ITS workspace, for both ping-pong buffers; the neighbour passes that description, together with this
+ * workspace as mapped in the neighbour's process (same process: the pointer itself; another process on the node:
+ * a CUDA IPC mapping, peer access over NVLink), to islbm_slab_set_peer on its facing side.  From then on the
+ * neighbour's step kernel stores the halo planes of its boundary layer straight into this ghost layer as it emits
+ * them, and no separate exchange is needed; the caller only has to order the steps (both ranks finish step t before
+ * either starts step t+1: a stream-ordered barrier).  Both handles must step in lockstep from the same
+ * islbm_init / islbm_set_populations.  peer_workspace = NULL detaches. */
+typedef struct {
+  int is_wall;
+  int cur;                    /* index of the buffer that holds the current state (the next step writes 1 - cur) */
+  size_t ghost_offset[2];     /* byte offset of the ghost layer of the first halo plane, per ping-pong buffer */
+  size_t plane_pitch_bytes;
+  size_t layer_bytes;
+} islbm_halo_layout_info;
+int islbm_halo_layout(islbm_t *h, int side, islbm_halo_layout_info *out);
+int islbm_slab_set_peer(islbm_t *h, int side, void *peer_workspace /* DEVICE */, const size_t ghost_offset[2],
+                        size_t plane_pitch_bytes);
+
 /* HOST s[8]: this handle's Eq. 29-weighted partial sums (ghost layers weigh 0); synchronises the stream. */
 int islbm_diag_sums(islbm_t *h, double s[8]);
 /* HOST out[6] = Nu_hot, Nu_cold, <Re>, <u*^2>_V, <Nu>, Nu_middle from sums added over all slabs (pure host). */

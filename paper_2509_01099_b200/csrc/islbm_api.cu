@@ -93,6 +93,11 @@ struct islbm {
   int npad;
   bool is_slab;                // slab of a larger cavity along the slowest axis (islbm_create_slab)
   islbm_slab slab;
+  // fused halo exchange: the neighbour's workspace as mapped in this process, the byte offsets of its ghost layer
+  // (first halo plane) in its two ping-pong buffers, and its plane pitch in bytes
+  char *peer_base[2];
+  size_t peer_ghost_off[2][2];
+  size_t peer_pitch_bytes[2];
   islbm_params prm;
   double buoy;
   double T0;               // reference temperature of the buoyancy force
@@ -319,6 +324,9 @@ static int create_impl(islbm_t **out, const islbm_mesh *mesh, int lattice, doubl
   dm.T_hot = 0.5;      // PAPER.md:237, 430; BASELINE.json configs (A11)
   dm.T_cold = -0.5;
   dm.stencil = 0;
+  dm.peer[0] = dm.peer[1] = nullptr;
+  dm.peer_pitch[0] = dm.peer_pitch[1] = 0;
+  h->peer_base[0] = h->peer_base[1] = nullptr;
   {
     const int nm = h->n[h->dim - 1];
     dm.wall_mlo = !slab || slab->lo_is_wall;
@@ -572,7 +580,14 @@ extern "C" int islbm_step(islbm_t *h, int n) {
   if (n < 0) return fail(ISLBM_ERR_ARG, "n < 0");
   if (!h->has_state) return fail(ISLBM_ERR_STATE, "islbm_step before islbm_init / islbm_set_populations");
   const int which = effective_kernel(h);
+  if ((h->peer_base[0] || h->peer_base[1]) && which == 3)
+    return fail(ISLBM_ERR_STATE, "the fused halo exchange is not available with the pure-shift kernel");
   for (int s = 0; s < n; ++s) {
+    // fused halo exchange: this step writes buffer 1 - cur, and so does the neighbour (both step in lockstep)
+    for (int sd = 0; sd < 2; ++sd) {
+      h->dm.peer[sd] = h->peer_base[sd] ? (void *)(h->peer_base[sd] + h->peer_ghost_off[sd][1 - h->cur]) : nullptr;
+      h->dm.peer_pitch[sd] = h->peer_base[sd] ? (long long)(h->peer_pitch_bytes[sd] / h->st_bytes) : 0;
+    }
     if (which == 2) {
       void *bufs[2] = {h->ws + h->cv.buf[0], h->ws + h->cv.buf[1]};
       cudaError_t e;
@@ -683,6 +698,39 @@ extern "C" int islbm_halo(islbm_t *h, int side, islbm_halo_info *out) {
   const int recv_layer = side == 0 ? 0 : nm - 1;
   out->send_offset = base + (size_t)send_layer * layer;
   out->recv_offset = base + (size_t)recv_layer * layer;
+  return ISLBM_OK;
+}
+
+extern "C" int islbm_halo_layout(islbm_t *h, int side, islbm_halo_layout_info *out) {
+  if (!h || !out) return fail(ISLBM_ERR_ARG, "NULL argument");
+  if (side != 0 && side != 1) return fail(ISLBM_ERR_ARG, "side must be 0 (low) or 1 (high)");
+  const int nm = h->n[h->dim - 1];
+  const size_t layer = (size_t)h->dm.nxp * (h->dim == 3 ? h->n[1] : 1) * h->st_bytes;
+  const size_t pitch = (size_t)h->dm.nnp * h->st_bytes;
+  const int first = h->dim == 2 ? 6 : 14;
+  out->is_wall = side == 0 ? h->dm.wall_mlo : h->dm.wall_mhi;
+  out->plane_pitch_bytes = pitch;
+  out->layer_bytes = layer;
+  out->cur = h->cur;
+  for (int b = 0; b < 2; ++b)
+    out->ghost_offset[b] = h->cv.buf[b] + (size_t)first * pitch + (size_t)(side == 0 ? 0 : nm - 1) * layer;
+  return ISLBM_OK;
+}
+
+extern "C" int islbm_slab_set_peer(islbm_t *h, int side, void *peer_workspace, const size_t ghost_offset[2],
+                                   size_t plane_pitch_bytes) {
+  if (!h) return fail(ISLBM_ERR_ARG, "NULL handle");
+  if (side != 0 && side != 1) return fail(ISLBM_ERR_ARG, "side must be 0 (low) or 1 (high)");
+  if (!h->is_slab) return fail(ISLBM_ERR_STATE, "not a slab handle");
+  if (side == 0 ? h->dm.wall_mlo : h->dm.wall_mhi) return fail(ISLBM_ERR_ARG, "this side is a wall: it has no neighbour");
+  if (peer_workspace && (!ghost_offset || plane_pitch_bytes == 0 || plane_pitch_bytes % h->st_bytes))
+    return fail(ISLBM_ERR_ARG, "bad peer layout");
+  h->peer_base[side] = (char *)peer_workspace;         // NULL detaches (exchange outside the kernel again)
+  if (peer_workspace) {
+    h->peer_ghost_off[side][0] = ghost_offset[0];
+    h->peer_ghost_off[side][1] = ghost_offset[1];
+    h->peer_pitch_bytes[side] = plane_pitch_bytes;
+  }
   return ISLBM_OK;
 }
 

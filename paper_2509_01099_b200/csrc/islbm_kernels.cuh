@@ -41,6 +41,13 @@ struct DevMesh {
   int em_lo, em_hi;
   int wall_mlo, wall_mhi;
   long long node_offset; // global linear index of local node 0 (islbm_init draws the noise by global index)
+  // fused halo exchange (islbm_slab_set_peer): peer[s] points at the neighbour's ghost layer, in the buffer the
+  // neighbour writes during this step, of the FIRST halo plane (plane index kHaloFirst<DIM>); peer_pitch[s] is the
+  // neighbour's plane pitch in elements.  The thread that emits this rank's first (s = 0) / last (s = 1) owned layer
+  // also stores the halo planes of its node there: NVLink peer stores from inside the step kernel, no separate
+  // exchange pass.  nullptr: no neighbour on that side, or the exchange is done outside (islbm_halo).
+  void *peer[2];
+  long long peer_pitch[2];
   int stencil;           // 0: {j-1,j,j+1} (A2); 1: upwind {j-2,j-1,j} for c=+1, {j,j+1,j+2} for c=-1
                          // (generic kernel only; the TMA kernels stage a 1-node halo and take stencil 0)
 };
@@ -206,6 +213,28 @@ __device__ __forceinline__ void pull_all_g(const DevMesh &m, const ST *src, cons
   ((g[Qs] = pull_g<DIM, Qs>(m, src, cx)), ...);
 }
 
+// fused halo exchange: the halo planes of this node into the neighbour's ghost layer (DevMesh::peer), plain stores
+template <int DIM, int K, typename ST>
+__device__ __forceinline__ void peer_plane(ST *p, const double *f, const double *g) {
+  constexpr int QF = Lat<DIM>::QF;
+  constexpr int code = pop_of_plane<DIM>(halo_first_plane<DIM>() + K);
+  if constexpr (code < QF) *p = to_storage<ST, DIM>(f[code], code);
+  else *p = (ST)g[code - QF];
+}
+template <int DIM, typename ST, int... Ks>
+__device__ __forceinline__ void peer_store(void *base, long long pitch, long long inplane, const double *f, const double *g,
+                                           std::integer_sequence<int, Ks...>) {
+  ST *p = reinterpret_cast<ST *>(base) + inplane;
+  (peer_plane<DIM, Ks>(p + (long long)Ks * pitch, f, g), ...);
+}
+template <int DIM, typename ST>
+__device__ __forceinline__ void peer_store_node(const DevMesh &m, int layer, long long inplane, const double *f, const double *g) {
+  if (m.peer[0] != nullptr && layer == m.em_lo)
+    peer_store<DIM, ST>(m.peer[0], m.peer_pitch[0], inplane, f, g, std::make_integer_sequence<int, halo_plane_count<DIM>()>{});
+  if (m.peer[1] != nullptr && layer == m.em_hi - 1)
+    peer_store<DIM, ST>(m.peer[1], m.peer_pitch[1], inplane, f, g, std::make_integer_sequence<int, halo_plane_count<DIM>()>{});
+}
+
 // ---------------------------------------------------------------------------
 // generic step: one thread per node, neighbours read from global memory
 // through L1/L2.  COLLIDE = false writes the pre-collision f_{t+1}, g_{t+1} as
@@ -233,6 +262,7 @@ k_step_generic(DevMesh m, NodeParams np, const ST *__restrict__ src, ST *__restr
     for (int q = 0; q < QF; ++q) dst[(long long)plane_f<DIM>(q) * m.nnp + cx.c] = to_storage<ST, DIM>(f[q], q);
 #pragma unroll
     for (int q = 0; q < QG; ++q) dst[(long long)plane_g<DIM>(q) * m.nnp + cx.c] = (ST)g[q];
+    peer_store_node<DIM, ST>(m, DIM == 3 ? iz : iy, DIM == 3 ? (long long)iy * m.nxp + ix : (long long)ix, f, g);
   } else {
 #pragma unroll
     for (int q = 0; q < QF; ++q) fout[(long long)q * m.nn + cx.cd] = f[q];

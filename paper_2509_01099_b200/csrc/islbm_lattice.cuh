@@ -92,6 +92,11 @@ ISLBM_HD constexpr int plane_g(int q) {
   }
 }
 
+// the planes whose velocity has a component along the slowest axis (the slab axis) form one contiguous range of
+// the storage order: the halo of a slab decomposition
+template <int DIM> ISLBM_HD constexpr int halo_first_plane() { return DIM == 2 ? 6 : 14; }
+template <int DIM> ISLBM_HD constexpr int halo_plane_count() { return DIM == 2 ? 8 : 12; }
+
 // inverse of plane_f / plane_g: the population stored in plane p (flow q as q, temperature q as QF + q)
 template <int DIM>
 ISLBM_HD constexpr int pop_of_plane(int p) {

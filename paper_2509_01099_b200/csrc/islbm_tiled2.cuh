@@ -228,7 +228,10 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
       }
       add_bias<ST, 2>(f);
       collide_node(f, g, np);
-      if (valid) store_node<2>(dst + c, m.nnp, f, g, spol, std::make_integer_sequence<int, 14>{});
+      if (valid) {
+        store_node<2>(dst + c, m.nnp, f, g, spol, std::make_integer_sequence<int, 14>{});
+        peer_store_node<2, ST>(m, y, x, f, g);
+      }
     } else {
       // hand the slot back; the warp whose release is the last one refills it at once with stage s + STAGES, so
       // STAGES - 1 stages are in flight whenever one is being consumed

@@ -383,7 +383,10 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
       }
       add_bias<ST, 3>(f);
       collide_node(f, g, np);
-      if (valid) store_node<3>(dst + c, m.nnp, f, g, spol, std::make_integer_sequence<int, 26>{});
+      if (valid) {
+        store_node<3>(dst + c, m.nnp, f, g, spol, std::make_integer_sequence<int, 26>{});
+        peer_store_node<3, ST>(m, z, cxy, f, g);
+      }
     } else {
       // hand the slot back (EARLY: the warp whose release is the last one refills it at once with stage s + STAGES)
       __syncwarp();

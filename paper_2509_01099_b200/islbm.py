@@ -20,7 +20,7 @@ F64, F32_STORAGE = 0, 1
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED, KERNEL_UNIFORM_SHIFT = 0, 1, 2, 3
 
 EXPORTS = (
-    "islbm_workspace_bytes", "islbm_create", "islbm_create_slab", "islbm_halo", "islbm_diag_sums", "islbm_diag_from_sums",
+    "islbm_workspace_bytes", "islbm_create", "islbm_create_slab", "islbm_halo", "islbm_halo_layout", "islbm_slab_set_peer", "islbm_diag_sums", "islbm_diag_from_sums",
     "islbm_residual_sums", "islbm_destroy", "islbm_get_params", "islbm_init",
     "islbm_set_populations", "islbm_set_populations_host", "islbm_get_populations", "islbm_step", "islbm_fields", "islbm_nusselt", "islbm_nusselt_middle",
     "islbm_steady_residual", "islbm_set_buoyancy_scale", "islbm_set_reference_temperature", "islbm_set_stencil", "islbm_set_kernel", "islbm_set_tuning", "islbm_launch_count",
@@ -39,6 +39,11 @@ class _Slab(C.Structure):
 class _Halo(C.Structure):
     _fields_ = [("is_wall", C.c_int), ("first_plane", C.c_int), ("n_planes", C.c_int), ("plane_pitch_bytes", C.c_size_t),
                 ("layer_bytes", C.c_size_t), ("send_offset", C.c_size_t), ("recv_offset", C.c_size_t)]
+
+
+class _HaloLayout(C.Structure):
+    _fields_ = [("is_wall", C.c_int), ("cur", C.c_int), ("ghost_offset", C.c_size_t * 2), ("plane_pitch_bytes", C.c_size_t),
+                ("layer_bytes", C.c_size_t)]
 
 
 class _Params(C.Structure):
@@ -64,6 +69,8 @@ def _load():
     lib.islbm_create_slab.argtypes = [C.POINTER(vp), C.POINTER(_Mesh), C.c_int, C.c_double, C.c_double, C.c_double,
                                       C.c_int, vp, C.c_size_t, vp, C.POINTER(_Slab)]
     lib.islbm_halo.argtypes = [vp, C.c_int, C.POINTER(_Halo)]
+    lib.islbm_halo_layout.argtypes = [vp, C.c_int, C.POINTER(_HaloLayout)]
+    lib.islbm_slab_set_peer.argtypes = [vp, C.c_int, vp, C.POINTER(C.c_size_t), C.c_size_t]
     lib.islbm_diag_sums.argtypes = [vp, dp]
     lib.islbm_diag_from_sums.argtypes = [vp, dp, dp]
     lib.islbm_residual_sums.argtypes = [vp, dp, C.POINTER(C.c_int)]
@@ -256,6 +263,22 @@ class Islbm:
         recv = [self.workspace[hi.recv_offset + p * hi.plane_pitch_bytes: hi.recv_offset + p * hi.plane_pitch_bytes + hi.layer_bytes]
                 for p in range(hi.n_planes)]
         return bool(hi.is_wall), send, recv
+
+    def halo_layout(self, side):
+        """Plain dict (picklable) describing this handle's ghost layer of `side` inside its workspace."""
+        hl = _HaloLayout()
+        _check(lib.islbm_halo_layout(self.h, int(side), C.byref(hl)))
+        return dict(is_wall=bool(hl.is_wall), cur=hl.cur, ghost_offset=[hl.ghost_offset[0], hl.ghost_offset[1]],
+                    plane_pitch_bytes=hl.plane_pitch_bytes, layer_bytes=hl.layer_bytes)
+
+    def set_peer(self, side, peer_workspace_ptr, layout):
+        """peer_workspace_ptr: device address of the neighbour's workspace as mapped in this process (0 detaches);
+        layout: the neighbour's halo_layout() of its facing side."""
+        if not peer_workspace_ptr:
+            _check(lib.islbm_slab_set_peer(self.h, int(side), None, None, 0))
+            return
+        off = (C.c_size_t * 2)(*layout["ghost_offset"])
+        _check(lib.islbm_slab_set_peer(self.h, int(side), C.c_void_p(int(peer_workspace_ptr)), off, layout["plane_pitch_bytes"]))
 
     def diag_sums(self):
         s = (C.c_double * 8)()

@@ -67,7 +67,12 @@ def exchange_p2p(send_lo, recv_lo, send_hi, recv_hi, rank: int, world: int, dist
 
 
 class SlabCavity:
-    """The cavity of `coords` decomposed over `world` ranks; this object is rank `rank`'s slab."""
+    """The cavity of `coords` decomposed over `world` ranks; this object is rank `rank`'s slab.
+
+    Two ways to move the halo: (default) after every step, batched isend/irecv of the halo layers
+    (`exchange_p2p`); or, after `connect_ipc()` / `connect_local()`, FUSED: each rank's step kernel stores its
+    boundary layers straight into the neighbour's ghost layers through peer-mapped memory (NVLink) while it emits
+    them, and the only thing left between two steps is a barrier."""
 
     def __init__(self, coords, delta, Ra, Pr, Ma, rank, world, precision=0, device="cuda", exchange=None):
         from . import islbm
@@ -75,6 +80,34 @@ class SlabCavity:
         local, slab, self.own, self.ghosts = slab_inputs(coords, delta, rank, world)
         self.sim = islbm.Islbm(local, delta, Ra, Pr, Ma, precision=precision, device=device, slab=slab)
         self._exchange = exchange or self._exchange_dist
+        self._peers = []          # keeps the IPC mappings of the neighbours' workspaces alive
+
+    # -- fused halo exchange ----------------------------------------------------------------------------------
+    def connect_ipc(self):
+        """One process per rank on one node: map the neighbours' workspaces with CUDA IPC (torch's tensor sharing),
+        hand them to the library, and switch to the fused exchange.  Collective over the default process group."""
+        import torch
+        import torch.distributed as dist
+        from torch.multiprocessing.reductions import reduce_tensor
+        mine = dict(tensor=reduce_tensor(self.sim.workspace), lo=self.sim.halo_layout(0), hi=self.sim.halo_layout(1))
+        everyone = [None] * self.world
+        dist.all_gather_object(everyone, mine)
+        for side, nb in ((0, self.rank - 1), (1, self.rank + 1)):
+            if 0 <= nb < self.world:
+                fn, args = everyone[nb]["tensor"]
+                t = fn(*args)                                   # the neighbour's workspace, mapped here
+                self._peers.append(t)
+                self.sim.set_peer(side, t.data_ptr(), everyone[nb]["hi" if side == 0 else "lo"])
+        backend = dist.get_backend()
+        flag = torch.zeros(1, device=self.sim.device if backend == "nccl" else "cpu")
+
+        def barrier():
+            if backend == "nccl":
+                dist.all_reduce(flag)                           # stream-ordered: completes when every rank's step has
+            else:
+                torch.cuda.synchronize(self.sim.device)
+                dist.barrier()
+        self._exchange = barrier
 
     # -- halo -------------------------------------------------------------------------------------------------
     def halo_views(self):
@@ -114,6 +147,17 @@ class SlabCavity:
 
     def close(self):
         self.sim.close()
+
+
+def connect_local(slabs):
+    """Fused halo exchange among slabs that live in ONE process on ONE device: each handle gets its neighbours'
+    workspaces as peers; the shared stream orders the steps, so no barrier is needed."""
+    for a in range(len(slabs) - 1):
+        lower, upper = slabs[a].sim, slabs[a + 1].sim
+        lower.set_peer(1, upper.workspace.data_ptr(), upper.halo_layout(0))
+        upper.set_peer(0, lower.workspace.data_ptr(), lower.halo_layout(1))
+    for s in slabs:
+        s._exchange = lambda: None
 
 
 def exchange_local(slabs):

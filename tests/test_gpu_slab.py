@@ -31,10 +31,11 @@ def mesh(dim, ns, st):
     return coords, delta, 0.71 * (0.1 * H_lu / 0.03) ** 2
 
 
+@pytest.mark.parametrize("fused", [False, True], ids=["exchange", "fused"])
 @pytest.mark.parametrize("dim,ns,world,prec,kernel", [
     (2, (70, 45), 2, 0, 0), (2, (70, 45), 4, 0, 0), (2, (131, 20), 5, 1, 0), (2, (40, 33), 3, 0, 1),
     (3, (40, 24, 37), 3, 0, 0), (3, (33, 17, 9), 2, 1, 0), (3, (36, 18, 16), 8, 0, 0), (3, (20, 12, 11), 2, 0, 1)])
-def test_slabs_equal_the_single_domain_bitwise(islbm, dim, ns, world, prec, kernel):
+def test_slabs_equal_the_single_domain_bitwise(islbm, dim, ns, world, prec, kernel, fused):
     coords, delta, Ra = mesh(dim, ns, (1.4, 1.2, 1.3))
     Ma = 0.1 * SQ3
     whole = islbm.Islbm(coords, delta, Ra, 0.71, Ma, precision=prec)
@@ -47,11 +48,14 @@ def test_slabs_equal_the_single_domain_bitwise(islbm, dim, ns, world, prec, kern
     for s in slabs:
         s.init(3, 1e-3)
         assert whole.params()["H_lu"] == s.sim.params()["H_lu"]
+    if fused:
+        slab.connect_local(slabs)        # the step kernels store the halo into the neighbours' ghost layers themselves
+    halo = (lambda: None) if fused else (lambda: slab.exchange_local(slabs))
     for _ in range(7):
         whole.step(1)
         for s in slabs:
             s.sim.step(1)
-        slab.exchange_local(slabs)
+        halo()
     fw = whole.fields()
     fw_pop, gw_pop = whole.get_populations()
     for s in slabs:
@@ -77,7 +81,7 @@ def test_slabs_equal_the_single_domain_bitwise(islbm, dim, ns, world, prec, kern
     whole.step(1)
     for s in slabs:
         s.sim.step(1)
-    slab.exchange_local(slabs)
+    halo()
     sums = np.sum([s.sim.residual_sums()[0] for s in slabs], axis=0)
     ru, rT = whole.steady_residual()
     assert sums[0] / sums[1] == pytest.approx(ru, rel=1e-10) and sums[2] / sums[3] == pytest.approx(rT, rel=1e-10)
@@ -105,3 +109,58 @@ def test_slabs_against_the_oracle(islbm):
         for k in ("u", "v", "w"):
             assert np.abs(s.owned(fl[k]).cpu().numpy() - fo[k][lo:hi]).max() <= 1e-10 * max(umax, 1e-4)
         assert np.abs(s.owned(fl["T"]).cpu().numpy() - fo["T"][lo:hi]).max() <= 1e-12
+
+
+_IPC_WORKER = r"""
+import os, sys, json
+sys.path.insert(0, {root!r})
+import numpy as np, torch, torch.distributed as dist
+from paper_2509_01099_b200 import inputs, slab, islbm
+rank, world = int(os.environ["RANK"]), 2
+dist.init_process_group(backend="gloo", init_method="tcp://127.0.0.1:{port}", rank=rank, world_size=world)
+coords = [inputs.tanh_mesh(n, s)[0] for n, s in zip((40, 24, 22), (1.4, 1.2, 1.3))]
+delta = min(float(np.diff(c).min()) for c in coords)
+H = (coords[1][-1] - coords[1][0] + delta) / delta
+Ra = 0.71 * (0.1 * H / 0.03) ** 2
+cav = slab.SlabCavity(coords, delta, Ra, 0.71, 0.1 * 3 ** 0.5, rank, world)
+cav.init(3, 1e-3)
+cav.connect_ipc()                       # CUDA IPC mapping of the neighbour's workspace + fused exchange
+cav.step(6)
+d = cav.diagnostics()
+lo, hi = cav.own
+T = cav.owned(cav.sim.fields(("T",))["T"]).cpu().numpy()
+np.save({out!r} + f"_{{rank}}.npy", T)
+print(json.dumps(dict(rank=rank, own=[lo, hi], **d)))
+dist.barrier()
+cav.close()
+dist.destroy_process_group()
+"""
+
+
+def test_two_processes_one_gpu_fused_exchange_over_cuda_ipc(islbm, tmp_path):
+    """Two ranks as two PROCESSES sharing the one GPU: control plane gloo, data plane CUDA IPC (each rank's step
+    kernel stores its boundary layer into the other process's workspace).  The ranks are ordered by a host barrier
+    after a device synchronise, so no kernel ever waits on another; result against the single-domain run."""
+    import subprocess, sys, json
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    port = 29900 + os.getpid() % 2000
+    script = tmp_path / "w.py"
+    script.write_text(_IPC_WORKER.format(root=root, port=port, out=str(tmp_path / "T")))
+    procs = [subprocess.Popen([sys.executable, str(script)], env={**os.environ, "RANK": str(r)}, stdout=subprocess.PIPE,
+                              stderr=subprocess.PIPE, text=True) for r in range(2)]
+    outs = []
+    for p in procs:
+        so, se = p.communicate(timeout=600)
+        assert p.returncode == 0, se[-2000:]
+        outs.append(json.loads(so.strip().splitlines()[-1]))
+    coords, delta, Ra = mesh(3, (40, 24, 22), (1.4, 1.2, 1.3))
+    whole = islbm.Islbm(coords, delta, Ra, 0.71, 0.1 * SQ3)
+    whole.init(3, 1e-3)
+    whole.step(6)
+    Tw = whole.fields(("T",))["T"].cpu().numpy()
+    nu = whole.nusselt()
+    for o in outs:
+        lo, hi = o["own"]
+        assert np.array_equal(np.load(str(tmp_path / "T") + f"_{o['rank']}.npy"), Tw[lo:hi])
+        for k in nu:
+            assert o[k] == pytest.approx(nu[k], rel=1e-11, abs=1e-13), k
