@@ -112,8 +112,10 @@ typedef struct {
 } islbm_halo_info;
 
 /* Bytes of DEVICE workspace islbm_create needs for this mesh / lattice /
- * precision (two ping-pong population buffers + interpolation tables +
- * reduction scratch).  Pure host arithmetic. */
+ * precision: two ping-pong population buffers (rows padded to 16 elements, planes
+ * in the storage order of DESIGN.md 5) + interpolation tables + reduction scratch
+ * + a 4*nn-double area used as the Eq. 30 snapshot and as the staging buffer of
+ * islbm_set_populations_host.  Pure host arithmetic. */
 int islbm_workspace_bytes(const islbm_mesh *mesh, int lattice, int precision,
                           size_t *bytes);
 
