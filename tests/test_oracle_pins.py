@@ -793,3 +793,43 @@ def test_upwind_and_central_stencils_differ_on_a_stretched_mesh_but_share_the_co
         o.step(50)
         res.append(o.fields()["T"].copy())
     assert 1e-9 < np.abs(res[0] - res[1]).max() < 1e-2
+
+
+# ---------------------------------------------------------------------------
+# normalisation of <Re>, <u*^2>_V and <Nu> (Eq. 31, 34)
+# ---------------------------------------------------------------------------
+@pytest.mark.parametrize("dim,n", [(2, 14), (3, 7)])
+def test_volume_diagnostics_closed_forms_for_uniform_velocity(dim, n):
+    """Uniform velocity (u0, v0[, w0]), buoyancy off, T = c + (antisymmetric about the cavity centre): the Eq. 29
+    weights are symmetric and sum to L_eff, so <Re> = sqrt(Ra/Pr)|u0|/U, <u*^2> = |u0|^2/U^2 and
+    <Nu> = 1 + sqrt(Ra Pr) (u0/U) c, whatever the stretching."""
+    w = inputs.custom_workload("d", dim, n, stretch=1.6, Ra=3e4)
+    o = Oracle(w.coords, w.delta, w.Ra, w.Pr, w.Ma)
+    o.set_buoyancy_scale(0.0)
+    p = o.params()
+    ef, _ = o.velocities()
+    o.init(0, 0.0)
+    f0, _ = o.get_populations()
+    wts = f0[:, 0, 0, 0].copy()
+    u0 = np.array([0.013, -0.007, 0.004])[:dim] * p["U"]
+    f = np.empty((o.qf,) + o.shape)
+    for i in range(o.qf):
+        eu = float(ef[i][:dim] @ u0)
+        f[i] = wts[i] * (1.0 + 3.0 * eu + 4.5 * eu * eu - 1.5 * float(u0 @ u0))     # second-order equilibrium: sum e f = rho u0
+    x = np.asarray(w.coords[0])
+    xc = 0.5 * (x[0] + x[-1])
+    c = 0.21
+    T = c + 0.4 * np.sin(3.0 * (x - xc)) + 0.1 * (x - xc) ** 3                      # c + odd function of (x - centre)
+    wg = np.full(o.qg, p["omega_bc"] / 2)
+    wg[0] = 1 - wg[1:].sum()
+    g = np.empty((o.qg,) + o.shape)
+    for i in range(o.qg):
+        g[i] = (wg[i] * T)[None, None, :]
+    o.set_populations(f, g)
+    fl = o.fields()
+    assert np.abs(fl["u"] - u0[0]).max() < 1e-15 and np.abs(fl["rho"] - 1).max() < 1e-14
+    d = o.nusselt()
+    speed = float(np.linalg.norm(u0))
+    assert d["Re"] == pytest.approx(math.sqrt(w.Ra / w.Pr) * speed / p["U"], rel=1e-12)
+    assert d["u2"] == pytest.approx(speed ** 2 / p["U"] ** 2, rel=1e-12)
+    assert d["Nu_vol"] == pytest.approx(1.0 + math.sqrt(w.Ra * w.Pr) * (u0[0] / p["U"]) * c, rel=1e-11)
