@@ -658,3 +658,14 @@ def test_paper_mode_table4_ra1e5_129(islbm, golden):
     assert nu["Nu_hot"] == pytest.approx(ref[1], rel=6e-3)
     assert nu["Nu_cold"] == pytest.approx(nu["Nu_hot"], rel=1e-6)
     assert math.sqrt(1e5 / 0.71 * nu["u2"]) == pytest.approx(ref[3], rel=3e-3)
+
+
+def test_command_line_driver(islbm, capsys):
+    """python -m paper_2509_01099_b200.run: a short paper-mode run prints parameters and a diagnostics line per report."""
+    import json as _json
+    from paper_2509_01099_b200 import run
+    run.main(["--paper", "--dim", "2", "--points", "65", "--Ra", "1e5", "--steps", "400", "--every", "200"])
+    lines = [_json.loads(l) for l in capsys.readouterr().out.strip().splitlines()]
+    assert lines[0]["T0"] == -0.5 and lines[0]["kernel"].startswith("tiled_ymarch_tma") and lines[0]["nodes"] == 63 * 63
+    assert [l["step"] for l in lines[1:]] == [200, 400]
+    assert all(np.isfinite(l["Nu_hot"]) and l["Re_rms"] >= l["Re"] for l in lines[1:])
