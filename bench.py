@@ -2,14 +2,22 @@
 """bench.py — MLUPS / roofline fraction / WCTpDT of the ISLBM hot path on B200.
 
     python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--workload NAME]
+                    [--precision f64|f32] [--kernel 0..3] [--decomp replicas|slab] [--halo fused|p2p] [--no-extras]
 
 One bench "step" is one pass of the whole hot path over one batch: LBM_PER_STEP
 time steps (collide + stream/interpolate + walls)
 followed by one Nusselt/Reynolds reduction (row a6).  `value` is whole-job MLUPS
-(Eq. 38) with the state resident in HBM; `e2e` is the same metric
-with the pre-collision state uploaded from pinned host memory inside the timed
-region.  N > 1 runs N independent cavities (one per rank, no data-path
-collective): weak scaling.  Rank 0 prints ONE JSON line.
+(Eq. 38) with the state resident in HBM; `roofline` is the step
+kernel alone (CUDA events around the islbm_step calls inside the timed region)
+against the measured copy bandwidth; `e2e` is the same metric with the
+pre-collision state passed in pinned HOST memory to islbm_set_populations_host
+every step (the H2D copies happen inside the C-ABI call) and the diagnostics read
+back to the host; `cpu_baseline` times the oracle on the host cores.  N > 1 runs
+N independent cavities (one per rank, no data-path collective): weak scaling —
+or, with --decomp slab, ONE cavity in slabs with the halo stored by the step
+kernels into peer memory: strong scaling.  Rank 0 prints ONE JSON line.
+`also` holds the other BASELINE.json configs, the uniform-mesh counterparts
+(general kernel and pure-shift kernel) and the non-uniform/uniform ratios.
 """
 from __future__ import annotations
 
