@@ -367,7 +367,9 @@ def main():
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
                 "traffic": read_traffic(args.workload, r["kernel"]), "kernel": r["kernel"],
                 "algorithmic_bytes_per_launch": bpu * w.nodes, "bytes_per_update": bpu,
-                "avg_launch_us": t_launch * 1e6, "peak_source": peak_src}
+                "avg_launch_us": t_launch * 1e6, "peak_source": peak_src,
+                "frac_of_nominal_8000GBs": achieved / 8000.0,      # secondary, against the nominal HBM3e figure
+                "dram_bytes_per_update": (read_traffic(args.workload, r["kernel"]) or 0) / w.nodes or None}
 
     e2e = None
     cpu = None
