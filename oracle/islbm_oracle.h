@@ -18,12 +18,19 @@
  *   pinned   : lattice algebra (P3), interpolation weights (P1), uniform-mesh
  *              reduction to textbook streaming (P2), mass (P4), conduction
  *              fixed point (P5), wall derivative (P6), brute-force step (P7),
- *              parameter map (P8), q_kappa (closed form from a_T).
+ *              parameter map (P8), q_kappa (closed form from a_T),
+ *              normalisation of <Re>, <u*^2>, <Nu> (P12), Nu_middle (P13: exact on
+ *              quadratic T and uniform advection, = 1 on the conduction state).
  *   parity unpinned : the choice of the destination-centred stencil
  *              {j-1,j,j+1} (A2; Fig. 1 and ref [28] are not in PAPER.md) and
  *              the relaxation rates s_e, s_eps, s_q, q_e, q_nu (A7; refs
  *              [8,37,38] are not in PAPER.md).  End-to-end evidence only
- *              (Table 2 / Table 4 reproduction on the GPU path).
+ *              (Table 2 / Table 4 reproduction on the GPU path: DESIGN.md 3.1).  The
+ *              alternative upwind stencil (oracle_set_stencil) is pinned the same way as
+ *              the central one; which of the two the authors used stays undecided.
+ *   readings without a formula to pin: the reference temperature T0 of the buoyancy force
+ *              (A9: 0 by default, T_cold in the paper's mode) and the form of <Re> the tables
+ *              print (A22) are choices of input / output convention, not of arithmetic.
  *
  * Layout of every population array: [q][z][y][x], x fastest, fp64.
  * Layout of every field array:      [z][y][x].
