@@ -231,7 +231,9 @@ int islbm_set_stencil(islbm_t *h, int kind);
 /* 0 = auto (fastest kernel for this mesh), 1 = generic global-memory kernel,
  * 2 = TMA-staged shared-memory kernel (y-marching in 2-D, z-marching in 3-D),
  * 3 = uniform-mesh pure-shift kernel (only valid when every spacing equals
- * delta bit-exactly; Eq. 17-20 on the uniform mesh of Eq. 24-25). */
+ * delta to within 1e-10 relative; Eq. 17-20 on the uniform mesh of Eq. 24-25;
+ * identical to the interpolating kernels when the spacings are bit-exact,
+ * e.g. N a power of two, otherwise to that relative accuracy per step). */
 int islbm_set_kernel(islbm_t *h, int which);
 /* Run-time knobs of the TMA-staged kernels.  key: "chunk" (marching
  * chunk length, 0 = automatic), "l2promo" (tensor-map L2 promotion 0 none, 1 64 B,

@@ -269,7 +269,9 @@ static int create_impl(islbm_t **out, const islbm_mesh *mesh, int lattice, doubl
       if (!(d > 0.0)) return fail(ISLBM_ERR_MESH, "coordinates must be strictly increasing");
       if (!(d >= mesh->delta * (1.0 - 1e-12)))
         return fail(ISLBM_ERR_MESH, "a mesh spacing is smaller than delta: the departure point would leave the adjacent cell");
-      if (d != mesh->delta) uniform = false;
+      // "uniform" enables the pure-shift kernel on request: spacings equal to delta to within 1e-10 relative (exactly
+      // equal for power-of-two N; otherwise the shift differs from the interpolation by that much per step)
+      if (std::fabs(d - mesh->delta) > 1e-10 * mesh->delta) uniform = false;
     }
   }
   islbm *h = new islbm();

@@ -281,16 +281,18 @@ inline bool plan2_setup(Plan2 &p, const int *n, int nxp, void *buf0, void *buf1,
     cudaGetLastError();
     occ = 1;
   }
-  // one full wave of resident CTAs; small meshes get chunks down to 2 rows (measured: a 2-D CTA needs ~1.5 us per
-  // row whatever the mesh, so latency, not the doubled prologue traffic, decides there)
+  // chunks (measured, profiles/): short chunks win (8 rows: 0.90-0.94 at 2049^2..8193^2 against 0.73-0.87 for 60-row
+  // chunks), and the CTA count should be a whole number of waves of resident CTAs.  So: k waves, k the smallest number
+  // for which a chunk is at most 8 rows; small meshes end up with one wave of chunks down to 2 rows.
   const int strips = (n[0] + T::TX - 1) / T::TX;
   int chunk;
   if (tn.chunk > 0) {
     chunk = tn.chunk;
   } else {
-    int nchunks = (sms * occ) / strips;
-    if (nchunks < 1) nchunks = 1;
-    chunk = (n[1] + nchunks - 1) / nchunks;
+    int per_wave = (sms * occ) / strips;          // chunks per wave
+    if (per_wave < 1) per_wave = 1;
+    const int k = (n[1] + 8 * per_wave - 1) / (8 * per_wave);
+    chunk = (n[1] + k * per_wave - 1) / (k * per_wave);
     if (chunk < 2) chunk = 2;
   }
   if (chunk > kMaxChunk) chunk = kMaxChunk;

@@ -438,13 +438,17 @@ inline bool plan3_setup(Plan3 &p, const int *n, int nxp, void *buf0, void *buf1,
     cudaGetLastError();
     return no("cudaFuncSetAttribute failed");
   }
-  // z-chunks (measured, profiles/): a CTA needs ~2 us per slice whatever the mesh, so small meshes want one
-  // full wave of short chunks; large meshes want >= ~12 waves of CTAs and chunks >= 8 to amortise the prologue
+  // z-chunks (measured, profiles/): short chunks win — neighbouring CTAs stay in step, so the halo overlap is found in
+  // L2, and the tail is fine-grained.  Meshes with at least one CTA per SM in every z-layer of tiles take 16 slices (the
+  // 2-slice prologue then re-reads 12 of 26 planes twice per 16: +6 % reads through L2); smaller meshes take one full
+  // wave of still shorter chunks (a CTA needs ~2 us per slice whatever the mesh).
   const int tiles = ((n[0] + T::TX - 1) / T::TX) * ((n[1] + T::TY - 1) / T::TY);
   auto ctas = [&](int c) { return (long long)tiles * ((n[2] + c - 1) / c); };
   int chunk = n[2] < kMaxChunk ? n[2] : kMaxChunk;
   if (tn.chunk > 0) {
     chunk = tn.chunk < n[2] ? tn.chunk : n[2];
+  } else if (tiles >= 148) {
+    chunk = n[2] < 16 ? n[2] : 16;
   } else {
     while (chunk > 4 && ctas((chunk + 1) / 2) <= 148 + 16) chunk = (chunk + 1) / 2;
     while (chunk > 8 && ctas(chunk) < 148 * 12) chunk = (chunk + 1) / 2;
