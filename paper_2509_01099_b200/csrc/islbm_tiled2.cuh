@@ -108,7 +108,7 @@ __device__ __forceinline__ void issue_stage2(int s, int yf, int ny, int x0, unsi
 template <typename ST, int TX, int STAGES, int MINB, int DIR>
 __global__ void __launch_bounds__(TX, MINB)
 k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const ST *__restrict__ src, ST *__restrict__ dst,
-              int ychunk, int load_policy, int store_policy) {
+              int load_policy, int store_policy) {
   using T = Tile2<ST, TX, STAGES>;
   using AT = typename Acc<ST>::type;   // fp32 storage interpolates the stored deviations in fp32 (islbm_tiled3.cuh)
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -120,7 +120,10 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
   pdl_launch_dependents();
 
   const int x0 = blockIdx.x * T::TX;
-  const int y0 = m.em_lo + blockIdx.y * ychunk, y1 = min(y0 + ychunk, m.em_hi);
+  // the emitted rows are split evenly over the gridDim.y chunks (lengths differ by at most one, all <= kMaxChunk)
+  const int rows = m.em_hi - m.em_lo;
+  const int y0 = m.em_lo + (int)((long long)blockIdx.y * rows / gridDim.y);
+  const int y1 = m.em_lo + (int)((long long)(blockIdx.y + 1) * rows / gridDim.y);
   const int yf = DIR > 0 ? y0 : y1 - 1;
   const int nstage = 2 + (y1 - y0);
   for (int i = threadIdx.x; i < 6 * (y1 - y0); i += T::TX) {
@@ -248,7 +251,7 @@ struct Plan2 {
   bool available = false;
   Maps2 maps[2];
   int tx = 128;
-  int ychunk = 32;
+  int per_wave = 1;      // chunks per strip in one wave of resident CTAs
   char why_not[96] = "";
 };
 
@@ -281,22 +284,9 @@ inline bool plan2_setup(Plan2 &p, const int *n, int nxp, void *buf0, void *buf1,
     cudaGetLastError();
     occ = 1;
   }
-  // chunks (measured, profiles/): short chunks win (8 rows: 0.90-0.94 at 2049^2..8193^2 against 0.73-0.87 for 60-row
-  // chunks), and the CTA count should be a whole number of waves of resident CTAs.  So: k waves, k the smallest number
-  // for which a chunk is at most 8 rows; small meshes end up with one wave of chunks down to 2 rows.
   const int strips = (n[0] + T::TX - 1) / T::TX;
-  int chunk;
-  if (tn.chunk > 0) {
-    chunk = tn.chunk;
-  } else {
-    int per_wave = (sms * occ) / strips;          // chunks per wave
-    if (per_wave < 1) per_wave = 1;
-    const int k = (n[1] + 8 * per_wave - 1) / (8 * per_wave);
-    chunk = (n[1] + k * per_wave - 1) / (k * per_wave);
-    if (chunk < 2) chunk = 2;
-  }
-  if (chunk > kMaxChunk) chunk = kMaxChunk;
-  p.ychunk = chunk < n[1] ? chunk : n[1];
+  p.per_wave = (sms * occ) / strips;
+  if (p.per_wave < 1) p.per_wave = 1;
   p.tx = T::TX;
   return true;
 }
@@ -318,17 +308,36 @@ inline bool plan2_create(Plan2 &p, const int *n, int nxp, void *buf0, void *buf1
   return true;
 }
 
+// Number of chunks a strip of `rows` emitted rows is cut into (measured, profiles/): short chunks win (4 rows:
+// 0.96-0.97 at 2049^2..8193^2, 8 rows: 0.88-0.93, 60 rows: 0.73-0.87; the doubled prologue rows are found in L2), and
+// the CTA count should be a whole number of waves of resident CTAs.  So: one wave if its chunks are at most 8 rows
+// (small and medium meshes, down to 2 rows), else k waves, k the smallest number for which a chunk is at most 4 rows.
+inline int chunks2(int rows, int per_wave, int forced_chunk) {
+  int nc;
+  if (forced_chunk > 0) {
+    nc = (rows + forced_chunk - 1) / forced_chunk;
+  } else {
+    nc = per_wave;
+    if ((rows + nc - 1) / nc > 8) nc = per_wave * ((rows + 4 * per_wave - 1) / (4 * per_wave));
+    if (nc > rows / 2) nc = rows / 2;
+  }
+  const int least = (rows + kMaxChunk - 1) / kMaxChunk;
+  if (nc < least) nc = least;
+  return nc < 1 ? 1 : nc;
+}
+
 template <typename ST, typename CFG>
 inline void launch2_cfg(const Plan2 &p, const int *n, const DevMesh &m, const NodeParams &np, int cur, void *const *buf,
                         const Tuning &tn, cudaStream_t stream) {
   using T = typename CFG::T;
-  dim3 grid((n[0] + T::TX - 1) / T::TX, (m.em_hi - m.em_lo + p.ychunk - 1) / p.ychunk, 1);
+  const int rows = m.em_hi - m.em_lo, nc = chunks2(rows, p.per_wave, tn.chunk);
+  dim3 grid((n[0] + T::TX - 1) / T::TX, nc, 1);
   if (tn.serpentine && cur)
     launch_step(k_step_ymarch<ST, T::TX, T::STAGES, CFG::MINB, -1>, grid, dim3(T::TX), T::SMEM_BYTES, stream, tn.pdl != 0,
-                p.maps[cur], m, np, (const ST *)buf[cur], (ST *)buf[1 - cur], p.ychunk, tn.load_policy, tn.store_policy);
+                p.maps[cur], m, np, (const ST *)buf[cur], (ST *)buf[1 - cur], tn.load_policy, tn.store_policy);
   else
     launch_step(k_step_ymarch<ST, T::TX, T::STAGES, CFG::MINB, 1>, grid, dim3(T::TX), T::SMEM_BYTES, stream, tn.pdl != 0,
-                p.maps[cur], m, np, (const ST *)buf[cur], (ST *)buf[1 - cur], p.ychunk, tn.load_policy, tn.store_policy);
+                p.maps[cur], m, np, (const ST *)buf[cur], (ST *)buf[1 - cur], tn.load_policy, tn.store_policy);
 }
 
 template <typename ST>
