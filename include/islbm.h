@@ -240,8 +240,9 @@ int islbm_set_kernel(islbm_t *h, int which);
  * 2 128 B, 3 256 B), "load_policy" / "store_policy" (L2 eviction policy 0 normal,
  * 1 evict_first, 2 evict_last), "tx2d" (2-D strip width 0 auto, 128, 224),
  * "serpentine" (2-D: march downwards on odd steps), "shape3d" (3-D tile 0 32x8, 1 64x4, 2 128x2), "pdl" (programmatic
- * dependent launch of consecutive step kernels, default 1).  Results do not depend on
- * any of them.  Unknown key or negative value: ISLBM_ERR_ARG. */
+ * dependent launch of consecutive step kernels, default 1), "fill" (first fill of the TMA
+ * ring: 1 before the weight rows and the CTA barrier, 2 after them, 0 automatic).  Results
+ * do not depend on any of them.  Unknown key or negative value: ISLBM_ERR_ARG. */
 int islbm_set_tuning(islbm_t *h, const char *key, int value);
 /* Number of kernels launched by this handle since creation. */
 long long islbm_launch_count(const islbm_t *h);

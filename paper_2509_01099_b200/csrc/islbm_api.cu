@@ -572,6 +572,7 @@ extern "C" int islbm_set_tuning(islbm_t *h, const char *key, int value) {
   else if (k == "serpentine") t.serpentine = value;
   else if (k == "shape3d") t.shape3d = value;
   else if (k == "pdl") t.pdl = value;
+  else if (k == "fill") { if (value > 2) return fail(ISLBM_ERR_ARG, "fill must be 0 (automatic), 1 (early) or 2 (late)"); t.fill = value; }
   else return fail(ISLBM_ERR_ARG, "unknown tuning key: " + k);
   make_tiled_plan(h);
   return ISLBM_OK;

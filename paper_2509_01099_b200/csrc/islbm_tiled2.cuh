@@ -108,7 +108,7 @@ __device__ __forceinline__ void issue_stage2(int s, int yf, int ny, int x0, unsi
 template <typename ST, int TX, int STAGES, int MINB, int DIR>
 __global__ void __launch_bounds__(TX, MINB)
 k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const ST *__restrict__ src, ST *__restrict__ dst,
-              int load_policy, int store_policy) {
+              int load_policy, int store_policy, int late_fill) {
   using T = Tile2<ST, TX, STAGES>;
   using AT = typename Acc<ST>::type;   // fp32 storage interpolates the stored deviations in fp32 (islbm_tiled3.cuh)
   extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -126,11 +126,11 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
   const int y1 = m.em_lo + (int)((long long)(blockIdx.y + 1) * rows / gridDim.y);
   const int yf = DIR > 0 ? y0 : y1 - 1;
   const int nstage = 2 + (y1 - y0);
-  for (int i = threadIdx.x; i < 6 * (y1 - y0); i += T::TX) {
-    const int sk = i / (y1 - y0), yi = i - sk * (y1 - y0);
-    wys[sk * kMaxChunk + yi] = (AT)__ldg(wrow(m, 1, sk / 3, sk % 3) + y0 + yi);
-  }
-
+  const uint64_t lpol = make_policy(load_policy);
+  const uint64_t spol = make_policy(store_policy);
+  // thread 0 sets up the ring and (unless late_fill) fills it BEFORE warps 1.. load the weight rows, so the two
+  // latencies overlap;
+  // griddepcontrol.wait comes before the first access to a population buffer (everything else reads only tables)
   if (threadIdx.x == 0) {
     for (int s = 0; s < T::STAGES; ++s) {
       mbar_init(&full[s], 1);
@@ -138,16 +138,21 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
       claim[s] = 0;
     }
     fence_barrier_init();
-  }
-  __syncthreads();
-
-  const uint64_t lpol = make_policy(load_policy);
-  const uint64_t spol = make_policy(store_policy);
-  pdl_wait();   // everything above read only the weight tables; the population buffers are touched from here on
-  if (threadIdx.x == 0) {
     tma_prefetch_desc(&mp.c2);
     tma_prefetch_desc(&mp.c4);
     tma_prefetch_desc(&mp.x);
+    if (!late_fill) {
+      pdl_wait();
+      for (int s = 0; s < T::STAGES && s < nstage; ++s) issue_stage2<T, DIR>(s, yf, m.ny, x0, stage0, full, empty, mp, lpol);
+    }
+  }
+  for (int i = (int)threadIdx.x - 32; i >= 0 && i < 6 * (y1 - y0); i += T::TX - 32) {   // warps 1..: warp 0 is waiting above
+    const int sk = i / (y1 - y0), yi = i - sk * (y1 - y0);
+    wys[sk * kMaxChunk + yi] = (AT)__ldg(wrow(m, 1, sk / 3, sk % 3) + y0 + yi);
+  }
+  pdl_wait();
+  __syncthreads();
+  if (late_fill && threadIdx.x == 0) {
     for (int s = 0; s < T::STAGES && s < nstage; ++s) issue_stage2<T, DIR>(s, yf, m.ny, x0, stage0, full, empty, mp, lpol);
   }
 
@@ -332,12 +337,15 @@ inline void launch2_cfg(const Plan2 &p, const int *n, const DevMesh &m, const No
   using T = typename CFG::T;
   const int rows = m.em_hi - m.em_lo, nc = chunks2(rows, p.per_wave, tn.chunk);
   dim3 grid((n[0] + T::TX - 1) / T::TX, nc, 1);
+  // first ring fill (measured, profiles/r1_c3_1024sq_ymarch_v4.md): a single-wave launch is 2-5 % faster with the
+  // fill after the CTA barrier, a multi-wave launch 2-6 % faster with the fill first
+  const int late = tn.fill ? (tn.fill == 2) : (nc <= p.per_wave);
   if (tn.serpentine && cur)
     launch_step(k_step_ymarch<ST, T::TX, T::STAGES, CFG::MINB, -1>, grid, dim3(T::TX), T::SMEM_BYTES, stream, tn.pdl != 0,
-                p.maps[cur], m, np, (const ST *)buf[cur], (ST *)buf[1 - cur], tn.load_policy, tn.store_policy);
+                p.maps[cur], m, np, (const ST *)buf[cur], (ST *)buf[1 - cur], tn.load_policy, tn.store_policy, late);
   else
     launch_step(k_step_ymarch<ST, T::TX, T::STAGES, CFG::MINB, 1>, grid, dim3(T::TX), T::SMEM_BYTES, stream, tn.pdl != 0,
-                p.maps[cur], m, np, (const ST *)buf[cur], (ST *)buf[1 - cur], tn.load_policy, tn.store_policy);
+                p.maps[cur], m, np, (const ST *)buf[cur], (ST *)buf[1 - cur], tn.load_policy, tn.store_policy, late);
 }
 
 template <typename ST>

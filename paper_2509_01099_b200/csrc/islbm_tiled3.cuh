@@ -231,7 +231,7 @@ __device__ __forceinline__ void issue_stage3(int s, int z0, int nz, int x0, int 
 template <typename ST, int TX, int TY>
 __global__ void __launch_bounds__(TX * TY, 1)
 k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const ST *__restrict__ src,
-              ST *__restrict__ dst, int zchunk, int load_policy, int store_policy) {
+              ST *__restrict__ dst, int zchunk, int load_policy, int store_policy, int late_fill) {
   using T = Tile3<ST, TX, TY>;
   using AT = typename Acc<ST>::type;
   // Ring refill policy (measured, profiles/): with fp64 storage the launch is DRAM-bound and thread 0 refilling the
@@ -252,11 +252,12 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
   const int x0 = blockIdx.x * T::TX, y0 = min((int)blockIdx.y * T::TY, max(m.ny - T::TY, 0));
   const int z0 = m.em_lo + blockIdx.z * zchunk, z1 = min(z0 + zchunk, m.em_hi);
   const int nstage = 2 + (z1 - z0);
-  for (int i = threadIdx.x; i < 6 * (z1 - z0); i += T::THREADS) {
-    const int sk = i / (z1 - z0), zi = i - sk * (z1 - z0);
-    wzs[sk * kMaxChunk + zi] = (AT)__ldg(wrow(m, 2, sk / 3, sk % 3) + z0 + zi);
-  }
-
+  const uint64_t lpol = make_policy(load_policy);
+  const uint64_t spol = make_policy(store_policy);
+  // thread 0 sets up the ring and (unless late_fill) fills it BEFORE warps 1.. load the weight rows, so the two
+  // latencies overlap;
+  // afterwards thread 0 (fp64 storage) or the last releasing warp (fp32) refills the slots.  griddepcontrol.wait
+  // comes before the first access to a population buffer (everything else reads only tables).
   if (threadIdx.x == 0) {
     for (int s = 0; s < T::STAGES; ++s) {
       mbar_init(&full[s], 1);
@@ -264,19 +265,24 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
       claim[s] = 0;
     }
     fence_barrier_init();
-  }
-  __syncthreads();
-
-  pdl_wait();   // everything above read only the weight tables; the population buffers are touched from here on
-  // thread 0 fills the ring; afterwards thread 0 (fp64 storage) or the last releasing warp (fp32) refills the slots
-  const uint64_t lpol = make_policy(load_policy);
-  const uint64_t spol = make_policy(store_policy);
-  if (threadIdx.x == 0) {
     tma_prefetch_desc(&mp.c2);
     tma_prefetch_desc(&mp.c4);
     tma_prefetch_desc(&mp.x);
     tma_prefetch_desc(&mp.y);
     tma_prefetch_desc(&mp.xy);
+    if (!late_fill) {
+      pdl_wait();
+      for (int s = 0; s < T::STAGES - (EARLY ? 0 : 1) && s < nstage; ++s)
+        issue_stage3<T>(s, z0, m.nz, x0, y0, stage0, full, empty, mp, lpol);
+    }
+  }
+  for (int i = (int)threadIdx.x - 32; i >= 0 && i < 6 * (z1 - z0); i += T::THREADS - 32) {   // warps 1..: warp 0 is waiting above
+    const int sk = i / (z1 - z0), zi = i - sk * (z1 - z0);
+    wzs[sk * kMaxChunk + zi] = (AT)__ldg(wrow(m, 2, sk / 3, sk % 3) + z0 + zi);
+  }
+  pdl_wait();
+  __syncthreads();
+  if (late_fill && threadIdx.x == 0) {
     for (int s = 0; s < T::STAGES - (EARLY ? 0 : 1) && s < nstage; ++s)
       issue_stage3<T>(s, z0, m.nz, x0, y0, stage0, full, empty, mp, lpol);
   }
@@ -474,7 +480,7 @@ inline void launch3_shape(const Plan3 &p, const int *n, const DevMesh &m, const 
   using T = Tile3<ST, TX, TY>;
   dim3 grid((n[0] + T::TX - 1) / T::TX, (n[1] + T::TY - 1) / T::TY, (m.em_hi - m.em_lo + p.zchunk - 1) / p.zchunk);
   launch_step(k_step_zmarch<ST, TX, TY>, grid, dim3(T::THREADS), T::SMEM_BYTES, stream, tn.pdl != 0, p.maps[cur], m, np,
-              (const ST *)buf[cur], (ST *)buf[1 - cur], p.zchunk, tn.load_policy, tn.store_policy);
+              (const ST *)buf[cur], (ST *)buf[1 - cur], p.zchunk, tn.load_policy, tn.store_policy, tn.fill == 2 ? 1 : 0);
 }
 
 template <typename ST>

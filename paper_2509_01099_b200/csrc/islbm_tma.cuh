@@ -187,6 +187,7 @@ struct Tuning {
   int shape3d = 0;      // 3-D tile shape: 0 32x8, 1 64x4, 2 128x2 (x by y nodes per CTA)
   int pdl = 1;          // programmatic dependent launch of consecutive step kernels
   int serpentine = 0;   // 2-D: reverse the CTA -> chunk map on odd steps (L2 reuse of the freshly written rows)
+  int fill = 0;         // first ring fill: 1 before the weight rows and the CTA barrier, 2 after them; 0 = automatic
 };
 
 }  // namespace islbmk

@@ -57,12 +57,13 @@ def ragged_coords(dim, ns, stretches):
 def kernels_for(islbm, sim):
     """(kernel, tuning) variants valid for this mesh: the generic kernel, the TMA-staged kernel in the
     launch configurations bench.py can select (strip width, chunk length incl. ragged chunks, L2 policies,
-    serpentine order), and the pure-shift kernel on uniform meshes."""
+    serpentine order, order of the first ring fill), and the pure-shift kernel on uniform meshes."""
     ks = [(islbm.KERNEL_GENERIC, {})]
     try:
         sim.set_kernel(islbm.KERNEL_TILED)
         ks.append((islbm.KERNEL_TILED, {}))
-        ks.append((islbm.KERNEL_TILED, dict(chunk=5, load_policy=1, store_policy=2, l2promo=3, pdl=0)))
+        ks.append((islbm.KERNEL_TILED, dict(chunk=5, load_policy=1, store_policy=2, l2promo=3, pdl=0, fill=2)))
+        ks.append((islbm.KERNEL_TILED, dict(chunk=2, fill=1)))
         if sim.dim == 2:
             ks.append((islbm.KERNEL_TILED, dict(tx2d=128, chunk=7, serpentine=1)))
             ks.append((islbm.KERNEL_TILED, dict(tx2d=224, chunk=3)))
@@ -78,7 +79,7 @@ def kernels_for(islbm, sim):
     return ks
 
 
-DEFAULT_TUNING = dict(chunk=0, l2promo=0, load_policy=0, store_policy=0, tx2d=0, serpentine=0, shape3d=0, pdl=1)
+DEFAULT_TUNING = dict(chunk=0, l2promo=0, load_policy=0, store_policy=0, tx2d=0, serpentine=0, shape3d=0, pdl=1, fill=0)
 
 
 def select(sim, k, tune):
