@@ -239,7 +239,7 @@ int islbm_set_kernel(islbm_t *h, int which);
  * chunk length, 0 = automatic), "l2promo" (tensor-map L2 promotion 0 none, 1 64 B,
  * 2 128 B, 3 256 B), "load_policy" / "store_policy" (L2 eviction policy 0 normal,
  * 1 evict_first, 2 evict_last), "tx2d" (2-D strip width 0 auto, 128, 224),
- * "serpentine" (2-D: march downwards on odd steps), "shape3d" (3-D tile 0 32x8, 1 64x4, 2 128x2), "pdl" (programmatic
+ * "serpentine" (2-D: march downwards on odd steps), "shape3d" (3-D tile 0 automatic, 1 64x4, 2 128x2, 3 32x6, 4 32x4, 5 32x8), "pdl" (programmatic
  * dependent launch of consecutive step kernels, default 1), "fill" (first fill of the TMA
  * ring: 1 before the weight rows and the CTA barrier, 2 after them, 0 automatic).  Results
  * do not depend on any of them.  Unknown key or negative value: ISLBM_ERR_ARG. */

@@ -570,7 +570,7 @@ extern "C" int islbm_set_tuning(islbm_t *h, const char *key, int value) {
   else if (k == "store_policy") t.store_policy = value;
   else if (k == "tx2d") { if (value != 0 && value != 128 && value != 224) return fail(ISLBM_ERR_ARG, "tx2d must be 0, 128 or 224"); t.tx2d = value; }
   else if (k == "serpentine") t.serpentine = value;
-  else if (k == "shape3d") t.shape3d = value;
+  else if (k == "shape3d") { if (value > 5) return fail(ISLBM_ERR_ARG, "shape3d must be 0 (automatic) .. 5"); t.shape3d = value; }
   else if (k == "pdl") t.pdl = value;
   else if (k == "fill") { if (value > 2) return fail(ISLBM_ERR_ARG, "fill must be 0 (automatic), 1 (early) or 2 (late)"); t.fill = value; }
   else return fail(ISLBM_ERR_ARG, "unknown tuning key: " + k);

@@ -229,7 +229,7 @@ __device__ __forceinline__ void issue_stage3(int s, int z0, int nz, int x0, int 
   } while (0)
 
 template <typename ST, int TX, int TY>
-__global__ void __launch_bounds__(TX * TY, 1)
+__global__ void __launch_bounds__(TX * TY, TX * TY <= 128 ? 3 : (TX * TY <= 192 ? 2 : 1))
 k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const ST *__restrict__ src,
               ST *__restrict__ dst, int zchunk, int load_policy, int store_policy, int late_fill) {
   using T = Tile3<ST, TX, TY>;
@@ -466,11 +466,19 @@ inline bool plan3_setup(Plan3 &p, const int *n, int nxp, void *buf0, void *buf1,
 
 template <typename ST>
 inline bool plan3_create(Plan3 &p, const int *n, int nxp, void *buf0, void *buf1, const Tuning &tn) {
-  p.shape = tn.shape3d;
-  switch (tn.shape3d) {
+  // tile shape (x by y nodes per CTA).  fp64 storage: 32x8 (250 registers, one CTA per SM; DRAM-bound).  fp32 storage
+  // is bound by latency at 8 warps per SM, so it takes smaller CTAs, capped at 168 registers by their launch bounds
+  // (14 spilled): 32x6 (two CTAs = 12 warps per SM; 256^3 0.56 -> 0.61) or 32x4 (three CTAs) on short y-axes
+  // (128^3 0.45 -> 0.52).  Measured in profiles/r1_c5_256cu_zmarch_v4.md.
+  int shape = tn.shape3d;
+  if (shape == 0) shape = sizeof(ST) == 4 ? (n[1] >= 192 ? 3 : 4) : 5;
+  p.shape = shape;
+  switch (shape) {
     case 1: return plan3_setup<ST, 64, 4>(p, n, nxp, buf0, buf1, tn);
     case 2: return plan3_setup<ST, 128, 2>(p, n, nxp, buf0, buf1, tn);
-    default: p.shape = 0; return plan3_setup<ST, 32, 8>(p, n, nxp, buf0, buf1, tn);
+    case 3: return plan3_setup<ST, 32, 6>(p, n, nxp, buf0, buf1, tn);
+    case 4: return plan3_setup<ST, 32, 4>(p, n, nxp, buf0, buf1, tn);
+    default: p.shape = 5; return plan3_setup<ST, 32, 8>(p, n, nxp, buf0, buf1, tn);
   }
 }
 
@@ -489,6 +497,8 @@ inline cudaError_t launch3(const Plan3 &p, const int *n, const DevMesh &m, const
   switch (p.shape) {
     case 1: launch3_shape<ST, 64, 4>(p, n, m, np, cur, buf, tn, stream); break;
     case 2: launch3_shape<ST, 128, 2>(p, n, m, np, cur, buf, tn, stream); break;
+    case 3: launch3_shape<ST, 32, 6>(p, n, m, np, cur, buf, tn, stream); break;
+    case 4: launch3_shape<ST, 32, 4>(p, n, m, np, cur, buf, tn, stream); break;
     default: launch3_shape<ST, 32, 8>(p, n, m, np, cur, buf, tn, stream);
   }
   return cudaPeekAtLastError();

@@ -184,7 +184,7 @@ struct Tuning {
   int load_policy = 0;  // L2 eviction policy of the TMA loads: 0 normal, 1 evict_first, 2 evict_last
   int store_policy = 0; // ... of the population stores
   int tx2d = 0;         // 2-D strip width: 128 or 224; 0 = automatic
-  int shape3d = 0;      // 3-D tile shape: 0 32x8, 1 64x4, 2 128x2 (x by y nodes per CTA)
+  int shape3d = 0;      // 3-D tile shape (x by y nodes per CTA): 0 automatic, 1 64x4, 2 128x2, 3 32x6, 4 32x4, 5 32x8
   int pdl = 1;          // programmatic dependent launch of consecutive step kernels
   int serpentine = 0;   // 2-D: reverse the CTA -> chunk map on odd steps (L2 reuse of the freshly written rows)
   int fill = 0;         // first ring fill: 1 before the weight rows and the CTA barrier, 2 after them; 0 = automatic

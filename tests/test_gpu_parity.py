@@ -64,6 +64,18 @@ def kernels_for(islbm, sim):
         ks.append((islbm.KERNEL_TILED, {}))
         ks.append((islbm.KERNEL_TILED, dict(chunk=5, load_policy=1, store_policy=2, l2promo=3, pdl=0, fill=2)))
         ks.append((islbm.KERNEL_TILED, dict(chunk=2, fill=1)))
+        if sim.dim == 3:
+            ks.append((islbm.KERNEL_TILED, dict(shape3d=3, chunk=3)))
+            ks.append((islbm.KERNEL_TILED, dict(shape3d=4, fill=2)))
+            ks.append((islbm.KERNEL_TILED, dict(shape3d=5)))
+            for tune in (dict(shape3d=1), dict(shape3d=2, chunk=7)):      # wide tiles: fp32 storage only (shared memory)
+                try:
+                    sim.set_tuning(**tune)
+                    sim.set_kernel(islbm.KERNEL_TILED)
+                    ks.append((islbm.KERNEL_TILED, tune))
+                except islbm.IslbmError:
+                    pass
+            sim.set_tuning(**DEFAULT_TUNING)
         if sim.dim == 2:
             ks.append((islbm.KERNEL_TILED, dict(tx2d=128, chunk=7, serpentine=1)))
             ks.append((islbm.KERNEL_TILED, dict(tx2d=224, chunk=3)))
