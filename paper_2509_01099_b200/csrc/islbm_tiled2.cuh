@@ -261,7 +261,8 @@ struct Plan2 {
 };
 
 // the two instantiated strip widths: (TX, STAGES, min CTAs/SM)
-template <typename ST> struct Cfg2a { using T = Tile2<ST, 128, 3>; static constexpr int MINB = 4; };
+// fp32 storage: five CTAs per SM (96 registers, 16 B spilled) measure 1-3 % above four; six (80 registers) lose 5 %
+template <typename ST> struct Cfg2a { using T = Tile2<ST, 128, 3>; static constexpr int MINB = sizeof(ST) == 4 ? 5 : 4; };
 template <typename ST> struct Cfg2b { using T = Tile2<ST, 224, 3>; static constexpr int MINB = 2; };
 
 template <typename ST, typename CFG>
