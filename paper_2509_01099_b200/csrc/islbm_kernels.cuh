@@ -87,8 +87,20 @@ __device__ __forceinline__ ST to_storage(double v, int q) {
   else return (ST)v;
 }
 
+// DEV = true: v already is the deviation f_q - w_q (collide_node<true>)
+template <typename ST, int DIM, bool DEV>
+__device__ __forceinline__ ST to_storage_from(double v, int q) {
+  if constexpr (DEV) return (ST)v;
+  else return to_storage<ST, DIM>(v, q);
+}
+
 template <typename ST>
 __device__ __forceinline__ double ldv(const ST *p) { return (double)__ldg(p); }
+
+// storage element -> fp64.  (An integer-instruction widening of fp32 - shift, re-bias the exponent - was measured
+// against the conversion instruction: 4 instructions instead of 1 on an issue/latency-bound kernel, no gain.)
+__device__ __forceinline__ double widen(float x) { return (double)x; }
+__device__ __forceinline__ double widen(double x) { return x; }
 
 // SplitMix64 by counter (A15): the (k+1)-th output for `seed`.
 __device__ __forceinline__ unsigned long long splitmix64_at(unsigned long long seed, unsigned long long k) {
@@ -214,25 +226,25 @@ __device__ __forceinline__ void pull_all_g(const DevMesh &m, const ST *src, cons
 }
 
 // fused halo exchange: the halo planes of this node into the neighbour's ghost layer (DevMesh::peer), plain stores
-template <int DIM, int K, typename ST>
+template <int DIM, int K, bool DEV, typename ST>
 __device__ __forceinline__ void peer_plane(ST *p, const double *f, const double *g) {
   constexpr int QF = Lat<DIM>::QF;
   constexpr int code = pop_of_plane<DIM>(halo_first_plane<DIM>() + K);
-  if constexpr (code < QF) *p = to_storage<ST, DIM>(f[code], code);
+  if constexpr (code < QF) *p = to_storage_from<ST, DIM, DEV>(f[code], code);
   else *p = (ST)g[code - QF];
 }
-template <int DIM, typename ST, int... Ks>
+template <int DIM, typename ST, bool DEV, int... Ks>
 __device__ __forceinline__ void peer_store(void *base, long long pitch, long long inplane, const double *f, const double *g,
                                            std::integer_sequence<int, Ks...>) {
   ST *p = reinterpret_cast<ST *>(base) + inplane;
-  (peer_plane<DIM, Ks>(p + (long long)Ks * pitch, f, g), ...);
+  (peer_plane<DIM, Ks, DEV>(p + (long long)Ks * pitch, f, g), ...);
 }
-template <int DIM, typename ST>
+template <int DIM, typename ST, bool DEV = false>
 __device__ __forceinline__ void peer_store_node(const DevMesh &m, int layer, long long inplane, const double *f, const double *g) {
   if (m.peer[0] != nullptr && layer == m.em_lo)
-    peer_store<DIM, ST>(m.peer[0], m.peer_pitch[0], inplane, f, g, std::make_integer_sequence<int, halo_plane_count<DIM>()>{});
+    peer_store<DIM, ST, DEV>(m.peer[0], m.peer_pitch[0], inplane, f, g, std::make_integer_sequence<int, halo_plane_count<DIM>()>{});
   if (m.peer[1] != nullptr && layer == m.em_hi - 1)
-    peer_store<DIM, ST>(m.peer[1], m.peer_pitch[1], inplane, f, g, std::make_integer_sequence<int, halo_plane_count<DIM>()>{});
+    peer_store<DIM, ST, DEV>(m.peer[1], m.peer_pitch[1], inplane, f, g, std::make_integer_sequence<int, halo_plane_count<DIM>()>{});
 }
 
 // ---------------------------------------------------------------------------

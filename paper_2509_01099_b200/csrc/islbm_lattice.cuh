@@ -118,11 +118,17 @@ ISLBM_HD constexpr double wflow(int q) {
 // ---------------------------------------------------------------------------
 // D2Q9 + D2Q5
 // ---------------------------------------------------------------------------
+// DEV = false: f holds the populations.  DEV = true (fp32 storage): f holds the deviations f_q - w_q from the rest
+// equilibrium and stays in that form: M w = m_eq(rho = 1, u = 0), so only rho (= 1 + sum of deviations) and the rho-
+// proportional rest parts of e_eq and eps_eq change, and f+ - w = (f - w) + M^T d needs no bias arithmetic at all
+// (2 extra additions instead of 2 per flow population).
+template <bool DEV = false>
 ISLBM_HD void collide_node(double (&f)[9], double (&g)[5], const NodeParams &p) {
   const double T = g[0] + g[1] + g[2] + g[3] + g[4];
   const double sa = (f[1] + f[3]) + (f[2] + f[4]);   // axis shell
   const double sd = (f[5] + f[7]) + (f[6] + f[8]);   // diagonal shell
-  const double rho = f[0] + sa + sd;
+  const double rsum = f[0] + sa + sd;
+  const double rho = DEV ? 1.0 + rsum : rsum;
   const double Fy = rho * p.gbeta * (T - p.T0);
   const double ax = f[1] - f[3], ay = f[2] - f[4];
   const double dx = (f[5] - f[7]) + (f[8] - f[6]);    // sum cx over diagonals
@@ -140,8 +146,10 @@ ISLBM_HD void collide_node(double (&f)[9], double (&g)[5], const NodeParams &p) 
   const double mpxy = (f[5] + f[7]) - (f[6] + f[8]);
   const double vF = v * Fy;
   // Delta m_k / |row_k|^2
-  const double de = (-p.s_nu * (me - rho * (-2.0 + 3.0 * u2)) + p.hs_nu * (6.0 * vF)) * (1.0 / 36.0);
-  const double deps = (-p.s_nu * (meps - rho * (1.0 - 3.0 * u2)) - p.hs_nu * (6.0 * vF)) * (1.0 / 36.0);
+  const double ee = DEV ? (me + 2.0 * rsum) - rho * (3.0 * u2) : me - rho * (-2.0 + 3.0 * u2);        // e - e_eq
+  const double eeps = DEV ? (meps - rsum) + rho * (3.0 * u2) : meps - rho * (1.0 - 3.0 * u2);        // eps - eps_eq
+  const double de = (-p.s_nu * ee + p.hs_nu * (6.0 * vF)) * (1.0 / 36.0);
+  const double deps = (-p.s_nu * eeps - p.hs_nu * (6.0 * vF)) * (1.0 / 36.0);
   const double djy = Fy * (1.0 / 6.0);
   const double dqx = (-p.s_q * (mqx + rho * u)) * (1.0 / 12.0);
   const double dqy = (-p.s_q * (mqy + rho * v) - p.hs_q * Fy) * (1.0 / 12.0);
@@ -194,6 +202,7 @@ ISLBM_HD void fields_from_post(const double (&f)[9], const double (&g)[5], const
 // ---------------------------------------------------------------------------
 // D3Q19 + D3Q7
 // ---------------------------------------------------------------------------
+template <bool DEV = false>
 ISLBM_HD void collide_node(double (&f)[19], double (&g)[7], const NodeParams &p) {
   const double T = g[0] + ((g[1] + g[2]) + (g[3] + g[4]) + (g[5] + g[6]));
   // pair sums / differences
@@ -217,7 +226,8 @@ ISLBM_HD void collide_node(double (&f)[19], double (&g)[7], const NodeParams &p)
 
   const double sa = px + py + pz;
   const double sd = xy_s + xz_s + yz_s;
-  const double rho = f[0] + sa + sd;
+  const double rsum = f[0] + sa + sd;
+  const double rho = DEV ? 1.0 + rsum : rsum;
   const double Fy = rho * p.gbeta * (T - p.T0);
   const double dxs = xy_x + xz_x, dys = xy_y + yz_y, dzs = xz_z + yz_z;
   const double jx = ax + dxs, jy = ay + dys, jz = az + dzs;
@@ -239,8 +249,10 @@ ISLBM_HD void collide_node(double (&f)[19], double (&g)[7], const NodeParams &p)
   const double vF = v * Fy;
   const double q3 = 2.0 * u * u - v * v - w * w, qw = v * v - w * w;
   // Delta m_k / |row_k|^2
-  const double de = (-p.s_nu * (me - rho * (-11.0 + 19.0 * u2)) + p.hs_nu * (38.0 * vF)) * (1.0 / 2394.0);
-  const double deps = (-p.s_nu * (meps - rho * (3.0 - 5.5 * u2)) - p.hs_nu * (11.0 * vF)) * (1.0 / 252.0);
+  const double ee = DEV ? (me + 11.0 * rsum) - rho * (19.0 * u2) : me - rho * (-11.0 + 19.0 * u2);     // e - e_eq
+  const double eeps = DEV ? (meps - 3.0 * rsum) + rho * (5.5 * u2) : meps - rho * (3.0 - 5.5 * u2);   // eps - eps_eq
+  const double de = (-p.s_nu * ee + p.hs_nu * (38.0 * vF)) * (1.0 / 2394.0);
+  const double deps = (-p.s_nu * eeps - p.hs_nu * (11.0 * vF)) * (1.0 / 252.0);
   const double djy = Fy * 0.1;
   const double dqx = (-p.s_q * (mqx + (2.0 / 3.0) * rho * u)) * (1.0 / 40.0);
   const double dqy = (-p.s_q * (mqy + (2.0 / 3.0) * rho * v) - p.hs_q * ((2.0 / 3.0) * Fy)) * (1.0 / 40.0);

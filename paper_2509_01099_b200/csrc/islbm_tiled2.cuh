@@ -95,14 +95,14 @@ __device__ __forceinline__ void issue_stage2(int s, int yf, int ny, int x0, unsi
 // y-direction of the separable interpolation; (P0,P1,P2) = stencil rows in ascending y
 #define ISLBM_YCOMB2(P0, P1, P2)                 \
   do {                                           \
-    f[2] = (double)comb3(wy[1], P0[0], P1[0], P2[0]);    \
-    f[4] = (double)comb3(wy[0], P0[1], P1[1], P2[1]);    \
-    g[2] = (double)comb3(wy[1], P0[2], P1[2], P2[2]);    \
-    g[4] = (double)comb3(wy[0], P0[3], P1[3], P2[3]);    \
-    f[5] = (double)comb3(wy[1], P0[4], P1[4], P2[4]);    \
-    f[6] = (double)comb3(wy[1], P0[5], P1[5], P2[5]);    \
-    f[7] = (double)comb3(wy[0], P0[6], P1[6], P2[6]);    \
-    f[8] = (double)comb3(wy[0], P0[7], P1[7], P2[7]);    \
+    f[2] = widen(comb3(wy[1], P0[0], P1[0], P2[0]));    \
+    f[4] = widen(comb3(wy[0], P0[1], P1[1], P2[1]));    \
+    g[2] = widen(comb3(wy[1], P0[2], P1[2], P2[2]));    \
+    g[4] = widen(comb3(wy[0], P0[3], P1[3], P2[3]));    \
+    f[5] = widen(comb3(wy[1], P0[4], P1[4], P2[4]));    \
+    f[6] = widen(comb3(wy[1], P0[5], P1[5], P2[5]));    \
+    f[7] = widen(comb3(wy[0], P0[6], P1[6], P2[6]));    \
+    f[8] = widen(comb3(wy[0], P0[7], P1[7], P2[7]));    \
   } while (0)
 
 template <typename ST, int TX, int STAGES, int MINB, int DIR>
@@ -205,12 +205,12 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
 #pragma unroll
         for (int k = 0; k < 3; ++k) wy[sg][k] = wys[(sg * 3 + k) * kMaxChunk + (y - y0)];
       double f[9], g[5];
-      f[0] = (double)PC2(0)[tx];
-      g[0] = (double)PC2(1)[tx];
-      f[1] = (double)tap3(PXR(0) + o_x, 1, wx[1]);
-      f[3] = (double)tap3(PXR(1) + o_x, 1, wx[0]);
-      g[1] = (double)tap3(PXR(2) + o_x, 1, wx[1]);
-      g[3] = (double)tap3(PXR(3) + o_x, 1, wx[0]);
+      f[0] = widen(PC2(0)[tx]);
+      g[0] = widen(PC2(1)[tx]);
+      f[1] = widen(tap3(PXR(0) + o_x, 1, wx[1]));
+      f[3] = widen(tap3(PXR(1) + o_x, 1, wx[0]));
+      g[1] = widen(tap3(PXR(2) + o_x, 1, wx[1]));
+      g[3] = widen(tap3(PXR(3) + o_x, 1, wx[0]));
       // hand the slot back; the warp whose release is the last one refills it at once with stage s + STAGES, so
       // STAGES - 1 stages are in flight whenever one is being consumed
       __syncwarp();
@@ -234,11 +234,11 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
         bb_fix_all_f<2>(f, wf, src, m.nnp, c, std::make_integer_sequence<int, 8>{});
         bb_fix_all_g<2>(g, wf, src, m.nnp, c, m, std::make_integer_sequence<int, 4>{});
       }
-      add_bias<ST, 2>(f);
-      collide_node(f, g, np);
+      constexpr bool DEV = Store<ST, 2>::kBiased;   // fp32 storage: collide the deviations as they are
+      collide_node<DEV>(f, g, np);
       if (valid) {
-        store_node<2>(dst + c, m.nnp, f, g, spol, std::make_integer_sequence<int, 14>{});
-        peer_store_node<2, ST>(m, y, x, f, g);
+        store_node<2, DEV>(dst + c, m.nnp, f, g, spol, std::make_integer_sequence<int, 14>{});
+        peer_store_node<2, ST, DEV>(m, y, x, f, g);
       }
     } else {
       // hand the slot back; the warp whose release is the last one refills it at once with stage s + STAGES, so

@@ -145,19 +145,19 @@ __device__ __forceinline__ void bb_fix_all_g(double *g, const WallFlags &wf, con
 
 // store the node's populations plane by plane in storage order.  The pointer is walked by the plane pitch and made
 // opaque after each step, so that ptxas keeps two integer adds per plane instead of a 64-bit multiply-add
-template <int DIM, int P, typename ST>
+template <int DIM, int P, bool DEV, typename ST>
 __device__ __forceinline__ void store_plane(ST *&p, long long nn, const double *f, const double *g, uint64_t spol) {
   constexpr int QF = Lat<DIM>::QF;
   constexpr int code = pop_of_plane<DIM>(P);
-  if constexpr (code < QF) st_hint(p, to_storage<ST, DIM>(f[code], code), spol);
+  if constexpr (code < QF) st_hint(p, to_storage_from<ST, DIM, DEV>(f[code], code), spol);
   else st_hint(p, (ST)g[code - QF], spol);
   p += nn;
   asm volatile("" : "+l"(p));
 }
-template <int DIM, typename ST, int... Ps>
+template <int DIM, bool DEV = false, typename ST, int... Ps>
 __device__ __forceinline__ void store_node(ST *p, long long nn, const double *f, const double *g, uint64_t spol,
                                            std::integer_sequence<int, Ps...>) {
-  (store_plane<DIM, Ps>(p, nn, f, g, spol), ...);
+  (store_plane<DIM, Ps, DEV>(p, nn, f, g, spol), ...);
 }
 
 __device__ __forceinline__ int sbase(int j, int n) { return min(max(j - 1, 0), n - 3); }
@@ -214,18 +214,18 @@ __device__ __forceinline__ void issue_stage3(int s, int z0, int nz, int x0, int 
 // z-direction of the separable interpolation; (P0,P1,P2) = stencil slices in ascending z
 #define ISLBM_ZCOMB3(P0, P1, P2)                  \
   do {                                            \
-    f[5] = (double)comb3(wz[1], P0[0], P1[0], P2[0]);     \
-    f[6] = (double)comb3(wz[0], P0[1], P1[1], P2[1]);     \
-    f[11] = (double)comb3(wz[1], P0[2], P1[2], P2[2]);    \
-    f[12] = (double)comb3(wz[1], P0[3], P1[3], P2[3]);    \
-    f[13] = (double)comb3(wz[0], P0[4], P1[4], P2[4]);    \
-    f[14] = (double)comb3(wz[0], P0[5], P1[5], P2[5]);    \
-    f[15] = (double)comb3(wz[1], P0[6], P1[6], P2[6]);    \
-    f[16] = (double)comb3(wz[1], P0[7], P1[7], P2[7]);    \
-    f[17] = (double)comb3(wz[0], P0[8], P1[8], P2[8]);    \
-    f[18] = (double)comb3(wz[0], P0[9], P1[9], P2[9]);    \
-    g[5] = (double)comb3(wz[1], P0[10], P1[10], P2[10]);  \
-    g[6] = (double)comb3(wz[0], P0[11], P1[11], P2[11]);  \
+    f[5] = widen(comb3(wz[1], P0[0], P1[0], P2[0]));     \
+    f[6] = widen(comb3(wz[0], P0[1], P1[1], P2[1]));     \
+    f[11] = widen(comb3(wz[1], P0[2], P1[2], P2[2]));    \
+    f[12] = widen(comb3(wz[1], P0[3], P1[3], P2[3]));    \
+    f[13] = widen(comb3(wz[0], P0[4], P1[4], P2[4]));    \
+    f[14] = widen(comb3(wz[0], P0[5], P1[5], P2[5]));    \
+    f[15] = widen(comb3(wz[1], P0[6], P1[6], P2[6]));    \
+    f[16] = widen(comb3(wz[1], P0[7], P1[7], P2[7]));    \
+    f[17] = widen(comb3(wz[0], P0[8], P1[8], P2[8]));    \
+    f[18] = widen(comb3(wz[0], P0[9], P1[9], P2[9]));    \
+    g[5] = widen(comb3(wz[1], P0[10], P1[10], P2[10]));  \
+    g[6] = widen(comb3(wz[0], P0[11], P1[11], P2[11]));  \
   } while (0)
 
 template <typename ST, int TX, int TY>
@@ -354,20 +354,20 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
 #pragma unroll
         for (int k = 0; k < 3; ++k) wz[sg][k] = wzs[(sg * 3 + k) * kMaxChunk + (s - 2)];
       double f[19], g[7];
-      f[0] = (double)PC2(0)[o_c];
-      g[0] = (double)PC2(1)[o_c];
-      f[1] = (double)tap3(PXZ(0) + o_x, 1, wx[1]);
-      f[2] = (double)tap3(PXZ(1) + o_x, 1, wx[0]);
-      g[1] = (double)tap3(PXZ(2) + o_x, 1, wx[1]);
-      g[2] = (double)tap3(PXZ(3) + o_x, 1, wx[0]);
-      f[3] = (double)tap3(PYZ(0) + o_y, T::TX, wy[1]);
-      f[4] = (double)tap3(PYZ(1) + o_y, T::TX, wy[0]);
-      g[3] = (double)tap3(PYZ(2) + o_y, T::TX, wy[1]);
-      g[4] = (double)tap3(PYZ(3) + o_y, T::TX, wy[0]);
-      f[7] = (double)tap9(PXY(0) + o_xy, T::HX, wx[1], wy[1]);
-      f[8] = (double)tap9(PXY(1) + o_xy, T::HX, wx[0], wy[1]);
-      f[9] = (double)tap9(PXY(2) + o_xy, T::HX, wx[1], wy[0]);
-      f[10] = (double)tap9(PXY(3) + o_xy, T::HX, wx[0], wy[0]);
+      f[0] = widen(PC2(0)[o_c]);
+      g[0] = widen(PC2(1)[o_c]);
+      f[1] = widen(tap3(PXZ(0) + o_x, 1, wx[1]));
+      f[2] = widen(tap3(PXZ(1) + o_x, 1, wx[0]));
+      g[1] = widen(tap3(PXZ(2) + o_x, 1, wx[1]));
+      g[2] = widen(tap3(PXZ(3) + o_x, 1, wx[0]));
+      f[3] = widen(tap3(PYZ(0) + o_y, T::TX, wy[1]));
+      f[4] = widen(tap3(PYZ(1) + o_y, T::TX, wy[0]));
+      g[3] = widen(tap3(PYZ(2) + o_y, T::TX, wy[1]));
+      g[4] = widen(tap3(PYZ(3) + o_y, T::TX, wy[0]));
+      f[7] = widen(tap9(PXY(0) + o_xy, T::HX, wx[1], wy[1]));
+      f[8] = widen(tap9(PXY(1) + o_xy, T::HX, wx[0], wy[1]));
+      f[9] = widen(tap9(PXY(2) + o_xy, T::HX, wx[1], wy[0]));
+      f[10] = widen(tap9(PXY(3) + o_xy, T::HX, wx[0], wy[0]));
       // all shared-memory reads of this stage are done: hand the slot back to the producer
       // hand the slot back (EARLY: the warp whose release is the last one refills it at once with stage s + STAGES)
       __syncwarp();
@@ -387,11 +387,11 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
         bb_fix_all_f<3>(f, wf, src, m.nnp, c, std::make_integer_sequence<int, 18>{});
         bb_fix_all_g<3>(g, wf, src, m.nnp, c, m, std::make_integer_sequence<int, 6>{});
       }
-      add_bias<ST, 3>(f);
-      collide_node(f, g, np);
+      constexpr bool DEV = Store<ST, 3>::kBiased;   // fp32 storage: collide the deviations as they are
+      collide_node<DEV>(f, g, np);
       if (valid) {
-        store_node<3>(dst + c, m.nnp, f, g, spol, std::make_integer_sequence<int, 26>{});
-        peer_store_node<3, ST>(m, z, cxy, f, g);
+        store_node<3, DEV>(dst + c, m.nnp, f, g, spol, std::make_integer_sequence<int, 26>{});
+        peer_store_node<3, ST, DEV>(m, z, cxy, f, g);
       }
     } else {
       // hand the slot back (EARLY: the warp whose release is the last one refills it at once with stage s + STAGES)

@@ -25,6 +25,29 @@ extern "C" void harness_collide(int dim, double *f, double *g, const double *prm
   }
 }
 
+// deviation form used by the fp32-storage kernels: collide f - w in place, return (f - w)+ + w
+extern "C" void harness_collide_dev(int dim, double *f, double *g, const double *prm) {
+  islbmk::NodeParams p;
+  p.gbeta = prm[0]; p.s_nu = prm[1]; p.s_q = prm[2];
+  p.hs_nu = 1.0 - 0.5 * p.s_nu; p.hs_q = 1.0 - 0.5 * p.s_q;
+  p.q_k = prm[3]; p.q_e = prm[4]; p.a_T = prm[5]; p.T0 = 0.0;
+  if (dim == 2) {
+    double ff[9], gg[5];
+    for (int i = 0; i < 9; ++i) ff[i] = f[i] - islbmk::wflow<2>(i);
+    for (int i = 0; i < 5; ++i) gg[i] = g[i];
+    islbmk::collide_node<true>(ff, gg, p);
+    for (int i = 0; i < 9; ++i) f[i] = ff[i] + islbmk::wflow<2>(i);
+    for (int i = 0; i < 5; ++i) g[i] = gg[i];
+  } else {
+    double ff[19], gg[7];
+    for (int i = 0; i < 19; ++i) ff[i] = f[i] - islbmk::wflow<3>(i);
+    for (int i = 0; i < 7; ++i) gg[i] = g[i];
+    islbmk::collide_node<true>(ff, gg, p);
+    for (int i = 0; i < 19; ++i) f[i] = ff[i] + islbmk::wflow<3>(i);
+    for (int i = 0; i < 7; ++i) g[i] = gg[i];
+  }
+}
+
 // out: rho,u,v,w,T from post-collision populations
 extern "C" void harness_fields_post(int dim, const double *f, const double *g, const double *prm, double *out) {
   islbmk::NodeParams p{};

@@ -51,6 +51,11 @@ def test_factored_collision_matches_oracle(harness, dim):
         harness.harness_collide(dim, dptr(fh), dptr(gh), dptr(prm))
         assert np.abs(fh - fo).max() < 2e-16 * 8
         assert np.abs(gh - go).max() < 2e-16 * 8
+        # deviation form (fp32-storage kernels collide f - w without re-adding the rest weights)
+        fd, gd = f.copy(), g.copy()
+        harness.harness_collide_dev(dim, dptr(fd), dptr(gd), dptr(prm))
+        assert np.abs(fd - fo).max() < 2e-16 * 8
+        assert np.abs(gd - go).max() < 2e-16 * 8
         # fields from post-collision populations == fields of the pre-collision state
         out = np.empty(5)
         harness.harness_fields_post(dim, dptr(fh), dptr(gh), dptr(prm), dptr(out))
