@@ -241,7 +241,10 @@ int islbm_set_kernel(islbm_t *h, int which);
  * 1 evict_first, 2 evict_last), "tx2d" (2-D strip width 0 auto, 128, 224),
  * "serpentine" (2-D: march downwards on odd steps), "shape3d" (3-D tile 0 automatic, 1 64x4, 2 128x2, 3 32x6, 4 32x4, 5 32x8), "pdl" (programmatic
  * dependent launch of consecutive step kernels, default 1), "fill" (first fill of the TMA
- * ring: 1 before the weight rows and the CTA barrier, 2 after them, 0 automatic).  Results
+ * ring: 1 before the weight rows and the CTA barrier, 2 after them, 0 automatic), "ring2d" (2-D fp64
+ * ring: 3 stages with four CTAs per SM or 4 stages with three, 0 automatic), "rows2d" / "rows2d1"
+ * (2-D chunk rule: longest chunk of a multi-wave launch / longest chunk for which a single wave
+ * of CTAs is taken, 0 automatic).  Results
  * do not depend on any of them.  Unknown key or negative value: ISLBM_ERR_ARG. */
 int islbm_set_tuning(islbm_t *h, const char *key, int value);
 /* Number of kernels launched by this handle since creation. */

@@ -573,6 +573,9 @@ extern "C" int islbm_set_tuning(islbm_t *h, const char *key, int value) {
   else if (k == "shape3d") { if (value > 5) return fail(ISLBM_ERR_ARG, "shape3d must be 0 (automatic) .. 5"); t.shape3d = value; }
   else if (k == "pdl") t.pdl = value;
   else if (k == "fill") { if (value > 2) return fail(ISLBM_ERR_ARG, "fill must be 0 (automatic), 1 (early) or 2 (late)"); t.fill = value; }
+  else if (k == "ring2d") { if (value != 0 && value != 3 && value != 4) return fail(ISLBM_ERR_ARG, "ring2d must be 0 (automatic), 3 or 4"); t.ring2d = value; }
+  else if (k == "rows2d") { if (value > kMaxChunk) return fail(ISLBM_ERR_ARG, "rows2d must be at most 64"); t.rows2d = value; }
+  else if (k == "rows2d1") { if (value > kMaxChunk) return fail(ISLBM_ERR_ARG, "rows2d1 must be at most 64"); t.rows2d1 = value; }
   else return fail(ISLBM_ERR_ARG, "unknown tuning key: " + k);
   make_tiled_plan(h);
   return ISLBM_OK;

@@ -88,8 +88,8 @@ __device__ __forceinline__ ST to_storage(double v, int q) {
 }
 
 // DEV = true: v already is the deviation f_q - w_q (collide_node<true>)
-template <typename ST, int DIM, bool DEV>
-__device__ __forceinline__ ST to_storage_from(double v, int q) {
+template <typename ST, int DIM, bool DEV, typename NT>
+__device__ __forceinline__ ST to_storage_from(NT v, int q) {
   if constexpr (DEV) return (ST)v;
   else return to_storage<ST, DIM>(v, q);
 }
@@ -226,25 +226,25 @@ __device__ __forceinline__ void pull_all_g(const DevMesh &m, const ST *src, cons
 }
 
 // fused halo exchange: the halo planes of this node into the neighbour's ghost layer (DevMesh::peer), plain stores
-template <int DIM, int K, bool DEV, typename ST>
-__device__ __forceinline__ void peer_plane(ST *p, const double *f, const double *g) {
+template <int DIM, int K, bool DEV, typename ST, typename NT>
+__device__ __forceinline__ void peer_plane(ST *p, const NT *f, const NT *g) {
   constexpr int QF = Lat<DIM>::QF;
   constexpr int code = pop_of_plane<DIM>(halo_first_plane<DIM>() + K);
   if constexpr (code < QF) *p = to_storage_from<ST, DIM, DEV>(f[code], code);
   else *p = (ST)g[code - QF];
 }
-template <int DIM, typename ST, bool DEV, int... Ks>
-__device__ __forceinline__ void peer_store(void *base, long long pitch, long long inplane, const double *f, const double *g,
+template <int DIM, typename ST, bool DEV, typename NT, int... Ks>
+__device__ __forceinline__ void peer_store(void *base, long long pitch, long long inplane, const NT *f, const NT *g,
                                            std::integer_sequence<int, Ks...>) {
   ST *p = reinterpret_cast<ST *>(base) + inplane;
   (peer_plane<DIM, Ks, DEV>(p + (long long)Ks * pitch, f, g), ...);
 }
-template <int DIM, typename ST, bool DEV = false>
-__device__ __forceinline__ void peer_store_node(const DevMesh &m, int layer, long long inplane, const double *f, const double *g) {
+template <int DIM, typename ST, bool DEV = false, typename NT>
+__device__ __forceinline__ void peer_store_node(const DevMesh &m, int layer, long long inplane, const NT *f, const NT *g) {
   if (m.peer[0] != nullptr && layer == m.em_lo)
-    peer_store<DIM, ST, DEV>(m.peer[0], m.peer_pitch[0], inplane, f, g, std::make_integer_sequence<int, halo_plane_count<DIM>()>{});
+    peer_store<DIM, ST, DEV, NT>(m.peer[0], m.peer_pitch[0], inplane, f, g, std::make_integer_sequence<int, halo_plane_count<DIM>()>{});
   if (m.peer[1] != nullptr && layer == m.em_hi - 1)
-    peer_store<DIM, ST, DEV>(m.peer[1], m.peer_pitch[1], inplane, f, g, std::make_integer_sequence<int, halo_plane_count<DIM>()>{});
+    peer_store<DIM, ST, DEV, NT>(m.peer[1], m.peer_pitch[1], inplane, f, g, std::make_integer_sequence<int, halo_plane_count<DIM>()>{});
 }
 
 // ---------------------------------------------------------------------------

@@ -42,7 +42,7 @@ struct Tile2 {
   static constexpr uint32_t Y_BYTES = 2u * P_C + 4u * P_X;   // planes of the emitted row
   static constexpr uint32_t M_BYTES = 4u * P_C + 4u * P_X;   // planes of the y-stencil row
   static constexpr int BAR_OFF = STAGES * STAGE_BYTES;
-  static constexpr int W_OFF = BAR_OFF + 64;                 // y-weights of the chunk [sign][k][kMaxChunk]
+  static constexpr int W_OFF = BAR_OFF + 128;                // y-weights of the chunk [sign][k][kMaxChunk]
   static constexpr size_t SMEM_BYTES = (size_t)W_OFF + 6 * kMaxChunk * 8 + 128;
 };
 
@@ -95,14 +95,14 @@ __device__ __forceinline__ void issue_stage2(int s, int yf, int ny, int x0, unsi
 // y-direction of the separable interpolation; (P0,P1,P2) = stencil rows in ascending y
 #define ISLBM_YCOMB2(P0, P1, P2)                 \
   do {                                           \
-    f[2] = widen(comb3(wy[1], P0[0], P1[0], P2[0]));    \
-    f[4] = widen(comb3(wy[0], P0[1], P1[1], P2[1]));    \
-    g[2] = widen(comb3(wy[1], P0[2], P1[2], P2[2]));    \
-    g[4] = widen(comb3(wy[0], P0[3], P1[3], P2[3]));    \
-    f[5] = widen(comb3(wy[1], P0[4], P1[4], P2[4]));    \
-    f[6] = widen(comb3(wy[1], P0[5], P1[5], P2[5]));    \
-    f[7] = widen(comb3(wy[0], P0[6], P1[6], P2[6]));    \
-    f[8] = widen(comb3(wy[0], P0[7], P1[7], P2[7]));    \
+    f[2] = comb3(wy[1], P0[0], P1[0], P2[0]);    \
+    f[4] = comb3(wy[0], P0[1], P1[1], P2[1]);    \
+    g[2] = comb3(wy[1], P0[2], P1[2], P2[2]);    \
+    g[4] = comb3(wy[0], P0[3], P1[3], P2[3]);    \
+    f[5] = comb3(wy[1], P0[4], P1[4], P2[4]);    \
+    f[6] = comb3(wy[1], P0[5], P1[5], P2[5]);    \
+    f[7] = comb3(wy[0], P0[6], P1[6], P2[6]);    \
+    f[8] = comb3(wy[0], P0[7], P1[7], P2[7]);    \
   } while (0)
 
 template <typename ST, int TX, int STAGES, int MINB, int DIR>
@@ -204,13 +204,13 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
       for (int sg = 0; sg < 2; ++sg)
 #pragma unroll
         for (int k = 0; k < 3; ++k) wy[sg][k] = wys[(sg * 3 + k) * kMaxChunk + (y - y0)];
-      double f[9], g[5];
-      f[0] = widen(PC2(0)[tx]);
-      g[0] = widen(PC2(1)[tx]);
-      f[1] = widen(tap3(PXR(0) + o_x, 1, wx[1]));
-      f[3] = widen(tap3(PXR(1) + o_x, 1, wx[0]));
-      g[1] = widen(tap3(PXR(2) + o_x, 1, wx[1]));
-      g[3] = widen(tap3(PXR(3) + o_x, 1, wx[0]));
+      AT f[9], g[5];   // fp64, or fp32 deviations (fp32 storage)
+      f[0] = PC2(0)[tx];
+      g[0] = PC2(1)[tx];
+      f[1] = tap3(PXR(0) + o_x, 1, wx[1]);
+      f[3] = tap3(PXR(1) + o_x, 1, wx[0]);
+      g[1] = tap3(PXR(2) + o_x, 1, wx[1]);
+      g[3] = tap3(PXR(3) + o_x, 1, wx[0]);
       // hand the slot back; the warp whose release is the last one refills it at once with stage s + STAGES, so
       // STAGES - 1 stages are in flight whenever one is being consumed
       __syncwarp();
@@ -256,13 +256,21 @@ struct Plan2 {
   bool available = false;
   Maps2 maps[2];
   int tx = 128;
+  int stages = 3;
   int per_wave = 1;      // chunks per strip in one wave of resident CTAs
   char why_not[96] = "";
 };
 
 // the two instantiated strip widths: (TX, STAGES, min CTAs/SM)
 // fp32 storage: five CTAs per SM (96 registers, 16 B spilled) measure 1-3 % above four; six (80 registers) lose 5 %
+// 128-wide strip, 3-stage ring: four CTAs per SM in fp64 (128 registers, 47 KB each), five with fp32 storage
 template <typename ST> struct Cfg2a { using T = Tile2<ST, 128, 3>; static constexpr int MINB = sizeof(ST) == 4 ? 5 : 4; };
+// 128-wide strip, fp64 only: 4-stage ring, three CTAs per SM (62 KB each): three rows in flight per CTA instead of two.
+// fp32 storage keeps the 3-stage ring (its stages are half as large; 4 and 5 stages measured 4-10 % slower).
+template <typename ST> struct Cfg2c {
+  using T = Tile2<ST, 128, sizeof(ST) == 4 ? 3 : 4>;
+  static constexpr int MINB = sizeof(ST) == 4 ? 5 : 3;
+};
 template <typename ST> struct Cfg2b { using T = Tile2<ST, 224, 3>; static constexpr int MINB = 2; };
 
 template <typename ST, typename CFG>
@@ -294,6 +302,7 @@ inline bool plan2_setup(Plan2 &p, const int *n, int nxp, void *buf0, void *buf1,
   p.per_wave = (sms * occ) / strips;
   if (p.per_wave < 1) p.per_wave = 1;
   p.tx = T::TX;
+  p.stages = T::STAGES;
   return true;
 }
 
@@ -308,7 +317,12 @@ inline bool plan2_create(Plan2 &p, const int *n, int nxp, void *buf0, void *buf1
   cudaDeviceGetAttribute(&cc_major, cudaDevAttrComputeCapabilityMajor, dev);
   if (cc_major < 10) return no("tiled kernel: needs sm_100");
   const int tx = tn.tx2d ? tn.tx2d : 128;   // a TMA box is at most 256 elements wide: TX + 2*XH <= 256
-  const bool ok = tx == 224 ? plan2_setup<ST, Cfg2b<ST>>(p, n, nxp, buf0, buf1, tn) : plan2_setup<ST, Cfg2a<ST>>(p, n, nxp, buf0, buf1, tn);
+  // ring depth (measured, profiles/r1_c3_1024sq_ymarch_v5.md): fp64 takes 4 stages x 3 CTAs per SM (512^2 +4 %,
+  // 1024^2 +1 %, 1538^2..8193^2 +0.3-2.3 %, 255^2 +20 %; 1026^2/1282^2 -1-2 %, inside the run-to-run spread)
+  const int ring = tn.ring2d ? tn.ring2d : 4;
+  const bool ok = tx == 224 ? plan2_setup<ST, Cfg2b<ST>>(p, n, nxp, buf0, buf1, tn)
+                            : (ring == 4 ? plan2_setup<ST, Cfg2c<ST>>(p, n, nxp, buf0, buf1, tn)
+                                         : plan2_setup<ST, Cfg2a<ST>>(p, n, nxp, buf0, buf1, tn));
   if (!ok) return no("tiled kernel: tensor map / attribute setup failed");
   p.available = true;
   return true;
@@ -316,15 +330,16 @@ inline bool plan2_create(Plan2 &p, const int *n, int nxp, void *buf0, void *buf1
 
 // Number of chunks a strip of `rows` emitted rows is cut into (measured, profiles/): short chunks win (4 rows:
 // 0.96-0.97 at 2049^2..8193^2, 8 rows: 0.88-0.93, 60 rows: 0.73-0.87; the doubled prologue rows are found in L2), and
-// the CTA count should be a whole number of waves of resident CTAs.  So: one wave if its chunks are at most 8 rows
-// (small and medium meshes, down to 2 rows), else k waves, k the smallest number for which a chunk is at most 4 rows.
-inline int chunks2(int rows, int per_wave, int forced_chunk) {
+// the CTA count should be a whole number of waves of resident CTAs.  So: one wave if its chunks are at most
+// max_single rows (8 with the 3-stage ring, 12 with the 4-stage one; small and medium meshes, down to 2 rows), else
+// k waves, k the smallest number for which a chunk is at most max_multi = 4 rows.
+inline int chunks2(int rows, int per_wave, int forced_chunk, int max_single = 8, int max_multi = 4) {
   int nc;
   if (forced_chunk > 0) {
     nc = (rows + forced_chunk - 1) / forced_chunk;
   } else {
     nc = per_wave;
-    if ((rows + nc - 1) / nc > 8) nc = per_wave * ((rows + 4 * per_wave - 1) / (4 * per_wave));
+    if ((rows + nc - 1) / nc > max_single) nc = per_wave * ((rows + max_multi * per_wave - 1) / (max_multi * per_wave));
     if (nc > rows / 2) nc = rows / 2;
   }
   const int least = (rows + kMaxChunk - 1) / kMaxChunk;
@@ -336,7 +351,10 @@ template <typename ST, typename CFG>
 inline void launch2_cfg(const Plan2 &p, const int *n, const DevMesh &m, const NodeParams &np, int cur, void *const *buf,
                         const Tuning &tn, cudaStream_t stream) {
   using T = typename CFG::T;
-  const int rows = m.em_hi - m.em_lo, nc = chunks2(rows, p.per_wave, tn.chunk);
+  const int rows = m.em_hi - m.em_lo;
+  // with three rows in flight per CTA a single wave pays up to 12-row chunks (642^2: 0.75 -> 0.82)
+  const int nc = chunks2(rows, p.per_wave, tn.chunk, tn.rows2d1 ? tn.rows2d1 : (p.stages >= 4 ? 12 : 8),
+                         tn.rows2d ? tn.rows2d : 4);
   dim3 grid((n[0] + T::TX - 1) / T::TX, nc, 1);
   // first ring fill (measured, profiles/r1_c3_1024sq_ymarch_v4.md): a single-wave launch is 2-5 % faster with the
   // fill after the CTA barrier, a multi-wave launch 2-6 % faster with the fill first
@@ -353,6 +371,7 @@ template <typename ST>
 inline cudaError_t launch2(const Plan2 &p, const int *n, const DevMesh &m, const NodeParams &np, int cur, void *const *buf,
                            const Tuning &tn, cudaStream_t stream) {
   if (p.tx == 224) launch2_cfg<ST, Cfg2b<ST>>(p, n, m, np, cur, buf, tn, stream);
+  else if (p.stages == Cfg2c<ST>::T::STAGES && p.stages != Cfg2a<ST>::T::STAGES) launch2_cfg<ST, Cfg2c<ST>>(p, n, m, np, cur, buf, tn, stream);
   else launch2_cfg<ST, Cfg2a<ST>>(p, n, m, np, cur, buf, tn, stream);
   return cudaPeekAtLastError();
 }

@@ -35,6 +35,11 @@
 
 namespace islbmk {
 
+// ring depth of the fp32-storage tiles (compile-time knob; the default is the measured optimum)
+#ifndef ISLBM_Z_STAGES_F32
+#define ISLBM_Z_STAGES_F32 3
+#endif
+
 constexpr int kMaxChunk = 64;   // longest marching chunk (its weights are staged in shared memory)
 
 template <typename ST, int TX_ = 32, int TY_ = 8>
@@ -58,13 +63,13 @@ struct Tile3 {
   static constexpr int OFF_XM = pad128(OFF_C4 + 4 * P_C);
   static constexpr int OFF_YM = pad128(OFF_XM + 4 * P_X);
   static constexpr int STAGE_BYTES = pad128(OFF_YM + 4 * P_Y);
-  static constexpr int STAGES = 3;
+  static constexpr int STAGES = sizeof(ST) == 4 ? ISLBM_Z_STAGES_F32 : 3;   // fp64: 3 x 62.7 KB is all that fits
   static constexpr int CONSUMER_WARPS = TX * TY / 32;
   static constexpr int THREADS = TX * TY;                // thread 0 doubles as the TMA producer
   static constexpr uint32_t Z_BYTES = 2u * P_C + 4u * P_X + 4u * P_Y + 4u * P_XY;   // planes of the emitted slice
   static constexpr uint32_t M_BYTES = 4u * P_C + 4u * P_X + 4u * P_Y;               // planes of the z-stencil slice
   static constexpr int BAR_OFF = STAGES * STAGE_BYTES;             // full[STAGES], empty[STAGES]
-  static constexpr int W_OFF = BAR_OFF + 64;                        // marching-axis weights [sign][k][kMaxChunk]
+  static constexpr int W_OFF = BAR_OFF + 128;                       // marching-axis weights [sign][k][kMaxChunk]
   static constexpr size_t SMEM_BYTES = (size_t)W_OFF + 6 * kMaxChunk * 8 + 128;
 };
 
@@ -74,11 +79,12 @@ struct Maps3 {
 };
 
 // ------------------------------ device helpers -----------------------------
-// Arithmetic type of the stencil interpolation: fp64 for fp64 storage (bit-compatible with the oracle's order of
-// operations).  For fp32 storage the stored deviations f_q - w_q are interpolated in fp32 and converted once per
-// population: the result then carries one or two more fp32 roundings of the deviation, the same size as the storage
-// rounding itself, and the node needs 52 instead of 116 conversions between 32- and 64-bit floats, which issue at a
-// quarter of the fp64 rate and were the bottleneck of the fp32-storage path (profiles/).  Collision: always fp64.
+// Arithmetic type of the stencil interpolation, and the type the node's 26 values are held in up to the collision:
+// fp64 for fp64 storage (bit-compatible with the oracle's order of operations).  For fp32 storage the stored
+// deviations f_q - w_q are interpolated in fp32 (one or two more fp32 roundings of the deviation, the size of the
+// storage rounding itself) and stay in fp32 registers: collide_node widens them for the moments and again for the
+// update f+ = fl32(fl64(f) + M^T d) (bit-identical to colliding an fp64 copy of the node, 26 fewer live registers):
+// 78 conversions per node instead of the 116 of an fp64 interpolation (they issue at a quarter of the fp64 rate).
 template <typename ST> struct Acc { using type = double; };
 template <> struct Acc<float> { using type = float; };
 
@@ -106,8 +112,8 @@ struct WallFlags {
 
 // Eq. 21: a flow population whose departure point lies beyond a wall takes the node's own
 // opposite post-collision value (storage form: the deviation, same lattice weight as its opposite).
-template <int DIM, int Q, typename ST>
-__device__ __forceinline__ void bb_fix_f(double &v, const WallFlags &wf, const ST *__restrict__ src, long long nn,
+template <int DIM, int Q, typename ST, typename NT>
+__device__ __forceinline__ void bb_fix_f(NT &v, const WallFlags &wf, const ST *__restrict__ src, long long nn,
                                          long long c) {
   constexpr int EX = evel<DIM>(Q, 0), EY = evel<DIM>(Q, 1), EZ = evel<DIM>(Q, 2);
   bool cross = false;
@@ -117,11 +123,11 @@ __device__ __forceinline__ void bb_fix_f(double &v, const WallFlags &wf, const S
   if (EY == -1) cross |= wf.hi[1];
   if (DIM == 3 && EZ == 1) cross |= wf.lo[2];
   if (DIM == 3 && EZ == -1) cross |= wf.hi[2];
-  if (cross) v = ldv(src + (long long)plane_f<DIM>(opposite<DIM>(Q)) * nn + c);
+  if (cross) v = (NT)__ldg(src + (long long)plane_f<DIM>(opposite<DIM>(Q)) * nn + c);
 }
 // Eq. 22 (isothermal x-walls) and Eq. 23 (adiabatic walls)
-template <int DIM, int Q, typename ST>
-__device__ __forceinline__ void bb_fix_g(double &v, const WallFlags &wf, const ST *__restrict__ src, long long nn,
+template <int DIM, int Q, typename ST, typename NT>
+__device__ __forceinline__ void bb_fix_g(NT &v, const WallFlags &wf, const ST *__restrict__ src, long long nn,
                                          long long c, const DevMesh &m) {
   constexpr int EX = evel<DIM>(Q, 0), EY = evel<DIM>(Q, 1), EZ = evel<DIM>(Q, 2);
   constexpr int A = EX != 0 ? 0 : (EY != 0 ? 1 : 2);
@@ -129,24 +135,24 @@ __device__ __forceinline__ void bb_fix_g(double &v, const WallFlags &wf, const S
   const bool cross = S == 1 ? wf.lo[A] : wf.hi[A];
   if (cross) {
     const double gb = ldv(src + (long long)plane_g<DIM>(opposite<DIM>(Q)) * nn + c);
-    v = A == 0 ? -gb + m.omega_bc * (wf.lo[0] ? m.T_hot : m.T_cold) : gb;
+    v = (NT)(A == 0 ? -gb + m.omega_bc * (wf.lo[0] ? m.T_hot : m.T_cold) : gb);
   }
 }
-template <int DIM, typename ST, int... Qs>
-__device__ __forceinline__ void bb_fix_all_f(double *f, const WallFlags &wf, const ST *src, long long nn, long long c,
+template <int DIM, typename ST, typename NT, int... Qs>
+__device__ __forceinline__ void bb_fix_all_f(NT *f, const WallFlags &wf, const ST *src, long long nn, long long c,
                                              std::integer_sequence<int, Qs...>) {
   (bb_fix_f<DIM, Qs + 1>(f[Qs + 1], wf, src, nn, c), ...);
 }
-template <int DIM, typename ST, int... Qs>
-__device__ __forceinline__ void bb_fix_all_g(double *g, const WallFlags &wf, const ST *src, long long nn, long long c,
+template <int DIM, typename ST, typename NT, int... Qs>
+__device__ __forceinline__ void bb_fix_all_g(NT *g, const WallFlags &wf, const ST *src, long long nn, long long c,
                                              const DevMesh &m, std::integer_sequence<int, Qs...>) {
   (bb_fix_g<DIM, Qs + 1>(g[Qs + 1], wf, src, nn, c, m), ...);
 }
 
 // store the node's populations plane by plane in storage order.  The pointer is walked by the plane pitch and made
 // opaque after each step, so that ptxas keeps two integer adds per plane instead of a 64-bit multiply-add
-template <int DIM, int P, bool DEV, typename ST>
-__device__ __forceinline__ void store_plane(ST *&p, long long nn, const double *f, const double *g, uint64_t spol) {
+template <int DIM, int P, bool DEV, typename ST, typename NT>
+__device__ __forceinline__ void store_plane(ST *&p, long long nn, const NT *f, const NT *g, uint64_t spol) {
   constexpr int QF = Lat<DIM>::QF;
   constexpr int code = pop_of_plane<DIM>(P);
   if constexpr (code < QF) st_hint(p, to_storage_from<ST, DIM, DEV>(f[code], code), spol);
@@ -154,8 +160,8 @@ __device__ __forceinline__ void store_plane(ST *&p, long long nn, const double *
   p += nn;
   asm volatile("" : "+l"(p));
 }
-template <int DIM, bool DEV = false, typename ST, int... Ps>
-__device__ __forceinline__ void store_node(ST *p, long long nn, const double *f, const double *g, uint64_t spol,
+template <int DIM, bool DEV = false, typename ST, typename NT, int... Ps>
+__device__ __forceinline__ void store_node(ST *p, long long nn, const NT *f, const NT *g, uint64_t spol,
                                            std::integer_sequence<int, Ps...>) {
   (store_plane<DIM, Ps, DEV>(p, nn, f, g, spol), ...);
 }
@@ -214,18 +220,18 @@ __device__ __forceinline__ void issue_stage3(int s, int z0, int nz, int x0, int 
 // z-direction of the separable interpolation; (P0,P1,P2) = stencil slices in ascending z
 #define ISLBM_ZCOMB3(P0, P1, P2)                  \
   do {                                            \
-    f[5] = widen(comb3(wz[1], P0[0], P1[0], P2[0]));     \
-    f[6] = widen(comb3(wz[0], P0[1], P1[1], P2[1]));     \
-    f[11] = widen(comb3(wz[1], P0[2], P1[2], P2[2]));    \
-    f[12] = widen(comb3(wz[1], P0[3], P1[3], P2[3]));    \
-    f[13] = widen(comb3(wz[0], P0[4], P1[4], P2[4]));    \
-    f[14] = widen(comb3(wz[0], P0[5], P1[5], P2[5]));    \
-    f[15] = widen(comb3(wz[1], P0[6], P1[6], P2[6]));    \
-    f[16] = widen(comb3(wz[1], P0[7], P1[7], P2[7]));    \
-    f[17] = widen(comb3(wz[0], P0[8], P1[8], P2[8]));    \
-    f[18] = widen(comb3(wz[0], P0[9], P1[9], P2[9]));    \
-    g[5] = widen(comb3(wz[1], P0[10], P1[10], P2[10]));  \
-    g[6] = widen(comb3(wz[0], P0[11], P1[11], P2[11]));  \
+    f[5] = comb3(wz[1], P0[0], P1[0], P2[0]);     \
+    f[6] = comb3(wz[0], P0[1], P1[1], P2[1]);     \
+    f[11] = comb3(wz[1], P0[2], P1[2], P2[2]);    \
+    f[12] = comb3(wz[1], P0[3], P1[3], P2[3]);    \
+    f[13] = comb3(wz[0], P0[4], P1[4], P2[4]);    \
+    f[14] = comb3(wz[0], P0[5], P1[5], P2[5]);    \
+    f[15] = comb3(wz[1], P0[6], P1[6], P2[6]);    \
+    f[16] = comb3(wz[1], P0[7], P1[7], P2[7]);    \
+    f[17] = comb3(wz[0], P0[8], P1[8], P2[8]);    \
+    f[18] = comb3(wz[0], P0[9], P1[9], P2[9]);    \
+    g[5] = comb3(wz[1], P0[10], P1[10], P2[10]);  \
+    g[6] = comb3(wz[0], P0[11], P1[11], P2[11]);  \
   } while (0)
 
 template <typename ST, int TX, int TY>
@@ -353,21 +359,21 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
       for (int sg = 0; sg < 2; ++sg)
 #pragma unroll
         for (int k = 0; k < 3; ++k) wz[sg][k] = wzs[(sg * 3 + k) * kMaxChunk + (s - 2)];
-      double f[19], g[7];
-      f[0] = widen(PC2(0)[o_c]);
-      g[0] = widen(PC2(1)[o_c]);
-      f[1] = widen(tap3(PXZ(0) + o_x, 1, wx[1]));
-      f[2] = widen(tap3(PXZ(1) + o_x, 1, wx[0]));
-      g[1] = widen(tap3(PXZ(2) + o_x, 1, wx[1]));
-      g[2] = widen(tap3(PXZ(3) + o_x, 1, wx[0]));
-      f[3] = widen(tap3(PYZ(0) + o_y, T::TX, wy[1]));
-      f[4] = widen(tap3(PYZ(1) + o_y, T::TX, wy[0]));
-      g[3] = widen(tap3(PYZ(2) + o_y, T::TX, wy[1]));
-      g[4] = widen(tap3(PYZ(3) + o_y, T::TX, wy[0]));
-      f[7] = widen(tap9(PXY(0) + o_xy, T::HX, wx[1], wy[1]));
-      f[8] = widen(tap9(PXY(1) + o_xy, T::HX, wx[0], wy[1]));
-      f[9] = widen(tap9(PXY(2) + o_xy, T::HX, wx[1], wy[0]));
-      f[10] = widen(tap9(PXY(3) + o_xy, T::HX, wx[0], wy[0]));
+      AT f[19], g[7];   // fp64, or fp32 deviations (fp32 storage)
+      f[0] = PC2(0)[o_c];
+      g[0] = PC2(1)[o_c];
+      f[1] = tap3(PXZ(0) + o_x, 1, wx[1]);
+      f[2] = tap3(PXZ(1) + o_x, 1, wx[0]);
+      g[1] = tap3(PXZ(2) + o_x, 1, wx[1]);
+      g[2] = tap3(PXZ(3) + o_x, 1, wx[0]);
+      f[3] = tap3(PYZ(0) + o_y, T::TX, wy[1]);
+      f[4] = tap3(PYZ(1) + o_y, T::TX, wy[0]);
+      g[3] = tap3(PYZ(2) + o_y, T::TX, wy[1]);
+      g[4] = tap3(PYZ(3) + o_y, T::TX, wy[0]);
+      f[7] = tap9(PXY(0) + o_xy, T::HX, wx[1], wy[1]);
+      f[8] = tap9(PXY(1) + o_xy, T::HX, wx[0], wy[1]);
+      f[9] = tap9(PXY(2) + o_xy, T::HX, wx[1], wy[0]);
+      f[10] = tap9(PXY(3) + o_xy, T::HX, wx[0], wy[0]);
       // all shared-memory reads of this stage are done: hand the slot back to the producer
       // hand the slot back (EARLY: the warp whose release is the last one refills it at once with stage s + STAGES)
       __syncwarp();

@@ -188,6 +188,9 @@ struct Tuning {
   int pdl = 1;          // programmatic dependent launch of consecutive step kernels
   int serpentine = 0;   // 2-D: reverse the CTA -> chunk map on odd steps (L2 reuse of the freshly written rows)
   int fill = 0;         // first ring fill: 1 before the weight rows and the CTA barrier, 2 after them; 0 = automatic
+  int ring2d = 0;       // 2-D fp64 ring: 3 stages x 4 CTAs per SM, or 4 stages x 3 CTAs; 0 = automatic
+  int rows2d = 0;       // 2-D chunk rule: longest chunk of a multi-wave launch (0 = automatic)
+  int rows2d1 = 0;      // 2-D chunk rule: longest chunk for which a single wave is taken (0 = automatic)
 };
 
 }  // namespace islbmk
