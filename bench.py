@@ -47,12 +47,12 @@ def read_peaks():
     return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
-def read_traffic(workload, kernel):
-    """dram bytes per launch from the committed ncu capture, if one exists for this kernel."""
+def read_traffic(workload, kernel, prec=0):
+    """dram bytes per launch from the committed ncu capture, if one exists for this kernel and storage precision."""
     path = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(path):
         with open(path) as fh:
-            return json.load(fh).get(f"{workload}:{kernel}")
+            return json.load(fh).get(f"{workload}:{kernel}" + (":f32" if prec else ""))
     return None
 
 
@@ -365,11 +365,11 @@ def main():
     t_launch = r["in_step_s"] / (args.steps * args.lbm_per_step)
     achieved = bpu * w.nodes / t_launch / 1e9
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": read_traffic(args.workload, r["kernel"]), "kernel": r["kernel"],
+                "traffic": read_traffic(args.workload, r["kernel"], prec), "kernel": r["kernel"],
                 "algorithmic_bytes_per_launch": bpu * w.nodes, "bytes_per_update": bpu,
                 "avg_launch_us": t_launch * 1e6, "peak_source": peak_src,
                 "frac_of_nominal_8000GBs": achieved / 8000.0,      # secondary, against the nominal HBM3e figure
-                "dram_bytes_per_update": (read_traffic(args.workload, r["kernel"]) or 0) / w.nodes or None}
+                "dram_bytes_per_update": (read_traffic(args.workload, r["kernel"], prec) or 0) / w.nodes or None}
 
     e2e = None
     cpu = None
