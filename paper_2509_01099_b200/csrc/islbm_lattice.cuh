@@ -125,8 +125,9 @@ ISLBM_HD constexpr double wflow(int q) {
 //
 // FT = float (fp32 storage, DEV only): the node's values stay in fp32 registers.  They are widened (exactly) once for
 // the moments and once more for the update f+ = fl32(fl64(f) + M^T d), so the result is bit-identical to colliding an
-// fp64 copy of the node, with 26 fewer live registers in 3-D while the moments and increments are computed
-// (measured: 256^3 fp32 storage 0.60 -> 0.65, 128^3 0.52 -> 0.58).  Rounding the increment to fp32 and adding it in
+// fp64 copy of the node, but no fp64 copy has to stay live from the interpolation to the end of the collision (the
+// compiler re-uses or re-creates the widened values as register pressure allows; measured: 256^3 fp32 storage
+// 0.60 -> 0.65, 128^3 0.52 -> 0.58).  Rounding the increment to fp32 and adding it in
 // fp32 (26 conversions fewer) measured only 1-2 % faster still and adds a second rounding per value and step, which
 // shows on far-from-equilibrium states (2.3e-6 against the 2e-6 bar of test_fp32_storage_every_kernel_three_steps;
 // the 1000-step error of 128^3 is unchanged, 4.3e-6): not taken.

@@ -83,8 +83,9 @@ struct Maps3 {
 // fp64 for fp64 storage (bit-compatible with the oracle's order of operations).  For fp32 storage the stored
 // deviations f_q - w_q are interpolated in fp32 (one or two more fp32 roundings of the deviation, the size of the
 // storage rounding itself) and stay in fp32 registers: collide_node widens them for the moments and again for the
-// update f+ = fl32(fl64(f) + M^T d) (bit-identical to colliding an fp64 copy of the node, 26 fewer live registers):
-// 78 conversions per node instead of the 116 of an fp64 interpolation (they issue at a quarter of the fp64 rate).
+// update f+ = fl32(fl64(f) + M^T d) (bit-identical to colliding an fp64 copy of the node, but no fp64 copy stays live
+// from the interpolation on): 52 conversions per node in the SASS instead of the 116 of an fp64 interpolation (they
+// issue at a quarter of the fp64 rate).
 template <typename ST> struct Acc { using type = double; };
 template <> struct Acc<float> { using type = float; };
 
