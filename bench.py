@@ -47,6 +47,15 @@ def read_peaks():
     return 6650.0, "fallback (B200_PROFILING.md: 6.65 TB/s)"
 
 
+def read_inst(workload, kernel, prec=0):
+    """warp instructions per launch (smsp__inst_executed.sum) from the committed ncu capture, if there is one."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            return json.load(fh).get("inst:" + f"{workload}:{kernel}" + (":f32" if prec else ""))
+    return None
+
+
 def read_traffic(workload, kernel, prec=0):
     """dram bytes per launch from the committed ncu capture, if one exists for this kernel and storage precision."""
     path = os.path.join(ROOT, "profiles", "traffic.json")
@@ -370,6 +379,16 @@ def main():
                 "avg_launch_us": t_launch * 1e6, "peak_source": peak_src,
                 "frac_of_nominal_8000GBs": achieved / 8000.0,      # secondary, against the nominal HBM3e figure
                 "dram_bytes_per_update": (read_traffic(args.workload, r["kernel"], prec) or 0) / w.nodes or None}
+
+    # fp32 storage is bound by instruction issue, not by HBM (profiles/r1_c5_256cu_f32_v5.md): report that roofline too.
+    # peak = 148 SMs x 4 warp schedulers x 1 warp instruction per clock x the maximum SM clock
+    inst = read_inst(args.workload, r["kernel"], prec)
+    if inst:
+        clk_hz = 1965e6
+        roofline["alu"] = {"bound": "alu", "achieved": inst / t_launch / 1e9, "peak": 148 * 4 * clk_hz / 1e9,
+                           "unit": "G warp instructions/s", "frac": inst / t_launch / (148 * 4 * clk_hz),
+                           "warp_instructions_per_launch": inst,
+                           "note": "issue-slot roofline; instruction count from the committed ncu capture"}
 
     e2e = None
     cpu = None
