@@ -186,6 +186,7 @@ static void set_node_params(islbm *h) {
   np.q_e = 4.0 * std::sqrt(3.0) - 6.0;
   np.a_T = h->prm.a_T;
   np.T0 = h->T0;
+  fold_node_params(np, h->dim);
   h->dp.T0 = h->T0;
 }
 

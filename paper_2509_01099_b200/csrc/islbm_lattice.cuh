@@ -12,6 +12,8 @@
 // Direction ordering: include/islbm.h.  Everything here is fp64.
 #pragma once
 
+#include <cmath>
+
 #ifndef ISLBM_HD
 #ifdef __CUDACC__
 #define ISLBM_HD __host__ __device__ __forceinline__
@@ -32,7 +34,34 @@ struct NodeParams {
   double q_e;     // 4 sqrt(3) - 6   (remaining temperature moments)
   double a_T;     // Eq. 15/16
   double T0;      // reference temperature of the buoyancy force
+  // relaxation rate x 1/|moment row|^2 (x the forcing factor), folded once on the host by fold_node_params: the
+  // kernels read them as constant-bank operands, so Delta m_k / |row_k|^2 is one multiply and one fused multiply-add
+  double k[21];
 };
+
+// k[] of NodeParams for the lattice of dimension dim, from s_nu, s_q, hs_nu, hs_q, q_k, q_e (index map: collide_node)
+inline void fold_node_params(NodeParams &p, int dim) {
+  for (int i = 0; i < 21; ++i) p.k[i] = 0.0;
+  if (dim == 2) {
+    p.k[0] = -p.s_nu / 36.0;  p.k[1] = 6.0 * p.hs_nu / 36.0;          // e:   k0 (e - e_eq) + k1 vF
+    p.k[2] = -p.s_nu / 36.0;  p.k[3] = -6.0 * p.hs_nu / 36.0;         // eps
+    p.k[4] = -p.s_q / 12.0;   p.k[5] = -p.hs_q / 12.0;                // q:   k4 (q - q_eq) + k5 Fy
+    p.k[6] = -p.s_nu / 4.0;   p.k[7] = -2.0 * p.hs_nu / 4.0;          // pxx: k6 (..) + k7 vF
+    p.k[14] = -p.s_nu / 4.0;  p.k[15] = p.hs_nu / 4.0;                // pxy: k14 (..) + k15 u Fy
+    p.k[17] = -p.q_k / 2.0;   p.k[18] = -p.q_e / 20.0;  p.k[20] = -p.q_e / 4.0;
+  } else {
+    p.k[0] = -p.s_nu / 2394.0;  p.k[1] = 38.0 * p.hs_nu / 2394.0;     // e
+    p.k[2] = -p.s_nu / 252.0;   p.k[3] = -11.0 * p.hs_nu / 252.0;     // eps
+    p.k[4] = -p.s_q / 40.0;     p.k[5] = -p.hs_q * (2.0 / 3.0) / 40.0;  // q
+    p.k[6] = -p.s_nu / 36.0;    p.k[7] = -2.0 * p.hs_nu / 36.0;       // 3pxx
+    p.k[8] = -p.s_nu / 72.0;    p.k[9] = p.hs_nu / 72.0;              // 3pixx
+    p.k[10] = -p.s_nu / 12.0;   p.k[11] = 2.0 * p.hs_nu / 12.0;       // pww
+    p.k[12] = -p.s_nu / 24.0;   p.k[13] = -p.hs_nu / 24.0;            // piww
+    p.k[14] = -p.s_nu / 4.0;    p.k[15] = p.hs_nu / 4.0;              // pxy, pyz, pxz
+    p.k[16] = -p.s_q / 8.0;                                           // m
+    p.k[17] = -p.q_k / 2.0;  p.k[18] = -p.q_e / 42.0;  p.k[19] = -p.q_e / 12.0;  p.k[20] = -p.q_e / 4.0;
+  }
+}
 
 template <int DIM> struct Lat;
 template <> struct Lat<2> { static constexpr int QF = 9, QG = 5; };
@@ -169,22 +198,22 @@ ISLBM_HD void collide_node(FT (&fio)[9], FT (&gio)[5], const NodeParams &p) {
   // Delta m_k / |row_k|^2
   const double ee = DEV ? (me + 2.0 * rsum) - rho * (3.0 * u2) : me - rho * (-2.0 + 3.0 * u2);        // e - e_eq
   const double eeps = DEV ? (meps - rsum) + rho * (3.0 * u2) : meps - rho * (1.0 - 3.0 * u2);        // eps - eps_eq
-  const double de = (-p.s_nu * ee + p.hs_nu * (6.0 * vF)) * (1.0 / 36.0);
-  const double deps = (-p.s_nu * eeps - p.hs_nu * (6.0 * vF)) * (1.0 / 36.0);
+  const double de = fma(p.k[0], ee, p.k[1] * vF);
+  const double deps = fma(p.k[2], eeps, p.k[3] * vF);
   const double djy = Fy * (1.0 / 6.0);
-  const double dqx = (-p.s_q * (mqx + rho * u)) * (1.0 / 12.0);
-  const double dqy = (-p.s_q * (mqy + rho * v) - p.hs_q * Fy) * (1.0 / 12.0);
-  const double dpxx = (-p.s_nu * (mpxx - rho * (u * u - v * v)) - p.hs_nu * (2.0 * vF)) * 0.25;
-  const double dpxy = (-p.s_nu * (mpxy - rho * (u * v)) + p.hs_nu * (u * Fy)) * 0.25;
+  const double dqx = p.k[4] * (mqx + rho * u);
+  const double dqy = fma(p.k[4], mqy + rho * v, p.k[5] * Fy);
+  const double dpxx = fma(p.k[6], mpxx - rho * (u * u - v * v), p.k[7] * vF);
+  const double dpxy = fma(p.k[14], mpxy - rho * (u * v), p.k[15] * (u * Fy));
   // temperature moments (Eq. 15 order)
   const double n1 = g[1] - g[3], n2 = g[2] - g[4];
   const double gs = (g[1] + g[3]) + (g[2] + g[4]);
   const double n3 = -4.0 * g[0] + gs;
   const double n4 = (g[1] + g[3]) - (g[2] + g[4]);
-  const double e1 = (-p.q_k * (n1 - u * T)) * 0.5;
-  const double e2 = (-p.q_k * (n2 - v * T)) * 0.5;
-  const double e3 = (-p.q_e * (n3 - p.a_T * T)) * (1.0 / 20.0);
-  const double e4 = (-p.q_e * n4) * 0.25;
+  const double e1 = p.k[17] * (n1 - u * T);
+  const double e2 = p.k[17] * (n2 - v * T);
+  const double e3 = p.k[18] * (n3 - p.a_T * T);
+  const double e4 = p.k[20] * n4;
   // f+ = f + M^T d
   const double ca = -de - 2.0 * deps;          // common part, axis shell
   const double cd = 2.0 * de + deps;           // common part, diagonal shell
@@ -281,28 +310,57 @@ ISLBM_HD void collide_node(FT (&fio)[19], FT (&gio)[7], const NodeParams &p) {
   // Delta m_k / |row_k|^2
   const double ee = DEV ? (me + 11.0 * rsum) - rho * (19.0 * u2) : me - rho * (-11.0 + 19.0 * u2);     // e - e_eq
   const double eeps = DEV ? (meps - 3.0 * rsum) + rho * (5.5 * u2) : meps - rho * (3.0 - 5.5 * u2);   // eps - eps_eq
-  const double de = (-p.s_nu * ee + p.hs_nu * (38.0 * vF)) * (1.0 / 2394.0);
-  const double deps = (-p.s_nu * eeps - p.hs_nu * (11.0 * vF)) * (1.0 / 252.0);
+  // Delta m_k / |row_k|^2.  FOLD: with the host-folded constants k[] (one multiply and one fused multiply-add per
+  // moment; 256^3 fp64 0.895 -> 0.905, 128^3 0.847 -> 0.859).  The fp32-storage 3-D kernels keep the unfolded
+  // expressions: under their 168-register cap the folded form spills 164 instead of 60 bytes and measures 11 % slower.
+  constexpr bool FOLD = sizeof(FT) == 8;
   const double djy = Fy * 0.1;
-  const double dqx = (-p.s_q * (mqx + (2.0 / 3.0) * rho * u)) * (1.0 / 40.0);
-  const double dqy = (-p.s_q * (mqy + (2.0 / 3.0) * rho * v) - p.hs_q * ((2.0 / 3.0) * Fy)) * (1.0 / 40.0);
-  const double dqz = (-p.s_q * (mqz + (2.0 / 3.0) * rho * w)) * (1.0 / 40.0);
-  const double d3pxx = (-p.s_nu * (m3pxx - rho * q3) - p.hs_nu * (2.0 * vF)) * (1.0 / 36.0);
-  const double d3pixx = (-p.s_nu * (m3pixx + 0.5 * rho * q3) + p.hs_nu * vF) * (1.0 / 72.0);
-  const double dpww = (-p.s_nu * (mpww - rho * qw) + p.hs_nu * (2.0 * vF)) * (1.0 / 12.0);
-  const double dpiww = (-p.s_nu * (mpiww + 0.5 * rho * qw) - p.hs_nu * vF) * (1.0 / 24.0);
-  const double dpxy = (-p.s_nu * (xy_p - rho * (u * v)) + p.hs_nu * (u * Fy)) * 0.25;
-  const double dpyz = (-p.s_nu * (yz_p - rho * (v * w)) + p.hs_nu * (w * Fy)) * 0.25;
-  const double dpxz = (-p.s_nu * (xz_p - rho * (u * w))) * 0.25;
-  const double dmx = (-p.s_q * mmx) * 0.125, dmy = (-p.s_q * mmy) * 0.125, dmz = (-p.s_q * mmz) * 0.125;
-  // temperature moments (Eq. 16 order)
   const double gx = g[1] + g[2], gy = g[3] + g[4], gz = g[5] + g[6];
-  const double e1 = (-p.q_k * ((g[1] - g[2]) - u * T)) * 0.5;
-  const double e2 = (-p.q_k * ((g[3] - g[4]) - v * T)) * 0.5;
-  const double e3 = (-p.q_k * ((g[5] - g[6]) - w * T)) * 0.5;
-  const double e4 = (-p.q_e * ((-6.0 * g[0] + (gx + gy + gz)) - p.a_T * T)) * (1.0 / 42.0);
-  const double e5 = (-p.q_e * (2.0 * gx - gy - gz)) * (1.0 / 12.0);
-  const double e6 = (-p.q_e * (gy - gz)) * 0.25;
+  double de, deps, dqx, dqy, dqz, d3pxx, d3pixx, dpww, dpiww, dpxy, dpyz, dpxz, dmx, dmy, dmz, e1, e2, e3, e4, e5, e6;
+  if constexpr (FOLD) {
+    const double r23 = (2.0 / 3.0) * rho;
+    de = fma(p.k[0], ee, p.k[1] * vF);
+    deps = fma(p.k[2], eeps, p.k[3] * vF);
+    dqx = p.k[4] * (mqx + r23 * u);
+    dqy = fma(p.k[4], mqy + r23 * v, p.k[5] * Fy);
+    dqz = p.k[4] * (mqz + r23 * w);
+    d3pxx = fma(p.k[6], m3pxx - rho * q3, p.k[7] * vF);
+    d3pixx = fma(p.k[8], m3pixx + 0.5 * rho * q3, p.k[9] * vF);
+    dpww = fma(p.k[10], mpww - rho * qw, p.k[11] * vF);
+    dpiww = fma(p.k[12], mpiww + 0.5 * rho * qw, p.k[13] * vF);
+    dpxy = fma(p.k[14], xy_p - rho * (u * v), p.k[15] * (u * Fy));
+    dpyz = fma(p.k[14], yz_p - rho * (v * w), p.k[15] * (w * Fy));
+    dpxz = p.k[14] * (xz_p - rho * (u * w));
+    dmx = p.k[16] * mmx, dmy = p.k[16] * mmy, dmz = p.k[16] * mmz;
+    // temperature moments (Eq. 16 order)
+    e1 = p.k[17] * ((g[1] - g[2]) - u * T);
+    e2 = p.k[17] * ((g[3] - g[4]) - v * T);
+    e3 = p.k[17] * ((g[5] - g[6]) - w * T);
+    e4 = p.k[18] * ((-6.0 * g[0] + (gx + gy + gz)) - p.a_T * T);
+    e5 = p.k[19] * (2.0 * gx - gy - gz);
+    e6 = p.k[20] * (gy - gz);
+  } else {
+    de = (-p.s_nu * ee + p.hs_nu * (38.0 * vF)) * (1.0 / 2394.0);
+    deps = (-p.s_nu * eeps - p.hs_nu * (11.0 * vF)) * (1.0 / 252.0);
+    dqx = (-p.s_q * (mqx + (2.0 / 3.0) * rho * u)) * (1.0 / 40.0);
+    dqy = (-p.s_q * (mqy + (2.0 / 3.0) * rho * v) - p.hs_q * ((2.0 / 3.0) * Fy)) * (1.0 / 40.0);
+    dqz = (-p.s_q * (mqz + (2.0 / 3.0) * rho * w)) * (1.0 / 40.0);
+    d3pxx = (-p.s_nu * (m3pxx - rho * q3) - p.hs_nu * (2.0 * vF)) * (1.0 / 36.0);
+    d3pixx = (-p.s_nu * (m3pixx + 0.5 * rho * q3) + p.hs_nu * vF) * (1.0 / 72.0);
+    dpww = (-p.s_nu * (mpww - rho * qw) + p.hs_nu * (2.0 * vF)) * (1.0 / 12.0);
+    dpiww = (-p.s_nu * (mpiww + 0.5 * rho * qw) - p.hs_nu * vF) * (1.0 / 24.0);
+    dpxy = (-p.s_nu * (xy_p - rho * (u * v)) + p.hs_nu * (u * Fy)) * 0.25;
+    dpyz = (-p.s_nu * (yz_p - rho * (v * w)) + p.hs_nu * (w * Fy)) * 0.25;
+    dpxz = (-p.s_nu * (xz_p - rho * (u * w))) * 0.25;
+    dmx = (-p.s_q * mmx) * 0.125, dmy = (-p.s_q * mmy) * 0.125, dmz = (-p.s_q * mmz) * 0.125;
+    // temperature moments (Eq. 16 order)
+    e1 = (-p.q_k * ((g[1] - g[2]) - u * T)) * 0.5;
+    e2 = (-p.q_k * ((g[3] - g[4]) - v * T)) * 0.5;
+    e3 = (-p.q_k * ((g[5] - g[6]) - w * T)) * 0.5;
+    e4 = (-p.q_e * ((-6.0 * g[0] + (gx + gy + gz)) - p.a_T * T)) * (1.0 / 42.0);
+    e5 = (-p.q_e * (2.0 * gx - gy - gz)) * (1.0 / 12.0);
+    e6 = (-p.q_e * (gy - gz)) * 0.25;
+  }
   // f+ = f + M^T d
   const double ca = -11.0 * de - 4.0 * deps;
   const double cd = 8.0 * de + deps;

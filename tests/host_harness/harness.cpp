@@ -8,6 +8,7 @@ extern "C" void harness_collide(int dim, double *f, double *g, const double *prm
   p.gbeta = prm[0]; p.s_nu = prm[1]; p.s_q = prm[2];
   p.hs_nu = 1.0 - 0.5 * p.s_nu; p.hs_q = 1.0 - 0.5 * p.s_q;
   p.q_k = prm[3]; p.q_e = prm[4]; p.a_T = prm[5]; p.T0 = 0.0;
+  islbmk::fold_node_params(p, dim);
   if (dim == 2) {
     double ff[9], gg[5];
     for (int i = 0; i < 9; ++i) ff[i] = f[i];
@@ -31,6 +32,7 @@ extern "C" void harness_collide_dev(int dim, double *f, double *g, const double 
   p.gbeta = prm[0]; p.s_nu = prm[1]; p.s_q = prm[2];
   p.hs_nu = 1.0 - 0.5 * p.s_nu; p.hs_q = 1.0 - 0.5 * p.s_q;
   p.q_k = prm[3]; p.q_e = prm[4]; p.a_T = prm[5]; p.T0 = 0.0;
+  islbmk::fold_node_params(p, dim);
   if (dim == 2) {
     double ff[9], gg[5];
     for (int i = 0; i < 9; ++i) ff[i] = f[i] - islbmk::wflow<2>(i);
@@ -44,6 +46,30 @@ extern "C" void harness_collide_dev(int dim, double *f, double *g, const double 
     for (int i = 0; i < 7; ++i) gg[i] = g[i];
     islbmk::collide_node<true>(ff, gg, p);
     for (int i = 0; i < 19; ++i) f[i] = ff[i] + islbmk::wflow<3>(i);
+    for (int i = 0; i < 7; ++i) g[i] = gg[i];
+  }
+}
+
+// the fp32-storage kernels' form: fp32 deviations in, fp32 deviations out (collide_node<true, float>)
+extern "C" void harness_collide_dev_f32(int dim, float *fdev, float *g, const double *prm) {
+  islbmk::NodeParams p;
+  p.gbeta = prm[0]; p.s_nu = prm[1]; p.s_q = prm[2];
+  p.hs_nu = 1.0 - 0.5 * p.s_nu; p.hs_q = 1.0 - 0.5 * p.s_q;
+  p.q_k = prm[3]; p.q_e = prm[4]; p.a_T = prm[5]; p.T0 = 0.0;
+  islbmk::fold_node_params(p, dim);
+  if (dim == 2) {
+    float ff[9], gg[5];
+    for (int i = 0; i < 9; ++i) ff[i] = fdev[i];
+    for (int i = 0; i < 5; ++i) gg[i] = g[i];
+    islbmk::collide_node<true>(ff, gg, p);
+    for (int i = 0; i < 9; ++i) fdev[i] = ff[i];
+    for (int i = 0; i < 5; ++i) g[i] = gg[i];
+  } else {
+    float ff[19], gg[7];
+    for (int i = 0; i < 19; ++i) ff[i] = fdev[i];
+    for (int i = 0; i < 7; ++i) gg[i] = g[i];
+    islbmk::collide_node<true>(ff, gg, p);
+    for (int i = 0; i < 19; ++i) fdev[i] = ff[i];
     for (int i = 0; i < 7; ++i) g[i] = gg[i];
   }
 }
