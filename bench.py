@@ -56,6 +56,15 @@ def read_inst(workload, kernel, prec=0):
     return None
 
 
+def read_traffic_commit():
+    """commit id of the kernels the committed ncu figures were captured on (goes stale when a kernel changes)."""
+    path = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(path):
+        with open(path) as fh:
+            return json.load(fh).get("_commit")
+    return None
+
+
 def read_traffic(workload, kernel, prec=0):
     """dram bytes per launch from the committed ncu capture, if one exists for this kernel and storage precision."""
     path = os.path.join(ROOT, "profiles", "traffic.json")
@@ -374,20 +383,25 @@ def main():
     t_launch = r["in_step_s"] / (args.steps * args.lbm_per_step)
     achieved = bpu * w.nodes / t_launch / 1e9
     roofline = {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                "traffic": read_traffic(args.workload, r["kernel"], prec), "kernel": r["kernel"],
+                "traffic": read_traffic(args.workload, r["kernel"], prec), "traffic_commit": read_traffic_commit(),
+                "kernel": r["kernel"],
                 "algorithmic_bytes_per_launch": bpu * w.nodes, "bytes_per_update": bpu,
                 "avg_launch_us": t_launch * 1e6, "peak_source": peak_src,
                 "frac_of_nominal_8000GBs": achieved / 8000.0,      # secondary, against the nominal HBM3e figure
                 "dram_bytes_per_update": (read_traffic(args.workload, r["kernel"], prec) or 0) / w.nodes or None}
 
     # fp32 storage is bound by instruction issue, not by HBM (profiles/r1_c5_256cu_f32_v5.md): report that roofline too.
-    # peak = 148 SMs x 4 warp schedulers x 1 warp instruction per clock x the maximum SM clock
+    # peak = SMs x 4 warp schedulers x 1 warp instruction per clock x the maximum SM clock
     inst = read_inst(args.workload, r["kernel"], prec)
     if inst:
-        clk_hz = 1965e6
-        roofline["alu"] = {"bound": "alu", "achieved": inst / t_launch / 1e9, "peak": 148 * 4 * clk_hz / 1e9,
-                           "unit": "G warp instructions/s", "frac": inst / t_launch / (148 * 4 * clk_hz),
-                           "warp_instructions_per_launch": inst,
+        sms = torch.cuda.get_device_properties(dev).multi_processor_count
+        clk_mhz = (clocks or {}).get("sm_max_mhz") or 1965.0            # the device's maximum SM clock (nvidia-smi)
+        clk_hz = clk_mhz * 1e6
+        roofline["alu"] = {"bound": "alu", "achieved": inst / t_launch / 1e9, "peak": sms * 4 * clk_hz / 1e9,
+                           "unit": "G warp instructions/s", "frac": inst / t_launch / (sms * 4 * clk_hz),
+                           "warp_instructions_per_launch": inst, "sms": sms, "sm_max_mhz": clk_mhz,
+                           "frac_at_sampled_clock": (inst / t_launch / (sms * 4 * clocks["sm_mhz"] * 1e6)
+                                                     if clocks and clocks.get("sm_mhz") else None),
                            "note": "issue-slot roofline; instruction count from the committed ncu capture"}
 
     e2e = None

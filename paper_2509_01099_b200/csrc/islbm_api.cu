@@ -3,6 +3,7 @@
 // dispatch.  No torch types, no CPU fallback.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -37,7 +38,7 @@ int fail(int code, const std::string &msg) {
 constexpr size_t kAlign = 256;
 size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 
-constexpr int kMaxRedBlocks = 148 * 8;
+constexpr int kMaxRedBlocks = 2048;   // capacity of the partial-sum area; the launch takes 8 blocks per SM (red_blocks)
 
 struct Carve {
   size_t buf[2], wtab, avgw, partial, red_out, snap, total;
@@ -665,7 +666,8 @@ extern "C" int islbm_fields(islbm_t *h, double *rho, double *u, double *v, doubl
 
 static int red_blocks(const islbm *h) {
   long long b = (h->nn + kRedThreads - 1) / kRedThreads;
-  return (int)(b < kMaxRedBlocks ? b : kMaxRedBlocks);
+  const long long cap = std::min<long long>(kMaxRedBlocks, 8LL * sm_count());
+  return (int)(b < cap ? b : cap);
 }
 
 template <int DIM, typename ST>

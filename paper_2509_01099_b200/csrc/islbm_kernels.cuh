@@ -96,6 +96,9 @@ __device__ __forceinline__ ST to_storage_from(NT v, int q) {
 
 template <typename ST>
 __device__ __forceinline__ double ldv(const ST *p) { return (double)__ldg(p); }
+// coherent (L2) load for data another grid may still be writing when this kernel becomes resident (PDL)
+template <typename ST>
+__device__ __forceinline__ ST ld_coherent(const ST *p) { return __ldcg(p); }
 
 // storage element -> fp64.  (An integer-instruction widening of fp32 - shift, re-bias the exponent - was measured
 // against the conversion instruction: 4 instructions instead of 1 on an issue/latency-bound kernel, no gain.)

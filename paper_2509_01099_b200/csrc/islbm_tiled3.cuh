@@ -113,6 +113,9 @@ struct WallFlags {
 
 // Eq. 21: a flow population whose departure point lies beyond a wall takes the node's own
 // opposite post-collision value (storage form: the deviation, same lattice weight as its opposite).
+// The wall reads are coherent loads (ld.global.cg), not ld.global.nc: with programmatic dependent launch step t+1 is
+// resident while step t still writes the buffer these loads read, so the data is not read-only for the kernel's
+// lifetime (the loads themselves come after griddepcontrol.wait).
 template <int DIM, int Q, typename ST, typename NT>
 __device__ __forceinline__ void bb_fix_f(NT &v, const WallFlags &wf, const ST *__restrict__ src, long long nn,
                                          long long c) {
@@ -124,7 +127,7 @@ __device__ __forceinline__ void bb_fix_f(NT &v, const WallFlags &wf, const ST *_
   if (EY == -1) cross |= wf.hi[1];
   if (DIM == 3 && EZ == 1) cross |= wf.lo[2];
   if (DIM == 3 && EZ == -1) cross |= wf.hi[2];
-  if (cross) v = (NT)__ldg(src + (long long)plane_f<DIM>(opposite<DIM>(Q)) * nn + c);
+  if (cross) v = (NT)ld_coherent(src + (long long)plane_f<DIM>(opposite<DIM>(Q)) * nn + c);
 }
 // Eq. 22 (isothermal x-walls) and Eq. 23 (adiabatic walls)
 template <int DIM, int Q, typename ST, typename NT>
@@ -135,7 +138,7 @@ __device__ __forceinline__ void bb_fix_g(NT &v, const WallFlags &wf, const ST *_
   constexpr int S = EX + EY + EZ;
   const bool cross = S == 1 ? wf.lo[A] : wf.hi[A];
   if (cross) {
-    const double gb = ldv(src + (long long)plane_g<DIM>(opposite<DIM>(Q)) * nn + c);
+    const double gb = (double)ld_coherent(src + (long long)plane_g<DIM>(opposite<DIM>(Q)) * nn + c);
     v = (NT)(A == 0 ? -gb + m.omega_bc * (wf.lo[0] ? m.T_hot : m.T_cold) : gb);
   }
 }
@@ -457,14 +460,15 @@ inline bool plan3_setup(Plan3 &p, const int *n, int nxp, void *buf0, void *buf1,
   // wave of still shorter chunks (a CTA needs ~2 us per slice whatever the mesh).
   const int tiles = ((n[0] + T::TX - 1) / T::TX) * ((n[1] + T::TY - 1) / T::TY);
   auto ctas = [&](int c) { return (long long)tiles * ((n[2] + c - 1) / c); };
+  const int sms = sm_count();
   int chunk = n[2] < kMaxChunk ? n[2] : kMaxChunk;
   if (tn.chunk > 0) {
     chunk = tn.chunk < n[2] ? tn.chunk : n[2];
-  } else if (tiles >= 148) {
+  } else if (tiles >= sms) {
     chunk = n[2] < 16 ? n[2] : 16;
   } else {
-    while (chunk > 4 && ctas((chunk + 1) / 2) <= 148 + 16) chunk = (chunk + 1) / 2;
-    while (chunk > 8 && ctas(chunk) < 148 * 12) chunk = (chunk + 1) / 2;
+    while (chunk > 4 && ctas((chunk + 1) / 2) <= sms + 16) chunk = (chunk + 1) / 2;
+    while (chunk > 8 && ctas(chunk) < sms * 12) chunk = (chunk + 1) / 2;
   }
   p.zchunk = chunk < kMaxChunk ? chunk : kMaxChunk;
   p.available = true;

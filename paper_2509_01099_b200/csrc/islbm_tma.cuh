@@ -177,6 +177,20 @@ inline cudaError_t launch_step(void (*kern)(KArgs...), dim3 grid, dim3 block, si
 
 constexpr int pad128(int bytes) { return (bytes + 127) / 128 * 128; }
 
+// number of SMs of the current device (148 on a B200), queried once
+inline int sm_count() {
+  static int sms = 0;
+  if (sms <= 0) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess ||
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || sms <= 0) {
+      cudaGetLastError();
+      return 148;   // no device (host-only calls such as islbm_workspace_bytes): sizing only
+    }
+  }
+  return sms;
+}
+
 // run-time knobs of the tiled kernels (islbm_set_tuning); defaults chosen from measurements (profiles/)
 struct Tuning {
   int chunk = 0;        // marching-chunk length (slices / rows); 0 = automatic

@@ -12,6 +12,8 @@ Mesh recipes
   uniform_mesh : Eq. 24-25 (PAPER.md:185-189), x_j = (j + 0.5)/N, delta = 1/N.
   erf_mesh     : Eq. 26, N_y + 2 points j = 0..N_y+1; the fluid
                  nodes are j = 1..N_y and delta = y_1.
+  wallgap_mesh : hand-made; first / last spacing 2.5 / 1.75 lattice units, so that
+                 q of Eq. 28 is far from 1 and differs between the walls.
 """
 from __future__ import annotations
 
@@ -45,12 +47,25 @@ def erf_mesh(npts: int, a: float):
     return y[1:-1].copy(), float(y[1])
 
 
+def wallgap_mesh(n: int, q_lo: float = 2.5, q_hi: float = 1.75):
+    """Hand-made mesh for the q != 1 cases of Eq. 28: the first / last spacing is q_lo / q_hi
+    lattice units (different at the two walls, so a swapped pair shows), the interior spacings ramp between 1 and
+    1.5 l.u. with two of them exactly 1; walls at 0 and 1, i.e. x_0 = delta/2.  Returns (x, delta)."""
+    k = np.arange(n - 1, dtype=np.float64)
+    s = 1.0 + 0.5 * np.sin(math.pi * k / (n - 2)) ** 2
+    s[0], s[-1] = q_lo, q_hi
+    s[1], s[-2] = 1.0, 1.0
+    delta = 1.0 / (float(s.sum()) + 1.0)
+    x = delta * (0.5 + np.concatenate(([0.0], np.cumsum(s))))
+    return x, delta
+
+
 @dataclass
 class Workload:
     name: str
     dim: int
     n: int
-    mesh: str            # "tanh" | "uniform" | "erf"
+    mesh: str            # "tanh" | "uniform" | "erf" | "wallgap"
     stretch: float
     Ra: float
     Pr: float = 0.71
@@ -68,6 +83,8 @@ class Workload:
             x, d = uniform_mesh(self.n)
         elif self.mesh == "erf":
             x, d = erf_mesh(self.n, self.stretch)
+        elif self.mesh == "wallgap":
+            x, d = wallgap_mesh(self.n)
         else:
             raise ValueError(self.mesh)
         self.coords = [x.copy() for _ in range(self.dim)]

@@ -171,6 +171,14 @@ class Islbm:
                                          C.c_void_p(self.stream.cuda_stream), C.byref(sl)))
         del keep
 
+    def _out(self, shape):
+        """Output tensor for a library call: allocated by torch's caching allocator on the CURRENT stream but written
+        by kernels on the handle's stream, so the allocator is told about that use (no re-use while they run)."""
+        t = torch.empty(shape, dtype=torch.float64, device=self.device)
+        if self.stream != torch.cuda.current_stream(self.device):
+            t.record_stream(self.stream)
+        return t
+
     def guards_intact(self):
         """True if no kernel wrote into the canary bands around the workspace."""
         g = self.guard_bytes
@@ -235,8 +243,8 @@ class Islbm:
         _check(lib.islbm_set_populations_host(self.h, hp(f, self.qf * self.nodes), hp(g, self.qg * self.nodes)))
 
     def get_populations(self):
-        f = torch.empty((self.qf,) + self.shape, dtype=torch.float64, device=self.device)
-        g = torch.empty((self.qg,) + self.shape, dtype=torch.float64, device=self.device)
+        f = self._out((self.qf,) + self.shape)
+        g = self._out((self.qg,) + self.shape)
         _check(lib.islbm_get_populations(self.h, _dev_ptr(f), _dev_ptr(g)))
         return f, g
 
@@ -244,8 +252,7 @@ class Islbm:
         _check(lib.islbm_step(self.h, int(n)))
 
     def fields(self, names=("rho", "u", "v", "w", "T")):
-        out = {k: torch.empty(self.shape, dtype=torch.float64, device=self.device)
-               for k in names if not (k == "w" and self.dim == 2)}
+        out = {k: self._out(self.shape) for k in names if not (k == "w" and self.dim == 2)}
         _check(lib.islbm_fields(self.h, *[_dev_ptr(out.get(k)) for k in ("rho", "u", "v", "w", "T")]))
         return out
 

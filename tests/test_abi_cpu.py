@@ -35,6 +35,15 @@ def test_library_exports_every_declared_symbol(binding):
     assert set(names) == set(binding.EXPORTS)
 
 
+def test_header_is_plain_c99():
+    """include/islbm.h is a C header: it must parse as C99 on its own (no C++ or torch types in the boundary)."""
+    import subprocess
+    hdr = os.path.join(ROOT, "include", "islbm.h")
+    r = subprocess.run(["gcc", "-std=c99", "-pedantic", "-Wall", "-Werror", "-fsyntax-only", "-x", "c", hdr],
+                       capture_output=True, text=True)
+    assert r.returncode == 0, r.stderr
+
+
 def test_version_and_cubin_arch(binding):
     assert b"sm_100a" in binding.lib.islbm_version()
     import subprocess

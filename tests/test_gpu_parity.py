@@ -46,6 +46,12 @@ def plane_err(a, b):
     return float((np.abs(a - b).max(1) / np.abs(b).max(1)).max())
 
 
+def elem_err(a, b):
+    """max element-wise relative error |a-b|/|b| — for the flow populations, which are strictly positive (~ w_q);
+    the plane-normalised metric above is kept for g, which crosses zero (reading A17)."""
+    return float((np.abs(a - b) / np.abs(b)).max())
+
+
 def ragged_coords(dim, ns, stretches):
     out = []
     for n, s in zip(ns[:dim], stretches[:dim]):
@@ -151,12 +157,12 @@ def test_one_step_all_populations(islbm, name, dim, ns, st):
         assert np.array_equal(f_back.cpu().numpy(), f0) and np.array_equal(g_back.cpu().numpy(), g0)
         sim.step(1)
         f1, g1 = sim.get_populations()
-        ef, eg = plane_err(f1.cpu().numpy(), fo), plane_err(g1.cpu().numpy(), go)
+        ef, eg = elem_err(f1.cpu().numpy(), fo), plane_err(g1.cpu().numpy(), go)      # f: every element (north_star)
         assert ef <= 1e-12 and eg <= 1e-12, (name, sim.kernel_name, tune, ef, eg)
         # second and third step (ping-pong both ways)
         sim.step(2)
         f3, g3 = sim.get_populations()
-        ef, eg = plane_err(f3.cpu().numpy(), fo3), plane_err(g3.cpu().numpy(), go3)
+        ef, eg = elem_err(f3.cpu().numpy(), fo3), plane_err(g3.cpu().numpy(), go3)
         assert ef <= 3e-12 and eg <= 3e-12, (name, sim.kernel_name, tune, ef, eg)
 
 
@@ -231,7 +237,7 @@ def test_upwind_stencil_parity(islbm, dim, ns):
         orc.step(n)
         f1, g1 = sim.get_populations()
         fo, go = orc.get_populations()
-        assert plane_err(f1.cpu().numpy(), fo) <= tol and plane_err(g1.cpu().numpy(), go) <= tol
+        assert elem_err(f1.cpu().numpy(), fo) <= tol and plane_err(g1.cpu().numpy(), go) <= tol
     with pytest.raises(islbm.IslbmError):
         sim.set_stencil(0)                      # the state exists: too late
 
@@ -251,7 +257,7 @@ def test_uniform_mesh_one_step(islbm):
             sim.set_populations(torch.from_numpy(f0).cuda(), torch.from_numpy(g0).cuda())
             sim.step(1)
             f1, g1 = sim.get_populations()
-            assert plane_err(f1.cpu().numpy(), fo) <= 1e-12 and plane_err(g1.cpu().numpy(), go) <= 1e-12, (dim, k, tune)
+            assert elem_err(f1.cpu().numpy(), fo) <= 1e-12 and plane_err(g1.cpu().numpy(), go) <= 1e-12, (dim, k, tune)
         # mass is conserved to round-off on the uniform mesh (pin P4 on the GPU path)
         sim.step(200)
         rho = sim.fields(("rho",))["rho"]
@@ -261,11 +267,14 @@ def test_uniform_mesh_one_step(islbm):
 # ---------------------------------------------------------------------------
 # BASELINE.json config 1: 1000 steps, populations and fields
 # ---------------------------------------------------------------------------
-def field_err(sim, orc):
+def field_err(sim, orc, floor=1e-4):
+    """u, v, w normalised by max|u| (reading A17), T by Delta_T = 1.  `floor` (lattice units) bounds the velocity
+    normaliser from below: the runs that start from rest + 1e-3 noise have |u| ~ 1e-7..1e-4 l.u. for the first
+    hundreds of steps, and the few-ulp ABSOLUTE error of sum(e f)/rho (~1e-16) would read as 1e-9 relative to
+    that; 1e-4 l.u. = 1e-3 U.  Tests of a developed flow (|u| ~ 0.1 U) pass floor=0."""
     fs, fo = sim.fields(), orc.fields()
-    # velocities are normalised by max|u|, floored at 1e-3 U = 1e-4 l.u.: a few steps after the noise start
-    # |u| ~ 1e-7 and the few-ulp absolute error of sum(e f)/rho (~1e-16) would otherwise read as 1e-9
-    umax = max(max(np.abs(fo[k]).max() for k in ("u", "v", "w")), 1e-4)
+    umax = max(max(np.abs(fo[k]).max() for k in ("u", "v", "w")), floor)
+    assert umax > 0.0
     out = {k: float(np.abs(fs[k].cpu().numpy() - fo[k]).max() / umax) for k in fs if k in ("u", "v", "w")}
     out["T"] = float(np.abs(fs["T"].cpu().numpy() - fo["T"]).max())      # Delta_T = 1
     out["rho"] = float(np.abs(fs["rho"].cpu().numpy() - fo["rho"]).max())
@@ -287,14 +296,14 @@ def test_config1_init_and_1000_steps(islbm):
     orc.step(1)
     f, g = sim.get_populations()
     fo, go = orc.get_populations()
-    assert plane_err(f.cpu().numpy(), fo) <= 1e-12 and plane_err(g.cpu().numpy(), go) <= 1e-12
+    assert elem_err(f.cpu().numpy(), fo) <= 1e-12 and plane_err(g.cpu().numpy(), go) <= 1e-12
     sim.step(999)
     orc.step(999)
     err = field_err(sim, orc)
     assert max(err.values()) <= 1e-9, err
     f, g = sim.get_populations()
     fo, go = orc.get_populations()
-    assert plane_err(f.cpu().numpy(), fo) <= 1e-9 and plane_err(g.cpu().numpy(), go) <= 1e-9
+    assert elem_err(f.cpu().numpy(), fo) <= 1e-9 and plane_err(g.cpu().numpy(), go) <= 1e-9
     ns, no = sim.nusselt(), orc.nusselt()
     for k in no:
         assert ns[k] == pytest.approx(no[k], rel=1e-9, abs=1e-12), k
@@ -347,7 +356,7 @@ def test_full_size_configs_few_steps(islbm, name, steps):
     orc.step(1)
     f, g = sim.get_populations()
     fo, go = orc.get_populations()
-    assert plane_err(f.cpu().numpy(), fo) <= 1e-12 and plane_err(g.cpu().numpy(), go) <= 1e-12
+    assert elem_err(f.cpu().numpy(), fo) <= 1e-12 and plane_err(g.cpu().numpy(), go) <= 1e-12
     del f, g
     sim.step(steps - 1)
     orc.step(steps - 1)
@@ -357,10 +366,9 @@ def test_full_size_configs_few_steps(islbm, name, steps):
     assert ns["Nu_hot"] == pytest.approx(no["Nu_hot"], rel=1e-10)
 
 
-@pytest.mark.parametrize("name,steps", [("c2_512sq", 1000), ("c4_128cu", 100)])
+@pytest.mark.parametrize("name,steps", [("c2_512sq", 1000)])
 def test_full_size_configs_long_runs(islbm, name, steps):
-    """north_star: 1e-9 on u, v, w and T after 1000 steps, at BASELINE.json's full size with the OpenMP oracle
-    (512^2: 1000 steps; 128^3: 100 steps to keep the oracle within ~20 s)."""
+    """north_star: 1e-9 on u, v and T after 1000 steps, at BASELINE.json's full size with the OpenMP oracle."""
     w = inputs.workload(name)
     sim, orc = pair(islbm, w.coords, w.delta, w.Ra, w.Pr, w.Ma, threads=len(os.sched_getaffinity(0)))
     sim.init(w.seed, w.noise_amp)
@@ -379,28 +387,43 @@ def test_full_size_configs_long_runs(islbm, name, steps):
     assert torch.equal(f0, f1) and torch.equal(g0, g1)
 
 
-@pytest.mark.skipif(os.environ.get("ISLBM_LONG") != "1", reason="20-30 min of host oracle time; set ISLBM_LONG=1")
-@pytest.mark.parametrize("name", ["c4_128cu", "c5_256cu"])
-def test_3d_configs_1000_steps_fp64_and_fp32_long(islbm, name):
-    """north_star bar on the 3-D configs at full size and the full 1000 steps (the default suite stops at 100 / 20
-    steps to keep the host oracle within seconds): fp64 within 1e-9 and fp32 storage within 1e-5 on u, v, w, T.
-    Opt-in: the OpenMP oracle needs ~3 min (128^3) / ~20 min (256^3) on 16 host threads.  Result of the last run:
-    DESIGN.md section 11."""
+def _long_3d(islbm, name, steps):
     w = inputs.workload(name)
     sim, orc = pair(islbm, w.coords, w.delta, w.Ra, w.Pr, w.Ma, threads=len(os.sched_getaffinity(0)))
     sim32 = islbm.Islbm(w.coords, w.delta, w.Ra, w.Pr, w.Ma, precision=1)
     assert sim.kernel_name == "tiled_zmarch_tma" and sim32.kernel_name == "tiled_zmarch_tma"
     for s_ in (sim, sim32, orc):
         s_.init(w.seed, w.noise_amp)
-        s_.step(1000)
+        s_.step(steps)
     err = field_err(sim, orc)
     e32 = field_err(sim32, orc)
     ns, no = sim.nusselt(), orc.nusselt()
-    print("LONG", name, "fp64", err, "fp32", e32, "Nu/Re", ns, no)
+    print("LONG", name, steps, "steps: fp64", err, "fp32", e32, "Nu/Re", ns, no)
     assert max(err.values()) <= 1e-9, err
     assert max(e32[k] for k in ("u", "v", "w", "T")) <= 1e-5, e32
     for k in no:
         assert ns[k] == pytest.approx(no[k], rel=1e-9, abs=1e-12), k
+    assert sim.nusselt_middle() == pytest.approx(orc.nusselt_middle(), rel=1e-9, abs=1e-12)
+
+
+def test_config4_128cu_1000_steps_fp64_and_fp32(islbm):
+    """BASELINE.json config 4 at full size and the full 1000 steps of north_star: fp64 within 1e-9 and fp32 storage
+    within 1e-5 on u, v, w, T; every diagnostic within 1e-9 (about 3 min of OpenMP oracle on the GPU box)."""
+    _long_3d(islbm, "c4_128cu", 1000)
+
+
+def test_config5_256cu_100_steps_fp64_and_fp32(islbm):
+    """BASELINE.json config 5 at full size, launch configuration of bench.py, the 100 steps SURVEY.md 8(d) prescribes
+    for it (about 2 min of OpenMP oracle); the full 1000 steps are the opt-in test below (21 min of oracle: beyond
+    the driver's pytest limit; its last result line is committed in profiles/r2_long_parity.md)."""
+    _long_3d(islbm, "c5_256cu", 100)
+
+
+@pytest.mark.skipif(os.environ.get("ISLBM_LONG") != "1", reason="~21 min of host oracle time; set ISLBM_LONG=1")
+def test_config5_256cu_1000_steps_fp64_and_fp32_long(islbm):
+    """north_star bar on config 5 at full size and the full 1000 steps.  Opt-in (the OpenMP oracle needs ~20 min for
+    256^3 x 1000 on 16 host threads); result of the last run: profiles/r2_long_parity.md."""
+    _long_3d(islbm, "c5_256cu", 1000)
 
 
 def test_config3_1024sq_1000_steps_fp64_and_fp32(islbm):
@@ -441,34 +464,130 @@ def test_config5_256cu_sampled_nodes(islbm):
     go = np.empty_like(gs)
     for k, (ix, iy, iz) in enumerate(pts):
         fo[:, k], go[:, k] = orc.step_node(int(ix), int(iy), int(iz))
-    assert plane_err(fs, fo) <= 1e-12 and plane_err(gs, go) <= 1e-12
+    assert elem_err(fs, fo) <= 1e-12 and plane_err(gs, go) <= 1e-12
     # properties that hold at any size: rho ~ 1, T within the noise amplitude, everything finite
     fl = sim.fields(("rho", "T"))
     assert torch.isfinite(fl["rho"]).all() and (fl["rho"] - 1).abs().max().item() < 1e-6
     assert fl["T"].abs().max().item() < 0.2     # one anti-bounce-back kick of omega*T_w at the x-walls
 
 
-def test_config5_256cu_full_mesh_20_steps(islbm):
-    """256^3 full size, launch configuration of bench.py: all fields after 20 steps against the OpenMP oracle
-    (bit-identical to its single-thread mode, test_threads_are_bit_identical), fp64 and fp32 storage."""
-    w = inputs.workload("c5_256cu")
-    sim, orc = pair(islbm, w.coords, w.delta, w.Ra, w.Pr, w.Ma, threads=len(os.sched_getaffinity(0)))
-    assert sim.kernel_name == "tiled_zmarch_tma"
-    sim.init(w.seed, w.noise_amp)
-    orc.init(w.seed, w.noise_amp)
-    sim.step(20)
-    orc.step(20)
-    err = field_err(sim, orc)
-    assert max(err.values()) <= 1e-10, err
+# ---------------------------------------------------------------------------
+# Eq. 28 with q != 1 (paper-mode erf mesh, hand-made mesh) and developed flows against the oracle
+# ---------------------------------------------------------------------------
+def _diag_close(sim, orc, rel=1e-9):
     ns, no = sim.nusselt(), orc.nusselt()
-    for k in no:
-        assert ns[k] == pytest.approx(no[k], rel=1e-9, abs=1e-12), k
-    sim.close()
-    sim32 = islbm.Islbm(w.coords, w.delta, w.Ra, w.Pr, w.Ma, precision=1)
-    sim32.init(w.seed, w.noise_amp)
-    sim32.step(20)
-    e32 = field_err(sim32, orc)
-    assert e32["u"] <= 1e-5 and e32["v"] <= 1e-5 and e32["w"] <= 1e-5 and e32["T"] <= 1e-5, e32
+    for k in no:                                           # Nu_hot, Nu_cold, Re, u2, Nu_vol
+        assert ns[k] == pytest.approx(no[k], rel=rel, abs=1e-12), (k, ns[k], no[k])
+    nm_s, nm_o = sim.nusselt_middle(), orc.nusselt_middle()
+    assert nm_s == pytest.approx(nm_o, rel=rel, abs=1e-12), ("Nu_middle", nm_s, nm_o)
+    return ns
+
+
+@pytest.mark.parametrize("kind,dim,n", [("erf", 2, 129), ("wallgap", 2, 40), ("erf", 3, 49), ("wallgap", 3, 22)])
+def test_q_not_one_meshes_populations_fields_and_all_six_diagnostics(islbm, kind, dim, n):
+    """Meshes on which q of Eq. 28 is NOT 1: the paper's erf mesh with delta = y_1 (paper mode,
+    Ma = 0.1, T0 = T_cold) and the hand-made mesh with q = 2.5 at the hot and 1.75 at the cold wall.  Populations
+    1e-12 after one step from a far-from-equilibrium state; fields and all six diagnostics (Nu_hot, Nu_cold, <Re>,
+    <u*^2>, <Nu>, Nu_middle) 1e-9 after 300 steps from the seeded start.  The oracle side of Eq. 28 at q != 1 is pinned by
+    test_P6b / test_P6c (tests/test_oracle_pins.py); a swapped or inverted q on the CUDA side fails here."""
+    if kind == "erf":
+        x, delta = inputs.erf_mesh(n, 1.5)
+        Ma, T0 = 0.1, -0.5
+    else:
+        x, delta = inputs.wallgap_mesh(n)
+        Ma, T0 = 0.1 * SQ3, 0.0
+    coords = [x.copy() for _ in range(dim)]
+    q_lo, q_hi = (x[1] - x[0]) / delta, (x[-1] - x[-2]) / delta
+    assert q_lo > 1.005 and q_hi > 1.005
+    H_lu = (x[-1] - x[0] + delta) / delta
+    # erf: the paper's Ra for these grids; hand-made mesh (H_lu = 52 / 29 l.u.): Ra such that nu = 0.03 l.u.
+    Ra = (1e6 if dim == 2 else 1e5) if kind == "erf" else 0.71 * (0.1 * H_lu / 0.03) ** 2
+    sim, orc = pair(islbm, coords, delta, Ra, 0.71, Ma)
+    sim.set_reference_temperature(T0)
+    orc.set_reference_temperature(T0)
+    f0, g0 = inputs.random_state(orc.shape, orc.qf, orc.qg, seed=17 + dim, amp=0.05)
+    orc.set_populations(f0, g0)
+    sim.set_populations(torch.from_numpy(f0).cuda(), torch.from_numpy(g0).cuda())
+    sim.step(1)
+    orc.step(1)
+    f1, g1 = sim.get_populations()
+    fo, go = orc.get_populations()
+    assert elem_err(f1.cpu().numpy(), fo) <= 1e-12 and plane_err(g1.cpu().numpy(), go) <= 1e-12
+    _diag_close(sim, orc)                                   # far from equilibrium: every term of every sum is O(1)
+    sim.init(0, 1e-3)
+    orc.init(0, 1e-3)
+    sim.step(300)
+    orc.step(300)
+    err = field_err(sim, orc)
+    assert max(err.values()) <= 1e-9, err
+    ns = _diag_close(sim, orc)
+    assert ns["Nu_hot"] > 1.5                               # the wall layer is developing: a curved profile at the wall
+
+
+@pytest.mark.parametrize("dim,n,Ra", [(2, 64, 1e5), (3, 32, 1e5)])
+def test_developed_flow_parity_1000_steps(islbm, dim, n, Ra):
+    """The nonlinear regime: config 1 (64^2, Ra = 1e5) and a 32^3 cavity are run on the GPU to the steady-state
+    criterion of Eq. 30, that state (f_t, g_t) is injected into the oracle, and both sides then
+    take 1000 steps: populations, fields (velocity normaliser NOT floored: |u| ~ 0.2 U) and all six diagnostics within
+    1e-9.  (The seeded-start tests above stay in the conduction transient, |u| <= 1e-4 l.u.)"""
+    w = inputs.workload("c1_64sq") if dim == 2 else inputs.custom_workload("dev3", 3, n, stretch=1.5, Ra=Ra)
+    sim, orc = pair(islbm, w.coords, w.delta, w.Ra, w.Pr, w.Ma)
+    sim.init(w.seed, w.noise_amp)
+    sim.steady_residual()
+    for _ in range(400):
+        sim.step(2000)
+        ru, rT = sim.steady_residual()
+        if ru < 1e-9 and rT < 1e-9:
+            break
+    assert ru < 1e-6 and rT < 1e-6, (ru, rT)               # developed (steady to 1e-9 in practice)
+    f, g = sim.get_populations()
+    orc.set_populations(f.cpu().numpy(), g.cpu().numpy())
+    nu0 = sim.nusselt()
+    assert nu0["Nu_hot"] > 2.0 and nu0["Re"] > 5.0          # a convecting cavity, not the conduction transient
+    sim.step(1)
+    orc.step(1)
+    f1, g1 = sim.get_populations()
+    fo, go = orc.get_populations()
+    assert elem_err(f1.cpu().numpy(), fo) <= 1e-12 and plane_err(g1.cpu().numpy(), go) <= 1e-12
+    sim.step(999)
+    orc.step(999)
+    err = field_err(sim, orc, floor=0.0)
+    assert max(err.values()) <= 1e-9, err
+    f1, g1 = sim.get_populations()
+    fo, go = orc.get_populations()
+    assert elem_err(f1.cpu().numpy(), fo) <= 1e-9 and plane_err(g1.cpu().numpy(), go) <= 1e-9
+    _diag_close(sim, orc)
+
+
+def test_paper_mode_convergence_order(islbm, golden):
+    """three paper-mode grids with refinement ratio 2 (65, 129, 257 points of
+    Eq. 26, a = 1.5, Ma = 0.1, Ra = 1e6, T0 = T_cold), each run to Eq. 30.  Observed order p of Eq. 35 for the
+    domain-integrated <Nu> and for Nu_hot in [2.2, 3.2] (the paper: "nearly third-order ... in domain-integrated
+    quantities", p = 2.6 for <Nu>), and the Richardson value of Nu_hot (Eq. 36) within 0.1 % of the 8.8206 Table 2
+    prints as its own grid-independent value."""
+    vals = {}
+    for npts in (65, 129, 257):
+        w = inputs.custom_workload("conv", 2, npts, mesh="erf", stretch=1.5, Ra=1e6, Ma=0.1)
+        sim = islbm.Islbm(w.coords, w.delta, w.Ra, w.Pr, w.Ma)
+        sim.set_reference_temperature(-0.5)
+        sim.init(0, 0.0)
+        sim.steady_residual()
+        for _ in range(1500):
+            sim.step(2000)
+            ru, rT = sim.steady_residual()
+            if ru < 1e-9 and rT < 1e-9:
+                break
+        assert ru < 1e-9 and rT < 1e-9, (npts, ru, rT)
+        nu = sim.nusselt()
+        vals[npts] = (nu["Nu_vol"], nu["Nu_hot"], sim.nusselt_middle())
+        sim.close()
+    print("CONVERGENCE", vals)
+    order = lambda k: math.log(abs((vals[65][k] - vals[129][k]) / (vals[129][k] - vals[257][k]))) / math.log(2.0)
+    p_vol, p_hot, p_mid = order(0), order(1), order(2)
+    assert 2.2 <= p_vol <= 3.2 and 2.2 <= p_hot <= 3.2 and 2.2 <= p_mid <= 3.2, (p_vol, p_hot, p_mid)
+    rp = 2.0 ** p_hot
+    nu_hot_inf = (rp * vals[257][1] - vals[129][1]) / (rp - 1.0)                 # Eq. 36
+    assert nu_hot_inf == pytest.approx(golden["table2"]["Ra1e6"]["inf"][1], rel=1e-3)
 
 
 # ---------------------------------------------------------------------------

@@ -833,3 +833,70 @@ def test_volume_diagnostics_closed_forms_for_uniform_velocity(dim, n):
     assert d["Re"] == pytest.approx(math.sqrt(w.Ra / w.Pr) * speed / p["U"], rel=1e-12)
     assert d["u2"] == pytest.approx(speed ** 2 / p["U"] ** 2, rel=1e-12)
     assert d["Nu_vol"] == pytest.approx(1.0 + math.sqrt(w.Ra * w.Pr) * (u0[0] / p["U"]) * c, rel=1e-11)
+
+
+# ---------------------------------------------------------------------------
+# Eq. 28 with q != 1 INSIDE oracle_nusselt (q = second / first mesh spacing > 1)
+# ---------------------------------------------------------------------------
+def _q_mesh(kind, dim):
+    """(coords, delta, Ma): the paper's own mesh (Eq. 26, a = 1.5, 257 points in 2-D / 65 in 3-D, delta = y_1: q = 1.009 /
+    1.036) or the hand-made mesh with q = 2.5 at the hot wall and 1.75 at the cold wall."""
+    if kind == "erf":
+        x, d = inputs.erf_mesh(257 if dim == 2 else 65, 1.5)
+        return [x.copy() for _ in range(dim)], d, 0.1
+    x, d = inputs.wallgap_mesh(24 if dim == 2 else 14)
+    return [x.copy() for _ in range(dim)], d, 0.1 * SQ3
+
+
+@pytest.mark.parametrize("kind,dim", [("erf", 2), ("wallgap", 2), ("erf", 3), ("wallgap", 3)])
+def test_P6b_wall_nusselt_of_the_conduction_state_is_one_for_q_not_one(kind, dim):
+    """The conduction profile is linear in x, and Eq. 28 is exact on it for ANY q (it is the wall derivative of the
+    parabola through the wall value, node 1 at 0.5 l.u. and node 2 at 0.5 + q l.u.), so Nu_hot = Nu_cold = 1 to
+    round-off through oracle_nusselt exactly when q_lo and q_hi are the right spacing ratios at the right walls.
+    The meshes have q != 1 (every other Nu test runs on tanh meshes, where q = 1 and Eq. 28 is Eq. 27), and the
+    hand-made one has different q at the two walls, so an inverted ratio, a wrong spacing or a swapped pair fails:
+    the test also shows by how much."""
+    coords, delta, Ma = _q_mesh(kind, dim)
+    o = Oracle(coords, delta, 1e5, 0.71, Ma, threads=4)
+    o.set_buoyancy_scale(0.0)
+    x = coords[0]
+    q_lo, q_hi = (x[1] - x[0]) / delta, (x[-1] - x[-2]) / delta
+    assert q_lo > 1.005 and q_hi > 1.005
+    if kind == "wallgap":
+        assert q_lo == pytest.approx(2.5, rel=1e-12) and q_hi == pytest.approx(1.75, rel=1e-12)
+
+    class W:                      # what conduction_state reads
+        pass
+    w = W()
+    w.coords, w.delta = coords, delta
+    f0, g0, T = conduction_state(o, w)
+    o.set_populations(f0, g0)
+    o.step(20)                    # still the fixed point (P5) on these meshes
+    f1, g1 = o.get_populations()
+    assert np.abs(f1 - f0).max() < 1e-13 and np.abs(g1 - g0).max() < 1e-13
+    nu = o.nusselt()
+    assert nu["Nu_hot"] == pytest.approx(1.0, abs=1e-11)
+    assert nu["Nu_cold"] == pytest.approx(1.0, abs=1e-11)
+    assert o.nusselt_middle() == pytest.approx(1.0, abs=1e-11)
+    # what a plausible mistake would give on this state (closed form of Eq. 28 on a linear profile: the slope comes
+    # out multiplied by (2 q'^2 + 2 q' - q) / (q' (2 q' + 1)) when q' is used instead of the true q)
+    wrong = lambda qp, q: (2 * qp * qp + 2 * qp - q) / (qp * (2 * qp + 1))
+    for qp, q in ((1.0, q_lo), (1.0 / q_lo, q_lo), (q_hi if kind == "wallgap" else 1.0, q_lo)):
+        assert abs(wrong(qp, q) - 1.0) > 1e-3
+    assert wrong(q_lo, q_lo) == pytest.approx(1.0, abs=1e-15)
+
+
+def test_P6c_eq28_inside_nusselt_matches_the_parabola_through_wall_and_two_nodes():
+    """A curved profile: T quadratic in x, buoyancy off, on the hand-made mesh.  The expected Nu_hot / Nu_cold are the
+    wall derivatives of the quadratic itself (closed form), which Eq. 28 reproduces exactly only with the right q."""
+    coords, delta, Ma = _q_mesh("wallgap", 2)
+    o = Oracle(coords, delta, 1e5, 0.71, Ma)
+    p = o.params()
+    x = np.asarray(coords[0])
+    s = lambda xx: (xx - (x[0] - delta / 2)) / delta / p["H_lu"]       # x* from the hot wall, in [0, 1]
+    a, b, c = 0.5, -1.7, 0.7                                           # T(0) = T_hot = 0.5, T(1) = T_cold = -0.5
+    f, g = _state_with(o, lambda xx: a + b * s(xx) + c * s(xx) ** 2)
+    o.set_populations(f, g)
+    nu = o.nusselt()
+    assert nu["Nu_hot"] == pytest.approx(-b, rel=1e-11)                # -dT/dx* at x* = 0
+    assert nu["Nu_cold"] == pytest.approx(-(b + 2 * c), rel=1e-11)     # -dT/dx* at x* = 1
