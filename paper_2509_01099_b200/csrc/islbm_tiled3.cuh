@@ -426,7 +426,7 @@ struct Plan3 {
 };
 
 template <typename ST, int TX, int TY>
-inline bool plan3_setup(Plan3 &p, const int *n, int nxp, void *buf0, void *buf1, const Tuning &tn) {
+inline bool plan3_maps(Plan3 &p, const int *n, int nxp, void *buf0, void *buf1, const Tuning &tn) {
   using T = Tile3<ST, TX, TY>;
   p.available = false;
   auto no = [&](const char *why) { snprintf(p.why_not, sizeof p.why_not, "%s", why); return false; };
@@ -450,10 +450,6 @@ inline bool plan3_setup(Plan3 &p, const int *n, int nxp, void *buf0, void *buf1,
         !make_map(&p.maps[i].xy, bufs[i], eb, 4, dims, b_xy, tn.l2promo, nxp))
       return no("cuTensorMapEncodeTiled failed");
   }
-  if (cudaFuncSetAttribute(k_step_zmarch<ST, TX, TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM_BYTES) != cudaSuccess) {
-    cudaGetLastError();
-    return no("cudaFuncSetAttribute failed");
-  }
   // z-chunks (measured, profiles/): short chunks win — neighbouring CTAs stay in step, so the halo overlap is found in
   // L2, and the tail is fine-grained.  Meshes with at least one CTA per SM in every z-layer of tiles take 16 slices (the
   // 2-slice prologue then re-reads 12 of 26 planes twice per 16: +6 % reads through L2); smaller meshes take one full
@@ -475,22 +471,17 @@ inline bool plan3_setup(Plan3 &p, const int *n, int nxp, void *buf0, void *buf1,
   return true;
 }
 
-template <typename ST>
-inline bool plan3_create(Plan3 &p, const int *n, int nxp, void *buf0, void *buf1, const Tuning &tn) {
-  // tile shape (x by y nodes per CTA).  fp64 storage: 32x8 (250 registers, one CTA per SM; DRAM-bound).  fp32 storage
-  // is bound by latency at 8 warps per SM, so it takes smaller CTAs, capped at 168 registers by their launch bounds
-  // (14 spilled): 32x6 (two CTAs = 12 warps per SM; 256^3 0.56 -> 0.61) or 32x4 (three CTAs) on short y-axes
-  // (128^3 0.45 -> 0.52).  Measured in profiles/r1_c5_256cu_zmarch_v4.md.
-  int shape = tn.shape3d;
-  if (shape == 0) shape = sizeof(ST) == 4 ? (n[1] >= 192 ? 3 : 4) : 5;
-  p.shape = shape;
-  switch (shape) {
-    case 1: return plan3_setup<ST, 64, 4>(p, n, nxp, buf0, buf1, tn);
-    case 2: return plan3_setup<ST, 128, 2>(p, n, nxp, buf0, buf1, tn);
-    case 3: return plan3_setup<ST, 32, 6>(p, n, nxp, buf0, buf1, tn);
-    case 4: return plan3_setup<ST, 32, 4>(p, n, nxp, buf0, buf1, tn);
-    default: p.shape = 5; return plan3_setup<ST, 32, 8>(p, n, nxp, buf0, buf1, tn);
+template <typename ST, int TX, int TY>
+inline bool plan3_setup(Plan3 &p, const int *n, int nxp, void *buf0, void *buf1, const Tuning &tn) {
+  using T = Tile3<ST, TX, TY>;
+  if (!plan3_maps<ST, TX, TY>(p, n, nxp, buf0, buf1, tn)) return false;
+  if (cudaFuncSetAttribute(k_step_zmarch<ST, TX, TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM_BYTES) != cudaSuccess) {
+    cudaGetLastError();
+    p.available = false;
+    snprintf(p.why_not, sizeof p.why_not, "cudaFuncSetAttribute failed");
+    return false;
   }
+  return true;
 }
 
 template <typename ST, int TX, int TY>
@@ -500,19 +491,6 @@ inline void launch3_shape(const Plan3 &p, const int *n, const DevMesh &m, const 
   dim3 grid((n[0] + T::TX - 1) / T::TX, (n[1] + T::TY - 1) / T::TY, (m.em_hi - m.em_lo + p.zchunk - 1) / p.zchunk);
   launch_step(k_step_zmarch<ST, TX, TY>, grid, dim3(T::THREADS), T::SMEM_BYTES, stream, tn.pdl != 0, p.maps[cur], m, np,
               (const ST *)buf[cur], (ST *)buf[1 - cur], p.zchunk, tn.load_policy, tn.store_policy, tn.fill == 2 ? 1 : 0);
-}
-
-template <typename ST>
-inline cudaError_t launch3(const Plan3 &p, const int *n, const DevMesh &m, const NodeParams &np, int cur, void *const *buf,
-                           const Tuning &tn, cudaStream_t stream) {
-  switch (p.shape) {
-    case 1: launch3_shape<ST, 64, 4>(p, n, m, np, cur, buf, tn, stream); break;
-    case 2: launch3_shape<ST, 128, 2>(p, n, m, np, cur, buf, tn, stream); break;
-    case 3: launch3_shape<ST, 32, 6>(p, n, m, np, cur, buf, tn, stream); break;
-    case 4: launch3_shape<ST, 32, 4>(p, n, m, np, cur, buf, tn, stream); break;
-    default: launch3_shape<ST, 32, 8>(p, n, m, np, cur, buf, tn, stream);
-  }
-  return cudaPeekAtLastError();
 }
 
 }  // namespace islbmk
