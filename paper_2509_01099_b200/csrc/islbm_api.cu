@@ -13,7 +13,6 @@
 #include "../../include/islbm.h"
 #include "islbm_kernels.cuh"
 #include "islbm_reduce.cuh"
-#include "islbm_pair.cuh"
 #include "islbm_tiled2.cuh"
 #include "islbm_tiled3.cuh"
 #include "islbm_uniform.cuh"
@@ -573,7 +572,7 @@ extern "C" int islbm_set_tuning(islbm_t *h, const char *key, int value) {
   else if (k == "store_policy") t.store_policy = value;
   else if (k == "tx2d") { if (value != 0 && value != 128 && value != 224) return fail(ISLBM_ERR_ARG, "tx2d must be 0, 128 or 224"); t.tx2d = value; }
   else if (k == "serpentine") t.serpentine = value;
-  else if (k == "shape3d") { if (value > 8) return fail(ISLBM_ERR_ARG, "shape3d must be 0 (automatic) .. 8"); t.shape3d = value; }
+  else if (k == "shape3d") { if (value > 5) return fail(ISLBM_ERR_ARG, "shape3d must be 0 (automatic) .. 5"); t.shape3d = value; }
   else if (k == "pdl") t.pdl = value;
   else if (k == "fill") { if (value > 2) return fail(ISLBM_ERR_ARG, "fill must be 0 (automatic), 1 (early) or 2 (late)"); t.fill = value; }
   else if (k == "ring2d") { if (value != 0 && value != 3 && value != 4) return fail(ISLBM_ERR_ARG, "ring2d must be 0 (automatic), 3 or 4"); t.ring2d = value; }

@@ -25,6 +25,11 @@
 
 namespace islbmk {
 
+// CTAs per SM of the fp32-storage kernels (launch bounds): five = 96 registers (measured, profiles/attempts.md)
+#ifndef ISLBM_F32_CTAS2D
+#define ISLBM_F32_CTAS2D 5
+#endif
+
 template <typename ST, int TX_, int STAGES_>
 struct Tile2 {
   static constexpr int TX = TX_, STAGES = STAGES_;
@@ -43,7 +48,11 @@ struct Tile2 {
   static constexpr uint32_t M_BYTES = 4u * P_C + 4u * P_X;   // planes of the y-stencil row
   static constexpr int BAR_OFF = STAGES * STAGE_BYTES;
   static constexpr int W_OFF = BAR_OFF + 128;                // y-weights of the chunk [sign][k][kMaxChunk]
-  static constexpr size_t SMEM_BYTES = (size_t)W_OFF + 6 * kMaxChunk * 8 + 128;
+  // fp32 storage: the x-interpolated values of the three y-stencil rows live in shared memory, [slot 3][pair 4][thread]
+  // float2, not in registers (Tile3::S_IN_SMEM, islbm_tiled3.cuh)
+  static constexpr bool S_IN_SMEM = sizeof(ST) == 4 && ISLBM_S_IN_SMEM;
+  static constexpr int S_OFF = W_OFF + 6 * kMaxChunk * 8 + 128;
+  static constexpr size_t SMEM_BYTES = (size_t)S_OFF + (S_IN_SMEM ? 3 * 4 * TX * 8 : 0);
 };
 
 // tensor maps over (x, y, plane): one per box shape
@@ -79,30 +88,27 @@ __device__ __forceinline__ void issue_stage2(int s, int yf, int ny, int x0, unsi
   }
 }
 
-// x-interpolated values of one y-stencil row for the 8 populations with e_y != 0:
-//   index: 0 f2, 1 f4, 2 g2, 3 g4, 4 f5, 5 f6, 6 f7, 7 f8
-#define ISLBM_LOAD_M2(S)                                     \
-  do {                                                       \
-    S[0] = (AT)PC4(0)[tx];                   /* f2 */        \
-    S[1] = (AT)PC4(1)[tx];                   /* f4 */        \
-    S[2] = (AT)PC4(2)[tx];                   /* g2 */        \
-    S[3] = (AT)PC4(3)[tx];                   /* g4 */        \
-    S[4] = tap3(PXM(0) + o_x, 1, wx[1]);     /* f5 ( 1, 1) */ \
-    S[5] = tap3(PXM(1) + o_x, 1, wx[0]);     /* f6 (-1, 1) */ \
-    S[6] = tap3(PXM(2) + o_x, 1, wx[0]);     /* f7 (-1,-1) */ \
-    S[7] = tap3(PXM(3) + o_x, 1, wx[1]);     /* f8 ( 1,-1) */ \
+// x-interpolated values of one y-stencil row for the 8 populations with e_y != 0, as 4 pairs (islbm_tiled3.cuh: Pr):
+//   0 (f2, f4)  1 (g2, g4)  2 (f5, f7)  3 (f8, f6)
+// (lane a has e_y = +1 in pairs 0, 1, 2 and e_y = -1 in pair 3, which takes the swapped y-weights)
+#define ISLBM_LOAD_M2(S)                                                            \
+  do {                                                                              \
+    S[0] = mkpr((AT)PC4(0)[0], (AT)PC4(1)[0]);         /* f2, f4 */                 \
+    S[1] = mkpr((AT)PC4(2)[0], (AT)PC4(3)[0]);         /* g2, g4 */                 \
+    S[2] = ptap3(PXM(0), PXM(2), 1, wxN);              /* f5 (+x,+y), f7 (-x,-y) */ \
+    S[3] = ptap3(PXM(3), PXM(1), 1, wxN);              /* f8 (+x,-y), f6 (-x,+y) */ \
   } while (0)
 // y-direction of the separable interpolation; (P0,P1,P2) = stencil rows in ascending y
-#define ISLBM_YCOMB2(P0, P1, P2)                 \
-  do {                                           \
-    f[2] = comb3(wy[1], P0[0], P1[0], P2[0]);    \
-    f[4] = comb3(wy[0], P0[1], P1[1], P2[1]);    \
-    g[2] = comb3(wy[1], P0[2], P1[2], P2[2]);    \
-    g[4] = comb3(wy[0], P0[3], P1[3], P2[3]);    \
-    f[5] = comb3(wy[1], P0[4], P1[4], P2[4]);    \
-    f[6] = comb3(wy[1], P0[5], P1[5], P2[5]);    \
-    f[7] = comb3(wy[0], P0[6], P1[6], P2[6]);    \
-    f[8] = comb3(wy[0], P0[7], P1[7], P2[7]);    \
+#define ISLBM_YCOMB2(P0, P1, P2)                          \
+  do {                                                    \
+    const Pr<AT> q0 = pcomb3(wyN, P0[0], P1[0], P2[0]);   \
+    const Pr<AT> q1 = pcomb3(wyN, P0[1], P1[1], P2[1]);   \
+    const Pr<AT> q2 = pcomb3(wyN, P0[2], P1[2], P2[2]);   \
+    const Pr<AT> q3 = pcomb3(wyS, P0[3], P1[3], P2[3]);   \
+    f[2] = lane_a(q0); f[4] = lane_b(q0);                 \
+    g[2] = lane_a(q1); g[4] = lane_b(q1);                 \
+    f[5] = lane_a(q2); f[7] = lane_b(q2);                 \
+    f[8] = lane_a(q3); f[6] = lane_b(q3);                 \
   } while (0)
 
 template <typename ST, int TX, int STAGES, int MINB, int DIR>
@@ -148,7 +154,7 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
   }
   for (int i = (int)threadIdx.x - 32; i >= 0 && i < 6 * (y1 - y0); i += T::TX - 32) {   // warps 1..: warp 0 is waiting above
     const int sk = i / (y1 - y0), yi = i - sk * (y1 - y0);
-    wys[sk * kMaxChunk + yi] = (AT)__ldg(wrow(m, 1, sk / 3, sk % 3) + y0 + yi);
+    stage_march_weight(wys, sk, yi, __ldg(wrow(m, 1, sk / 3, sk % 3) + y0 + yi));
   }
   pdl_wait();
   __syncthreads();
@@ -166,59 +172,85 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
   const bool wall_x = wf.lo[0] | wf.hi[0];
   const int sx = wf.lo[0] ? 1 : (wf.hi[0] ? -1 : 0);
   const int o_x = tx + T::XH - 1 + sx;
-  AT wx[2][3];
+  Pr<AT> wxN[3];
 #pragma unroll
-  for (int s = 0; s < 2; ++s)
-#pragma unroll
-    for (int k = 0; k < 3; ++k) wx[s][k] = valid ? (AT)__ldg(wrow(m, 0, s, k) + x) : (AT)0;
+  for (int k = 0; k < 3; ++k)
+    wxN[k] = mkpr(valid ? (AT)__ldg(wrow(m, 0, 1, k) + x) : (AT)0, valid ? (AT)__ldg(wrow(m, 0, 0, k) + x) : (AT)0);
+  // the node's index in plane 0 at the chunk's first row; advanced by one row (DIR) per emitted row
+  long long c = (long long)yf * m.nxp + x;
 
   // three register sets hold the y-stencil rows; `newest` names the one written last, so the marching order
   // (oldest first) is (newest+1, newest+2, newest) mod 3 and nothing is ever copied between sets
-  AT S0[8], S1[8], S2[8];
+  Pr<AT> S0[4], S1[4], S2[4];
   int newest = 2;
+  Pr<AT> *ssm = reinterpret_cast<Pr<AT> *>(smem_raw + T::S_OFF) + threadIdx.x;   // S_IN_SMEM: [slot][pair][thread]
+  constexpr int SSLOT = 4 * T::TX;
 
 #pragma unroll 1
   for (int s = 0; s < nstage; ++s) {
-    const int st = s % T::STAGES;
+    const int st = s % T::STAGES;     // warp-uniform (uniform datapath)
     const uint32_t ph = (uint32_t)(s / T::STAGES) & 1u;
     const int y = yf + DIR * (s - 2);
     const bool has_emit = s >= 2;
-    const bool has_mov = s <= 2 || sbase(y, m.ny) != sbase(y - DIR, m.ny);
-    const unsigned char *sb = stage0 + (size_t)st * T::STAGE_BYTES;
-    auto PC2 = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_C2 + k * T::P_C); };
-    auto PXR = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_XR + k * T::P_X); };
-    auto PC4 = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_C4 + k * T::P_C); };
-    auto PXM = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_XM + k * T::P_X); };
+    const bool has_mov = s <= 2 || sbase_moves(DIR > 0 ? y : y + 1, m.ny);
+    const ST *sb = reinterpret_cast<const ST *>(stage0 + (size_t)st * T::STAGE_BYTES);
+    const ST *sbc = sb + tx, *sbx = sb + o_x;
+    constexpr int ES = (int)sizeof(ST);
+#define PC2(k) (sbc + (T::OFF_C2 + (k) * T::P_C) / ES)
+#define PXR(k) (sbx + (T::OFF_XR + (k) * T::P_X) / ES)
+#define PC4(k) (sbc + (T::OFF_C4 + (k) * T::P_C) / ES)
+#define PXM(k) (sbx + (T::OFF_XM + (k) * T::P_X) / ES)
     mbar_wait(&full[st], ph);
 
     if (has_mov) {
       newest = newest == 2 ? 0 : newest + 1;
-      if (newest == 0) ISLBM_LOAD_M2(S0);
-      else if (newest == 1) ISLBM_LOAD_M2(S1);
-      else ISLBM_LOAD_M2(S2);
+      if constexpr (T::S_IN_SMEM) {
+        ISLBM_LOAD_M2(S2);       // S2 = the newest row, in registers for this iteration and in its shared-memory slot
+#pragma unroll
+        for (int k = 0; k < 4; ++k) ssm[newest * SSLOT + k * T::TX] = S2[k];
+      } else {
+        if (newest == 0) ISLBM_LOAD_M2(S0);
+        else if (newest == 1) ISLBM_LOAD_M2(S1);
+        else ISLBM_LOAD_M2(S2);
+      }
     }
 
+    AT f[9], g[5];   // fp64, or fp32 deviations (fp32 storage)
     if (has_emit) {
-      AT wy[2][3];
-#pragma unroll
-      for (int sg = 0; sg < 2; ++sg)
-#pragma unroll
-        for (int k = 0; k < 3; ++k) wy[sg][k] = wys[(sg * 3 + k) * kMaxChunk + (y - y0)];
-      AT f[9], g[5];   // fp64, or fp32 deviations (fp32 storage)
-      f[0] = PC2(0)[tx];
-      g[0] = PC2(1)[tx];
-      f[1] = tap3(PXR(0) + o_x, 1, wx[1]);
-      f[3] = tap3(PXR(1) + o_x, 1, wx[0]);
-      g[1] = tap3(PXR(2) + o_x, 1, wx[1]);
-      g[3] = tap3(PXR(3) + o_x, 1, wx[0]);
-      // hand the slot back; the warp whose release is the last one refills it at once with stage s + STAGES, so
-      // STAGES - 1 stages are in flight whenever one is being consumed
-      __syncwarp();
-      if ((threadIdx.x & 31) == 0 && mbar_arrive_is_last(&empty[st]) && s + T::STAGES < nstage &&
-          atomicCAS(&claim[st], s / T::STAGES, s / T::STAGES + 1) == s / T::STAGES)
-        issue_stage2<T, DIR>(s + T::STAGES, yf, m.ny, x0, stage0, full, empty, mp, lpol);
+      f[0] = PC2(0)[0];
+      g[0] = PC2(1)[0];
+      const Pr<AT> p1 = ptap3(PXR(0), PXR(1), 1, wxN);   // f1 (+x), f3 (-x)
+      const Pr<AT> p2 = ptap3(PXR(2), PXR(3), 1, wxN);   // g1, g3
+      f[1] = lane_a(p1); f[3] = lane_b(p1);
+      g[1] = lane_a(p2); g[3] = lane_b(p2);
+    }
+    // hand the slot back; the warp whose release is the last one refills it at once with stage s + STAGES, so
+    // STAGES - 1 stages are in flight whenever one is being consumed
+    __syncwarp();
+    if ((threadIdx.x & 31) == 0 && mbar_arrive_is_last(&empty[st]) && s + T::STAGES < nstage &&
+        atomicCAS(&claim[st], s / T::STAGES, s / T::STAGES + 1) == s / T::STAGES)
+      issue_stage2<T, DIR>(s + T::STAGES, yf, m.ny, x0, stage0, full, empty, mp, lpol);
+
+    if (has_emit) {
+      Pr<AT> wyN[3], wyS[3];
+      load_march_weights(wys, y - y0, wyN, wyS);
       // ascending-y order of the stencil rows: the marching order when DIR = +1, its reverse when DIR = -1
-      if (DIR > 0) {
+      if constexpr (T::S_IN_SMEM) {
+        // marching order = slots (newest+1, newest+2, newest) mod 3; the newest row is still in registers unless the
+        // stencil base did not move (first / last two rows of the mesh)
+        const Pr<AT> *p0 = ssm + (newest == 2 ? 0 : newest + 1) * SSLOT, *p1 = ssm + (newest == 0 ? 2 : newest - 1) * SSLOT;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+          S0[k] = p0[k * T::TX];
+          S1[k] = p1[k * T::TX];
+        }
+        if (!has_mov) {
+#pragma unroll
+          for (int k = 0; k < 4; ++k) S2[k] = ssm[newest * SSLOT + k * T::TX];
+        }
+        if (DIR > 0) ISLBM_YCOMB2(S0, S1, S2);
+        else ISLBM_YCOMB2(S2, S1, S0);
+      } else if (DIR > 0) {
         if (newest == 0) ISLBM_YCOMB2(S1, S2, S0);
         else if (newest == 1) ISLBM_YCOMB2(S2, S0, S1);
         else ISLBM_YCOMB2(S0, S1, S2);
@@ -227,27 +259,21 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
         else if (newest == 1) ISLBM_YCOMB2(S1, S0, S2);
         else ISLBM_YCOMB2(S2, S1, S0);
       }
-      const long long c = (long long)y * m.nxp + x;
       wf.lo[1] = y == 0 && m.wall_mlo;
       wf.hi[1] = y == m.ny - 1 && m.wall_mhi;
-      if (valid && (wall_x | wf.lo[1] | wf.hi[1])) {
-        bb_fix_all_f<2>(f, wf, src, m.nnp, c, std::make_integer_sequence<int, 8>{});
-        bb_fix_all_g<2>(g, wf, src, m.nnp, c, m, std::make_integer_sequence<int, 4>{});
-      }
+      if (valid && (wall_x | wf.lo[1] | wf.hi[1])) wall_fix_node<2>(f, g, wf, src + c, m.nnp, m);
       constexpr bool DEV = Store<ST, 2>::kBiased;   // fp32 storage: collide the deviations as they are
       collide_node<DEV>(f, g, np);
       if (valid) {
         store_node<2, DEV>(dst + c, m.nnp, f, g, spol, std::make_integer_sequence<int, 14>{});
         peer_store_node<2, ST, DEV>(m, y, x, f, g);
       }
-    } else {
-      // hand the slot back; the warp whose release is the last one refills it at once with stage s + STAGES, so
-      // STAGES - 1 stages are in flight whenever one is being consumed
-      __syncwarp();
-      if ((threadIdx.x & 31) == 0 && mbar_arrive_is_last(&empty[st]) && s + T::STAGES < nstage &&
-          atomicCAS(&claim[st], s / T::STAGES, s / T::STAGES + 1) == s / T::STAGES)
-        issue_stage2<T, DIR>(s + T::STAGES, yf, m.ny, x0, stage0, full, empty, mp, lpol);
+      c += DIR * (long long)m.nxp;
     }
+#undef PC2
+#undef PXR
+#undef PC4
+#undef PXM
   }
 }
 
@@ -264,12 +290,12 @@ struct Plan2 {
 // the two instantiated strip widths: (TX, STAGES, min CTAs/SM)
 // fp32 storage: five CTAs per SM (96 registers, 16 B spilled) measure 1-3 % above four; six (80 registers) lose 5 %
 // 128-wide strip, 3-stage ring: four CTAs per SM in fp64 (128 registers, 47 KB each), five with fp32 storage
-template <typename ST> struct Cfg2a { using T = Tile2<ST, 128, 3>; static constexpr int MINB = sizeof(ST) == 4 ? 5 : 4; };
+template <typename ST> struct Cfg2a { using T = Tile2<ST, 128, 3>; static constexpr int MINB = sizeof(ST) == 4 ? ISLBM_F32_CTAS2D : 4; };
 // 128-wide strip, fp64 only: 4-stage ring, three CTAs per SM (62 KB each): three rows in flight per CTA instead of two.
 // fp32 storage keeps the 3-stage ring (its stages are half as large; 4 and 5 stages measured 4-10 % slower).
 template <typename ST> struct Cfg2c {
   using T = Tile2<ST, 128, sizeof(ST) == 4 ? 3 : 4>;
-  static constexpr int MINB = sizeof(ST) == 4 ? 5 : 3;
+  static constexpr int MINB = sizeof(ST) == 4 ? ISLBM_F32_CTAS2D : 3;
 };
 template <typename ST> struct Cfg2b { using T = Tile2<ST, 224, 3>; static constexpr int MINB = 2; };
 

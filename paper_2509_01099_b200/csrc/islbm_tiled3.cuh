@@ -40,6 +40,10 @@ namespace islbmk {
 #define ISLBM_Z_STAGES_F32 3
 #endif
 
+#ifndef ISLBM_S_IN_SMEM
+#define ISLBM_S_IN_SMEM 1
+#endif
+
 constexpr int kMaxChunk = 64;   // longest marching chunk (its weights are staged in shared memory)
 
 template <typename ST, int TX_ = 32, int TY_ = 8>
@@ -70,7 +74,13 @@ struct Tile3 {
   static constexpr uint32_t M_BYTES = 4u * P_C + 4u * P_X + 4u * P_Y;               // planes of the z-stencil slice
   static constexpr int BAR_OFF = STAGES * STAGE_BYTES;             // full[STAGES], empty[STAGES]
   static constexpr int W_OFF = BAR_OFF + 128;                       // marching-axis weights [sign][k][kMaxChunk]
-  static constexpr size_t SMEM_BYTES = (size_t)W_OFF + 6 * kMaxChunk * 8 + 128;
+  // fp32 storage: the in-plane-interpolated values of the three z-stencil slices live in shared memory, not in
+  // registers: [slot 3][pair 6][thread] float2 (each thread reads back only what it wrote: no barrier).  The kernel is
+  // latency-bound at three warps per scheduler under a 168-register cap, and 36 registers of carried state put loop
+  // invariants into local memory on the critical path (profiles/r2_c5_256cu_f32.md)
+  static constexpr bool S_IN_SMEM = sizeof(ST) == 4 && ISLBM_S_IN_SMEM;
+  static constexpr int S_OFF = W_OFF + 6 * kMaxChunk * 8 + 128;
+  static constexpr size_t SMEM_BYTES = (size_t)S_OFF + (S_IN_SMEM ? 3 * 6 * THREADS * 8 : 0);
 };
 
 // tensor maps over (x, y, z, plane): one per box shape
@@ -89,72 +99,100 @@ struct Maps3 {
 template <typename ST> struct Acc { using type = double; };
 template <> struct Acc<float> { using type = float; };
 
-// 3-point sums in the oracle's order: ((w0*v0) + w1*v1) + w2*v2
+// A PAIR of populations of one node that share their stencil shape and differ in the sign of their velocity
+// components, e.g. (f1, f2) = (+x, -x).  The separable interpolation works on such pairs: the two
+// lanes take the same taps of two different planes with the weights of the two signs.  In fp32 a pair is one float2
+// and a tap is ONE packed instruction (fma.rn.f32x2 / mul.rn.f32x2, sm_100), which halves the fp32 instruction
+// stream of the issue-bound fp32-storage kernels; in fp64 a pair is two doubles and two scalar instructions.  Either
+// way each lane performs exactly the operations of the scalar form ((w0*v0) + w1*v1) + w2*v2, the oracle's order.
+template <typename AT> struct Pr;
+template <> struct Pr<double> { double a, b; };
+template <> struct Pr<float> { float2 v; };
+__device__ __forceinline__ Pr<double> mkpr(double a, double b) { return Pr<double>{a, b}; }
+__device__ __forceinline__ Pr<float> mkpr(float a, float b) { Pr<float> p; p.v = make_float2(a, b); return p; }
+__device__ __forceinline__ double lane_a(const Pr<double> &p) { return p.a; }
+__device__ __forceinline__ double lane_b(const Pr<double> &p) { return p.b; }
+__device__ __forceinline__ float lane_a(const Pr<float> &p) { return p.v.x; }
+__device__ __forceinline__ float lane_b(const Pr<float> &p) { return p.v.y; }
+__device__ __forceinline__ Pr<double> pmul(const Pr<double> &w, const Pr<double> &v) { return Pr<double>{w.a * v.a, w.b * v.b}; }
+__device__ __forceinline__ Pr<double> pfma(const Pr<double> &w, const Pr<double> &v, const Pr<double> &c) {
+  return Pr<double>{fma(w.a, v.a, c.a), fma(w.b, v.b, c.b)};
+}
+__device__ __forceinline__ Pr<float> pmul(const Pr<float> &w, const Pr<float> &v) { Pr<float> r; r.v = __fmul2_rn(w.v, v.v); return r; }
+__device__ __forceinline__ Pr<float> pfma(const Pr<float> &w, const Pr<float> &v, const Pr<float> &c) {
+  Pr<float> r;
+  r.v = __ffma2_rn(w.v, v.v, c.v);
+  return r;
+}
+
+// 3-point sums of a pair in the oracle's order ((w0*v0) + w1*v1) + w2*v2; pa / pb: first tap in the two planes
 template <typename ST, typename AT>
-__device__ __forceinline__ AT tap3(const ST *__restrict__ s, int stride, const AT (&w)[3]) {
-  AT a = w[0] * (AT)s[0];
-  a = fma(w[1], (AT)s[stride], a);
-  return fma(w[2], (AT)s[2 * stride], a);
+__device__ __forceinline__ Pr<AT> ptap3(const ST *__restrict__ pa, const ST *__restrict__ pb, int stride, const Pr<AT> (&w)[3]) {
+  Pr<AT> a = pmul(w[0], mkpr((AT)pa[0], (AT)pb[0]));
+  a = pfma(w[1], mkpr((AT)pa[stride], (AT)pb[stride]), a);
+  return pfma(w[2], mkpr((AT)pa[2 * stride], (AT)pb[2 * stride]), a);
 }
 template <typename ST, typename AT>
-__device__ __forceinline__ AT tap9(const ST *__restrict__ s, int pitch, const AT (&wx)[3], const AT (&wy)[3]) {
-  AT a = wy[0] * tap3(s, 1, wx);
-  a = fma(wy[1], tap3(s + pitch, 1, wx), a);
-  return fma(wy[2], tap3(s + 2 * pitch, 1, wx), a);
+__device__ __forceinline__ Pr<AT> ptap9(const ST *__restrict__ pa, const ST *__restrict__ pb, int pitch, const Pr<AT> (&wx)[3],
+                                        const Pr<AT> (&wy)[3]) {
+  Pr<AT> a = pmul(wy[0], ptap3(pa, pb, 1, wx));
+  a = pfma(wy[1], ptap3(pa + pitch, pb + pitch, 1, wx), a);
+  return pfma(wy[2], ptap3(pa + 2 * pitch, pb + 2 * pitch, 1, wx), a);
 }
 template <typename AT>
-__device__ __forceinline__ AT comb3(const AT (&w)[3], AT a, AT b, AT c) {
-  return fma(w[2], c, fma(w[1], b, w[0] * a));
+__device__ __forceinline__ Pr<AT> pcomb3(const Pr<AT> (&w)[3], const Pr<AT> &a, const Pr<AT> &b, const Pr<AT> &c) {
+  return pfma(w[2], c, pfma(w[1], b, pmul(w[0], a)));
 }
 
 struct WallFlags {
   bool lo[3], hi[3];
 };
 
-// Eq. 21: a flow population whose departure point lies beyond a wall takes the node's own
-// opposite post-collision value (storage form: the deviation, same lattice weight as its opposite).
+// Eq. 21: a flow population whose departure point lies beyond a wall takes the node's own opposite
+// post-collision value (storage form: the deviation, same lattice weight as its opposite); Eq. 22 (isothermal x-walls)
+// and Eq. 23 (adiabatic walls), for the temperature populations.  One call fixes the populations that
+// cross ONE wall (AXIS, SIGN = +1: the low wall, crossed by e_AXIS = +1; -1: the high wall); a node on an edge or in a
+// corner is fixed once per wall it touches, and a diagonal population that crosses two walls is loaded twice with the
+// same value (A4: bounce back as soon as any component crosses).  sc = src + node index.
 // The wall reads are coherent loads (ld.global.cg), not ld.global.nc: with programmatic dependent launch step t+1 is
 // resident while step t still writes the buffer these loads read, so the data is not read-only for the kernel's
 // lifetime (the loads themselves come after griddepcontrol.wait).
-template <int DIM, int Q, typename ST, typename NT>
-__device__ __forceinline__ void bb_fix_f(NT &v, const WallFlags &wf, const ST *__restrict__ src, long long nn,
-                                         long long c) {
-  constexpr int EX = evel<DIM>(Q, 0), EY = evel<DIM>(Q, 1), EZ = evel<DIM>(Q, 2);
-  bool cross = false;
-  if (EX == 1) cross |= wf.lo[0];
-  if (EX == -1) cross |= wf.hi[0];
-  if (EY == 1) cross |= wf.lo[1];
-  if (EY == -1) cross |= wf.hi[1];
-  if (DIM == 3 && EZ == 1) cross |= wf.lo[2];
-  if (DIM == 3 && EZ == -1) cross |= wf.hi[2];
-  if (cross) v = (NT)ld_coherent(src + (long long)plane_f<DIM>(opposite<DIM>(Q)) * nn + c);
+template <int DIM, int AXIS, int SIGN, int Q, typename ST, typename NT>
+__device__ __forceinline__ void wall_fix_f1(NT *f, const ST *__restrict__ sc, long long nn) {
+  if constexpr (evel<DIM>(Q, AXIS) == SIGN) f[Q] = (NT)ld_coherent(sc + (long long)plane_f<DIM>(opposite<DIM>(Q)) * nn);
 }
-// Eq. 22 (isothermal x-walls) and Eq. 23 (adiabatic walls)
-template <int DIM, int Q, typename ST, typename NT>
-__device__ __forceinline__ void bb_fix_g(NT &v, const WallFlags &wf, const ST *__restrict__ src, long long nn,
-                                         long long c, const DevMesh &m) {
-  constexpr int EX = evel<DIM>(Q, 0), EY = evel<DIM>(Q, 1), EZ = evel<DIM>(Q, 2);
-  constexpr int A = EX != 0 ? 0 : (EY != 0 ? 1 : 2);
-  constexpr int S = EX + EY + EZ;
-  const bool cross = S == 1 ? wf.lo[A] : wf.hi[A];
-  if (cross) {
-    const double gb = (double)ld_coherent(src + (long long)plane_g<DIM>(opposite<DIM>(Q)) * nn + c);
-    v = (NT)(A == 0 ? -gb + m.omega_bc * (wf.lo[0] ? m.T_hot : m.T_cold) : gb);
+template <int DIM, int AXIS, int SIGN, int Q, typename ST, typename NT>
+__device__ __forceinline__ void wall_fix_g1(NT *g, const ST *__restrict__ sc, long long nn, const DevMesh &m) {
+  if constexpr (evel<DIM>(Q, AXIS) == SIGN) {
+    const double gb = (double)ld_coherent(sc + (long long)plane_g<DIM>(opposite<DIM>(Q)) * nn);
+    g[Q] = (NT)(AXIS == 0 ? -gb + m.omega_bc * (SIGN > 0 ? m.T_hot : m.T_cold) : gb);
   }
 }
-template <int DIM, typename ST, typename NT, int... Qs>
-__device__ __forceinline__ void bb_fix_all_f(NT *f, const WallFlags &wf, const ST *src, long long nn, long long c,
-                                             std::integer_sequence<int, Qs...>) {
-  (bb_fix_f<DIM, Qs + 1>(f[Qs + 1], wf, src, nn, c), ...);
+template <int DIM, int AXIS, int SIGN, typename ST, typename NT, int... Qf, int... Qg>
+__device__ __forceinline__ void wall_fix(NT *f, NT *g, const ST *__restrict__ sc, long long nn, const DevMesh &m,
+                                         std::integer_sequence<int, Qf...>, std::integer_sequence<int, Qg...>) {
+  (wall_fix_f1<DIM, AXIS, SIGN, Qf + 1>(f, sc, nn), ...);
+  (wall_fix_g1<DIM, AXIS, SIGN, Qg + 1>(g, sc, nn, m), ...);
 }
-template <int DIM, typename ST, typename NT, int... Qs>
-__device__ __forceinline__ void bb_fix_all_g(NT *g, const WallFlags &wf, const ST *src, long long nn, long long c,
-                                             const DevMesh &m, std::integer_sequence<int, Qs...>) {
-  (bb_fix_g<DIM, Qs + 1>(g[Qs + 1], wf, src, nn, c, m), ...);
+template <int DIM, typename ST, typename NT>
+__device__ __forceinline__ void wall_fix_node(NT *f, NT *g, const WallFlags &wf, const ST *__restrict__ sc, long long nn,
+                                              const DevMesh &m) {
+  using QF = std::make_integer_sequence<int, Lat<DIM>::QF - 1>;
+  using QG = std::make_integer_sequence<int, Lat<DIM>::QG - 1>;
+  if (wf.lo[0]) wall_fix<DIM, 0, 1>(f, g, sc, nn, m, QF{}, QG{});
+  if (wf.hi[0]) wall_fix<DIM, 0, -1>(f, g, sc, nn, m, QF{}, QG{});
+  if (wf.lo[1]) wall_fix<DIM, 1, 1>(f, g, sc, nn, m, QF{}, QG{});
+  if (wf.hi[1]) wall_fix<DIM, 1, -1>(f, g, sc, nn, m, QF{}, QG{});
+  if constexpr (DIM == 3) {
+    if (wf.lo[2]) wall_fix<DIM, 2, 1>(f, g, sc, nn, m, QF{}, QG{});
+    if (wf.hi[2]) wall_fix<DIM, 2, -1>(f, g, sc, nn, m, QF{}, QG{});
+  }
 }
 
 // store the node's populations plane by plane in storage order.  The pointer is walked by the plane pitch and made
-// opaque after each step, so that ptxas keeps two integer adds per plane instead of a 64-bit multiply-add
+// opaque after each step, so that ptxas keeps two integer adds per plane (a 64-bit address per plane is the floor: STG
+// takes no uniform-base + 32-bit-offset form, and a 32 x 32 -> 64-bit multiply-add per plane compiles to 2.6
+// instructions, measured: profiles/attempts.md)
 template <int DIM, int P, bool DEV, typename ST, typename NT>
 __device__ __forceinline__ void store_plane(ST *&p, long long nn, const NT *f, const NT *g, uint64_t spol) {
   constexpr int QF = Lat<DIM>::QF;
@@ -171,6 +209,8 @@ __device__ __forceinline__ void store_node(ST *p, long long nn, const NT *f, con
 }
 
 __device__ __forceinline__ int sbase(int j, int n) { return min(max(j - 1, 0), n - 3); }
+// does the stencil base move from layer j-1 to layer j?  (sbase(j) != sbase(j-1)  <=>  2 <= j <= n-2)
+__device__ __forceinline__ bool sbase_moves(int j, int n) { return j >= 2 && j <= n - 2; }
 
 // One pipeline stage = the TMA boxes one z-iteration needs.  Issued by one thread.
 //   stage s < 2 : the first two slices of the z-stencil of the chunk's first slice;
@@ -184,7 +224,7 @@ __device__ __forceinline__ void issue_stage3(int s, int z0, int nz, int x0, int 
     mslice = sbase(z0, nz) + s;
   } else {
     zslice = z0 + (s - 2);
-    if (s == 2 || sbase(zslice, nz) != sbase(zslice - 1, nz)) mslice = sbase(zslice, nz) + 2;
+    if (s == 2 || sbase_moves(zslice, nz)) mslice = sbase(zslice, nz) + 2;
   }
   mbar_expect_tx(&full[st], (mslice >= 0 ? T::M_BYTES : 0u) + (zslice >= 0 ? T::Z_BYTES : 0u));
   unsigned char *sb = stage0 + (size_t)st * T::STAGE_BYTES;
@@ -203,39 +243,61 @@ __device__ __forceinline__ void issue_stage3(int s, int z0, int nz, int x0, int 
   }
 }
 
+// marching-axis weights of one layer as pairs: N = (weight of c=+1, weight of c=-1), S = the two swapped.
+// fp64: the chunk's weights sit in shared memory as scalars [sign][k][kMaxChunk] (a pair is just two registers);
+// fp32: both forms sit there as float2 [form][k][kMaxChunk], one 64-bit load each.
+__device__ __forceinline__ void stage_march_weight(double *ws, int sk, int i, double w) { ws[sk * kMaxChunk + i] = w; }
+__device__ __forceinline__ void stage_march_weight(float *ws, int sk, int i, double w) {
+  // sk = sign * 3 + k; lane a of N[k] and lane b of S[k] take sign 1, the other two lanes sign 0
+  const int sign = sk / 3, k = sk - 3 * sign;
+  ws[((0 * 3 + k) * kMaxChunk + i) * 2 + (sign ? 0 : 1)] = (float)w;
+  ws[((1 * 3 + k) * kMaxChunk + i) * 2 + (sign ? 1 : 0)] = (float)w;
+}
+__device__ __forceinline__ void load_march_weights(const double *ws, int i, Pr<double> (&N)[3], Pr<double> (&S)[3]) {
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    const double w1 = ws[(3 + k) * kMaxChunk + i], w0 = ws[k * kMaxChunk + i];
+    N[k] = mkpr(w1, w0);
+    S[k] = mkpr(w0, w1);
+  }
+}
+__device__ __forceinline__ void load_march_weights(const float *ws, int i, Pr<float> (&N)[3], Pr<float> (&S)[3]) {
+  const float2 *w2 = reinterpret_cast<const float2 *>(ws);
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    N[k].v = w2[k * kMaxChunk + i];
+    S[k].v = w2[(3 + k) * kMaxChunk + i];
+  }
+}
+
 // ------------------------------ the kernel --------------------------------
-// in-plane-interpolated values of one z-stencil slice for the 12 populations with e_z != 0:
-//   index: 0 f5, 1 f6, 2..5 f11..f14, 6..9 f15..f18, 10 g5, 11 g6
-#define ISLBM_LOAD_M3(S)                                        \
-  do {                                                          \
-    S[0] = (AT)PC4(0)[o_c];                     /* f5 */        \
-    S[1] = (AT)PC4(1)[o_c];                     /* f6 */        \
-    S[2] = tap3(PXM(0) + o_x, 1, wx[1]);        /* f11 ( 1,0, 1) */ \
-    S[3] = tap3(PXM(1) + o_x, 1, wx[0]);        /* f12 (-1,0, 1) */ \
-    S[4] = tap3(PXM(2) + o_x, 1, wx[1]);        /* f13 ( 1,0,-1) */ \
-    S[5] = tap3(PXM(3) + o_x, 1, wx[0]);        /* f14 (-1,0,-1) */ \
-    S[6] = tap3(PYM(0) + o_y, T::TX, wy[1]);    /* f15 (0, 1, 1) */ \
-    S[7] = tap3(PYM(1) + o_y, T::TX, wy[0]);    /* f16 (0,-1, 1) */ \
-    S[8] = tap3(PYM(2) + o_y, T::TX, wy[1]);    /* f17 (0, 1,-1) */ \
-    S[9] = tap3(PYM(3) + o_y, T::TX, wy[0]);    /* f18 (0,-1,-1) */ \
-    S[10] = (AT)PC4(2)[o_c];                    /* g5 */        \
-    S[11] = (AT)PC4(3)[o_c];                    /* g6 */        \
+// in-plane-interpolated values of one z-stencil slice for the 12 populations with e_z != 0, as 6 pairs:
+//   0 (f5, f6)  1 (g5, g6)  2 (f11, f14)  3 (f13, f12)  4 (f15, f18)  5 (f17, f16)
+// (lane a has e_z = +1 in pairs 0, 1, 2, 4 and e_z = -1 in pairs 3 and 5, which take the swapped z-weights)
+#define ISLBM_LOAD_M3(S)                                                                     \
+  do {                                                                                       \
+    S[0] = mkpr((AT)PC4(0)[0], (AT)PC4(1)[0]);              /* f5, f6 */             \
+    S[1] = mkpr((AT)PC4(2)[0], (AT)PC4(3)[0]);              /* g5, g6 */             \
+    S[2] = ptap3(PXM(0), PXM(3), 1, wxN);                   /* f11 (+x), f14 (-x) */ \
+    S[3] = ptap3(PXM(2), PXM(1), 1, wxN);                   /* f13 (+x), f12 (-x) */ \
+    S[4] = ptap3(PYM(0), PYM(3), T::TX, wyN);               /* f15 (+y), f18 (-y) */ \
+    S[5] = ptap3(PYM(2), PYM(1), T::TX, wyN);               /* f17 (+y), f16 (-y) */ \
   } while (0)
 // z-direction of the separable interpolation; (P0,P1,P2) = stencil slices in ascending z
-#define ISLBM_ZCOMB3(P0, P1, P2)                  \
-  do {                                            \
-    f[5] = comb3(wz[1], P0[0], P1[0], P2[0]);     \
-    f[6] = comb3(wz[0], P0[1], P1[1], P2[1]);     \
-    f[11] = comb3(wz[1], P0[2], P1[2], P2[2]);    \
-    f[12] = comb3(wz[1], P0[3], P1[3], P2[3]);    \
-    f[13] = comb3(wz[0], P0[4], P1[4], P2[4]);    \
-    f[14] = comb3(wz[0], P0[5], P1[5], P2[5]);    \
-    f[15] = comb3(wz[1], P0[6], P1[6], P2[6]);    \
-    f[16] = comb3(wz[1], P0[7], P1[7], P2[7]);    \
-    f[17] = comb3(wz[0], P0[8], P1[8], P2[8]);    \
-    f[18] = comb3(wz[0], P0[9], P1[9], P2[9]);    \
-    g[5] = comb3(wz[1], P0[10], P1[10], P2[10]);  \
-    g[6] = comb3(wz[0], P0[11], P1[11], P2[11]);  \
+#define ISLBM_ZCOMB3(P0, P1, P2)                                     \
+  do {                                                               \
+    const Pr<AT> q0 = pcomb3(wzN, P0[0], P1[0], P2[0]);              \
+    const Pr<AT> q1 = pcomb3(wzN, P0[1], P1[1], P2[1]);              \
+    const Pr<AT> q2 = pcomb3(wzN, P0[2], P1[2], P2[2]);              \
+    const Pr<AT> q3 = pcomb3(wzS, P0[3], P1[3], P2[3]);              \
+    const Pr<AT> q4 = pcomb3(wzN, P0[4], P1[4], P2[4]);              \
+    const Pr<AT> q5 = pcomb3(wzS, P0[5], P1[5], P2[5]);              \
+    f[5] = lane_a(q0);  f[6] = lane_b(q0);                           \
+    g[5] = lane_a(q1);  g[6] = lane_b(q1);                           \
+    f[11] = lane_a(q2); f[14] = lane_b(q2);                          \
+    f[13] = lane_a(q3); f[12] = lane_b(q3);                          \
+    f[15] = lane_a(q4); f[18] = lane_b(q4);                          \
+    f[17] = lane_a(q5); f[16] = lane_b(q5);                          \
   } while (0)
 
 template <typename ST, int TX, int TY>
@@ -288,7 +350,7 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
   }
   for (int i = (int)threadIdx.x - 32; i >= 0 && i < 6 * (z1 - z0); i += T::THREADS - 32) {   // warps 1..: warp 0 is waiting above
     const int sk = i / (z1 - z0), zi = i - sk * (z1 - z0);
-    wzs[sk * kMaxChunk + zi] = (AT)__ldg(wrow(m, 2, sk / 3, sk % 3) + z0 + zi);
+    stage_march_weight(wzs, sk, zi, __ldg(wrow(m, 2, sk / 3, sk % 3) + z0 + zi));
   }
   pdl_wait();
   __syncthreads();
@@ -306,42 +368,53 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
   const bool wall_xy = wf.lo[0] | wf.hi[0] | wf.lo[1] | wf.hi[1];
   const int sx = wf.lo[0] ? 1 : (wf.hi[0] ? -1 : 0);
   const int sy = wf.lo[1] ? 1 : (wf.hi[1] ? -1 : 0);
-  // per-thread element offsets inside the four box shapes
-  const int o_xy = (ty + sy) * T::HX + (tx + T::XH - 1 + sx);    // 3x3 stencil, pitch HX
-  const int o_x = ty * T::HX + (tx + T::XH - 1 + sx);            // x-stencil, taps +0,+1,+2
-  const int o_y = (ty + sy) * T::TX + tx;                        // y-stencil, taps +0,+TX,+2TX
-  const int o_c = ty * T::TX + tx;
-  AT wx[2][3], wy[2][3];
+  // per-thread element offsets inside the four box shapes.  Made opaque so that they stay in registers: under
+  // register pressure the compiler otherwise re-derives them from threadIdx in every iteration (~40 instructions)
+  int o_xy = (ty + sy) * T::HX + (tx + T::XH - 1 + sx);    // 3x3 stencil, pitch HX
+  int o_x = ty * T::HX + (tx + T::XH - 1 + sx);            // x-stencil, taps +0,+1,+2
+  int o_y = (ty + sy) * T::TX + tx;                        // y-stencil, taps +0,+TX,+2TX
+  int o_c = ty * T::TX + tx;
+#ifdef ISLBM_OPAQUE_OFFSETS
+  asm volatile("" : "+r"(o_xy), "+r"(o_x), "+r"(o_y), "+r"(o_c));
+#endif
+  // weights of the two signs as pairs: N = (c = +1, c = -1), S = swapped
+  Pr<AT> wxN[3], wyN[3], wyS[3];
 #pragma unroll
-  for (int s = 0; s < 2; ++s)
-#pragma unroll
-    for (int k = 0; k < 3; ++k) {
-      wx[s][k] = valid ? (AT)__ldg(wrow(m, 0, s, k) + x) : (AT)0;
-      wy[s][k] = valid ? (AT)__ldg(wrow(m, 1, s, k) + y) : (AT)0;
-    }
+  for (int k = 0; k < 3; ++k) {
+    const AT x1 = valid ? (AT)__ldg(wrow(m, 0, 1, k) + x) : (AT)0, x0w = valid ? (AT)__ldg(wrow(m, 0, 0, k) + x) : (AT)0;
+    const AT y1 = valid ? (AT)__ldg(wrow(m, 1, 1, k) + y) : (AT)0, y0w = valid ? (AT)__ldg(wrow(m, 1, 0, k) + y) : (AT)0;
+    wxN[k] = mkpr(x1, x0w);
+    wyN[k] = mkpr(y1, y0w);
+    wyS[k] = mkpr(y0w, y1);
+  }
   const long long plane = (long long)m.nxp * m.ny;
-  const long long cxy = (long long)y * m.nxp + x;
+  // the node's index in plane 0 at the chunk's first slice; advanced by one slice per emitted slice
+  long long c = (long long)z0 * plane + (long long)y * m.nxp + x;
 
   // three register sets hold the z-stencil slices; `newest` names the one written last, so the ascending-z
   // order is (newest+1, newest+2, newest) mod 3 and nothing is ever copied between sets
-  AT S0[12], S1[12], S2[12];
+  Pr<AT> S0[6], S1[6], S2[6];
   int newest = 2;
+  Pr<AT> *ssm = reinterpret_cast<Pr<AT> *>(smem_raw + T::S_OFF) + threadIdx.x;   // S_IN_SMEM: [slot][pair][thread]
+  constexpr int SSLOT = 6 * T::THREADS;
 
 #pragma unroll 1
   for (int s = 0; s < nstage; ++s) {
-    const int st = s % T::STAGES;
+    const int st = s % T::STAGES;     // warp-uniform: these live on the uniform datapath, not in vector registers
     const uint32_t ph = (uint32_t)(s / T::STAGES) & 1u;
     const int z = z0 + (s - 2);
     const bool has_emit = s >= 2;
-    const bool has_mov = s <= 2 || sbase(z, m.nz) != sbase(z - 1, m.nz);
-    const unsigned char *sb = stage0 + (size_t)st * T::STAGE_BYTES;
-    auto PC2 = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_C2 + k * T::P_C); };
-    auto PXZ = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_XZ + k * T::P_X); };
-    auto PYZ = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_YZ + k * T::P_Y); };
-    auto PXY = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_XY + k * T::P_XY); };
-    auto PC4 = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_C4 + k * T::P_C); };
-    auto PXM = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_XM + k * T::P_X); };
-    auto PYM = [&](int k) { return reinterpret_cast<const ST *>(sb + T::OFF_YM + k * T::P_Y); };
+    const bool has_mov = s <= 2 || sbase_moves(z, m.nz);
+    const ST *sb = reinterpret_cast<const ST *>(stage0 + (size_t)st * T::STAGE_BYTES);
+    const ST *sbc = sb + o_c, *sbx = sb + o_x, *sby = sb + o_y, *sbxy = sb + o_xy;
+    constexpr int ES = (int)sizeof(ST);
+#define PC2(k) (sbc + (T::OFF_C2 + (k) * T::P_C) / ES)
+#define PXZ(k) (sbx + (T::OFF_XZ + (k) * T::P_X) / ES)
+#define PYZ(k) (sby + (T::OFF_YZ + (k) * T::P_Y) / ES)
+#define PXY(k) (sbxy + (T::OFF_XY + (k) * T::P_XY) / ES)
+#define PC4(k) (sbc + (T::OFF_C4 + (k) * T::P_C) / ES)
+#define PXM(k) (sbx + (T::OFF_XM + (k) * T::P_X) / ES)
+#define PYM(k) (sby + (T::OFF_YM + (k) * T::P_Y) / ES)
     if (!EARLY && threadIdx.x == 0 && s + T::STAGES - 1 < nstage) {
       const int sn = s + T::STAGES - 1;
       if (sn >= T::STAGES) mbar_wait(&empty[sn % T::STAGES], ((uint32_t)(sn / T::STAGES) & 1u) ^ 1u);
@@ -352,67 +425,84 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
 
     if (has_mov) {
       newest = newest == 2 ? 0 : newest + 1;
-      if (newest == 0) ISLBM_LOAD_M3(S0);
-      else if (newest == 1) ISLBM_LOAD_M3(S1);
-      else ISLBM_LOAD_M3(S2);
+      if constexpr (T::S_IN_SMEM) {
+        ISLBM_LOAD_M3(S2);       // S2 = the newest slice, in registers for this iteration and in its shared-memory slot
+#pragma unroll
+        for (int k = 0; k < 6; ++k) ssm[newest * SSLOT + k * T::THREADS] = S2[k];
+      } else {
+        if (newest == 0) ISLBM_LOAD_M3(S0);
+        else if (newest == 1) ISLBM_LOAD_M3(S1);
+        else ISLBM_LOAD_M3(S2);
+      }
+    }
+
+    AT f[19], g[7];   // fp64, or fp32 deviations (fp32 storage)
+    if (has_emit) {
+      f[0] = PC2(0)[0];
+      g[0] = PC2(1)[0];
+      const Pr<AT> p1 = ptap3(PXZ(0), PXZ(1), 1, wxN);               // f1 (+x), f2 (-x)
+      const Pr<AT> p2 = ptap3(PXZ(2), PXZ(3), 1, wxN);               // g1, g2
+      const Pr<AT> p3 = ptap3(PYZ(0), PYZ(1), T::TX, wyN);           // f3 (+y), f4 (-y)
+      const Pr<AT> p4 = ptap3(PYZ(2), PYZ(3), T::TX, wyN);           // g3, g4
+      const Pr<AT> p5 = ptap9(PXY(0), PXY(3), T::HX, wxN, wyN);      // f7 (+x,+y), f10 (-x,-y)
+      const Pr<AT> p6 = ptap9(PXY(2), PXY(1), T::HX, wxN, wyS);      // f9 (+x,-y), f8 (-x,+y)
+      f[1] = lane_a(p1); f[2] = lane_b(p1);
+      g[1] = lane_a(p2); g[2] = lane_b(p2);
+      f[3] = lane_a(p3); f[4] = lane_b(p3);
+      g[3] = lane_a(p4); g[4] = lane_b(p4);
+      f[7] = lane_a(p5); f[10] = lane_b(p5);
+      f[9] = lane_a(p6); f[8] = lane_b(p6);
+    }
+    // all shared-memory reads of this stage are done: hand the slot back to the producer (EARLY: the warp whose
+    // release is the last one refills it at once with stage s + STAGES)
+    __syncwarp();
+    if ((threadIdx.x & 31) == 0) {
+      if (!EARLY) mbar_arrive(&empty[st]);
+      else if (mbar_arrive_is_last(&empty[st]) && s + T::STAGES < nstage &&
+               atomicCAS(&claim[st], s / T::STAGES, s / T::STAGES + 1) == s / T::STAGES)
+        issue_stage3<T>(s + T::STAGES, z0, m.nz, x0, y0, stage0, full, empty, mp, lpol);
     }
 
     if (has_emit) {
-      AT wz[2][3];
+      Pr<AT> wzN[3], wzS[3];
+      load_march_weights(wzs, s - 2, wzN, wzS);
+      if constexpr (T::S_IN_SMEM) {
+        // ascending z = slots (newest+1, newest+2, newest) mod 3; the newest slice is still in registers unless the
+        // stencil base did not move (first / last two slices of the mesh)
+        const Pr<AT> *p0 = ssm + (newest == 2 ? 0 : newest + 1) * SSLOT, *p1 = ssm + (newest == 0 ? 2 : newest - 1) * SSLOT;
 #pragma unroll
-      for (int sg = 0; sg < 2; ++sg)
+        for (int k = 0; k < 6; ++k) {
+          S0[k] = p0[k * T::THREADS];
+          S1[k] = p1[k * T::THREADS];
+        }
+        if (!has_mov) {
 #pragma unroll
-        for (int k = 0; k < 3; ++k) wz[sg][k] = wzs[(sg * 3 + k) * kMaxChunk + (s - 2)];
-      AT f[19], g[7];   // fp64, or fp32 deviations (fp32 storage)
-      f[0] = PC2(0)[o_c];
-      g[0] = PC2(1)[o_c];
-      f[1] = tap3(PXZ(0) + o_x, 1, wx[1]);
-      f[2] = tap3(PXZ(1) + o_x, 1, wx[0]);
-      g[1] = tap3(PXZ(2) + o_x, 1, wx[1]);
-      g[2] = tap3(PXZ(3) + o_x, 1, wx[0]);
-      f[3] = tap3(PYZ(0) + o_y, T::TX, wy[1]);
-      f[4] = tap3(PYZ(1) + o_y, T::TX, wy[0]);
-      g[3] = tap3(PYZ(2) + o_y, T::TX, wy[1]);
-      g[4] = tap3(PYZ(3) + o_y, T::TX, wy[0]);
-      f[7] = tap9(PXY(0) + o_xy, T::HX, wx[1], wy[1]);
-      f[8] = tap9(PXY(1) + o_xy, T::HX, wx[0], wy[1]);
-      f[9] = tap9(PXY(2) + o_xy, T::HX, wx[1], wy[0]);
-      f[10] = tap9(PXY(3) + o_xy, T::HX, wx[0], wy[0]);
-      // all shared-memory reads of this stage are done: hand the slot back to the producer
-      // hand the slot back (EARLY: the warp whose release is the last one refills it at once with stage s + STAGES)
-      __syncwarp();
-      if ((threadIdx.x & 31) == 0) {
-        if (!EARLY) mbar_arrive(&empty[st]);
-        else if (mbar_arrive_is_last(&empty[st]) && s + T::STAGES < nstage &&
-                 atomicCAS(&claim[st], s / T::STAGES, s / T::STAGES + 1) == s / T::STAGES)
-          issue_stage3<T>(s + T::STAGES, z0, m.nz, x0, y0, stage0, full, empty, mp, lpol);
+          for (int k = 0; k < 6; ++k) S2[k] = ssm[newest * SSLOT + k * T::THREADS];
+        }
+        ISLBM_ZCOMB3(S0, S1, S2);
+      } else {
+        if (newest == 0) ISLBM_ZCOMB3(S1, S2, S0);
+        else if (newest == 1) ISLBM_ZCOMB3(S2, S0, S1);
+        else ISLBM_ZCOMB3(S0, S1, S2);
       }
-      if (newest == 0) ISLBM_ZCOMB3(S1, S2, S0);
-      else if (newest == 1) ISLBM_ZCOMB3(S2, S0, S1);
-      else ISLBM_ZCOMB3(S0, S1, S2);
-      const long long c = (long long)z * plane + cxy;
       wf.lo[2] = z == 0 && m.wall_mlo;
       wf.hi[2] = z == m.nz - 1 && m.wall_mhi;
-      if (valid && (wall_xy | wf.lo[2] | wf.hi[2])) {
-        bb_fix_all_f<3>(f, wf, src, m.nnp, c, std::make_integer_sequence<int, 18>{});
-        bb_fix_all_g<3>(g, wf, src, m.nnp, c, m, std::make_integer_sequence<int, 6>{});
-      }
+      if (valid && (wall_xy | wf.lo[2] | wf.hi[2])) wall_fix_node<3>(f, g, wf, src + c, m.nnp, m);
       constexpr bool DEV = Store<ST, 3>::kBiased;   // fp32 storage: collide the deviations as they are
       collide_node<DEV>(f, g, np);
       if (valid) {
         store_node<3, DEV>(dst + c, m.nnp, f, g, spol, std::make_integer_sequence<int, 26>{});
-        peer_store_node<3, ST, DEV>(m, z, cxy, f, g);
+        peer_store_node<3, ST, DEV>(m, z, c - (long long)z * plane, f, g);
       }
-    } else {
-      // hand the slot back (EARLY: the warp whose release is the last one refills it at once with stage s + STAGES)
-      __syncwarp();
-      if ((threadIdx.x & 31) == 0) {
-        if (!EARLY) mbar_arrive(&empty[st]);
-        else if (mbar_arrive_is_last(&empty[st]) && s + T::STAGES < nstage &&
-                 atomicCAS(&claim[st], s / T::STAGES, s / T::STAGES + 1) == s / T::STAGES)
-          issue_stage3<T>(s + T::STAGES, z0, m.nz, x0, y0, stage0, full, empty, mp, lpol);
-      }
+      c += plane;
     }
+#undef PC2
+#undef PXZ
+#undef PYZ
+#undef PXY
+#undef PC4
+#undef PXM
+#undef PYM
   }
 }
 
@@ -491,6 +581,36 @@ inline void launch3_shape(const Plan3 &p, const int *n, const DevMesh &m, const 
   dim3 grid((n[0] + T::TX - 1) / T::TX, (n[1] + T::TY - 1) / T::TY, (m.em_hi - m.em_lo + p.zchunk - 1) / p.zchunk);
   launch_step(k_step_zmarch<ST, TX, TY>, grid, dim3(T::THREADS), T::SMEM_BYTES, stream, tn.pdl != 0, p.maps[cur], m, np,
               (const ST *)buf[cur], (ST *)buf[1 - cur], p.zchunk, tn.load_policy, tn.store_policy, tn.fill == 2 ? 1 : 0);
+}
+
+template <typename ST>
+inline bool plan3_create(Plan3 &p, const int *n, int nxp, void *buf0, void *buf1, const Tuning &tn) {
+  // tile shape (x by y nodes per CTA).  fp64 storage: 32x8 (254 registers, one CTA per SM; DRAM-bound).  fp32 storage
+  // is bound by instruction issue and latency at 8 warps per SM, so it takes smaller CTAs, capped at 168 registers by
+  // their launch bounds: 32x6 (two CTAs = 12 warps per SM) or 32x4 (three CTAs) on short y-axes (profiles/attempts.md).
+  int shape = tn.shape3d;
+  if (shape == 0) shape = sizeof(ST) == 4 ? (n[1] >= 192 ? 3 : 4) : 5;
+  p.shape = shape;
+  switch (shape) {
+    case 1: return plan3_setup<ST, 64, 4>(p, n, nxp, buf0, buf1, tn);
+    case 2: return plan3_setup<ST, 128, 2>(p, n, nxp, buf0, buf1, tn);
+    case 3: return plan3_setup<ST, 32, 6>(p, n, nxp, buf0, buf1, tn);
+    case 4: return plan3_setup<ST, 32, 4>(p, n, nxp, buf0, buf1, tn);
+    default: p.shape = 5; return plan3_setup<ST, 32, 8>(p, n, nxp, buf0, buf1, tn);
+  }
+}
+
+template <typename ST>
+inline cudaError_t launch3(const Plan3 &p, const int *n, const DevMesh &m, const NodeParams &np, int cur, void *const *buf,
+                           const Tuning &tn, cudaStream_t stream) {
+  switch (p.shape) {
+    case 1: launch3_shape<ST, 64, 4>(p, n, m, np, cur, buf, tn, stream); break;
+    case 2: launch3_shape<ST, 128, 2>(p, n, m, np, cur, buf, tn, stream); break;
+    case 3: launch3_shape<ST, 32, 6>(p, n, m, np, cur, buf, tn, stream); break;
+    case 4: launch3_shape<ST, 32, 4>(p, n, m, np, cur, buf, tn, stream); break;
+    default: launch3_shape<ST, 32, 8>(p, n, m, np, cur, buf, tn, stream);
+  }
+  return cudaPeekAtLastError();
 }
 
 }  // namespace islbmk

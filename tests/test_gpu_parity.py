@@ -88,9 +88,6 @@ def kernels_for(islbm, sim):
                     ks.append((islbm.KERNEL_TILED, tune))
                 except islbm.IslbmError:
                     pass
-            if sim.precision == 1 and sim.n[0] % 2 == 0:                  # two nodes per thread (fp32 storage, even nx)
-                ks += [(islbm.KERNEL_TILED, dict(shape3d=6)), (islbm.KERNEL_TILED, dict(shape3d=7, chunk=5, fill=2)),
-                       (islbm.KERNEL_TILED, dict(shape3d=8, chunk=2, pdl=0))]
             sim.set_tuning(**DEFAULT_TUNING)
         if sim.dim == 2:
             ks.append((islbm.KERNEL_TILED, dict(tx2d=128, chunk=7, serpentine=1)))
@@ -201,26 +198,6 @@ def test_fp32_storage_every_kernel_three_steps(islbm, dim, ns, st):
         f3, g3 = sim.get_populations()
         ef, eg = plane_err(f3.cpu().numpy(), fo), plane_err(g3.cpu().numpy(), go)
         assert ef <= 2e-6 and eg <= 2e-6, (sim.kernel_name, tune, ef, eg)
-
-
-@pytest.mark.parametrize("ns", [(4, 3, 3), (36, 18, 9), (66, 10, 35), (64, 24, 40), (130, 7, 12), (96, 50, 33)])
-def test_fp32_pair_kernels_equal_the_one_node_kernel_bitwise(islbm, ns):
-    """The two-nodes-per-thread fp32-storage kernels (packed fma.rn.f32x2, islbm_pair.cuh) perform, lane by lane, the
-    operations of the one-node kernel in the same order: identical bits after 5 steps, every pair tile shape."""
-    coords, delta = ragged_coords(3, ns, (1.4, 1.2, 1.3))
-    H_lu = (coords[1][-1] - coords[1][0] + delta) / delta
-    sim = islbm.Islbm(coords, delta, 0.71 * (0.1 * H_lu / 0.03) ** 2, 0.71, 0.1 * SQ3, precision=1)
-    f0, g0 = inputs.random_state(sim.shape, sim.qf, sim.qg, seed=23, amp=0.05)
-    f0, g0 = torch.from_numpy(f0).cuda(), torch.from_numpy(g0).cuda()
-    out = {}
-    for shape in (3, 6, 7, 8):
-        sim.set_tuning(**{**DEFAULT_TUNING, "shape3d": shape})
-        sim.set_kernel(islbm.KERNEL_TILED)
-        sim.set_populations(f0, g0)
-        sim.step(5)
-        out[shape] = sim.get_populations()
-    for shape in (6, 7, 8):
-        assert torch.equal(out[shape][0], out[3][0]) and torch.equal(out[shape][1], out[3][1]), shape
 
 
 @pytest.mark.parametrize("dim,ns,prec", [(2, (70, 45, 1), 0), (3, (37, 21, 19), 0), (3, (33, 17, 9), 1), (2, (3, 3, 1), 0)])
