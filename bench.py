@@ -229,7 +229,7 @@ def time_device(sim, nodes, steps, warmup, lbm_per_step, flush=None):
     in_step = sum(ev[1 + 2 * k].elapsed_time(ev[2 + 2 * k]) for k in range(steps)) * 1e-3
     # time averages over the timed window (BASELINE.json config 3; A20: plain mean of the samples)
     nu = dict(nu, Nu_hot_mean=sum(n["Nu_hot"] for n in nus) / len(nus), Re_mean=sum(n["Re"] for n in nus) / len(nus),
-              samples=len(nus))
+              u2_mean=sum(n["u2"] for n in nus) / len(nus), samples=len(nus))
     return total, in_step, sim.launch_count - l0, nu
 
 
@@ -273,6 +273,7 @@ def measure_workload(islbm, inputs, name, precision, steps, warmup, lbm_per_step
         "wctpdt_s": (total / (steps * lbm_per_step)) * p["H_lu"] / p["U"],
         "kernel": sim.kernel_name, "launches": launches, "Nu_hot": nu["Nu_hot"], "Re": nu["Re"],
         "Nu_hot_mean": nu["Nu_hot_mean"], "Re_mean": nu["Re_mean"], "nu_samples": nu["samples"],
+        "Re_rms": math.sqrt(w.Ra / w.Pr * nu["u2"]), "Re_rms_mean": math.sqrt(w.Ra / w.Pr * nu["u2_mean"]),
         "total_s": total, "in_step_s": in_step, "H_lu": p["H_lu"],
     }
     return sim, w, out
@@ -342,6 +343,72 @@ def run_slab(args):
         dist.destroy_process_group()
 
 
+FULL_RUNS = (("c2_512sq", 0), ("c2_512sq_uniform", 0), ("c3_1024sq", 0), ("c3_1024sq", 1), ("c3_1024sq_uniform", 0),
+             ("c4_128cu", 0), ("c5_256cu", 0), ("c5_256cu", 1), ("c5_256cu_uniform", 0))
+
+
+def run_full(args):
+    """--full: the step counts BASELINE.json states (configs 2-5: 20 000 / 50 000 / 5 000 / 10 000 LBM steps, the
+    uniform counterparts alike), timed as ONE region per run with Nu_hot / <Re> sampled every 100 steps (DESIGN.md
+    A20: plain mean of the samples over the timed window), after a 200-step warm-up.  One JSON line."""
+    import torch
+    from paper_2509_01099_b200 import inputs, islbm
+    dev = torch.device("cuda", 0)
+    peak, peak_src = read_peaks()
+    out = {}
+    for name, prec in FULL_RUNS:
+        if args.workload not in (DEFAULT_WORKLOAD, name):       # --workload X --full: only X
+            continue
+        w = inputs.workload(name)
+        sim = islbm.Islbm(w.coords, w.delta, w.Ra, w.Pr, w.Ma, precision=prec, device=dev)
+        sim.init(w.seed, w.noise_amp)
+        sim.step(200)
+        sim.nusselt()
+        sampler = ClockSampler(0)
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        nus, in_step = [], 0.0
+        evs = []
+        e0.record()
+        for _ in range(w.steps // 100):
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record()
+            sim.step(100)
+            b.record()
+            evs.append((a, b))
+            nus.append(sim.nusselt())
+        e1.record()
+        torch.cuda.synchronize()
+        clocks = sampler.stop()
+        total = e0.elapsed_time(e1) * 1e-3
+        in_step = sum(a.elapsed_time(b) for a, b in evs) * 1e-3
+        p = sim.params()
+        bpu = BYTES_PER_UPDATE[(w.dim, prec)]
+        n_lbm = (w.steps // 100) * 100
+        out[name + ("_f32" if prec else "")] = {
+            "lbm_steps_timed": n_lbm, "seconds": total, "mlups": w.nodes * n_lbm / total / 1e6,
+            "us_per_lbm_step_kernel": in_step / n_lbm * 1e6,
+            "roofline_frac": bpu * w.nodes / (in_step / n_lbm) / 1e9 / peak,
+            "wctpdt_s": total / n_lbm * p["H_lu"] / p["U"], "t_ff_advanced": n_lbm * p["dt_star"], "kernel": sim.kernel_name,
+            "Nu_hot_time_mean": sum(n["Nu_hot"] for n in nus) / len(nus), "Nu_hot_final": nus[-1]["Nu_hot"],
+            "Re_time_mean": sum(n["Re"] for n in nus) / len(nus),
+            "Re_rms_time_mean": math.sqrt(w.Ra / w.Pr * sum(n["u2"] for n in nus) / len(nus)),
+            "nu_samples": len(nus), "clocks": clocks}
+        sim.close()
+        del sim
+        torch.cuda.empty_cache()
+    for nu, un in (("c2_512sq", "c2_512sq_uniform"), ("c3_1024sq", "c3_1024sq_uniform"), ("c5_256cu", "c5_256cu_uniform")):
+        if nu in out and un in out:
+            out[nu]["mlups_nonuniform_over_uniform"] = out[nu]["mlups"] / out[un]["mlups"]
+            out[nu]["wctpdt_nonuniform_over_uniform"] = out[nu]["wctpdt_s"] / out[un]["wctpdt_s"]
+    print(json.dumps({"mode": "full", "metric": METRIC, "unit": "MLUPS", "n_gpus": 1, "dtype": "f64 (keys *_f32: fp32 storage)",
+                      "data": "synthetic", "peak_gbs": peak, "peak_source": peak_src,
+                      "config": {"workload": "BASELINE.json configs 2-5 at their stated step counts",
+                                 "sampling": "Nu_hot, <Re> every 100 steps over the timed window (DESIGN.md A20)",
+                                 "uniform": "uniform counterparts through the general TMA kernel"},
+                      "runs": out}), flush=True)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -357,12 +424,17 @@ def main():
     ap.add_argument("--halo", default="fused", choices=["fused", "p2p"],
                     help="--decomp slab: halo stored by the step kernel into peer memory (default) or exchanged with isend/irecv")
     ap.add_argument("--no-extras", action="store_true", help="skip the secondary workloads, e2e and CPU baseline")
+    ap.add_argument("--full", action="store_true",
+                    help="time BASELINE.json's configs 2-5 at their stated step counts (20 000 / 50 000 / 5 000 / 10 000) "
+                         "with Nu/Re sampled every 100 steps; about one minute on a B200")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         return run_reference(args)
     if args.decomp == "slab":
         return run_slab(args)
+    if args.full:
+        return run_full(args)
 
     import torch
     from paper_2509_01099_b200 import inputs, islbm     # raises if libislbm.so is missing: no fallback
@@ -431,7 +503,8 @@ def main():
         # 3 = the pure-shift kernel (the paper's "uniform" runs)
         for nm, pr, kn in (("c5_256cu_uniform", 0, 0), ("c5_256cu_uniform", 0, 3), ("c5_256cu", 1, 0), ("c5_256cu_uniform", 1, 3),
                            ("c3_1024sq", 0, 0), ("c3_1024sq_uniform", 0, 0), ("c3_1024sq_uniform", 0, 3), ("c3_1024sq", 1, 0),
-                           ("c2_512sq", 0, 0), ("c2_512sq_uniform", 0, 3), ("c4_128cu", 0, 0), ("c1_64sq", 0, 0)):
+                           ("c2_512sq", 0, 0), ("c2_512sq_uniform", 0, 0), ("c2_512sq_uniform", 0, 3), ("c4_128cu", 0, 0),
+                           ("c1_64sq", 0, 0)):
             if nm == args.workload and pr == prec and kn == args.kernel:
                 continue
             key = nm + ("_f32" if pr else "") + ("_shift" if kn == 3 else "")
@@ -442,23 +515,30 @@ def main():
                 extras[key] = {
                     "mlups": r2["mlups"], "roofline_frac": b2 * w2.nodes / (r2["us_per_lbm_step"] * 1e-6) / 1e9 / peak,
                     "us_per_lbm_step": r2["us_per_lbm_step"], "wctpdt_s": r2["wctpdt_s"], "kernel": r2["kernel"],
-                    "Nu_hot_time_mean": r2["Nu_hot_mean"], "Re_time_mean": r2["Re_mean"], "nu_samples": r2["nu_samples"],
+                    "Nu_hot_transient_mean": r2["Nu_hot_mean"], "Re_transient_mean": r2["Re_mean"],
+                    "Re_rms_transient_mean": r2["Re_rms_mean"], "nu_samples": r2["nu_samples"],
+                    "transient_window": f"{r2['nu_samples']} samples, one per {lps} steps from the rest + noise start",
                     "state_bytes_per_buffer": (w2.nodes * b2) // 2}
                 s2.close()
                 del s2
                 torch.cuda.empty_cache()
             except Exception as exc:   # a secondary workload must not take the headline down
                 extras[key] = {"error": str(exc)[:200]}
-        # non-uniform / uniform ratios the paper reports: MLUPS ratio and WCTpDT ratio
+        # non-uniform / uniform ratios the paper reports: MLUPS ratio and WCTpDT ratio.  The
+        # uniform counterpart is the FASTER of the two uniform-mesh runs (general TMA kernel on the uniform mesh, or the
+        # pure-shift kernel): the ratio is not flattered by a weak denominator
         ratios = {}
         head = {"mlups": r["mlups"], "wctpdt_s": r["wctpdt_s"]}
-        for nu, un in ((args.workload if prec == 0 else None, "c5_256cu_uniform_shift"), ("c3_1024sq", "c3_1024sq_uniform_shift"),
-                       ("c2_512sq", "c2_512sq_uniform_shift")):
+        for nu, un in ((args.workload if prec == 0 else None, "c5_256cu_uniform"), ("c3_1024sq", "c3_1024sq_uniform"),
+                       ("c2_512sq", "c2_512sq_uniform")):
             a = head if nu == args.workload else extras.get(nu)
-            b = extras.get(un)
-            if a and b and "mlups" in a and "mlups" in b:
+            cands = [(k, extras[k]) for k in (un, un + "_shift") if k in extras and "mlups" in extras[k]]
+            if a and cands and "mlups" in a:
+                kb, b = max(cands, key=lambda kv: kv[1]["mlups"])
                 ratios[nu] = {"mlups_nonuniform_over_uniform": a["mlups"] / b["mlups"],
-                              "wctpdt_nonuniform_over_uniform": a["wctpdt_s"] / b["wctpdt_s"]}
+                              "wctpdt_nonuniform_over_uniform": a["wctpdt_s"] / b["wctpdt_s"],
+                              "uniform_run": kb, "uniform_kernel": b["kernel"],
+                              "uniform_runs_mlups": {k: v["mlups"] for k, v in cands}}
         extras["ratios"] = ratios
         cores = oracle_threads()
         mlups_cpu, _, what, nodes_s = time_oracle(w, 3, 1, cores)
@@ -477,7 +557,13 @@ def main():
                              if w.nodes * bpu > 3e8 else "state fits in L2: fraction is not an HBM fraction",
                        "parallelism": f"{world} independent cavities (replicas, no data-path collective)"},
             "wctpdt_s": r["wctpdt_s"], "Nu_hot": r["Nu_hot"], "Re": r["Re"],
-            "Nu_hot_time_mean": r["Nu_hot_mean"], "Re_time_mean": r["Re_mean"], "nu_samples": r["nu_samples"],
+            # start-up transient out of the rest + noise state, NOT the statistic of BASELINE.json config 3 (that is
+            # `bench.py --full`): mean of one sample per bench step; Re = Eq. 34 as printed (mean speed), Re_rms =
+            # sqrt(Ra/Pr <u*^2>), the form the paper's tables print (A22)
+            "Nu_hot_transient_mean": r["Nu_hot_mean"], "Re_transient_mean": r["Re_mean"], "Re_rms": r["Re_rms"],
+            "Re_rms_transient_mean": r["Re_rms_mean"], "nu_samples": r["nu_samples"],
+            "transient_window": f"{r['nu_samples']} samples, one per {args.lbm_per_step} steps, steps "
+                                f"{args.warmup * args.lbm_per_step}..{(args.warmup + args.steps) * args.lbm_per_step} after the rest + noise start",
             "roofline": roofline, "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": r["launches"], "clocks": clocks,
             "also": extras,
         }

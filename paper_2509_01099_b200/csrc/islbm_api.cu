@@ -126,11 +126,11 @@ struct islbm {
 static void make_tiled_plan(islbm *h) {
   void *b0 = h->ws + h->cv.buf[0], *b1 = h->ws + h->cv.buf[1];
   if (h->dim == 2) {
-    if (h->precision == ISLBM_F64) plan2_create<double>(h->plan2, h->n, h->dm.nxp, b0, b1, h->tune);
-    else plan2_create<float>(h->plan2, h->n, h->dm.nxp, b0, b1, h->tune);
+    if (h->precision == ISLBM_F64) plan2_create<double>(h->plan2, h->n, h->dm.nxp, b0, b1, h->tune, h->stencil);
+    else plan2_create<float>(h->plan2, h->n, h->dm.nxp, b0, b1, h->tune, h->stencil);
   } else {
-    if (h->precision == ISLBM_F64) plan3_create<double>(h->plan3, h->n, h->dm.nxp, b0, b1, h->tune);
-    else plan3_create<float>(h->plan3, h->n, h->dm.nxp, b0, b1, h->tune);
+    if (h->precision == ISLBM_F64) plan3_create<double>(h->plan3, h->n, h->dm.nxp, b0, b1, h->tune, h->stencil);
+    else plan3_create<float>(h->plan3, h->n, h->dm.nxp, b0, b1, h->tune, h->stencil);
   }
 }
 
@@ -412,10 +412,13 @@ extern "C" int islbm_set_stencil(islbm_t *h, int kind) {
   if (kind != 0 && kind != 1) return fail(ISLBM_ERR_ARG, "stencil must be 0 (central) or 1 (upwind)");
   if (h->has_state && kind != h->stencil)
     return fail(ISLBM_ERR_STATE, "set the stencil before islbm_init / islbm_set_populations");
-  if (kind == 1 && h->kernel_choice == 2) return fail(ISLBM_ERR_ARG, "the TMA kernels take the central stencil only");
+  if (kind == 1 && h->is_slab)
+    return fail(ISLBM_ERR_ARG, "the upwind stencil reaches two layers upstream: not available on slab handles (one ghost layer)");
+  if (kind == 1 && h->kernel_choice == 3) return fail(ISLBM_ERR_ARG, "the pure-shift kernel has no stencil");
   h->stencil = kind;
   h->dm.stencil = kind;
   CUDA_TRY(cudaStreamSynchronize(h->stream));
+  make_tiled_plan(h);     // the TMA kernels of the chosen stencil (2-row halo and split z-stencil groups for the upwind one)
   return upload_tables(h);
 }
 
@@ -537,7 +540,6 @@ static void launch_shift_step(islbm *h) {
 }
 
 static int effective_kernel(const islbm *h) {
-  if (h->stencil != 0 && h->kernel_choice != 3) return 1;   // only the generic kernel reads a 2-node upwind stencil
   if (h->kernel_choice != 0) return h->kernel_choice;
   return h->tiled_ok() ? 2 : 1;
 }
@@ -545,7 +547,9 @@ static int effective_kernel(const islbm *h) {
 extern "C" const char *islbm_kernel_name(const islbm_t *h) {
   if (!h) return "";
   switch (effective_kernel(h)) {
-    case 2: return h->dim == 2 ? (h->plan2.tx == 224 ? "tiled_ymarch_tma_tx224" : "tiled_ymarch_tma_tx128") : "tiled_zmarch_tma";
+    case 2:
+      if (h->stencil) return h->dim == 2 ? "tiled_ymarch_tma_upwind" : "tiled_zmarch_tma_upwind";
+      return h->dim == 2 ? (h->plan2.tx == 224 ? "tiled_ymarch_tma_tx224" : "tiled_ymarch_tma_tx128") : "tiled_zmarch_tma";
     case 3: return "uniform_shift";
     default: return "generic_global";
   }
@@ -554,7 +558,7 @@ extern "C" const char *islbm_kernel_name(const islbm_t *h) {
 extern "C" int islbm_set_kernel(islbm_t *h, int which) {
   if (!h) return fail(ISLBM_ERR_ARG, "NULL handle");
   if (which < 0 || which > 3) return fail(ISLBM_ERR_ARG, "kernel selector must be 0..3");
-  if (which == 2 && h->stencil != 0) return fail(ISLBM_ERR_ARG, "the TMA kernels take the central stencil only");
+  if (which == 3 && h->stencil != 0) return fail(ISLBM_ERR_ARG, "the pure-shift kernel has no stencil");
   if (which == 2 && !h->tiled_ok()) return fail(ISLBM_ERR_ARG, std::string("tiled kernel not available: ") + h->tiled_why_not());
   if (which == 3 && !h->uniform) return fail(ISLBM_ERR_ARG, "uniform-shift kernel needs every spacing to equal delta");
   h->kernel_choice = which;

@@ -98,25 +98,27 @@ ISLBM_HD constexpr int opposite(int q) {
 // Storage plane of flow population q / temperature population q inside a population buffer.  The public
 // arrays of include/islbm.h are [q][z][y][x] in direction order; INSIDE the workspace the planes are ordered
 // by the halo group the TMA-staged kernels load with one box:
-//   2-D: f0 g0 | f1 f3 g1 g3 | f2 f4 g2 g4 | f5 f6 f7 f8
-//   3-D: f0 g0 | f1 f2 g1 g2 | f3 f4 g3 g4 | f7..f10 | f5 f6 g5 g6 | f11..f14 | f15..f18
+//   2-D: f0 g0 | f1 f3 g1 g3 | f2 g2 f4 g4 | f5 f6 f7 f8
+//   3-D: f0 g0 | f1 f2 g1 g2 | f3 f4 g3 g4 | f7..f10 | f5 g5 f6 g6 | f11..f14 | f15..f18
+// (inside the last three groups the populations with a positive component along the marching axis come first: the
+// upwind-stencil kernels load the two halves of a group from different layers)
 template <int DIM>
 ISLBM_HD constexpr int plane_f(int q) {
   if (DIM == 2) {
-    constexpr int t[9] = {0, 2, 6, 3, 7, 10, 11, 12, 13};
+    constexpr int t[9] = {0, 2, 6, 3, 8, 10, 11, 12, 13};
     return t[q];
   } else {
-    constexpr int t[19] = {0, 2, 3, 6, 7, 14, 15, 10, 11, 12, 13, 18, 19, 20, 21, 22, 23, 24, 25};
+    constexpr int t[19] = {0, 2, 3, 6, 7, 14, 16, 10, 11, 12, 13, 18, 19, 20, 21, 22, 23, 24, 25};
     return t[q];
   }
 }
 template <int DIM>
 ISLBM_HD constexpr int plane_g(int q) {
   if (DIM == 2) {
-    constexpr int t[5] = {1, 4, 8, 5, 9};
+    constexpr int t[5] = {1, 4, 7, 5, 9};
     return t[q];
   } else {
-    constexpr int t[7] = {1, 4, 5, 8, 9, 16, 17};
+    constexpr int t[7] = {1, 4, 5, 8, 9, 15, 17};
     return t[q];
   }
 }

@@ -8,7 +8,7 @@
 //     are ordered so that a box covers consecutive planes, plane_f / plane_g)
 //     into a ring of shared-memory stages guarded by full/empty mbarriers;
 //     planes with e_x != 0 (f1 f3 g1 g3 | f5..f8) carry a 16-byte x-halo on each
-//     side, the others (f0 g0 | f2 f4 g2 g4) none;
+//     side, the others (f0 g0 | f2 g2 f4 g4) none;
 //   * consumers interpolate along x from shared memory; the y-direction of the
 //     separable interpolation is a 3-row combination kept
 //     in REGISTERS (three rotating register sets) for the 8 populations with
@@ -30,22 +30,27 @@ namespace islbmk {
 #define ISLBM_F32_CTAS2D 5
 #endif
 
-template <typename ST, int TX_, int STAGES_>
+template <typename ST, int TX_, int STAGES_, int SK_ = 0>
 struct Tile2 {
-  static constexpr int TX = TX_, STAGES = STAGES_;
+  static constexpr int TX = TX_, STAGES = STAGES_, SK = SK_;   // SK: stencil kind (Tile3)
   static constexpr int XH = 16 / (int)sizeof(ST);
   static constexpr int HX = TX + 2 * XH;
   static constexpr int P_X = HX * (int)sizeof(ST), P_C = TX * (int)sizeof(ST);   // bytes of one plane row in a box
   // groups of a stage, in storage-plane order (each starts 128-byte aligned):
-  //   emitted row y:      C2 = f0 g0, XR = f1 f3 g1 g3        y-stencil row (m):  C4 = f2 f4 g2 g4, XM = f5..f8
+  //   emitted row y:      C2 = f0 g0, XR = f1 f3 g1 g3        y-stencil row (m):  C4 = f2 g2 f4 g4, XM = f5..f8
   static constexpr int OFF_C2 = 0;
   static constexpr int OFF_XR = pad128(OFF_C2 + 2 * P_C);
+  // halves of a y-stencil group (e_y = +1, then e_y = -1): loaded by separate boxes with the upwind stencil, whose
+  // shared-memory destinations must be 128-byte aligned (Tile3::H_*)
+  static constexpr int H_C = SK ? pad128(2 * P_C) : 2 * P_C, H_X = SK ? pad128(2 * P_X) : 2 * P_X;
   static constexpr int OFF_C4 = pad128(OFF_XR + 4 * P_X);
-  static constexpr int OFF_XM = pad128(OFF_C4 + 4 * P_C);
-  static constexpr int STAGE_BYTES = pad128(OFF_XM + 4 * P_X);
+  static constexpr int OFF_XM = pad128(OFF_C4 + 2 * H_C);
+  static constexpr int STAGE_BYTES = pad128(OFF_XM + 2 * H_X);
+  static __host__ __device__ constexpr int moff(int off, int k, int pbytes, int half) { return off + (k / 2) * half + (k % 2) * pbytes; }
   static constexpr int WARPS = TX / 32;
   static constexpr uint32_t Y_BYTES = 2u * P_C + 4u * P_X;   // planes of the emitted row
   static constexpr uint32_t M_BYTES = 4u * P_C + 4u * P_X;   // planes of the y-stencil row
+  static constexpr uint32_t F_BYTES = M_BYTES / 2;           // ... of one half of it (upwind stencil)
   static constexpr int BAR_OFF = STAGES * STAGE_BYTES;
   static constexpr int W_OFF = BAR_OFF + 128;                // y-weights of the chunk [sign][k][kMaxChunk]
   // fp32 storage: the x-interpolated values of the three y-stencil rows live in shared memory, [slot 3][pair 4][thread]
@@ -58,6 +63,7 @@ struct Tile2 {
 // tensor maps over (x, y, plane): one per box shape
 struct Maps2 {
   CUtensorMap c2, c4, x;
+  CUtensorMap x2;   // two-plane box of the x shape (upwind stencil: half of the group f5..f8)
 };
 
 // yf = first emitted row of the chunk (its lowest row for DIR = +1, its highest for DIR = -1).
@@ -83,7 +89,7 @@ __device__ __forceinline__ void issue_stage2(int s, int yf, int ny, int x0, unsi
     tma_load_3d(sb + T::OFF_XR, &mp.x, bar, xh, yrow, 2, pol);     // f1 f3 g1 g3
   }
   if (mrow >= 0) {
-    tma_load_3d(sb + T::OFF_C4, &mp.c4, bar, x0, mrow, 6, pol);    // f2 f4 g2 g4
+    tma_load_3d(sb + T::OFF_C4, &mp.c4, bar, x0, mrow, 6, pol);    // f2 g2 f4 g4
     tma_load_3d(sb + T::OFF_XM, &mp.x, bar, xh, mrow, 10, pol);    // f5..f8
   }
 }
@@ -93,8 +99,8 @@ __device__ __forceinline__ void issue_stage2(int s, int yf, int ny, int x0, unsi
 // (lane a has e_y = +1 in pairs 0, 1, 2 and e_y = -1 in pair 3, which takes the swapped y-weights)
 #define ISLBM_LOAD_M2(S)                                                            \
   do {                                                                              \
-    S[0] = mkpr((AT)PC4(0)[0], (AT)PC4(1)[0]);         /* f2, f4 */                 \
-    S[1] = mkpr((AT)PC4(2)[0], (AT)PC4(3)[0]);         /* g2, g4 */                 \
+    S[0] = mkpr((AT)PC4(0)[0], (AT)PC4(2)[0]);         /* f2, f4 */                 \
+    S[1] = mkpr((AT)PC4(1)[0], (AT)PC4(3)[0]);         /* g2, g4 */                 \
     S[2] = ptap3(PXM(0), PXM(2), 1, wxN);              /* f5 (+x,+y), f7 (-x,-y) */ \
     S[3] = ptap3(PXM(3), PXM(1), 1, wxN);              /* f8 (+x,-y), f6 (-x,+y) */ \
   } while (0)
@@ -154,7 +160,7 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
   }
   for (int i = (int)threadIdx.x - 32; i >= 0 && i < 6 * (y1 - y0); i += T::TX - 32) {   // warps 1..: warp 0 is waiting above
     const int sk = i / (y1 - y0), yi = i - sk * (y1 - y0);
-    stage_march_weight(wys, sk, yi, __ldg(wrow(m, 1, sk / 3, sk % 3) + y0 + yi));
+    stage_march_weight<0>(wys, sk, yi, __ldg(wrow(m, 1, sk / 3, sk % 3) + y0 + yi));
   }
   pdl_wait();
   __syncthreads();
@@ -233,7 +239,7 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
 
     if (has_emit) {
       Pr<AT> wyN[3], wyS[3];
-      load_march_weights(wys, y - y0, wyN, wyS);
+      load_march_weights<0>(wys, y - y0, wyN, wyS);
       // ascending-y order of the stencil rows: the marching order when DIR = +1, its reverse when DIR = -1
       if constexpr (T::S_IN_SMEM) {
         // marching order = slots (newest+1, newest+2, newest) mod 3; the newest row is still in registers unless the
@@ -277,6 +283,222 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
   }
 }
 
+// ------------------------------ upwind stencil (islbm_set_stencil(h, 1)) ----------------------------------------
+// Stage content for the A2-alternative stencil {j-2,j-1,j} / {j,j+1,j+2}: the e_y = +1 half of the y-stencil group
+// (f2 g2 | f5 f6) trails the emitted row, the e_y = -1 half (f4 g4 | f7 f8) leads it by two rows.  Marches upwards.
+template <typename T>
+__device__ __forceinline__ void issue_stage2_up(int s, int yf, int ny, int x0, unsigned char *stage0, uint64_t *full,
+                                                const Maps2 &mp, uint64_t pol) {
+  const int st = s % T::STAGES;
+  int prow = -1, mrow = -1, yrow = -1;
+  if (s < 2) {
+    prow = ubase_p(yf, ny) + s;
+    mrow = ubase_m(yf, ny) + s;
+  } else {
+    yrow = yf + (s - 2);
+    if (s == 2 || ubase_p_moves(yrow, ny)) prow = ubase_p(yrow, ny) + 2;
+    if (s == 2 || ubase_m_moves(yrow, ny)) mrow = ubase_m(yrow, ny) + 2;
+  }
+  uint64_t *bar = &full[st];
+  mbar_expect_tx(bar, (prow >= 0 ? T::F_BYTES : 0u) + (mrow >= 0 ? T::F_BYTES : 0u) + (yrow >= 0 ? T::Y_BYTES : 0u));
+  unsigned char *sb = stage0 + (size_t)st * T::STAGE_BYTES;
+  const int xh = x0 - T::XH;
+  if (yrow >= 0) {
+    tma_load_3d(sb + T::OFF_C2, &mp.c2, bar, x0, yrow, 0, pol);                    // f0 g0
+    tma_load_3d(sb + T::OFF_XR, &mp.x, bar, xh, yrow, 2, pol);                     // f1 f3 g1 g3
+  }
+  if (prow >= 0) {
+    tma_load_3d(sb + T::OFF_C4, &mp.c2, bar, x0, prow, 6, pol);                    // f2 g2
+    tma_load_3d(sb + T::OFF_XM, &mp.x2, bar, xh, prow, 10, pol);                   // f5 f6
+  }
+  if (mrow >= 0) {
+    tma_load_3d(sb + T::OFF_C4 + T::H_C, &mp.c2, bar, x0, mrow, 8, pol);           // f4 g4
+    tma_load_3d(sb + T::OFF_XM + T::H_X, &mp.x2, bar, xh, mrow, 12, pol);          // f7 f8
+  }
+}
+
+// family P (e_y = +1): (f2, g2) (f5, f6), rows {y-2, y-1, y}; family M (e_y = -1): (f4, g4) (f8, f7), rows {y, y+1, y+2};
+// lane a of the x-interpolated pairs is the +x population (window starts two nodes upstream), lane b the -x one
+#define ISLBM_LOAD_U2(S, H)                                                                                     \
+  do {                                                                                                          \
+    S[0] = mkpr((AT)PC4(2 * H)[tx], (AT)PC4(2 * H + 1)[tx]);                          /* f2 g2 | f4 g4 */        \
+    S[1] = H == 0 ? ptap3(PXM(0) + o_xa, PXM(1) + o_xb, 1, wxN)                       /* f5 (+x), f6 (-x) */     \
+                  : ptap3(PXM(3) + o_xa, PXM(2) + o_xb, 1, wxN);                      /* f8 (+x), f7 (-x) */     \
+  } while (0)
+#define ISLBM_YCOMB_U2(W, P0, P1, P2, F0, G0, F1A, F1B)   \
+  do {                                                    \
+    const Pr<AT> q0 = pcomb3(W, P0[0], P1[0], P2[0]);     \
+    const Pr<AT> q1 = pcomb3(W, P0[1], P1[1], P2[1]);     \
+    f[F0] = lane_a(q0);  g[G0] = lane_b(q0);              \
+    f[F1A] = lane_a(q1); f[F1B] = lane_b(q1);             \
+  } while (0)
+
+template <typename ST, int TX, int STAGES, int MINB>
+__global__ void __launch_bounds__(TX, MINB)
+k_step_ymarch_up(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const ST *__restrict__ src, ST *__restrict__ dst,
+                 int load_policy, int store_policy, int late_fill) {
+  using T = Tile2<ST, TX, STAGES, 1>;
+  using AT = typename Acc<ST>::type;
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  unsigned char *stage0 = smem_raw;
+  uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + T::BAR_OFF);
+  uint64_t *empty = full + T::STAGES;
+  AT *wys = reinterpret_cast<AT *>(smem_raw + T::W_OFF);
+  int *claim = reinterpret_cast<int *>(smem_raw + T::BAR_OFF + 2 * T::STAGES * 8);
+  pdl_launch_dependents();
+
+  const int x0 = blockIdx.x * T::TX;
+  const int rows = m.em_hi - m.em_lo;
+  const int y0 = m.em_lo + (int)((long long)blockIdx.y * rows / gridDim.y);
+  const int y1 = m.em_lo + (int)((long long)(blockIdx.y + 1) * rows / gridDim.y);
+  const int nstage = 2 + (y1 - y0);
+  const uint64_t lpol = make_policy(load_policy);
+  const uint64_t spol = make_policy(store_policy);
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < T::STAGES; ++s) {
+      mbar_init(&full[s], 1);
+      mbar_init(&empty[s], T::WARPS);
+      claim[s] = 0;
+    }
+    fence_barrier_init();
+    tma_prefetch_desc(&mp.c2);
+    tma_prefetch_desc(&mp.x);
+    tma_prefetch_desc(&mp.x2);
+    if (!late_fill) {
+      pdl_wait();
+      for (int s = 0; s < T::STAGES && s < nstage; ++s) issue_stage2_up<T>(s, y0, m.ny, x0, stage0, full, mp, lpol);
+    }
+  }
+  for (int i = (int)threadIdx.x - 32; i >= 0 && i < 6 * (y1 - y0); i += T::TX - 32) {
+    const int sk = i / (y1 - y0), yi = i - sk * (y1 - y0);
+    stage_march_weight<1>(wys, sk, yi, __ldg(wrow(m, 1, sk / 3, sk % 3) + y0 + yi));
+  }
+  pdl_wait();
+  __syncthreads();
+  if (late_fill && threadIdx.x == 0) {
+    for (int s = 0; s < T::STAGES && s < nstage; ++s) issue_stage2_up<T>(s, y0, m.ny, x0, stage0, full, mp, lpol);
+  }
+
+  const int tx = threadIdx.x;
+  const int x = x0 + tx;
+  const bool valid = x < m.nx;
+  WallFlags wf;
+  wf.lo[0] = valid && x == 0;
+  wf.hi[0] = valid && x == m.nx - 1;
+  wf.lo[2] = wf.hi[2] = false;
+  const bool wall_x = wf.lo[0] | wf.hi[0];
+  const int o_xa = ubase_p(min(x, m.nx - 1), m.nx) - x0 + T::XH, o_xb = ubase_m(min(x, m.nx - 1), m.nx) - x0 + T::XH;
+  Pr<AT> wxN[3];
+#pragma unroll
+  for (int k = 0; k < 3; ++k)
+    wxN[k] = mkpr(valid ? (AT)__ldg(wrow(m, 0, 1, k) + x) : (AT)0, valid ? (AT)__ldg(wrow(m, 0, 0, k) + x) : (AT)0);
+  long long c = (long long)y0 * m.nxp + x;
+
+  Pr<AT> P0[2], P1[2], P2[2], M0[2], M1[2], M2[2];
+  int newest_p = 2, newest_m = 2;
+  Pr<AT> *ssm = reinterpret_cast<Pr<AT> *>(smem_raw + T::S_OFF) + threadIdx.x;   // S_IN_SMEM: [family][slot][pair][thread]
+  constexpr int SSLOT = 2 * T::TX;
+
+#pragma unroll 1
+  for (int s = 0; s < nstage; ++s) {
+    const int st = s % T::STAGES;
+    const uint32_t ph = (uint32_t)(s / T::STAGES) & 1u;
+    const int y = y0 + (s - 2);
+    const bool has_emit = s >= 2;
+    const bool mov_p = s <= 2 || ubase_p_moves(y, m.ny), mov_m = s <= 2 || ubase_m_moves(y, m.ny);
+    const ST *sb = reinterpret_cast<const ST *>(stage0 + (size_t)st * T::STAGE_BYTES);
+    constexpr int ES = (int)sizeof(ST);
+#define PC2(k) (sb + (T::OFF_C2 + (k) * T::P_C) / ES)
+#define PXR(k) (sb + (T::OFF_XR + (k) * T::P_X) / ES)
+#define PC4(k) (sb + T::moff(T::OFF_C4, k, T::P_C, T::H_C) / ES)
+#define PXM(k) (sb + T::moff(T::OFF_XM, k, T::P_X, T::H_X) / ES)
+    mbar_wait(&full[st], ph);
+
+    if (mov_p) {
+      newest_p = newest_p == 2 ? 0 : newest_p + 1;
+      if constexpr (T::S_IN_SMEM) {
+        ISLBM_LOAD_U2(P2, 0);
+#pragma unroll
+        for (int k = 0; k < 2; ++k) ssm[newest_p * SSLOT + k * T::TX] = P2[k];
+      } else {
+        if (newest_p == 0) ISLBM_LOAD_U2(P0, 0);
+        else if (newest_p == 1) ISLBM_LOAD_U2(P1, 0);
+        else ISLBM_LOAD_U2(P2, 0);
+      }
+    }
+    if (mov_m) {
+      newest_m = newest_m == 2 ? 0 : newest_m + 1;
+      if constexpr (T::S_IN_SMEM) {
+        ISLBM_LOAD_U2(M2, 1);
+#pragma unroll
+        for (int k = 0; k < 2; ++k) ssm[(3 + newest_m) * SSLOT + k * T::TX] = M2[k];
+      } else {
+        if (newest_m == 0) ISLBM_LOAD_U2(M0, 1);
+        else if (newest_m == 1) ISLBM_LOAD_U2(M1, 1);
+        else ISLBM_LOAD_U2(M2, 1);
+      }
+    }
+
+    AT f[9], g[5];
+    if (has_emit) {
+      f[0] = PC2(0)[tx];
+      g[0] = PC2(1)[tx];
+      const Pr<AT> p1 = ptap3(PXR(0) + o_xa, PXR(1) + o_xb, 1, wxN);   // f1 (+x), f3 (-x)
+      const Pr<AT> p2 = ptap3(PXR(2) + o_xa, PXR(3) + o_xb, 1, wxN);   // g1, g3
+      f[1] = lane_a(p1); f[3] = lane_b(p1);
+      g[1] = lane_a(p2); g[3] = lane_b(p2);
+    }
+    __syncwarp();
+    if ((threadIdx.x & 31) == 0 && mbar_arrive_is_last(&empty[st]) && s + T::STAGES < nstage &&
+        atomicCAS(&claim[st], s / T::STAGES, s / T::STAGES + 1) == s / T::STAGES)
+      issue_stage2_up<T>(s + T::STAGES, y0, m.ny, x0, stage0, full, mp, lpol);
+
+    if (has_emit) {
+      Pr<AT> wyA[3], wyB[3];    // (c=+1, c=+1) for family P, (c=-1, c=-1) for family M
+      load_march_weights<1>(wys, y - y0, wyA, wyB);
+      if constexpr (T::S_IN_SMEM) {
+        const Pr<AT> *pp0 = ssm + (newest_p == 2 ? 0 : newest_p + 1) * SSLOT, *pp1 = ssm + (newest_p == 0 ? 2 : newest_p - 1) * SSLOT;
+        const Pr<AT> *pm0 = ssm + (3 + (newest_m == 2 ? 0 : newest_m + 1)) * SSLOT, *pm1 = ssm + (3 + (newest_m == 0 ? 2 : newest_m - 1)) * SSLOT;
+#pragma unroll
+        for (int k = 0; k < 2; ++k) {
+          P0[k] = pp0[k * T::TX];
+          P1[k] = pp1[k * T::TX];
+          M0[k] = pm0[k * T::TX];
+          M1[k] = pm1[k * T::TX];
+        }
+        if (!mov_p) {
+#pragma unroll
+          for (int k = 0; k < 2; ++k) P2[k] = ssm[newest_p * SSLOT + k * T::TX];
+        }
+        if (!mov_m) {
+#pragma unroll
+          for (int k = 0; k < 2; ++k) M2[k] = ssm[(3 + newest_m) * SSLOT + k * T::TX];
+        }
+        ISLBM_YCOMB_U2(wyA, P0, P1, P2, 2, 2, 5, 6);
+        ISLBM_YCOMB_U2(wyB, M0, M1, M2, 4, 4, 8, 7);
+      } else {
+        if (newest_p == 0) ISLBM_YCOMB_U2(wyA, P1, P2, P0, 2, 2, 5, 6);
+        else if (newest_p == 1) ISLBM_YCOMB_U2(wyA, P2, P0, P1, 2, 2, 5, 6);
+        else ISLBM_YCOMB_U2(wyA, P0, P1, P2, 2, 2, 5, 6);
+        if (newest_m == 0) ISLBM_YCOMB_U2(wyB, M1, M2, M0, 4, 4, 8, 7);
+        else if (newest_m == 1) ISLBM_YCOMB_U2(wyB, M2, M0, M1, 4, 4, 8, 7);
+        else ISLBM_YCOMB_U2(wyB, M0, M1, M2, 4, 4, 8, 7);
+      }
+      wf.lo[1] = y == 0 && m.wall_mlo;
+      wf.hi[1] = y == m.ny - 1 && m.wall_mhi;
+      if (valid && (wall_x | wf.lo[1] | wf.hi[1])) wall_fix_node<2>(f, g, wf, src + c, m.nnp, m);
+      constexpr bool DEV = Store<ST, 2>::kBiased;
+      collide_node<DEV>(f, g, np);
+      if (valid) store_node<2, DEV>(dst + c, m.nnp, f, g, spol, std::make_integer_sequence<int, 14>{});
+      c += m.nxp;
+    }
+#undef PC2
+#undef PXR
+#undef PC4
+#undef PXM
+  }
+}
+
 // ------------------------------ host side ---------------------------------
 struct Plan2 {
   bool available = false;
@@ -284,6 +506,7 @@ struct Plan2 {
   int tx = 128;
   int stages = 3;
   int per_wave = 1;      // chunks per strip in one wave of resident CTAs
+  int sk = 0;            // stencil kind the plan was built for: 0 central, 1 upwind (always Cfg2c, marches upwards)
   char why_not[96] = "";
 };
 
@@ -299,28 +522,38 @@ template <typename ST> struct Cfg2c {
 };
 template <typename ST> struct Cfg2b { using T = Tile2<ST, 224, 3>; static constexpr int MINB = 2; };
 
-template <typename ST, typename CFG>
+template <typename ST, typename CFG, int SK = 0>
 inline bool plan2_setup(Plan2 &p, const int *n, int nxp, void *buf0, void *buf1, const Tuning &tn) {
   using T = typename CFG::T;
   auto kern = k_step_ymarch<ST, T::TX, T::STAGES, CFG::MINB, 1>;
   auto kern_dn = k_step_ymarch<ST, T::TX, T::STAGES, CFG::MINB, -1>;
   void *bufs[2] = {buf0, buf1};
   const long long dims[3] = {n[0], n[1], 14};
-  const int b_c2[3] = {T::TX, 1, 2}, b_c4[3] = {T::TX, 1, 4}, b_x[3] = {T::HX, 1, 4};
+  const int b_c2[3] = {T::TX, 1, 2}, b_c4[3] = {T::TX, 1, 4}, b_x[3] = {T::HX, 1, 4}, b_x2[3] = {T::HX, 1, 2};
   for (int i = 0; i < 2; ++i)
     if (!make_map(&p.maps[i].c2, bufs[i], (int)sizeof(ST), 3, dims, b_c2, tn.l2promo, nxp) ||
         !make_map(&p.maps[i].c4, bufs[i], (int)sizeof(ST), 3, dims, b_c4, tn.l2promo, nxp) ||
-        !make_map(&p.maps[i].x, bufs[i], (int)sizeof(ST), 3, dims, b_x, tn.l2promo, nxp))
+        !make_map(&p.maps[i].x, bufs[i], (int)sizeof(ST), 3, dims, b_x, tn.l2promo, nxp) ||
+        !make_map(&p.maps[i].x2, bufs[i], (int)sizeof(ST), 3, dims, b_x2, tn.l2promo, nxp))
       return false;
-  if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM_BYTES) != cudaSuccess ||
-      cudaFuncSetAttribute(kern_dn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM_BYTES) != cudaSuccess) {
+  using TU = Tile2<ST, T::TX, T::STAGES, 1>;   // the upwind kernel's stage layout (padded halves)
+  if constexpr (SK == 1) {
+    if (cudaFuncSetAttribute(k_step_ymarch_up<ST, T::TX, T::STAGES, CFG::MINB>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                             (int)TU::SMEM_BYTES) != cudaSuccess) {
+      cudaGetLastError();
+      return false;
+    }
+  } else if (cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM_BYTES) != cudaSuccess ||
+             cudaFuncSetAttribute(kern_dn, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM_BYTES) != cudaSuccess) {
     cudaGetLastError();
     return false;
   }
   int occ = 1, dev = 0, sms = 148;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, T::TX, T::SMEM_BYTES) != cudaSuccess || occ < 1) {
+  const cudaError_t eo = SK == 1 ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, k_step_ymarch_up<ST, T::TX, T::STAGES, CFG::MINB>, T::TX, TU::SMEM_BYTES)
+                                 : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, kern, T::TX, T::SMEM_BYTES);
+  if (eo != cudaSuccess || occ < 1) {
     cudaGetLastError();
     occ = 1;
   }
@@ -333,8 +566,9 @@ inline bool plan2_setup(Plan2 &p, const int *n, int nxp, void *buf0, void *buf1,
 }
 
 template <typename ST>
-inline bool plan2_create(Plan2 &p, const int *n, int nxp, void *buf0, void *buf1, const Tuning &tn) {
+inline bool plan2_create(Plan2 &p, const int *n, int nxp, void *buf0, void *buf1, const Tuning &tn, int sk) {
   p.available = false;
+  p.sk = sk;
   auto no = [&](const char *why) { snprintf(p.why_not, sizeof p.why_not, "%s", why); return false; };
   if (n[0] < 3 || n[1] < 3) return no("tiled kernel: n >= 3");
   if ((nxp * (int)sizeof(ST)) % 16) return no("tiled kernel: TMA needs a 16-byte row pitch");
@@ -346,9 +580,10 @@ inline bool plan2_create(Plan2 &p, const int *n, int nxp, void *buf0, void *buf1
   // ring depth (measured, profiles/r1_c3_1024sq_ymarch_v5.md): fp64 takes 4 stages x 3 CTAs per SM (512^2 +4 %,
   // 1024^2 +1 %, 1538^2..8193^2 +0.3-2.3 %, 255^2 +20 %; 1026^2/1282^2 -1-2 %, inside the run-to-run spread)
   const int ring = tn.ring2d ? tn.ring2d : 4;
-  const bool ok = tx == 224 ? plan2_setup<ST, Cfg2b<ST>>(p, n, nxp, buf0, buf1, tn)
-                            : (ring == 4 ? plan2_setup<ST, Cfg2c<ST>>(p, n, nxp, buf0, buf1, tn)
-                                         : plan2_setup<ST, Cfg2a<ST>>(p, n, nxp, buf0, buf1, tn));
+  const bool ok = sk ? plan2_setup<ST, Cfg2c<ST>, 1>(p, n, nxp, buf0, buf1, tn)
+                     : (tx == 224 ? plan2_setup<ST, Cfg2b<ST>>(p, n, nxp, buf0, buf1, tn)
+                                  : (ring == 4 ? plan2_setup<ST, Cfg2c<ST>>(p, n, nxp, buf0, buf1, tn)
+                                               : plan2_setup<ST, Cfg2a<ST>>(p, n, nxp, buf0, buf1, tn)));
   if (!ok) return no("tiled kernel: tensor map / attribute setup failed");
   p.available = true;
   return true;
@@ -385,7 +620,10 @@ inline void launch2_cfg(const Plan2 &p, const int *n, const DevMesh &m, const No
   // first ring fill (measured, profiles/r1_c3_1024sq_ymarch_v4.md): a single-wave launch is 2-5 % faster with the
   // fill after the CTA barrier, a multi-wave launch 2-6 % faster with the fill first
   const int late = tn.fill ? (tn.fill == 2) : (nc <= p.per_wave);
-  if (tn.serpentine && cur)
+  if (p.sk)
+    launch_step(k_step_ymarch_up<ST, T::TX, T::STAGES, CFG::MINB>, grid, dim3(T::TX), Tile2<ST, T::TX, T::STAGES, 1>::SMEM_BYTES, stream, tn.pdl != 0,
+                p.maps[cur], m, np, (const ST *)buf[cur], (ST *)buf[1 - cur], tn.load_policy, tn.store_policy, late);
+  else if (tn.serpentine && cur)
     launch_step(k_step_ymarch<ST, T::TX, T::STAGES, CFG::MINB, -1>, grid, dim3(T::TX), T::SMEM_BYTES, stream, tn.pdl != 0,
                 p.maps[cur], m, np, (const ST *)buf[cur], (ST *)buf[1 - cur], tn.load_policy, tn.store_policy, late);
   else
@@ -396,7 +634,8 @@ inline void launch2_cfg(const Plan2 &p, const int *n, const DevMesh &m, const No
 template <typename ST>
 inline cudaError_t launch2(const Plan2 &p, const int *n, const DevMesh &m, const NodeParams &np, int cur, void *const *buf,
                            const Tuning &tn, cudaStream_t stream) {
-  if (p.tx == 224) launch2_cfg<ST, Cfg2b<ST>>(p, n, m, np, cur, buf, tn, stream);
+  if (p.sk) launch2_cfg<ST, Cfg2c<ST>>(p, n, m, np, cur, buf, tn, stream);
+  else if (p.tx == 224) launch2_cfg<ST, Cfg2b<ST>>(p, n, m, np, cur, buf, tn, stream);
   else if (p.stages == Cfg2c<ST>::T::STAGES && p.stages != Cfg2a<ST>::T::STAGES) launch2_cfg<ST, Cfg2c<ST>>(p, n, m, np, cur, buf, tn, stream);
   else launch2_cfg<ST, Cfg2a<ST>>(p, n, m, np, cur, buf, tn, stream);
   return cudaPeekAtLastError();

@@ -9,7 +9,7 @@
 //     are ordered so that each box covers the 2 or 4 consecutive planes that
 //     share a halo shape (plane_f / plane_g in islbm_lattice.cuh), and a plane
 //     carries a halo only along the axes its velocity has a component on:
-//        C  TX x TY: f0 g0 | f5 f6 g5 g6          X (TX+2XH)xTY: f1 f2 g1 g2 | f11..f14
+//        C  TX x TY: f0 g0 | f5 g5 f6 g6          X (TX+2XH)xTY: f1 f2 g1 g2 | f11..f14
 //        Y  TX x(TY+2): f3 f4 g3 g4 | f15..f18     XY (TX+2XH)x(TY+2): f7..f10
 //   * consumer threads interpolate in-plane (x, then y) from shared memory;
 //     the z-direction of the separable interpolation is a
@@ -46,32 +46,43 @@ namespace islbmk {
 
 constexpr int kMaxChunk = 64;   // longest marching chunk (its weights are staged in shared memory)
 
-template <typename ST, int TX_ = 32, int TY_ = 8>
+// SK = stencil kind: 0 destination-centred {j-1,j,j+1} (A2), 1 upwind {j-2,j-1,j} for c = +1 and
+// {j,j+1,j+2} for c = -1 (the A2 alternative): a 2-row y-halo, and the two halves of each z-stencil group (the
+// populations with e_z = +1 / -1) come from different slices (z and z+2).
+template <typename ST, int TX_ = 32, int TY_ = 8, int SK_ = 0>
 struct Tile3 {
-  static constexpr int TX = TX_, TY = TY_;
+  static constexpr int TX = TX_, TY = TY_, SK = SK_;
+  static constexpr int YH = SK ? 2 : 1;
   // TMA needs a 16-byte aligned box origin (measured: a misaligned origin raises an illegal-instruction
   // fault), so the x-halo is 16 bytes wide on each side: 2 nodes in fp64, 4 in fp32 storage
   static constexpr int XH = 16 / (int)sizeof(ST);
-  static constexpr int HX = TX + 2 * XH, HY = TY + 2;
+  static constexpr int HX = TX + 2 * XH, HY = TY + 2 * YH;
   // bytes of one plane inside a box of each shape
   static constexpr int P_XY = HX * HY * (int)sizeof(ST), P_X = HX * TY * (int)sizeof(ST);
   static constexpr int P_Y = TX * HY * (int)sizeof(ST), P_C = TX * TY * (int)sizeof(ST);
   // groups of a stage, in storage-plane order (each starts 128-byte aligned):
   //   emitted slice z:      C2 = f0 g0, XZ = f1 f2 g1 g2, YZ = f3 f4 g3 g4, XY = f7..f10
-  //   z-stencil slice (m):  C4 = f5 f6 g5 g6, XM = f11..f14, YM = f15..f18
+  //   z-stencil slice (m):  C4 = f5 g5 f6 g6, XM = f11..f14, YM = f15..f18  (first half of each: e_z = +1)
+  // a z-stencil group is two halves of two planes (e_z = +1, then e_z = -1); the upwind kernels load the halves with
+  // separate boxes, whose shared-memory destinations must be 128-byte aligned: H_* = distance between the halves
+  static constexpr int H_C = SK ? pad128(2 * P_C) : 2 * P_C, H_X = SK ? pad128(2 * P_X) : 2 * P_X;
+  static constexpr int H_Y = SK ? pad128(2 * P_Y) : 2 * P_Y;
   static constexpr int OFF_C2 = 0;
   static constexpr int OFF_XZ = pad128(OFF_C2 + 2 * P_C);
   static constexpr int OFF_YZ = pad128(OFF_XZ + 4 * P_X);
   static constexpr int OFF_XY = pad128(OFF_YZ + 4 * P_Y);
   static constexpr int OFF_C4 = pad128(OFF_XY + 4 * P_XY);
-  static constexpr int OFF_XM = pad128(OFF_C4 + 4 * P_C);
-  static constexpr int OFF_YM = pad128(OFF_XM + 4 * P_X);
-  static constexpr int STAGE_BYTES = pad128(OFF_YM + 4 * P_Y);
+  static constexpr int OFF_XM = pad128(OFF_C4 + 2 * H_C);
+  static constexpr int OFF_YM = pad128(OFF_XM + 2 * H_X);
+  static constexpr int STAGE_BYTES = pad128(OFF_YM + 2 * H_Y);
+  // byte offset of plane k (0..3) of a z-stencil group that starts at `off`, planes of `pbytes`, halves `half` apart
+  static __host__ __device__ constexpr int moff(int off, int k, int pbytes, int half) { return off + (k / 2) * half + (k % 2) * pbytes; }
   static constexpr int STAGES = sizeof(ST) == 4 ? ISLBM_Z_STAGES_F32 : 3;   // fp64: 3 x 62.7 KB is all that fits
   static constexpr int CONSUMER_WARPS = TX * TY / 32;
   static constexpr int THREADS = TX * TY;                // thread 0 doubles as the TMA producer
   static constexpr uint32_t Z_BYTES = 2u * P_C + 4u * P_X + 4u * P_Y + 4u * P_XY;   // planes of the emitted slice
   static constexpr uint32_t M_BYTES = 4u * P_C + 4u * P_X + 4u * P_Y;               // planes of the z-stencil slice
+  static constexpr uint32_t F_BYTES = M_BYTES / 2;                                  // ... of one half (SK = 1)
   static constexpr int BAR_OFF = STAGES * STAGE_BYTES;             // full[STAGES], empty[STAGES]
   static constexpr int W_OFF = BAR_OFF + 128;                       // marching-axis weights [sign][k][kMaxChunk]
   // fp32 storage: the in-plane-interpolated values of the three z-stencil slices live in shared memory, not in
@@ -86,6 +97,7 @@ struct Tile3 {
 // tensor maps over (x, y, z, plane): one per box shape
 struct Maps3 {
   CUtensorMap c2, c4, x, y, xy;
+  CUtensorMap x2, y2;   // two-plane boxes of the x / y shapes (upwind stencil: half a z-stencil group)
 };
 
 // ------------------------------ device helpers -----------------------------
@@ -211,6 +223,11 @@ __device__ __forceinline__ void store_node(ST *p, long long nn, const NT *f, con
 __device__ __forceinline__ int sbase(int j, int n) { return min(max(j - 1, 0), n - 3); }
 // does the stencil base move from layer j-1 to layer j?  (sbase(j) != sbase(j-1)  <=>  2 <= j <= n-2)
 __device__ __forceinline__ bool sbase_moves(int j, int n) { return j >= 2 && j <= n - 2; }
+// upwind stencil: base of the populations with c = +1 ({j-2,j-1,j}) and with c = -1 ({j,j+1,j+2}), clamped alike
+__device__ __forceinline__ int ubase_p(int j, int n) { return min(max(j - 2, 0), n - 3); }
+__device__ __forceinline__ int ubase_m(int j, int n) { return min(max(j, 0), n - 3); }
+__device__ __forceinline__ bool ubase_p_moves(int j, int n) { return j >= 3; }             // ubase_p(j) != ubase_p(j-1), j < n
+__device__ __forceinline__ bool ubase_m_moves(int j, int n) { return j >= 1 && j <= n - 3; }
 
 // One pipeline stage = the TMA boxes one z-iteration needs.  Issued by one thread.
 //   stage s < 2 : the first two slices of the z-stencil of the chunk's first slice;
@@ -219,54 +236,88 @@ template <typename T>
 __device__ __forceinline__ void issue_stage3(int s, int z0, int nz, int x0, int y0, unsigned char *stage0, uint64_t *full,
                                              uint64_t *empty, const Maps3 &mp, uint64_t pol) {
   const int st = s % T::STAGES;   // the caller knows the slot is free (initial fill, or it saw the last release)
-  int mslice = -1, zslice = -1;
-  if (s < 2) {
-    mslice = sbase(z0, nz) + s;
-  } else {
-    zslice = z0 + (s - 2);
-    if (s == 2 || sbase_moves(zslice, nz)) mslice = sbase(zslice, nz) + 2;
-  }
-  mbar_expect_tx(&full[st], (mslice >= 0 ? T::M_BYTES : 0u) + (zslice >= 0 ? T::Z_BYTES : 0u));
   unsigned char *sb = stage0 + (size_t)st * T::STAGE_BYTES;
   uint64_t *bar = &full[st];
-  const int xh = x0 - T::XH, yh = y0 - 1;
+  const int xh = x0 - T::XH, yh = y0 - T::YH;
+  int zslice = -1;
+  if constexpr (T::SK == 0) {
+    int mslice = -1;
+    if (s < 2) {
+      mslice = sbase(z0, nz) + s;
+    } else {
+      zslice = z0 + (s - 2);
+      if (s == 2 || sbase_moves(zslice, nz)) mslice = sbase(zslice, nz) + 2;
+    }
+    mbar_expect_tx(bar, (mslice >= 0 ? T::M_BYTES : 0u) + (zslice >= 0 ? T::Z_BYTES : 0u));
+    if (mslice >= 0) {
+      tma_load_4d(sb + T::OFF_C4, &mp.c4, bar, x0, y0, mslice, 14, pol);    // f5 g5 f6 g6
+      tma_load_4d(sb + T::OFF_XM, &mp.x, bar, xh, y0, mslice, 18, pol);     // f11..f14
+      tma_load_4d(sb + T::OFF_YM, &mp.y, bar, x0, yh, mslice, 22, pol);     // f15..f18
+    }
+  } else {
+    // the e_z = +1 halves (f5 g5 | f11 f12 | f15 f16) trail the emitted slice, the e_z = -1 halves lead it by two
+    int pslice = -1, mslice = -1;
+    if (s < 2) {
+      pslice = ubase_p(z0, nz) + s;
+      mslice = ubase_m(z0, nz) + s;
+    } else {
+      zslice = z0 + (s - 2);
+      if (s == 2 || ubase_p_moves(zslice, nz)) pslice = ubase_p(zslice, nz) + 2;
+      if (s == 2 || ubase_m_moves(zslice, nz)) mslice = ubase_m(zslice, nz) + 2;
+    }
+    mbar_expect_tx(bar, (pslice >= 0 ? T::F_BYTES : 0u) + (mslice >= 0 ? T::F_BYTES : 0u) + (zslice >= 0 ? T::Z_BYTES : 0u));
+    if (pslice >= 0) {
+      tma_load_4d(sb + T::OFF_C4, &mp.c2, bar, x0, y0, pslice, 14, pol);                   // f5 g5
+      tma_load_4d(sb + T::OFF_XM, &mp.x2, bar, xh, y0, pslice, 18, pol);                   // f11 f12
+      tma_load_4d(sb + T::OFF_YM, &mp.y2, bar, x0, yh, pslice, 22, pol);                   // f15 f16
+    }
+    if (mslice >= 0) {
+      tma_load_4d(sb + T::OFF_C4 + T::H_C, &mp.c2, bar, x0, y0, mslice, 16, pol);          // f6 g6
+      tma_load_4d(sb + T::OFF_XM + T::H_X, &mp.x2, bar, xh, y0, mslice, 20, pol);          // f13 f14
+      tma_load_4d(sb + T::OFF_YM + T::H_Y, &mp.y2, bar, x0, yh, mslice, 24, pol);          // f17 f18
+    }
+  }
   if (zslice >= 0) {
     tma_load_4d(sb + T::OFF_C2, &mp.c2, bar, x0, y0, zslice, 0, pol);     // f0 g0
     tma_load_4d(sb + T::OFF_XZ, &mp.x, bar, xh, y0, zslice, 2, pol);      // f1 f2 g1 g2
     tma_load_4d(sb + T::OFF_YZ, &mp.y, bar, x0, yh, zslice, 6, pol);      // f3 f4 g3 g4
     tma_load_4d(sb + T::OFF_XY, &mp.xy, bar, xh, yh, zslice, 10, pol);    // f7..f10
   }
-  if (mslice >= 0) {
-    tma_load_4d(sb + T::OFF_C4, &mp.c4, bar, x0, y0, mslice, 14, pol);    // f5 f6 g5 g6
-    tma_load_4d(sb + T::OFF_XM, &mp.x, bar, xh, y0, mslice, 18, pol);     // f11..f14
-    tma_load_4d(sb + T::OFF_YM, &mp.y, bar, x0, yh, mslice, 22, pol);     // f15..f18
-  }
 }
 
-// marching-axis weights of one layer as pairs: N = (weight of c=+1, weight of c=-1), S = the two swapped.
-// fp64: the chunk's weights sit in shared memory as scalars [sign][k][kMaxChunk] (a pair is just two registers);
-// fp32: both forms sit there as float2 [form][k][kMaxChunk], one 64-bit load each.
+// marching-axis weights of one layer as pairs.  Central stencil (SK = 0): A = (weight of c=+1, weight of c=-1),
+// B = the two swapped.  Upwind (SK = 1): A = (c=+1, c=+1), B = (c=-1, c=-1), because a pair then holds two
+// populations of the same sign.  fp64: the chunk's weights sit in shared memory as scalars [sign][k][kMaxChunk] (a
+// pair is just two registers); fp32: both forms sit there as float2 [form][k][kMaxChunk], one 64-bit load each.
+template <int SK>
 __device__ __forceinline__ void stage_march_weight(double *ws, int sk, int i, double w) { ws[sk * kMaxChunk + i] = w; }
+template <int SK>
 __device__ __forceinline__ void stage_march_weight(float *ws, int sk, int i, double w) {
-  // sk = sign * 3 + k; lane a of N[k] and lane b of S[k] take sign 1, the other two lanes sign 0
-  const int sign = sk / 3, k = sk - 3 * sign;
-  ws[((0 * 3 + k) * kMaxChunk + i) * 2 + (sign ? 0 : 1)] = (float)w;
-  ws[((1 * 3 + k) * kMaxChunk + i) * 2 + (sign ? 1 : 0)] = (float)w;
+  const int sign = sk / 3, k = sk - 3 * sign;   // sk = sign * 3 + k
+  if constexpr (SK == 0) {
+    ws[((0 * 3 + k) * kMaxChunk + i) * 2 + (sign ? 0 : 1)] = (float)w;
+    ws[((1 * 3 + k) * kMaxChunk + i) * 2 + (sign ? 1 : 0)] = (float)w;
+  } else {
+    ws[(((sign ? 0 : 1) * 3 + k) * kMaxChunk + i) * 2 + 0] = (float)w;
+    ws[(((sign ? 0 : 1) * 3 + k) * kMaxChunk + i) * 2 + 1] = (float)w;
+  }
 }
-__device__ __forceinline__ void load_march_weights(const double *ws, int i, Pr<double> (&N)[3], Pr<double> (&S)[3]) {
+template <int SK>
+__device__ __forceinline__ void load_march_weights(const double *ws, int i, Pr<double> (&A)[3], Pr<double> (&B)[3]) {
 #pragma unroll
   for (int k = 0; k < 3; ++k) {
     const double w1 = ws[(3 + k) * kMaxChunk + i], w0 = ws[k * kMaxChunk + i];
-    N[k] = mkpr(w1, w0);
-    S[k] = mkpr(w0, w1);
+    A[k] = SK == 0 ? mkpr(w1, w0) : mkpr(w1, w1);
+    B[k] = SK == 0 ? mkpr(w0, w1) : mkpr(w0, w0);
   }
 }
-__device__ __forceinline__ void load_march_weights(const float *ws, int i, Pr<float> (&N)[3], Pr<float> (&S)[3]) {
+template <int SK>
+__device__ __forceinline__ void load_march_weights(const float *ws, int i, Pr<float> (&A)[3], Pr<float> (&B)[3]) {
   const float2 *w2 = reinterpret_cast<const float2 *>(ws);
 #pragma unroll
   for (int k = 0; k < 3; ++k) {
-    N[k].v = w2[k * kMaxChunk + i];
-    S[k].v = w2[(3 + k) * kMaxChunk + i];
+    A[k].v = w2[k * kMaxChunk + i];
+    B[k].v = w2[(3 + k) * kMaxChunk + i];
   }
 }
 
@@ -276,8 +327,8 @@ __device__ __forceinline__ void load_march_weights(const float *ws, int i, Pr<fl
 // (lane a has e_z = +1 in pairs 0, 1, 2, 4 and e_z = -1 in pairs 3 and 5, which take the swapped z-weights)
 #define ISLBM_LOAD_M3(S)                                                                     \
   do {                                                                                       \
-    S[0] = mkpr((AT)PC4(0)[0], (AT)PC4(1)[0]);              /* f5, f6 */             \
-    S[1] = mkpr((AT)PC4(2)[0], (AT)PC4(3)[0]);              /* g5, g6 */             \
+    S[0] = mkpr((AT)PC4(0)[0], (AT)PC4(2)[0]);              /* f5, f6 */             \
+    S[1] = mkpr((AT)PC4(1)[0], (AT)PC4(3)[0]);              /* g5, g6 */             \
     S[2] = ptap3(PXM(0), PXM(3), 1, wxN);                   /* f11 (+x), f14 (-x) */ \
     S[3] = ptap3(PXM(2), PXM(1), 1, wxN);                   /* f13 (+x), f12 (-x) */ \
     S[4] = ptap3(PYM(0), PYM(3), T::TX, wyN);               /* f15 (+y), f18 (-y) */ \
@@ -350,7 +401,7 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
   }
   for (int i = (int)threadIdx.x - 32; i >= 0 && i < 6 * (z1 - z0); i += T::THREADS - 32) {   // warps 1..: warp 0 is waiting above
     const int sk = i / (z1 - z0), zi = i - sk * (z1 - z0);
-    stage_march_weight(wzs, sk, zi, __ldg(wrow(m, 2, sk / 3, sk % 3) + z0 + zi));
+    stage_march_weight<0>(wzs, sk, zi, __ldg(wrow(m, 2, sk / 3, sk % 3) + z0 + zi));
   }
   pdl_wait();
   __syncthreads();
@@ -412,9 +463,9 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
 #define PXZ(k) (sbx + (T::OFF_XZ + (k) * T::P_X) / ES)
 #define PYZ(k) (sby + (T::OFF_YZ + (k) * T::P_Y) / ES)
 #define PXY(k) (sbxy + (T::OFF_XY + (k) * T::P_XY) / ES)
-#define PC4(k) (sbc + (T::OFF_C4 + (k) * T::P_C) / ES)
-#define PXM(k) (sbx + (T::OFF_XM + (k) * T::P_X) / ES)
-#define PYM(k) (sby + (T::OFF_YM + (k) * T::P_Y) / ES)
+#define PC4(k) (sbc + T::moff(T::OFF_C4, k, T::P_C, T::H_C) / ES)
+#define PXM(k) (sbx + T::moff(T::OFF_XM, k, T::P_X, T::H_X) / ES)
+#define PYM(k) (sby + T::moff(T::OFF_YM, k, T::P_Y, T::H_Y) / ES)
     if (!EARLY && threadIdx.x == 0 && s + T::STAGES - 1 < nstage) {
       const int sn = s + T::STAGES - 1;
       if (sn >= T::STAGES) mbar_wait(&empty[sn % T::STAGES], ((uint32_t)(sn / T::STAGES) & 1u) ^ 1u);
@@ -465,7 +516,7 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
 
     if (has_emit) {
       Pr<AT> wzN[3], wzS[3];
-      load_march_weights(wzs, s - 2, wzN, wzS);
+      load_march_weights<0>(wzs, s - 2, wzN, wzS);
       if constexpr (T::S_IN_SMEM) {
         // ascending z = slots (newest+1, newest+2, newest) mod 3; the newest slice is still in registers unless the
         // stencil base did not move (first / last two slices of the mesh)
@@ -506,18 +557,251 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
   }
 }
 
+// ------------------------------ the kernel, upwind stencil -----------------------------------------------------
+// Same march with the A2-alternative stencil {j-2,j-1,j} (c = +1) / {j,j+1,j+2} (c = -1) (islbm_set_stencil(h, 1);
+// SURVEY.md 8(f)-3).  What changes against k_step_zmarch: the two lanes of a pair read different
+// windows (lane a, the c = +1 population, starts two nodes upstream; lane b, c = -1, at the node itself), the y-halo
+// is two rows, and the z-stencil state splits into two families of three pairs each:
+//   family P (e_z = +1): (f5, g5) (f11, f12) (f15, f16), slices {z-2, z-1, z};
+//   family M (e_z = -1): (f6, g6) (f13, f14) (f17, f18), slices {z, z+1, z+2};
+// each with its own rotating register sets (fp64) or shared-memory slots (fp32 storage) and its own stencil-base
+// bookkeeping at the ends of the axis.  Both lanes of a family pair take the z-weights of the same sign.
+#define ISLBM_LOAD_U3(S, H)                                                                           \
+  do {                                                                                                \
+    S[0] = mkpr((AT)PC4(2 * H)[o_c], (AT)PC4(2 * H + 1)[o_c]);              /* f5 g5 | f6 g6 */       \
+    S[1] = ptap3(PXM(2 * H) + o_xa, PXM(2 * H + 1) + o_xb, 1, wxN);         /* f11 f12 | f13 f14 */   \
+    S[2] = ptap3(PYM(2 * H) + o_ya, PYM(2 * H + 1) + o_yb, T::TX, wyN);     /* f15 f16 | f17 f18 */   \
+  } while (0)
+#define ISLBM_ZCOMB_U3(W, P0, P1, P2, F0, G0, F1A, F1B, F2A, F2B)   \
+  do {                                                              \
+    const Pr<AT> q0 = pcomb3(W, P0[0], P1[0], P2[0]);               \
+    const Pr<AT> q1 = pcomb3(W, P0[1], P1[1], P2[1]);               \
+    const Pr<AT> q2 = pcomb3(W, P0[2], P1[2], P2[2]);               \
+    f[F0] = lane_a(q0);  g[G0] = lane_b(q0);                        \
+    f[F1A] = lane_a(q1); f[F1B] = lane_b(q1);                       \
+    f[F2A] = lane_a(q2); f[F2B] = lane_b(q2);                       \
+  } while (0)
+
+template <typename ST, int TX, int TY>
+__global__ void __launch_bounds__(TX * TY, TX * TY <= 128 ? 3 : (TX * TY <= 192 ? 2 : 1))
+k_step_zmarch_up(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const ST *__restrict__ src,
+                 ST *__restrict__ dst, int zchunk, int load_policy, int store_policy, int late_fill) {
+  using T = Tile3<ST, TX, TY, 1>;
+  using AT = typename Acc<ST>::type;
+  constexpr bool EARLY = sizeof(ST) == 4;   // ring refill policy: see k_step_zmarch
+  extern __shared__ __align__(128) unsigned char smem_raw[];
+  unsigned char *stage0 = smem_raw;
+  uint64_t *full = reinterpret_cast<uint64_t *>(smem_raw + T::BAR_OFF);
+  uint64_t *empty = full + T::STAGES;
+  AT *wzs = reinterpret_cast<AT *>(smem_raw + T::W_OFF);
+  int *claim = reinterpret_cast<int *>(smem_raw + T::BAR_OFF + 2 * T::STAGES * 8);
+  pdl_launch_dependents();
+
+  const int x0 = blockIdx.x * T::TX, y0 = min((int)blockIdx.y * T::TY, max(m.ny - T::TY, 0));
+  const int z0 = m.em_lo + blockIdx.z * zchunk, z1 = min(z0 + zchunk, m.em_hi);
+  const int nstage = 2 + (z1 - z0);
+  const uint64_t lpol = make_policy(load_policy);
+  const uint64_t spol = make_policy(store_policy);
+  if (threadIdx.x == 0) {
+    for (int s = 0; s < T::STAGES; ++s) {
+      mbar_init(&full[s], 1);
+      mbar_init(&empty[s], T::CONSUMER_WARPS);
+      claim[s] = 0;
+    }
+    fence_barrier_init();
+    tma_prefetch_desc(&mp.c2);
+    tma_prefetch_desc(&mp.x);
+    tma_prefetch_desc(&mp.y);
+    tma_prefetch_desc(&mp.xy);
+    tma_prefetch_desc(&mp.x2);
+    tma_prefetch_desc(&mp.y2);
+    if (!late_fill) {
+      pdl_wait();
+      for (int s = 0; s < T::STAGES - (EARLY ? 0 : 1) && s < nstage; ++s)
+        issue_stage3<T>(s, z0, m.nz, x0, y0, stage0, full, empty, mp, lpol);
+    }
+  }
+  for (int i = (int)threadIdx.x - 32; i >= 0 && i < 6 * (z1 - z0); i += T::THREADS - 32) {
+    const int sk = i / (z1 - z0), zi = i - sk * (z1 - z0);
+    stage_march_weight<1>(wzs, sk, zi, __ldg(wrow(m, 2, sk / 3, sk % 3) + z0 + zi));
+  }
+  pdl_wait();
+  __syncthreads();
+  if (late_fill && threadIdx.x == 0) {
+    for (int s = 0; s < T::STAGES - (EARLY ? 0 : 1) && s < nstage; ++s)
+      issue_stage3<T>(s, z0, m.nz, x0, y0, stage0, full, empty, mp, lpol);
+  }
+
+  const int tx = threadIdx.x % T::TX, ty = threadIdx.x / T::TX;
+  const int x = x0 + tx, y = y0 + ty;
+  const bool valid = x < m.nx && y < m.ny;
+  WallFlags wf;
+  wf.lo[0] = valid && x == 0;  wf.hi[0] = valid && x == m.nx - 1;
+  wf.lo[1] = valid && y == 0;  wf.hi[1] = valid && y == m.ny - 1;
+  const bool wall_xy = wf.lo[0] | wf.hi[0] | wf.lo[1] | wf.hi[1];
+  // first stencil node of lane a (c = +1) / lane b (c = -1) inside the boxes: columns of the x-haloed shapes, rows of
+  // the y-haloed ones (a thread outside the mesh reads inside the box all the same; its results are not stored)
+  const int col_a = ubase_p(min(x, m.nx - 1), m.nx) - x0 + T::XH, col_b = ubase_m(min(x, m.nx - 1), m.nx) - x0 + T::XH;
+  const int row_a = ubase_p(min(y, m.ny - 1), m.ny) - y0 + T::YH, row_b = ubase_m(min(y, m.ny - 1), m.ny) - y0 + T::YH;
+  const int o_xa = ty * T::HX + col_a, o_xb = ty * T::HX + col_b;                 // x-stencil, taps +0,+1,+2
+  const int o_ya = row_a * T::TX + tx, o_yb = row_b * T::TX + tx;                 // y-stencil, taps +0,+TX,+2TX
+  const int o_aa = row_a * T::HX + col_a, o_bb = row_b * T::HX + col_b;           // 3x3 stencils, pitch HX
+  const int o_ba = row_b * T::HX + col_a, o_ab = row_a * T::HX + col_b;           // (row of -y, column of +x), (+y, -x)
+  const int o_c = ty * T::TX + tx;
+  Pr<AT> wxN[3], wyN[3], wyS[3];
+#pragma unroll
+  for (int k = 0; k < 3; ++k) {
+    const AT x1 = valid ? (AT)__ldg(wrow(m, 0, 1, k) + x) : (AT)0, x0w = valid ? (AT)__ldg(wrow(m, 0, 0, k) + x) : (AT)0;
+    const AT y1 = valid ? (AT)__ldg(wrow(m, 1, 1, k) + y) : (AT)0, y0w = valid ? (AT)__ldg(wrow(m, 1, 0, k) + y) : (AT)0;
+    wxN[k] = mkpr(x1, x0w);
+    wyN[k] = mkpr(y1, y0w);
+    wyS[k] = mkpr(y0w, y1);
+  }
+  const long long plane = (long long)m.nxp * m.ny;
+  long long c = (long long)z0 * plane + (long long)y * m.nxp + x;
+
+  // per family three sets; `newest_*` names the one written last, ascending z = (newest+1, newest+2, newest) mod 3
+  Pr<AT> P0[3], P1[3], P2[3], M0[3], M1[3], M2[3];
+  int newest_p = 2, newest_m = 2;
+  Pr<AT> *ssm = reinterpret_cast<Pr<AT> *>(smem_raw + T::S_OFF) + threadIdx.x;   // S_IN_SMEM: [family][slot][pair][thread]
+  constexpr int SSLOT = 3 * T::THREADS;
+
+#pragma unroll 1
+  for (int s = 0; s < nstage; ++s) {
+    const int st = s % T::STAGES;
+    const uint32_t ph = (uint32_t)(s / T::STAGES) & 1u;
+    const int z = z0 + (s - 2);
+    const bool has_emit = s >= 2;
+    const bool mov_p = s <= 2 || ubase_p_moves(z, m.nz), mov_m = s <= 2 || ubase_m_moves(z, m.nz);
+    const ST *sb = reinterpret_cast<const ST *>(stage0 + (size_t)st * T::STAGE_BYTES);
+    constexpr int ES = (int)sizeof(ST);
+#define PC2(k) (sb + (T::OFF_C2 + (k) * T::P_C) / ES)
+#define PXZ(k) (sb + (T::OFF_XZ + (k) * T::P_X) / ES)
+#define PYZ(k) (sb + (T::OFF_YZ + (k) * T::P_Y) / ES)
+#define PXY(k) (sb + (T::OFF_XY + (k) * T::P_XY) / ES)
+#define PC4(k) (sb + T::moff(T::OFF_C4, k, T::P_C, T::H_C) / ES)
+#define PXM(k) (sb + T::moff(T::OFF_XM, k, T::P_X, T::H_X) / ES)
+#define PYM(k) (sb + T::moff(T::OFF_YM, k, T::P_Y, T::H_Y) / ES)
+    if (!EARLY && threadIdx.x == 0 && s + T::STAGES - 1 < nstage) {
+      const int sn = s + T::STAGES - 1;
+      if (sn >= T::STAGES) mbar_wait(&empty[sn % T::STAGES], ((uint32_t)(sn / T::STAGES) & 1u) ^ 1u);
+      issue_stage3<T>(sn, z0, m.nz, x0, y0, stage0, full, empty, mp, lpol);
+    }
+    __syncwarp();
+    mbar_wait(&full[st], ph);
+
+    if (mov_p) {
+      newest_p = newest_p == 2 ? 0 : newest_p + 1;
+      if constexpr (T::S_IN_SMEM) {
+        ISLBM_LOAD_U3(P2, 0);
+#pragma unroll
+        for (int k = 0; k < 3; ++k) ssm[newest_p * SSLOT + k * T::THREADS] = P2[k];
+      } else {
+        if (newest_p == 0) ISLBM_LOAD_U3(P0, 0);
+        else if (newest_p == 1) ISLBM_LOAD_U3(P1, 0);
+        else ISLBM_LOAD_U3(P2, 0);
+      }
+    }
+    if (mov_m) {
+      newest_m = newest_m == 2 ? 0 : newest_m + 1;
+      if constexpr (T::S_IN_SMEM) {
+        ISLBM_LOAD_U3(M2, 1);
+#pragma unroll
+        for (int k = 0; k < 3; ++k) ssm[(3 + newest_m) * SSLOT + k * T::THREADS] = M2[k];
+      } else {
+        if (newest_m == 0) ISLBM_LOAD_U3(M0, 1);
+        else if (newest_m == 1) ISLBM_LOAD_U3(M1, 1);
+        else ISLBM_LOAD_U3(M2, 1);
+      }
+    }
+
+    AT f[19], g[7];
+    if (has_emit) {
+      f[0] = PC2(0)[o_c];
+      g[0] = PC2(1)[o_c];
+      const Pr<AT> p1 = ptap3(PXZ(0) + o_xa, PXZ(1) + o_xb, 1, wxN);                 // f1 (+x), f2 (-x)
+      const Pr<AT> p2 = ptap3(PXZ(2) + o_xa, PXZ(3) + o_xb, 1, wxN);                 // g1, g2
+      const Pr<AT> p3 = ptap3(PYZ(0) + o_ya, PYZ(1) + o_yb, T::TX, wyN);             // f3 (+y), f4 (-y)
+      const Pr<AT> p4 = ptap3(PYZ(2) + o_ya, PYZ(3) + o_yb, T::TX, wyN);             // g3, g4
+      const Pr<AT> p5 = ptap9(PXY(0) + o_aa, PXY(3) + o_bb, T::HX, wxN, wyN);        // f7 (+x,+y), f10 (-x,-y)
+      const Pr<AT> p6 = ptap9(PXY(2) + o_ba, PXY(1) + o_ab, T::HX, wxN, wyS);        // f9 (+x,-y), f8 (-x,+y)
+      f[1] = lane_a(p1); f[2] = lane_b(p1);
+      g[1] = lane_a(p2); g[2] = lane_b(p2);
+      f[3] = lane_a(p3); f[4] = lane_b(p3);
+      g[3] = lane_a(p4); g[4] = lane_b(p4);
+      f[7] = lane_a(p5); f[10] = lane_b(p5);
+      f[9] = lane_a(p6); f[8] = lane_b(p6);
+    }
+    __syncwarp();
+    if ((threadIdx.x & 31) == 0) {
+      if (!EARLY) mbar_arrive(&empty[st]);
+      else if (mbar_arrive_is_last(&empty[st]) && s + T::STAGES < nstage &&
+               atomicCAS(&claim[st], s / T::STAGES, s / T::STAGES + 1) == s / T::STAGES)
+        issue_stage3<T>(s + T::STAGES, z0, m.nz, x0, y0, stage0, full, empty, mp, lpol);
+    }
+
+    if (has_emit) {
+      Pr<AT> wzA[3], wzB[3];    // (c=+1, c=+1) for family P, (c=-1, c=-1) for family M
+      load_march_weights<1>(wzs, s - 2, wzA, wzB);
+      if constexpr (T::S_IN_SMEM) {
+        const Pr<AT> *pp0 = ssm + (newest_p == 2 ? 0 : newest_p + 1) * SSLOT, *pp1 = ssm + (newest_p == 0 ? 2 : newest_p - 1) * SSLOT;
+        const Pr<AT> *pm0 = ssm + (3 + (newest_m == 2 ? 0 : newest_m + 1)) * SSLOT, *pm1 = ssm + (3 + (newest_m == 0 ? 2 : newest_m - 1)) * SSLOT;
+#pragma unroll
+        for (int k = 0; k < 3; ++k) {
+          P0[k] = pp0[k * T::THREADS];
+          P1[k] = pp1[k * T::THREADS];
+          M0[k] = pm0[k * T::THREADS];
+          M1[k] = pm1[k * T::THREADS];
+        }
+        if (!mov_p) {
+#pragma unroll
+          for (int k = 0; k < 3; ++k) P2[k] = ssm[newest_p * SSLOT + k * T::THREADS];
+        }
+        if (!mov_m) {
+#pragma unroll
+          for (int k = 0; k < 3; ++k) M2[k] = ssm[(3 + newest_m) * SSLOT + k * T::THREADS];
+        }
+        ISLBM_ZCOMB_U3(wzA, P0, P1, P2, 5, 5, 11, 12, 15, 16);
+        ISLBM_ZCOMB_U3(wzB, M0, M1, M2, 6, 6, 13, 14, 17, 18);
+      } else {
+        if (newest_p == 0) ISLBM_ZCOMB_U3(wzA, P1, P2, P0, 5, 5, 11, 12, 15, 16);
+        else if (newest_p == 1) ISLBM_ZCOMB_U3(wzA, P2, P0, P1, 5, 5, 11, 12, 15, 16);
+        else ISLBM_ZCOMB_U3(wzA, P0, P1, P2, 5, 5, 11, 12, 15, 16);
+        if (newest_m == 0) ISLBM_ZCOMB_U3(wzB, M1, M2, M0, 6, 6, 13, 14, 17, 18);
+        else if (newest_m == 1) ISLBM_ZCOMB_U3(wzB, M2, M0, M1, 6, 6, 13, 14, 17, 18);
+        else ISLBM_ZCOMB_U3(wzB, M0, M1, M2, 6, 6, 13, 14, 17, 18);
+      }
+      wf.lo[2] = z == 0 && m.wall_mlo;
+      wf.hi[2] = z == m.nz - 1 && m.wall_mhi;
+      if (valid && (wall_xy | wf.lo[2] | wf.hi[2])) wall_fix_node<3>(f, g, wf, src + c, m.nnp, m);
+      constexpr bool DEV = Store<ST, 3>::kBiased;
+      collide_node<DEV>(f, g, np);
+      if (valid) store_node<3, DEV>(dst + c, m.nnp, f, g, spol, std::make_integer_sequence<int, 26>{});
+      c += plane;
+    }
+#undef PC2
+#undef PXZ
+#undef PYZ
+#undef PXY
+#undef PC4
+#undef PXM
+#undef PYM
+  }
+}
+
 // ------------------------------ host side ---------------------------------
 struct Plan3 {
   bool available = false;
   Maps3 maps[2];            // per ping-pong buffer
   int zchunk = 32;
-  int shape = 0;            // tile shape index: 0 32x8, 1 64x4, 2 128x2
+  int shape = 0;            // tile shape index (Tuning::shape3d)
+  int sk = 0;               // stencil kind the plan was built for: 0 central, 1 upwind
   char why_not[96] = "";
 };
 
-template <typename ST, int TX, int TY>
-inline bool plan3_maps(Plan3 &p, const int *n, int nxp, void *buf0, void *buf1, const Tuning &tn) {
-  using T = Tile3<ST, TX, TY>;
+template <typename ST, int TX, int TY, int SK>
+inline bool plan3_setup(Plan3 &p, const int *n, int nxp, void *buf0, void *buf1, const Tuning &tn) {
+  using T = Tile3<ST, TX, TY, SK>;
   p.available = false;
   auto no = [&](const char *why) { snprintf(p.why_not, sizeof p.why_not, "%s", why); return false; };
   if (n[0] < 3 || n[1] < 3 || n[2] < 3) return no("tiled kernel: n >= 3");
@@ -532,13 +816,23 @@ inline bool plan3_maps(Plan3 &p, const int *n, int nxp, void *buf0, void *buf1, 
   const long long dims[4] = {n[0], n[1], n[2], 26};
   const int b_c2[4] = {T::TX, T::TY, 1, 2}, b_c4[4] = {T::TX, T::TY, 1, 4}, b_x[4] = {T::HX, T::TY, 1, 4};
   const int b_y[4] = {T::TX, T::HY, 1, 4}, b_xy[4] = {T::HX, T::HY, 1, 4};
+  const int b_x2[4] = {T::HX, T::TY, 1, 2}, b_y2[4] = {T::TX, T::HY, 1, 2};
   for (int i = 0; i < 2; ++i) {
     if (!make_map(&p.maps[i].c2, bufs[i], eb, 4, dims, b_c2, tn.l2promo, nxp) ||
         !make_map(&p.maps[i].c4, bufs[i], eb, 4, dims, b_c4, tn.l2promo, nxp) ||
         !make_map(&p.maps[i].x, bufs[i], eb, 4, dims, b_x, tn.l2promo, nxp) ||
         !make_map(&p.maps[i].y, bufs[i], eb, 4, dims, b_y, tn.l2promo, nxp) ||
-        !make_map(&p.maps[i].xy, bufs[i], eb, 4, dims, b_xy, tn.l2promo, nxp))
+        !make_map(&p.maps[i].xy, bufs[i], eb, 4, dims, b_xy, tn.l2promo, nxp) ||
+        !make_map(&p.maps[i].x2, bufs[i], eb, 4, dims, b_x2, tn.l2promo, nxp) ||
+        !make_map(&p.maps[i].y2, bufs[i], eb, 4, dims, b_y2, tn.l2promo, nxp))
       return no("cuTensorMapEncodeTiled failed");
+  }
+  cudaError_t e;
+  if constexpr (SK == 0) e = cudaFuncSetAttribute(k_step_zmarch<ST, TX, TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM_BYTES);
+  else e = cudaFuncSetAttribute(k_step_zmarch_up<ST, TX, TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM_BYTES);
+  if (e != cudaSuccess) {
+    cudaGetLastError();
+    return no("cudaFuncSetAttribute failed");
   }
   // z-chunks (measured, profiles/): short chunks win — neighbouring CTAs stay in step, so the halo overlap is found in
   // L2, and the tail is fine-grained.  Meshes with at least one CTA per SM in every z-layer of tiles take 16 slices (the
@@ -561,54 +855,66 @@ inline bool plan3_maps(Plan3 &p, const int *n, int nxp, void *buf0, void *buf1, 
   return true;
 }
 
-template <typename ST, int TX, int TY>
-inline bool plan3_setup(Plan3 &p, const int *n, int nxp, void *buf0, void *buf1, const Tuning &tn) {
-  using T = Tile3<ST, TX, TY>;
-  if (!plan3_maps<ST, TX, TY>(p, n, nxp, buf0, buf1, tn)) return false;
-  if (cudaFuncSetAttribute(k_step_zmarch<ST, TX, TY>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)T::SMEM_BYTES) != cudaSuccess) {
-    cudaGetLastError();
-    p.available = false;
-    snprintf(p.why_not, sizeof p.why_not, "cudaFuncSetAttribute failed");
-    return false;
-  }
-  return true;
-}
-
-template <typename ST, int TX, int TY>
+template <typename ST, int TX, int TY, int SK>
 inline void launch3_shape(const Plan3 &p, const int *n, const DevMesh &m, const NodeParams &np, int cur, void *const *buf,
                           const Tuning &tn, cudaStream_t stream) {
-  using T = Tile3<ST, TX, TY>;
+  using T = Tile3<ST, TX, TY, SK>;
   dim3 grid((n[0] + T::TX - 1) / T::TX, (n[1] + T::TY - 1) / T::TY, (m.em_hi - m.em_lo + p.zchunk - 1) / p.zchunk);
-  launch_step(k_step_zmarch<ST, TX, TY>, grid, dim3(T::THREADS), T::SMEM_BYTES, stream, tn.pdl != 0, p.maps[cur], m, np,
-              (const ST *)buf[cur], (ST *)buf[1 - cur], p.zchunk, tn.load_policy, tn.store_policy, tn.fill == 2 ? 1 : 0);
+  if constexpr (SK == 0)
+    launch_step(k_step_zmarch<ST, TX, TY>, grid, dim3(T::THREADS), T::SMEM_BYTES, stream, tn.pdl != 0, p.maps[cur], m, np,
+                (const ST *)buf[cur], (ST *)buf[1 - cur], p.zchunk, tn.load_policy, tn.store_policy, tn.fill == 2 ? 1 : 0);
+  else
+    launch_step(k_step_zmarch_up<ST, TX, TY>, grid, dim3(T::THREADS), T::SMEM_BYTES, stream, tn.pdl != 0, p.maps[cur], m, np,
+                (const ST *)buf[cur], (ST *)buf[1 - cur], p.zchunk, tn.load_policy, tn.store_policy, tn.fill == 2 ? 1 : 0);
 }
 
+// sk = 0: the destination-centred stencil; 1: the upwind stencil (islbm_set_stencil)
 template <typename ST>
-inline bool plan3_create(Plan3 &p, const int *n, int nxp, void *buf0, void *buf1, const Tuning &tn) {
+inline bool plan3_create(Plan3 &p, const int *n, int nxp, void *buf0, void *buf1, const Tuning &tn, int sk) {
   // tile shape (x by y nodes per CTA).  fp64 storage: 32x8 (254 registers, one CTA per SM; DRAM-bound).  fp32 storage
-  // is bound by instruction issue and latency at 8 warps per SM, so it takes smaller CTAs, capped at 168 registers by
-  // their launch bounds: 32x6 (two CTAs = 12 warps per SM) or 32x4 (three CTAs) on short y-axes (profiles/attempts.md).
+  // is bound by the latency of the fp64 collision at the 12 warps per SM its 168 registers allow: 32x6 CTAs (two per
+  // SM) or 32x4 (three per SM) on short y-axes (profiles/attempts.md).  The upwind kernels exist in these three shapes.
   int shape = tn.shape3d;
-  if (shape == 0) shape = sizeof(ST) == 4 ? (n[1] >= 192 ? 3 : 4) : 5;
+  if (shape == 0 || (sk && shape != 3 && shape != 4)) shape = sizeof(ST) == 4 ? (n[1] >= 192 ? 3 : 4) : 5;
   p.shape = shape;
+  p.sk = sk;
+  if (sk) {
+    if constexpr (sizeof(ST) == 4) {
+      if (shape == 4) return plan3_setup<ST, 32, 4, 1>(p, n, nxp, buf0, buf1, tn);
+      p.shape = 3;
+      return plan3_setup<ST, 32, 6, 1>(p, n, nxp, buf0, buf1, tn);
+    } else {
+      p.shape = 5;
+      return plan3_setup<ST, 32, 8, 1>(p, n, nxp, buf0, buf1, tn);
+    }
+  }
   switch (shape) {
-    case 1: return plan3_setup<ST, 64, 4>(p, n, nxp, buf0, buf1, tn);
-    case 2: return plan3_setup<ST, 128, 2>(p, n, nxp, buf0, buf1, tn);
-    case 3: return plan3_setup<ST, 32, 6>(p, n, nxp, buf0, buf1, tn);
-    case 4: return plan3_setup<ST, 32, 4>(p, n, nxp, buf0, buf1, tn);
-    default: p.shape = 5; return plan3_setup<ST, 32, 8>(p, n, nxp, buf0, buf1, tn);
+    case 1: return plan3_setup<ST, 64, 4, 0>(p, n, nxp, buf0, buf1, tn);
+    case 2: return plan3_setup<ST, 128, 2, 0>(p, n, nxp, buf0, buf1, tn);
+    case 3: return plan3_setup<ST, 32, 6, 0>(p, n, nxp, buf0, buf1, tn);
+    case 4: return plan3_setup<ST, 32, 4, 0>(p, n, nxp, buf0, buf1, tn);
+    default: p.shape = 5; return plan3_setup<ST, 32, 8, 0>(p, n, nxp, buf0, buf1, tn);
   }
 }
 
 template <typename ST>
 inline cudaError_t launch3(const Plan3 &p, const int *n, const DevMesh &m, const NodeParams &np, int cur, void *const *buf,
                            const Tuning &tn, cudaStream_t stream) {
+  if (p.sk) {
+    if constexpr (sizeof(ST) == 4) {
+      if (p.shape == 4) launch3_shape<ST, 32, 4, 1>(p, n, m, np, cur, buf, tn, stream);
+      else launch3_shape<ST, 32, 6, 1>(p, n, m, np, cur, buf, tn, stream);
+    } else {
+      launch3_shape<ST, 32, 8, 1>(p, n, m, np, cur, buf, tn, stream);
+    }
+    return cudaPeekAtLastError();
+  }
   switch (p.shape) {
-    case 1: launch3_shape<ST, 64, 4>(p, n, m, np, cur, buf, tn, stream); break;
-    case 2: launch3_shape<ST, 128, 2>(p, n, m, np, cur, buf, tn, stream); break;
-    case 3: launch3_shape<ST, 32, 6>(p, n, m, np, cur, buf, tn, stream); break;
-    case 4: launch3_shape<ST, 32, 4>(p, n, m, np, cur, buf, tn, stream); break;
-    default: launch3_shape<ST, 32, 8>(p, n, m, np, cur, buf, tn, stream);
+    case 1: launch3_shape<ST, 64, 4, 0>(p, n, m, np, cur, buf, tn, stream); break;
+    case 2: launch3_shape<ST, 128, 2, 0>(p, n, m, np, cur, buf, tn, stream); break;
+    case 3: launch3_shape<ST, 32, 6, 0>(p, n, m, np, cur, buf, tn, stream); break;
+    case 4: launch3_shape<ST, 32, 4, 0>(p, n, m, np, cur, buf, tn, stream); break;
+    default: launch3_shape<ST, 32, 8, 0>(p, n, m, np, cur, buf, tn, stream);
   }
   return cudaPeekAtLastError();
 }

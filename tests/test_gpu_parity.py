@@ -225,28 +225,84 @@ def test_set_populations_host_equals_device_path(islbm, dim, ns, prec):
     assert b.steady_residual() == (1.0, 1.0)                 # the upload invalidated the Eq. 30 snapshot
 
 
-@pytest.mark.parametrize("dim,ns", [(2, (70, 45, 1)), (2, (3, 5, 1)), (3, (37, 21, 19)), (3, (4, 3, 6))])
-def test_upwind_stencil_parity(islbm, dim, ns):
-    """A2 alternative ({j-2,j-1,j} / {j,j+1,j+2}): generic kernel against the oracle's table-driven stream."""
-    coords, delta = ragged_coords(dim, ns, (1.4, 1.2, 1.3))
+@pytest.mark.parametrize("name,dim,ns,st", CASES_1STEP, ids=[c[0] for c in CASES_1STEP])
+def test_upwind_stencil_parity(islbm, name, dim, ns, st):
+    """A2 alternative ({j-2,j-1,j} for c = +1, {j,j+1,j+2} for c = -1): the TMA kernels of that
+    stencil (2-row halo, split z-stencil groups) and the generic kernel against the oracle's table-driven stream, on
+    the same 20 meshes and tuning variants as the central stencil, 1e-12 after one step and 3e-12 after three."""
+    coords, delta = ragged_coords(dim, ns, st)
     H_lu = (coords[1][-1] - coords[1][0] + delta) / delta
     sim, orc = pair(islbm, coords, delta, Ra=0.71 * (0.1 * H_lu / 0.03) ** 2)
     sim.set_stencil(1)
     orc.set_stencil(1)
-    assert sim.kernel_name == "generic_global"
+    assert sim.kernel_name in ("tiled_ymarch_tma_upwind", "tiled_zmarch_tma_upwind")
     with pytest.raises(islbm.IslbmError):
-        sim.set_kernel(islbm.KERNEL_TILED)
-    f0, g0 = inputs.random_state(orc.shape, orc.qf, orc.qg, seed=3, amp=0.05)
+        sim.set_kernel(islbm.KERNEL_UNIFORM_SHIFT)
+    f0, g0 = inputs.random_state(orc.shape, orc.qf, orc.qg, seed=zlib.crc32(name.encode()) % 1000 + 1, amp=0.05)
     orc.set_populations(f0, g0)
-    sim.set_populations(torch.from_numpy(f0).cuda(), torch.from_numpy(g0).cuda())
-    for n, tol in ((1, 1e-12), (2, 3e-12)):
-        sim.step(n)
-        orc.step(n)
+    orc.step(1)
+    fo, go = orc.get_populations()
+    orc.step(2)
+    fo3, go3 = orc.get_populations()
+    variants = kernels_for(islbm, sim)
+    assert sum(k == islbm.KERNEL_TILED for k, _ in variants) >= 3
+    for k, tune in variants:
+        select(sim, k, tune)
+        assert sim.kernel_name.endswith("upwind") == (k != islbm.KERNEL_GENERIC)
+        sim.set_populations(torch.from_numpy(f0).cuda(), torch.from_numpy(g0).cuda())
+        sim.step(1)
         f1, g1 = sim.get_populations()
-        fo, go = orc.get_populations()
-        assert elem_err(f1.cpu().numpy(), fo) <= tol and plane_err(g1.cpu().numpy(), go) <= tol
+        ef, eg = elem_err(f1.cpu().numpy(), fo), plane_err(g1.cpu().numpy(), go)
+        assert ef <= 1e-12 and eg <= 1e-12, (name, sim.kernel_name, tune, ef, eg)
+        sim.step(2)
+        f3, g3 = sim.get_populations()
+        ef, eg = elem_err(f3.cpu().numpy(), fo3), plane_err(g3.cpu().numpy(), go3)
+        assert ef <= 3e-12 and eg <= 3e-12, (name, sim.kernel_name, tune, ef, eg)
     with pytest.raises(islbm.IslbmError):
         sim.set_stencil(0)                      # the state exists: too late
+
+
+@pytest.mark.parametrize("dim,ns,st", [(2, (132, 45, 1), (1.5, 1.2, 0)), (2, (131, 67, 1), (1.3, 1.9, 0)),
+                                       (3, (36, 18, 9), (1.3, 1.2, 1.1)), (3, (68, 27, 20), (1.5, 1.1, 1.4)),
+                                       (3, (37, 21, 19), (1.5, 1.2, 1.7))])
+def test_upwind_stencil_fp32_storage(islbm, dim, ns, st):
+    """Upwind stencil with fp32 storage (packed f32x2 interpolation, stencil sets in shared memory): 2e-6 after 3 steps."""
+    coords, delta = ragged_coords(dim, ns, st)
+    H_lu = (coords[1][-1] - coords[1][0] + delta) / delta
+    sim, orc = pair(islbm, coords, delta, Ra=0.71 * (0.1 * H_lu / 0.03) ** 2, precision=1)
+    sim.set_stencil(1)
+    orc.set_stencil(1)
+    f0, g0 = inputs.random_state(orc.shape, orc.qf, orc.qg, seed=13 + dim, amp=0.05)
+    orc.set_populations(f0, g0)
+    orc.step(3)
+    fo, go = orc.get_populations()
+    for k, tune in kernels_for(islbm, sim):
+        select(sim, k, tune)
+        sim.set_populations(torch.from_numpy(f0).cuda(), torch.from_numpy(g0).cuda())
+        sim.step(3)
+        f3, g3 = sim.get_populations()
+        ef, eg = plane_err(f3.cpu().numpy(), fo), plane_err(g3.cpu().numpy(), go)
+        assert ef <= 2e-6 and eg <= 2e-6, (sim.kernel_name, tune, ef, eg)
+
+
+def test_upwind_stencil_1000_steps_and_slab_refusal(islbm):
+    """Upwind stencil on config 1 from the seeded start: fields and diagnostics 1e-9 after 1000 steps; a slab handle
+    (one ghost layer) refuses the stencil."""
+    w = inputs.workload("c1_64sq")
+    sim, orc = pair(islbm, w.coords, w.delta, w.Ra, w.Pr, w.Ma)
+    sim.set_stencil(1)
+    orc.set_stencil(1)
+    sim.init(w.seed, w.noise_amp)
+    orc.init(w.seed, w.noise_amp)
+    sim.step(1000)
+    orc.step(1000)
+    err = field_err(sim, orc)
+    assert max(err.values()) <= 1e-9, err
+    _diag_close(sim, orc)
+    from paper_2509_01099_b200 import slab
+    cav = slab.SlabCavity(w.coords, w.delta, w.Ra, w.Pr, w.Ma, 0, 2, exchange=lambda: None)
+    with pytest.raises(islbm.IslbmError):
+        cav.sim.set_stencil(1)
 
 
 def test_uniform_mesh_one_step(islbm):
