@@ -77,7 +77,9 @@ struct Tile3 {
   static constexpr int STAGE_BYTES = pad128(OFF_YM + 2 * H_Y);
   // byte offset of plane k (0..3) of a z-stencil group that starts at `off`, planes of `pbytes`, halves `half` apart
   static __host__ __device__ constexpr int moff(int off, int k, int pbytes, int half) { return off + (k / 2) * half + (k % 2) * pbytes; }
-  static constexpr int STAGES = sizeof(ST) == 4 ? ISLBM_Z_STAGES_F32 : 3;   // fp64: 3 x 62.7 KB is all that fits
+  // fp64: 3 x 62.7 KB is all that fits.  fp32 storage, upwind stencil: 2 stages, so that two CTAs (2 x (58 KB ring + 27 KB
+  // of stencil sets)) still share an SM; for 32x6 tiles a 2-stage ring measures the same as a 3-stage one (profiles/attempts.md)
+  static constexpr int STAGES = sizeof(ST) == 4 ? (SK ? 2 : ISLBM_Z_STAGES_F32) : 3;
   static constexpr int CONSUMER_WARPS = TX * TY / 32;
   static constexpr int THREADS = TX * TY;                // thread 0 doubles as the TMA producer
   static constexpr uint32_t Z_BYTES = 2u * P_C + 4u * P_X + 4u * P_Y + 4u * P_XY;   // planes of the emitted slice

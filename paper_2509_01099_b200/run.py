@@ -31,6 +31,8 @@ def main(argv=None):
     ap.add_argument("--every", type=int, default=2000, help="report (and test Eq. 30) every this many steps")
     ap.add_argument("--until-steady", action="store_true", help="stop when both residuals of Eq. 30 fall below --tol")
     ap.add_argument("--tol", type=float, default=1e-9)
+    ap.add_argument("--stencil", type=int, default=0, choices=[0, 1],
+                    help="0: destination-centred {j-1,j,j+1} (default); 1: upwind {j-2,j-1,j} / {j,j+1,j+2} (DESIGN.md A2)")
     ap.add_argument("--seed", type=int, default=0)
     ap.add_argument("--noise", type=float, default=None, help="amplitude of the initial temperature noise (default 1e-3; --paper: 0)")
     args = ap.parse_args(argv)
@@ -48,6 +50,7 @@ def main(argv=None):
     noise = args.noise if args.noise is not None else (0.0 if args.paper else w.noise_amp)
     sim = islbm.Islbm(w.coords, w.delta, w.Ra, w.Pr, w.Ma, precision=0 if args.precision == "f64" else 1)
     sim.set_reference_temperature(T0)
+    sim.set_stencil(args.stencil)
     sim.init(args.seed, noise)
     p = sim.params()
     print(json.dumps({"nodes": sim.nodes, "shape": sim.shape, "kernel": sim.kernel_name, "T0": T0,
