@@ -280,9 +280,11 @@ def measure_workload(islbm, inputs, name, precision, steps, warmup, lbm_per_step
 
 
 def run_slab(args):
-    """--decomp slab: ONE cavity decomposed into z-slabs (y-slabs in 2-D), one rank per GPU, a halo exchange of one
-    layer of the planes with a velocity component along the slab axis after every time step (torch.distributed
-    point-to-point over NCCL) and an all-reduce of 8 doubles per Nu/Re reduction: strong scaling.  The default
+    """--decomp slab: ONE cavity decomposed into z-slabs (y-slabs in 2-D), one rank per GPU; per time step one layer
+    of the planes with a velocity component along the slab axis crosses each face — stored by the step kernel itself
+    into the neighbour's ghost layer over NVLink and ordered by step flags in peer memory (--halo fused, default: one
+    launch per step and rank, no collective), or exchanged by torch.distributed point-to-point over NCCL after every
+    step (--halo p2p) — and an all-reduce of 8 doubles per Nu/Re reduction: strong scaling.  The default
     multi-GPU mode stays `replicas` (BASELINE.json: everything runs on one GPU)."""
     import torch
     from paper_2509_01099_b200 import inputs, slab
@@ -329,13 +331,16 @@ def run_slab(args):
                        "step": f"{args.lbm_per_step} LBM time steps (each followed by a halo exchange) + 1 Nu/Re reduction",
                        "parallelism": f"slab decomposition over {world} rank(s) along the slowest axis, 1-layer halo, "
                                       f"{'12 of 26' if w.dim == 3 else '8 of 14'} planes per face per step, halo "
-                                      f"{'stored by the step kernel into peer memory (CUDA IPC) + 1 barrier per step' if args.halo == 'fused' else 'by batched isend/irecv after each step'}"},
+                                      f"{'stored by the step kernel into peer memory (CUDA IPC), neighbours ordered by step flags in peer memory (no collective between steps)' if args.halo == 'fused' else 'by batched isend/irecv after each step'}"},
             "wctpdt_s": (t_max / (args.steps * args.lbm_per_step)) * p["H_lu"] / p["U"], "Nu_hot": nu["Nu_hot"], "Re": nu["Re"],
             "roofline": {"bound": "hbm", "achieved": bpu * w.nodes / world / (t_max / (args.steps * args.lbm_per_step)) / 1e9,
                          "peak": peak, "unit": "GB/s", "frac": bpu * w.nodes / world / (t_max / (args.steps * args.lbm_per_step)) / 1e9 / peak,
                          "traffic": None, "kernel": cav.sim.kernel_name, "peak_source": peak_src,
                          "note": "per rank, whole step including the halo exchange and the reduction"},
-            "cpu_baseline": None, "e2e": None, "gpu_launches": cav.sim.launch_count - l0, "clocks": clocks,
+            "cpu_baseline": None, "e2e": None, "gpu_launches": cav.sim.launch_count - l0,
+            # step kernels per LBM time step (the Nu/Re reduction adds two launches per bench step)
+            "launches_per_lbm_step": (cav.sim.launch_count - l0 - 2 * args.steps) / (args.steps * args.lbm_per_step),
+            "clocks": clocks,
         }
         print(json.dumps(line), flush=True)
     if world > 1:

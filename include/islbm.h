@@ -138,24 +138,37 @@ int islbm_create(islbm_t **out, const islbm_mesh *mesh, int lattice, double Ra,
 int islbm_create_slab(islbm_t **out, const islbm_mesh *mesh, int lattice, double Ra, double Pr, double Ma,
                       int precision, void *dev_workspace, size_t bytes, void *cuda_stream, const islbm_slab *slab);
 int islbm_halo(islbm_t *h, int side /* 0 low, 1 high */, islbm_halo_info *out);
-/* Fused halo exchange over peer memory.  islbm_halo_layout describes where this handle's ghost layer of `side`
- * lives in ITS workspace, for both ping-pong buffers; the neighbour passes that description, together with this
- * workspace as mapped in the neighbour's process (same process: the pointer itself; another process on the node:
- * a CUDA IPC mapping, peer access over NVLink), to islbm_slab_set_peer on its facing side.  From then on the
- * neighbour's step kernel stores the halo planes of its boundary layer straight into this ghost layer as it emits
- * them, and no separate exchange is needed; the caller only has to order the steps (both ranks finish step t before
- * either starts step t+1: a stream-ordered barrier).  Both handles must step in lockstep from the same
- * islbm_init / islbm_set_populations.  peer_workspace = NULL detaches. */
+/* Fused halo exchange over peer memory, synchronised between NEIGHBOURS on the device (no collective per step).
+ * islbm_halo_layout describes where this handle's ghost layer of `side` lives in ITS workspace, for both ping-pong
+ * buffers, where its step flag of that side lives, which buffer holds its current state and how many steps it has
+ * taken; the neighbour passes that description, together with this workspace as mapped in the neighbour's process
+ * (same process: the pointer itself; another process on the node: a CUDA IPC mapping, peer access over NVLink), to
+ * islbm_slab_set_peer on its facing side.  From then on
+ *   - the neighbour's step kernel stores the halo planes of its boundary layer straight into this ghost layer as it
+ *     emits them (no pack / unpack, no exchange pass);
+ *   - when the last of the neighbour's CTAs that touch the boundary has finished step t, it publishes t into this
+ *     handle's flag (st.release.sys after its peer stores); this handle's CTAs that read the ghost layer in step t+1,
+ *     or store into the neighbour's ghost layer, first wait for it (ld.acquire.sys).  With ping-pong buffers that one
+ *     flag per side and step orders both the ghost-layer reads (data of step t) and the peer stores of step t+1 (into
+ *     the buffer the neighbour read during step t);
+ *   - islbm_step(h, n) therefore enqueues its n step kernels back to back, with no host or NCCL synchronisation.
+ * Both handles must have taken the same number of steps since their last islbm_init / islbm_set_populations when
+ * they are connected (checked), and both must then be stepped the same number of times; islbm_init /
+ * islbm_set_populations detach the peers (connect again).  The kernels of different ranks wait on one another, so
+ * every rank must run on its OWN GPU (or the caller must order the steps on the host so that no kernel ever has to
+ * wait, as the single-GPU tests do).  peer_workspace = NULL detaches. */
 typedef struct {
   int is_wall;
   int cur;                    /* index of the buffer that holds the current state (the next step writes 1 - cur) */
   size_t ghost_offset[2];     /* byte offset of the ghost layer of the first halo plane, per ping-pong buffer */
   size_t plane_pitch_bytes;
   size_t layer_bytes;
+  size_t flag_offset;         /* byte offset of this handle's 8-byte step flag of `side` (written by the neighbour) */
+  long long steps;            /* steps taken since the last islbm_init / islbm_set_populations */
 } islbm_halo_layout_info;
 int islbm_halo_layout(islbm_t *h, int side, islbm_halo_layout_info *out);
-int islbm_slab_set_peer(islbm_t *h, int side, void *peer_workspace /* DEVICE */, const size_t ghost_offset[2],
-                        size_t plane_pitch_bytes);
+int islbm_slab_set_peer(islbm_t *h, int side, void *peer_workspace /* DEVICE */,
+                        const islbm_halo_layout_info *peer_layout /* HOST: the neighbour's layout of its facing side */);
 
 /* HOST s[8]: this handle's Eq. 29-weighted partial sums (ghost layers weigh 0); synchronises the stream. */
 int islbm_diag_sums(islbm_t *h, double s[8]);

@@ -41,7 +41,7 @@ size_t align_up(size_t v) { return (v + kAlign - 1) / kAlign * kAlign; }
 constexpr int kMaxRedBlocks = 2048;   // capacity of the partial-sum area; the launch takes 8 blocks per SM (red_blocks)
 
 struct Carve {
-  size_t buf[2], wtab, avgw, partial, red_out, snap, total;
+  size_t buf[2], wtab, avgw, partial, red_out, flags, snap, total;
 };
 
 // row pitch of the workspace planes: nx rounded up to 16 elements (see DevMesh::nxp)
@@ -58,6 +58,7 @@ Carve carve(long long nn, long long nnp, int q, size_t st_bytes, int npad) {
   c.avgw = off;    off = align_up(off + sizeof(double) * 3 * (size_t)npad);
   c.partial = off; off = align_up(off + sizeof(double) * kRedSlots * kMaxRedBlocks);
   c.red_out = off; off = align_up(off + sizeof(double) * 8);
+  c.flags = off;   off = align_up(off + 256);   // neighbour step flags [2] (u64, written by the neighbours) + done counters [2]
   c.snap = off;    off = align_up(off + sizeof(double) * 4 * (size_t)nn);
   c.total = off;
   return c;
@@ -99,6 +100,9 @@ struct islbm {
   char *peer_base[2];
   size_t peer_ghost_off[2][2];
   size_t peer_pitch_bytes[2];
+  size_t peer_flag_off[2];     // the neighbour's step flag of its facing side
+  int peer_flip[2];            // neighbour's `cur` XOR ours at connect time (both flip once per step)
+  long long steps;             // steps since the last islbm_init / islbm_set_populations
   islbm_params prm;
   double buoy;
   double T0;               // reference temperature of the buoyancy force
@@ -331,6 +335,12 @@ static int create_impl(islbm_t **out, const islbm_mesh *mesh, int lattice, doubl
   dm.peer[0] = dm.peer[1] = nullptr;
   dm.peer_pitch[0] = dm.peer_pitch[1] = 0;
   h->peer_base[0] = h->peer_base[1] = nullptr;
+  h->peer_flip[0] = h->peer_flip[1] = 0;
+  h->steps = 0;
+  dm.flag_in[0] = dm.flag_in[1] = dm.flag_out[0] = dm.flag_out[1] = nullptr;
+  dm.done_cnt = (unsigned long long *)(h->ws + h->cv.flags + 64);
+  dm.step = 0;
+  dm.bctas = 1;
   {
     const int nm = h->n[h->dim - 1];
     dm.wall_mlo = !slab || slab->lo_is_wall;
@@ -474,6 +484,8 @@ static int load_state(islbm *h, const double *f, const double *g, bool generate,
   h->has_state = true;
   h->other_is_pre = true;
   h->snap_valid = false;
+  h->steps = 0;
+  h->peer_base[0] = h->peer_base[1] = nullptr;   // a new state: the neighbours must be connected again
   return ISLBM_OK;
 }
 
@@ -511,6 +523,8 @@ extern "C" int islbm_set_populations_host(islbm_t *h, const double *f, const dou
   h->has_state = true;
   h->other_is_pre = true;
   h->snap_valid = false;
+  h->steps = 0;
+  h->peer_base[0] = h->peer_base[1] = nullptr;
   return ISLBM_OK;
 }
 
@@ -594,11 +608,23 @@ extern "C" int islbm_step(islbm_t *h, int n) {
   const int which = effective_kernel(h);
   if ((h->peer_base[0] || h->peer_base[1]) && which == 3)
     return fail(ISLBM_ERR_STATE, "the fused halo exchange is not available with the pure-shift kernel");
+  const bool fused = h->peer_base[0] || h->peer_base[1];
   for (int s = 0; s < n; ++s) {
-    // fused halo exchange: this step writes buffer 1 - cur, and so does the neighbour (both step in lockstep)
+    // fused halo exchange: this step writes buffer 1 - cur; the neighbour's `cur` is ours XOR the parity difference
+    // recorded at connect time (both flip once per step), and it reads the ghost layer we store from ITS buffer
+    // 1 - cur in its next step
     for (int sd = 0; sd < 2; ++sd) {
-      h->dm.peer[sd] = h->peer_base[sd] ? (void *)(h->peer_base[sd] + h->peer_ghost_off[sd][1 - h->cur]) : nullptr;
-      h->dm.peer_pitch[sd] = h->peer_base[sd] ? (long long)(h->peer_pitch_bytes[sd] / h->st_bytes) : 0;
+      const bool on = h->peer_base[sd] != nullptr;
+      const int peer_cur = h->cur ^ h->peer_flip[sd];
+      h->dm.peer[sd] = on ? (void *)(h->peer_base[sd] + h->peer_ghost_off[sd][1 - peer_cur]) : nullptr;
+      h->dm.peer_pitch[sd] = on ? (long long)(h->peer_pitch_bytes[sd] / h->st_bytes) : 0;
+      h->dm.flag_in[sd] = on ? (unsigned long long *)(h->ws + h->cv.flags) + sd : nullptr;
+      h->dm.flag_out[sd] = on ? (unsigned long long *)(h->peer_base[sd] + h->peer_flag_off[sd]) : nullptr;
+    }
+    h->dm.step = (unsigned long long)h->steps + 1ull;
+    if (fused && which != 2) {
+      k_slab_wait<<<1, 1, 0, h->stream>>>(h->dm);
+      h->launches++;
     }
     if (which == 2) {
       void *bufs[2] = {h->ws + h->cv.buf[0], h->ws + h->cv.buf[1]};
@@ -620,7 +646,12 @@ extern "C" int islbm_step(islbm_t *h, int n) {
       DISPATCH(h, CALL);
 #undef CALL
     }
+    if (fused && which != 2) {
+      k_slab_publish<<<1, 1, 0, h->stream>>>(h->dm);
+      h->launches++;
+    }
     h->cur ^= 1;
+    h->steps++;
     h->other_is_pre = false;
   }
   CUDA_TRY(cudaPeekAtLastError());
@@ -725,25 +756,38 @@ extern "C" int islbm_halo_layout(islbm_t *h, int side, islbm_halo_layout_info *o
   out->plane_pitch_bytes = pitch;
   out->layer_bytes = layer;
   out->cur = h->cur;
+  out->steps = h->steps;
+  out->flag_offset = h->cv.flags + 8 * (size_t)side;
   for (int b = 0; b < 2; ++b)
     out->ghost_offset[b] = h->cv.buf[b] + (size_t)first * pitch + (size_t)(side == 0 ? 0 : nm - 1) * layer;
   return ISLBM_OK;
 }
 
-extern "C" int islbm_slab_set_peer(islbm_t *h, int side, void *peer_workspace, const size_t ghost_offset[2],
-                                   size_t plane_pitch_bytes) {
+extern "C" int islbm_slab_set_peer(islbm_t *h, int side, void *peer_workspace, const islbm_halo_layout_info *pl) {
   if (!h) return fail(ISLBM_ERR_ARG, "NULL handle");
   if (side != 0 && side != 1) return fail(ISLBM_ERR_ARG, "side must be 0 (low) or 1 (high)");
   if (!h->is_slab) return fail(ISLBM_ERR_STATE, "not a slab handle");
   if (side == 0 ? h->dm.wall_mlo : h->dm.wall_mhi) return fail(ISLBM_ERR_ARG, "this side is a wall: it has no neighbour");
-  if (peer_workspace && (!ghost_offset || plane_pitch_bytes == 0 || plane_pitch_bytes % h->st_bytes))
-    return fail(ISLBM_ERR_ARG, "bad peer layout");
-  h->peer_base[side] = (char *)peer_workspace;         // NULL detaches (exchange outside the kernel again)
-  if (peer_workspace) {
-    h->peer_ghost_off[side][0] = ghost_offset[0];
-    h->peer_ghost_off[side][1] = ghost_offset[1];
-    h->peer_pitch_bytes[side] = plane_pitch_bytes;
+  if (!peer_workspace) {                               // detach (exchange outside the kernel again)
+    h->peer_base[side] = nullptr;
+    return ISLBM_OK;
   }
+  if (!pl || pl->plane_pitch_bytes == 0 || pl->plane_pitch_bytes % h->st_bytes || pl->is_wall || (pl->cur != 0 && pl->cur != 1))
+    return fail(ISLBM_ERR_ARG, "bad peer layout");
+  if (pl->steps != h->steps)
+    return fail(ISLBM_ERR_STATE, "the neighbour has taken a different number of steps: both slabs must be connected "
+                                 "at the same step count (the step flags count steps)");
+  // our flag of this side starts at the common step count: "the neighbour has finished step `steps`"
+  const unsigned long long init = (unsigned long long)h->steps;
+  CUDA_TRY(cudaMemcpyAsync(h->ws + h->cv.flags + 8 * (size_t)side, &init, 8, cudaMemcpyHostToDevice, h->stream));
+  CUDA_TRY(cudaMemsetAsync(h->ws + h->cv.flags + 64 + 8 * (size_t)side, 0, 8, h->stream));   // done counter
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  h->peer_base[side] = (char *)peer_workspace;
+  h->peer_ghost_off[side][0] = pl->ghost_offset[0];
+  h->peer_ghost_off[side][1] = pl->ghost_offset[1];
+  h->peer_pitch_bytes[side] = pl->plane_pitch_bytes;
+  h->peer_flag_off[side] = pl->flag_offset;
+  h->peer_flip[side] = pl->cur ^ h->cur;
   return ISLBM_OK;
 }
 

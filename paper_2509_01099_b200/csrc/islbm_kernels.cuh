@@ -48,6 +48,14 @@ struct DevMesh {
   // exchange pass.  nullptr: no neighbour on that side, or the exchange is done outside (islbm_halo).
   void *peer[2];
   long long peer_pitch[2];
+  // neighbour-only synchronisation of the fused exchange (include/islbm.h: islbm_slab_set_peer).  flag_in[s]: this
+  // rank's step flag of side s, written by that neighbour; flag_out[s]: the neighbour's flag in peer memory; step: the
+  // 1-based index of the step this launch performs; done_cnt: two counters of finished boundary CTAs (monotonic);
+  // bctas: CTAs of this launch that touch one boundary layer
+  unsigned long long *flag_in[2], *flag_out[2];
+  unsigned long long *done_cnt;
+  unsigned long long step;
+  int bctas;
   int stencil;           // 0: {j-1,j,j+1} (A2); 1: upwind {j-2,j-1,j} for c=+1, {j,j+1,j+2} for c=-1
                          // (generic kernel only; the TMA kernels stage a 1-node halo and take stencil 0)
 };
@@ -248,6 +256,45 @@ __device__ __forceinline__ void peer_store_node(const DevMesh &m, int layer, lon
     peer_store<DIM, ST, DEV, NT>(m.peer[0], m.peer_pitch[0], inplane, f, g, std::make_integer_sequence<int, halo_plane_count<DIM>()>{});
   if (m.peer[1] != nullptr && layer == m.em_hi - 1)
     peer_store<DIM, ST, DEV, NT>(m.peer[1], m.peer_pitch[1], inplane, f, g, std::make_integer_sequence<int, halo_plane_count<DIM>()>{});
+}
+
+// ---- neighbour flags of the fused halo exchange -----------------------------------------------------------------
+__device__ __forceinline__ unsigned long long ld_acquire_sys(const unsigned long long *p) {
+  unsigned long long v;
+  asm volatile("ld.acquire.sys.global.u64 %0, [%1];" : "=l"(v) : "l"(p) : "memory");
+  return v;
+}
+__device__ __forceinline__ void st_release_sys(unsigned long long *p, unsigned long long v) {
+  asm volatile("st.release.sys.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+}
+// one thread: wait until the neighbour of `side` has finished step m.step - 1 (its halo of that step is in our ghost
+// layer, and it no longer reads the ghost layer we are about to overwrite)
+__device__ __forceinline__ void slab_wait_neighbour(const DevMesh &m, int side) {
+  if (m.flag_in[side] == nullptr) return;
+  while (ld_acquire_sys(m.flag_in[side]) + 1ull < m.step) __nanosleep(64);
+}
+// one thread of a CTA whose threads have all finished (after a CTA barrier): count it; the last boundary CTA of this
+// launch publishes the step number to the neighbour
+__device__ __forceinline__ void slab_publish(const DevMesh &m, int side) {
+  if (m.flag_out[side] == nullptr) return;
+  __threadfence_system();                                                 // this CTA's peer stores, cumulatively
+  const unsigned long long old = atomicAdd(m.done_cnt + side, 1ull);
+  if ((old + 1ull) % (unsigned long long)m.bctas == 0ull) {
+    __threadfence_system();                                               // ... and those of every CTA counted before
+    st_release_sys(m.flag_out[side], m.step);
+  }
+}
+// generic-kernel path: the same protocol as two single-thread kernels around the step
+__global__ void k_slab_wait(DevMesh m) {
+  slab_wait_neighbour(m, 0);
+  slab_wait_neighbour(m, 1);
+}
+__global__ void k_slab_publish(DevMesh m) {
+  for (int side = 0; side < 2; ++side)
+    if (m.flag_out[side] != nullptr) {
+      __threadfence_system();
+      st_release_sys(m.flag_out[side], m.step);
+    }
 }
 
 // ---------------------------------------------------------------------------

@@ -138,6 +138,7 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
   const int y1 = m.em_lo + (int)((long long)(blockIdx.y + 1) * rows / gridDim.y);
   const int yf = DIR > 0 ? y0 : y1 - 1;
   const int nstage = 2 + (y1 - y0);
+  const bool b_lo = y0 == m.em_lo, b_hi = y1 == m.em_hi;   // slab boundary CTAs (fused exchange; islbm_tiled3.cuh)
   const uint64_t lpol = make_policy(load_policy);
   const uint64_t spol = make_policy(store_policy);
   // thread 0 sets up the ring and (unless late_fill) fills it BEFORE warps 1.. load the weight rows, so the two
@@ -155,6 +156,8 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
     tma_prefetch_desc(&mp.x);
     if (!late_fill) {
       pdl_wait();
+      if (b_lo) slab_wait_neighbour(m, 0);
+      if (b_hi) slab_wait_neighbour(m, 1);
       for (int s = 0; s < T::STAGES && s < nstage; ++s) issue_stage2<T, DIR>(s, yf, m.ny, x0, stage0, full, empty, mp, lpol);
     }
   }
@@ -165,6 +168,8 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
   pdl_wait();
   __syncthreads();
   if (late_fill && threadIdx.x == 0) {
+    if (b_lo) slab_wait_neighbour(m, 0);
+    if (b_hi) slab_wait_neighbour(m, 1);
     for (int s = 0; s < T::STAGES && s < nstage; ++s) issue_stage2<T, DIR>(s, yf, m.ny, x0, stage0, full, empty, mp, lpol);
   }
 
@@ -280,6 +285,13 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
 #undef PXR
 #undef PC4
 #undef PXM
+  }
+  if ((b_lo && m.flag_out[0] != nullptr) || (b_hi && m.flag_out[1] != nullptr)) {   // CTA-uniform
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      if (b_lo) slab_publish(m, 0);
+      if (b_hi) slab_publish(m, 1);
+    }
   }
 }
 
@@ -620,15 +632,17 @@ inline void launch2_cfg(const Plan2 &p, const int *n, const DevMesh &m, const No
   // first ring fill (measured, profiles/r1_c3_1024sq_ymarch_v4.md): a single-wave launch is 2-5 % faster with the
   // fill after the CTA barrier, a multi-wave launch 2-6 % faster with the fill first
   const int late = tn.fill ? (tn.fill == 2) : (nc <= p.per_wave);
+  DevMesh mm = m;
+  mm.bctas = (int)grid.x;   // CTAs that touch one boundary row of a slab
   if (p.sk)
     launch_step(k_step_ymarch_up<ST, T::TX, T::STAGES, CFG::MINB>, grid, dim3(T::TX), Tile2<ST, T::TX, T::STAGES, 1>::SMEM_BYTES, stream, tn.pdl != 0,
                 p.maps[cur], m, np, (const ST *)buf[cur], (ST *)buf[1 - cur], tn.load_policy, tn.store_policy, late);
   else if (tn.serpentine && cur)
     launch_step(k_step_ymarch<ST, T::TX, T::STAGES, CFG::MINB, -1>, grid, dim3(T::TX), T::SMEM_BYTES, stream, tn.pdl != 0,
-                p.maps[cur], m, np, (const ST *)buf[cur], (ST *)buf[1 - cur], tn.load_policy, tn.store_policy, late);
+                p.maps[cur], mm, np, (const ST *)buf[cur], (ST *)buf[1 - cur], tn.load_policy, tn.store_policy, late);
   else
     launch_step(k_step_ymarch<ST, T::TX, T::STAGES, CFG::MINB, 1>, grid, dim3(T::TX), T::SMEM_BYTES, stream, tn.pdl != 0,
-                p.maps[cur], m, np, (const ST *)buf[cur], (ST *)buf[1 - cur], tn.load_policy, tn.store_policy, late);
+                p.maps[cur], mm, np, (const ST *)buf[cur], (ST *)buf[1 - cur], tn.load_policy, tn.store_policy, late);
 }
 
 template <typename ST>

@@ -377,6 +377,9 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
   const int x0 = blockIdx.x * T::TX, y0 = min((int)blockIdx.y * T::TY, max(m.ny - T::TY, 0));
   const int z0 = m.em_lo + blockIdx.z * zchunk, z1 = min(z0 + zchunk, m.em_hi);
   const int nstage = 2 + (z1 - z0);
+  // slab decomposition with the fused exchange: does this CTA touch the low / high boundary layer?  Then it waits for
+  // that neighbour's step flag before its first load, and is counted when it is done (islbm_kernels.cuh)
+  const bool b_lo = z0 == m.em_lo, b_hi = z1 == m.em_hi;
   const uint64_t lpol = make_policy(load_policy);
   const uint64_t spol = make_policy(store_policy);
   // thread 0 sets up the ring and (unless late_fill) fills it BEFORE warps 1.. load the weight rows, so the two
@@ -397,6 +400,8 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
     tma_prefetch_desc(&mp.xy);
     if (!late_fill) {
       pdl_wait();
+      if (b_lo) slab_wait_neighbour(m, 0);
+      if (b_hi) slab_wait_neighbour(m, 1);
       for (int s = 0; s < T::STAGES - (EARLY ? 0 : 1) && s < nstage; ++s)
         issue_stage3<T>(s, z0, m.nz, x0, y0, stage0, full, empty, mp, lpol);
     }
@@ -408,6 +413,8 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
   pdl_wait();
   __syncthreads();
   if (late_fill && threadIdx.x == 0) {
+    if (b_lo) slab_wait_neighbour(m, 0);
+    if (b_hi) slab_wait_neighbour(m, 1);
     for (int s = 0; s < T::STAGES - (EARLY ? 0 : 1) && s < nstage; ++s)
       issue_stage3<T>(s, z0, m.nz, x0, y0, stage0, full, empty, mp, lpol);
   }
@@ -556,6 +563,13 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
 #undef PC4
 #undef PXM
 #undef PYM
+  }
+  if ((b_lo && m.flag_out[0] != nullptr) || (b_hi && m.flag_out[1] != nullptr)) {   // CTA-uniform
+    __syncthreads();
+    if (threadIdx.x == 0) {
+      if (b_lo) slab_publish(m, 0);
+      if (b_hi) slab_publish(m, 1);
+    }
   }
 }
 
@@ -862,8 +876,10 @@ inline void launch3_shape(const Plan3 &p, const int *n, const DevMesh &m, const 
                           const Tuning &tn, cudaStream_t stream) {
   using T = Tile3<ST, TX, TY, SK>;
   dim3 grid((n[0] + T::TX - 1) / T::TX, (n[1] + T::TY - 1) / T::TY, (m.em_hi - m.em_lo + p.zchunk - 1) / p.zchunk);
+  DevMesh mm = m;
+  mm.bctas = (int)(grid.x * grid.y);   // CTAs that touch one boundary layer of a slab
   if constexpr (SK == 0)
-    launch_step(k_step_zmarch<ST, TX, TY>, grid, dim3(T::THREADS), T::SMEM_BYTES, stream, tn.pdl != 0, p.maps[cur], m, np,
+    launch_step(k_step_zmarch<ST, TX, TY>, grid, dim3(T::THREADS), T::SMEM_BYTES, stream, tn.pdl != 0, p.maps[cur], mm, np,
                 (const ST *)buf[cur], (ST *)buf[1 - cur], p.zchunk, tn.load_policy, tn.store_policy, tn.fill == 2 ? 1 : 0);
   else
     launch_step(k_step_zmarch_up<ST, TX, TY>, grid, dim3(T::THREADS), T::SMEM_BYTES, stream, tn.pdl != 0, p.maps[cur], m, np,

@@ -43,7 +43,7 @@ class _Halo(C.Structure):
 
 class _HaloLayout(C.Structure):
     _fields_ = [("is_wall", C.c_int), ("cur", C.c_int), ("ghost_offset", C.c_size_t * 2), ("plane_pitch_bytes", C.c_size_t),
-                ("layer_bytes", C.c_size_t)]
+                ("layer_bytes", C.c_size_t), ("flag_offset", C.c_size_t), ("steps", C.c_longlong)]
 
 
 class _Params(C.Structure):
@@ -70,7 +70,7 @@ def _load():
                                       C.c_int, vp, C.c_size_t, vp, C.POINTER(_Slab)]
     lib.islbm_halo.argtypes = [vp, C.c_int, C.POINTER(_Halo)]
     lib.islbm_halo_layout.argtypes = [vp, C.c_int, C.POINTER(_HaloLayout)]
-    lib.islbm_slab_set_peer.argtypes = [vp, C.c_int, vp, C.POINTER(C.c_size_t), C.c_size_t]
+    lib.islbm_slab_set_peer.argtypes = [vp, C.c_int, vp, C.POINTER(_HaloLayout)]
     lib.islbm_diag_sums.argtypes = [vp, dp]
     lib.islbm_diag_from_sums.argtypes = [vp, dp, dp]
     lib.islbm_residual_sums.argtypes = [vp, dp, C.POINTER(C.c_int)]
@@ -276,16 +276,18 @@ class Islbm:
         hl = _HaloLayout()
         _check(lib.islbm_halo_layout(self.h, int(side), C.byref(hl)))
         return dict(is_wall=bool(hl.is_wall), cur=hl.cur, ghost_offset=[hl.ghost_offset[0], hl.ghost_offset[1]],
-                    plane_pitch_bytes=hl.plane_pitch_bytes, layer_bytes=hl.layer_bytes)
+                    plane_pitch_bytes=hl.plane_pitch_bytes, layer_bytes=hl.layer_bytes, flag_offset=hl.flag_offset,
+                    steps=hl.steps)
 
     def set_peer(self, side, peer_workspace_ptr, layout):
         """peer_workspace_ptr: device address of the neighbour's workspace as mapped in this process (0 detaches);
         layout: the neighbour's halo_layout() of its facing side."""
         if not peer_workspace_ptr:
-            _check(lib.islbm_slab_set_peer(self.h, int(side), None, None, 0))
+            _check(lib.islbm_slab_set_peer(self.h, int(side), None, None))
             return
-        off = (C.c_size_t * 2)(*layout["ghost_offset"])
-        _check(lib.islbm_slab_set_peer(self.h, int(side), C.c_void_p(int(peer_workspace_ptr)), off, layout["plane_pitch_bytes"]))
+        hl = _HaloLayout(int(layout["is_wall"]), int(layout["cur"]), (C.c_size_t * 2)(*layout["ghost_offset"]),
+                         layout["plane_pitch_bytes"], layout["layer_bytes"], layout["flag_offset"], int(layout["steps"]))
+        _check(lib.islbm_slab_set_peer(self.h, int(side), C.c_void_p(int(peer_workspace_ptr)), C.byref(hl)))
 
     def diag_sums(self):
         s = (C.c_double * 8)()

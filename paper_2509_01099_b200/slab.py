@@ -80,12 +80,21 @@ class SlabCavity:
         local, slab, self.own, self.ghosts = slab_inputs(coords, delta, rank, world)
         self.sim = islbm.Islbm(local, delta, Ra, Pr, Ma, precision=precision, device=device, slab=slab)
         self._exchange = exchange or self._exchange_dist
+        self._fused = False
         self._peers = []          # keeps the IPC mappings of the neighbours' workspaces alive
 
     # -- fused halo exchange ----------------------------------------------------------------------------------
-    def connect_ipc(self):
+    def connect_ipc(self, host_barrier=None):
         """One process per rank on one node: map the neighbours' workspaces with CUDA IPC (torch's tensor sharing),
-        hand them to the library, and switch to the fused exchange.  Collective over the default process group."""
+        hand them and the neighbours' halo layouts (ghost layers, step flags, buffer parity, step count) to the
+        library, and switch to the fused exchange.  Collective over the default process group.
+
+        From then on a step is ONE kernel per rank: boundary layers go into the neighbours' ghost layers by peer
+        stores, and neighbours order their steps through flags in each other's memory (st.release.sys by the last
+        boundary CTA of a step, ld.acquire.sys by the boundary CTAs of the next) — no collective between steps.
+        host_barrier: order the steps on the host instead (device synchronise + barrier after every step), so that no
+        kernel ever has to WAIT for another rank; required when several ranks share one GPU (kernels of different
+        ranks are then not guaranteed to run at the same time: the tests), default when the backend is not NCCL."""
         import torch
         import torch.distributed as dist
         from torch.multiprocessing.reductions import reduce_tensor
@@ -98,16 +107,18 @@ class SlabCavity:
                 t = fn(*args)                                   # the neighbour's workspace, mapped here
                 self._peers.append(t)
                 self.sim.set_peer(side, t.data_ptr(), everyone[nb]["hi" if side == 0 else "lo"])
-        backend = dist.get_backend()
-        flag = torch.zeros(1, device=self.sim.device if backend == "nccl" else "cpu")
-
-        def barrier():
-            if backend == "nccl":
-                dist.all_reduce(flag)                           # stream-ordered: completes when every rank's step has
-            else:
+        torch.cuda.synchronize(self.sim.device)
+        dist.barrier()                                          # every rank has initialised its flags before any step
+        if host_barrier is None:
+            host_barrier = dist.get_backend() != "nccl"
+        self._fused = True
+        if host_barrier:
+            def barrier():
                 torch.cuda.synchronize(self.sim.device)
                 dist.barrier()
-        self._exchange = barrier
+            self._exchange = barrier
+        else:
+            self._exchange = None                               # nothing between steps: islbm_step(n) runs n kernels
 
     # -- halo -------------------------------------------------------------------------------------------------
     def halo_views(self):
@@ -124,6 +135,9 @@ class SlabCavity:
         self.sim.init(seed, noise_amp)          # noise is drawn by GLOBAL node index: ghost layers come out right
 
     def step(self, n=1):
+        if self._exchange is None:              # fused exchange with device-side neighbour flags
+            self.sim.step(n)
+            return
         for _ in range(n):
             self.sim.step(1)
             self._exchange()
@@ -151,12 +165,15 @@ class SlabCavity:
 
 def connect_local(slabs):
     """Fused halo exchange among slabs that live in ONE process on ONE device: each handle gets its neighbours'
-    workspaces as peers; the shared stream orders the steps, so no barrier is needed."""
+    workspaces as peers.  The slabs must be stepped ONE STEP AT A TIME in turn on the shared stream (as the tests do):
+    then every neighbour flag is already set when a kernel starts and no kernel ever waits."""
     for a in range(len(slabs) - 1):
         lower, upper = slabs[a].sim, slabs[a + 1].sim
-        lower.set_peer(1, upper.workspace.data_ptr(), upper.halo_layout(0))
-        upper.set_peer(0, lower.workspace.data_ptr(), lower.halo_layout(1))
+        lo_layout, up_layout = lower.halo_layout(1), upper.halo_layout(0)
+        lower.set_peer(1, upper.workspace.data_ptr(), up_layout)
+        upper.set_peer(0, lower.workspace.data_ptr(), lo_layout)
     for s in slabs:
+        s._fused = True
         s._exchange = lambda: None
 
 

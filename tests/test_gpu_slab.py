@@ -89,6 +89,45 @@ def test_slabs_equal_the_single_domain_bitwise(islbm, dim, ns, world, prec, kern
         slabs[0].sim.nusselt()
 
 
+def test_fused_exchange_is_one_launch_per_step_and_flags_count_steps(islbm):
+    """Fused exchange with the neighbour-only device-side synchronisation: one kernel per slab and step and no other
+    launch (no collective, no exchange pass); each slab's step flags hold the number of steps its neighbours have
+    finished; a neighbour at a different step count is refused; a buffer-parity difference between neighbours (one
+    of them re-initialised after an odd number of steps) is handled (it used to corrupt silently)."""
+    coords, delta, Ra = mesh(3, (40, 24, 21), (1.4, 1.2, 1.3))
+    Ma = 0.1 * SQ3
+    whole = islbm.Islbm(coords, delta, Ra, 0.71, Ma)
+    slabs = [slab.SlabCavity(coords, delta, Ra, 0.71, Ma, r, 3, exchange=lambda: None) for r in range(3)]
+    whole.init(5, 1e-3)
+    for s in slabs:
+        s.init(5, 1e-3)
+    slabs[1].sim.step(1)                   # slab 1: one step on its own, then a fresh state: cur = 1, steps = 0
+    with pytest.raises(islbm.IslbmError) as e:
+        slab.connect_local(slabs)          # step counts 0 / 1 / 0
+    assert e.value.code == -6 and "steps" in str(e.value)
+    slabs[1].init(5, 1e-3)
+    assert [s.sim.halo_layout(0)["cur"] for s in slabs] == [0, 1, 0]
+    slab.connect_local(slabs)
+    l0 = [s.sim.launch_count for s in slabs]
+    for _ in range(6):
+        whole.step(1)
+        for s in slabs:                    # in turn on one stream: every flag is set before the kernel that reads it
+            s.sim.step(1)
+    assert [s.sim.launch_count - a for s, a in zip(slabs, l0)] == [6, 6, 6]
+    torch.cuda.synchronize()
+    for r, s in enumerate(slabs):
+        lay = [s.sim.halo_layout(side) for side in (0, 1)]
+        flags = [int(s.sim.workspace[l["flag_offset"]:l["flag_offset"] + 8].view(torch.int64).item()) for l in lay]
+        assert (r == 0 or flags[0] == 6) and (r == 2 or flags[1] == 6), (r, flags)      # wall sides have no flag
+        assert lay[0]["steps"] == 6
+    fw = whole.fields()
+    for s in slabs:
+        lo, hi = s.own
+        fl = s.sim.fields()
+        for k in fl:
+            assert torch.equal(s.owned(fl[k]), fw[k][lo:hi]), (k, s.rank)
+
+
 def test_slabs_against_the_oracle(islbm):
     coords, delta, Ra = mesh(3, (24, 16, 21), (1.3, 1.2, 1.4))
     orc = Oracle(coords, delta, Ra, 0.71, 0.1 * SQ3, threads=max(1, min(16, len(os.sched_getaffinity(0)))))
@@ -139,8 +178,11 @@ dist.destroy_process_group()
 
 def test_two_processes_one_gpu_fused_exchange_over_cuda_ipc(islbm, tmp_path):
     """Two ranks as two PROCESSES sharing the one GPU: control plane gloo, data plane CUDA IPC (each rank's step
-    kernel stores its boundary layer into the other process's workspace).  The ranks are ordered by a host barrier
-    after a device synchronise, so no kernel ever waits on another; result against the single-domain run."""
+    kernel stores its boundary layer into the other process's workspace and publishes its step flag there).  The
+    ranks share ONE GPU here, so connect_ipc orders the steps by a host barrier after a device synchronise (its
+    default for a non-NCCL backend): every flag is already set when the kernel that reads it starts, and no kernel
+    ever waits on another process's kernel (B200_PROFILING.md: such waits on one GPU can time out the context
+    switch).  Result against the single-domain run."""
     import subprocess, sys, json
     root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
     port = 29900 + os.getpid() % 2000
