@@ -596,6 +596,7 @@ extern "C" int islbm_set_tuning(islbm_t *h, const char *key, int value) {
   else if (k == "ring2d") { if (value != 0 && value != 3 && value != 4) return fail(ISLBM_ERR_ARG, "ring2d must be 0 (automatic), 3 or 4"); t.ring2d = value; }
   else if (k == "rows2d") { if (value > kMaxChunk) return fail(ISLBM_ERR_ARG, "rows2d must be at most 64"); t.rows2d = value; }
   else if (k == "rows2d1") { if (value > kMaxChunk) return fail(ISLBM_ERR_ARG, "rows2d1 must be at most 64"); t.rows2d1 = value; }
+  else if (k == "walls") { if (value > 1) return fail(ISLBM_ERR_ARG, "walls must be 0 (fused) or 1 (separate boundary kernel)"); t.walls = value; }
   else return fail(ISLBM_ERR_ARG, "unknown tuning key: " + k);
   make_tiled_plan(h);
   return ISLBM_OK;
@@ -636,7 +637,7 @@ extern "C" int islbm_step(islbm_t *h, int n) {
         e = h->precision == ISLBM_F64 ? launch3<double>(h->plan3, h->n, h->dm, h->np, h->cur, bufs, h->tune, h->stream)
                                       : launch3<float>(h->plan3, h->n, h->dm, h->np, h->cur, bufs, h->tune, h->stream);
       if (e != cudaSuccess) return fail(ISLBM_ERR_CUDA, std::string("tiled step launch: ") + cudaGetErrorString(e));
-      h->launches++;
+      h->launches += (h->dim == 3 && h->tune.walls == 1 && !h->is_slab && h->stencil == 0) ? 2 : 1;
     } else if (which == 3) {
 #define CALL(D, T) launch_shift_step<D, T>(h)
       DISPATCH(h, CALL);

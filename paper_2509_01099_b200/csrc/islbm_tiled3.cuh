@@ -356,8 +356,11 @@ __device__ __forceinline__ void load_march_weights(const float *ws, int i, Pr<fl
 template <typename ST, int TX, int TY>
 __global__ void __launch_bounds__(TX * TY, TX * TY <= 128 ? 3 : (TX * TY <= 192 ? 2 : 1))
 k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const ST *__restrict__ src,
-              ST *__restrict__ dst, int zchunk, int load_policy, int store_policy, int late_fill) {
+              ST *__restrict__ dst, int zchunk, int load_policy, int store_policy, int flags) {
   using T = Tile3<ST, TX, TY>;
+  // flags: bit 0 = first ring fill after the CTA barrier; bit 1 = leave the wall rules to k_step_shell3 (the
+  // separate-boundary-kernel variant of BASELINE.json north_star, islbm_set_tuning("walls", 1); measured slower)
+  const bool late_fill = flags & 1, skip_walls = flags & 2;
   using AT = typename Acc<ST>::type;
   // Ring refill policy (measured, profiles/): with fp64 storage the launch is DRAM-bound and thread 0 refilling the
   // slot released in the previous iteration (STAGES - 2 .. STAGES - 1 stages in flight) is 1.7 % faster; with fp32
@@ -547,7 +550,7 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
       }
       wf.lo[2] = z == 0 && m.wall_mlo;
       wf.hi[2] = z == m.nz - 1 && m.wall_mhi;
-      if (valid && (wall_xy | wf.lo[2] | wf.hi[2])) wall_fix_node<3>(f, g, wf, src + c, m.nnp, m);
+      if (!skip_walls && valid && (wall_xy | wf.lo[2] | wf.hi[2])) wall_fix_node<3>(f, g, wf, src + c, m.nnp, m);
       constexpr bool DEV = Store<ST, 3>::kBiased;   // fp32 storage: collide the deviations as they are
       collide_node<DEV>(f, g, np);
       if (valid) {
@@ -805,6 +808,34 @@ k_step_zmarch_up(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, con
   }
 }
 
+// ------------------------------ separate boundary kernel (A/B variant) ----------------------------------------
+// BASELINE.json north_star names "wall nodes handled by a separate boundary kernel".  This is that design, kept as a
+// measurable alternative (islbm_set_tuning("walls", 1)): the march skips the wall rules, and this kernel then
+// recomputes the shell of wall-adjacent nodes (6 faces, 2.3 % of the nodes at 256^3) from the source buffer — pull,
+// Eq. 21-23, collide — and overwrites what the march stored there.  It moves more bytes (the shell is read through
+// the stencil and written twice) and two of its faces are strided by a whole row; profiles/attempts.md has the A/B.
+template <typename ST>
+__global__ void __launch_bounds__(256)
+k_step_shell3(DevMesh m, NodeParams np, const ST *__restrict__ src, ST *__restrict__ dst) {
+  const int face = blockIdx.z, a = blockIdx.x * blockDim.x + threadIdx.x, b = blockIdx.y * blockDim.y + threadIdx.y;
+  int ix, iy, iz;
+  if (face < 2) { ix = face == 0 ? 0 : m.nx - 1; iy = a; iz = b; }
+  else if (face < 4) { ix = a; iy = face == 2 ? 0 : m.ny - 1; iz = b; }
+  else { ix = a; iy = b; iz = face == 4 ? 0 : m.nz - 1; }
+  if (ix >= m.nx || iy >= m.ny || iz >= m.nz) return;
+  NodeCtx<3> cx;
+  make_ctx<3>(m, ix, iy, iz, cx);
+  double f[19], g[7];
+  pull_all_f<3>(m, src, cx, f, std::make_integer_sequence<int, 19>{});
+  pull_all_g<3>(m, src, cx, g, std::make_integer_sequence<int, 7>{});
+  add_bias<ST, 3>(f);
+  collide_node(f, g, np);
+#pragma unroll
+  for (int q = 0; q < 19; ++q) dst[(long long)plane_f<3>(q) * m.nnp + cx.c] = to_storage<ST, 3>(f[q], q);
+#pragma unroll
+  for (int q = 0; q < 7; ++q) dst[(long long)plane_g<3>(q) * m.nnp + cx.c] = (ST)g[q];
+}
+
 // ------------------------------ host side ---------------------------------
 struct Plan3 {
   bool available = false;
@@ -879,8 +910,17 @@ inline void launch3_shape(const Plan3 &p, const int *n, const DevMesh &m, const 
   DevMesh mm = m;
   mm.bctas = (int)(grid.x * grid.y);   // CTAs that touch one boundary layer of a slab
   if constexpr (SK == 0)
-    launch_step(k_step_zmarch<ST, TX, TY>, grid, dim3(T::THREADS), T::SMEM_BYTES, stream, tn.pdl != 0, p.maps[cur], mm, np,
-                (const ST *)buf[cur], (ST *)buf[1 - cur], p.zchunk, tn.load_policy, tn.store_policy, tn.fill == 2 ? 1 : 0);
+  {
+    const bool shell = tn.walls == 1 && m.em_lo == 0 && m.em_hi == m.nz && m.peer[0] == nullptr && m.peer[1] == nullptr;
+    launch_step(k_step_zmarch<ST, TX, TY>, grid, dim3(T::THREADS), T::SMEM_BYTES, stream, tn.pdl != 0 && !shell, p.maps[cur], mm,
+                np, (const ST *)buf[cur], (ST *)buf[1 - cur], p.zchunk, tn.load_policy, tn.store_policy,
+                (tn.fill == 2 ? 1 : 0) | (shell ? 2 : 0));
+    if (shell) {
+      const int e1 = n[0] > n[1] ? n[0] : n[1], e2 = n[1] > n[2] ? n[1] : n[2];
+      dim3 sg((e1 + 31) / 32, (e2 + 7) / 8, 6);
+      k_step_shell3<ST><<<sg, dim3(32, 8), 0, stream>>>(m, np, (const ST *)buf[cur], (ST *)buf[1 - cur]);
+    }
+  }
   else
     launch_step(k_step_zmarch_up<ST, TX, TY>, grid, dim3(T::THREADS), T::SMEM_BYTES, stream, tn.pdl != 0, p.maps[cur], m, np,
                 (const ST *)buf[cur], (ST *)buf[1 - cur], p.zchunk, tn.load_policy, tn.store_policy, tn.fill == 2 ? 1 : 0);

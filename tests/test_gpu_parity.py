@@ -81,6 +81,7 @@ def kernels_for(islbm, sim):
             ks.append((islbm.KERNEL_TILED, dict(shape3d=3, chunk=3)))
             ks.append((islbm.KERNEL_TILED, dict(shape3d=4, fill=2)))
             ks.append((islbm.KERNEL_TILED, dict(shape3d=5)))
+            ks.append((islbm.KERNEL_TILED, dict(walls=1, chunk=6)))      # separate boundary kernel over the shell (A/B variant)
             for tune in (dict(shape3d=1), dict(shape3d=2, chunk=7)):      # wide tiles: fp32 storage only (shared memory)
                 try:
                     sim.set_tuning(**tune)
@@ -108,7 +109,7 @@ def kernels_for(islbm, sim):
 
 
 DEFAULT_TUNING = dict(chunk=0, l2promo=0, load_policy=0, store_policy=0, tx2d=0, serpentine=0, shape3d=0, pdl=1, fill=0,
-                      ring2d=0, rows2d=0, rows2d1=0)
+                      ring2d=0, rows2d=0, rows2d1=0, walls=0)
 
 
 def select(sim, k, tune):
