@@ -257,7 +257,9 @@ int islbm_set_kernel(islbm_t *h, int which);
  * ring: 1 before the weight rows and the CTA barrier, 2 after them, 0 automatic), "ring2d" (2-D fp64
  * ring: 3 stages with four CTAs per SM or 4 stages with three, 0 automatic), "rows2d" / "rows2d1"
  * (2-D chunk rule: longest chunk of a multi-wave launch / longest chunk for which a single wave
- * of CTAs is taken, 0 automatic), "walls" (3-D whole cavity: 0 wall rules inside the step kernel, 1 a separate
+ * of CTAs is taken, 0 automatic), "graph" (islbm_step(n) with n >= 32 replays a captured CUDA graph of 32 PDL-chained
+ * step kernels: 0 automatic = meshes of at most 2^18 nodes, whose steps are bound by the host's launch rate, 1 always,
+ * 2 never), "walls" (3-D whole cavity: 0 wall rules inside the step kernel, 1 a separate
  * boundary kernel over the shell of wall-adjacent nodes: the design BASELINE.json names, measured slower).  Results
  * do not depend on any of them.  Unknown key or negative value: ISLBM_ERR_ARG. */
 int islbm_set_tuning(islbm_t *h, const char *key, int value);

@@ -103,6 +103,9 @@ struct islbm {
   size_t peer_flag_off[2];     // the neighbour's step flag of its facing side
   int peer_flip[2];            // neighbour's `cur` XOR ours at connect time (both flip once per step)
   long long steps;             // steps since the last islbm_init / islbm_set_populations
+  cudaGraphExec_t graph_exec;  // kGraphSteps captured step kernels (small meshes), valid for buffer parity graph_cur
+  int graph_cur;
+  cudaStream_t cap_stream;     // private stream the graph is captured on (the caller's may be the legacy stream, which cannot capture)
   islbm_params prm;
   double buoy;
   double T0;               // reference temperature of the buoyancy force
@@ -127,7 +130,9 @@ struct islbm {
 };
 
 // (re)build the TMA plan of the tiled kernel for the current tuning
+static void drop_graph(islbm *h);
 static void make_tiled_plan(islbm *h) {
+  drop_graph(h);     // the captured launches hold the old tensor maps and launch configuration
   void *b0 = h->ws + h->cv.buf[0], *b1 = h->ws + h->cv.buf[1];
   if (h->dim == 2) {
     if (h->precision == ISLBM_F64) plan2_create<double>(h->plan2, h->n, h->dm.nxp, b0, b1, h->tune, h->stencil);
@@ -179,7 +184,9 @@ static int derive_params(islbm *h, const islbm_mesh *mesh) {
   return ISLBM_OK;
 }
 
+static void drop_graph(islbm *h);
 static void set_node_params(islbm *h) {
+  drop_graph(h);     // captured launches hold the node parameters by value
   const double tau = h->prm.tau_f;
   NodeParams &np = h->np;
   np.gbeta = h->prm.gbeta * h->buoy;
@@ -337,6 +344,9 @@ static int create_impl(islbm_t **out, const islbm_mesh *mesh, int lattice, doubl
   h->peer_base[0] = h->peer_base[1] = nullptr;
   h->peer_flip[0] = h->peer_flip[1] = 0;
   h->steps = 0;
+  h->graph_exec = nullptr;
+  h->graph_cur = 0;
+  h->cap_stream = nullptr;
   dm.flag_in[0] = dm.flag_in[1] = dm.flag_out[0] = dm.flag_out[1] = nullptr;
   dm.done_cnt = (unsigned long long *)(h->ws + h->cv.flags + 64);
   dm.step = 0;
@@ -388,7 +398,14 @@ static int create_impl(islbm_t **out, const islbm_mesh *mesh, int lattice, doubl
   return ISLBM_OK;
 }
 
-extern "C" void islbm_destroy(islbm_t *h) { delete h; }
+static void drop_graph(islbm *h);
+extern "C" void islbm_destroy(islbm_t *h) {
+  if (h) {
+    drop_graph(h);
+    if (h->cap_stream) cudaStreamDestroy(h->cap_stream);
+  }
+  delete h;
+}
 
 extern "C" int islbm_get_params(const islbm_t *h, islbm_params *out) {
   if (!h || !out) return fail(ISLBM_ERR_ARG, "NULL argument");
@@ -596,10 +613,73 @@ extern "C" int islbm_set_tuning(islbm_t *h, const char *key, int value) {
   else if (k == "ring2d") { if (value != 0 && value != 3 && value != 4) return fail(ISLBM_ERR_ARG, "ring2d must be 0 (automatic), 3 or 4"); t.ring2d = value; }
   else if (k == "rows2d") { if (value > kMaxChunk) return fail(ISLBM_ERR_ARG, "rows2d must be at most 64"); t.rows2d = value; }
   else if (k == "rows2d1") { if (value > kMaxChunk) return fail(ISLBM_ERR_ARG, "rows2d1 must be at most 64"); t.rows2d1 = value; }
+  else if (k == "graph") { if (value > 2) return fail(ISLBM_ERR_ARG, "graph must be 0 (automatic), 1 (always) or 2 (never)"); t.graph = value; }
   else if (k == "walls") { if (value > 1) return fail(ISLBM_ERR_ARG, "walls must be 0 (fused) or 1 (separate boundary kernel)"); t.walls = value; }
   else return fail(ISLBM_ERR_ARG, "unknown tuning key: " + k);
   make_tiled_plan(h);
   return ISLBM_OK;
+}
+
+// enqueue ONE time step on the handle's stream (kernel `which` of effective_kernel)
+static int enqueue_one_step(islbm *h, int which, bool fused) {
+  // fused halo exchange: this step writes buffer 1 - cur; the neighbour's `cur` is ours XOR the parity difference
+  // recorded at connect time (both flip once per step), and it reads the ghost layer we store from ITS buffer
+  // 1 - cur in its next step
+  for (int sd = 0; sd < 2; ++sd) {
+    const bool on = h->peer_base[sd] != nullptr;
+    const int peer_cur = h->cur ^ h->peer_flip[sd];
+    h->dm.peer[sd] = on ? (void *)(h->peer_base[sd] + h->peer_ghost_off[sd][1 - peer_cur]) : nullptr;
+    h->dm.peer_pitch[sd] = on ? (long long)(h->peer_pitch_bytes[sd] / h->st_bytes) : 0;
+    h->dm.flag_in[sd] = on ? (unsigned long long *)(h->ws + h->cv.flags) + sd : nullptr;
+    h->dm.flag_out[sd] = on ? (unsigned long long *)(h->peer_base[sd] + h->peer_flag_off[sd]) : nullptr;
+  }
+  h->dm.step = (unsigned long long)h->steps + 1ull;
+  if (fused && which != 2) {
+    k_slab_wait<<<1, 1, 0, h->stream>>>(h->dm);
+    h->launches++;
+  }
+  if (which == 2) {
+    void *bufs[2] = {h->ws + h->cv.buf[0], h->ws + h->cv.buf[1]};
+    cudaError_t e;
+    if (h->dim == 2)
+      e = h->precision == ISLBM_F64 ? launch2<double>(h->plan2, h->n, h->dm, h->np, h->cur, bufs, h->tune, h->stream)
+                                    : launch2<float>(h->plan2, h->n, h->dm, h->np, h->cur, bufs, h->tune, h->stream);
+    else
+      e = h->precision == ISLBM_F64 ? launch3<double>(h->plan3, h->n, h->dm, h->np, h->cur, bufs, h->tune, h->stream)
+                                    : launch3<float>(h->plan3, h->n, h->dm, h->np, h->cur, bufs, h->tune, h->stream);
+    if (e != cudaSuccess) return fail(ISLBM_ERR_CUDA, std::string("tiled step launch: ") + cudaGetErrorString(e));
+    h->launches += (h->dim == 3 && h->tune.walls == 1 && !h->is_slab && h->stencil == 0) ? 2 : 1;
+  } else if (which == 3) {
+#define CALL(D, T) launch_shift_step<D, T>(h)
+    DISPATCH(h, CALL);
+#undef CALL
+  } else {
+#define CALL(D, T) launch_generic_step<D, T>(h, true, nullptr, nullptr)
+    DISPATCH(h, CALL);
+#undef CALL
+  }
+  if (fused && which != 2) {
+    k_slab_publish<<<1, 1, 0, h->stream>>>(h->dm);
+    h->launches++;
+  }
+  h->cur ^= 1;
+  h->steps++;
+  h->other_is_pre = false;
+  return ISLBM_OK;
+}
+
+static void drop_graph(islbm *h) {
+  if (h->graph_exec) cudaGraphExecDestroy(h->graph_exec);
+  h->graph_exec = nullptr;
+}
+
+// Small meshes (a step kernel of a few microseconds): kGraphSteps consecutive step kernels, PDL-chained, are captured
+// once into a CUDA graph and replayed, so that islbm_step(n) costs n / kGraphSteps host launches instead of n (the
+// 64^2 mesh of BASELINE.json config 1 is bound by the host's launch rate otherwise).  The graph holds an even number
+// of steps, so it always starts on the same ping-pong buffer parity it was captured on.
+constexpr int kGraphSteps = 32;
+static bool graph_eligible(const islbm *h, int which, bool fused) {
+  return which == 2 && !fused && h->tune.graph != 2 && (h->tune.graph == 1 || h->nn <= (1LL << 18));
 }
 
 extern "C" int islbm_step(islbm_t *h, int n) {
@@ -610,50 +690,44 @@ extern "C" int islbm_step(islbm_t *h, int n) {
   if ((h->peer_base[0] || h->peer_base[1]) && which == 3)
     return fail(ISLBM_ERR_STATE, "the fused halo exchange is not available with the pure-shift kernel");
   const bool fused = h->peer_base[0] || h->peer_base[1];
-  for (int s = 0; s < n; ++s) {
-    // fused halo exchange: this step writes buffer 1 - cur; the neighbour's `cur` is ours XOR the parity difference
-    // recorded at connect time (both flip once per step), and it reads the ghost layer we store from ITS buffer
-    // 1 - cur in its next step
-    for (int sd = 0; sd < 2; ++sd) {
-      const bool on = h->peer_base[sd] != nullptr;
-      const int peer_cur = h->cur ^ h->peer_flip[sd];
-      h->dm.peer[sd] = on ? (void *)(h->peer_base[sd] + h->peer_ghost_off[sd][1 - peer_cur]) : nullptr;
-      h->dm.peer_pitch[sd] = on ? (long long)(h->peer_pitch_bytes[sd] / h->st_bytes) : 0;
-      h->dm.flag_in[sd] = on ? (unsigned long long *)(h->ws + h->cv.flags) + sd : nullptr;
-      h->dm.flag_out[sd] = on ? (unsigned long long *)(h->peer_base[sd] + h->peer_flag_off[sd]) : nullptr;
+  int left = n;
+  if (left >= kGraphSteps && graph_eligible(h, which, fused)) {
+    if (h->graph_exec && h->graph_cur != h->cur) drop_graph(h);
+    if (!h->graph_exec) {
+      cudaGraph_t g = nullptr;
+      const long long l0 = h->launches, s0 = h->steps;
+      const int c0 = h->cur;
+      const bool pre0 = h->other_is_pre;
+      if (!h->cap_stream) CUDA_TRY(cudaStreamCreateWithFlags(&h->cap_stream, cudaStreamNonBlocking));
+      cudaStream_t user = h->stream;
+      CUDA_TRY(cudaStreamBeginCapture(h->cap_stream, cudaStreamCaptureModeThreadLocal));
+      h->stream = h->cap_stream;       // the launches of the capture go to the private stream ...
+      int rc = ISLBM_OK;
+      for (int s = 0; s < kGraphSteps && rc == ISLBM_OK; ++s) rc = enqueue_one_step(h, which, false);
+      h->stream = user;                // ... the graph itself is launched on the caller's
+      const cudaError_t ec = cudaStreamEndCapture(h->cap_stream, &g);
+      h->launches = l0; h->steps = s0; h->cur = c0; h->other_is_pre = pre0;      // nothing has run yet
+      if (rc != ISLBM_OK || ec != cudaSuccess || !g) {
+        if (g) cudaGraphDestroy(g);
+        cudaGetLastError();
+        return rc != ISLBM_OK ? rc : fail(ISLBM_ERR_CUDA, std::string("graph capture: ") + cudaGetErrorString(ec));
+      }
+      const cudaError_t ei = cudaGraphInstantiate(&h->graph_exec, g, 0);
+      cudaGraphDestroy(g);
+      if (ei != cudaSuccess) { h->graph_exec = nullptr; return fail(ISLBM_ERR_CUDA, std::string("graph instantiate: ") + cudaGetErrorString(ei)); }
+      h->graph_cur = h->cur;
     }
-    h->dm.step = (unsigned long long)h->steps + 1ull;
-    if (fused && which != 2) {
-      k_slab_wait<<<1, 1, 0, h->stream>>>(h->dm);
-      h->launches++;
+    while (left >= kGraphSteps) {
+      CUDA_TRY(cudaGraphLaunch(h->graph_exec, h->stream));
+      h->launches += kGraphSteps;
+      h->steps += kGraphSteps;
+      h->other_is_pre = false;
+      left -= kGraphSteps;           // an even number of steps: `cur` is unchanged
     }
-    if (which == 2) {
-      void *bufs[2] = {h->ws + h->cv.buf[0], h->ws + h->cv.buf[1]};
-      cudaError_t e;
-      if (h->dim == 2)
-        e = h->precision == ISLBM_F64 ? launch2<double>(h->plan2, h->n, h->dm, h->np, h->cur, bufs, h->tune, h->stream)
-                                      : launch2<float>(h->plan2, h->n, h->dm, h->np, h->cur, bufs, h->tune, h->stream);
-      else
-        e = h->precision == ISLBM_F64 ? launch3<double>(h->plan3, h->n, h->dm, h->np, h->cur, bufs, h->tune, h->stream)
-                                      : launch3<float>(h->plan3, h->n, h->dm, h->np, h->cur, bufs, h->tune, h->stream);
-      if (e != cudaSuccess) return fail(ISLBM_ERR_CUDA, std::string("tiled step launch: ") + cudaGetErrorString(e));
-      h->launches += (h->dim == 3 && h->tune.walls == 1 && !h->is_slab && h->stencil == 0) ? 2 : 1;
-    } else if (which == 3) {
-#define CALL(D, T) launch_shift_step<D, T>(h)
-      DISPATCH(h, CALL);
-#undef CALL
-    } else {
-#define CALL(D, T) launch_generic_step<D, T>(h, true, nullptr, nullptr)
-      DISPATCH(h, CALL);
-#undef CALL
-    }
-    if (fused && which != 2) {
-      k_slab_publish<<<1, 1, 0, h->stream>>>(h->dm);
-      h->launches++;
-    }
-    h->cur ^= 1;
-    h->steps++;
-    h->other_is_pre = false;
+  }
+  for (int s = 0; s < left; ++s) {
+    const int rc = enqueue_one_step(h, which, fused);
+    if (rc) return rc;
   }
   CUDA_TRY(cudaPeekAtLastError());
   return ISLBM_OK;

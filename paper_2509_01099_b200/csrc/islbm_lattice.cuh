@@ -37,7 +37,18 @@ struct NodeParams {
   // relaxation rate x 1/|moment row|^2 (x the forcing factor), folded once on the host by fold_node_params: the
   // kernels read them as constant-bank operands, so Delta m_k / |row_k|^2 is one multiply and one fused multiply-add
   double k[21];
+  // the same temperature constants in fp32, for the fp32-storage kernels, which collide the temperature populations in
+  // fp32 (ISLBM_G_FP32): kf[0] = -q_k/2, kf[1] = -q_e/20 | -q_e/42, kf[2] = -q_e/12 (3-D), kf[3] = -q_e/4, kf[4] = a_T
+  float kf[5];
 };
+
+// fp32-storage kernels: collide the temperature populations g in fp32 (they are stored in fp32 and T tolerates it:
+// BASELINE.json asks 1e-5 on T after 1000 steps, the fp64 collision gives 7e-7, this one the same order; the flow
+// populations keep the fp64 collision, whose error on u sits at 4-6e-6 of the same bar).  Saves 14 of the 54
+// conversions and 50 of the 293 fp64 instructions per node of the latency-bound fp32-storage step.
+#ifndef ISLBM_G_FP32
+#define ISLBM_G_FP32 1
+#endif
 
 // k[] of NodeParams for the lattice of dimension dim, from s_nu, s_q, hs_nu, hs_q, q_k, q_e (index map: collide_node)
 inline void fold_node_params(NodeParams &p, int dim) {
@@ -49,6 +60,7 @@ inline void fold_node_params(NodeParams &p, int dim) {
     p.k[6] = -p.s_nu / 4.0;   p.k[7] = -2.0 * p.hs_nu / 4.0;          // pxx: k6 (..) + k7 vF
     p.k[14] = -p.s_nu / 4.0;  p.k[15] = p.hs_nu / 4.0;                // pxy: k14 (..) + k15 u Fy
     p.k[17] = -p.q_k / 2.0;   p.k[18] = -p.q_e / 20.0;  p.k[20] = -p.q_e / 4.0;
+    p.kf[2] = 0.f;
   } else {
     p.k[0] = -p.s_nu / 2394.0;  p.k[1] = 38.0 * p.hs_nu / 2394.0;     // e
     p.k[2] = -p.s_nu / 252.0;   p.k[3] = -11.0 * p.hs_nu / 252.0;     // eps
@@ -60,7 +72,12 @@ inline void fold_node_params(NodeParams &p, int dim) {
     p.k[14] = -p.s_nu / 4.0;    p.k[15] = p.hs_nu / 4.0;              // pxy, pyz, pxz
     p.k[16] = -p.s_q / 8.0;                                           // m
     p.k[17] = -p.q_k / 2.0;  p.k[18] = -p.q_e / 42.0;  p.k[19] = -p.q_e / 12.0;  p.k[20] = -p.q_e / 4.0;
+    p.kf[2] = (float)p.k[19];
   }
+  p.kf[0] = (float)p.k[17];
+  p.kf[1] = (float)p.k[18];
+  p.kf[3] = (float)p.k[20];
+  p.kf[4] = (float)p.a_T;
 }
 
 template <int DIM> struct Lat;
@@ -167,16 +184,22 @@ ISLBM_HD void upd(float &a, double d) { a = (float)((double)a + d); }
 
 template <bool DEV = false, typename FT>
 ISLBM_HD void collide_node(FT (&fio)[9], FT (&gio)[5], const NodeParams &p) {
-  double f[9], g[5];
+  constexpr bool GF = sizeof(FT) == 4 && ISLBM_G_FP32;   // temperature collision in fp32 (fp32 storage)
+  double f[9], g[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
 #ifdef __CUDA_ARCH__
 #pragma unroll
 #endif
   for (int q = 0; q < 9; ++q) f[q] = (double)fio[q];
+  float Tf = 0.f;
+  if constexpr (GF) {
+    Tf = (float)gio[0] + (float)gio[1] + (float)gio[2] + (float)gio[3] + (float)gio[4];
+  } else {
 #ifdef __CUDA_ARCH__
 #pragma unroll
 #endif
-  for (int q = 0; q < 5; ++q) g[q] = (double)gio[q];
-  const double T = g[0] + g[1] + g[2] + g[3] + g[4];
+    for (int q = 0; q < 5; ++q) g[q] = (double)gio[q];
+  }
+  const double T = GF ? (double)Tf : g[0] + g[1] + g[2] + g[3] + g[4];
   const double sa = (f[1] + f[3]) + (f[2] + f[4]);   // axis shell
   const double sd = (f[5] + f[7]) + (f[6] + f[8]);   // diagonal shell
   const double rsum = f[0] + sa + sd;
@@ -208,14 +231,29 @@ ISLBM_HD void collide_node(FT (&fio)[9], FT (&gio)[5], const NodeParams &p) {
   const double dpxx = fma(p.k[6], mpxx - rho * (u * u - v * v), p.k[7] * vF);
   const double dpxy = fma(p.k[14], mpxy - rho * (u * v), p.k[15] * (u * Fy));
   // temperature moments (Eq. 15 order)
-  const double n1 = g[1] - g[3], n2 = g[2] - g[4];
-  const double gs = (g[1] + g[3]) + (g[2] + g[4]);
-  const double n3 = -4.0 * g[0] + gs;
-  const double n4 = (g[1] + g[3]) - (g[2] + g[4]);
-  const double e1 = p.k[17] * (n1 - u * T);
-  const double e2 = p.k[17] * (n2 - v * T);
-  const double e3 = p.k[18] * (n3 - p.a_T * T);
-  const double e4 = p.k[20] * n4;
+  double n1 = 0, n2 = 0, gs = 0, n3 = 0, n4 = 0, e1 = 0, e2 = 0, e3 = 0, e4 = 0;
+  if constexpr (GF) {
+    const float g0 = (float)gio[0], g1 = (float)gio[1], g2 = (float)gio[2], g3 = (float)gio[3], g4 = (float)gio[4];
+    const float uf = (float)u, vf = (float)v;
+    const float a1 = p.kf[0] * ((g1 - g3) - uf * Tf);
+    const float a2 = p.kf[0] * ((g2 - g4) - vf * Tf);
+    const float a3 = p.kf[1] * ((-4.0f * g0 + ((g1 + g3) + (g2 + g4))) - p.kf[4] * Tf);
+    const float a4 = p.kf[3] * ((g1 + g3) - (g2 + g4));
+    gio[0] = (FT)(g0 + -4.0f * a3);
+    gio[1] = (FT)(g1 + (a1 + a3 + a4));
+    gio[2] = (FT)(g2 + (a2 + a3 - a4));
+    gio[3] = (FT)(g3 + (-a1 + a3 + a4));
+    gio[4] = (FT)(g4 + (-a2 + a3 - a4));
+  } else {
+    n1 = g[1] - g[3], n2 = g[2] - g[4];
+    gs = (g[1] + g[3]) + (g[2] + g[4]);
+    n3 = -4.0 * g[0] + gs;
+    n4 = (g[1] + g[3]) - (g[2] + g[4]);
+    e1 = p.k[17] * (n1 - u * T);
+    e2 = p.k[17] * (n2 - v * T);
+    e3 = p.k[18] * (n3 - p.a_T * T);
+    e4 = p.k[20] * n4;
+  }
   // f+ = f + M^T d
   const double ca = -de - 2.0 * deps;          // common part, axis shell
   const double cd = 2.0 * de + deps;           // common part, diagonal shell
@@ -230,11 +268,13 @@ ISLBM_HD void collide_node(FT (&fio)[9], FT (&gio)[5], const NodeParams &p) {
   upd(fio[6], cd - sx + sy - dpxy);
   upd(fio[7], cd - sx - sy + dpxy);
   upd(fio[8], cd + sx - sy - dpxy);
-  upd(gio[0], -4.0 * e3);
-  upd(gio[1], e1 + e3 + e4);
-  upd(gio[2], e2 + e3 - e4);
-  upd(gio[3], -e1 + e3 + e4);
-  upd(gio[4], -e2 + e3 - e4);
+  if constexpr (!GF) {
+    upd(gio[0], -4.0 * e3);
+    upd(gio[1], e1 + e3 + e4);
+    upd(gio[2], e2 + e3 - e4);
+    upd(gio[3], -e1 + e3 + e4);
+    upd(gio[4], -e2 + e3 - e4);
+  }
 }
 
 // macroscopic fields from POST-collision populations: rho and T are collision
@@ -256,16 +296,22 @@ ISLBM_HD void fields_from_post(const double (&f)[9], const double (&g)[5], const
 // ---------------------------------------------------------------------------
 template <bool DEV = false, typename FT>
 ISLBM_HD void collide_node(FT (&fio)[19], FT (&gio)[7], const NodeParams &p) {
-  double f[19], g[7];
+  constexpr bool GF = sizeof(FT) == 4 && ISLBM_G_FP32;   // temperature collision in fp32 (fp32 storage)
+  double f[19], g[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
 #ifdef __CUDA_ARCH__
 #pragma unroll
 #endif
   for (int q = 0; q < 19; ++q) f[q] = (double)fio[q];
+  float Tf = 0.f;
+  if constexpr (GF) {
+    Tf = (float)gio[0] + (((float)gio[1] + (float)gio[2]) + ((float)gio[3] + (float)gio[4]) + ((float)gio[5] + (float)gio[6]));
+  } else {
 #ifdef __CUDA_ARCH__
 #pragma unroll
 #endif
-  for (int q = 0; q < 7; ++q) g[q] = (double)gio[q];
-  const double T = g[0] + ((g[1] + g[2]) + (g[3] + g[4]) + (g[5] + g[6]));
+    for (int q = 0; q < 7; ++q) g[q] = (double)gio[q];
+  }
+  const double T = GF ? (double)Tf : g[0] + ((g[1] + g[2]) + (g[3] + g[4]) + (g[5] + g[6]));
   // pair sums / differences
   const double px = f[1] + f[2], py = f[3] + f[4], pz = f[5] + f[6];
   const double ax = f[1] - f[2], ay = f[3] - f[4], az = f[5] - f[6];
@@ -317,7 +363,27 @@ ISLBM_HD void collide_node(FT (&fio)[19], FT (&gio)[7], const NodeParams &p) {
   // expressions: under their 168-register cap the folded form spills 164 instead of 60 bytes and measures 11 % slower.
   constexpr bool FOLD = sizeof(FT) == 8;
   const double djy = Fy * 0.1;
-  const double gx = g[1] + g[2], gy = g[3] + g[4], gz = g[5] + g[6];
+  double gx = 0, gy = 0, gz = 0;
+  if constexpr (!GF) gx = g[1] + g[2], gy = g[3] + g[4], gz = g[5] + g[6];
+  if constexpr (GF) {
+    const float g0 = (float)gio[0], g1 = (float)gio[1], g2 = (float)gio[2], g3 = (float)gio[3], g4 = (float)gio[4],
+                g5 = (float)gio[5], g6 = (float)gio[6];
+    const float uf = (float)u, vf = (float)v, wf = (float)w;
+    const float hx = g1 + g2, hy = g3 + g4, hz = g5 + g6;
+    const float a1 = p.kf[0] * ((g1 - g2) - uf * Tf);
+    const float a2 = p.kf[0] * ((g3 - g4) - vf * Tf);
+    const float a3 = p.kf[0] * ((g5 - g6) - wf * Tf);
+    const float a4 = p.kf[1] * ((-6.0f * g0 + (hx + hy + hz)) - p.kf[4] * Tf);
+    const float a5 = p.kf[2] * (2.0f * hx - hy - hz);
+    const float a6 = p.kf[3] * (hy - hz);
+    gio[0] = (FT)(g0 + -6.0f * a4);
+    gio[1] = (FT)(g1 + (a1 + a4 + 2.0f * a5));
+    gio[2] = (FT)(g2 + (-a1 + a4 + 2.0f * a5));
+    gio[3] = (FT)(g3 + (a2 + a4 - a5 + a6));
+    gio[4] = (FT)(g4 + (-a2 + a4 - a5 + a6));
+    gio[5] = (FT)(g5 + (a3 + a4 - a5 - a6));
+    gio[6] = (FT)(g6 + (-a3 + a4 - a5 - a6));
+  }
   double de, deps, dqx, dqy, dqz, d3pxx, d3pixx, dpww, dpiww, dpxy, dpyz, dpxz, dmx, dmy, dmz, e1, e2, e3, e4, e5, e6;
   if constexpr (FOLD) {
     const double r23 = (2.0 / 3.0) * rho;
@@ -396,13 +462,15 @@ ISLBM_HD void collide_node(FT (&fio)[19], FT (&gio)[7], const NodeParams &p) {
   upd(fio[16], cd + nyz - (sy + dmy) + (sz - dmz) - dpyz);
   upd(fio[17], cd + nyz + (sy + dmy) - (sz - dmz) - dpyz);
   upd(fio[18], cd + nyz - (sy + dmy) - (sz - dmz) + dpyz);
-  upd(gio[0], -6.0 * e4);
-  upd(gio[1], e1 + e4 + 2.0 * e5);
-  upd(gio[2], -e1 + e4 + 2.0 * e5);
-  upd(gio[3], e2 + e4 - e5 + e6);
-  upd(gio[4], -e2 + e4 - e5 + e6);
-  upd(gio[5], e3 + e4 - e5 - e6);
-  upd(gio[6], -e3 + e4 - e5 - e6);
+  if constexpr (!GF) {
+    upd(gio[0], -6.0 * e4);
+    upd(gio[1], e1 + e4 + 2.0 * e5);
+    upd(gio[2], -e1 + e4 + 2.0 * e5);
+    upd(gio[3], e2 + e4 - e5 + e6);
+    upd(gio[4], -e2 + e4 - e5 + e6);
+    upd(gio[5], e3 + e4 - e5 - e6);
+    upd(gio[6], -e3 + e4 - e5 - e6);
+  }
 }
 
 ISLBM_HD void fields_from_post(const double (&f)[19], const double (&g)[7], const NodeParams &p,

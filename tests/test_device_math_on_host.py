@@ -56,7 +56,7 @@ def test_factored_collision_matches_oracle(harness, dim):
         harness.harness_collide_dev(dim, dptr(fd), dptr(gd), dptr(prm))
         assert np.abs(fd - fo).max() < 2e-16 * 8
         assert np.abs(gd - go).max() < 2e-16 * 8
-        # fp32-storage form: fp32 deviations in and out, all arithmetic in fp64 (3-D: the unfolded expressions);
+        # fp32-storage form: fp32 deviations in and out, flow arithmetic in fp64 (3-D: the unfolded expressions);
         # on fp32-representable inputs the result is the oracle's, rounded once to fp32
         wts = np.empty(o.qf); e_ = np.empty(3 * o.qf, dtype=np.int32); opp_ = np.empty(o.qf, dtype=np.int32)
         harness.harness_tables(dim, e_.ctypes.data_as(C.POINTER(C.c_int)), opp_.ctypes.data_as(C.POINTER(C.c_int)), dptr(wts))
@@ -66,7 +66,10 @@ def test_factored_collision_matches_oracle(harness, dim):
         d_io, g_io = dev32.copy(), g32.copy()
         harness.harness_collide_dev_f32(dim, d_io.ctypes.data_as(C.POINTER(C.c_float)), g_io.ctypes.data_as(C.POINTER(C.c_float)), dptr(prm))
         assert np.abs(d_io.astype(np.float64) - (fo32 - wts)).max() <= 2.0 ** -24 * np.abs(fo32 - wts).max() * 1.01
-        assert np.abs(g_io.astype(np.float64) - go32).max() <= 2.0 ** -24 * np.abs(go32).max() * 1.01
+        # temperature populations: the fp32-storage kernels collide them in fp32 (ISLBM_G_FP32: a dozen fp32 operations
+        # on values of the input's size), so the bound is in units of the INPUT's magnitude: 16 x 2^-24 (measured over
+        # 5000 far-from-equilibrium nodes: 7.7 in 2-D, 12.0 in 3-D)
+        assert np.abs(g_io.astype(np.float64) - go32).max() <= 16 * 2.0 ** -24 * np.abs(g32).max()
         # fields from post-collision populations == fields of the pre-collision state
         out = np.empty(5)
         harness.harness_fields_post(dim, dptr(fh), dptr(gh), dptr(prm), dptr(out))

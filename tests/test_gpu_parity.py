@@ -109,7 +109,7 @@ def kernels_for(islbm, sim):
 
 
 DEFAULT_TUNING = dict(chunk=0, l2promo=0, load_policy=0, store_policy=0, tx2d=0, serpentine=0, shape3d=0, pdl=1, fill=0,
-                      ring2d=0, rows2d=0, rows2d1=0, walls=0)
+                      ring2d=0, rows2d=0, rows2d1=0, walls=0, graph=0)
 
 
 def select(sim, k, tune):
@@ -733,6 +733,33 @@ def test_no_kernel_writes_outside_the_workspace(islbm, dim, ns, prec):
     sim.nusselt(), sim.nusselt_middle(), sim.steady_residual(), sim.steady_residual(), sim.fields()
     torch.cuda.synchronize()
     assert sim.guards_intact()
+
+
+@pytest.mark.parametrize("dim,ns,prec", [(2, (64, 64), 0), (2, (70, 45), 1), (3, (37, 21, 19), 0)])
+def test_graph_replay_equals_plain_launches_bitwise(islbm, dim, ns, prec):
+    """islbm_step(n >= 32) on a small mesh replays a captured CUDA graph of 32 PDL-chained step kernels: identical
+    bits to launching the kernels one by one (graph = 2), whatever mix of call sizes, and after re-planning."""
+    coords, delta = ragged_coords(dim, ns + (1,), (1.3, 1.2, 1.1))
+    H_lu = (coords[1][-1] - coords[1][0] + delta) / delta
+    mk = lambda: islbm.Islbm(coords, delta, 0.71 * (0.1 * H_lu / 0.03) ** 2, 0.71, 0.1 * SQ3, precision=prec)
+    a, b = mk(), mk()
+    b.set_tuning(graph=2)
+    for s_ in (a, b):
+        s_.init(1, 1e-3)
+    for n in (100, 1, 33, 64, 7):
+        l0 = a.launch_count
+        a.step(n)
+        b.step(n)
+        assert a.launch_count - l0 == n                        # the count is of kernels, not of host launches
+    fa, ga = a.get_populations()
+    fb, gb = b.get_populations()
+    assert torch.equal(fa, fb) and torch.equal(ga, gb)
+    a.set_tuning(chunk=3)                                      # re-plan: the captured graph is dropped
+    a.step(70)
+    b.step(70)
+    fa, ga = a.get_populations()
+    fb, gb = b.get_populations()
+    assert torch.equal(fa, fb) and torch.equal(ga, gb)
 
 
 def test_state_errors_and_launch_accounting(islbm):
