@@ -132,10 +132,13 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
   pdl_launch_dependents();
 
   const int x0 = blockIdx.x * T::TX;
-  // the emitted rows are split evenly over the gridDim.y chunks (lengths differ by at most one, all <= kMaxChunk)
+  // the emitted rows are split evenly over the gridDim.y chunks (lengths differ by at most one, all <= kMaxChunk):
+  // the first rows % chunks chunks are one row longer
   const int rows = m.em_hi - m.em_lo;
-  const int y0 = m.em_lo + (int)((long long)blockIdx.y * rows / gridDim.y);
-  const int y1 = m.em_lo + (int)((long long)(blockIdx.y + 1) * rows / gridDim.y);
+  // (32-bit arithmetic: a 64-bit division here cost every thread ~90 instructions per 3-4-row CTA)
+  const int cbase = rows / (int)gridDim.y, crem = rows - cbase * (int)gridDim.y;
+  const int y0 = m.em_lo + (int)blockIdx.y * cbase + min((int)blockIdx.y, crem);
+  const int y1 = y0 + cbase + ((int)blockIdx.y < crem ? 1 : 0);
   const int yf = DIR > 0 ? y0 : y1 - 1;
   const int nstage = 2 + (y1 - y0);
   const bool b_lo = y0 == m.em_lo, b_hi = y1 == m.em_hi;   // slab boundary CTAs (fused exchange; islbm_tiled3.cuh)
@@ -361,8 +364,10 @@ k_step_ymarch_up(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, con
 
   const int x0 = blockIdx.x * T::TX;
   const int rows = m.em_hi - m.em_lo;
-  const int y0 = m.em_lo + (int)((long long)blockIdx.y * rows / gridDim.y);
-  const int y1 = m.em_lo + (int)((long long)(blockIdx.y + 1) * rows / gridDim.y);
+  // (32-bit arithmetic: a 64-bit division here cost every thread ~90 instructions per 3-4-row CTA)
+  const int cbase = rows / (int)gridDim.y, crem = rows - cbase * (int)gridDim.y;
+  const int y0 = m.em_lo + (int)blockIdx.y * cbase + min((int)blockIdx.y, crem);
+  const int y1 = y0 + cbase + ((int)blockIdx.y < crem ? 1 : 0);
   const int nstage = 2 + (y1 - y0);
   const uint64_t lpol = make_policy(load_policy);
   const uint64_t spol = make_policy(store_policy);
@@ -627,7 +632,7 @@ inline void launch2_cfg(const Plan2 &p, const int *n, const DevMesh &m, const No
   const int rows = m.em_hi - m.em_lo;
   // with three rows in flight per CTA a single wave pays up to 12-row chunks (642^2: 0.75 -> 0.82)
   const int nc = chunks2(rows, p.per_wave, tn.chunk, tn.rows2d1 ? tn.rows2d1 : (p.stages >= 4 ? 12 : 8),
-                         tn.rows2d ? tn.rows2d : 4);
+                         tn.rows2d ? tn.rows2d : (sizeof(ST) == 4 ? 8 : 4));   // fp32 storage: 8 (1024^2 0.637 -> 0.672, 4096^2 0.71 -> 0.75)
   dim3 grid((n[0] + T::TX - 1) / T::TX, nc, 1);
   // first ring fill (measured, profiles/r1_c3_1024sq_ymarch_v4.md): a single-wave launch is 2-5 % faster with the
   // fill after the CTA barrier, a multi-wave launch 2-6 % faster with the fill first
