@@ -555,7 +555,8 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
       collide_node<DEV>(f, g, np);
       if (valid) {
         store_node<3, DEV>(dst + c, m.nnp, f, g, spol, std::make_integer_sequence<int, 26>{});
-        peer_store_node<3, ST, DEV>(m, z, c - (long long)z * plane, f, g);
+        if (m.peer[0] != nullptr || m.peer[1] != nullptr)     // slab boundary layers only: keep the 64-bit index arithmetic out of the march
+          peer_store_node<3, ST, DEV>(m, z, c - (long long)z * plane, f, g);
       }
       c += plane;
     }
