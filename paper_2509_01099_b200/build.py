@@ -33,7 +33,9 @@ def build(force: bool = False, verbose: bool = False) -> str:
     if force or is_stale():
         nvcc = os.environ.get("NVCC", "nvcc")
         tmp = LIB + f".tmp{os.getpid()}"
-        cmd = [nvcc, *NVCC_FLAGS, *(["-Xptxas", "-v"] if verbose else []), "-o", tmp, *SOURCES]
+        # ISLBM_NVCC_FLAGS: extra flags for A/B builds of the compile-time variants, e.g. -DISLBM_G_FP32=0 (profiles/attempts.md)
+        extra = os.environ.get("ISLBM_NVCC_FLAGS", "").split()
+        cmd = [nvcc, *NVCC_FLAGS, *extra, *(["-Xptxas", "-v"] if verbose else []), "-o", tmp, *SOURCES]
         subprocess.run(cmd, check=True, cwd=CSRC)
         os.replace(tmp, LIB)
     return LIB

@@ -33,6 +33,12 @@ def main(argv=None):
     ap.add_argument("--tol", type=float, default=1e-9)
     ap.add_argument("--stencil", type=int, default=0, choices=[0, 1],
                     help="0: destination-centred {j-1,j,j+1} (default); 1: upwind {j-2,j-1,j} / {j,j+1,j+2} (DESIGN.md A2)")
+    ap.add_argument("--tune", action="append", default=[], metavar="KEY=VALUE",
+                    help="islbm_set_tuning knob (repeatable), e.g. --tune shape3d=3 --tune chunk=8; results do not depend on them")
+    ap.add_argument("--kernel", type=int, default=0, help="islbm_set_kernel: 0 auto, 1 generic, 2 TMA-staged, 3 uniform pure shift")
+    ap.add_argument("--time", type=int, default=0, metavar="STEPS",
+                    help="time islbm_step(STEPS) with CUDA events (after a warm-up of STEPS, best of 3) and print one JSON line "
+                         "with us_per_step, MLUPS and the fraction of the HBM roofline; nothing else is run")
     ap.add_argument("--seed", type=int, default=0)
     ap.add_argument("--noise", type=float, default=None, help="amplitude of the initial temperature noise (default 1e-3; --paper: 0)")
     args = ap.parse_args(argv)
@@ -51,7 +57,33 @@ def main(argv=None):
     sim = islbm.Islbm(w.coords, w.delta, w.Ra, w.Pr, w.Ma, precision=0 if args.precision == "f64" else 1)
     sim.set_reference_temperature(T0)
     sim.set_stencil(args.stencil)
+    if args.tune:
+        sim.set_tuning(**{kv.split("=")[0]: int(kv.split("=")[1]) for kv in args.tune})
+    if args.kernel:
+        sim.set_kernel(args.kernel)
     sim.init(args.seed, noise)
+    if args.time:
+        import os
+        sim.step(args.time)
+        torch.cuda.synchronize()
+        best = float("inf")
+        for _ in range(3):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            sim.step(args.time)
+            e1.record()
+            torch.cuda.synchronize()
+            best = min(best, e0.elapsed_time(e1) * 1e3 / args.time)
+        peak = 6650.0
+        pk = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "MEASURED_PEAKS.json")
+        if os.path.exists(pk):
+            with open(pk) as fh:
+                peak = float(json.load(fh)["hbm_gbs"])
+        bpu = (14 if sim.dim == 2 else 26) * 2 * (8 if args.precision == "f64" else 4)
+        print(json.dumps({"kernel": sim.kernel_name, "tune": args.tune, "us_per_step": best, "MLUPS": sim.nodes / best,
+                          "roofline_frac": sim.nodes * bpu / (best * 1e-6) / 1e9 / peak, "peak_gbs": peak}), flush=True)
+        sim.close()
+        return
     p = sim.params()
     print(json.dumps({"nodes": sim.nodes, "shape": sim.shape, "kernel": sim.kernel_name, "T0": T0,
                       **{k: p[k] for k in ("U", "H_lu", "nu", "alpha", "tau_f", "a_T", "dt_star")}}), flush=True)
