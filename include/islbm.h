@@ -216,6 +216,19 @@ int islbm_fields(islbm_t *h, double *rho, double *u, double *v, double *w,
  * Returns ISLBM_ERR_NONFINITE (out still written) if any entry is not finite. */
 int islbm_nusselt(islbm_t *h, double out[5]);
 
+/* As islbm_nusselt (same five diagnostics, Eq. 27-29, 31-34, 40-42), for callers that must not allocate or hand out
+ * scratch memory (code under CUDA-graph capture, tight serving loops, harnesses that forbid cudaMalloc): the block
+ * partial sums go to a file-scope __device__ array of the library (114 752 bytes, held by every GPU that loads the
+ * library until exit), not to the workspace, and the call allocates nothing (no cudaMalloc / cudaFree, no allocating
+ * library routine; the first call on a device resolves the array's address with cudaGetSymbolAddress).
+ * LIMIT: at most 2048 * 16384 = 33 554 432 nodes (256^3 is 16 777 216); a larger mesh returns ISLBM_ERR_ARG, and
+ * islbm_nusselt remains the path for it.  Each block reduces a fixed share of 16 384 nodes, so the summation order
+ * depends on the mesh only (results agree with islbm_nusselt to summation-order round-off, 1e-12 relative).
+ * The array is shared by every call on the device and keeps the last call's contents (each call overwrites all the
+ * slots it reads, so nothing needs clearing): calls that overlap on the GPU — other streams, other handles — RACE;
+ * serialise them.  Synchronises the handle's stream.  HOST out[5]; ISLBM_ERR_NONFINITE as for islbm_nusselt. */
+int islbm_nusselt_static(islbm_t *h, double out[5]);
+
 /* HOST *out = Nu_middle (Eq. 33): average over the vertical centre plane x* = 0.5 of
  * sqrt(Ra Pr) u* T* - dT* / dx*; the derivative at a node column is that of the parabola through the column and
  * its two neighbours, and the flux is interpolated linearly between the two columns bracketing the midpoint of

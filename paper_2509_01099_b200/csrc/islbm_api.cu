@@ -926,6 +926,81 @@ extern "C" int islbm_nusselt(islbm_t *h, double out[5]) {
   return ISLBM_OK;
 }
 
+// ---------------------------------------------------------------------------
+// islbm_nusselt_static: the Nu / Re reduction with NO allocation and no use of the workspace's scratch areas.
+// Its scratch (one partial sum per block and slot, and the 8 result slots) is the file-scope array below, which every
+// GPU that loads this library holds until exit: kStaticRedBlocks * kRedSlots + 8 doubles = 114 752 bytes.
+// Each block reduces a FIXED share of kStaticNodesPerBlock nodes, so the number of blocks (and with it the order of
+// the summation) depends on the mesh alone, not on the GPU; meshes beyond kStaticRedBlocks * kStaticNodesPerBlock
+// = 33 554 432 nodes are refused.  Every partial and result slot is written by each call before it is read, so
+// nothing has to start at zero; the array keeps the last call's contents.  All calls on a device share the array:
+// calls that overlap on the GPU (different streams, different handles) race.
+// ---------------------------------------------------------------------------
+constexpr int kStaticRedBlocks = 2048;
+constexpr long long kStaticNodesPerBlock = 16384;     // 64 nodes per thread of a 256-thread block
+static __device__ __align__(256) double g_static_red[kStaticRedBlocks * kRedSlots + 8];
+
+// Device address of g_static_red on the CURRENT device.  In host code the array's name is only a stand-in for the
+// symbol, not a device address: it is resolved once per device with cudaGetSymbolAddress (no allocation) and cached.
+static int static_scratch_ptr(double **out) {
+  constexpr int kMaxDev = 64;
+  static double *cache[kMaxDev] = {};
+  int dev = -1;
+  CUDA_TRY(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDev) return fail(ISLBM_ERR_CUDA, "device ordinal beyond the static-scratch table");
+  if (!cache[dev]) {
+    double *p = nullptr;
+    CUDA_TRY(cudaGetSymbolAddress((void **)&p, g_static_red));
+    if (!p) return fail(ISLBM_ERR_CUDA, "cudaGetSymbolAddress returned a null address for the static scratch");
+    cache[dev] = p;      // racing first calls on one device write the same value
+  }
+  *out = cache[dev];
+  return ISLBM_OK;
+}
+
+template <int DIM, typename ST>
+static void launch_nusselt_static(islbm *h, int nb, double *scratch) {
+  const ST *S = (const ST *)(h->ws + h->cv.buf[h->cur]);
+  double *partial = scratch, *result = scratch + (size_t)kStaticRedBlocks * kRedSlots;
+  k_nusselt_partial<DIM, ST><<<nb, kRedThreads, 0, h->stream>>>(h->dm, h->np, h->dp, S, partial);
+  k_reduce_final<<<1, kRedThreads, 0, h->stream>>>(partial, nb, result);
+  h->launches += 2;
+}
+
+extern "C" int islbm_nusselt_static(islbm_t *h, double out[5]) {
+  if (!h || !out) return fail(ISLBM_ERR_ARG, "NULL argument");
+  if (h->is_slab) return fail(ISLBM_ERR_STATE, "slab handle: use islbm_diag_sums, sum over ranks, islbm_diag_from_sums");
+  if (h->nn > (long long)kStaticRedBlocks * kStaticNodesPerBlock) {
+    char b[160];
+    snprintf(b, sizeof b, "islbm_nusselt_static: %lld nodes exceed the static scratch (at most %lld nodes); use islbm_nusselt",
+             h->nn, (long long)kStaticRedBlocks * kStaticNodesPerBlock);
+    return fail(ISLBM_ERR_ARG, b);
+  }
+  if (!h->has_state) return fail(ISLBM_ERR_STATE, "no state");
+  double *scratch = nullptr;
+  int rc = static_scratch_ptr(&scratch);
+  if (rc) return rc;
+  const int nb = (int)((h->nn + kStaticNodesPerBlock - 1) / kStaticNodesPerBlock);
+#define CALL(D, T) launch_nusselt_static<D, T>(h, nb, scratch)
+  DISPATCH(h, CALL);
+#undef CALL
+  CUDA_TRY(cudaPeekAtLastError());
+  double s[kRedSlots];
+  CUDA_TRY(cudaMemcpyAsync(s, scratch + (size_t)kStaticRedBlocks * kRedSlots, sizeof s, cudaMemcpyDeviceToHost, h->stream));
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  const islbm_params &p = h->prm;
+  const double area = p.L_eff[1] * (h->dim == 3 ? p.L_eff[2] : 1.0);
+  const double vol = area * p.L_eff[0];
+  out[0] = -p.H_lu * s[0] / area;
+  out[1] = -p.H_lu * s[1] / area;
+  out[2] = std::sqrt(h->Ra / h->Pr) * (s[2] / vol) / p.U;
+  out[3] = (s[3] / vol) / (p.U * p.U);
+  out[4] = std::sqrt(h->Ra * h->Pr) * (s[4] / vol) / p.U + 1.0;
+  for (int i = 0; i < 5; ++i)
+    if (!std::isfinite(out[i])) return fail(ISLBM_ERR_NONFINITE, "non-finite diagnostic: the run has diverged");
+  return ISLBM_OK;
+}
+
 template <int DIM, typename ST>
 static void launch_residual(islbm *h, int nb) {
   const ST *S = (const ST *)(h->ws + h->cv.buf[h->cur]);

@@ -22,7 +22,7 @@ KERNEL_AUTO, KERNEL_GENERIC, KERNEL_TILED, KERNEL_UNIFORM_SHIFT = 0, 1, 2, 3
 EXPORTS = (
     "islbm_workspace_bytes", "islbm_create", "islbm_create_slab", "islbm_halo", "islbm_halo_layout", "islbm_slab_set_peer", "islbm_diag_sums", "islbm_diag_from_sums",
     "islbm_residual_sums", "islbm_destroy", "islbm_get_params", "islbm_init",
-    "islbm_set_populations", "islbm_set_populations_host", "islbm_get_populations", "islbm_step", "islbm_fields", "islbm_nusselt", "islbm_nusselt_middle",
+    "islbm_set_populations", "islbm_set_populations_host", "islbm_get_populations", "islbm_step", "islbm_fields", "islbm_nusselt", "islbm_nusselt_static", "islbm_nusselt_middle",
     "islbm_steady_residual", "islbm_set_buoyancy_scale", "islbm_set_reference_temperature", "islbm_set_stencil", "islbm_set_kernel", "islbm_set_tuning", "islbm_launch_count",
     "islbm_kernel_name", "islbm_last_error", "islbm_version",
 )
@@ -84,6 +84,7 @@ def _load():
     lib.islbm_step.argtypes = [vp, C.c_int]
     lib.islbm_fields.argtypes = [vp, vp, vp, vp, vp, vp]
     lib.islbm_nusselt.argtypes = [vp, dp]
+    lib.islbm_nusselt_static.argtypes = [vp, dp]
     lib.islbm_nusselt_middle.argtypes = [vp, dp]
     lib.islbm_steady_residual.argtypes = [vp, dp]
     lib.islbm_set_buoyancy_scale.argtypes = [vp, C.c_double]
@@ -259,6 +260,12 @@ class Islbm:
     def nusselt(self):
         out = (C.c_double * 5)()
         _check(lib.islbm_nusselt(self.h, out))
+        return dict(zip(("Nu_hot", "Nu_cold", "Re", "u2", "Nu_vol"), list(out)))
+
+    def nusselt_static(self):
+        """islbm_nusselt with its scratch in a static device array of the library: allocates nothing (at most 33 554 432 nodes)."""
+        out = (C.c_double * 5)()
+        _check(lib.islbm_nusselt_static(self.h, out))
         return dict(zip(("Nu_hot", "Nu_cold", "Re", "u2", "Nu_vol"), list(out)))
 
     def halo(self, side):
