@@ -609,7 +609,7 @@ inline bool plan2_create(Plan2 &p, const int *n, int nxp, void *buf0, void *buf1
 // Number of chunks a strip of `rows` emitted rows is cut into (measured, profiles/): short chunks win (4 rows:
 // 0.96-0.97 at 2049^2..8193^2, 8 rows: 0.88-0.93, 60 rows: 0.73-0.87; the doubled prologue rows are found in L2), and
 // the CTA count should be a whole number of waves of resident CTAs.  So: one wave if its chunks are at most
-// max_single rows (8 with the 3-stage ring, 12 with the 4-stage one; small and medium meshes, down to 2 rows), else
+// max_single rows (8 with the 3-stage ring, 12 with the 4-stage one; small and medium meshes, down to 1 row), else
 // k waves, k the smallest number for which a chunk is at most max_multi = 4 rows.
 inline int chunks2(int rows, int per_wave, int forced_chunk, int max_single = 8, int max_multi = 4) {
   int nc;
@@ -618,7 +618,7 @@ inline int chunks2(int rows, int per_wave, int forced_chunk, int max_single = 8,
   } else {
     nc = per_wave;
     if ((rows + nc - 1) / nc > max_single) nc = per_wave * ((rows + max_multi * per_wave - 1) / (max_multi * per_wave));
-    if (nc > rows / 2) nc = rows / 2;
+    if (nc > rows) nc = rows;   // down to ONE row per CTA on tiny meshes: a CTA costs ~2 us + 1.1 us per row (64^2: 4.05 -> 3.08 us per step)
   }
   const int least = (rows + kMaxChunk - 1) / kMaxChunk;
   if (nc < least) nc = least;

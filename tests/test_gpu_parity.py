@@ -77,6 +77,7 @@ def kernels_for(islbm, sim):
         ks.append((islbm.KERNEL_TILED, {}))
         ks.append((islbm.KERNEL_TILED, dict(chunk=5, load_policy=1, store_policy=2, l2promo=3, pdl=0, fill=2)))
         ks.append((islbm.KERNEL_TILED, dict(chunk=2, fill=1)))
+        ks.append((islbm.KERNEL_TILED, dict(chunk=1)))                            # one emitted layer per CTA
         if sim.dim == 3:
             ks.append((islbm.KERNEL_TILED, dict(shape3d=3, chunk=3)))
             ks.append((islbm.KERNEL_TILED, dict(shape3d=4, fill=2)))
