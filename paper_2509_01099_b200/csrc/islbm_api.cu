@@ -614,6 +614,7 @@ extern "C" int islbm_set_tuning(islbm_t *h, const char *key, int value) {
   else if (k == "rows2d") { if (value > kMaxChunk) return fail(ISLBM_ERR_ARG, "rows2d must be at most 64"); t.rows2d = value; }
   else if (k == "rows2d1") { if (value > kMaxChunk) return fail(ISLBM_ERR_ARG, "rows2d1 must be at most 64"); t.rows2d1 = value; }
   else if (k == "graph") { if (value > 2) return fail(ISLBM_ERR_ARG, "graph must be 0 (automatic), 1 (always) or 2 (never)"); t.graph = value; }
+  else if (k == "slab_wait_ms") t.slab_wait_ms = value;
   else if (k == "walls") { if (value > 1) return fail(ISLBM_ERR_ARG, "walls must be 0 (fused) or 1 (separate boundary kernel)"); t.walls = value; }
   else return fail(ISLBM_ERR_ARG, "unknown tuning key: " + k);
   make_tiled_plan(h);
@@ -634,6 +635,7 @@ static int enqueue_one_step(islbm *h, int which, bool fused) {
     h->dm.flag_out[sd] = on ? (unsigned long long *)(h->peer_base[sd] + h->peer_flag_off[sd]) : nullptr;
   }
   h->dm.step = (unsigned long long)h->steps + 1ull;
+  h->dm.wait_ns = (unsigned long long)h->tune.slab_wait_ms * 1000000ull;
   if (fused && which != 2) {
     k_slab_wait<<<1, 1, 0, h->stream>>>(h->dm);
     h->launches++;
@@ -856,6 +858,7 @@ extern "C" int islbm_slab_set_peer(islbm_t *h, int side, void *peer_workspace, c
   const unsigned long long init = (unsigned long long)h->steps;
   CUDA_TRY(cudaMemcpyAsync(h->ws + h->cv.flags + 8 * (size_t)side, &init, 8, cudaMemcpyHostToDevice, h->stream));
   CUDA_TRY(cudaMemsetAsync(h->ws + h->cv.flags + 64 + 8 * (size_t)side, 0, 8, h->stream));   // done counter
+  CUDA_TRY(cudaMemsetAsync(h->ws + h->cv.flags + 64 + 16, 0, 8, h->stream));                  // time-out counter
   CUDA_TRY(cudaStreamSynchronize(h->stream));
   h->peer_base[side] = (char *)peer_workspace;
   h->peer_ghost_off[side][0] = pl->ghost_offset[0];
@@ -866,11 +869,29 @@ extern "C" int islbm_slab_set_peer(islbm_t *h, int side, void *peer_workspace, c
   return ISLBM_OK;
 }
 
+// fused slab exchange: did a step kernel give up waiting for a neighbour's flag?  (stream already synchronised)
+static int check_slab_timeouts(islbm *h) {
+  if (!h->peer_base[0] && !h->peer_base[1]) return ISLBM_OK;
+  unsigned long long n = 0;
+  CUDA_TRY(cudaMemcpyAsync(&n, h->ws + h->cv.flags + 64 + 16, 8, cudaMemcpyDeviceToHost, h->stream));
+  CUDA_TRY(cudaStreamSynchronize(h->stream));
+  if (n) {
+    char b[256];
+    snprintf(b, sizeof b, "fused slab exchange: %llu boundary CTA(s) gave up waiting for a neighbour's step flag after %d ms "
+                          "(neighbour not stepping, or connected at a different step count): this rank's state is invalid", n,
+             h->tune.slab_wait_ms);
+    return fail(ISLBM_ERR_STATE, b);
+  }
+  return ISLBM_OK;
+}
+
 extern "C" int islbm_diag_sums(islbm_t *h, double s[8]) {
   if (!h || !s) return fail(ISLBM_ERR_ARG, "NULL argument");
   if (!h->has_state) return fail(ISLBM_ERR_STATE, "no state");
   double t[kRedSlots];
   int rc = run_diag_reduction(h, t);
+  if (rc) return rc;
+  rc = check_slab_timeouts(h);
   if (rc) return rc;
   for (int i = 0; i < 8; ++i) s[i] = i < kRedSlots ? t[i] : 0.0;
   return ISLBM_OK;
@@ -1034,6 +1055,7 @@ extern "C" int islbm_residual_sums(islbm_t *h, double s[4], int *first) {
   bool f = false;
   int rc = run_residual(h, s, &f);
   *first = f ? 1 : 0;
+  if (rc == ISLBM_OK) rc = check_slab_timeouts(h);
   return rc;
 }
 

@@ -56,6 +56,9 @@ struct DevMesh {
   unsigned long long *done_cnt;
   unsigned long long step;
   int bctas;
+  // the wait for a neighbour's flag is bounded: after wait_ns nanoseconds (0 = wait for ever) the CTA counts a
+  // time-out in done_cnt[2] and goes on; the host reports it at the next synchronising slab call instead of hanging
+  unsigned long long wait_ns;
   int stencil;           // 0: {j-1,j,j+1} (A2); 1: upwind {j-2,j-1,j} for c=+1, {j,j+1,j+2} for c=-1
                          // (generic kernel only; the TMA kernels stage a 1-node halo and take stencil 0)
 };
@@ -271,7 +274,20 @@ __device__ __forceinline__ void st_release_sys(unsigned long long *p, unsigned l
 // layer, and it no longer reads the ghost layer we are about to overwrite)
 __device__ __forceinline__ void slab_wait_neighbour(const DevMesh &m, int side) {
   if (m.flag_in[side] == nullptr) return;
-  while (ld_acquire_sys(m.flag_in[side]) + 1ull < m.step) __nanosleep(64);
+  if (ld_acquire_sys(m.flag_in[side]) + 1ull >= m.step) return;          // the usual case: already there
+  unsigned long long t0;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t0));
+  while (ld_acquire_sys(m.flag_in[side]) + 1ull < m.step) {
+    __nanosleep(64);
+    if (m.wait_ns != 0ull) {
+      unsigned long long t1;
+      asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t1));
+      if (t1 - t0 > m.wait_ns) {
+        atomicAdd(m.done_cnt + 2, 1ull);      // gave up: the results of this rank are invalid from here on
+        return;
+      }
+    }
+  }
 }
 // one thread of a CTA whose threads have all finished (after a CTA barrier): count it; the last boundary CTA of this
 // launch publishes the step number to the neighbour

@@ -128,6 +128,29 @@ def test_fused_exchange_is_one_launch_per_step_and_flags_count_steps(islbm):
             assert torch.equal(s.owned(fl[k]), fw[k][lo:hi]), (k, s.rank)
 
 
+def test_fused_exchange_wait_is_bounded(islbm):
+    """A neighbour that never steps must not hang the GPU: the boundary CTAs of the waiting slab give up after
+    `slab_wait_ms` (200 ms here; default 10 s), count the time-out, and the next synchronising slab call reports it."""
+    import time
+    coords, delta, Ra = mesh(3, (40, 24, 21), (1.4, 1.2, 1.3))
+    slabs = [slab.SlabCavity(coords, delta, Ra, 0.71, 0.1 * SQ3, r, 2, exchange=lambda: None) for r in range(2)]
+    for s in slabs:
+        s.init(5, 1e-3)
+    slabs[0].sim.set_tuning(slab_wait_ms=200)
+    slab.connect_local(slabs)
+    slabs[0].sim.step(1)                       # step 1 needs the neighbour's step 0: there from the start
+    slabs[0].sim.diag_sums()                   # fine so far
+    t0 = time.time()
+    slabs[0].sim.step(1)                       # step 2 needs the neighbour's step 1, which never comes
+    with pytest.raises(islbm.IslbmError) as e:
+        slabs[0].sim.diag_sums()
+    dt = time.time() - t0
+    assert e.value.code == -6 and "gave up waiting" in str(e.value)
+    assert 0.15 < dt < 5.0, dt
+    for s in slabs:
+        s.close()
+
+
 def test_slabs_against_the_oracle(islbm):
     coords, delta, Ra = mesh(3, (24, 16, 21), (1.3, 1.2, 1.4))
     orc = Oracle(coords, delta, Ra, 0.71, 0.1 * SQ3, threads=max(1, min(16, len(os.sched_getaffinity(0)))))
