@@ -43,6 +43,18 @@ namespace islbmk {
 #ifndef ISLBM_S_IN_SMEM
 #define ISLBM_S_IN_SMEM 1
 #endif
+// The fp64 32x8 kernel runs a dedicated TMA producer warpgroup: 4 extra warps, of which one lane waits for each ring
+// slot to be released and issues the next stage into it; `setmaxnreg` hands the group's registers to the 8 consumer
+// warps (launch at 168 per thread, then 40 / 232), so no consumer warp stalls on the empty barriers or spends issue
+// slots on the 7 TMA instructions per slice.  Measured +1-2 % on the sustained 256^3 step (profiles/attempts.md);
+// 0 = thread 0 of consumer warp 0 is the producer (round 1).  fp32 storage keeps its last-releasing-warp refill
+// (6 consumer warps per CTA are not a whole number of warpgroups).
+#ifndef ISLBM_PRODUCER_WG
+#define ISLBM_PRODUCER_WG 1
+#endif
+template <typename ST, int TX, int TY> __host__ __device__ constexpr int producer_threads() {
+  return (ISLBM_PRODUCER_WG && sizeof(ST) == 8 && TX * TY == 256) ? 128 : 0;
+}
 
 constexpr int kMaxChunk = 64;   // longest marching chunk (its weights are staged in shared memory)
 
@@ -354,10 +366,12 @@ __device__ __forceinline__ void load_march_weights(const float *ws, int i, Pr<fl
   } while (0)
 
 template <typename ST, int TX, int TY>
-__global__ void __launch_bounds__(TX * TY, TX * TY <= 128 ? 3 : (TX * TY <= 192 ? 2 : 1))
+__global__ void __launch_bounds__(TX * TY + producer_threads<ST, TX, TY>(), TX * TY <= 128 ? 3 : (TX * TY <= 192 ? 2 : 1))
 k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const ST *__restrict__ src,
               ST *__restrict__ dst, int zchunk, int load_policy, int store_policy, int flags) {
   using T = Tile3<ST, TX, TY>;
+  constexpr bool PW = producer_threads<ST, TX, TY>() != 0;
+  constexpr int ALL_THREADS = T::THREADS + producer_threads<ST, TX, TY>();
   // flags: bit 0 = first ring fill after the CTA barrier; bit 1 = leave the wall rules to k_step_shell3 (the
   // separate-boundary-kernel variant of BASELINE.json north_star, islbm_set_tuning("walls", 1); measured slower)
   const bool late_fill = flags & 1, skip_walls = flags & 2;
@@ -401,7 +415,7 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
     tma_prefetch_desc(&mp.x);
     tma_prefetch_desc(&mp.y);
     tma_prefetch_desc(&mp.xy);
-    if (!late_fill) {
+    if (!late_fill && !PW) {
       pdl_wait();
       if (b_lo) slab_wait_neighbour(m, 0);
       if (b_hi) slab_wait_neighbour(m, 1);
@@ -409,13 +423,28 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
         issue_stage3<T>(s, z0, m.nz, x0, y0, stage0, full, empty, mp, lpol);
     }
   }
-  for (int i = (int)threadIdx.x - 32; i >= 0 && i < 6 * (z1 - z0); i += T::THREADS - 32) {   // warps 1..: warp 0 is waiting above
+  for (int i = (int)threadIdx.x - 32; i >= 0 && i < 6 * (z1 - z0); i += ALL_THREADS - 32) {   // warps 1..: warp 0 is waiting above
     const int sk = i / (z1 - z0), zi = i - sk * (z1 - z0);
     stage_march_weight<0>(wzs, sk, zi, __ldg(wrow(m, 2, sk / 3, sk % 3) + z0 + zi));
   }
   pdl_wait();
   __syncthreads();
-  if (late_fill && threadIdx.x == 0) {
+  if constexpr (PW) {
+    if (threadIdx.x >= T::THREADS) {          // the producer warpgroup: one lane streams every stage, the rest retire
+      asm volatile("setmaxnreg.dec.sync.aligned.u32 40;");
+      if (threadIdx.x == T::THREADS) {
+        if (b_lo) slab_wait_neighbour(m, 0);
+        if (b_hi) slab_wait_neighbour(m, 1);
+        for (int s = 0; s < nstage; ++s) {
+          if (s >= T::STAGES) mbar_wait(&empty[s % T::STAGES], ((uint32_t)(s / T::STAGES) & 1u) ^ 1u);
+          issue_stage3<T>(s, z0, m.nz, x0, y0, stage0, full, empty, mp, lpol);
+        }
+      }
+      return;
+    }
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 232;");
+  }
+  if (!PW && late_fill && threadIdx.x == 0) {
     if (b_lo) slab_wait_neighbour(m, 0);
     if (b_hi) slab_wait_neighbour(m, 1);
     for (int s = 0; s < T::STAGES - (EARLY ? 0 : 1) && s < nstage; ++s)
@@ -478,7 +507,7 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
 #define PC4(k) (sbc + T::moff(T::OFF_C4, k, T::P_C, T::H_C) / ES)
 #define PXM(k) (sbx + T::moff(T::OFF_XM, k, T::P_X, T::H_X) / ES)
 #define PYM(k) (sby + T::moff(T::OFF_YM, k, T::P_Y, T::H_Y) / ES)
-    if (!EARLY && threadIdx.x == 0 && s + T::STAGES - 1 < nstage) {
+    if (!EARLY && !PW && threadIdx.x == 0 && s + T::STAGES - 1 < nstage) {
       const int sn = s + T::STAGES - 1;
       if (sn >= T::STAGES) mbar_wait(&empty[sn % T::STAGES], ((uint32_t)(sn / T::STAGES) & 1u) ^ 1u);
       issue_stage3<T>(sn, z0, m.nz, x0, y0, stage0, full, empty, mp, lpol);
@@ -569,7 +598,8 @@ k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const 
 #undef PYM
   }
   if ((b_lo && m.flag_out[0] != nullptr) || (b_hi && m.flag_out[1] != nullptr)) {   // CTA-uniform
-    __syncthreads();
+    if constexpr (PW) asm volatile("bar.sync 1, %0;" ::"n"(T::THREADS) : "memory");   // the consumer warps only
+    else __syncthreads();
     if (threadIdx.x == 0) {
       if (b_lo) slab_publish(m, 0);
       if (b_hi) slab_publish(m, 1);
@@ -913,7 +943,7 @@ inline void launch3_shape(const Plan3 &p, const int *n, const DevMesh &m, const 
   if constexpr (SK == 0)
   {
     const bool shell = tn.walls == 1 && m.em_lo == 0 && m.em_hi == m.nz && m.peer[0] == nullptr && m.peer[1] == nullptr;
-    launch_step(k_step_zmarch<ST, TX, TY>, grid, dim3(T::THREADS), T::SMEM_BYTES, stream, tn.pdl != 0 && !shell, p.maps[cur], mm,
+    launch_step(k_step_zmarch<ST, TX, TY>, grid, dim3(T::THREADS + producer_threads<ST, TX, TY>()), T::SMEM_BYTES, stream, tn.pdl != 0 && !shell, p.maps[cur], mm,
                 np, (const ST *)buf[cur], (ST *)buf[1 - cur], p.zchunk, tn.load_policy, tn.store_policy,
                 (tn.fill == 2 ? 1 : 0) | (shell ? 2 : 0));
     if (shell) {

@@ -56,6 +56,8 @@ def test_library_holds_tma_and_mbarrier_instructions(binding):
     import subprocess
     sass = subprocess.run(["cuobjdump", "-sass", binding.LIB_PATH], capture_output=True, text=True).stdout
     assert "UTMALDG" in sass and "SYNCS" in sass
+    assert "USETMAXREG" in sass      # the fp64 3-D kernel's producer warpgroup donates its registers (setmaxnreg)
+    assert "FFMA2" in sass           # packed fp32 interpolation of the fp32-storage kernels (fma.rn.f32x2)
     for kern in ("k_step_zmarch", "k_step_ymarch", "k_step_shift", "k_step_generic", "k_nusselt_partial"):
         assert kern in sass, kern
 

@@ -71,3 +71,22 @@ def test_clock_sampler_parses_nvidia_smi_lines(monkeypatch):
     out = s.stop()
     assert out["sm_mhz"] == 1800 and out["sm_max_mhz"] == 1965
     assert out["reasons"] == ["hw_thermal_slowdown", "sw_power_cap"]
+
+
+def test_full_mode_times_the_step_counts_baseline_json_states():
+    """bench.py --full: configs 2-5 (and their uniform counterparts) at the step counts BASELINE.json states."""
+    import re
+    sys.path.insert(0, ROOT)
+    import bench
+    from paper_2509_01099_b200 import inputs
+    cfgs = json.load(open(os.path.join(ROOT, "BASELINE.json")))["configs"]
+    stated = [int(re.search(r"(\d+) steps timed", c).group(1)) for c in cfgs[1:]]
+    assert stated == [20000, 50000, 5000, 10000]
+    names = [n for n, _ in bench.FULL_RUNS]
+    for key, steps in zip(("c2_512sq", "c3_1024sq", "c4_128cu", "c5_256cu"), stated):
+        assert key in names
+        assert inputs.workload(key).steps == steps and steps % 100 == 0        # sampled every 100 steps (A20)
+    for key in ("c2_512sq", "c3_1024sq", "c5_256cu"):                          # the configs that ask for a uniform counterpart
+        assert key + "_uniform" in names
+        assert inputs.workload(key + "_uniform").steps == inputs.workload(key).steps
+    assert ("c3_1024sq", 1) in bench.FULL_RUNS and ("c5_256cu", 1) in bench.FULL_RUNS   # "fp64 and fp32 storage"

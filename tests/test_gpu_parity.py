@@ -961,3 +961,8 @@ def test_command_line_driver(islbm, capsys):
     assert lines[0]["T0"] == -0.5 and lines[0]["kernel"].startswith("tiled_ymarch_tma") and lines[0]["nodes"] == 63 * 63
     assert [l["step"] for l in lines[1:]] == [200, 400]
     assert all(np.isfinite(l["Nu_hot"]) and l["Re_rms"] >= l["Re"] for l in lines[1:])
+    # --time: one JSON line with the timing of a tuning variant (the A/B rows of profiles/attempts.md)
+    run.main(["--workload", "c1_64sq", "--time", "64", "--tune", "chunk=2", "--tune", "graph=2", "--stencil", "1"])
+    t = _json.loads(capsys.readouterr().out.strip().splitlines()[-1])
+    assert t["kernel"] == "tiled_ymarch_tma_upwind" and t["tune"] == ["chunk=2", "graph=2"] and 0.5 < t["us_per_step"] < 100
+    assert t["MLUPS"] == pytest.approx(64 * 64 / t["us_per_step"])
