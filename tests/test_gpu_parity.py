@@ -922,6 +922,22 @@ def test_paper_mode_table4_ra1e5_129(islbm, golden):
     assert nu["Nu_hot"] == pytest.approx(ref[1], rel=6e-3)
     assert nu["Nu_cold"] == pytest.approx(nu["Nu_hot"], rel=1e-6)
     assert math.sqrt(1e5 / 0.71 * nu["u2"]) == pytest.approx(ref[3], rel=3e-3)
+    # reading A10: Eq. 42 prints sqrt(u*^2 + v*^2) in 3-D; the library takes the full speed.  Both forms from the fields
+    # with the Eq. 29 weights (ghost coordinates one delta outside, normalised by the effective lengths): the full
+    # speed reproduces the library's <u*^2> and Table 4's <Re>; the two-component form as printed does not.
+    flA = sim.fields(("u", "v", "w"))
+    xx = np.asarray(w.coords[0])
+    xe = np.concatenate(([xx[0] - w.delta], xx, [xx[-1] + w.delta]))
+    w1 = torch.from_numpy(0.5 * (xe[2:] - xe[:-2])).cuda()
+    W = w1[:, None, None] * w1[None, :, None] * w1[None, None, :]
+    vol = (xx[-1] - xx[0] + w.delta) ** 3
+    Ulu = sim.params()["U"]
+    u2_full = ((flA["u"] ** 2 + flA["v"] ** 2 + flA["w"] ** 2) * W).sum().item() / vol / Ulu ** 2
+    u2_uv = ((flA["u"] ** 2 + flA["v"] ** 2) * W).sum().item() / vol / Ulu ** 2
+    assert u2_full == pytest.approx(nu["u2"], rel=1e-10)
+    re_uv = math.sqrt(1e5 / 0.71 * u2_uv)
+    print("A10", math.sqrt(1e5 / 0.71 * u2_full), re_uv, ref[3])
+    assert abs(re_uv / ref[3] - 1.0) > 2 * abs(math.sqrt(1e5 / 0.71 * u2_full) / ref[3] - 1.0)
     # cell-centre values, Table 5: node 63 of the 127 sits at 0.5 exactly.  The vorticity there
     # (3-point Lagrange derivative on the stretched mesh, free-fall units) is physics: within 0.5 %.  T_c - 0.5, u_c
     # and v_c are the O(Ma^2) signature of T0 = T_cold in a weakly compressible model; ours come out at 0.78-0.86 of
