@@ -467,7 +467,8 @@ def main():
                 "frac_of_nominal_8000GBs": achieved / 8000.0,      # secondary, against the nominal HBM3e figure
                 "dram_bytes_per_update": (read_traffic(args.workload, r["kernel"], prec) or 0) / w.nodes or None}
 
-    # fp32 storage is bound by instruction issue, not by HBM (profiles/r1_c5_256cu_f32_v5.md): report that roofline too.
+    # fp32 storage is not bound by HBM (latency of the fp64 collision at 12 warps per SM, profiles/r2_c5_256cu_f32.md):
+    # report the issue-slot roofline too, as the second bound it does not reach either.
     # peak = SMs x 4 warp schedulers x 1 warp instruction per clock x the maximum SM clock
     inst = read_inst(args.workload, r["kernel"], prec)
     if inst:

@@ -62,7 +62,8 @@ typedef struct {
 enum { ISLBM_D2Q9_D2Q5 = 0, ISLBM_D3Q19_D3Q7 = 1 };
 /* ISLBM_F32_STORAGE: the workspace holds f_q - w_q and g_q as fp32; the TMA kernels interpolate those stored
  * deviations in fp32 (one or two more fp32 roundings of the deviation per step, the size of the storage rounding
- * itself) and collide in fp64; everything else (API arrays, diagnostics, weights) is fp64.  Tolerance against the
+ * itself), collide the flow populations in fp64 and the temperature populations in fp32; everything else (API arrays,
+ * diagnostics, weights) is fp64.  Tolerance against the
  * fp64 oracle: 1e-5 on u and T after 1000 steps (BASELINE.json). */
 enum { ISLBM_F64 = 0, ISLBM_F32_STORAGE = 1 };
 
@@ -251,7 +252,8 @@ int islbm_set_buoyancy_scale(islbm_t *h, double s); /* multiplies g*beta; 0 for 
  * Must be called before islbm_init / islbm_set_populations. */
 int islbm_set_reference_temperature(islbm_t *h, double T0);
 /* Interpolation stencil: 0 = destination-centred {j-1,j,j+1} (default, reading A2), 1 = upwind
- * {j-2,j-1,j} for c = +1 and {j,j+1,j+2} for c = -1 (the A2 alternative; study mode, generic kernel only).
+ * {j-2,j-1,j} for c = +1 and {j,j+1,j+2} for c = -1 (the A2 alternative; TMA kernels of its own and the generic kernel;
+ * not on slab handles, whose single ghost layer is one short of its reach).
  * Before islbm_init / islbm_set_populations. */
 int islbm_set_stencil(islbm_t *h, int kind);
 /* 0 = auto (fastest kernel for this mesh), 1 = generic global-memory kernel,

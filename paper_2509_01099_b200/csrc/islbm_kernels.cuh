@@ -60,7 +60,7 @@ struct DevMesh {
   // time-out in done_cnt[2] and goes on; the host reports it at the next synchronising slab call instead of hanging
   unsigned long long wait_ns;
   int stencil;           // 0: {j-1,j,j+1} (A2); 1: upwind {j-2,j-1,j} for c=+1, {j,j+1,j+2} for c=-1
-                         // (generic kernel only; the TMA kernels stage a 1-node halo and take stencil 0)
+                         // (generic kernel; the TMA kernels exist per stencil: k_step_*march / k_step_*march_up)
 };
 
 // workspace (padded-row) index of dense node index c

@@ -129,7 +129,7 @@ template <> struct Acc<float> { using type = float; };
 // components, e.g. (f1, f2) = (+x, -x).  The separable interpolation works on such pairs: the two
 // lanes take the same taps of two different planes with the weights of the two signs.  In fp32 a pair is one float2
 // and a tap is ONE packed instruction (fma.rn.f32x2 / mul.rn.f32x2, sm_100), which halves the fp32 instruction
-// stream of the issue-bound fp32-storage kernels; in fp64 a pair is two doubles and two scalar instructions.  Either
+// stream of the fp32-storage kernels; in fp64 a pair is two doubles and two scalar instructions.  Either
 // way each lane performs exactly the operations of the scalar form ((w0*v0) + w1*v1) + w2*v2, the oracle's order.
 template <typename AT> struct Pr;
 template <> struct Pr<double> { double a, b; };
