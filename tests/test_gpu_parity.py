@@ -875,6 +875,32 @@ def test_paper_mode_table2_ra1e6_257(islbm, golden):
     assert fl["v"][0, 127, 127].item() > 0.0
 
 
+def test_paper_mode_table2_ra1e7_513(islbm, golden):
+    """A second Rayleigh number end to end: paper mode (erf a = 1.5, Ma = 0.1, T0 = T_cold), Ra = 1e7 on the 513-point
+    mesh, run to the Eq. 30 criterion (5.4e6 steps, about a minute), against Table 2 and Table 3
+    (PAPER.md:371): Nu_hot 0.2 %, <Nu> and Nu_middle 0.3 % (the estimator offset of reading A9), rms <Re> (A22) 0.2 %."""
+    ref = golden["table2"]["Ra1e7"]["513"]
+    w = inputs.custom_workload("paper7", 2, 513, mesh="erf", stretch=1.5, Ra=1e7, Ma=0.1)
+    sim = islbm.Islbm(w.coords, w.delta, w.Ra, w.Pr, w.Ma)
+    sim.set_reference_temperature(-0.5)
+    sim.init(0, 0.0)
+    sim.steady_residual()
+    for _ in range(4000):
+        sim.step(2000)
+        ru, rT = sim.steady_residual()
+        if ru < 1e-9 and rT < 1e-9:
+            break
+    assert ru < 1e-9 and rT < 1e-9
+    nu = sim.nusselt()
+    nm = sim.nusselt_middle()
+    print("TABLE2 Ra1e7 513", nu, nm, math.sqrt(1e7 / 0.71 * nu["u2"]), ref)
+    assert nu["Nu_hot"] == pytest.approx(ref[1], rel=2e-3)
+    assert nu["Nu_vol"] == pytest.approx(ref[0], rel=3e-3)
+    assert nm == pytest.approx(ref[2], rel=3e-3)
+    assert nu["Nu_cold"] == pytest.approx(nu["Nu_hot"], rel=5e-6)
+    assert math.sqrt(1e7 / 0.71 * nu["u2"]) == pytest.approx(ref[3], rel=2e-3)
+
+
 def test_reference_temperature_parity_and_symmetry(islbm):
     """T0 = T_cold (paper) against the oracle; T0 = mean keeps the centro-symmetry T(1-x,1-y) = -T(x,y)."""
     w = inputs.custom_workload("t0", 2, 41, stretch=1.4, Ra=1e5)
