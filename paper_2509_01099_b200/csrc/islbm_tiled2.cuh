@@ -142,6 +142,7 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
   const int yf = DIR > 0 ? y0 : y1 - 1;
   const int nstage = 2 + (y1 - y0);
   const bool b_lo = y0 == m.em_lo, b_hi = y1 == m.em_hi;   // slab boundary CTAs (fused exchange; islbm_tiled3.cuh)
+  const bool any_peer = m.peer[0] != nullptr || m.peer[1] != nullptr;
   const uint64_t lpol = make_policy(load_policy);
   const uint64_t spol = make_policy(store_policy);
   // thread 0 sets up the ring and (unless late_fill) fills it BEFORE warps 1.. load the weight rows, so the two
@@ -280,7 +281,7 @@ k_step_ymarch(const __grid_constant__ Maps2 mp, DevMesh m, NodeParams np, const 
       collide_node<DEV>(f, g, np);
       if (valid) {
         store_node<2, DEV>(dst + c, m.nnp, f, g, spol, std::make_integer_sequence<int, 14>{});
-        peer_store_node<2, ST, DEV>(m, y, x, f, g);
+        if (any_peer) peer_store_node<2, ST, DEV>(m, y, x, f, g);   // slab boundary rows only
       }
       c += DIR * (long long)m.nxp;
     }
