@@ -744,6 +744,19 @@ def test_no_kernel_writes_outside_the_workspace(islbm, dim, ns, prec):
     sim.nusselt(), sim.nusselt_middle(), sim.steady_residual(), sim.steady_residual(), sim.fields()
     torch.cuda.synchronize()
     assert sim.guards_intact()
+    # the upwind-stencil kernels (2-row halo boxes, half-group boxes, per-lane window offsets) on the same mesh
+    up = islbm.Islbm(coords, delta, 0.71 * (0.1 * H_lu / 0.03) ** 2, 0.71, 0.1 * SQ3, precision=prec, guard_bytes=1 << 20)
+    up.set_stencil(1)
+    up.init(0, 1e-3)
+    for k, tune in kernels_for(islbm, up):
+        select(up, k, tune)
+        up.step(3)
+        f, g = up.get_populations()
+        up.set_populations(f, g)
+        up.step(2)
+    up.nusselt(), up.nusselt_static(), up.fields()
+    torch.cuda.synchronize()
+    assert up.guards_intact()
 
 
 @pytest.mark.parametrize("dim,ns,prec", [(2, (64, 64), 0), (2, (70, 45), 1), (3, (37, 21, 19), 0)])
