@@ -273,7 +273,7 @@ int islbm_set_kernel(islbm_t *h, int which);
  * ring: 3 stages with four CTAs per SM or 4 stages with three, 0 automatic), "rows2d" / "rows2d1"
  * (2-D chunk rule: longest chunk of a multi-wave launch / longest chunk for which a single wave
  * of CTAs is taken, 0 automatic), "graph" (islbm_step(n) with n >= 32 replays a captured CUDA graph of 32 PDL-chained
- * step kernels: 0 automatic = meshes of at most 2^18 nodes, whose steps are bound by the host's launch rate, 1 always,
+ * step kernels: 0 automatic = meshes of at most 2^20 nodes, whose steps are short enough for the host's launch rate to show, 1 always,
  * 2 never), "slab_wait_ms" (fused slab exchange: the longest a boundary CTA waits for its neighbour's step flag, default
  * 10 000 ms, 0 = for ever; a CTA that gives up is counted, and islbm_diag_sums / islbm_residual_sums then return
  * ISLBM_ERR_STATE instead of the GPU hanging on a neighbour that never steps), "walls" (3-D whole cavity: 0 wall rules inside the step kernel, 1 a separate

@@ -678,10 +678,11 @@ static void drop_graph(islbm *h) {
 // Small meshes (a step kernel of a few microseconds): kGraphSteps consecutive step kernels, PDL-chained, are captured
 // once into a CUDA graph and replayed, so that islbm_step(n) costs n / kGraphSteps host launches instead of n (the
 // 64^2 mesh of BASELINE.json config 1 is bound by the host's launch rate otherwise).  The graph holds an even number
-// of steps, so it always starts on the same ping-pong buffer parity it was captured on.
+// of steps, so it always starts on the same ping-pong buffer parity it was captured on.  Automatic up to 2^20 nodes:
+// measured gain 13-23 % at 64^2, 6-8 % at 512^2, 1-3 % at 1024^2, none from 128^3 on (profiles/attempts.md).
 constexpr int kGraphSteps = 32;
 static bool graph_eligible(const islbm *h, int which, bool fused) {
-  return which == 2 && !fused && h->tune.graph != 2 && (h->tune.graph == 1 || h->nn <= (1LL << 18));
+  return which == 2 && !fused && h->tune.graph != 2 && (h->tune.graph == 1 || h->nn <= (1LL << 20));
 }
 
 extern "C" int islbm_step(islbm_t *h, int n) {

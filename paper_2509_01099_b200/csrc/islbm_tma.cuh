@@ -205,7 +205,7 @@ struct Tuning {
   int ring2d = 0;       // 2-D fp64 ring: 3 stages x 4 CTAs per SM, or 4 stages x 3 CTAs; 0 = automatic
   int rows2d = 0;       // 2-D chunk rule: longest chunk of a multi-wave launch (0 = automatic)
   int rows2d1 = 0;      // 2-D chunk rule: longest chunk for which a single wave is taken (0 = automatic)
-  int graph = 0;        // islbm_step(n >= 32): replay a captured CUDA graph of 32 step kernels; 0 = meshes up to 2^18 nodes, 1 always, 2 never
+  int graph = 0;        // islbm_step(n >= 32): replay a captured CUDA graph of 32 step kernels; 0 = meshes up to 2^20 nodes, 1 always, 2 never
   int slab_wait_ms = 10000;  // fused slab exchange: longest wait for a neighbour's step flag in milliseconds (0 = for ever)
   int walls = 0;        // 3-D: 0 wall rules inside the step kernel; 1 a separate boundary kernel over the shell (A/B variant)
 };
