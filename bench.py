@@ -39,6 +39,16 @@ BYTES_PER_UPDATE = {(2, 0): 224, (2, 1): 112, (3, 0): 416, (3, 1): 208}   # SURV
 METRIC = "MLUPS"
 
 
+def dtype_name(prec, dim):
+    """The arithmetic the path computes in.  fp32 storage: the stencil interpolation and the temperature collision run in
+    fp32; the flow collision in fp32 in 3-D and in fp64 in 2-D."""
+    if prec == 0:
+        return "f64"
+    if dim == 3:
+        return "f32 (storage, stencil interpolation and collision)"
+    return "f64 flow collision, f32 storage, stencil interpolation and temperature collision"
+
+
 def read_peaks():
     path = os.path.join(ROOT, "MEASURED_PEAKS.json")
     if os.path.exists(path):
@@ -324,7 +334,7 @@ def run_slab(args):
         line = {
             "metric": METRIC, "value": units / t_max / 1e6, "unit": "MLUPS", "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": t_max / args.steps * 1e3, "higher_is_better": True, "scaling": "strong",
-            "vs_baseline": None, "dtype": "f64" if prec == 0 else "f64 collision, f32 storage and stencil interpolation",
+            "vs_baseline": None, "dtype": dtype_name(prec, w.dim),
             "data": "synthetic",
             "config": {"workload": args.workload, "nodes_total": w.nodes, "lattice": "D2Q9+D2Q5" if w.dim == 2 else "D3Q19+D3Q7",
                        "mesh": f"{w.mesh} stretch {w.stretch}", "Ra": w.Ra, "Pr": w.Pr, "U_lu": 0.1,
@@ -555,7 +565,7 @@ def main():
         line = {
             "metric": METRIC, "value": value, "unit": "MLUPS", "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": t_max / args.steps * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-            "dtype": "f64" if prec == 0 else "f64 collision, f32 storage and stencil interpolation", "data": "synthetic",
+            "dtype": dtype_name(prec, w.dim), "data": "synthetic",
             "config": {"workload": args.workload, "nodes_per_gpu": w.nodes, "lattice": "D2Q9+D2Q5" if w.dim == 2 else "D3Q19+D3Q7",
                        "mesh": f"{w.mesh} stretch {w.stretch}", "Ra": w.Ra, "Pr": w.Pr, "U_lu": 0.1,
                        "step": f"{args.lbm_per_step} LBM time steps + 1 Nu/Re reduction",

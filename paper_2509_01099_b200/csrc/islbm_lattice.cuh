@@ -40,6 +40,9 @@ struct NodeParams {
   // the same temperature constants in fp32, for the fp32-storage kernels, which collide the temperature populations in
   // fp32 (ISLBM_G_FP32): kf[0] = -q_k/2, kf[1] = -q_e/20 | -q_e/42, kf[2] = -q_e/12 (3-D), kf[3] = -q_e/4, kf[4] = a_T
   float kf[5];
+  // fp32 copies for the all-fp32 3-D collision of the fp32-storage kernels (ISLBM_F_FP32_3D): kq[i] = k[i] for the 17
+  // flow constants, kq[17] = gbeta, kq[18] = T0
+  float kq[19];
 };
 
 // fp32-storage kernels: collide the temperature populations g in fp32 (they are stored in fp32 and T tolerates it:
@@ -48,6 +51,15 @@ struct NodeParams {
 // conversions and 50 of the 293 fp64 instructions per node of the latency-bound fp32-storage step.
 #ifndef ISLBM_G_FP32
 #define ISLBM_G_FP32 1
+#endif
+// fp32-storage 3-D kernels: the flow populations (deviations f - w) are collided in fp32 as well, so no fp64
+// instruction and no conversion is left in the step: 134 -> 120 registers, which lets 16 instead of 12 warps share an
+// SM (256^3 sustained 832 -> 712 us, 0.64 -> 0.75 of the roofline; profiles/attempts.md).  Every parity bar holds as
+// it stood (3 steps from a far-from-equilibrium state within 2e-6 of the plane maximum, 1000 steps of
+// config 4 / 5 within 1e-5 on u, v, w, T).  The 2-D kernels keep the fp64 flow collision: there the same change
+// fails the 3-step bar (6-7e-6).  -DISLBM_F_FP32_3D=0 restores the fp64 flow collision for an A/B build.
+#ifndef ISLBM_F_FP32_3D
+#define ISLBM_F_FP32_3D 1
 #endif
 
 // k[] of NodeParams for the lattice of dimension dim, from s_nu, s_q, hs_nu, hs_q, q_k, q_e (index map: collide_node)
@@ -78,6 +90,9 @@ inline void fold_node_params(NodeParams &p, int dim) {
   p.kf[1] = (float)p.k[18];
   p.kf[3] = (float)p.k[20];
   p.kf[4] = (float)p.a_T;
+  for (int i = 0; i < 17; ++i) p.kq[i] = (float)p.k[i];
+  p.kq[17] = (float)p.gbeta;
+  p.kq[18] = (float)p.T0;
 }
 
 template <int DIM> struct Lat;
@@ -294,9 +309,119 @@ ISLBM_HD void fields_from_post(const double (&f)[9], const double (&g)[5], const
 // ---------------------------------------------------------------------------
 // D3Q19 + D3Q7
 // ---------------------------------------------------------------------------
+// Deviation form, every temporary in fp32 (ISLBM_F_FP32_3D): the same factored M^T D M as collide_node<true> below,
+// with the host-folded constants rounded to fp32.  f holds f_q - w_q and g the temperature populations, in and out.
+ISLBM_HD void collide_node_dev_f32(float (&f)[19], float (&g)[7], const NodeParams &p) {
+  const float *k = p.kq;
+  const float T = g[0] + (((g[1] + g[2]) + (g[3] + g[4])) + (g[5] + g[6]));
+  const float px = f[1] + f[2], py = f[3] + f[4], pz = f[5] + f[6];
+  const float ax = f[1] - f[2], ay = f[3] - f[4], az = f[5] - f[6];
+  const float xy_s = (f[7] + f[10]) + (f[8] + f[9]);
+  const float xy_x = (f[7] - f[10]) + (f[9] - f[8]);
+  const float xy_y = (f[7] - f[10]) + (f[8] - f[9]);
+  const float xy_p = (f[7] + f[10]) - (f[8] + f[9]);
+  const float xz_s = (f[11] + f[14]) + (f[12] + f[13]);
+  const float xz_x = (f[11] - f[14]) + (f[13] - f[12]);
+  const float xz_z = (f[11] - f[14]) + (f[12] - f[13]);
+  const float xz_p = (f[11] + f[14]) - (f[12] + f[13]);
+  const float yz_s = (f[15] + f[18]) + (f[16] + f[17]);
+  const float yz_y = (f[15] - f[18]) + (f[17] - f[16]);
+  const float yz_z = (f[15] - f[18]) + (f[16] - f[17]);
+  const float yz_p = (f[15] + f[18]) - (f[16] + f[17]);
+  const float sa = px + py + pz;
+  const float sd = xy_s + xz_s + yz_s;
+  const float rsum = f[0] + sa + sd;
+  const float rho = 1.0f + rsum;
+  const float Fy = rho * k[17] * (T - k[18]);
+  const float dxs = xy_x + xz_x, dys = xy_y + yz_y, dzs = xz_z + yz_z;
+  const float jx = ax + dxs, jy = ay + dys, jz = az + dzs;
+#ifdef __CUDA_ARCH__
+  const float inv = __frcp_rn(rho);
+#else
+  const float inv = 1.0f / rho;
+#endif
+  const float u = jx * inv, v = (jy + 0.5f * Fy) * inv, w = jz * inv;
+  const float u2 = u * u + v * v + w * w;
+  const float mqx = -4.0f * ax + dxs, mqy = -4.0f * ay + dys, mqz = -4.0f * az + dzs;
+  const float a3 = 2.0f * px - py - pz, d3 = xy_s + xz_s - 2.0f * yz_s;
+  const float aw = py - pz, dw = xy_s - xz_s;
+  const float vF = v * Fy;
+  const float q3 = 2.0f * u * u - v * v - w * w, qw = v * v - w * w;
+  // e - e_eq and eps - eps_eq with the rho-proportional rest parts cancelled: (m_e + 11 rsum) = 19 (sd - f0),
+  // (m_eps - 3 rsum) = 9 f0 - 7 sa - 2 sd
+  const float ee = 19.0f * ((sd - f[0]) - rho * u2);
+  const float eeps = (9.0f * f[0] - 7.0f * sa - 2.0f * sd) + rho * (5.5f * u2);
+  const float r23 = (2.0f / 3.0f) * rho;
+  const float djy = Fy * 0.1f;
+  const float de = fmaf(k[0], ee, k[1] * vF);
+  const float deps = fmaf(k[2], eeps, k[3] * vF);
+  const float dqx = k[4] * (mqx + r23 * u);
+  const float dqy = fmaf(k[4], mqy + r23 * v, k[5] * Fy);
+  const float dqz = k[4] * (mqz + r23 * w);
+  const float d3pxx = fmaf(k[6], (a3 + d3) - rho * q3, k[7] * vF);
+  const float d3pixx = fmaf(k[8], (-2.0f * a3 + d3) + 0.5f * rho * q3, k[9] * vF);
+  const float dpww = fmaf(k[10], (aw + dw) - rho * qw, k[11] * vF);
+  const float dpiww = fmaf(k[12], (-2.0f * aw + dw) + 0.5f * rho * qw, k[13] * vF);
+  const float dpxy = fmaf(k[14], xy_p - rho * (u * v), k[15] * (u * Fy));
+  const float dpyz = fmaf(k[14], yz_p - rho * (v * w), k[15] * (w * Fy));
+  const float dpxz = k[14] * (xz_p - rho * (u * w));
+  const float dmx = k[16] * (xy_x - xz_x), dmy = k[16] * (yz_y - xy_y), dmz = k[16] * (xz_z - yz_z);
+  // temperature (Eq. 16 order), as in the ISLBM_G_FP32 branch of collide_node
+  {
+    const float hx = g[1] + g[2], hy = g[3] + g[4], hz = g[5] + g[6];
+    const float a1 = p.kf[0] * ((g[1] - g[2]) - u * T);
+    const float a2 = p.kf[0] * ((g[3] - g[4]) - v * T);
+    const float a3g = p.kf[0] * ((g[5] - g[6]) - w * T);
+    const float a4 = p.kf[1] * ((-6.0f * g[0] + (hx + hy + hz)) - p.kf[4] * T);
+    const float a5 = p.kf[2] * (2.0f * hx - hy - hz);
+    const float a6 = p.kf[3] * (hy - hz);
+    g[0] += -6.0f * a4;
+    g[1] += a1 + a4 + 2.0f * a5;
+    g[2] += -a1 + a4 + 2.0f * a5;
+    g[3] += a2 + a4 - a5 + a6;
+    g[4] += -a2 + a4 - a5 + a6;
+    g[5] += a3g + a4 - a5 - a6;
+    g[6] += -a3g + a4 - a5 - a6;
+  }
+  // f+ = f + M^T d
+  const float ca = -11.0f * de - 4.0f * deps;
+  const float cd = 8.0f * de + deps;
+  const float tx = -4.0f * dqx, ty = djy - 4.0f * dqy, tz = -4.0f * dqz;
+  const float sx = dqx, sy = djy + dqy, sz = dqz;
+  const float nax = 2.0f * d3pxx - 4.0f * d3pixx;
+  const float nay = -d3pxx + 2.0f * d3pixx + dpww - 2.0f * dpiww;
+  const float naz = -d3pxx + 2.0f * d3pixx - dpww + 2.0f * dpiww;
+  const float nxy = d3pxx + d3pixx + dpww + dpiww;
+  const float nxz = d3pxx + d3pixx - dpww - dpiww;
+  const float nyz = -2.0f * (d3pxx + d3pixx);
+  f[0] += -30.0f * de + 12.0f * deps;
+  f[1] += ca + tx + nax;
+  f[2] += ca - tx + nax;
+  f[3] += ca + ty + nay;
+  f[4] += ca - ty + nay;
+  f[5] += ca + tz + naz;
+  f[6] += ca - tz + naz;
+  f[7] += cd + nxy + (sx + dmx) + (sy - dmy) + dpxy;
+  f[8] += cd + nxy - (sx + dmx) + (sy - dmy) - dpxy;
+  f[9] += cd + nxy + (sx + dmx) - (sy - dmy) - dpxy;
+  f[10] += cd + nxy - (sx + dmx) - (sy - dmy) + dpxy;
+  f[11] += cd + nxz + (sx - dmx) + (sz + dmz) + dpxz;
+  f[12] += cd + nxz - (sx - dmx) + (sz + dmz) - dpxz;
+  f[13] += cd + nxz + (sx - dmx) - (sz + dmz) - dpxz;
+  f[14] += cd + nxz - (sx - dmx) - (sz + dmz) + dpxz;
+  f[15] += cd + nyz + (sy + dmy) + (sz - dmz) + dpyz;
+  f[16] += cd + nyz - (sy + dmy) + (sz - dmz) - dpyz;
+  f[17] += cd + nyz + (sy + dmy) - (sz - dmz) - dpyz;
+  f[18] += cd + nyz - (sy + dmy) - (sz - dmz) + dpyz;
+}
+
 template <bool DEV = false, typename FT>
 ISLBM_HD void collide_node(FT (&fio)[19], FT (&gio)[7], const NodeParams &p) {
   constexpr bool GF = sizeof(FT) == 4 && ISLBM_G_FP32;   // temperature collision in fp32 (fp32 storage)
+  if constexpr (DEV && GF && ISLBM_F_FP32_3D) {
+    collide_node_dev_f32(fio, gio, p);
+    return;
+  }
   double f[19], g[7] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
 #ifdef __CUDA_ARCH__
 #pragma unroll

@@ -56,6 +56,19 @@ template <typename ST, int TX, int TY> __host__ __device__ constexpr int produce
   return (ISLBM_PRODUCER_WG && sizeof(ST) == 8 && TX * TY == 256) ? 128 : 0;
 }
 
+// resident CTAs per SM the step kernels are compiled for (the register cap follows).  fp32 storage, 32x8 tiles: two
+// CTAs per SM = 16 warps at 128 registers on a 2-stage ring (2 x (66 KB ring + 37 KB of stencil sets)): the all-fp32
+// node arithmetic (ISLBM_F_FP32_3D) needs 120 registers, and the step is bound by latency, not by bytes in flight
+// (256^3: 32x6 x 2 CTAs on 3 stages 741-745 us, 32x5 x 3 CTAs on 2 stages 719 us, 32x8 x 2 CTAs 711-713 us;
+// profiles/attempts.md).
+template <typename ST, int TX, int TY> __host__ __device__ constexpr bool f32_two_wide_ctas() {
+  return sizeof(ST) == 4 && TX == 32 && TY == 8;
+}
+template <typename ST, int TX, int TY> __host__ __device__ constexpr int min_ctas3() {
+  if (f32_two_wide_ctas<ST, TX, TY>()) return 2;
+  return TX * TY <= 128 ? 3 : (TX * TY <= 192 ? 2 : 1);
+}
+
 constexpr int kMaxChunk = 64;   // longest marching chunk (its weights are staged in shared memory)
 
 // SK = stencil kind: 0 destination-centred {j-1,j,j+1} (A2), 1 upwind {j-2,j-1,j} for c = +1 and
@@ -91,7 +104,7 @@ struct Tile3 {
   static __host__ __device__ constexpr int moff(int off, int k, int pbytes, int half) { return off + (k / 2) * half + (k % 2) * pbytes; }
   // fp64: 3 x 62.7 KB is all that fits.  fp32 storage, upwind stencil: 2 stages, so that two CTAs (2 x (58 KB ring + 27 KB
   // of stencil sets)) still share an SM; for 32x6 tiles a 2-stage ring measures the same as a 3-stage one (profiles/attempts.md)
-  static constexpr int STAGES = sizeof(ST) == 4 ? (SK ? 2 : ISLBM_Z_STAGES_F32) : 3;
+  static constexpr int STAGES = sizeof(ST) == 4 ? ((SK || f32_two_wide_ctas<ST, TX, TY>()) ? 2 : ISLBM_Z_STAGES_F32) : 3;
   static constexpr int CONSUMER_WARPS = TX * TY / 32;
   static constexpr int THREADS = TX * TY;                // thread 0 doubles as the TMA producer
   static constexpr uint32_t Z_BYTES = 2u * P_C + 4u * P_X + 4u * P_Y + 4u * P_XY;   // planes of the emitted slice
@@ -366,7 +379,7 @@ __device__ __forceinline__ void load_march_weights(const float *ws, int i, Pr<fl
   } while (0)
 
 template <typename ST, int TX, int TY>
-__global__ void __launch_bounds__(TX * TY + producer_threads<ST, TX, TY>(), TX * TY <= 128 ? 3 : (TX * TY <= 192 ? 2 : 1))
+__global__ void __launch_bounds__(TX * TY + producer_threads<ST, TX, TY>(), min_ctas3<ST, TX, TY>())
 k_step_zmarch(const __grid_constant__ Maps3 mp, DevMesh m, NodeParams np, const ST *__restrict__ src,
               ST *__restrict__ dst, int zchunk, int load_policy, int store_policy, int flags) {
   using T = Tile3<ST, TX, TY>;
@@ -960,11 +973,16 @@ inline void launch3_shape(const Plan3 &p, const int *n, const DevMesh &m, const 
 // sk = 0: the destination-centred stencil; 1: the upwind stencil (islbm_set_stencil)
 template <typename ST>
 inline bool plan3_create(Plan3 &p, const int *n, int nxp, void *buf0, void *buf1, const Tuning &tn, int sk) {
-  // tile shape (x by y nodes per CTA).  fp64 storage: 32x8 (254 registers, one CTA per SM; DRAM-bound).  fp32 storage
-  // is bound by the latency of the fp64 collision at the 12 warps per SM its 168 registers allow: 32x6 CTAs (two per
-  // SM) or 32x4 (three per SM) on short y-axes (profiles/attempts.md).  The upwind kernels exist in these three shapes.
+  // tile shape (x by y nodes per CTA).  fp64 storage: 32x8 (one CTA of 8 consumer warps per SM; DRAM-bound).  fp32
+  // storage is bound by latency: 32x8 with two CTAs per SM (16 warps at 128 registers, 2-stage ring) for the central
+  // stencil; the upwind kernels (168 registers) exist as 32x6 (two per SM) and 32x4 (three per SM, short y-axes) and
+  // as 32x8 for fp64 (profiles/attempts.md).
   int shape = tn.shape3d;
-  if (shape == 0 || (sk && shape != 3 && shape != 4)) shape = sizeof(ST) == 4 ? (n[1] >= 192 ? 3 : 4) : 5;
+  if (sk) {
+    if (shape != 3 && shape != 4) shape = sizeof(ST) == 4 ? (n[1] >= 192 ? 3 : 4) : 5;
+  } else if (shape == 0) {
+    shape = 5;
+  }
   p.shape = shape;
   p.sk = sk;
   if (sk) {

@@ -56,8 +56,10 @@ def test_factored_collision_matches_oracle(harness, dim):
         harness.harness_collide_dev(dim, dptr(fd), dptr(gd), dptr(prm))
         assert np.abs(fd - fo).max() < 2e-16 * 8
         assert np.abs(gd - go).max() < 2e-16 * 8
-        # fp32-storage form: fp32 deviations in and out, flow arithmetic in fp64 (3-D: the unfolded expressions);
-        # on fp32-representable inputs the result is the oracle's, rounded once to fp32
+        # fp32-storage form: fp32 deviations in and out.  2-D: flow arithmetic in fp64, so on fp32-representable inputs
+        # the result is the oracle's, rounded once to fp32.  3-D (ISLBM_F_FP32_3D): every temporary in fp32, a few dozen
+        # fp32 operations on values of the input's size: the bound is in units of the INPUT deviations' magnitude,
+        # 16 x 2^-24 (measured over 9000 nodes with deviations of 0.5 %, 5 % and 15 % of the weights: 7.0)
         wts = np.empty(o.qf); e_ = np.empty(3 * o.qf, dtype=np.int32); opp_ = np.empty(o.qf, dtype=np.int32)
         harness.harness_tables(dim, e_.ctypes.data_as(C.POINTER(C.c_int)), opp_.ctypes.data_as(C.POINTER(C.c_int)), dptr(wts))
         dev32 = (f - wts).astype(np.float32)
@@ -65,7 +67,10 @@ def test_factored_collision_matches_oracle(harness, dim):
         fo32, go32 = o.collide_node(wts + dev32.astype(np.float64), g32.astype(np.float64))
         d_io, g_io = dev32.copy(), g32.copy()
         harness.harness_collide_dev_f32(dim, d_io.ctypes.data_as(C.POINTER(C.c_float)), g_io.ctypes.data_as(C.POINTER(C.c_float)), dptr(prm))
-        assert np.abs(d_io.astype(np.float64) - (fo32 - wts)).max() <= 2.0 ** -24 * np.abs(fo32 - wts).max() * 1.01
+        if dim == 2:
+            assert np.abs(d_io.astype(np.float64) - (fo32 - wts)).max() <= 2.0 ** -24 * np.abs(fo32 - wts).max() * 1.01
+        else:
+            assert np.abs(d_io.astype(np.float64) - (fo32 - wts)).max() <= 16 * 2.0 ** -24 * np.abs(dev32).max()
         # temperature populations: the fp32-storage kernels collide them in fp32 (ISLBM_G_FP32: a dozen fp32 operations
         # on values of the input's size), so the bound is in units of the INPUT's magnitude: 16 x 2^-24 (measured over
         # 5000 far-from-equilibrium nodes: 7.7 in 2-D, 12.0 in 3-D)
