@@ -62,8 +62,9 @@ typedef struct {
 enum { ISLBM_D2Q9_D2Q5 = 0, ISLBM_D3Q19_D3Q7 = 1 };
 /* ISLBM_F32_STORAGE: the workspace holds f_q - w_q and g_q as fp32; the TMA kernels interpolate those stored
  * deviations in fp32 (one or two more fp32 roundings of the deviation per step, the size of the storage rounding
- * itself), collide the flow populations in fp64 and the temperature populations in fp32; everything else (API arrays,
- * diagnostics, weights) is fp64.  Tolerance against the
+ * itself) and collide the temperature populations in fp32; the flow populations are collided in fp64 by the 2-D
+ * kernels and in fp32 by the 3-D kernels (the precision is the cheapest one that holds the parity bars
+ * of each lattice); everything else (API arrays, diagnostics, weights) is fp64.  Tolerance against the
  * fp64 oracle: 1e-5 on u and T after 1000 steps (BASELINE.json). */
 enum { ISLBM_F64 = 0, ISLBM_F32_STORAGE = 1 };
 

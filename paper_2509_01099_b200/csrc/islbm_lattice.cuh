@@ -197,9 +197,75 @@ ISLBM_HD constexpr double wflow(int q) {
 ISLBM_HD void upd(double &a, double d) { a += d; }
 ISLBM_HD void upd(float &a, double d) { a = (float)((double)a + d); }
 
+// Deviation form with every temporary in fp32 (ISLBM_F_FP32_2D, an A/B switch): the factored M^T D M of collide_node<true>
+// below with the host-folded constants rounded to fp32; f holds f_q - w_q, g the temperature populations, in and out.
+ISLBM_HD void collide_node_dev_f32(float (&f)[9], float (&g)[5], const NodeParams &p) {
+  const float *k = p.kq;
+  const float T = g[0] + ((g[1] + g[3]) + (g[2] + g[4]));
+  const float p13 = f[1] + f[3], p24 = f[2] + f[4], p57 = f[5] + f[7], p68 = f[6] + f[8];
+  const float sa = p13 + p24, sd = p57 + p68;
+  const float rsum = f[0] + sa + sd;
+  const float rho = 1.0f + rsum;
+  const float Fy = rho * k[17] * (T - k[18]);
+  const float ax = f[1] - f[3], ay = f[2] - f[4];
+  const float d57 = f[5] - f[7], d86 = f[8] - f[6];
+  const float dx = d57 + d86, dy = d57 - d86;
+  const float jx = ax + dx, jy = ay + dy;
+#ifdef __CUDA_ARCH__
+  const float inv = __frcp_rn(rho);
+#else
+  const float inv = 1.0f / rho;
+#endif
+  const float u = jx * inv, v = (jy + 0.5f * Fy) * inv;
+  const float u2 = u * u + v * v;
+  const float vF = v * Fy;
+  // e - e_eq and eps - eps_eq with the rho-proportional rest parts cancelled before any rounding:
+  // (m_e + 2 rsum) = -2 f0 + sa + 4 sd, (m_eps - rsum) = 3 (f0 - sa)
+  const float ee = ((4.0f * sd + sa) - 2.0f * f[0]) - rho * (3.0f * u2);
+  const float eeps = 3.0f * (f[0] - sa) + rho * (3.0f * u2);
+  const float de = fmaf(k[0], ee, k[1] * vF);
+  const float deps = fmaf(k[2], eeps, k[3] * vF);
+  const float djy = Fy * (1.0f / 6.0f);
+  const float dqx = k[4] * ((-2.0f * ax + dx) + rho * u);
+  const float dqy = fmaf(k[4], (-2.0f * ay + dy) + rho * v, k[5] * Fy);
+  const float dpxx = fmaf(k[6], (p13 - p24) - rho * (u * u - v * v), k[7] * vF);
+  const float dpxy = fmaf(k[14], (p57 - p68) - rho * (u * v), k[15] * (u * Fy));
+  {
+    const float a1 = p.kf[0] * ((g[1] - g[3]) - u * T);
+    const float a2 = p.kf[0] * ((g[2] - g[4]) - v * T);
+    const float a3 = p.kf[1] * ((-4.0f * g[0] + ((g[1] + g[3]) + (g[2] + g[4]))) - p.kf[4] * T);
+    const float a4 = p.kf[3] * ((g[1] + g[3]) - (g[2] + g[4]));
+    g[0] += -4.0f * a3;
+    const float g1 = g[1] + (a1 + a3 + a4), g2 = g[2] + (a2 + a3 - a4);
+    const float g3 = g[3] + (-a1 + a3 + a4), g4 = g[4] + (-a2 + a3 - a4);
+    g[1] = g1; g[2] = g2; g[3] = g3; g[4] = g4;
+  }
+  const float ca = -de - 2.0f * deps;
+  const float cd = 2.0f * de + deps;
+  const float tx = -2.0f * dqx, ty = djy - 2.0f * dqy;
+  const float sx = dqx, sy = djy + dqy;
+  f[0] += -4.0f * de + 4.0f * deps;
+  f[1] += ca + tx + dpxx;
+  f[2] += ca + ty - dpxx;
+  f[3] += ca - tx + dpxx;
+  f[4] += ca - ty - dpxx;
+  f[5] += cd + sx + sy + dpxy;
+  f[6] += cd - sx + sy - dpxy;
+  f[7] += cd - sx - sy + dpxy;
+  f[8] += cd + sx - sy - dpxy;
+}
+
+#ifndef ISLBM_F_FP32_2D
+#define ISLBM_F_FP32_2D 0
+#endif
+
 template <bool DEV = false, typename FT>
 ISLBM_HD void collide_node(FT (&fio)[9], FT (&gio)[5], const NodeParams &p) {
   constexpr bool GF = sizeof(FT) == 4 && ISLBM_G_FP32;   // temperature collision in fp32 (fp32 storage)
+  if constexpr (DEV && GF && ISLBM_F_FP32_2D) {
+    collide_node_dev_f32(fio, gio, p);
+    return;
+  }
   double f[9], g[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
 #ifdef __CUDA_ARCH__
 #pragma unroll
