@@ -74,6 +74,31 @@ extern "C" void harness_collide_dev_f32(int dim, float *fdev, float *g, const do
   }
 }
 
+// the all-fp32 deviation-form collisions called directly (3-D: what the fp32-storage kernels run; 2-D: the A/B switch
+// ISLBM_F_FP32_2D, off by default)
+extern "C" void harness_collide_dev_allf32(int dim, float *fdev, float *g, const double *prm) {
+  islbmk::NodeParams p;
+  p.gbeta = prm[0]; p.s_nu = prm[1]; p.s_q = prm[2];
+  p.hs_nu = 1.0 - 0.5 * p.s_nu; p.hs_q = 1.0 - 0.5 * p.s_q;
+  p.q_k = prm[3]; p.q_e = prm[4]; p.a_T = prm[5]; p.T0 = 0.0;
+  islbmk::fold_node_params(p, dim);
+  if (dim == 2) {
+    float ff[9], gg[5];
+    for (int i = 0; i < 9; ++i) ff[i] = fdev[i];
+    for (int i = 0; i < 5; ++i) gg[i] = g[i];
+    islbmk::collide_node_dev_f32(ff, gg, p);
+    for (int i = 0; i < 9; ++i) fdev[i] = ff[i];
+    for (int i = 0; i < 5; ++i) g[i] = gg[i];
+  } else {
+    float ff[19], gg[7];
+    for (int i = 0; i < 19; ++i) ff[i] = fdev[i];
+    for (int i = 0; i < 7; ++i) gg[i] = g[i];
+    islbmk::collide_node_dev_f32(ff, gg, p);
+    for (int i = 0; i < 19; ++i) fdev[i] = ff[i];
+    for (int i = 0; i < 7; ++i) g[i] = gg[i];
+  }
+}
+
 // out: rho,u,v,w,T from post-collision populations
 extern "C" void harness_fields_post(int dim, const double *f, const double *g, const double *prm, double *out) {
   islbmk::NodeParams p{};

@@ -75,6 +75,12 @@ def test_factored_collision_matches_oracle(harness, dim):
         # on values of the input's size), so the bound is in units of the INPUT's magnitude: 16 x 2^-24 (measured over
         # 5000 far-from-equilibrium nodes: 7.7 in 2-D, 12.0 in 3-D)
         assert np.abs(g_io.astype(np.float64) - go32).max() <= 16 * 2.0 ** -24 * np.abs(g32).max()
+        # the all-fp32 deviation-form collisions themselves (3-D: the default of the fp32-storage kernels, same call as
+        # above; 2-D: the ISLBM_F_FP32_2D A/B switch): same bound (measured 7.0 in 3-D, 5.5 in 2-D)
+        d_io, g_io = dev32.copy(), g32.copy()
+        harness.harness_collide_dev_allf32(dim, d_io.ctypes.data_as(C.POINTER(C.c_float)), g_io.ctypes.data_as(C.POINTER(C.c_float)), dptr(prm))
+        assert np.abs(d_io.astype(np.float64) - (fo32 - wts)).max() <= 16 * 2.0 ** -24 * np.abs(dev32).max()
+        assert np.abs(g_io.astype(np.float64) - go32).max() <= 16 * 2.0 ** -24 * np.abs(g32).max()
         # fields from post-collision populations == fields of the pre-collision state
         out = np.empty(5)
         harness.harness_fields_post(dim, dptr(fh), dptr(gh), dptr(prm), dptr(out))
