@@ -550,8 +550,9 @@ ISLBM_HD void collide_node(FT (&fio)[19], FT (&gio)[7], const NodeParams &p) {
   const double ee = DEV ? (me + 11.0 * rsum) - rho * (19.0 * u2) : me - rho * (-11.0 + 19.0 * u2);     // e - e_eq
   const double eeps = DEV ? (meps - 3.0 * rsum) + rho * (5.5 * u2) : meps - rho * (3.0 - 5.5 * u2);   // eps - eps_eq
   // Delta m_k / |row_k|^2.  FOLD: with the host-folded constants k[] (one multiply and one fused multiply-add per
-  // moment; 256^3 fp64 0.895 -> 0.905, 128^3 0.847 -> 0.859).  The fp32-storage 3-D kernels keep the unfolded
-  // expressions: under their 168-register cap the folded form spills 164 instead of 60 bytes and measures 11 % slower.
+  // moment; 256^3 fp64 0.895 -> 0.905, 128^3 0.847 -> 0.859).  FT = float reaches this point only in the A/B build
+  // -DISLBM_F_FP32_3D=0 (fp64 flow collision on fp32 storage), which keeps the unfolded expressions: under its
+  // 168-register cap the folded form spilled 164 instead of 60 bytes and measured 11 % slower.
   constexpr bool FOLD = sizeof(FT) == 8;
   const double djy = Fy * 0.1;
   double gx = 0, gy = 0, gz = 0;

@@ -114,8 +114,8 @@ struct Tile3 {
   static constexpr int W_OFF = BAR_OFF + 128;                       // marching-axis weights [sign][k][kMaxChunk]
   // fp32 storage: the in-plane-interpolated values of the three z-stencil slices live in shared memory, not in
   // registers: [slot 3][pair 6][thread] float2 (each thread reads back only what it wrote: no barrier).  The kernel is
-  // latency-bound at three warps per scheduler under a 168-register cap, and 36 registers of carried state put loop
-  // invariants into local memory on the critical path (profiles/r2_c5_256cu_f32.md)
+  // latency-bound, and 36 registers of carried state put loop invariants into local memory on the critical path under
+  // the 168-register cap of 12 warps per SM, let alone the 128 of the 16 warps it runs at now (profiles/r2_c5_256cu_f32.md)
   static constexpr bool S_IN_SMEM = sizeof(ST) == 4 && ISLBM_S_IN_SMEM;
   static constexpr int S_OFF = W_OFF + 6 * kMaxChunk * 8 + 128;
   static constexpr size_t SMEM_BYTES = (size_t)S_OFF + (S_IN_SMEM ? 3 * 6 * THREADS * 8 : 0);
@@ -131,10 +131,10 @@ struct Maps3 {
 // Arithmetic type of the stencil interpolation, and the type the node's 26 values are held in up to the collision:
 // fp64 for fp64 storage (bit-compatible with the oracle's order of operations).  For fp32 storage the stored
 // deviations f_q - w_q are interpolated in fp32 (one or two more fp32 roundings of the deviation, the size of the
-// storage rounding itself) and stay in fp32 registers: collide_node widens them for the moments and again for the
-// update f+ = fl32(fl64(f) + M^T d) (bit-identical to colliding an fp64 copy of the node, but no fp64 copy stays live
-// from the interpolation on): 52 conversions per node in the SASS instead of the 116 of an fp64 interpolation (they
-// issue at a quarter of the fp64 rate).
+// storage rounding itself) and stay in fp32 registers, and the 3-D node is collided in fp32 too (ISLBM_F_FP32_3D,
+// islbm_lattice.cuh): no conversion and no fp64 instruction is left in the step.  (The A/B build with the fp64 flow
+// collision widens each value for the moments and again for the update f+ = fl32(fl64(f) + M^T d): 52 conversions
+// per node in the SASS instead of the 116 of an fp64 interpolation; they issue at a quarter of the fp64 rate.)
 template <typename ST> struct Acc { using type = double; };
 template <> struct Acc<float> { using type = float; };
 
