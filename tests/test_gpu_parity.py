@@ -941,6 +941,31 @@ def test_reference_temperature_parity_and_symmetry(islbm):
     assert (T + torch.flip(T, (0, 1))).abs().max().item() < 1e-12 and T.abs().max().item() > 0.3
 
 
+def test_paper_mode_table4_ra1e5_129_fp32_storage(islbm, golden):
+    """The same 3-D paper-mode case on the fp32-storage path, whose 3-D kernels do ALL node arithmetic in fp32
+    (interpolation and both collisions): 4e5 steps from rest (the fp64 run meets Eq. 30 at 1e-9 after
+    3.8e5), then the Table 4 values within the tolerances of the fp64 test.  The Eq. 30 residuals of an
+    fp32 state floor at its rounding noise, so they are only required to be small, not 1e-9."""
+    ref = golden["table4"]["Ra1e5"]["129"]
+    w = inputs.custom_workload("paper3", 3, 129, mesh="erf", stretch=1.5, Ra=1e5, Ma=0.1)
+    sim = islbm.Islbm(w.coords, w.delta, w.Ra, w.Pr, w.Ma, precision=islbm.F32_STORAGE)
+    assert sim.kernel_name == "tiled_zmarch_tma"
+    sim.set_reference_temperature(-0.5)
+    sim.init(0, 0.0)
+    sim.step(398000)
+    sim.steady_residual()
+    sim.step(2000)
+    ru, rT = sim.steady_residual()
+    nu = sim.nusselt()
+    re_rms = math.sqrt(1e5 / 0.71 * nu["u2"])
+    print("T4 fp32", nu, re_rms, "residuals", ru, rT, "Table 4", ref)
+    assert ru < 1e-5 and rT < 1e-5
+    assert nu["Nu_vol"] == pytest.approx(ref[0], rel=3e-3)
+    assert nu["Nu_hot"] == pytest.approx(ref[1], rel=6e-3)
+    assert nu["Nu_cold"] == pytest.approx(nu["Nu_hot"], rel=1e-4)
+    assert re_rms == pytest.approx(ref[3], rel=3e-3)
+
+
 def test_paper_mode_table4_ra1e5_129(islbm, golden):
     """3-D paper mode (erf a = 1.5, 129 points -> 127^3 fluid nodes, Ma = 0.1, Ra = 1e5) to the Eq. 30 criterion
     against Table 4: <Nu> within 0.3 %, Nu_hot within 0.6 % (the paper's Nu_hot falls by 0.24 %
