@@ -15,6 +15,7 @@
 #include "islbm_reduce.cuh"
 #include "islbm_tiled2.cuh"
 #include "islbm_tiled3.cuh"
+#include "islbm_cluster2.cuh"
 #include "islbm_uniform.cuh"
 
 using namespace islbmk;
@@ -125,6 +126,7 @@ struct islbm {
   Tuning tune;
   Plan2 plan2;
   Plan3 plan3;
+  PlanC2 planc2;           // multi-step cluster kernel for tiny 2-D fp64 meshes (islbm_cluster2.cuh)
   bool tiled_ok() const { return dim == 2 ? plan2.available : plan3.available; }
   const char *tiled_why_not() const { return dim == 2 ? plan2.why_not : plan3.why_not; }
 };
@@ -137,6 +139,8 @@ static void make_tiled_plan(islbm *h) {
   if (h->dim == 2) {
     if (h->precision == ISLBM_F64) plan2_create<double>(h->plan2, h->n, h->dm.nxp, b0, b1, h->tune, h->stencil);
     else plan2_create<float>(h->plan2, h->n, h->dm.nxp, b0, b1, h->tune, h->stencil);
+    h->planc2.available = false;
+    if (h->precision == ISLBM_F64 && h->stencil == 0 && !h->is_slab && h->tune.cluster != 2) planc2_create(h->planc2, h->n);
   } else {
     if (h->precision == ISLBM_F64) plan3_create<double>(h->plan3, h->n, h->dm.nxp, b0, b1, h->tune, h->stencil);
     else plan3_create<float>(h->plan3, h->n, h->dm.nxp, b0, b1, h->tune, h->stencil);
@@ -615,6 +619,7 @@ extern "C" int islbm_set_tuning(islbm_t *h, const char *key, int value) {
   else if (k == "rows2d1") { if (value > kMaxChunk) return fail(ISLBM_ERR_ARG, "rows2d1 must be at most 64"); t.rows2d1 = value; }
   else if (k == "graph") { if (value > 2) return fail(ISLBM_ERR_ARG, "graph must be 0 (automatic), 1 (always) or 2 (never)"); t.graph = value; }
   else if (k == "slab_wait_ms") t.slab_wait_ms = value;
+  else if (k == "cluster") { if (value != 0 && value != 2) return fail(ISLBM_ERR_ARG, "cluster must be 0 (automatic) or 2 (never)"); t.cluster = value; }
   else if (k == "walls") { if (value > 1) return fail(ISLBM_ERR_ARG, "walls must be 0 (fused) or 1 (separate boundary kernel)"); t.walls = value; }
   else return fail(ISLBM_ERR_ARG, "unknown tuning key: " + k);
   make_tiled_plan(h);
@@ -694,6 +699,18 @@ extern "C" int islbm_step(islbm_t *h, int n) {
     return fail(ISLBM_ERR_STATE, "the fused halo exchange is not available with the pure-shift kernel");
   const bool fused = h->peer_base[0] || h->peer_base[1];
   int left = n;
+  // tiny 2-D fp64 meshes: all n steps in ONE launch of a thread-block cluster, state in distributed shared memory
+  if (left >= 2 && which == 2 && !fused && h->dim == 2 && h->planc2.available && h->tune.cluster != 2) {
+    double *srcb = (double *)(h->ws + h->cv.buf[h->cur]);     // rewritten at the end with the state of step n-1
+    double *dstb = (double *)(h->ws + h->cv.buf[1 - h->cur]);
+    const cudaError_t e = launch_cluster2(h->planc2, h->dm, h->np, srcb, dstb, left, h->stream);
+    if (e != cudaSuccess) return fail(ISLBM_ERR_CUDA, std::string("cluster step launch: ") + cudaGetErrorString(e));
+    h->launches++;
+    h->cur ^= 1;
+    h->steps += left;
+    h->other_is_pre = false;
+    left = 0;
+  }
   if (left >= kGraphSteps && graph_eligible(h, which, fused)) {
     if (h->graph_exec && h->graph_cur != h->cur) drop_graph(h);
     if (!h->graph_exec) {

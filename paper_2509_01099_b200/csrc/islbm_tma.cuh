@@ -208,6 +208,8 @@ struct Tuning {
   int graph = 0;        // islbm_step(n >= 32): replay a captured CUDA graph of 32 step kernels; 0 = meshes up to 2^20 nodes, 1 always, 2 never
   int slab_wait_ms = 10000;  // fused slab exchange: longest wait for a neighbour's step flag in milliseconds (0 = for ever)
   int walls = 0;        // 3-D: 0 wall rules inside the step kernel; 1 a separate boundary kernel over the shell (A/B variant)
+  int cluster = 0;      // islbm_step(n >= 2) on a tiny 2-D fp64 mesh: all n steps in one launch of a thread-block cluster
+                        // with the state in distributed shared memory (islbm_cluster2.cuh); 0 automatic, 2 never
 };
 
 }  // namespace islbmk

@@ -98,6 +98,7 @@ def kernels_for(islbm, sim):
             ks.append((islbm.KERNEL_TILED, dict(ring2d=3, rows2d=3, rows2d1=5)))
             ks.append((islbm.KERNEL_TILED, dict(ring2d=4, chunk=9, serpentine=1, fill=2)))
             ks.append((islbm.KERNEL_TILED, dict(ring2d=3, chunk=2, pdl=0)))
+            ks.append((islbm.KERNEL_TILED, dict(cluster=2)))      # tiny meshes: per-step launches instead of the cluster kernel
     except islbm.IslbmError:
         pass
     try:
@@ -110,7 +111,7 @@ def kernels_for(islbm, sim):
 
 
 DEFAULT_TUNING = dict(chunk=0, l2promo=0, load_policy=0, store_policy=0, tx2d=0, serpentine=0, shape3d=0, pdl=1, fill=0,
-                      ring2d=0, rows2d=0, rows2d1=0, walls=0, graph=0)
+                      ring2d=0, rows2d=0, rows2d1=0, walls=0, graph=0, cluster=0)
 
 
 def select(sim, k, tune):
@@ -769,7 +770,8 @@ def test_graph_replay_equals_plain_launches_bitwise(islbm, dim, ns, prec):
     H_lu = (coords[1][-1] - coords[1][0] + delta) / delta
     mk = lambda: islbm.Islbm(coords, delta, 0.71 * (0.1 * H_lu / 0.03) ** 2, 0.71, 0.1 * SQ3, precision=prec)
     a, b = mk(), mk()
-    b.set_tuning(graph=2)
+    a.set_tuning(cluster=2)                                    # (the 64^2 fp64 case would otherwise take the cluster kernel)
+    b.set_tuning(graph=2, cluster=2)
     for s_ in (a, b):
         s_.init(1, 1e-3)
     for n in (100, 1, 33, 64, 7):
@@ -788,6 +790,43 @@ def test_graph_replay_equals_plain_launches_bitwise(islbm, dim, ns, prec):
     assert torch.equal(fa, fb) and torch.equal(ga, gb)
 
 
+@pytest.mark.parametrize("nx,ny", [(64, 64), (32, 32), (48, 48), (16, 64), (128, 32), (20, 6), (7, 4), (84, 6)])
+def test_cluster_multistep_kernel_equals_per_step_launches_bitwise(islbm, nx, ny):
+    """Tiny 2-D fp64 meshes: islbm_step(n >= 2) runs all n steps in ONE launch of a thread-block cluster (bands of whole
+    rows, state in distributed shared memory, halo rows by remote shared-memory stores, one cluster barrier per step).
+    Same bits as the per-step TMA kernel (cluster = 2) from a far-from-equilibrium state, whatever mix of call sizes,
+    and 1e-12 against the oracle after 3 steps; every cluster size from 2 to 16 CTAs and bands of 2 to 8 rows."""
+    coords = [inputs.tanh_mesh(nx, 1.3)[0], inputs.tanh_mesh(ny, 1.6)[0]]
+    delta = min(float(np.diff(c).min()) for c in coords)
+    H_lu = (coords[1][-1] - coords[1][0] + delta) / delta
+    Ra = 0.71 * (0.1 * H_lu / 0.03) ** 2
+    a, orc = pair(islbm, coords, delta, Ra=Ra)
+    b = islbm.Islbm(coords, delta, Ra, 0.71, 0.1 * SQ3)
+    b.set_tuning(cluster=2)
+    f0, g0 = inputs.random_state(orc.shape, orc.qf, orc.qg, seed=3, amp=0.05)
+    orc.set_populations(f0, g0)
+    for s_ in (a, b):
+        s_.set_populations(torch.from_numpy(f0).cuda(), torch.from_numpy(g0).cuda())
+    l0 = a.launch_count
+    a.step(3)
+    assert a.launch_count - l0 == 1
+    b.step(3)
+    orc.step(3)
+    fa, ga = a.get_populations()
+    fb, gb = b.get_populations()
+    assert torch.equal(fa, fb) and torch.equal(ga, gb)
+    fo, go = orc.get_populations()
+    assert elem_err(fa.cpu().numpy(), fo) <= 3e-12 and plane_err(ga.cpu().numpy(), go) <= 3e-12
+    for n in (2, 1, 37, 100, 5):
+        a.step(n)
+        b.step(n)
+    fa, ga = a.get_populations()
+    fb, gb = b.get_populations()
+    assert torch.equal(fa, fb) and torch.equal(ga, gb)
+    na, nb = a.nusselt(), b.nusselt()
+    assert na == nb
+
+
 def test_state_errors_and_launch_accounting(islbm):
     w = inputs.custom_workload("s", 2, 16)
     sim = islbm.Islbm(w.coords, w.delta, w.Ra, w.Pr, w.Ma)
@@ -795,6 +834,10 @@ def test_state_errors_and_launch_accounting(islbm):
         sim.step(1)
     assert e.value.code == -6
     sim.init(0, 1e-3)
+    n0 = sim.launch_count
+    sim.step(10)
+    assert sim.launch_count - n0 == 1          # 16^2 fp64: the multi-step cluster kernel, one launch for the ten steps
+    sim.set_tuning(cluster=2)
     n0 = sim.launch_count
     sim.step(10)
     assert sim.launch_count - n0 >= 10
