@@ -277,7 +277,9 @@ int islbm_set_kernel(islbm_t *h, int which);
  * step kernels: 0 automatic = meshes of at most 2^20 nodes, whose steps are short enough for the host's launch rate to show, 1 always,
  * 2 never), "slab_wait_ms" (fused slab exchange: the longest a boundary CTA waits for its neighbour's step flag, default
  * 10 000 ms, 0 = for ever; a CTA that gives up is counted, and islbm_diag_sums / islbm_residual_sums then return
- * ISLBM_ERR_STATE instead of the GPU hanging on a neighbour that never steps), "walls" (3-D whole cavity: 0 wall rules inside the step kernel, 1 a separate
+ * ISLBM_ERR_STATE instead of the GPU hanging on a neighbour that never steps), "cluster" (2-D fp64 meshes of at most 16 bands of 256
+ * nodes: islbm_step(n >= 2) runs all n steps in one launch of a thread-block cluster with the state in distributed shared
+ * memory; 0 automatic, 2 never), "walls" (3-D whole cavity: 0 wall rules inside the step kernel, 1 a separate
  * boundary kernel over the shell of wall-adjacent nodes: the design BASELINE.json names, measured slower).  Results
  * do not depend on any of them.  Unknown key or negative value: ISLBM_ERR_ARG. */
 int islbm_set_tuning(islbm_t *h, const char *key, int value);
