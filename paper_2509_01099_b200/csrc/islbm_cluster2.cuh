@@ -6,8 +6,10 @@
 // `rows` mesh rows each, one thread per node) keeps both ping-pong buffers of its band in shared memory, with one halo
 // row on either side; a step is: interpolate from the local buffer, wall rules (Eq. 21-23),
 // collision (Eq. 17, 19), store into the other local buffer, and the two boundary rows of the band ALSO store the
-// eight populations with e_y != 0 into the neighbour CTAs' halo rows through distributed shared memory
-// (st.shared::cluster); one barrier.cluster (release / acquire) per step orders it all.  Reads are always local.
+// eight populations with e_y != 0 into the neighbour CTAs' halo rows through distributed shared memory.  Those stores
+// are st.async with mbarrier::complete_tx: each CTA has one mbarrier per buffer that counts the bytes its neighbours
+// deliver, the rows that read a halo wait on it, and a CTA-local barrier orders the local buffers — a neighbour-only
+// hand-shake, no cluster-wide barrier inside the step loop (ISLBM_CLUSTER_MBAR).  Reads are always local.
 // The arithmetic is that of k_step_ymarch (same ptap3 / pcomb3 / collide_node, same order): results are bit-identical.
 //
 // Scope: D2Q9 + D2Q5, fp64 storage, destination-centred stencil, whole cavity (no slab decomposition), ny = ncta * rows
@@ -18,6 +20,14 @@
 namespace islbmk {
 
 constexpr int kClusterThreads = 256;
+
+// Step synchronisation.  1: neighbour-only hand-shake — the halo values travel as st.async stores that complete bytes on
+// an mbarrier of the receiving CTA (one per buffer), the receiving boundary rows wait on it, and a CTA-local barrier
+// orders the local buffers: no cluster-wide barrier and no memory fence inside the step loop.  0: one
+// barrier.cluster.arrive.release / wait.acquire per step (an A/B build; profiles/attempts.md).
+#ifndef ISLBM_CLUSTER_MBAR
+#define ISLBM_CLUSTER_MBAR 1
+#endif
 
 struct PlanC2 {
   bool available = false;
@@ -37,6 +47,11 @@ __device__ __forceinline__ uint32_t mapa_shared(uint32_t addr, uint32_t rank) {
 }
 __device__ __forceinline__ void st_cluster_f64(uint32_t addr, double v) {
   asm volatile("st.shared::cluster.f64 [%0], %1;" ::"r"(addr), "d"(v) : "memory");
+}
+// remote store that completes 8 bytes on the mbarrier `mbar` of the receiving CTA (both shared::cluster addresses)
+__device__ __forceinline__ void st_async_f64(uint32_t addr, double v, uint32_t mbar) {
+  asm volatile("st.async.shared::cluster.mbarrier::complete_tx::bytes.f64 [%0], %1, [%2];" ::"r"(addr), "d"(v), "r"(mbar)
+               : "memory");
 }
 __device__ __forceinline__ void cluster_sync_all() {
   asm volatile("barrier.cluster.arrive.release;\n\tbarrier.cluster.wait.acquire;" ::: "memory");
@@ -111,14 +126,61 @@ k_multistep_cluster2(DevMesh m, NodeParams np, double *src, double *dst, int row
   if (feed_dn) remote = mapa_shared(sm_s + (uint32_t)(((rows + 1) * nx + x) * 8), (uint32_t)(rank - 1));
   if (feed_up) remote = mapa_shared(sm_s + (uint32_t)(x * 8), (uint32_t)(rank + 1));
   const bool feed = feed_dn | feed_up;
+  // which threads READ a halo row: the band's first / last row, and with 2-row bands also the other row of the first and
+  // last CTA, whose stencil is clamped at the wall and reaches across the band ({0,1,2} for y = 0)
+  const bool reads_halo = valid && ((ysl == 0 && rank > 0) || (ysl + 2 == rows + 1 && rank < nrank - 1));
+  // ... in which case a row that does not feed a neighbour reads what that neighbour overwrites two steps later, and the
+  // neighbour's go-ahead (this band's boundary row) must not leave before the whole CTA has finished reading
+  const bool late_send = rows == 2;
+  // halo hand-shake: hfull[k] counts the bytes the neighbours store into the halo rows of buffer k
+  uint64_t *hfull = reinterpret_cast<uint64_t *>(sm + 2 * BUF);
+  uint32_t rbar = 0;        // the neighbour's hfull[0], shared::cluster address
+  const uint32_t halo_bytes = (uint32_t)(((rank > 0) + (rank < nrank - 1)) * 8 * nx * 8);
+  if constexpr (ISLBM_CLUSTER_MBAR) {
+    if (tid == 0) {
+      mbar_init(&hfull[0], 1);
+      mbar_init(&hfull[1], 1);
+      fence_barrier_init();
+    }
+    if (feed_dn) rbar = mapa_shared(smem_u32(hfull), (uint32_t)(rank - 1));
+    if (feed_up) rbar = mapa_shared(smem_u32(hfull), (uint32_t)(rank + 1));
+  }
 
-  cluster_sync_all();       // every CTA of the cluster is running and has its band loaded
+  cluster_sync_all();       // every CTA of the cluster is running, has its band loaded and its barriers initialised
 
   int b = 0;
 #pragma unroll 1
   for (int s = 0; s < nsteps; ++s) {
     const double *cb = sm + b * BUF;
     double *nb = sm + (1 - b) * BUF;
+    if constexpr (ISLBM_CLUSTER_MBAR) {
+      // arm this step's phase of the receiving barrier (bytes may already have arrived: the count is signed)
+      if (tid == 0) mbar_expect_tx(&hfull[1 - b], halo_bytes);
+    }
+    double h2 = 0, h4 = 0, h5 = 0, h6 = 0, h7 = 0, h8 = 0, k2 = 0, k4 = 0;   // what the neighbour's halo row takes
+    auto send_halo = [&]() {
+      const uint32_t rb = remote + (uint32_t)((1 - b) * BUF * 8);
+      if constexpr (ISLBM_CLUSTER_MBAR) {
+        const uint32_t mb = rbar + (uint32_t)((1 - b) * 8);
+        st_async_f64(rb + (uint32_t)(2 * PL * 8), h2, mb);
+        st_async_f64(rb + (uint32_t)(4 * PL * 8), h4, mb);
+        st_async_f64(rb + (uint32_t)(5 * PL * 8), h5, mb);
+        st_async_f64(rb + (uint32_t)(6 * PL * 8), h6, mb);
+        st_async_f64(rb + (uint32_t)(7 * PL * 8), h7, mb);
+        st_async_f64(rb + (uint32_t)(8 * PL * 8), h8, mb);
+        st_async_f64(rb + (uint32_t)(11 * PL * 8), k2, mb);
+        st_async_f64(rb + (uint32_t)(13 * PL * 8), k4, mb);
+      } else {
+        st_cluster_f64(rb + (uint32_t)(2 * PL * 8), h2);
+        st_cluster_f64(rb + (uint32_t)(4 * PL * 8), h4);
+        st_cluster_f64(rb + (uint32_t)(5 * PL * 8), h5);
+        st_cluster_f64(rb + (uint32_t)(6 * PL * 8), h6);
+        st_cluster_f64(rb + (uint32_t)(7 * PL * 8), h7);
+        st_cluster_f64(rb + (uint32_t)(8 * PL * 8), h8);
+        st_cluster_f64(rb + (uint32_t)(11 * PL * 8), k2);
+        st_cluster_f64(rb + (uint32_t)(13 * PL * 8), k4);
+      }
+    };
     if (valid) {
       double f[9], g[5];
       f[0] = cb[own];
@@ -159,21 +221,22 @@ k_multistep_cluster2(DevMesh m, NodeParams np, double *src, double *dst, int row
       for (int q = 0; q < 9; ++q) nb[q * PL + own] = f[q];
 #pragma unroll
       for (int q = 0; q < 5; ++q) nb[(9 + q) * PL + own] = g[q];
-      if (feed) {
-        const uint32_t rb = remote + (uint32_t)((1 - b) * BUF * 8);
-        st_cluster_f64(rb + (uint32_t)(2 * PL * 8), f[2]);
-        st_cluster_f64(rb + (uint32_t)(4 * PL * 8), f[4]);
-        st_cluster_f64(rb + (uint32_t)(5 * PL * 8), f[5]);
-        st_cluster_f64(rb + (uint32_t)(6 * PL * 8), f[6]);
-        st_cluster_f64(rb + (uint32_t)(7 * PL * 8), f[7]);
-        st_cluster_f64(rb + (uint32_t)(8 * PL * 8), f[8]);
-        st_cluster_f64(rb + (uint32_t)(11 * PL * 8), g[2]);
-        st_cluster_f64(rb + (uint32_t)(13 * PL * 8), g[4]);
-      }
+      h2 = f[2]; h4 = f[4]; h5 = f[5]; h6 = f[6]; h7 = f[7]; h8 = f[8]; k2 = g[2]; k4 = g[4];
+      if (feed && !(ISLBM_CLUSTER_MBAR && late_send)) send_halo();
     }
-    cluster_sync_all();     // the new buffer (own rows and halo rows) is complete everywhere; the old one is free
+    if constexpr (ISLBM_CLUSTER_MBAR) {
+      // local rows of the new buffer complete, old buffer free in this CTA; then the rows that read a halo wait for the
+      // neighbour's bytes.  A neighbour cannot run two steps ahead (it needs this band's next boundary row first), so
+      // the two barriers and the two buffers never alias across steps.
+      __syncthreads();
+      if (feed && late_send) send_halo();
+      if (reads_halo) mbar_wait(&hfull[1 - b], (uint32_t)(s >> 1) & 1u);
+    } else {
+      cluster_sync_all();   // the new buffer (own rows and halo rows) is complete everywhere; the old one is free
+    }
     b ^= 1;
   }
+  if constexpr (ISLBM_CLUSTER_MBAR) cluster_sync_all();   // nobody leaves while a neighbour could still store into it
 
   // The library's two HBM buffers hold the post-collision states of the last two time levels (the newer one is the
   // state, the older one is what islbm_get_populations streams to recover f_t): dst takes level n, src level n-1.
@@ -205,7 +268,7 @@ inline bool planc2_create(PlanC2 &p, const int *n) {
     if (n[1] % c) continue;
     const int rows = n[1] / c;
     if (rows < 2 || (long long)rows * n[0] > kClusterThreads) continue;
-    const size_t smem = (size_t)2 * 14 * (rows + 2) * n[0] * sizeof(double);
+    const size_t smem = (size_t)2 * 14 * (rows + 2) * n[0] * sizeof(double) + 16;   // + two mbarriers
     if (cudaFuncSetAttribute(k_multistep_cluster2, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess ||
         (c > 8 && cudaFuncSetAttribute(k_multistep_cluster2, cudaFuncAttributeNonPortableClusterSizeAllowed, 1) != cudaSuccess)) {
       cudaGetLastError();
