@@ -58,7 +58,8 @@ def test_library_holds_tma_and_mbarrier_instructions(binding):
     assert "UTMALDG" in sass and "SYNCS" in sass
     assert "USETMAXREG" in sass      # the fp64 3-D kernel's producer warpgroup donates its registers (setmaxnreg)
     assert "FFMA2" in sass           # packed fp32 interpolation of the fp32-storage kernels (fma.rn.f32x2)
-    for kern in ("k_step_zmarch", "k_step_ymarch", "k_step_shift", "k_step_generic", "k_nusselt_partial"):
+    assert "STAS.64" in sass and "UCGABAR_ARV" in sass   # the cluster kernel: st.async into a neighbour CTA's shared memory, barrier.cluster
+    for kern in ("k_step_zmarch", "k_step_ymarch", "k_step_shift", "k_step_generic", "k_nusselt_partial", "k_multistep_cluster2"):
         assert kern in sass, kern
 
 
